@@ -1,0 +1,215 @@
+"""FP64 CPU oracle for the NOLSM hot path (arXiv 2205.12182).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this file. It shares no code with the CUDA path (paper_2205_12182_b200/), does not
+import it, and takes plain numpy arrays.
+
+What it computes (citations are PAPER.md line numbers):
+  * submatrix method, steps 1-3 (L54-58) in its non-orthogonal form (L60): for every atom i,
+    the retained rows/columns are the atoms j whose block (j, i) is present in the combined
+    pattern of H0 and S; T_i(H0), T_i(S) are the dense principal submatrices on that set;
+  * the per-submatrix matrix function Eq. 8 (L62)
+        T_i(D) = 1/2 (I - sign(T_i(S)^-1 T_i(H0) - mu I)) T_i(S)^-1
+    evaluated EXACTLY by symmetric eigendecomposition (the iterations of Eq. 6-7, converge
+    to this; BASELINE.json north_star asks for the eigendecomposition route);
+  * write-back of the columns of atom i (L58) and E_elec = Tr(D H0), Eq. 4 (L37).
+
+Readings of silent points: structural pattern with
+optional max-abs block filter (C-1), union pattern supplied by the caller (C-2), ascending atom
+order inside a submatrix (C-3), one submatrix per atom (C-4), structurally symmetric pattern (C-5),
+sign(0) = 0 (C-9), block (j,i) of D comes from submatrix i and is stored transposed in slot
+(i,j) (C-10), no spin factor (C-11).
+
+Parity pins: tests/test_oracle_pins.py (P1-P14 of SURVEY.md 8(c)). Parity with the paper's OWN
+numbers is UNPINNED: PAPER.md prints no worked numerical example and Table II depends on the
+spike-protein dataset, which is not available.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+
+class NotSPDError(ValueError):
+    """Raised when a submatrix of S is not positive definite (Eq. 8 undefined)."""
+
+
+# ------------------------------------------------------------------------------------------
+# step 1: index sets and dense submatrices
+# ------------------------------------------------------------------------------------------
+def block_offsets(atom_nb, row_ptr, col_idx):
+    """Element offset of every block slot: slot s = (i, j) holds nb(i) x nb(j) values row-major."""
+    rows = np.repeat(np.arange(len(atom_nb)), np.diff(np.asarray(row_ptr, dtype=np.int64)))
+    size = np.asarray(atom_nb, dtype=np.int64)[rows] * np.asarray(atom_nb, dtype=np.int64)[col_idx]
+    off = np.zeros(len(col_idx) + 1, dtype=np.int64)
+    off[1:] = np.cumsum(size)
+    return off
+
+
+def index_set(i, row_ptr, col_idx, atom_nb=None, blk_off=None, H_vals=None, S_vals=None,
+              eps_filter=0.0):
+    """N(i): ascending atom ids j whose block (j, i) is non-negligible in column i (L56).
+
+    The pattern is structurally symmetric (C-5), so column i is read from row i. With
+    eps_filter > 0 a block is negligible iff max(|H0 block|_max, |S block|_max) <= eps_filter
+    (C-1); the diagonal block is always kept."""
+    out = []
+    for p in range(int(row_ptr[i]), int(row_ptr[i + 1])):
+        j = int(col_idx[p])
+        keep = True
+        if eps_filter > 0.0 and j != i:
+            lo, hi = int(blk_off[p]), int(blk_off[p + 1])
+            m = max(np.abs(H_vals[lo:hi]).max(), np.abs(S_vals[lo:hi]).max())
+            keep = m > eps_filter
+        if keep:
+            out.append(j)
+    if i not in out:
+        raise ValueError(f"atom {i}: diagonal block missing from the pattern")
+    out = np.array(sorted(out), dtype=np.int32)
+    return out
+
+
+def find_slot(j, k, row_ptr, col_idx):
+    """Slot of block (j, k) or -1 (columns are ascending inside a row)."""
+    lo, hi = int(row_ptr[j]), int(row_ptr[j + 1])
+    p = lo + int(np.searchsorted(col_idx[lo:hi], k))
+    return p if p < hi and col_idx[p] == k else -1
+
+
+def submatrix(N_i, atom_nb, row_ptr, col_idx, blk_off, vals):
+    """T_i(A): dense principal submatrix on the atoms N_i; absent blocks are zero (L56, L60)."""
+    nb = [int(atom_nb[j]) for j in N_i]
+    off = np.concatenate([[0], np.cumsum(nb)]).astype(np.int64)
+    n = int(off[-1])
+    T = np.zeros((n, n), dtype=np.float64)
+    for a, j in enumerate(N_i):
+        for b, k in enumerate(N_i):
+            s = find_slot(int(j), int(k), row_ptr, col_idx)
+            if s >= 0:
+                T[off[a]:off[a + 1], off[b]:off[b + 1]] = \
+                    np.asarray(vals[blk_off[s]:blk_off[s + 1]], dtype=np.float64).reshape(nb[a], nb[b])
+    return T, off
+
+
+# ------------------------------------------------------------------------------------------
+# step 2 (Eq. 5, L62 Eq. 8): the matrix function
+# ------------------------------------------------------------------------------------------
+def sign_scalar(x):
+    """sign with sign(0) = 0 (C-9)."""
+    return np.sign(x)
+
+
+def density_eigh(H, S, mu):
+    """D = 1/2 (I - sign(S^-1 H - mu I)) S^-1 for symmetric H and SPD S, by two symmetric
+    eigendecompositions.
+
+    S = U s U^T, Z = U s^-1/2 U^T (= S^-1/2), Ht = Z H Z = V e V^T. S^-1 H = Z Ht Z^-1 is similar
+    to Ht, so sign(S^-1 H - mu I) = Z sign(Ht - mu I) Z^-1 and
+    D = Z 1/2(I - sign(Ht - mu I)) Z = (Z V) theta(e) (Z V)^T, theta(e) = 1/2 (1 - sign(e - mu)).
+    Returns (D, e, s)."""
+    s, U = np.linalg.eigh(S)
+    if not s[0] > 0.0:
+        raise NotSPDError(f"S not positive definite: lambda_min = {s[0]:.3e}")
+    Z = (U / np.sqrt(s)) @ U.T
+    Ht = Z @ H @ Z
+    Ht = 0.5 * (Ht + Ht.T)
+    e, V = np.linalg.eigh(Ht)
+    theta = 0.5 * (1.0 - sign_scalar(e - mu))
+    C = Z @ V
+    D = (C * theta) @ C.T
+    return D, e, s
+
+
+def sign_matrix(A):
+    """sign(A) for a diagonalisable A with real spectrum: A = P diag(l) P^-1 -> P diag(sign l) P^-1.
+    This is the definition the Newton-Schulz iteration Eq. 6-7 (L47-50) converges to."""
+    l, P = np.linalg.eig(A)
+    if np.abs(l.imag).max() > 1e-8 * max(1.0, np.abs(l.real).max()):
+        raise ValueError("spectrum is not real")
+    X = (P * sign_scalar(l.real)) @ np.linalg.inv(P)
+    return X.real
+
+
+def density_literal(H, S, mu):
+    """Eq. 5 written out literally with a general (non-symmetric) eigendecomposition for the sign."""
+    n = len(H)
+    Sinv = np.linalg.inv(S)
+    A = Sinv @ H - mu * np.eye(n)
+    return 0.5 * (np.eye(n) - sign_matrix(A)) @ Sinv
+
+
+# ------------------------------------------------------------------------------------------
+# step 3 + Eq. 4 (L37)
+# ------------------------------------------------------------------------------------------
+def atom_result(i, atom_nb, row_ptr, col_idx, blk_off, H_vals, S_vals, mu, eps_filter=0.0):
+    """Everything submatrix i produces: index set, dims, D columns of atom i, energy partial.
+
+    Returns dict(N=index set, n=dimension, pos=column offset of atom i inside the submatrix,
+    Dcols = D_sub[:, cols(i)] (n x nb(i)), e_i = sum(Dcols * H_sub[:, cols(i)]),
+    eps = generalised eigenvalues, s = eigenvalues of S_sub)."""
+    N_i = index_set(i, row_ptr, col_idx, atom_nb, blk_off, H_vals, S_vals, eps_filter)
+    H_sub, off = submatrix(N_i, atom_nb, row_ptr, col_idx, blk_off, H_vals)
+    S_sub, _ = submatrix(N_i, atom_nb, row_ptr, col_idx, blk_off, S_vals)
+    D_sub, eps, s = density_eigh(H_sub, S_sub, mu)
+    a = int(np.searchsorted(N_i, i))
+    c0, c1 = int(off[a]), int(off[a + 1])
+    Dcols = D_sub[:, c0:c1].copy()
+    e_i = float((Dcols * H_sub[:, c0:c1]).sum())
+    return dict(N=N_i, n=int(off[-1]), pos=c0, off=off, Dcols=Dcols, e_i=e_i, eps=eps, s=s,
+                H_sub=H_sub, S_sub=S_sub, D_sub=D_sub)
+
+
+def scatter_atom(i, res, atom_nb, row_ptr, col_idx, blk_off, D_vals):
+    """Write block (j, i) of D for all j in N(i) (L58). Storage (C-10): the output uses the input
+    pattern and slot (i, j) holds (D_ji)^T, i.e. the array is D^T in block-CSR; blocks of the
+    pattern that the filter dropped stay zero."""
+    nbi = int(atom_nb[i])
+    for a, j in enumerate(res["N"]):
+        s = find_slot(i, int(j), row_ptr, col_idx)
+        Dji = res["Dcols"][res["off"][a]:res["off"][a + 1], :]          # nb(j) x nb(i)
+        D_vals[blk_off[s]:blk_off[s + 1]] = Dji.T.reshape(-1)
+    return D_vals
+
+
+def nolsm(atom_nb, row_ptr, col_idx, H_vals, S_vals, mu, atoms=None, eps_filter=0.0):
+    """The whole path for all (or the listed) atoms.
+
+    Returns (D_vals, e_atom, info): D_vals float64 in the C-10 layout (zero for atoms not
+    listed), e_atom float64[n_atoms] energy partials (E_elec = e_atom.sum() when all atoms are
+    evaluated), info = per-atom dict(N, n, min_gap)."""
+    n_at = len(atom_nb)
+    blk_off = block_offsets(atom_nb, row_ptr, col_idx)
+    D_vals = np.zeros(int(blk_off[-1]), dtype=np.float64)
+    e_atom = np.zeros(n_at, dtype=np.float64)
+    info = {}
+    for i in (range(n_at) if atoms is None else atoms):
+        i = int(i)
+        res = atom_result(i, atom_nb, row_ptr, col_idx, blk_off, H_vals, S_vals, mu, eps_filter)
+        scatter_atom(i, res, atom_nb, row_ptr, col_idx, blk_off, D_vals)
+        e_atom[i] = res["e_i"]
+        info[i] = dict(N=res["N"], n=res["n"], min_gap=float(np.abs(res["eps"] - mu).min()),
+                       s_min=float(res["s"][0]), s_max=float(res["s"][-1]),
+                       eps_min=float(res["eps"][0]), eps_max=float(res["eps"][-1]))
+    return D_vals, e_atom, info
+
+
+# ------------------------------------------------------------------------------------------
+# full-matrix helpers used by the pins (dense, small systems only)
+# ------------------------------------------------------------------------------------------
+def dense_from_blocks(atom_nb, row_ptr, col_idx, vals, transpose_blocks=False):
+    """Dense N x N matrix from block-CSR values. With transpose_blocks=True the array is read in
+    the C-10 output layout (slot (i,j) holds (M_ji)^T) and the dense M is returned."""
+    blk_off = block_offsets(atom_nb, row_ptr, col_idx)
+    first = np.concatenate([[0], np.cumsum(atom_nb)]).astype(np.int64)
+    M = np.zeros((int(first[-1]), int(first[-1])), dtype=np.float64)
+    s = 0
+    for i in range(len(atom_nb)):
+        for p in range(int(row_ptr[i]), int(row_ptr[i + 1])):
+            j = int(col_idx[p])
+            blk = np.asarray(vals[blk_off[s]:blk_off[s + 1]], dtype=np.float64).reshape(
+                int(atom_nb[i]), int(atom_nb[j]))
+            if transpose_blocks:
+                M[first[j]:first[j + 1], first[i]:first[i + 1]] = blk.T
+            else:
+                M[first[i]:first[i + 1], first[j]:first[j + 1]] = blk
+            s += 1
+    return M

@@ -1,0 +1,440 @@
+"""Seeded synthetic NOLSM inputs: atom positions, block-CSR pattern, H0 and S block values.
+
+This module is *data only*. It holds none of the method's arithmetic (no index-set logic,
+no submatrix extraction, no matrix functions) and is the one piece of code that both the
+CPU oracle's tests and the CUDA path's tests/bench may import, so that both sides see the
+same bytes (BASELINE.json `configs[0..4]`; recipe restated in DESIGN.md "Input recipe").
+
+The synthetic systems stand in for the paper's SARS-CoV-2 spike-protein workload
+(§V-A1), which is not available here: same atom density
+(1 693 134 atoms / (204.7 x 199.5 x 408.5 A^3) = 0.1015 atoms/A^3) and the same per-atom
+submatrix regime (Table II, column "no").
+
+Layout of the generated matrices (what `nolsm_assemble` consumes, include/nolsm.h):
+  atom_nb  int32[n_atoms]          basis functions per atom
+  row_ptr  int64[n_atoms+1]        block-CSR row pointers
+  col_idx  int32[nnzb]             block-CSR column (atom) ids, ascending inside each row
+  blk_off  int64[nnzb+1]           element offset of slot s in the value arrays
+  values   float64[blk_off[-1]]    slot s = block (i, j) = nb(i) x nb(j), row-major
+
+Block values come from a stateless counter-based hash of (seed, matrix id, min(i,j),
+max(i,j), a, b), so any subset of blocks can be regenerated without building the whole matrix
+and the numpy (uint64) and torch (int64, CPU or CUDA) fillers agree bit for bit.
+"""
+from __future__ import annotations
+
+import json
+import math
+import os
+from dataclasses import dataclass, field
+
+import numpy as np
+
+MAT_S = 1
+MAT_H = 2
+MAT_ONSITE = 3
+
+_M1 = 0xBF58476D1CE4E5B9
+_M2 = 0x94D049BB133111EB
+_C_LO = 0x9E3779B97F4A7C15
+_C_HI = 0xD1B54A32D192ED03
+_C_EL = 0x8CB92BA72F3D8DD7
+_MASK = (1 << 64) - 1
+
+
+# --------------------------------------------------------------------------------------
+# counter-based hash: numpy (uint64) flavour
+# --------------------------------------------------------------------------------------
+def _mix_np(z: np.ndarray) -> np.ndarray:
+    z = (z ^ (z >> np.uint64(30))) * np.uint64(_M1)
+    z = (z ^ (z >> np.uint64(27))) * np.uint64(_M2)
+    return z ^ (z >> np.uint64(31))
+
+
+def _seed_key(seed: int, mat: int) -> int:
+    """Scalar pre-mix of (seed, matrix id) done in Python ints (identical for both flavours)."""
+    z = (seed * _C_LO + mat * _C_HI + 0x1234567) & _MASK
+    z = ((z ^ (z >> 30)) * _M1) & _MASK
+    z = ((z ^ (z >> 27)) * _M2) & _MASK
+    return z ^ (z >> 31)
+
+
+def hash_uniform_np(seed: int, mat: int, lo, hi, el) -> np.ndarray:
+    """U[0,1) float64 from (seed, mat, lo, hi, el); lo/hi/el are broadcastable integer arrays."""
+    with np.errstate(over="ignore"):
+        h = np.uint64(_seed_key(seed, mat))
+        h = _mix_np(h + np.asarray(lo).astype(np.uint64) * np.uint64(_C_LO))
+        h = _mix_np(h + np.asarray(hi).astype(np.uint64) * np.uint64(_C_HI))
+        h = _mix_np(h + np.asarray(el).astype(np.uint64) * np.uint64(_C_EL))
+    return (h >> np.uint64(11)).astype(np.float64) * (1.0 / 9007199254740992.0)
+
+
+# --------------------------------------------------------------------------------------
+# counter-based hash: torch (int64, wraps like uint64) flavour -- runs on CPU or CUDA
+# --------------------------------------------------------------------------------------
+def _s64(x: int) -> int:
+    x &= _MASK
+    return x - (1 << 64) if x >= (1 << 63) else x
+
+
+def _lsr_t(z, s: int):
+    return (z >> s) & ((1 << (64 - s)) - 1)
+
+
+def _mix_t(z):
+    z = (z ^ _lsr_t(z, 30)) * _s64(_M1)
+    z = (z ^ _lsr_t(z, 27)) * _s64(_M2)
+    return z ^ _lsr_t(z, 31)
+
+
+def hash_uniform_torch(seed: int, mat: int, lo, hi, el):
+    import torch
+
+    h = _mix_t(lo.to(torch.int64) * _s64(_C_LO) + _s64(_seed_key(seed, mat)))
+    h = _mix_t(h + hi.to(torch.int64) * _s64(_C_HI))
+    h = _mix_t(h + el.to(torch.int64) * _s64(_C_EL))
+    return _lsr_t(h, 11).to(torch.float64) * (1.0 / 9007199254740992.0)
+
+
+# --------------------------------------------------------------------------------------
+# geometry
+# --------------------------------------------------------------------------------------
+def _thin_sequential(cand: np.ndarray, minsep: float, box: float | None) -> np.ndarray:
+    """Sequential rejection: candidate c is kept iff no *kept* earlier candidate is closer than
+    minsep (minimum-image if box is given). Returns the boolean keep mask."""
+    from scipy.spatial import cKDTree
+
+    tree = cKDTree(cand, boxsize=box)
+    pairs = tree.query_pairs(minsep, output_type="ndarray")
+    keep = np.ones(len(cand), dtype=bool)
+    if len(pairs) == 0:
+        return keep
+    lo = np.minimum(pairs[:, 0], pairs[:, 1])
+    hi = np.maximum(pairs[:, 0], pairs[:, 1])
+    order = np.lexsort((lo, hi))
+    lo, hi = lo[order], hi[order]
+    # for each hi (ascending) the list of lower-index conflicting candidates
+    start = np.searchsorted(hi, np.arange(len(cand)), side="left")
+    end = np.searchsorted(hi, np.arange(len(cand)), side="right")
+    for c in np.unique(hi):
+        if keep[lo[start[c]:end[c]]].any():
+            keep[c] = False
+    return keep
+
+
+def uniform_positions(n: int, edge: float, seed: int, minsep: float, periodic: bool) -> np.ndarray:
+    """n points uniform in [0, edge)^3 with pairwise (min-image if periodic) separation >= minsep."""
+    rng = np.random.default_rng(seed)
+    kept = np.empty((0, 3))
+    while len(kept) < n:
+        m = int((n - len(kept)) * 1.7) + 16
+        cand = np.concatenate([kept, rng.random((m, 3)) * edge])
+        keep = _thin_sequential(cand, minsep, edge if periodic else None)
+        kept = cand[keep]
+    return np.ascontiguousarray(kept[:n])
+
+
+def blob_positions(n_solvent: int, n_blob: int, edge: float, sigma: float, seed: int, minsep: float):
+    """Config 3 (SURVEY C-16 reading): n_solvent uniform atoms plus n_blob atoms drawn from an
+    isotropic Gaussian (sigma) centred in a non-periodic cube; min separation overall.
+    Returns (positions, is_blob)."""
+    rng = np.random.default_rng(seed)
+    pos = np.empty((0, 3))
+    kind = np.empty((0,), dtype=bool)
+    n_s = n_b = 0
+    while n_s < n_solvent or n_b < n_blob:
+        ms = int((n_solvent - n_s) * 1.7) + 16 if n_s < n_solvent else 0
+        mb = int((n_blob - n_b) * 2.5) + 16 if n_b < n_blob else 0
+        cs = rng.random((ms, 3)) * edge
+        cb = rng.normal(edge / 2, sigma, (mb, 3))
+        cb = cb[((cb >= 0) & (cb < edge)).all(1)]
+        new = np.concatenate([cs, cb])
+        newk = np.concatenate([np.zeros(len(cs), bool), np.ones(len(cb), bool)])
+        perm = rng.permutation(len(new))
+        cand = np.concatenate([pos, new[perm]])
+        ck = np.concatenate([kind, newk[perm]])
+        keep = _thin_sequential(cand, minsep, None)
+        cand, ck = cand[keep], ck[keep]
+        # trim surplus of either kind (keep the earliest ones)
+        idx_s = np.flatnonzero(~ck)[:n_solvent]
+        idx_b = np.flatnonzero(ck)[:n_blob]
+        sel = np.sort(np.concatenate([idx_s, idx_b]))
+        pos, kind = cand[sel], ck[sel]
+        n_s, n_b = int((~kind).sum()), int(kind.sum())
+    return np.ascontiguousarray(pos), kind
+
+
+def neighbour_pattern(pos: np.ndarray, r_c: float, box: float | None):
+    """Block-CSR pattern: slot (i,j) present iff i == j or |r_i - r_j| (min-image) < r_c.
+    Returns row_ptr int64[n+1], col_idx int32[nnzb] (ascending per row), dist float64[nnzb]."""
+    from scipy.spatial import cKDTree
+
+    n = len(pos)
+    if box is not None and box < 2 * r_c:
+        raise ValueError("periodic box edge must be >= 2 r_c (one image per pair)")
+    tree = cKDTree(pos, boxsize=box)
+    pairs = tree.query_pairs(r_c, output_type="ndarray")
+    d = pos[pairs[:, 0]] - pos[pairs[:, 1]]
+    if box is not None:
+        d -= box * np.round(d / box)
+    r = np.sqrt((d * d).sum(1))
+    ok = r < r_c  # strict, FP64
+    pairs, r = pairs[ok], r[ok]
+    rows = np.concatenate([pairs[:, 0], pairs[:, 1], np.arange(n)])
+    cols = np.concatenate([pairs[:, 1], pairs[:, 0], np.arange(n)])
+    dist = np.concatenate([r, r, np.zeros(n)])
+    order = np.lexsort((cols, rows))
+    rows, cols, dist = rows[order], cols[order], dist[order]
+    row_ptr = np.zeros(n + 1, dtype=np.int64)
+    np.add.at(row_ptr, rows + 1, 1)
+    row_ptr = np.cumsum(row_ptr)
+    return row_ptr, cols.astype(np.int32), dist
+
+
+# --------------------------------------------------------------------------------------
+# the system object
+# --------------------------------------------------------------------------------------
+@dataclass
+class System:
+    name: str
+    seed: int
+    pos: np.ndarray
+    box: float | None            # periodic box edge or None
+    atom_nb: np.ndarray          # int32[n]
+    row_ptr: np.ndarray          # int64[n+1]
+    col_idx: np.ndarray          # int32[nnzb]
+    dist: np.ndarray             # float64[nnzb] pair distance per slot (0 on the diagonal)
+    gamma: float                 # SURVEY C-12 rescale of off-site S blocks
+    mu: float = 0.0
+    meta: dict = field(default_factory=dict)
+    orig: np.ndarray | None = None   # original atom ids (hash keys) when this is a restriction
+
+    def _orig(self) -> np.ndarray:
+        return np.arange(self.n_atoms, dtype=np.int64) if self.orig is None else self.orig
+
+    @property
+    def n_atoms(self) -> int:
+        return len(self.atom_nb)
+
+    @property
+    def nnzb(self) -> int:
+        return len(self.col_idx)
+
+    def slot_rows(self) -> np.ndarray:
+        return np.repeat(np.arange(self.n_atoms, dtype=np.int64), np.diff(self.row_ptr))
+
+    def blk_off(self) -> np.ndarray:
+        rows = self.slot_rows()
+        sz = self.atom_nb[rows].astype(np.int64) * self.atom_nb[self.col_idx].astype(np.int64)
+        off = np.zeros(self.nnzb + 1, dtype=np.int64)
+        np.cumsum(sz, out=off[1:])
+        return off
+
+    # -- radial amplitudes per slot (CPU, numpy: exp is not bit-reproducible across devices) --
+    def amp_S(self) -> np.ndarray:
+        return self.gamma * 0.3 * np.exp(-self.dist * self.dist / 8.0)
+
+    def amp_H(self) -> np.ndarray:
+        return -0.5 * np.exp(-self.dist / 1.5)
+
+    def onsite_H(self) -> np.ndarray:
+        """float64[sum nb]: on-site diagonal energies, N(-1,0.1) for the first floor(nb/2) orbitals
+        of each atom and N(+1,0.1) for the rest (Box-Muller on hashed uniforms)."""
+        nb = self.atom_nb.astype(np.int64)
+        atom = np.repeat(np.arange(self.n_atoms, dtype=np.int64), nb)
+        first = np.concatenate([[0], np.cumsum(nb)[:-1]])
+        orb = np.arange(nb.sum(), dtype=np.int64) - np.repeat(first, nb)
+        atom = self._orig()[atom]
+        u1 = hash_uniform_np(self.seed, MAT_ONSITE, atom, orb, 0)
+        u2 = hash_uniform_np(self.seed, MAT_ONSITE, atom, orb, 1)
+        z = np.sqrt(-2.0 * np.log(1.0 - u1)) * np.cos(2.0 * math.pi * u2)
+        centre = np.where(orb < np.repeat(nb // 2, nb), -1.0, 1.0)
+        return centre + 0.1 * z
+
+    # -- block values -------------------------------------------------------------------
+    def _slot_elements_np(self, slots: np.ndarray):
+        rows_all = self.slot_rows()
+        i = rows_all[slots]
+        j = self.col_idx[slots].astype(np.int64)
+        nbi = self.atom_nb[i].astype(np.int64)
+        nbj = self.atom_nb[j].astype(np.int64)
+        sz = nbi * nbj
+        off = np.zeros(len(slots) + 1, dtype=np.int64)
+        np.cumsum(sz, out=off[1:])
+        which = np.repeat(np.arange(len(slots), dtype=np.int64), sz)
+        e = np.arange(off[-1], dtype=np.int64) - off[which]
+        a = e // nbj[which]
+        b = e - a * nbj[which]
+        return i, j, nbi, nbj, which, a, b, off
+
+    def fill_np(self, mat: int, slots: np.ndarray | None = None) -> np.ndarray:
+        """Values (float64, concatenated row-major blocks) of the chosen slots of S or H0."""
+        if slots is None:
+            slots = np.arange(self.nnzb, dtype=np.int64)
+        slots = np.asarray(slots, dtype=np.int64)
+        i, j, nbi, nbj, which, a, b, _ = self._slot_elements_np(slots)
+        iw, jw = i[which], j[which]
+        og = self._orig()
+        lo = np.minimum(og[iw], og[jw])
+        hi = np.maximum(og[iw], og[jw])
+        swap = iw > jw
+        ca = np.where(swap, b, a)
+        cb = np.where(swap, a, b)
+        sym = (nbi == nbj)[which]
+        ea = np.where(sym, np.minimum(ca, cb), ca)
+        eb = np.where(sym, np.maximum(ca, cb), cb)
+        u = hash_uniform_np(self.seed, mat, lo, hi, ea * 64 + eb)
+        amp = (self.amp_S() if mat == MAT_S else self.amp_H())[slots]
+        vals = amp[which] * (2.0 * u - 1.0)
+        diag = iw == jw
+        if diag.any():
+            if mat == MAT_S:
+                vals[diag] = (a[diag] == b[diag]).astype(np.float64)
+            else:
+                first = np.concatenate([[0], np.cumsum(self.atom_nb.astype(np.int64))[:-1]])
+                on = self.onsite_H()
+                vals[diag] = np.where(a[diag] == b[diag], on[first[iw[diag]] + a[diag]], 0.0)
+        return vals
+
+    def fill_torch(self, mat: int, device="cpu", chunk_slots: int = 1 << 16):
+        """Same values as fill_np for all slots, produced with torch on `device` (CUDA for the
+        large configs). Returns a float64 tensor of blk_off()[-1] elements."""
+        import torch
+
+        dev = torch.device(device)
+        rows_all = self.slot_rows()
+        blk_off = self.blk_off()
+        out = torch.empty(int(blk_off[-1]), dtype=torch.float64, device=dev)
+        amp_all = self.amp_S() if mat == MAT_S else self.amp_H()
+        nb64 = self.atom_nb.astype(np.int64)
+        first = np.concatenate([[0], np.cumsum(nb64)[:-1]])
+        on = torch.from_numpy(self.onsite_H()).to(dev)
+        first_t = torch.from_numpy(first).to(dev)
+        og_t = torch.from_numpy(self._orig()).to(dev)
+        for s0 in range(0, self.nnzb, chunk_slots):
+            s1 = min(self.nnzb, s0 + chunk_slots)
+            i = torch.from_numpy(rows_all[s0:s1]).to(dev)
+            j = torch.from_numpy(self.col_idx[s0:s1].astype(np.int64)).to(dev)
+            nbj = torch.from_numpy(nb64[self.col_idx[s0:s1]]).to(dev)
+            nbi = torch.from_numpy(nb64[rows_all[s0:s1]]).to(dev)
+            sz = nbi * nbj
+            off = torch.zeros(s1 - s0 + 1, dtype=torch.int64, device=dev)
+            off[1:] = torch.cumsum(sz, 0)
+            which = torch.repeat_interleave(torch.arange(s1 - s0, device=dev), sz)
+            e = torch.arange(int(off[-1]), device=dev) - off[which]
+            nbjw = nbj[which]
+            a = torch.div(e, nbjw, rounding_mode="floor")
+            b = e - a * nbjw
+            iw, jw = i[which], j[which]
+            lo = torch.minimum(og_t[iw], og_t[jw])
+            hi = torch.maximum(og_t[iw], og_t[jw])
+            swap = iw > jw
+            ca = torch.where(swap, b, a)
+            cb = torch.where(swap, a, b)
+            sym = (nbi == nbj)[which]
+            ea = torch.where(sym, torch.minimum(ca, cb), ca)
+            eb = torch.where(sym, torch.maximum(ca, cb), cb)
+            u = hash_uniform_torch(self.seed, mat, lo, hi, ea * 64 + eb)
+            amp = torch.from_numpy(amp_all[s0:s1]).to(dev)
+            vals = amp[which] * (2.0 * u - 1.0)
+            diag = iw == jw
+            if mat == MAT_S:
+                vals = torch.where(diag, (a == b).to(torch.float64), vals)
+            else:
+                idx = torch.where(diag, first_t[iw] + a, torch.zeros_like(a))
+                dv = torch.where(a == b, on[idx], torch.zeros_like(vals))
+                vals = torch.where(diag, dv, vals)
+            out[int(blk_off[s0]):int(blk_off[s1])] = vals
+        return out
+
+    def restrict(self, atoms) -> "System":
+        """Sub-system on a sorted subset of atoms (relative order kept, so index sets map
+        monotonically). Blocks between kept atoms keep their values (hash keys use the original
+        ids). Used to hand the oracle only the neighbourhoods of sampled atoms of a large config."""
+        atoms = np.unique(np.asarray(atoms, dtype=np.int64))
+        new_id = -np.ones(self.n_atoms, dtype=np.int64)
+        new_id[atoms] = np.arange(len(atoms))
+        rows = self.slot_rows()
+        keep = (new_id[rows] >= 0) & (new_id[self.col_idx] >= 0)
+        r, c = new_id[rows[keep]], new_id[self.col_idx[keep]]
+        row_ptr = np.zeros(len(atoms) + 1, dtype=np.int64)
+        np.add.at(row_ptr, r + 1, 1)
+        sub = System(name=self.name + "|sub", seed=self.seed, pos=self.pos[atoms], box=self.box,
+                     atom_nb=self.atom_nb[atoms].copy(), row_ptr=np.cumsum(row_ptr),
+                     col_idx=c.astype(np.int32), dist=self.dist[keep], gamma=self.gamma, mu=self.mu,
+                     meta=dict(self.meta), orig=self._orig()[atoms])
+        sub.meta["parent_slots"] = np.flatnonzero(keep)
+        sub.meta["parent_atoms"] = atoms
+        return sub
+
+    def manifest(self) -> dict:
+        return dict(name=self.name, seed=self.seed, n_atoms=self.n_atoms, nnzb=self.nnzb,
+                    periodic=self.box is not None, box=self.box, gamma=self.gamma, mu=self.mu,
+                    n_basis=int(self.atom_nb.sum()),
+                    **{k: v for k, v in self.meta.items() if not isinstance(v, np.ndarray)})
+
+
+# --------------------------------------------------------------------------------------
+# configs (BASELINE.json configs[0..4]) and the gamma table (SURVEY C-12)
+# --------------------------------------------------------------------------------------
+DENSITY = 0.1
+R_C = 6.0
+MINSEP = 1.0
+LAMBDA_FLOOR = 0.2
+_GAMMA_PATH = os.path.join(os.path.dirname(__file__), "gamma_table.json")
+
+
+def gamma_table() -> dict:
+    with open(_GAMMA_PATH) as f:
+        return json.load(f)
+
+
+def _geometry(name: str, n_atoms: int | None, seed: int):
+    if name == "cfg0":
+        n = n_atoms or 64
+        edge = (n / DENSITY) ** (1.0 / 3.0)
+        return uniform_positions(n, edge, seed, MINSEP, False), None, np.full(n, 4, np.int32), {}
+    if name in ("cfg1", "cfg2", "cfg4"):
+        n, nb = {"cfg1": (3000, 6), "cfg2": (32768, 13), "cfg4": (262144, 6)}[name]
+        n = n_atoms or n
+        edge = (n / DENSITY) ** (1.0 / 3.0)
+        return uniform_positions(n, edge, seed, MINSEP, True), edge, np.full(n, nb, np.int32), {}
+    if name == "cfg3":
+        n = n_atoms or 20000
+        n_blob = int(round(n * 6378 / 20000))
+        n_solv = n - n_blob
+        edge = (n_solv / DENSITY) ** (1.0 / 3.0)
+        sigma = 15.0 * (n / 20000) ** (1.0 / 3.0)
+        pos, is_blob = blob_positions(n_solv, n_blob, edge, sigma, seed, MINSEP)
+        return pos, None, np.where(is_blob, 13, 5).astype(np.int32), dict(n_blob=n_blob, edge=edge)
+    raise KeyError(name)
+
+
+def make_system(name: str, n_atoms: int | None = None, seed: int = 0, gamma: float | None = None) -> System:
+    """Build the pattern and per-slot distances of a config. `n_atoms` overrides the atom count
+    (same density and basis; used for proxies and small parity cases). `gamma` overrides the
+    tabulated C-12 rescale (key f"{name}" or f"{name}@{n_atoms}" in gamma_table.json)."""
+    pos, box, atom_nb, meta = _geometry(name, n_atoms, seed)
+    row_ptr, col_idx, dist = neighbour_pattern(pos, R_C, box)
+    if gamma is None:
+        tab = gamma_table()
+        key = name if n_atoms is None else f"{name}@{n_atoms}"
+        if key not in tab and name in tab and tab[name].get("proxy_ok"):
+            key = name
+        if key not in tab:
+            raise KeyError(f"no gamma for {key}; run workloads/calibrate_gamma.py")
+        gamma = float(tab[key]["gamma"])
+    return System(name=name if n_atoms is None else f"{name}@{n_atoms}", seed=seed, pos=pos, box=box,
+                  atom_nb=atom_nb, row_ptr=row_ptr, col_idx=col_idx, dist=dist, gamma=gamma, meta=meta)
+
+
+def to_scipy(system: System, values: np.ndarray):
+    """Expand block-CSR values to a scalar scipy CSR matrix (test / calibration helper)."""
+    import scipy.sparse as sp
+
+    i, j, nbi, nbj, which, a, b, _ = system._slot_elements_np(np.arange(system.nnzb, dtype=np.int64))
+    first = np.concatenate([[0], np.cumsum(system.atom_nb.astype(np.int64))[:-1]])
+    r = first[i[which]] + a
+    c = first[j[which]] + b
+    n = int(system.atom_nb.sum())
+    return sp.csr_matrix((values, (r, c)), shape=(n, n))

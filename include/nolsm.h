@@ -1,0 +1,143 @@
+/* nolsm.h -- C ABI of the B200-native NOLSM hot path (arXiv 2205.12182).
+ *
+ * The library evaluates, one atom-block at a time, the density matrix
+ *     D = 1/2 (I - sign(S^-1 H0 - mu I)) S^-1                          (Eq. 5)
+ * with the non-orthogonal local submatrix method (per-submatrix form Eq. 8)
+ * and the electronic energy E_elec = Tr(D H0) (Eq. 4).
+ *
+ * Inputs are the sparse H0, S and the scalar mu; outputs are D with the input
+ * sparsity pattern and the scalar E_elec. Everything runs on one GPU (sm_100a).
+ *
+ * Conventions
+ *   - Every pointer argument documented "host or device" may point to host memory (pageable or
+ *     pinned) or to device memory of `cuda_device`; the library detects which. Device arrays are
+ *     BORROWED until nolsm_destroy or the next nolsm_assemble and never freed by the library. Host
+ *     arrays are copied during the call and may be released when it returns (for asynchronous
+ *     outputs: after nolsm_energy returned).
+ *   - Block-CSR: row i lists the atoms j with a block (i, j), ascending. Slot s = (i, j) holds the
+ *     nb(i) x nb(j) block row-major; slot s starts at element blk_off[s] = sum over earlier slots of
+ *     nb(i') * nb(j'). H0 and S share one pattern (the union of their patterns), which
+ *     must be structurally symmetric with every diagonal block present.
+ *   - Output layout: D_vals uses the same pattern and offsets; slot (i, j) holds (D_ji)^T, where block
+ *     D_ji (rows of atom j, columns of atom i) is taken from submatrix i. The array is
+ *     therefore D^T in block-CSR and row i is written by submatrix i alone. D is not symmetrised.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *   - All functions return a nolsm_status; none throws or aborts. Numerical failures of single
+ *     submatrices are reported asynchronously: they set per-atom status bits (nolsm_get_atom_stats) and
+ *     make nolsm_energy return NOLSM_ENOTSPD / NOLSM_ENOCONV after writing the result.
+ */
+#ifndef NOLSM_H
+#define NOLSM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nolsm_ctx nolsm_ctx; /* opaque, owned by the library */
+
+typedef enum {
+    NOLSM_OK = 0,
+    NOLSM_EINVAL = 1,   /* bad argument / malformed pattern */
+    NOLSM_ECUDA = 2,    /* a CUDA call failed (nolsm_last_error has the text) */
+    NOLSM_ENOMEM = 3,
+    NOLSM_ESTATE = 4,   /* call out of order */
+    NOLSM_ENOTSPD = 5,  /* some S_sub inverse iteration diverged or did not converge */
+    NOLSM_ENOCONV = 6   /* some sign iteration hit max_sign_iters (result written, flagged) */
+} nolsm_status;
+
+enum { NOLSM_PREC_FP16_FP32 = 0, /* FP16 operands, FP32 accumulate, tcgen05 tensor cores */
+       NOLSM_PREC_FP32 = 1 };    /* all-FP32 validation mode (FFMA, no tensor cores, no TF32) */
+enum { NOLSM_DTYPE_F64 = 0, NOLSM_DTYPE_F32 = 1 };
+enum { NOLSM_GEMM_AUTO = 0, NOLSM_GEMM_UMMA = 1, NOLSM_GEMM_SIMT = 2 };
+enum { NOLSM_MAT_NOTSPD = 1, NOLSM_MAT_NOCONV = 2 }; /* per-atom status bits */
+
+/* Zero in any field selects the default given in brackets. */
+typedef struct {
+    int precision;           /* NOLSM_PREC_* [FP16_FP32] */
+    int gemm_backend;        /* NOLSM_GEMM_* [AUTO: UMMA for FP16_FP32, SIMT for FP32] */
+    int max_inv_iters;       /* cap on Schulz inverse iterations [24] */
+    int max_sign_iters;      /* cap on Newton-Schulz sign iterations, Eq. 6 [64] */
+    float tol_inv;           /* stop when ||I - S Y||_F / sqrt(n) < tol_inv [2e-3 mixed, 1e-5 FP32] */
+    float tol_sign;          /* stop when ||X^2 - I||_F / sqrt(n) < tol_sign [2e-3 mixed, 1e-5 FP32] */
+    int power_iters_s;       /* power iterations for rho(S_sub) [6] */
+    int power_iters_a;       /* power iterations for rho(A_sub) [12] */
+    double eps_filter;       /* block (j,i) enters N(i) iff max(|H0_ji|max, |S_ji|max) > eps_filter [0 = structural] */
+    int batch_atoms;         /* max submatrices resident at once [auto] */
+    size_t workspace_bytes;  /* cap on the library-owned dense workspace [auto] */
+} nolsm_options;
+
+typedef struct {
+    int64_t n_atoms;
+    int64_t n_batches;
+    int64_t dim_min, dim_max;
+    double dim_mean;
+    int64_t sum_inv_iters, sum_sign_iters;
+    int64_t gemms_executed;       /* square GEMMs actually run, summed over submatrices */
+    double flops_useful;          /* sum_i 2 n_i^3 * gemms_i   (PAPER.md:L156 convention) */
+    double flops_padded;          /* same with tile-padded dimensions (what the tensor cores executed) */
+    int64_t n_notspd, n_noconv;
+    double gather_bytes, scatter_bytes; /* algorithmic bytes of the last density_matrix call */
+} nolsm_stats;
+
+/* Creates a context on `cuda_device`. opt may be NULL. */
+int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt);
+
+/* a0: takes the block-CSR pattern and values of H0 and S, validates it, builds the
+ * index sets N(i), dimensions n_i, and the batch plan; uploads what lives on the host.
+ *   atom_nb  int32[n_atoms]     basis functions per atom (> 0)                 host or device
+ *   row_ptr  int64[n_atoms+1]                                                  host or device
+ *   col_idx  int32[nnzb]        ascending inside each row                      host or device
+ *   H0_vals, S_vals             val_dtype[blk_off[nnzb]]                        host or device
+ * Returns NOLSM_EINVAL for unsorted columns, a non-symmetric pattern, a missing diagonal block,
+ * atom_nb <= 0 or null pointers. Synchronises `cuda_stream` before returning. */
+int nolsm_assemble(nolsm_ctx* ctx, int64_t n_atoms, const int32_t* atom_nb, const int64_t* row_ptr,
+                   const int32_t* col_idx, const void* H0_vals, const void* S_vals, int val_dtype,
+                   void* cuda_stream);
+
+/* a1-a7 for all atoms: gather, Schulz inverse, spectral scaling, Newton-Schulz sign (Eq. 6),
+ * convergence tests, D columns, scatter and energy partials. Asynchronous on `cuda_stream`.
+ *   D_vals   d_dtype[blk_off[nnzb]]   host or device; blocks outside every N(i) are zeroed. */
+int nolsm_density_matrix(nolsm_ctx* ctx, double mu, void* D_vals, int d_dtype, void* cuda_stream);
+
+/* Same for atoms [atom_begin, atom_end) only; other rows of D_vals are left untouched. If
+ * e_partial_host is not NULL the call synchronises and stores sum of e_i over the range. */
+int nolsm_density_matrix_range(nolsm_ctx* ctx, double mu, int64_t atom_begin, int64_t atom_end, void* D_vals,
+                               int d_dtype, double* e_partial_host, void* cuda_stream);
+
+/* Eq. 4: synchronises the stream of the last density_matrix call, finishes pending device-to-host
+ * copies and returns E_elec = sum_i e_i over the atoms evaluated by that call. */
+int nolsm_energy(nolsm_ctx* ctx, double* e_elec);
+
+int nolsm_destroy(nolsm_ctx* ctx);
+
+/* ---- diagnostics used by the parity tests and the benchmark ---- */
+
+/* N(i) (ascending atom ids) and n_i. atoms_out may be NULL to query the count; capacity in *n_inout. */
+int nolsm_get_index_set(nolsm_ctx* ctx, int64_t atom, int32_t* atoms_out, int32_t* n_inout, int32_t* dim_out);
+
+/* Runs the gather kernel for one atom and copies the dense n_i x n_i submatrix (row-major, tight) to
+ * host memory. which: 0 = T_i(S), 1 = T_i(H0). out_fp16 != 0 -> uint16 FP16 bits, else float. */
+int nolsm_gather_submatrix(nolsm_ctx* ctx, int64_t atom, int which, int out_fp16, void* out_host);
+
+int nolsm_get_stats(nolsm_ctx* ctx, nolsm_stats* out);
+
+/* Per-atom results of the last density_matrix call for atoms [atom_begin, atom_begin + count); any
+ * output pointer may be NULL. Host arrays. */
+int nolsm_get_atom_stats(nolsm_ctx* ctx, int64_t atom_begin, int64_t count, int32_t* dims, int32_t* inv_iters,
+                         int32_t* sign_iters, int32_t* status, int32_t* gemms, float* residual, double* e_atom);
+
+/* Device time (ms, CUDA events on the call's stream) spent in the phases of the last density_matrix
+ * call: out[0] gather, out[1] GEMM chain incl. scaling mat-vecs, out[2] D columns + scatter,
+ * out[3] GEMM kernels only, out[4] number of GEMM launches. Requires NOLSM_TIMING=1 in the
+ * environment at nolsm_create (adds stream synchronisations; not for headline timing). */
+int nolsm_get_phase_times(nolsm_ctx* ctx, double* out5);
+
+const char* nolsm_last_error(const nolsm_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NOLSM_H */

@@ -1,0 +1,208 @@
+"""ctypes binding of include/nolsm.h. Argument marshalling only: every step of the path runs in the
+CUDA kernels behind the C ABI. Arrays may be torch tensors (CPU or CUDA) or numpy arrays."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+PREC_FP16_FP32, PREC_FP32 = 0, 1
+DTYPE_F64, DTYPE_F32 = 0, 1
+GEMM_AUTO, GEMM_UMMA, GEMM_SIMT = 0, 1, 2
+STATUS_NAMES = {0: "OK", 1: "EINVAL", 2: "ECUDA", 3: "ENOMEM", 4: "ESTATE", 5: "ENOTSPD", 6: "ENOCONV"}
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+
+class NolsmOptions(C.Structure):
+    _fields_ = [("precision", C.c_int), ("gemm_backend", C.c_int), ("max_inv_iters", C.c_int),
+                ("max_sign_iters", C.c_int), ("tol_inv", C.c_float), ("tol_sign", C.c_float),
+                ("power_iters_s", C.c_int), ("power_iters_a", C.c_int), ("eps_filter", C.c_double),
+                ("batch_atoms", C.c_int), ("workspace_bytes", C.c_size_t)]
+
+
+class NolsmStats(C.Structure):
+    _fields_ = [("n_atoms", C.c_int64), ("n_batches", C.c_int64), ("dim_min", C.c_int64), ("dim_max", C.c_int64),
+                ("dim_mean", C.c_double), ("sum_inv_iters", C.c_int64), ("sum_sign_iters", C.c_int64),
+                ("gemms_executed", C.c_int64), ("flops_useful", C.c_double), ("flops_padded", C.c_double),
+                ("n_notspd", C.c_int64), ("n_noconv", C.c_int64), ("gather_bytes", C.c_double),
+                ("scatter_bytes", C.c_double)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class NolsmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"nolsm: {STATUS_NAMES.get(code, code)}: {msg}")
+        self.code = code
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libnolsm.so")
+
+
+def load_library():
+    """Loads libnolsm.so (built in-tree by paper_2205_12182_b200/build.py). Fails loudly if absent."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = lib_path()
+    if not os.path.exists(path):
+        raise ImportError(f"{path} is missing: run `python -m paper_2205_12182_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(path)
+    P, I64, I32 = C.c_void_p, C.c_int64, C.c_int
+    lib.nolsm_create.argtypes = [C.POINTER(P), I32, C.POINTER(NolsmOptions)]
+    lib.nolsm_assemble.argtypes = [P, I64, P, P, P, P, P, I32, P]
+    lib.nolsm_density_matrix.argtypes = [P, C.c_double, P, I32, P]
+    lib.nolsm_density_matrix_range.argtypes = [P, C.c_double, I64, I64, P, I32, C.POINTER(C.c_double), P]
+    lib.nolsm_energy.argtypes = [P, C.POINTER(C.c_double)]
+    lib.nolsm_destroy.argtypes = [P]
+    lib.nolsm_get_index_set.argtypes = [P, I64, P, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+    lib.nolsm_gather_submatrix.argtypes = [P, I64, I32, I32, P]
+    lib.nolsm_get_stats.argtypes = [P, C.POINTER(NolsmStats)]
+    lib.nolsm_get_atom_stats.argtypes = [P, I64, I64, P, P, P, P, P, P, P]
+    lib.nolsm_get_phase_times.argtypes = [P, C.POINTER(C.c_double)]
+    lib.nolsm_last_error.argtypes = [P]
+    lib.nolsm_last_error.restype = C.c_char_p
+    for f in ("nolsm_create", "nolsm_assemble", "nolsm_density_matrix", "nolsm_density_matrix_range", "nolsm_energy",
+              "nolsm_destroy", "nolsm_get_index_set", "nolsm_gather_submatrix", "nolsm_get_stats",
+              "nolsm_get_atom_stats", "nolsm_get_phase_times"):
+        getattr(lib, f).restype = C.c_int
+    _LIB = lib
+    return lib
+
+
+def _ptr(a, dtype_np=None, dtype_name=None):
+    """(address, keepalive) of a contiguous torch tensor or numpy array."""
+    if a is None:
+        return None, None
+    if hasattr(a, "data_ptr"):                       # torch tensor, any device
+        if not a.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        if dtype_name is not None and str(a.dtype) != "torch." + dtype_name:
+            raise TypeError(f"expected torch.{dtype_name}, got {a.dtype}")
+        return a.data_ptr(), a
+    arr = np.ascontiguousarray(a, dtype=dtype_np)
+    return arr.ctypes.data, arr
+
+
+_VAL = {"float64": DTYPE_F64, "float32": DTYPE_F32}
+
+
+def _val_dtype(a) -> int:
+    name = str(a.dtype).replace("torch.", "")
+    if name not in _VAL:
+        raise TypeError(f"values must be float64 or float32, got {a.dtype}")
+    return _VAL[name]
+
+
+class Nolsm:
+    """nolsm_create / assemble / density_matrix / energy / destroy with the names of include/nolsm.h."""
+
+    def __init__(self, device: int = 0, **opts):
+        self._lib = load_library()
+        self._h = C.c_void_p()
+        o = NolsmOptions()
+        for k, v in opts.items():
+            if not hasattr(o, k):
+                raise TypeError(f"unknown option {k}")
+            setattr(o, k, v)
+        rc = self._lib.nolsm_create(C.byref(self._h), device, C.byref(o))
+        if rc:
+            self._h = C.c_void_p()
+            raise NolsmError(rc, "nolsm_create failed (is a CUDA device visible?)")
+        self._keep = []
+        self.n_atoms = 0
+
+    def _check(self, rc, soft=()):
+        if rc and rc not in soft:
+            raise NolsmError(rc, self._lib.nolsm_last_error(self._h).decode())
+        return rc
+
+    def assemble(self, atom_nb, row_ptr, col_idx, H0_vals, S_vals, stream: int = 0):
+        pa, ka = _ptr(atom_nb, np.int32, "int32")
+        pr, kr = _ptr(row_ptr, np.int64, "int64")
+        pc, kc = _ptr(col_idx, np.int32, "int32")
+        ph, kh = _ptr(H0_vals)
+        ps, ks = _ptr(S_vals)
+        vd = _val_dtype(kh)
+        if _val_dtype(ks) != vd:
+            raise TypeError("H0_vals and S_vals must share a dtype")
+        self.n_atoms = int(ka.shape[0])
+        self._keep = [ka, kr, kc, kh, ks]            # device arrays are borrowed by the library
+        self._check(self._lib.nolsm_assemble(self._h, self.n_atoms, pa, pr, pc, ph, ps, vd, stream))
+
+    def density_matrix(self, mu: float, D_vals, stream: int = 0):
+        pd, kd = _ptr(D_vals)
+        self._keep_out = kd
+        self._check(self._lib.nolsm_density_matrix(self._h, float(mu), pd, _val_dtype(kd), stream))
+
+    def density_matrix_range(self, mu: float, atom_begin: int, atom_end: int, D_vals, want_energy=False, stream: int = 0):
+        pd, kd = _ptr(D_vals)
+        self._keep_out = kd
+        e = C.c_double()
+        rc = self._lib.nolsm_density_matrix_range(self._h, float(mu), atom_begin, atom_end, pd, _val_dtype(kd),
+                                                  C.byref(e) if want_energy else None, stream)
+        self._check(rc, soft=(5, 6) if want_energy else ())
+        return e.value if want_energy else None
+
+    def energy(self, strict: bool = True) -> float:
+        e = C.c_double()
+        rc = self._lib.nolsm_energy(self._h, C.byref(e))
+        self._check(rc, soft=() if strict else (5, 6))
+        return e.value
+
+    def index_set(self, atom: int):
+        n = C.c_int32(0)
+        dim = C.c_int32(0)
+        self._check(self._lib.nolsm_get_index_set(self._h, atom, None, C.byref(n), C.byref(dim)))
+        out = np.empty(n.value, dtype=np.int32)
+        self._check(self._lib.nolsm_get_index_set(self._h, atom, out.ctypes.data, C.byref(n), C.byref(dim)))
+        return out, dim.value
+
+    def gather_submatrix(self, atom: int, which: int, fp16: bool):
+        _, dim = self.index_set(atom)
+        out = np.empty((dim, dim), dtype=np.float16 if fp16 else np.float32)
+        self._check(self._lib.nolsm_gather_submatrix(self._h, atom, which, 1 if fp16 else 0, out.ctypes.data))
+        return out
+
+    def stats(self) -> dict:
+        s = NolsmStats()
+        self._check(self._lib.nolsm_get_stats(self._h, C.byref(s)))
+        return s.as_dict()
+
+    def atom_stats(self, atom_begin: int = 0, count: int | None = None) -> dict:
+        count = self.n_atoms - atom_begin if count is None else count
+        d = {k: np.zeros(count, dtype=np.int32) for k in ("dims", "inv_iters", "sign_iters", "status", "gemms")}
+        d["residual"] = np.zeros(count, dtype=np.float32)
+        d["e_atom"] = np.zeros(count, dtype=np.float64)
+        self._check(self._lib.nolsm_get_atom_stats(self._h, atom_begin, count, *[d[k].ctypes.data for k in
+                    ("dims", "inv_iters", "sign_iters", "status", "gemms", "residual", "e_atom")]))
+        return d
+
+    def phase_times(self):
+        out = (C.c_double * 5)()
+        self._check(self._lib.nolsm_get_phase_times(self._h, out))
+        return dict(gather_ms=out[0], chain_ms=out[1], scatter_ms=out[2], gemm_ms=out[3], gemm_launches=out[4])
+
+    def destroy(self):
+        if self._h:
+            self._lib.nolsm_destroy(self._h)
+            self._h = C.c_void_p()
+        self._keep = []
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.destroy()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

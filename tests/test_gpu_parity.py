@@ -1,0 +1,227 @@
+"""GPU parity tests: the CUDA path, called through the C ABI (include/nolsm.h), against the FP64 oracle
+on the same seeded inputs. Tolerances are BASELINE.json's: index sets bit-exact; FP16/FP32 mixed
+max|dD| <= 2e-2 and |dE|/|E| <= 1e-3; all-FP32 <= 1e-5 on both."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import nolsm_oracle as orc
+from tests.helpers import compare_atoms, oracle_on_atoms
+from workloads import MAT_H, MAT_S, make_system
+
+pytestmark = pytest.mark.gpu
+
+TOL_MIXED_D, TOL_MIXED_E = 2e-2, 1e-3
+TOL_FP32 = 1e-5
+
+
+def _nolsm(**kw):
+    from paper_2205_12182_b200 import Nolsm
+    return Nolsm(0, **kw)
+
+
+def _arrays(s, device="cuda"):
+    Hv = torch.from_numpy(s.fill_np(MAT_H)).to(device)
+    Sv = torch.from_numpy(s.fill_np(MAT_S)).to(device)
+    return (torch.from_numpy(s.atom_nb).to(device), torch.from_numpy(s.row_ptr).to(device),
+            torch.from_numpy(s.col_idx).to(device), Hv, Sv)
+
+
+def _run(s, atoms=None, device="cuda", d_dtype=torch.float64, **kw):
+    from paper_2205_12182_b200 import PREC_FP32
+    nb, rp, ci, Hv, Sv = _arrays(s, device)
+    with _nolsm(**kw) as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        D = torch.zeros(Hv.shape[0], dtype=d_dtype, device=device)
+        ctx.density_matrix(s.mu, D)
+        E = ctx.energy()
+        st = ctx.atom_stats()
+        stats = ctx.stats()
+    return D.cpu().numpy(), E, st, stats
+
+
+@pytest.fixture(scope="module")
+def cfg0():
+    return make_system("cfg0")
+
+
+def test_index_sets_bit_exact_cfg0(cfg0):
+    s = cfg0
+    with _nolsm() as ctx:
+        ctx.assemble(*_arrays(s))
+        for i in range(s.n_atoms):
+            N, dim = ctx.index_set(i)
+            ref = orc.index_set(i, s.row_ptr, s.col_idx)
+            assert N.dtype == np.int32 and np.array_equal(N, ref)
+            assert dim == int(s.atom_nb[ref].sum())
+
+
+def test_index_sets_with_eps_filter_bit_exact(cfg0):
+    s = cfg0
+    Hv, Sv = s.fill_np(MAT_H), s.fill_np(MAT_S)
+    blk = s.blk_off()
+    eps = 0.02
+    with _nolsm(eps_filter=eps) as ctx:
+        ctx.assemble(*_arrays(s))
+        smaller = 0
+        for i in range(s.n_atoms):
+            N, dim = ctx.index_set(i)
+            ref = orc.index_set(i, s.row_ptr, s.col_idx, s.atom_nb, blk, Hv, Sv, eps)
+            assert np.array_equal(N, ref)
+            smaller += len(ref) < (s.row_ptr[i + 1] - s.row_ptr[i])
+        assert smaller > 0
+
+
+def test_gather_bit_exact(cfg0):
+    """P13: no arithmetic happens in a gather -- FP32 output equals float32(oracle), FP16 output equals
+    the RN-even rounding of the oracle's FP64 submatrix, bit for bit."""
+    s = cfg0
+    Hv, Sv = s.fill_np(MAT_H), s.fill_np(MAT_S)
+    blk = s.blk_off()
+    with _nolsm() as ctx:
+        ctx.assemble(*_arrays(s))
+        for i in (0, 7, 63):
+            N = orc.index_set(i, s.row_ptr, s.col_idx)
+            for which, vals in ((0, Sv), (1, Hv)):
+                T, _ = orc.submatrix(N, s.atom_nb, s.row_ptr, s.col_idx, blk, vals)
+                g16 = ctx.gather_submatrix(i, which, fp16=True)
+                g32 = ctx.gather_submatrix(i, which, fp16=False)
+                assert np.array_equal(g16.view(np.uint16), T.astype(np.float16).view(np.uint16))
+                assert np.array_equal(g32, T.astype(np.float32))
+
+
+def test_cfg0_fp32_mode(cfg0):
+    from paper_2205_12182_b200 import PREC_FP32
+    s = cfg0
+    D, E, st, stats = _run(s, precision=PREC_FP32)
+    cmp = compare_atoms(s, D, st["e_atom"], range(s.n_atoms))
+    print("fp32 cfg0", {k: v for k, v in cmp.items() if k != "ref"}, stats)
+    assert (st["status"] == 0).all()
+    assert cmp["max_abs_dD"] <= TOL_FP32
+    assert cmp["rel_dE"] <= TOL_FP32
+    assert abs(E - cmp["e_ref"]) / abs(cmp["e_ref"]) <= TOL_FP32
+
+
+@pytest.mark.parametrize("backend", ["umma", "simt"])
+def test_cfg0_mixed_mode(cfg0, backend):
+    from paper_2205_12182_b200 import GEMM_SIMT, GEMM_UMMA
+    s = cfg0
+    D, E, st, stats = _run(s, gemm_backend=GEMM_UMMA if backend == "umma" else GEMM_SIMT)
+    cmp = compare_atoms(s, D, st["e_atom"], range(s.n_atoms))
+    print("mixed cfg0", backend, {k: v for k, v in cmp.items() if k != "ref"}, stats)
+    assert (st["status"] == 0).all()
+    assert cmp["max_abs_dD"] <= TOL_MIXED_D
+    assert cmp["rel_dE"] <= TOL_MIXED_E
+    assert abs(E - cmp["e_ref"]) / abs(cmp["e_ref"]) <= TOL_MIXED_E
+
+
+def test_cfg0_host_buffers_and_fp32_output(cfg0):
+    """Host (numpy) inputs and a host float32 output go through the same C-ABI calls."""
+    s = cfg0
+    Hv, Sv = s.fill_np(MAT_H), s.fill_np(MAT_S)
+    with _nolsm() as ctx:
+        ctx.assemble(s.atom_nb, s.row_ptr, s.col_idx, Hv, Sv)
+        D = np.zeros(len(Hv), dtype=np.float32)
+        ctx.density_matrix(s.mu, D)
+        E = ctx.energy()
+        st = ctx.atom_stats()
+    cmp = compare_atoms(s, D, st["e_atom"], range(0, s.n_atoms, 5))
+    assert cmp["max_abs_dD"] <= TOL_MIXED_D and cmp["rel_dE"] <= TOL_MIXED_E
+    assert np.isfinite(E)
+
+
+def test_density_matrix_range_touches_only_its_rows(cfg0):
+    s = cfg0
+    nb, rp, ci, Hv, Sv = _arrays(s)
+    blk = s.blk_off()
+    with _nolsm() as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        D = torch.full((Hv.shape[0],), 7.0, dtype=torch.float64, device="cuda")
+        e = ctx.density_matrix_range(s.mu, 10, 20, D, want_energy=True)
+        st = ctx.atom_stats()
+    Dh = D.cpu().numpy()
+    v0, v1 = blk[s.row_ptr[10]], blk[s.row_ptr[20]]
+    assert (Dh[:v0] == 7.0).all() and (Dh[v1:] == 7.0).all()
+    cmp = compare_atoms(s, Dh, st["e_atom"], range(10, 20))
+    assert cmp["max_abs_dD"] <= TOL_MIXED_D
+    assert abs(e - cmp["e_ref"]) / abs(cmp["e_ref"]) <= TOL_MIXED_E
+
+
+@pytest.mark.parametrize("name,n_atoms,sample", [("cfg1", 600, 6), ("cfg2", 300, 3), ("cfg3", 1500, 6)])
+def test_small_proxies_mixed(name, n_atoms, sample):
+    """Reduced-size versions of configs 1-3 (same density, basis and generator): several tiles per
+    matrix, ragged tails, mixed 5/13 basis for cfg3. Oracle on a seeded sample of atoms."""
+    s = make_system(name, n_atoms=n_atoms)
+    atoms = np.random.default_rng(1).choice(s.n_atoms, sample, replace=False)
+    D, E, st, stats = _run(s)
+    cmp = compare_atoms(s, D, st["e_atom"], atoms)
+    print(name, {k: v for k, v in cmp.items() if k != "ref"}, stats)
+    assert (st["status"] == 0).all()
+    assert cmp["max_abs_dD"] <= TOL_MIXED_D
+    assert cmp["rel_dE"] <= TOL_MIXED_E
+
+
+def test_small_proxy_fp32():
+    from paper_2205_12182_b200 import PREC_FP32
+    s = make_system("cfg1", n_atoms=400)
+    atoms = np.random.default_rng(2).choice(s.n_atoms, 4, replace=False)
+    D, E, st, stats = _run(s, precision=PREC_FP32)
+    cmp = compare_atoms(s, D, st["e_atom"], atoms)
+    print("fp32 cfg1@400", {k: v for k, v in cmp.items() if k != "ref"})
+    assert cmp["max_abs_dD"] <= TOL_FP32 and cmp["rel_dE"] <= TOL_FP32
+
+
+def test_single_atom_and_errors():
+    from paper_2205_12182_b200 import NolsmError
+    nb = np.array([3], np.int32)
+    rp = np.array([0, 1], np.int64)
+    ci = np.array([0], np.int32)
+    H = np.diag([-1.0, 0.5, 2.0]).reshape(-1)
+    S = np.eye(3).reshape(-1)
+    with _nolsm() as ctx:
+        with pytest.raises(NolsmError) as ei:
+            ctx.density_matrix(0.0, np.zeros(9))
+        assert ei.value.code == 4                                   # ESTATE
+        ctx.assemble(nb, rp, ci, H, S)
+        D = np.zeros(9)
+        ctx.density_matrix(0.0, D)
+        E = ctx.energy()
+        assert np.allclose(D.reshape(3, 3), np.diag([1.0, 0.0, 0.0]), atol=2e-3)   # P2/P7: projector on eps < mu
+        assert abs(E + 1.0) < 2e-3
+        with pytest.raises(NolsmError) as ei:                       # unsorted columns
+            ctx.assemble(np.array([1, 1], np.int32), np.array([0, 2, 4], np.int64), np.array([1, 0, 0, 1], np.int32),
+                         np.ones(4), np.ones(4))
+        assert ei.value.code == 1
+        with pytest.raises(NolsmError) as ei:                       # non-symmetric pattern
+            ctx.assemble(np.array([1, 1], np.int32), np.array([0, 2, 3], np.int64), np.array([0, 1, 1], np.int32),
+                         np.ones(3), np.ones(3))
+        assert ei.value.code == 1
+        with pytest.raises(NolsmError) as ei:                       # missing diagonal
+            ctx.assemble(np.array([1, 1], np.int32), np.array([0, 1, 2], np.int64), np.array([1, 0], np.int32),
+                         np.ones(2), np.ones(2))
+        assert ei.value.code == 1
+
+
+def test_indefinite_S_is_reported(cfg0):
+    """gamma = 1 (BASELINE.json's literal amplitude 0.3) is indefinite on cfg0 (SURVEY finding 1): the
+    Schulz inverse cannot converge for the affected submatrices and the library must say so."""
+    from paper_2205_12182_b200 import NolsmError
+    s = make_system("cfg0", gamma=1.0)
+    with _nolsm() as ctx:
+        ctx.assemble(*_arrays(s))
+        D = torch.zeros(int(s.blk_off()[-1]), dtype=torch.float64, device="cuda")
+        ctx.density_matrix(s.mu, D)
+        with pytest.raises(NolsmError) as ei:
+            ctx.energy()
+        assert ei.value.code == 5
+        st = ctx.atom_stats()
+    bad_gpu = set(np.flatnonzero(st["status"] & 1))
+    bad_ref = set()
+    Hv, Sv = s.fill_np(MAT_H), s.fill_np(MAT_S)
+    blk = s.blk_off()
+    for i in range(s.n_atoms):
+        N = orc.index_set(i, s.row_ptr, s.col_idx)
+        T, _ = orc.submatrix(N, s.atom_nb, s.row_ptr, s.col_idx, blk, Sv)
+        if np.linalg.eigvalsh(T)[0] <= 0:
+            bad_ref.add(i)
+    assert bad_ref and bad_ref <= bad_gpu

@@ -67,6 +67,7 @@ typedef struct {
     double eps_filter;       /* block (j,i) enters N(i) iff max(|H0_ji|max, |S_ji|max) > eps_filter [0 = structural] */
     int batch_atoms;         /* max submatrices resident at once [auto] */
     size_t workspace_bytes;  /* cap on the library-owned dense workspace [auto] */
+    int profile_every;       /* > 0: time every kernel launch of every k-th batch with CUDA events [0 = off] */
 } nolsm_options;
 
 typedef struct {
@@ -129,11 +130,17 @@ int nolsm_get_stats(nolsm_ctx* ctx, nolsm_stats* out);
 int nolsm_get_atom_stats(nolsm_ctx* ctx, int64_t atom_begin, int64_t count, int32_t* dims, int32_t* inv_iters,
                          int32_t* sign_iters, int32_t* status, int32_t* gemms, float* residual, double* e_atom);
 
-/* Device time (ms, CUDA events on the call's stream) spent in the phases of the last density_matrix
- * call: out[0] gather, out[1] GEMM chain incl. scaling mat-vecs, out[2] D columns + scatter,
- * out[3] GEMM kernels only, out[4] number of GEMM launches. Requires NOLSM_TIMING=1 in the
- * environment at nolsm_create (adds stream synchronisations; not for headline timing). */
-int nolsm_get_phase_times(nolsm_ctx* ctx, double* out5);
+/* Per-launch device times of the batches sampled by options.profile_every during the last
+ * density_matrix call (CUDA events recorded on the call's stream around each launch; the sampled
+ * batches only). The gather kernel counts the source elements it read while this is on.
+ *   out[0..2]   gather:  total ms, launches, algorithmic bytes (source blocks read + dense FP16/FP32 written)
+ *   out[3..6]   GEMM:    total ms, launches, useful FLOP (2 n^3 per executed GEMM), tile-padded FLOP
+ *   out[7..9]   D columns + scatter: total ms, launches, algorithmic bytes (X and Y columns read, D row written, H0 row read)
+ *   out[10..11] other kernels (mat-vecs, state, flags): total ms, launches
+ *   out[12]     submatrices in the sampled batches;  out[13] kernel launches of the whole call
+ * n must be >= NOLSM_PROFILE_LEN. Synchronises the stream. */
+#define NOLSM_PROFILE_LEN 14
+int nolsm_get_profile(nolsm_ctx* ctx, double* out, int n);
 
 const char* nolsm_last_error(const nolsm_ctx* ctx);
 

@@ -20,7 +20,7 @@ class NolsmOptions(C.Structure):
     _fields_ = [("precision", C.c_int), ("gemm_backend", C.c_int), ("max_inv_iters", C.c_int),
                 ("max_sign_iters", C.c_int), ("tol_inv", C.c_float), ("tol_sign", C.c_float),
                 ("power_iters_s", C.c_int), ("power_iters_a", C.c_int), ("eps_filter", C.c_double),
-                ("batch_atoms", C.c_int), ("workspace_bytes", C.c_size_t)]
+                ("batch_atoms", C.c_int), ("workspace_bytes", C.c_size_t), ("profile_every", C.c_int)]
 
 
 class NolsmStats(C.Structure):
@@ -65,12 +65,12 @@ def load_library():
     lib.nolsm_gather_submatrix.argtypes = [P, I64, I32, I32, P]
     lib.nolsm_get_stats.argtypes = [P, C.POINTER(NolsmStats)]
     lib.nolsm_get_atom_stats.argtypes = [P, I64, I64, P, P, P, P, P, P, P]
-    lib.nolsm_get_phase_times.argtypes = [P, C.POINTER(C.c_double)]
+    lib.nolsm_get_profile.argtypes = [P, C.POINTER(C.c_double), I32]
     lib.nolsm_last_error.argtypes = [P]
     lib.nolsm_last_error.restype = C.c_char_p
     for f in ("nolsm_create", "nolsm_assemble", "nolsm_density_matrix", "nolsm_density_matrix_range", "nolsm_energy",
               "nolsm_destroy", "nolsm_get_index_set", "nolsm_gather_submatrix", "nolsm_get_stats",
-              "nolsm_get_atom_stats", "nolsm_get_phase_times"):
+              "nolsm_get_atom_stats", "nolsm_get_profile"):
         getattr(lib, f).restype = C.c_int
     _LIB = lib
     return lib
@@ -184,10 +184,13 @@ class Nolsm:
                     ("dims", "inv_iters", "sign_iters", "status", "gemms", "residual", "e_atom")]))
         return d
 
-    def phase_times(self):
-        out = (C.c_double * 5)()
-        self._check(self._lib.nolsm_get_phase_times(self._h, out))
-        return dict(gather_ms=out[0], chain_ms=out[1], scatter_ms=out[2], gemm_ms=out[3], gemm_launches=out[4])
+    def profile(self) -> dict:
+        out = (C.c_double * 14)()
+        self._check(self._lib.nolsm_get_profile(self._h, out, 14))
+        keys = ("gather_ms", "gather_launches", "gather_bytes", "gemm_ms", "gemm_launches", "gemm_flops_useful",
+                "gemm_flops_padded", "dcols_ms", "dcols_launches", "dcols_bytes", "other_ms", "other_launches",
+                "sampled_submatrices", "kernel_launches")
+        return dict(zip(keys, list(out)))
 
     def destroy(self):
         if self._h:

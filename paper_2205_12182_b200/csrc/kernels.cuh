@@ -39,7 +39,7 @@ struct SysView {
 // ---------------------------------------------------------------------------------------------
 template <typename TV, typename T>
 __global__ void __launch_bounds__(256) k_gather(SysView sv, const MatInfo* mats, const TV* S_vals, const TV* H_vals,
-                                                T* base, int max_nset, int max_ld) {
+                                                T* base, int max_nset, int max_ld, unsigned long long* src_elems) {
     extern __shared__ unsigned char sm_raw[];
     long long* s_boff = reinterpret_cast<long long*>(sm_raw);           // [max_nset] blk_off of (j_a, j_b) or -1
     int* s_off = reinterpret_cast<int*>(s_boff + max_nset);             // [max_nset + 1]
@@ -73,6 +73,7 @@ __global__ void __launch_bounds__(256) k_gather(SysView sv, const MatInfo* mats,
         const int nbj = sv.atom_nb[j];
         const int row0 = s_off[a];
         const int total = nbj * mi.ld;
+        int nread = 0;
         for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
             const int rr = idx / mi.ld;
             const int c = idx - rr * mi.ld;
@@ -83,9 +84,15 @@ __global__ void __launch_bounds__(256) k_gather(SysView sv, const MatInfo* mats,
                 if (bo >= 0) {
                     const int nbb = s_off[b + 1] - s_off[b];
                     out = Num<T>::from_d((double)vals[bo + (long long)rr * nbb + (c - s_off[b])]);
+                    ++nread;
                 }
             }
             dst[(long long)(row0 + rr) * mi.ld + c] = out;
+        }
+        if (src_elems) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) nread += __shfl_xor_sync(0xffffffffu, nread, o);
+            if ((threadIdx.x & 31) == 0 && nread) atomicAdd(src_elems, (unsigned long long)nread);
         }
         __syncthreads();
     }

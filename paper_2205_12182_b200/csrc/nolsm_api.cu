@@ -57,7 +57,6 @@ struct nolsm_ctx {
     nolsm_options opt{};
     std::string err;
     bool assembled = false;
-    bool timing = false;
     int sms = 148;
     int tile_target = 0;
 
@@ -97,10 +96,22 @@ struct nolsm_ctx {
     void* d_D_stage = nullptr;
     size_t d_D_stage_bytes = 0;
     int inv_check_from = 3, sign_check_from = 6;
-    double t_phase[5] = {0, 0, 0, 0, 0};
-    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     double gather_bytes = 0, scatter_bytes = 0;
+    size_t last_ds = 8;
+
+    // sampled per-launch profiling (options.profile_every): CUDA events on the launching stream
+    struct Rec { int kind; size_t ev; };
+    std::vector<cudaEvent_t> ev_pool;
+    size_t ev_used = 0;
+    std::vector<Rec> recs;
+    std::vector<std::pair<int64_t, int64_t>> prof_ranges;   // atom ranges of the sampled batches
+    bool prof_on = false;
+    double prof[NOLSM_PROFILE_LEN] = {};
+    unsigned long long* d_gather_elems = nullptr;
+    int64_t launches = 0;
 };
+
+enum { K_GATHER = 0, K_GEMM = 1, K_DCOLS = 2, K_OTHER = 3 };
 
 namespace {
 
@@ -111,6 +122,31 @@ namespace {
             (ctx)->err = std::string(#expr) + ": " + cudaGetErrorString(e_);                       \
             return e_ == cudaErrorMemoryAllocation ? NOLSM_ENOMEM : NOLSM_ECUDA;                   \
         }                                                                                           \
+    } while (0)
+
+size_t prof_begin(nolsm_ctx* c, int kind, cudaStream_t s) {
+    c->launches += 1;
+    if (!c->prof_on) return 0;
+    while (c->ev_pool.size() < c->ev_used + 2) {
+        cudaEvent_t e;
+        cudaEventCreate(&e);
+        c->ev_pool.push_back(e);
+    }
+    const size_t i = c->ev_used;
+    c->ev_used += 2;
+    cudaEventRecord(c->ev_pool[i], s);
+    c->recs.push_back({kind, i});
+    return i;
+}
+void prof_end(nolsm_ctx* c, size_t i, cudaStream_t s) {
+    if (c->prof_on) cudaEventRecord(c->ev_pool[i + 1], s);
+}
+
+#define LAUNCH(c, kind, s, ...)                      \
+    do {                                             \
+        const size_t pi_ = prof_begin(c, kind, s);   \
+        __VA_ARGS__;                                 \
+        prof_end(c, pi_, s);                         \
     } while (0)
 
 int fail(nolsm_ctx* c, int code, const std::string& msg) {
@@ -262,11 +298,11 @@ int launch_gather(nolsm_ctx* c, const Batch& b, const MatInfo* d_mats, cudaStrea
     if (c->val_dtype == NOLSM_DTYPE_F64) {
         auto k = k_gather<double, T>;
         CU_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 48 * 1024)));
-        k<<<grid, 256, smem, s>>>(sys_view(c), d_mats, (const double*)c->dS, (const double*)c->dH, (T*)c->ws, b.max_nset, b.max_ld);
+        LAUNCH(c, K_GATHER, s, k<<<grid, 256, smem, s>>>(sys_view(c), d_mats, (const double*)c->dS, (const double*)c->dH, (T*)c->ws, b.max_nset, b.max_ld, c->prof_on ? c->d_gather_elems : nullptr));
     } else {
         auto k = k_gather<float, T>;
         CU_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 48 * 1024)));
-        k<<<grid, 256, smem, s>>>(sys_view(c), d_mats, (const float*)c->dS, (const float*)c->dH, (T*)c->ws, b.max_nset, b.max_ld);
+        LAUNCH(c, K_GATHER, s, k<<<grid, 256, smem, s>>>(sys_view(c), d_mats, (const float*)c->dS, (const float*)c->dH, (T*)c->ws, b.max_nset, b.max_ld, c->prof_on ? c->d_gather_elems : nullptr));
     }
     CU_TRY(c, cudaGetLastError());
     return NOLSM_OK;
@@ -279,17 +315,16 @@ int launch_gemm(nolsm_ctx* c, const Batch& b, GemmOp op, const CUtensorMap* d_ma
         a.op = op;
         a.maps = d_maps;
         a.base = (__half*)c->ws;
-        gemm_umma_kernel<<<std::min(c->sms, b.ntiles), UMMA_THREADS, UMMA_SMEM_BYTES, s>>>(a);
+        LAUNCH(c, K_GEMM, s, gemm_umma_kernel<<<std::min(c->sms, b.ntiles), UMMA_THREADS, UMMA_SMEM_BYTES, s>>>(a));
     } else {
-        k_gemm_simt<T><<<dim3(b.max_tiles64, b.nmat), 256, 0, s>>>(op, (T*)c->ws);
+        LAUNCH(c, K_GEMM, s, k_gemm_simt<T><<<dim3(b.max_tiles64, b.nmat), 256, 0, s>>>(op, (T*)c->ws));
     }
     CU_TRY(c, cudaGetLastError());
-    c->t_phase[4] += 1;
     return NOLSM_OK;
 }
 
 int count_active(nolsm_ctx* c, int nmat, int phase, cudaStream_t s, int* out) {
-    k_count_active<<<1, 256, 0, s>>>(c->st, nmat, phase, c->d_flag);
+    LAUNCH(c, K_OTHER, s, k_count_active<<<1, 256, 0, s>>>(c->st, nmat, phase, c->d_flag));
     CU_TRY(c, cudaMemcpyAsync(c->h_flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, s));
     CU_TRY(c, cudaStreamSynchronize(s));
     *out = *c->h_flag;
@@ -300,16 +335,16 @@ template <typename T>
 int power_iterations(nolsm_ctx* c, const Batch& b, const MatInfo* d_mats, int buf, int iters, int which, cudaStream_t s) {
     const int nm = b.nmat;
     CU_TRY(c, cudaMemsetAsync(c->d_nrm, 0, sizeof(float) * (size_t)(iters + 1) * c->max_batch, s));
-    k_vec_init<<<dim3((b.max_n + 255) / 256, nm), 256, 0, s>>>(d_mats, c->d_vec, c->d_nrm, c->ldx);
+    LAUNCH(c, K_OTHER, s, k_vec_init<<<dim3((b.max_n + 255) / 256, nm), 256, 0, s>>>(d_mats, c->d_vec, c->d_nrm, c->ldx));
     float* x = c->d_vec;
     float* y = c->d_vec + (size_t)c->max_batch * c->ldx;
     const int gx = std::max(1, std::min((b.max_n + 7) / 8, (4 * c->sms + nm - 1) / nm));
     for (int it = 0; it < iters; ++it) {
-        k_matvec<T><<<dim3(gx, nm), 256, 0, s>>>(d_mats, (const T*)c->ws, buf, x, c->d_nrm + (size_t)it * c->max_batch, y,
-                                                c->d_nrm + (size_t)(it + 1) * c->max_batch, c->ldx);
+        LAUNCH(c, K_OTHER, s, k_matvec<T><<<dim3(gx, nm), 256, 0, s>>>(d_mats, (const T*)c->ws, buf, x, c->d_nrm + (size_t)it * c->max_batch, y,
+                                                                      c->d_nrm + (size_t)(it + 1) * c->max_batch, c->ldx));
         std::swap(x, y);
     }
-    k_rho_finish<<<(nm + 127) / 128, 128, 0, s>>>(c->st, c->d_nrm + (size_t)iters * c->max_batch, nm, which, 1.05f);
+    LAUNCH(c, K_OTHER, s, k_rho_finish<<<(nm + 127) / 128, 128, 0, s>>>(c->st, c->d_nrm + (size_t)iters * c->max_batch, nm, which, 1.05f));
     CU_TRY(c, cudaGetLastError());
     return NOLSM_OK;
 }
@@ -322,11 +357,11 @@ int launch_dcols(nolsm_ctx* c, const Batch& b, const MatInfo* d_mats, TD* D, cud
     if (c->val_dtype == NOLSM_DTYPE_F64) {
         auto k = k_dcols_scatter<T, double, TD>;
         CU_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 48 * 1024)));
-        k<<<grid, 256, smem, s>>>(sys_view(c), d_mats, c->st, (const T*)c->ws, (const double*)c->dH, D, c->d_e_atom, b.max_nset);
+        LAUNCH(c, K_DCOLS, s, k<<<grid, 256, smem, s>>>(sys_view(c), d_mats, c->st, (const T*)c->ws, (const double*)c->dH, D, c->d_e_atom, b.max_nset));
     } else {
         auto k = k_dcols_scatter<T, float, TD>;
         CU_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 48 * 1024)));
-        k<<<grid, 256, smem, s>>>(sys_view(c), d_mats, c->st, (const T*)c->ws, (const float*)c->dH, D, c->d_e_atom, b.max_nset);
+        LAUNCH(c, K_DCOLS, s, k<<<grid, 256, smem, s>>>(sys_view(c), d_mats, c->st, (const T*)c->ws, (const float*)c->dH, D, c->d_e_atom, b.max_nset));
     }
     CU_TRY(c, cudaGetLastError());
     return NOLSM_OK;
@@ -339,11 +374,8 @@ int run_batch(nolsm_ctx* c, const Batch& b, double mu, void* D, int d_dtype, cud
     const CUtensorMap* d_maps = c->plan.d_maps ? c->plan.d_maps + b.first * NBUF : nullptr;
     const int nm = b.nmat;
     int r;
-    float ms;
-    k_state_init<<<(nm + 127) / 128, 128, 0, s>>>(c->st, nm);
-    if (c->timing) cudaEventRecord(c->ev[0], s);
+    LAUNCH(c, K_OTHER, s, k_state_init<<<(nm + 127) / 128, 128, 0, s>>>(c->st, nm));
     if ((r = launch_gather<T>(c, b, d_mats, s))) return r;
-    if (c->timing) cudaEventRecord(c->ev[1], s);
 
     GemmOp op{};
     op.nmat = nm; op.ntiles = b.ntiles; op.mats = d_mats; op.st = c->st;
@@ -351,8 +383,8 @@ int run_batch(nolsm_ctx* c, const Batch& b, double mu, void* D, int d_dtype, cud
 
     // ---- a2: S_sub^-1 by the Schulz iteration, Y0 = I / rho(S) ----
     if ((r = power_iterations<T>(c, b, d_mats, 0, c->opt.power_iters_s, 0, s))) return r;
-    k_schulz_first<T><<<dim3(std::max(1, std::min(64, (b.max_n * b.max_ld + 2047) / 2048)), nm), 256, 0, s>>>(
-        d_mats, c->st, (T*)c->ws, 0, 2);
+    LAUNCH(c, K_OTHER, s, k_schulz_first<T><<<dim3(std::max(1, std::min(64, (b.max_n * b.max_ld + 2047) / 2048)), nm), 256, 0, s>>>(
+                              d_mats, c->st, (T*)c->ws, 0, 2));
     int ran = 1;
     for (int k = 1; k < c->opt.max_inv_iters; ++k) {
         const int ycur = (k & 1) ? 2 : 3, ynext = 5 - ycur;
@@ -398,21 +430,13 @@ int run_batch(nolsm_ctx* c, const Batch& b, double mu, void* D, int d_dtype, cud
         }
     }
     c->sign_check_from = std::max(2, ran - 1);
-    if (c->timing) cudaEventRecord(c->ev[2], s);
 
     // ---- a6 + a7: D columns, scatter, energy partials ----
     if (d_dtype == NOLSM_DTYPE_F64) r = launch_dcols<T, double>(c, b, d_mats, (double*)D, s);
     else r = launch_dcols<T, float>(c, b, d_mats, (float*)D, s);
     if (r) return r;
-    k_save_stats<<<(nm + 127) / 128, 128, 0, s>>>(d_mats, c->st, nm, c->a_inv, c->a_sign, c->a_status, c->a_gemms,
-                                                  c->a_res, c->a_rho);
-    if (c->timing) {
-        cudaEventRecord(c->ev[3], s);
-        CU_TRY(c, cudaEventSynchronize(c->ev[3]));
-        cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]); c->t_phase[0] += ms;
-        cudaEventElapsedTime(&ms, c->ev[1], c->ev[2]); c->t_phase[1] += ms;
-        cudaEventElapsedTime(&ms, c->ev[2], c->ev[3]); c->t_phase[2] += ms;
-    }
+    LAUNCH(c, K_OTHER, s, k_save_stats<<<(nm + 127) / 128, 128, 0, s>>>(d_mats, c->st, nm, c->a_inv, c->a_sign, c->a_status,
+                                                                        c->a_gemms, c->a_res, c->a_rho));
     CU_TRY(c, cudaGetLastError());
     return NOLSM_OK;
 }
@@ -453,7 +477,7 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
     if (o.eps_filter < 0) { delete c; return NOLSM_EINVAL; }
     cudaSetDevice(cuda_device);
     cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, cuda_device);
-    c->timing = getenv_int("NOLSM_TIMING", 0) != 0;
+    if (getenv_int("NOLSM_PROFILE_EVERY", 0) > 0) o.profile_every = getenv_int("NOLSM_PROFILE_EVERY", 0);
     c->tile_target = getenv_int("NOLSM_BATCH_TILES", 8 * c->sms);
     if (use_umma(c)) {
         if (cudaFuncSetAttribute(gemm_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, UMMA_SMEM_BYTES) != cudaSuccess) {
@@ -462,7 +486,6 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
             return NOLSM_ECUDA;
         }
     }
-    for (int i = 0; i < 4; ++i) cudaEventCreate(&c->ev[i]);
     *out = c;
     return NOLSM_OK;
 }
@@ -474,7 +497,7 @@ int nolsm_destroy(nolsm_ctx* c) {
     if (c->plan.d_maps) cudaFree(c->plan.d_maps);
     c->plan.d_mats = nullptr; c->plan.d_maps = nullptr;
     free_assembled(c);
-    for (int i = 0; i < 4; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return NOLSM_OK;
 }
@@ -652,6 +675,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     if ((r = dmalloc(c, (void**)&c->d_vec, sizeof(float) * 2 * (size_t)mb * c->ldx))) return r;
     if ((r = dmalloc(c, (void**)&c->d_nrm, sizeof(float) * (size_t)pit * mb))) return r;
     if ((r = dmalloc(c, (void**)&c->d_flag, 16))) return r;
+    if ((r = dmalloc(c, (void**)&c->d_gather_elems, 16))) return r;
     CU_TRY(c, cudaMallocHost((void**)&c->h_flag, 16));
     if ((r = dmalloc(c, (void**)&c->a_inv, 4 * n_atoms))) return r;
     if ((r = dmalloc(c, (void**)&c->a_sign, 4 * n_atoms))) return r;
@@ -683,6 +707,7 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
     int r;
     if ((r = build_plan(c, a0, a1, s))) return r;
     const size_t ds = d_dtype == NOLSM_DTYPE_F64 ? 8 : 4;
+    c->last_ds = ds;
     const int64_t v0 = c->blk_off[c->row_ptr[a0]], v1 = c->blk_off[c->row_ptr[a1]];
     // device view of the output rows [a0, a1): D_dev points at element 0 of the whole array
     char* D_dev;
@@ -701,11 +726,16 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
     }
     CU_TRY(c, cudaMemsetAsync(D_dev + (size_t)v0 * ds, 0, (size_t)(v1 - v0) * ds, s));
     CU_TRY(c, cudaMemsetAsync(c->d_e_atom + a0, 0, 8 * (a1 - a0), s));
-    for (int i = 0; i < 5; ++i) c->t_phase[i] = 0;
     c->gather_bytes = 0; c->scatter_bytes = 0;
+    c->ev_used = 0; c->recs.clear(); c->prof_ranges.clear(); c->launches = 0;
+    CU_TRY(c, cudaMemsetAsync(c->d_gather_elems, 0, 8, s));
+    int64_t bi = 0;
     for (const Batch& b : c->plan.batches) {
+        c->prof_on = c->opt.profile_every > 0 && (bi++ % c->opt.profile_every) == 0;
+        if (c->prof_on) c->prof_ranges.push_back({a0 + b.first, a0 + b.first + b.nmat});
         r = c->opt.precision == NOLSM_PREC_FP32 ? run_batch<float>(c, b, mu, D_dev, d_dtype, s)
                                                 : run_batch<__half>(c, b, mu, D_dev, d_dtype, s);
+        c->prof_on = false;
         if (r) return r;
     }
     const size_t es = elem_size(c);
@@ -837,9 +867,43 @@ int nolsm_get_stats(nolsm_ctx* c, nolsm_stats* out) {
     return NOLSM_OK;
 }
 
-int nolsm_get_phase_times(nolsm_ctx* c, double* out5) {
-    if (!c || !out5) return NOLSM_EINVAL;
-    for (int i = 0; i < 5; ++i) out5[i] = c->t_phase[i];
+int nolsm_get_profile(nolsm_ctx* c, double* out, int n) {
+    if (!c || !out || n < NOLSM_PROFILE_LEN) return NOLSM_EINVAL;
+    if (!c->have_result) return fail(c, NOLSM_ESTATE, "no density matrix has been computed");
+    cudaSetDevice(c->dev);
+    CU_TRY(c, cudaStreamSynchronize(c->last_stream));
+    double ms[4] = {0, 0, 0, 0}, cnt[4] = {0, 0, 0, 0};
+    for (const nolsm_ctx::Rec& r : c->recs) {
+        float t = 0;
+        if (cudaEventElapsedTime(&t, c->ev_pool[r.ev], c->ev_pool[r.ev + 1]) != cudaSuccess) { cudaGetLastError(); continue; }
+        ms[r.kind] += t; cnt[r.kind] += 1;
+    }
+    double fl_useful = 0, fl_padded = 0, gbytes_w = 0, sbytes = 0, natoms = 0;
+    const size_t es = elem_size(c), vs = c->val_dtype == NOLSM_DTYPE_F64 ? 8 : 4;
+    for (auto& pr : c->prof_ranges) {
+        const int64_t cntA = pr.second - pr.first;
+        std::vector<int32_t> gm(cntA);
+        CU_TRY(c, cudaMemcpy(gm.data(), c->a_gemms + pr.first, 4 * cntA, cudaMemcpyDeviceToHost));
+        for (int64_t a = pr.first; a < pr.second; ++a) {
+            MatInfo mi;
+            fill_matinfo(c, a, mi);
+            const double d = mi.n;
+            fl_useful += 2.0 * d * d * d * gm[a - pr.first];
+            const double pm = (double)((mi.n + BM - 1) / BM) * BM, pn = (double)mi.ntn * mi.bn, pk = (double)((mi.n + 15) / 16) * 16;
+            fl_padded += 2.0 * pm * pn * pk * gm[a - pr.first];
+            gbytes_w += 2.0 * d * mi.ld * es;
+            const double nv = (double)(c->blk_off[c->row_ptr[a + 1]] - c->blk_off[c->row_ptr[a]]);
+            sbytes += nv * (c->last_ds + vs) + d * mi.ld * es + d * mi.nbi * es;
+            natoms += 1;
+        }
+    }
+    unsigned long long ge = 0;
+    CU_TRY(c, cudaMemcpy(&ge, c->d_gather_elems, 8, cudaMemcpyDeviceToHost));
+    out[0] = ms[K_GATHER]; out[1] = cnt[K_GATHER]; out[2] = gbytes_w + (double)ge * vs;
+    out[3] = ms[K_GEMM]; out[4] = cnt[K_GEMM]; out[5] = fl_useful; out[6] = fl_padded;
+    out[7] = ms[K_DCOLS]; out[8] = cnt[K_DCOLS]; out[9] = sbytes;
+    out[10] = ms[K_OTHER]; out[11] = cnt[K_OTHER];
+    out[12] = natoms; out[13] = (double)c->launches;
     return NOLSM_OK;
 }
 

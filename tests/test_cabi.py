@@ -1,0 +1,76 @@
+"""CPU-side checks of the boundary: the C-ABI library builds, loads, exports every symbol that
+include/nolsm.h declares, and the binding's structs match the header. No compute calls (no GPU here)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2205_12182_b200 import build, load_library
+    build.build()
+    return load_library()
+
+
+def _declared_functions():
+    text = open(os.path.join(ROOT, "include", "nolsm.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(nolsm_[a-z_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    names = _declared_functions()
+    assert {"nolsm_create", "nolsm_assemble", "nolsm_density_matrix", "nolsm_energy", "nolsm_destroy"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in nolsm.h but not exported"
+
+
+def test_option_and_stats_structs_match_header():
+    from paper_2205_12182_b200 import NolsmOptions, NolsmStats
+    text = open(os.path.join(ROOT, "include", "nolsm.h")).read()
+    opt = re.search(r"typedef struct \{(.*?)\} nolsm_options;", text, flags=re.S).group(1)
+    opt = re.sub(r"/\*.*?\*/", "", opt, flags=re.S)
+    fields = [m.group(1) for m in re.finditer(r"\b([a-z_0-9]+)\s*;", opt)]
+    assert fields == [f for f, _ in NolsmOptions._fields_]
+    st = re.search(r"typedef struct \{((?:(?!typedef).)*?)\} nolsm_stats;", text, flags=re.S).group(1)
+    st = re.sub(r"/\*.*?\*/", "", st, flags=re.S)
+    names = []
+    for decl in st.split(";"):
+        decl = decl.strip()
+        if decl:
+            names += [x.strip() for x in decl.split(None, 1)[1].split(",")]
+    assert names == [f for f, _ in NolsmStats._fields_]
+
+
+def test_create_fails_loudly_without_a_gpu(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    from paper_2205_12182_b200 import Nolsm, NolsmError
+    with pytest.raises(NolsmError):
+        Nolsm(0)
+
+
+def test_null_arguments_are_rejected(lib):
+    assert lib.nolsm_create(None, 0, None) == 1
+    assert lib.nolsm_destroy(None) == 1
+    e = ctypes.c_double()
+    assert lib.nolsm_energy(None, ctypes.byref(e)) == 1
+    assert lib.nolsm_last_error(None) == b"null context"
+
+
+def test_product_path_does_not_touch_the_oracle():
+    """The package must not import, link or execute anything under oracle/ (and vice versa)."""
+    pkg = os.path.join(ROOT, "paper_2205_12182_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                assert "oracle" not in open(os.path.join(dirpath, f)).read().lower(), f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith(".py"):
+            assert "paper_2205_12182_b200" not in open(os.path.join(ROOT, "oracle", f)).read().replace(
+                "(paper_2205_12182_b200/)", "")

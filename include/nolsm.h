@@ -65,14 +65,14 @@ typedef struct {
     int power_iters_s;       /* power iterations for rho(S_sub) [6] */
     int power_iters_a;       /* power iterations for rho(A_sub) [12] */
     double eps_filter;       /* block (j,i) enters N(i) iff max(|H0_ji|max, |S_ji|max) > eps_filter [0 = structural] */
-    int batch_atoms;         /* max submatrices resident at once [auto] */
+    int batch_atoms;         /* workspace slots = submatrices resident at once [auto: ~16 waves of GEMM tiles] */
     size_t workspace_bytes;  /* cap on the library-owned dense workspace [auto] */
-    int profile_every;       /* > 0: time every kernel launch of every k-th batch with CUDA events [0 = off] */
+    int profile_every;       /* > 0: every k-th round runs eagerly with CUDA events around each launch [0 = off] */
 } nolsm_options;
 
 typedef struct {
     int64_t n_atoms;
-    int64_t n_batches;
+    int64_t n_batches;            /* engine rounds of the last density_matrix call */
     int64_t dim_min, dim_max;
     double dim_mean;
     int64_t sum_inv_iters, sum_sign_iters;
@@ -99,7 +99,10 @@ int nolsm_assemble(nolsm_ctx* ctx, int64_t n_atoms, const int32_t* atom_nb, cons
                    void* cuda_stream);
 
 /* a1-a7 for all atoms: gather, Schulz inverse, spectral scaling, Newton-Schulz sign (Eq. 6),
- * convergence tests, D columns, scatter and energy partials. Asynchronous on `cuda_stream`.
+ * convergence tests, D columns, scatter and energy partials. The work is ordered after everything
+ * already enqueued on `cuda_stream`, and `cuda_stream` is made to wait for it; the call itself returns
+ * once the last engine round has been enqueued (the host replays one CUDA graph per round and reads a
+ * device-written progress counter to know when to stop).
  *   D_vals   d_dtype[blk_off[nnzb]]   host or device; blocks outside every N(i) are zeroed. */
 int nolsm_density_matrix(nolsm_ctx* ctx, double mu, void* D_vals, int d_dtype, void* cuda_stream);
 
@@ -130,14 +133,14 @@ int nolsm_get_stats(nolsm_ctx* ctx, nolsm_stats* out);
 int nolsm_get_atom_stats(nolsm_ctx* ctx, int64_t atom_begin, int64_t count, int32_t* dims, int32_t* inv_iters,
                          int32_t* sign_iters, int32_t* status, int32_t* gemms, float* residual, double* e_atom);
 
-/* Per-launch device times of the batches sampled by options.profile_every during the last
- * density_matrix call (CUDA events recorded on the call's stream around each launch; the sampled
- * batches only). The gather kernel counts the source elements it read while this is on.
+/* Per-launch device times of the rounds sampled by options.profile_every during the last
+ * density_matrix call (those rounds run eagerly on one stream with CUDA events recorded around each
+ * launch; all other rounds replay the CUDA graph). FLOP and byte counts cover the sampled rounds only.
  *   out[0..2]   gather:  total ms, launches, algorithmic bytes (source blocks read + dense FP16/FP32 written)
  *   out[3..6]   GEMM:    total ms, launches, useful FLOP (2 n^3 per executed GEMM), tile-padded FLOP
  *   out[7..9]   D columns + scatter: total ms, launches, algorithmic bytes (X and Y columns read, D row written, H0 row read)
  *   out[10..11] other kernels (mat-vecs, state, flags): total ms, launches
- *   out[12]     submatrices in the sampled batches;  out[13] kernel launches of the whole call
+ *   out[12]     submatrices gathered in the sampled rounds;  out[13] kernel launches of the whole call
  * n must be >= NOLSM_PROFILE_LEN. Synchronises the stream. */
 #define NOLSM_PROFILE_LEN 14
 int nolsm_get_profile(nolsm_ctx* ctx, double* out, int n);

@@ -7,7 +7,8 @@
 // matrices are row-major, so A is a K-major operand and B an MN-major operand of the UMMA; X*X
 // therefore needs no transposed copy of X.
 //
-// Persistent kernel: grid = #SMs, each CTA walks the batch tile list with stride gridDim.x.
+// Persistent kernel: grid = #SMs, each CTA walks the round's tile list (all slots that take part in
+// this launch, nolsm_device.cuh) with stride gridDim.x; the tile count is read from device memory.
 // Warp roles: warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer, warps 2..5 = epilogue.
 #pragma once
 #include "nolsm_device.cuh"
@@ -134,9 +135,10 @@ __device__ __forceinline__ uint32_t make_idesc_f16(int m, int n) {
 }
 
 struct UmmaArgs {
-    GemmOp op;
-    const CUtensorMap* maps;    // [nmat][NBUF], box 64 x 64, SWIZZLE_128B, true dims n x n
+    Engine e;
+    const CUtensorMap* maps;    // [S][NBUF]: cap x cap, row pitch ld, box 64 x 64, SWIZZLE_128B
     __half* base;               // workspace base
+    int launch;                 // 0 or 1: which op table of the round
 };
 
 __device__ __forceinline__ void st_half8(__half* p, const float* v) {
@@ -154,7 +156,9 @@ __device__ __forceinline__ void st_half8(__half* p, const float* v) {
 
 __global__ void __launch_bounds__(UMMA_THREADS, 1) gemm_umma_kernel(const __grid_constant__ UmmaArgs args) {
     extern __shared__ uint8_t smem_raw[];
-    const GemmOp& op = args.op;
+    const Engine& e = args.e;
+    const SlotOp* ops = e.ops + args.launch * e.S;
+    const int ntiles = e.ntiles[args.launch];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_base = smem_base + UMMA_STAGES * STAGE_BYTES;
     // barrier layout (8 B each): full[S], empty[S], tmem_full[2], tmem_empty[2], then tmem ptr
@@ -166,6 +170,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) gemm_umma_kernel(const __grid
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
+    if ((int)blockIdx.x >= ntiles) return;           // whole CTA idle this launch (uniform)
 
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < UMMA_STAGES; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
@@ -183,17 +188,17 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) gemm_umma_kernel(const __grid
         // ================= TMA producer =================
         if (lane == 0) {
             int stage = 0; uint32_t phase = 0;
-            for (int tile = blockIdx.x; tile < op.ntiles; tile += gridDim.x) {
-                const int m = find_matrix(op.mats, op.nmat, tile);
-                if (!gate_open(op, m)) continue;
-                const MatInfo mi = op.mats[m];
-                const int t = tile - mi.tile_start;
-                const int tm = t / mi.ntn, tn = t - tm * mi.ntn;
-                const int a_buf = op.a_buf >= 0 ? op.a_buf : op.st.ybuf[m];
-                const CUtensorMap* map_a = args.maps + (size_t)m * NBUF + a_buf;
-                const CUtensorMap* map_b = args.maps + (size_t)m * NBUF + op.b_buf;
-                const int nkb = (mi.n + BK - 1) / BK;
-                const int nbox = (mi.bn + 63) >> 6;
+            for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+                const int slot = find_slot(ops, e.S, tile);
+                const SlotOp op = ops[slot];
+                const Slot& sl = e.slots[slot];
+                const int n16 = sl.n16, bn = sl.bn, ntn = sl.ntn;
+                const int t = tile - op.tile_start;
+                const int tm = t / ntn, tn = t - tm * ntn;
+                const CUtensorMap* map_a = args.maps + (size_t)slot * NBUF + op.a_buf;
+                const CUtensorMap* map_b = args.maps + (size_t)slot * NBUF + op.b_buf;
+                const int nkb = (n16 + BK - 1) / BK;
+                const int nbox = (bn + 63) >> 6;
                 const uint32_t bytes = A_STAGE_BYTES + nbox * B_BOX_BYTES;
                 for (int kb = 0; kb < nkb; ++kb) {
                     ptx::mbar_wait(empty_bar(stage), phase ^ 1);
@@ -203,7 +208,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) gemm_umma_kernel(const __grid
                     ptx::tma_load_2d(sa, map_a, kb * BK, tm * BM, full_bar(stage));
                     ptx::tma_load_2d(sa + 8192, map_a, kb * BK, tm * BM + 64, full_bar(stage));
                     for (int q = 0; q < nbox; ++q)
-                        ptx::tma_load_2d(sb + q * B_BOX_BYTES, map_b, tn * mi.bn + q * 64, kb * BK, full_bar(stage));
+                        ptx::tma_load_2d(sb + q * B_BOX_BYTES, map_b, tn * bn + q * 64, kb * BK, full_bar(stage));
                     if (++stage == UMMA_STAGES) { stage = 0; phase ^= 1; }
                 }
             }
@@ -212,12 +217,12 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) gemm_umma_kernel(const __grid
         // ================= MMA issuer =================
         int stage = 0; uint32_t phase = 0;
         int acc = 0; uint32_t acc_phase = 0;
-        for (int tile = blockIdx.x; tile < op.ntiles; tile += gridDim.x) {
-            const int m = find_matrix(op.mats, op.nmat, tile);
-            if (!gate_open(op, m)) continue;
-            const MatInfo mi = op.mats[m];
-            const int nkb = (mi.n + BK - 1) / BK;
-            const uint32_t idesc = make_idesc_f16(BM, mi.bn);
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            const int slot = find_slot(ops, e.S, tile);
+            const Slot& sl = e.slots[slot];
+            const int n16 = sl.n16;
+            const int nkb = (n16 + BK - 1) / BK;
+            const uint32_t idesc = make_idesc_f16(BM, sl.bn);
             ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1);
             ptx::tc_fence_after();
             const uint32_t d_tmem = tmem_base + acc * 256;
@@ -227,7 +232,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) gemm_umma_kernel(const __grid
                 if (lane == 0) {
                     const uint32_t sa = smem_base + stage * STAGE_BYTES;
                     const uint32_t sb = sa + A_STAGE_BYTES;
-                    int k16 = (mi.n - kb * BK + 15) >> 4;
+                    int k16 = (n16 - kb * BK) >> 4;
                     k16 = k16 > 4 ? 4 : k16;
                     for (int k = 0; k < k16; ++k) {
                         const uint64_t da = make_smem_desc(sa + k * 32, 16, 1024);
@@ -246,46 +251,43 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) gemm_umma_kernel(const __grid
         // ================= epilogue (warps 2..5) =================
         const int q = warp & 3;                       // TMEM lane group this warp may access
         int acc = 0; uint32_t acc_phase = 0;
-        for (int tile = blockIdx.x; tile < op.ntiles; tile += gridDim.x) {
-            const int m = find_matrix(op.mats, op.nmat, tile);
-            if (!gate_open(op, m)) continue;
-            const MatInfo mi = op.mats[m];
-            const int t = tile - mi.tile_start;
-            const int tm = t / mi.ntn, tn = t - tm * mi.ntn;
-            const int ntm = (mi.n + BM - 1) / BM;
-            const float alpha = op.alpha_arr ? op.alpha_arr[m] : op.alpha;
-            __half* C = args.base + mi.off + (long long)op.c_buf * mi.bufsz;
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            const int slot = find_slot(ops, e.S, tile);
+            const SlotOp op = ops[slot];
+            const Slot& sl = e.slots[slot];
+            const int n = sl.n, n16 = sl.n16, bn = sl.bn, ntn = sl.ntn;
+            const int t = tile - op.tile_start;
+            const int tm = t / ntn, tn = t - tm * ntn;
+            __half* C = args.base + buf_off(e, slot, op.c_buf);
             const int row = tm * BM + q * 32 + lane;
-            const int col0 = tn * mi.bn;
+            const int col0 = tn * bn;
             ptx::mbar_wait(tfull_bar(acc), acc_phase);
             ptx::tc_fence_after();
             float rsum = 0.f;
-            for (int c = 0; c < mi.bn; c += 32) {
-                if (col0 + c >= mi.n) break;                       // warp-uniform
+            for (int c = 0; c < bn; c += 32) {
+                if (col0 + c >= n16) break;                        // warp-uniform
                 uint32_t v[32];
                 ptx::tmem_ld_32x32(tmem_base + acc * 256 + ((uint32_t)(q * 32) << 16) + c, v);
                 ptx::tmem_ld_wait();
-                const int cw = min(32, mi.bn - c);                 // columns of this chunk inside the tile
-                if (row < mi.n) {
+                if (row < n16) {
                     float f[32];
 #pragma unroll
                     for (int j = 0; j < 32; ++j) {
                         const int col = col0 + c + j;
-                        const float x = alpha * __uint_as_float(v[j]);
-                        const float delta = (col == row) ? 1.f : 0.f;
-                        if (op.want_res && j < cw && col < mi.n) {
-                            const float d = x - delta;
+                        const float x = op.alpha * __uint_as_float(v[j]);
+                        const float delta = (col == row && row < n) ? 1.f : 0.f;
+                        if (op.want_res) {                             // pad rows / columns contribute exactly 0
+                            const float d = (c + j < bn && col < n16) ? x - delta : 0.f;
                             rsum += d * d;
                         }
                         f[j] = op.sgn * x + op.beta * delta;
                     }
-                    __half* crow = C + (size_t)row * mi.ld + col0 + c;
-                    if (cw == 32 && col0 + c + 32 <= mi.n) {
+                    __half* crow = C + (size_t)row * e.ld + col0 + c;
+                    // bn and n16 are multiples of 16: the valid part of this chunk is 16 or 32 columns
+                    const int cw = min(min(32, bn - c), n16 - (col0 + c));
 #pragma unroll
-                        for (int j = 0; j < 32; j += 8) st_half8(crow + j, f + j);
-                    } else {
-                        for (int j = 0; j < cw && col0 + c + j < mi.n; ++j) crow[j] = __float2half_rn(f[j]);
-                    }
+                    for (int j = 0; j < 32; j += 8)
+                        if (j < cw) st_half8(crow + j, f + j);
                 }
             }
             ptx::tc_fence_before();
@@ -294,11 +296,11 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) gemm_umma_kernel(const __grid
             if (op.want_res) {
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) rsum += __shfl_xor_sync(0xffffffffu, rsum, o);
-                if (lane == 0 && rsum != 0.f) atomicAdd(&op.st.res_acc[m], rsum);
+                if (lane == 0 && rsum != 0.f) atomicAdd(&e.slots[slot].res_acc, rsum);
             }
             // all four epilogue warps done with this tile -> one thread reports it
             asm volatile("bar.sync 1, 128;" ::: "memory");
-            if (warp == 2 && lane == 0) tile_finished(op, m, ntm * mi.ntn);
+            if (warp == 2 && lane == 0) tile_finished(e, slot, op);
             if (++acc == 2) { acc = 0; acc_phase ^= 1; }
         }
     }

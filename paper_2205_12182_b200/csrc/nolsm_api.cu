@@ -20,22 +20,6 @@ using namespace nolsm;
 
 namespace {
 
-struct Batch {
-    int64_t first;   // index of the first matrix in the plan's MatInfo array
-    int nmat;
-    int ntiles;      // UMMA tiles (128 x bn)
-    int max_tiles64; // max over matrices of ceil(n/64)^2 (SIMT grid)
-    int max_n, max_ld, max_nset, max_nbi;
-};
-
-struct Plan {
-    int64_t a0 = -1, a1 = -1;
-    std::vector<Batch> batches;
-    std::vector<MatInfo> mats;
-    MatInfo* d_mats = nullptr;
-    CUtensorMap* d_maps = nullptr;
-};
-
 template <typename F>
 void parallel_for(int64_t n, F f) {
     unsigned nt = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
@@ -50,6 +34,9 @@ void parallel_for(int64_t n, F f) {
     for (auto& x : th) x.join();
 }
 
+enum { K_GATHER = 0, K_GEMM = 1, K_DCOLS = 2, K_OTHER = 3 };
+constexpr int ROUND_DEPTH = 4;    // rounds kept in flight ahead of the device
+
 }  // namespace
 
 struct nolsm_ctx {
@@ -58,13 +45,13 @@ struct nolsm_ctx {
     std::string err;
     bool assembled = false;
     int sms = 148;
-    int tile_target = 0;
 
     // host copy of the pattern and derived index data
     int64_t n_atoms = 0, nnzb = 0, nvals = 0;
     std::vector<int32_t> atom_nb, col_idx, nset_atom, nset_slot, nset_off, dim, pos;
     std::vector<int64_t> row_ptr, blk_off, nset_ptr;
     bool filtered = false;
+    int max_n = 0, max_nset = 0, max_nbi = 0;
 
     // device arrays
     std::vector<void*> owned;           // everything cudaMalloc'ed by assemble (freed on re-assemble / destroy)
@@ -73,21 +60,20 @@ struct nolsm_ctx {
     const void *dH = nullptr, *dS = nullptr;
     int val_dtype = NOLSM_DTYPE_F64;
 
+    // engine (nolsm_device.cuh): slots, op tables, feed, workspace, tensor maps
+    Engine eng{};
     void* ws = nullptr;
     size_t ws_bytes = 0;
-    int max_batch = 0;
-    Plan plan;
-
-    // batch state + per-atom results
-    void* state_mem = nullptr;
-    BatchState st{};
+    CUtensorMap* d_maps = nullptr;
     float *d_vec = nullptr, *d_nrm = nullptr;
-    int ldx = 0;
-    int* d_flag = nullptr;
-    int* h_flag = nullptr;
-    int *a_inv = nullptr, *a_sign = nullptr, *a_status = nullptr, *a_gemms = nullptr;
-    float *a_res = nullptr, *a_rho = nullptr;
+    int* h_done = nullptr;              // pinned, mapped
+    int *d_dim = nullptr, *d_pos = nullptr;
     double* d_e_atom = nullptr;
+    cudaStream_t s_main = nullptr, s_x = nullptr, s_f = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_x = nullptr, ev_f = nullptr, ev_in = nullptr, ev_out = nullptr;
+    cudaEvent_t ev_round[ROUND_DEPTH] = {};
+    cudaGraphExec_t graph_exec = nullptr;
+    bool use_graph = true;
 
     // last density call
     cudaStream_t last_stream = nullptr;
@@ -95,23 +81,17 @@ struct nolsm_ctx {
     bool have_result = false;
     void* d_D_stage = nullptr;
     size_t d_D_stage_bytes = 0;
-    int inv_check_from = 3, sign_check_from = 6;
-    double gather_bytes = 0, scatter_bytes = 0;
     size_t last_ds = 8;
+    int64_t rounds = 0;
 
     // sampled per-launch profiling (options.profile_every): CUDA events on the launching stream
     struct Rec { int kind; size_t ev; };
     std::vector<cudaEvent_t> ev_pool;
     size_t ev_used = 0;
     std::vector<Rec> recs;
-    std::vector<std::pair<int64_t, int64_t>> prof_ranges;   // atom ranges of the sampled batches
     bool prof_on = false;
-    double prof[NOLSM_PROFILE_LEN] = {};
-    unsigned long long* d_gather_elems = nullptr;
     int64_t launches = 0;
 };
-
-enum { K_GATHER = 0, K_GEMM = 1, K_DCOLS = 2, K_OTHER = 3 };
 
 namespace {
 
@@ -169,9 +149,10 @@ int dmalloc(nolsm_ctx* c, void** p, size_t bytes) {
 void free_assembled(nolsm_ctx* c) {
     for (void* p : c->owned) cudaFree(p);
     c->owned.clear();
-    if (c->h_flag) { cudaFreeHost(c->h_flag); c->h_flag = nullptr; }
+    if (c->h_done) { cudaFreeHost(c->h_done); c->h_done = nullptr; }
     if (c->d_D_stage) { cudaFree(c->d_D_stage); c->d_D_stage = nullptr; c->d_D_stage_bytes = 0; }
-    c->ws = nullptr; c->plan = Plan(); c->assembled = false; c->have_result = false;
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    c->ws = nullptr; c->assembled = false; c->have_result = false;
 }
 
 // Obtains a device view of a host-or-device array (copies host data into an owned buffer).
@@ -201,87 +182,12 @@ bool use_umma(const nolsm_ctx* c) {
     return c->opt.gemm_backend != NOLSM_GEMM_SIMT;
 }
 
-void fill_matinfo(const nolsm_ctx* c, int64_t atom, MatInfo& mi) {
-    const int n = c->dim[atom];
-    mi.n = n;
-    mi.ld = (n + 7) / 8 * 8;
-    mi.pos = c->pos[atom];
-    mi.nbi = c->atom_nb[atom];
-    mi.ntn = (n + 255) / 256;
-    int bn = ((n + mi.ntn - 1) / mi.ntn + 15) / 16 * 16;
-    mi.bn = std::min(bn, 256);
-    mi.ntn = (n + mi.bn - 1) / mi.bn;
-    mi.atom = (int)atom;
-    mi.bufsz = ((long long)n * mi.ld + 63) / 64 * 64;
-    mi.tile_start = 0;
-    mi.off = 0;
-}
-
-// Greedy batch plan over atoms [a0, a1): a batch is closed when it reaches the tile target, the
-// matrix cap or the workspace capacity.
-int build_plan(nolsm_ctx* c, int64_t a0, int64_t a1, cudaStream_t s) {
-    Plan& p = c->plan;
-    if (p.a0 == a0 && p.a1 == a1) return NOLSM_OK;
-    if (p.d_mats) { cudaFree(p.d_mats); p.d_mats = nullptr; }
-    if (p.d_maps) { cudaFree(p.d_maps); p.d_maps = nullptr; }
-    p = Plan();
-    p.mats.resize(a1 - a0);
-    const size_t es = elem_size(c);
-    Batch cur{};
-    cur.first = 0;
-    long long off = 0;
-    auto close = [&]() { if (cur.nmat) { p.batches.push_back(cur); } };
-    for (int64_t a = a0; a < a1; ++a) {
-        MatInfo mi;
-        fill_matinfo(c, a, mi);
-        const long long need = mi.bufsz * NBUF;
-        if ((size_t)(need * es) > c->ws_bytes) return fail(c, NOLSM_ENOMEM, "workspace too small for one submatrix");
-        const bool full = cur.nmat > 0 && (cur.nmat >= c->max_batch || cur.ntiles >= c->tile_target ||
-                                           (size_t)((off + need) * es) > c->ws_bytes);
-        if (full) {
-            close();
-            cur = Batch{};
-            cur.first = a - a0;
-            off = 0;
-        }
-        mi.off = off;
-        mi.tile_start = cur.ntiles;
-        off += need;
-        const int ntm = (mi.n + BM - 1) / BM;
-        cur.ntiles += ntm * mi.ntn;
-        const int t64 = (mi.n + 63) / 64;
-        cur.max_tiles64 = std::max(cur.max_tiles64, t64 * t64);
-        cur.max_n = std::max(cur.max_n, mi.n);
-        cur.max_ld = std::max(cur.max_ld, mi.ld);
-        cur.max_nset = std::max<int>(cur.max_nset, (int)(c->nset_ptr[a + 1] - c->nset_ptr[a]));
-        cur.max_nbi = std::max(cur.max_nbi, mi.nbi);
-        cur.nmat += 1;
-        p.mats[a - a0] = mi;
-    }
-    close();
-    CU_TRY(c, cudaMalloc((void**)&p.d_mats, std::max<size_t>(1, p.mats.size()) * sizeof(MatInfo)));
-    CU_TRY(c, cudaMemcpyAsync(p.d_mats, p.mats.data(), p.mats.size() * sizeof(MatInfo), cudaMemcpyHostToDevice, s));
-    if (use_umma(c)) {
-        std::vector<CUtensorMap> maps(p.mats.size() * NBUF);
-        std::atomic<bool> ok{true};
-        if (!encode_tiled_fn()) return fail(c, NOLSM_ECUDA, "cuTensorMapEncodeTiled not available");
-        parallel_for((int64_t)p.mats.size(), [&](int64_t b, int64_t e) {
-            for (int64_t i = b; i < e; ++i) {
-                const MatInfo& mi = p.mats[i];
-                for (int k = 0; k < NBUF; ++k) {
-                    const __half* base = (const __half*)c->ws + mi.off + (long long)k * mi.bufsz;
-                    if (!make_tmap_f16_64x64(&maps[i * NBUF + k], base, mi.n, mi.ld)) ok = false;
-                }
-            }
-        });
-        if (!ok) return fail(c, NOLSM_ECUDA, "cuTensorMapEncodeTiled failed");
-        CU_TRY(c, cudaMalloc((void**)&p.d_maps, std::max<size_t>(1, maps.size()) * sizeof(CUtensorMap)));
-        CU_TRY(c, cudaMemcpyAsync(p.d_maps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, s));
-        CU_TRY(c, cudaStreamSynchronize(s));   // `maps` is a local
-    }
-    p.a0 = a0;
-    p.a1 = a1;
-    return NOLSM_OK;
+void host_tiling(int n16, int& ntm, int& ntn, int& bn) {      // mirrors choose_tiling (kernels.cuh)
+    ntm = (n16 + BM - 1) / BM;
+    ntn = (n16 + 255) / 256;
+    bn = ((n16 + ntn - 1) / ntn + 15) / 16 * 16;
+    if (bn > 256) bn = 256;
+    ntn = (n16 + bn - 1) / bn;
 }
 
 SysView sys_view(const nolsm_ctx* c) {
@@ -291,152 +197,98 @@ SysView sys_view(const nolsm_ctx* c) {
     return v;
 }
 
+size_t gather_smem(int max_nset, int cap) { return (size_t)max_nset * 8 + (size_t)(max_nset + 1) * 4 + (size_t)cap * 2 + 16; }
+
 template <typename T>
-int launch_gather(nolsm_ctx* c, const Batch& b, const MatInfo* d_mats, cudaStream_t s) {
-    const size_t smem = (size_t)b.max_nset * 8 + (size_t)(b.max_nset + 1) * 4 + (size_t)b.max_ld * 2 + 16;
-    dim3 grid(std::min(b.max_nset, 64), b.nmat, 2);
+int launch_gather(nolsm_ctx* c, const Engine& e, int max_nset, cudaStream_t s) {
+    const size_t smem = gather_smem(max_nset, e.cap);
+    dim3 grid(std::min(max_nset, 48), e.S, 2);
     if (c->val_dtype == NOLSM_DTYPE_F64) {
         auto k = k_gather<double, T>;
-        CU_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 48 * 1024)));
-        LAUNCH(c, K_GATHER, s, k<<<grid, 256, smem, s>>>(sys_view(c), d_mats, (const double*)c->dS, (const double*)c->dH, (T*)c->ws, b.max_nset, b.max_ld, c->prof_on ? c->d_gather_elems : nullptr));
+        LAUNCH(c, K_GATHER, s, k<<<grid, 256, smem, s>>>(e, sys_view(c), (const double*)c->dS, (const double*)c->dH, (T*)c->ws, max_nset));
     } else {
         auto k = k_gather<float, T>;
-        CU_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 48 * 1024)));
-        LAUNCH(c, K_GATHER, s, k<<<grid, 256, smem, s>>>(sys_view(c), d_mats, (const float*)c->dS, (const float*)c->dH, (T*)c->ws, b.max_nset, b.max_ld, c->prof_on ? c->d_gather_elems : nullptr));
+        LAUNCH(c, K_GATHER, s, k<<<grid, 256, smem, s>>>(e, sys_view(c), (const float*)c->dS, (const float*)c->dH, (T*)c->ws, max_nset));
     }
-    CU_TRY(c, cudaGetLastError());
     return NOLSM_OK;
 }
 
 template <typename T>
-int launch_gemm(nolsm_ctx* c, const Batch& b, GemmOp op, const CUtensorMap* d_maps, cudaStream_t s) {
+void launch_gemm(nolsm_ctx* c, const Engine& e, int launch, cudaStream_t s) {
     if (use_umma(c)) {
         UmmaArgs a;
-        a.op = op;
-        a.maps = d_maps;
-        a.base = (__half*)c->ws;
-        LAUNCH(c, K_GEMM, s, gemm_umma_kernel<<<std::min(c->sms, b.ntiles), UMMA_THREADS, UMMA_SMEM_BYTES, s>>>(a));
+        a.e = e; a.maps = c->d_maps; a.base = (__half*)c->ws; a.launch = launch;
+        LAUNCH(c, K_GEMM, s, gemm_umma_kernel<<<c->sms, UMMA_THREADS, UMMA_SMEM_BYTES, s>>>(a));
     } else {
-        LAUNCH(c, K_GEMM, s, k_gemm_simt<T><<<dim3(b.max_tiles64, b.nmat), 256, 0, s>>>(op, (T*)c->ws));
+        const int t64 = (e.cap + 63) / 64;
+        LAUNCH(c, K_GEMM, s, k_gemm_simt<T><<<dim3(t64 * t64, e.S), 256, 0, s>>>(e, (T*)c->ws, launch));
     }
-    CU_TRY(c, cudaGetLastError());
-    return NOLSM_OK;
 }
 
-int count_active(nolsm_ctx* c, int nmat, int phase, cudaStream_t s, int* out) {
-    LAUNCH(c, K_OTHER, s, k_count_active<<<1, 256, 0, s>>>(c->st, nmat, phase, c->d_flag));
-    CU_TRY(c, cudaMemcpyAsync(c->h_flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, s));
-    CU_TRY(c, cudaStreamSynchronize(s));
-    *out = *c->h_flag;
-    return NOLSM_OK;
-}
-
-template <typename T>
-int power_iterations(nolsm_ctx* c, const Batch& b, const MatInfo* d_mats, int buf, int iters, int which, cudaStream_t s) {
-    const int nm = b.nmat;
-    CU_TRY(c, cudaMemsetAsync(c->d_nrm, 0, sizeof(float) * (size_t)(iters + 1) * c->max_batch, s));
-    LAUNCH(c, K_OTHER, s, k_vec_init<<<dim3((b.max_n + 255) / 256, nm), 256, 0, s>>>(d_mats, c->d_vec, c->d_nrm, c->ldx));
-    float* x = c->d_vec;
-    float* y = c->d_vec + (size_t)c->max_batch * c->ldx;
-    const int gx = std::max(1, std::min((b.max_n + 7) / 8, (4 * c->sms + nm - 1) / nm));
-    for (int it = 0; it < iters; ++it) {
-        LAUNCH(c, K_OTHER, s, k_matvec<T><<<dim3(gx, nm), 256, 0, s>>>(d_mats, (const T*)c->ws, buf, x, c->d_nrm + (size_t)it * c->max_batch, y,
-                                                                      c->d_nrm + (size_t)(it + 1) * c->max_batch, c->ldx));
-        std::swap(x, y);
-    }
-    LAUNCH(c, K_OTHER, s, k_rho_finish<<<(nm + 127) / 128, 128, 0, s>>>(c->st, c->d_nrm + (size_t)iters * c->max_batch, nm, which, 1.05f));
-    CU_TRY(c, cudaGetLastError());
-    return NOLSM_OK;
-}
+size_t dcols_smem(const nolsm_ctx* c) { return (size_t)(c->max_nset + 1) * 4 + (size_t)c->max_n * c->max_nbi * 4 + 16; }
 
 template <typename T, typename TD>
-int launch_dcols(nolsm_ctx* c, const Batch& b, const MatInfo* d_mats, TD* D, cudaStream_t s) {
-    const size_t smem = (size_t)(b.max_nset + 1) * 4 + (size_t)b.max_n * b.max_nbi * 4 + 16;
-    const int gx = std::max(1, std::min((b.max_n + 7) / 8, (3 * c->sms + b.nmat - 1) / b.nmat));
-    dim3 grid(gx, b.nmat);
+void launch_dcols(nolsm_ctx* c, const Engine& e, TD* D, cudaStream_t s) {
+    const size_t smem = dcols_smem(c);
+    const int gx = std::max(1, std::min((c->max_n + 7) / 8, 12));
+    dim3 grid(gx, e.S);
     if (c->val_dtype == NOLSM_DTYPE_F64) {
         auto k = k_dcols_scatter<T, double, TD>;
-        CU_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 48 * 1024)));
-        LAUNCH(c, K_DCOLS, s, k<<<grid, 256, smem, s>>>(sys_view(c), d_mats, c->st, (const T*)c->ws, (const double*)c->dH, D, c->d_e_atom, b.max_nset));
+        LAUNCH(c, K_DCOLS, s, k<<<grid, 256, smem, s>>>(e, sys_view(c), (const T*)c->ws, (const double*)c->dH, D, c->d_e_atom, c->max_nset));
     } else {
         auto k = k_dcols_scatter<T, float, TD>;
-        CU_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 48 * 1024)));
-        LAUNCH(c, K_DCOLS, s, k<<<grid, 256, smem, s>>>(sys_view(c), d_mats, c->st, (const T*)c->ws, (const float*)c->dH, D, c->d_e_atom, b.max_nset));
+        LAUNCH(c, K_DCOLS, s, k<<<grid, 256, smem, s>>>(e, sys_view(c), (const T*)c->ws, (const float*)c->dH, D, c->d_e_atom, c->max_nset));
     }
-    CU_TRY(c, cudaGetLastError());
+}
+
+// Raises the dynamic shared memory limits of the templated kernels once per assemble (must not happen
+// during stream capture).
+template <typename T>
+int set_smem_limits(nolsm_ctx* c) {
+    const int g = (int)std::max<size_t>(gather_smem(c->max_nset, c->eng.cap), 48 * 1024);
+    const int d = (int)std::max<size_t>(dcols_smem(c), 48 * 1024);
+    if (d > 227 * 1024) return fail(c, NOLSM_EINVAL, "n_i * nb(i) too large for the D-columns kernel");
+    CU_TRY(c, cudaFuncSetAttribute(k_gather<double, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, g));
+    CU_TRY(c, cudaFuncSetAttribute(k_gather<float, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, g));
+    CU_TRY(c, cudaFuncSetAttribute(k_dcols_scatter<T, double, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, d));
+    CU_TRY(c, cudaFuncSetAttribute(k_dcols_scatter<T, double, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, d));
+    CU_TRY(c, cudaFuncSetAttribute(k_dcols_scatter<T, float, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, d));
+    CU_TRY(c, cudaFuncSetAttribute(k_dcols_scatter<T, float, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, d));
     return NOLSM_OK;
 }
 
-// One batch through a1-a7.
+// One round (nolsm_device.cuh). forked == true: three concurrent branches (used under stream capture):
+//   s_main: round begin -> GEMM launch 0 -> GEMM launch 1 ;  s_x: gather + power iterations + first Schulz step ;
+//   s_f: D columns + scatter.  forked == false: the same kernels serially on s_main (profiled rounds).
 template <typename T>
-int run_batch(nolsm_ctx* c, const Batch& b, double mu, void* D, int d_dtype, cudaStream_t s) {
-    const MatInfo* d_mats = c->plan.d_mats + b.first;
-    const CUtensorMap* d_maps = c->plan.d_maps ? c->plan.d_maps + b.first * NBUF : nullptr;
-    const int nm = b.nmat;
+int enqueue_round(nolsm_ctx* c, const Engine& e, void* D, int d_dtype, bool forked) {
+    cudaStream_t sm = c->s_main, sx = forked ? c->s_x : c->s_main, sf = forked ? c->s_f : c->s_main;
+    LAUNCH(c, K_OTHER, sm, k_round_begin<<<1, MAX_SLOTS, 0, sm>>>(e));
+    if (forked) {
+        CU_TRY(c, cudaEventRecord(c->ev_fork, sm));
+        CU_TRY(c, cudaStreamWaitEvent(sx, c->ev_fork, 0));
+        CU_TRY(c, cudaStreamWaitEvent(sf, c->ev_fork, 0));
+    }
+    // branch s_f: a6 + a7 for the slots in phase FIN
+    if (d_dtype == NOLSM_DTYPE_F64) launch_dcols<T, double>(c, e, (double*)D, sf);
+    else launch_dcols<T, float>(c, e, (float*)D, sf);
+    // branch s_x: a1 for the slots in phase NEW, power iterations for NEW (S) and PA (A)
     int r;
-    LAUNCH(c, K_OTHER, s, k_state_init<<<(nm + 127) / 128, 128, 0, s>>>(c->st, nm));
-    if ((r = launch_gather<T>(c, b, d_mats, s))) return r;
-
-    GemmOp op{};
-    op.nmat = nm; op.ntiles = b.ntiles; op.mats = d_mats; op.st = c->st;
-    op.alpha = 1.f; op.alpha_arr = nullptr;
-
-    // ---- a2: S_sub^-1 by the Schulz iteration, Y0 = I / rho(S) ----
-    if ((r = power_iterations<T>(c, b, d_mats, 0, c->opt.power_iters_s, 0, s))) return r;
-    LAUNCH(c, K_OTHER, s, k_schulz_first<T><<<dim3(std::max(1, std::min(64, (b.max_n * b.max_ld + 2047) / 2048)), nm), 256, 0, s>>>(
-                              d_mats, c->st, (T*)c->ws, 0, 2));
-    int ran = 1;
-    for (int k = 1; k < c->opt.max_inv_iters; ++k) {
-        const int ycur = (k & 1) ? 2 : 3, ynext = 5 - ycur;
-        op.a_buf = 0; op.b_buf = ycur; op.c_buf = 4; op.sgn = -1.f; op.beta = 2.f; op.want_res = 1;
-        op.alpha = 1.f; op.alpha_arr = nullptr;
-        op.gate = GATE_INV_ACTIVE; op.finish = FIN_INV_G1; op.tol = c->opt.tol_inv; op.max_iters = c->opt.max_inv_iters;
-        if ((r = launch_gemm<T>(c, b, op, d_maps, s))) return r;
-        op.a_buf = ycur; op.b_buf = 4; op.c_buf = ynext; op.sgn = 1.f; op.beta = 0.f; op.want_res = 0;
-        op.finish = FIN_INV_G2;
-        if ((r = launch_gemm<T>(c, b, op, d_maps, s))) return r;
-        ran = k + 1;
-        if (k + 1 >= c->inv_check_from) {
-            int active;
-            if ((r = count_active(c, nm, 0, s, &active))) return r;
-            if (!active) break;
-        }
+    if ((r = launch_gather<T>(c, e, c->max_nset, sx))) return r;
+    const int P = std::max(e.p_s, e.p_a);
+    LAUNCH(c, K_OTHER, sx, k_vec_init<<<dim3((e.cap + 255) / 256, e.S), 256, 0, sx>>>(e, c->d_vec, c->d_nrm, P));
+    for (int it = 0; it < P; ++it)
+        LAUNCH(c, K_OTHER, sx, k_matvec<T><<<dim3(16, e.S), 256, 0, sx>>>(e, (const T*)c->ws, c->d_vec, c->d_nrm, it));
+    LAUNCH(c, K_OTHER, sx, k_power_finish<T><<<dim3(32, e.S), 256, 0, sx>>>(e, (T*)c->ws, c->d_nrm));
+    // main branch: the two grouped GEMM launches of the round
+    launch_gemm<T>(c, e, 0, sm);
+    launch_gemm<T>(c, e, 1, sm);
+    if (forked) {
+        CU_TRY(c, cudaEventRecord(c->ev_x, sx));
+        CU_TRY(c, cudaEventRecord(c->ev_f, sf));
+        CU_TRY(c, cudaStreamWaitEvent(sm, c->ev_x, 0));
+        CU_TRY(c, cudaStreamWaitEvent(sm, c->ev_f, 0));
     }
-    c->inv_check_from = std::max(2, ran - 1);
-
-    // ---- a3: A = S^-1 H - mu I (into buffer 0), rho(A) ----
-    op.a_buf = -1; op.b_buf = 1; op.c_buf = 0; op.sgn = 1.f; op.beta = (float)(-mu); op.want_res = 0;
-    op.alpha = 1.f; op.alpha_arr = nullptr; op.gate = GATE_INV_OK; op.finish = FIN_COUNT_ONLY;
-    if ((r = launch_gemm<T>(c, b, op, d_maps, s))) return r;
-    if ((r = power_iterations<T>(c, b, d_mats, 0, c->opt.power_iters_a, 1, s))) return r;
-
-    // ---- a4 + a5: Newton-Schulz sign iteration (Eq. 6) with fused residual ----
-    ran = 0;
-    for (int k = 0; k < c->opt.max_sign_iters; ++k) {
-        const int xcur = k & 1, xnext = 1 - xcur;
-        op.a_buf = xcur; op.b_buf = xcur; op.c_buf = 4; op.sgn = -1.f; op.beta = 3.f; op.want_res = 1;
-        op.alpha = 1.f; op.alpha_arr = k == 0 ? c->st.alpha1 : nullptr;
-        op.gate = GATE_SIGN_ACTIVE; op.finish = FIN_SIGN_G1; op.tol = c->opt.tol_sign; op.max_iters = c->opt.max_sign_iters;
-        if ((r = launch_gemm<T>(c, b, op, d_maps, s))) return r;
-        op.a_buf = xcur; op.b_buf = 4; op.c_buf = xnext; op.sgn = 1.f; op.beta = 0.f; op.want_res = 0;
-        op.alpha = 0.5f; op.alpha_arr = k == 0 ? c->st.alpha2 : nullptr;
-        op.finish = FIN_SIGN_G2;
-        if ((r = launch_gemm<T>(c, b, op, d_maps, s))) return r;
-        ran = k + 1;
-        if (k + 1 >= c->sign_check_from) {
-            int active;
-            if ((r = count_active(c, nm, 1, s, &active))) return r;
-            if (!active) break;
-        }
-    }
-    c->sign_check_from = std::max(2, ran - 1);
-
-    // ---- a6 + a7: D columns, scatter, energy partials ----
-    if (d_dtype == NOLSM_DTYPE_F64) r = launch_dcols<T, double>(c, b, d_mats, (double*)D, s);
-    else r = launch_dcols<T, float>(c, b, d_mats, (float*)D, s);
-    if (r) return r;
-    LAUNCH(c, K_OTHER, s, k_save_stats<<<(nm + 127) / 128, 128, 0, s>>>(d_mats, c->st, nm, c->a_inv, c->a_sign, c->a_status,
-                                                                        c->a_gemms, c->a_res, c->a_rho));
     CU_TRY(c, cudaGetLastError());
     return NOLSM_OK;
 }
@@ -478,7 +330,15 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
     cudaSetDevice(cuda_device);
     cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, cuda_device);
     if (getenv_int("NOLSM_PROFILE_EVERY", 0) > 0) o.profile_every = getenv_int("NOLSM_PROFILE_EVERY", 0);
-    c->tile_target = getenv_int("NOLSM_BATCH_TILES", 8 * c->sms);
+    if (getenv_int("NOLSM_SLOTS", 0) > 0) o.batch_atoms = getenv_int("NOLSM_SLOTS", 0);
+    c->use_graph = getenv_int("NOLSM_GRAPH", 1) != 0;
+    bool ok = cudaStreamCreateWithFlags(&c->s_main, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&c->s_x, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&c->s_f, cudaStreamNonBlocking) == cudaSuccess;
+    cudaEvent_t* evs[] = {&c->ev_fork, &c->ev_x, &c->ev_f, &c->ev_in, &c->ev_out};
+    for (cudaEvent_t* e : evs) ok = ok && cudaEventCreateWithFlags(e, cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; i < ROUND_DEPTH; ++i) ok = ok && cudaEventCreateWithFlags(&c->ev_round[i], cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) { cudaGetLastError(); delete c; return NOLSM_ECUDA; }
     if (use_umma(c)) {
         if (cudaFuncSetAttribute(gemm_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, UMMA_SMEM_BYTES) != cudaSuccess) {
             cudaGetLastError();
@@ -493,11 +353,14 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
 int nolsm_destroy(nolsm_ctx* c) {
     if (!c) return NOLSM_EINVAL;
     cudaSetDevice(c->dev);
-    if (c->plan.d_mats) cudaFree(c->plan.d_mats);
-    if (c->plan.d_maps) cudaFree(c->plan.d_maps);
-    c->plan.d_mats = nullptr; c->plan.d_maps = nullptr;
     free_assembled(c);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    cudaEvent_t evs[] = {c->ev_fork, c->ev_x, c->ev_f, c->ev_in, c->ev_out};
+    for (cudaEvent_t e : evs) if (e) cudaEventDestroy(e);
+    for (int i = 0; i < ROUND_DEPTH; ++i) if (c->ev_round[i]) cudaEventDestroy(c->ev_round[i]);
+    if (c->s_main) cudaStreamDestroy(c->s_main);
+    if (c->s_x) cudaStreamDestroy(c->s_x);
+    if (c->s_f) cudaStreamDestroy(c->s_f);
     delete c;
     return NOLSM_OK;
 }
@@ -512,8 +375,6 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     if (val_dtype != NOLSM_DTYPE_F64 && val_dtype != NOLSM_DTYPE_F32) return fail(c, NOLSM_EINVAL, "bad val_dtype");
     cudaStream_t s = (cudaStream_t)cuda_stream;
     cudaSetDevice(c->dev);
-    if (c->plan.d_mats) { cudaFree(c->plan.d_mats); c->plan.d_mats = nullptr; }
-    if (c->plan.d_maps) { cudaFree(c->plan.d_maps); c->plan.d_maps = nullptr; }
     free_assembled(c);
     int r;
     c->n_atoms = n_atoms;
@@ -621,9 +482,20 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
             c->dim[i] = off;
         }
     });
-    int max_n = 0;
-    for (int64_t i = 0; i < n_atoms; ++i) max_n = std::max(max_n, c->dim[i]);
+    int max_n = 0, min_n = 1 << 30, max_nset = 0, max_nbi = 0;
+    double mean_tiles = 0;
+    for (int64_t i = 0; i < n_atoms; ++i) {
+        max_n = std::max(max_n, c->dim[i]);
+        min_n = std::min(min_n, c->dim[i]);
+        max_nset = std::max<int>(max_nset, (int)(c->nset_ptr[i + 1] - c->nset_ptr[i]));
+        max_nbi = std::max(max_nbi, c->atom_nb[i]);
+        int ntm, ntn, bn;
+        host_tiling((c->dim[i] + 15) & ~15, ntm, ntn, bn);
+        mean_tiles += (double)ntm * ntn;
+    }
+    mean_tiles /= (double)n_atoms;
     if (max_n > 65535) return fail(c, NOLSM_EINVAL, "submatrix dimension > 65535 not supported");
+    c->max_n = max_n; c->max_nset = max_nset; c->max_nbi = max_nbi;
     if (!c->filtered) {
         c->d_nset_ptr = c->d_row_ptr;
         c->d_nset_atom = c->d_col_idx;
@@ -637,62 +509,84 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     c->d_nset_slot = (int*)tmp;
     if ((r = to_device(c, c->nset_off.data(), sizeof(int32_t) * nn, &tmp, s))) return r;
     c->d_nset_off = (int*)tmp;
+    if ((r = to_device(c, c->dim.data(), sizeof(int32_t) * n_atoms, &tmp, s))) return r;
+    c->d_dim = (int*)tmp;
+    if ((r = to_device(c, c->pos.data(), sizeof(int32_t) * n_atoms, &tmp, s))) return r;
+    c->d_pos = (int*)tmp;
 
-    // ---- workspace, batch capacity, state ----
+    // ---- engine: slots, workspace, tensor maps ----
+    Engine& e = c->eng;
+    e = Engine{};
     const size_t es = elem_size(c);
-    const long long max_ld = (max_n + 7) / 8 * 8;
-    const size_t one = (size_t)(((long long)max_n * max_ld + 63) / 64 * 64) * NBUF * es;
+    e.cap = (max_n + 15) & ~15;
+    e.ld = e.cap;
+    e.bufsz = (long long)e.cap * e.ld;
+    e.slotsz = e.bufsz * NBUF;
     size_t free_b = 0, total_b = 0;
     CU_TRY(c, cudaMemGetInfo(&free_b, &total_b));
-    // enough slots of the largest matrix to reach the tile target, within the caps
-    const int tiles_one = std::max(1, ((max_n + BM - 1) / BM) * ((max_n + 255) / 256));
-    size_t want = one * (size_t)std::max(2, (c->tile_target + tiles_one - 1) / tiles_one + 1) * 2;
-    size_t cap = c->opt.workspace_bytes ? c->opt.workspace_bytes : std::min<size_t>(free_b / 2, (size_t)32 << 30);
-    c->ws_bytes = std::max(one, std::min(want, cap));
+    const size_t slot_bytes = (size_t)e.slotsz * es;
+    const size_t cap_bytes = c->opt.workspace_bytes ? c->opt.workspace_bytes : std::min<size_t>(free_b / 2, (size_t)48 << 30);
+    // default: enough slots for ~16 waves of 128 x bn tiles per GEMM launch
+    int S = c->opt.batch_atoms > 0 ? c->opt.batch_atoms : (int)std::ceil(16.0 * c->sms / std::max(1.0, mean_tiles));
+    S = std::max(S, 2);
+    S = (int)std::min<size_t>(S, std::max<size_t>(2, cap_bytes / slot_bytes));
+    S = std::min(S, MAX_SLOTS);
+    S = (int)std::min<int64_t>(S, std::max<int64_t>(2, n_atoms));
+    e.S = S;
+    c->ws_bytes = slot_bytes * S;
     if ((r = dmalloc(c, &c->ws, c->ws_bytes))) return r;
-    c->max_batch = c->opt.batch_atoms > 0 ? c->opt.batch_atoms : 4096;
-    // smallest matrix bounds how many fit
-    int min_n = max_n;
-    for (int64_t i = 0; i < n_atoms; ++i) min_n = std::min(min_n, c->dim[i]);
-    const size_t smallest = (size_t)(((long long)min_n * ((min_n + 7) / 8 * 8) + 63) / 64 * 64) * NBUF * es;
-    c->max_batch = (int)std::min<size_t>(c->max_batch, std::max<size_t>(1, c->ws_bytes / smallest));
-    c->max_batch = (int)std::min<int64_t>(c->max_batch, n_atoms);
-    const int mb = c->max_batch;
-    {
-        const size_t nf = 7, ni = 11;
-        if ((r = dmalloc(c, &c->state_mem, (nf * 4 + ni * 4) * (size_t)mb))) return r;
-        float* f = (float*)c->state_mem;
-        int* ii = (int*)(f + nf * mb);
-        BatchState& st = c->st;
-        st.res_acc = f; st.res_prev = f + mb; st.res_last = f + 2 * mb; st.rho_s = f + 3 * mb; st.rho_a = f + 4 * mb;
-        st.alpha1 = f + 5 * mb; st.alpha2 = f + 6 * mb;
-        st.tiles_done = ii; st.inv_conv = ii + mb; st.inv_done = ii + 2 * mb; st.inv_iters = ii + 3 * mb; st.ybuf = ii + 4 * mb;
-        st.sign_conv = ii + 5 * mb; st.sign_done = ii + 6 * mb; st.sign_iters = ii + 7 * mb; st.xbuf = ii + 8 * mb;
-        st.status = ii + 9 * mb; st.gemm_count = ii + 10 * mb;
+    CU_TRY(c, cudaMemsetAsync(c->ws, 0, c->ws_bytes, s));
+    if ((r = dmalloc(c, (void**)&e.slots, sizeof(Slot) * S))) return r;
+    if ((r = dmalloc(c, (void**)&e.ops, sizeof(SlotOp) * 2 * S))) return r;
+    if ((r = dmalloc(c, (void**)&e.ntiles, 16))) return r;
+    if ((r = dmalloc(c, (void**)&e.next_atom, 16))) return r;
+    if ((r = dmalloc(c, (void**)&e.finished, 16))) return r;
+    if ((r = dmalloc(c, (void**)&e.prof, sizeof(double) * PF_LEN))) return r;
+    CU_TRY(c, cudaMemsetAsync(e.slots, 0, sizeof(Slot) * S, s));
+    CU_TRY(c, cudaMemsetAsync(e.ops, 0, sizeof(SlotOp) * 2 * S, s));
+    CU_TRY(c, cudaMemsetAsync(e.ntiles, 0, 16, s));
+    CU_TRY(c, cudaHostAlloc((void**)&c->h_done, 64, cudaHostAllocMapped));
+    *c->h_done = 0;
+    int* h_done_dev = nullptr;
+    CU_TRY(c, cudaHostGetDevicePointer((void**)&h_done_dev, c->h_done, 0));
+    e.h_done = h_done_dev;
+    e.tol_inv = c->opt.tol_inv; e.tol_sign = c->opt.tol_sign;
+    e.max_inv = c->opt.max_inv_iters; e.max_sign = c->opt.max_sign_iters;
+    e.p_s = c->opt.power_iters_s; e.p_a = c->opt.power_iters_a;
+    const int P = std::max(e.p_s, e.p_a);
+    if (P + 1 > 256) return fail(c, NOLSM_EINVAL, "too many power iterations");
+    if ((r = dmalloc(c, (void**)&c->d_vec, sizeof(float) * 2 * (size_t)S * e.ld))) return r;
+    if ((r = dmalloc(c, (void**)&c->d_nrm, sizeof(float) * (size_t)(P + 1) * S))) return r;
+    int** res_i[] = {&e.at.inv, &e.at.sign, &e.at.status, &e.at.gemms};
+    for (int** pp : res_i) {
+        if ((r = dmalloc(c, (void**)pp, 4 * n_atoms))) return r;
+        CU_TRY(c, cudaMemsetAsync(*pp, 0, 4 * n_atoms, s));
     }
-    c->ldx = (int)max_ld;
-    const int pit = std::max(c->opt.power_iters_s, c->opt.power_iters_a) + 1;
-    if ((r = dmalloc(c, (void**)&c->d_vec, sizeof(float) * 2 * (size_t)mb * c->ldx))) return r;
-    if ((r = dmalloc(c, (void**)&c->d_nrm, sizeof(float) * (size_t)pit * mb))) return r;
-    if ((r = dmalloc(c, (void**)&c->d_flag, 16))) return r;
-    if ((r = dmalloc(c, (void**)&c->d_gather_elems, 16))) return r;
-    CU_TRY(c, cudaMallocHost((void**)&c->h_flag, 16));
-    if ((r = dmalloc(c, (void**)&c->a_inv, 4 * n_atoms))) return r;
-    if ((r = dmalloc(c, (void**)&c->a_sign, 4 * n_atoms))) return r;
-    if ((r = dmalloc(c, (void**)&c->a_status, 4 * n_atoms))) return r;
-    if ((r = dmalloc(c, (void**)&c->a_gemms, 4 * n_atoms))) return r;
-    if ((r = dmalloc(c, (void**)&c->a_res, 4 * n_atoms))) return r;
-    if ((r = dmalloc(c, (void**)&c->a_rho, 4 * n_atoms))) return r;
+    float** res_f[] = {&e.at.res, &e.at.rho};
+    for (float** pp : res_f) {
+        if ((r = dmalloc(c, (void**)pp, 4 * n_atoms))) return r;
+        CU_TRY(c, cudaMemsetAsync(*pp, 0, 4 * n_atoms, s));
+    }
+    e.at.dim = c->d_dim; e.at.pos = c->d_pos; e.at.nb = c->d_atom_nb;
     if ((r = dmalloc(c, (void**)&c->d_e_atom, 8 * n_atoms))) return r;
-    CU_TRY(c, cudaMemsetAsync(c->a_inv, 0, 4 * n_atoms, s));
-    CU_TRY(c, cudaMemsetAsync(c->a_sign, 0, 4 * n_atoms, s));
-    CU_TRY(c, cudaMemsetAsync(c->a_status, 0, 4 * n_atoms, s));
-    CU_TRY(c, cudaMemsetAsync(c->a_gemms, 0, 4 * n_atoms, s));
-    CU_TRY(c, cudaMemsetAsync(c->a_res, 0, 4 * n_atoms, s));
     CU_TRY(c, cudaMemsetAsync(c->d_e_atom, 0, 8 * n_atoms, s));
-    c->assembled = true;   // build_plan needs the workspace pointer
-    if ((r = build_plan(c, 0, n_atoms, s))) { c->assembled = false; return r; }
+    if (use_umma(c)) {
+        if (!encode_tiled_fn()) return fail(c, NOLSM_ECUDA, "cuTensorMapEncodeTiled not available");
+        std::vector<CUtensorMap> maps((size_t)S * NBUF);
+        for (int sl = 0; sl < S; ++sl)
+            for (int b = 0; b < NBUF; ++b) {
+                const __half* base = (const __half*)c->ws + (long long)sl * e.slotsz + (long long)b * e.bufsz;
+                if (!make_tmap_f16_64x64(&maps[(size_t)sl * NBUF + b], base, e.cap, e.ld))
+                    return fail(c, NOLSM_ECUDA, "cuTensorMapEncodeTiled failed");
+            }
+        if ((r = dmalloc(c, (void**)&c->d_maps, maps.size() * sizeof(CUtensorMap)))) return r;
+        CU_TRY(c, cudaMemcpyAsync(c->d_maps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, s));
+        CU_TRY(c, cudaStreamSynchronize(s));      // `maps` is a local
+    }
+    r = c->opt.precision == NOLSM_PREC_FP32 ? set_smem_limits<float>(c) : set_smem_limits<__half>(c);
+    if (r) return r;
     CU_TRY(c, cudaStreamSynchronize(s));
+    c->assembled = true;
     return NOLSM_OK;
 }
 
@@ -702,10 +596,10 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "nolsm_assemble has not been called");
     if (!D_vals || a0 < 0 || a1 > c->n_atoms || a0 >= a1) return fail(c, NOLSM_EINVAL, "bad range or null D_vals");
     if (d_dtype != NOLSM_DTYPE_F64 && d_dtype != NOLSM_DTYPE_F32) return fail(c, NOLSM_EINVAL, "bad d_dtype");
-    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaStream_t us = (cudaStream_t)cuda_stream;
+    cudaStream_t s = c->s_main;
     cudaSetDevice(c->dev);
     int r;
-    if ((r = build_plan(c, a0, a1, s))) return r;
     const size_t ds = d_dtype == NOLSM_DTYPE_F64 ? 8 : 4;
     c->last_ds = ds;
     const int64_t v0 = c->blk_off[c->row_ptr[a0]], v1 = c->blk_off[c->row_ptr[a1]];
@@ -724,30 +618,73 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
     } else {
         D_dev = (char*)D_vals;
     }
+    // the engine runs on the library's own streams (the caller's stream may be the legacy default
+    // stream, which cannot be captured); order them after the caller's stream
+    CU_TRY(c, cudaEventRecord(c->ev_in, us));
+    CU_TRY(c, cudaStreamWaitEvent(s, c->ev_in, 0));
     CU_TRY(c, cudaMemsetAsync(D_dev + (size_t)v0 * ds, 0, (size_t)(v1 - v0) * ds, s));
     CU_TRY(c, cudaMemsetAsync(c->d_e_atom + a0, 0, 8 * (a1 - a0), s));
-    c->gather_bytes = 0; c->scatter_bytes = 0;
-    c->ev_used = 0; c->recs.clear(); c->prof_ranges.clear(); c->launches = 0;
-    CU_TRY(c, cudaMemsetAsync(c->d_gather_elems, 0, 8, s));
-    int64_t bi = 0;
-    for (const Batch& b : c->plan.batches) {
-        c->prof_on = c->opt.profile_every > 0 && (bi++ % c->opt.profile_every) == 0;
-        if (c->prof_on) c->prof_ranges.push_back({a0 + b.first, a0 + b.first + b.nmat});
-        r = c->opt.precision == NOLSM_PREC_FP32 ? run_batch<float>(c, b, mu, D_dev, d_dtype, s)
-                                                : run_batch<__half>(c, b, mu, D_dev, d_dtype, s);
-        c->prof_on = false;
-        if (r) return r;
+    Engine e = c->eng;
+    e.mu = (float)mu;
+    e.a_end = (int)a1;
+    e.profiling = 0;
+    const int a0i = (int)a0;
+    CU_TRY(c, cudaMemsetAsync(e.slots, 0, sizeof(Slot) * e.S, s));
+    CU_TRY(c, cudaMemcpyAsync(e.next_atom, &a0i, 4, cudaMemcpyHostToDevice, s));
+    CU_TRY(c, cudaMemsetAsync(e.finished, 0, 4, s));
+    CU_TRY(c, cudaMemsetAsync(e.prof, 0, sizeof(double) * PF_LEN, s));
+    CU_TRY(c, cudaStreamSynchronize(s));       // a0i is a local; also makes *h_done = 0 below race-free
+    *c->h_done = 0;
+    c->ev_used = 0; c->recs.clear(); c->launches = 0; c->prof_on = false;
+    const bool fp32 = c->opt.precision == NOLSM_PREC_FP32;
+
+    // ---- one round captured as a CUDA graph ----
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    int64_t launches_per_round = 0;
+    if (c->use_graph) {
+        cudaGraph_t g = nullptr;
+        CU_TRY(c, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
+        r = fp32 ? enqueue_round<float>(c, e, D_dev, d_dtype, true) : enqueue_round<__half>(c, e, D_dev, d_dtype, true);
+        cudaError_t ce = cudaStreamEndCapture(s, &g);
+        if (r) { if (g) cudaGraphDestroy(g); return r; }
+        if (ce != cudaSuccess) { c->err = std::string("stream capture: ") + cudaGetErrorString(ce); return NOLSM_ECUDA; }
+        ce = cudaGraphInstantiate(&c->graph_exec, g, 0);
+        cudaGraphDestroy(g);
+        if (ce != cudaSuccess) { c->err = std::string("graph instantiate: ") + cudaGetErrorString(ce); return NOLSM_ECUDA; }
+        launches_per_round = c->launches;
+        c->launches = 0;
     }
-    const size_t es = elem_size(c);
-    const size_t vs = c->val_dtype == NOLSM_DTYPE_F64 ? 8 : 4;
-    for (int64_t a = a0; a < a1; ++a) {
-        const double n = c->dim[a], ld = (c->dim[a] + 7) / 8 * 8;
-        const double nv = (double)(c->blk_off[c->row_ptr[a + 1]] - c->blk_off[c->row_ptr[a]]);
-        c->gather_bytes += 2.0 * n * ld * es;                    // dense S_sub and H_sub written
-        c->scatter_bytes += nv * (ds + vs) + 2.0 * n * ld * es;  // D row written, H0 row read, X and Y columns read
+
+    // ---- replay rounds until the device reports every atom finished ----
+    const int64_t total = a1 - a0;
+    const int64_t max_rounds = ((total + e.S - 1) / e.S + 2) * (int64_t)(e.max_inv + e.max_sign + 8);
+    int64_t round = 0, graph_rounds = 0;
+    for (;; ++round) {
+        if (round >= ROUND_DEPTH) {
+            CU_TRY(c, cudaEventSynchronize(c->ev_round[round % ROUND_DEPTH]));
+            if (*(volatile int*)c->h_done >= total) break;
+        }
+        if (round > max_rounds) return fail(c, NOLSM_ECUDA, "engine did not terminate");
+        const bool prof = c->opt.profile_every > 0 && (round % c->opt.profile_every) == c->opt.profile_every / 2;
+        if (prof || !c->use_graph) {
+            Engine ep = e;
+            ep.profiling = prof ? 1 : 0;
+            c->prof_on = prof;
+            r = fp32 ? enqueue_round<float>(c, ep, D_dev, d_dtype, false) : enqueue_round<__half>(c, ep, D_dev, d_dtype, false);
+            c->prof_on = false;
+            if (r) return r;
+        } else {
+            CU_TRY(c, cudaGraphLaunch(c->graph_exec, s));
+            ++graph_rounds;
+        }
+        CU_TRY(c, cudaEventRecord(c->ev_round[round % ROUND_DEPTH], s));
     }
+    c->launches += graph_rounds * launches_per_round;
+    c->rounds = round;
     if (host_out) CU_TRY(c, cudaMemcpyAsync((char*)D_vals + (size_t)v0 * ds, c->d_D_stage, (size_t)(v1 - v0) * ds, cudaMemcpyDeviceToHost, s));
-    c->last_stream = s; c->last_a0 = a0; c->last_a1 = a1; c->have_result = true;
+    CU_TRY(c, cudaEventRecord(c->ev_out, s));
+    CU_TRY(c, cudaStreamWaitEvent(us, c->ev_out, 0));
+    c->last_stream = us; c->last_a0 = a0; c->last_a1 = a1; c->have_result = true;
     if (e_partial_host) return nolsm_energy(c, e_partial_host);
     return NOLSM_OK;
 }
@@ -766,7 +703,7 @@ int nolsm_energy(nolsm_ctx* c, double* e_elec) {
     std::vector<double> e(n);
     std::vector<int> st(n);
     CU_TRY(c, cudaMemcpy(e.data(), c->d_e_atom + c->last_a0, 8 * n, cudaMemcpyDeviceToHost));
-    CU_TRY(c, cudaMemcpy(st.data(), c->a_status + c->last_a0, 4 * n, cudaMemcpyDeviceToHost));
+    CU_TRY(c, cudaMemcpy(st.data(), c->eng.at.status + c->last_a0, 4 * n, cudaMemcpyDeviceToHost));
     double sum = 0;
     int bits = 0;
     for (int64_t i = 0; i < n; ++i) { sum += e[i]; bits |= st[i]; }
@@ -795,22 +732,32 @@ int nolsm_gather_submatrix(nolsm_ctx* c, int64_t atom, int which, int out_fp16, 
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "not assembled");
     if (atom < 0 || atom >= c->n_atoms) return fail(c, NOLSM_EINVAL, "atom out of range");
     cudaSetDevice(c->dev);
-    MatInfo mi;
-    fill_matinfo(c, atom, mi);
-    Batch b{};
-    b.first = 0; b.nmat = 1; b.max_n = mi.n; b.max_ld = mi.ld; b.max_nbi = mi.nbi;
-    b.max_nset = (int)(c->nset_ptr[atom + 1] - c->nset_ptr[atom]);
-    MatInfo* d_mi;
-    CU_TRY(c, cudaMalloc((void**)&d_mi, sizeof(MatInfo)));
-    CU_TRY(c, cudaMemcpy(d_mi, &mi, sizeof(MatInfo), cudaMemcpyHostToDevice));
-    int r = out_fp16 ? launch_gather<__half>(c, b, d_mi, nullptr) : launch_gather<float>(c, b, d_mi, nullptr);
     const size_t es = out_fp16 ? 2 : 4;
+    if ((size_t)c->eng.slotsz * es > c->ws_bytes) return fail(c, NOLSM_ENOMEM, "workspace too small for an FP32 gather");
+    // a one-slot view of the engine with the slot forced into phase NEW
+    Engine e = c->eng;
+    e.S = 1;
+    e.profiling = 0;
+    Slot sl{};
+    sl.atom = (int)atom; sl.n = c->dim[atom]; sl.n16 = (sl.n + 15) & ~15; sl.pos = c->pos[atom]; sl.nbi = c->atom_nb[atom];
+    sl.phase = sl.snap = PH_NEW;
+    Slot* d_sl;
+    CU_TRY(c, cudaMalloc((void**)&d_sl, sizeof(Slot)));
+    CU_TRY(c, cudaMemcpy(d_sl, &sl, sizeof(Slot), cudaMemcpyHostToDevice));
+    e.slots = d_sl;
+    int r;
+    const int dflt_prec = c->opt.precision;
+    if (out_fp16) { r = set_smem_limits<__half>(c); if (!r) r = launch_gather<__half>(c, e, c->max_nset, c->s_main); }
+    else { r = set_smem_limits<float>(c); if (!r) r = launch_gather<float>(c, e, c->max_nset, c->s_main); }
+    (void)dflt_prec;
     if (!r) {
-        cudaError_t e = cudaMemcpy2D(out_host, (size_t)mi.n * es, (const char*)c->ws + (size_t)which * mi.bufsz * es,
-                                     (size_t)mi.ld * es, (size_t)mi.n * es, mi.n, cudaMemcpyDeviceToHost);
-        if (e != cudaSuccess) { c->err = cudaGetErrorString(e); r = NOLSM_ECUDA; }
+        cudaError_t ce = cudaStreamSynchronize(c->s_main);
+        if (ce == cudaSuccess)
+            ce = cudaMemcpy2D(out_host, (size_t)sl.n * es, (const char*)c->ws + (size_t)which * e.bufsz * es,
+                              (size_t)e.ld * es, (size_t)sl.n * es, sl.n, cudaMemcpyDeviceToHost);
+        if (ce != cudaSuccess) { c->err = cudaGetErrorString(ce); r = NOLSM_ECUDA; }
     }
-    cudaFree(d_mi);
+    cudaFree(d_sl);
     return r;
 }
 
@@ -822,11 +769,11 @@ int nolsm_get_atom_stats(nolsm_ctx* c, int64_t a0, int64_t count, int32_t* dims,
     cudaSetDevice(c->dev);
     if (c->have_result) CU_TRY(c, cudaStreamSynchronize(c->last_stream));
     if (dims) memcpy(dims, c->dim.data() + a0, 4 * count);
-    if (inv_iters) CU_TRY(c, cudaMemcpy(inv_iters, c->a_inv + a0, 4 * count, cudaMemcpyDeviceToHost));
-    if (sign_iters) CU_TRY(c, cudaMemcpy(sign_iters, c->a_sign + a0, 4 * count, cudaMemcpyDeviceToHost));
-    if (status) CU_TRY(c, cudaMemcpy(status, c->a_status + a0, 4 * count, cudaMemcpyDeviceToHost));
-    if (gemms) CU_TRY(c, cudaMemcpy(gemms, c->a_gemms + a0, 4 * count, cudaMemcpyDeviceToHost));
-    if (residual) CU_TRY(c, cudaMemcpy(residual, c->a_res + a0, 4 * count, cudaMemcpyDeviceToHost));
+    if (inv_iters) CU_TRY(c, cudaMemcpy(inv_iters, c->eng.at.inv + a0, 4 * count, cudaMemcpyDeviceToHost));
+    if (sign_iters) CU_TRY(c, cudaMemcpy(sign_iters, c->eng.at.sign + a0, 4 * count, cudaMemcpyDeviceToHost));
+    if (status) CU_TRY(c, cudaMemcpy(status, c->eng.at.status + a0, 4 * count, cudaMemcpyDeviceToHost));
+    if (gemms) CU_TRY(c, cudaMemcpy(gemms, c->eng.at.gemms + a0, 4 * count, cudaMemcpyDeviceToHost));
+    if (residual) CU_TRY(c, cudaMemcpy(residual, c->eng.at.res + a0, 4 * count, cudaMemcpyDeviceToHost));
     if (e_atom) CU_TRY(c, cudaMemcpy(e_atom, c->d_e_atom + a0, 8 * count, cudaMemcpyDeviceToHost));
     return NOLSM_OK;
 }
@@ -837,7 +784,7 @@ int nolsm_get_stats(nolsm_ctx* c, nolsm_stats* out) {
     memset(out, 0, sizeof(*out));
     const int64_t n = c->n_atoms;
     out->n_atoms = n;
-    out->n_batches = (int64_t)c->plan.batches.size();
+    out->n_batches = c->rounds;
     out->dim_min = 1 << 30;
     double dsum = 0;
     for (int64_t i = 0; i < n; ++i) {
@@ -854,15 +801,20 @@ int nolsm_get_stats(nolsm_ctx* c, nolsm_stats* out) {
             out->sum_inv_iters += inv[i]; out->sum_sign_iters += sg[i]; out->gemms_executed += gm[i];
             const double d = c->dim[i];
             out->flops_useful += 2.0 * d * d * d * gm[i];
-            MatInfo mi;
-            fill_matinfo(c, i, mi);
-            const double pm = (double)((mi.n + BM - 1) / BM) * BM, pn = (double)mi.ntn * mi.bn, pk = (double)((mi.n + 15) / 16) * 16;
-            out->flops_padded += 2.0 * pm * pn * pk * gm[i];
+            int ntm, ntn, bn;
+            const int n16 = (c->dim[i] + 15) & ~15;
+            host_tiling(n16, ntm, ntn, bn);
+            out->flops_padded += 2.0 * (double)(ntm * BM) * (double)(ntn * bn) * (double)n16 * gm[i];
             out->n_notspd += (st[i] & ST_NOTSPD) ? 1 : 0;
             out->n_noconv += (st[i] & ST_NOCONV) ? 1 : 0;
         }
-        out->gather_bytes = c->gather_bytes;
-        out->scatter_bytes = c->scatter_bytes;
+        const size_t es = elem_size(c), vs = c->val_dtype == NOLSM_DTYPE_F64 ? 8 : 4;
+        for (int64_t i = c->last_a0; i < c->last_a1; ++i) {
+            const double n16 = (c->dim[i] + 15) & ~15, n = c->dim[i];
+            const double nv = (double)(c->blk_off[c->row_ptr[i + 1]] - c->blk_off[c->row_ptr[i]]);
+            out->gather_bytes += 2.0 * n16 * n16 * es;                       // dense S_sub and H_sub written
+            out->scatter_bytes += nv * (c->last_ds + vs) + (n * n + n * c->atom_nb[i]) * es;
+        }
     }
     return NOLSM_OK;
 }
@@ -878,32 +830,14 @@ int nolsm_get_profile(nolsm_ctx* c, double* out, int n) {
         if (cudaEventElapsedTime(&t, c->ev_pool[r.ev], c->ev_pool[r.ev + 1]) != cudaSuccess) { cudaGetLastError(); continue; }
         ms[r.kind] += t; cnt[r.kind] += 1;
     }
-    double fl_useful = 0, fl_padded = 0, gbytes_w = 0, sbytes = 0, natoms = 0;
+    double pf[PF_LEN];
+    CU_TRY(c, cudaMemcpy(pf, c->eng.prof, sizeof(pf), cudaMemcpyDeviceToHost));
     const size_t es = elem_size(c), vs = c->val_dtype == NOLSM_DTYPE_F64 ? 8 : 4;
-    for (auto& pr : c->prof_ranges) {
-        const int64_t cntA = pr.second - pr.first;
-        std::vector<int32_t> gm(cntA);
-        CU_TRY(c, cudaMemcpy(gm.data(), c->a_gemms + pr.first, 4 * cntA, cudaMemcpyDeviceToHost));
-        for (int64_t a = pr.first; a < pr.second; ++a) {
-            MatInfo mi;
-            fill_matinfo(c, a, mi);
-            const double d = mi.n;
-            fl_useful += 2.0 * d * d * d * gm[a - pr.first];
-            const double pm = (double)((mi.n + BM - 1) / BM) * BM, pn = (double)mi.ntn * mi.bn, pk = (double)((mi.n + 15) / 16) * 16;
-            fl_padded += 2.0 * pm * pn * pk * gm[a - pr.first];
-            gbytes_w += 2.0 * d * mi.ld * es;
-            const double nv = (double)(c->blk_off[c->row_ptr[a + 1]] - c->blk_off[c->row_ptr[a]]);
-            sbytes += nv * (c->last_ds + vs) + d * mi.ld * es + d * mi.nbi * es;
-            natoms += 1;
-        }
-    }
-    unsigned long long ge = 0;
-    CU_TRY(c, cudaMemcpy(&ge, c->d_gather_elems, 8, cudaMemcpyDeviceToHost));
-    out[0] = ms[K_GATHER]; out[1] = cnt[K_GATHER]; out[2] = gbytes_w + (double)ge * vs;
-    out[3] = ms[K_GEMM]; out[4] = cnt[K_GEMM]; out[5] = fl_useful; out[6] = fl_padded;
-    out[7] = ms[K_DCOLS]; out[8] = cnt[K_DCOLS]; out[9] = sbytes;
+    out[0] = ms[K_GATHER]; out[1] = cnt[K_GATHER]; out[2] = pf[PF_GATHER_SRC] * vs + pf[PF_GATHER_DENSE] * es;
+    out[3] = ms[K_GEMM]; out[4] = cnt[K_GEMM]; out[5] = pf[PF_FLOP_USEFUL]; out[6] = pf[PF_FLOP_PADDED];
+    out[7] = ms[K_DCOLS]; out[8] = cnt[K_DCOLS]; out[9] = pf[PF_DCOLS_BYTES];
     out[10] = ms[K_OTHER]; out[11] = cnt[K_OTHER];
-    out[12] = natoms; out[13] = (double)c->launches;
+    out[12] = pf[PF_SUBMATS]; out[13] = (double)c->launches;
     return NOLSM_OK;
 }
 

@@ -1,10 +1,24 @@
-// Device-side data structures shared by the NOLSM kernels (gather, grouped GEMM chain, D columns).
+// Device-side data structures of the NOLSM engine.
 //
-// One "batch" is a set of atom submatrices T_i(H0), T_i(S) that live in the
-// workspace at the same time; every matrix of the batch owns one fixed-size workspace slot holding
-// NBUF square buffers. All matrix iterations (Schulz inverse, ref [14] PAPER.md:L217; Newton-Schulz
-// sign, Eq. 6) are sequences of grouped GEMM launches over the batch; convergence is
-// decided on the device by the epilogue of the GEMM that forms the residual.
+// The workspace is a fixed set of SLOTS; each slot holds NBUF square FP16 (or FP32) buffers of
+// capacity cap x ld and evaluates one atom submatrix T_i(H0), T_i(S) at a time.
+// A slot walks through the phases
+//     NEW   gather + rho(S) power iteration + closed-form first Schulz step
+//     INV   Schulz iterations  R = 2I - S Y,  Y <- Y R            (ref [14])
+//     AMAT  A = S^-1 H0 - mu I                                   (Eq. 5/8)
+//     PA    rho(A) power iteration (spectral scaling of X0)
+//     SIGN  Newton-Schulz  T = 3I - X^2,  X <- 1/2 X T           (Eq. 6)
+//     FIN   D columns of atom i, scatter, energy partial         (Eq. 4)
+// and is refilled with the next atom when it finishes (continuous batching). All slots advance
+// together in ROUNDS; a round is a fixed sequence of kernel launches (captured once as a CUDA graph)
+// whose kernels act on the slots that were in the matching phase when the round began. Phase
+// transitions, convergence tests and the refill are decided on the device; the host only replays the
+// graph until the device reports that every atom is done.
+//
+// Zero-pad invariant: every buffer that is used as a GEMM operand holds exact zeros in rows and
+// columns [n, n16) (n16 = n rounded up to 16). The TMA tensor maps describe the full slot capacity,
+// the GEMM k-loop stops at n16, and every writer (gather, first Schulz step, GEMM epilogues) writes
+// the zero strips, so nothing outside [0, n16)^2 is ever multiplied into a stored element.
 #pragma once
 #include <cuda.h>
 #include <cuda_fp16.h>
@@ -13,125 +27,115 @@
 
 namespace nolsm {
 
-constexpr int NBUF = 5;          // workspace buffers per matrix slot
+constexpr int NBUF = 5;          // B0 = S then X(even), B1 = H0 then X(odd), B2/B3 = Y ping-pong, B4 = R / T
 constexpr int BM = 128;          // GEMM tile rows
 constexpr int BK = 64;           // GEMM k-block (one 128-byte swizzle atom of fp16)
+constexpr int MAX_SLOTS = 1024;
 
-// status bits per submatrix (nolsm.h: NOLSM_MAT_*)
-constexpr int ST_NOTSPD = 1;     // Schulz inverse iteration did not converge / diverged
+constexpr int ST_NOTSPD = 1;     // Schulz inverse iteration diverged / did not converge
 constexpr int ST_NOCONV = 2;     // sign iteration hit max_sign_iters
 
-// Per-matrix geometry of the current batch (device array, written at assemble time).
-struct MatInfo {
-    int n;            // true dimension n_i
-    int ld;           // leading dimension (elements), multiple of 8
-    int pos;          // first column of atom i inside its own submatrix
-    int nbi;          // basis functions of atom i
-    int tile_start;   // first tile id of this matrix in the batch tile list
-    int ntn;          // tiles along N
-    int bn;           // tile width along N (multiple of 16, <= 256)
-    int atom;         // global atom id
-    long long off;    // element offset of buffer 0 of this matrix in the workspace
-    long long bufsz;  // elements per buffer (>= n * ld, multiple of 64)
+enum Phase { PH_FREE = 0, PH_NEW, PH_INV, PH_AMAT, PH_PA, PH_SIGN, PH_FIN };
+enum OpKind { OP_NONE = 0, OP_INV_G1, OP_INV_G2, OP_AMAT, OP_SIGN_G1, OP_SIGN_G2 };
+
+struct __align__(16) Slot {
+    // geometry of the atom in the slot (written at refill)
+    int atom, n, n16, pos, nbi, ntm, ntn, bn;
+    // phase machine
+    int phase;       // current phase (advanced by the kernels of the running round)
+    int snap;        // phase when the running round began; kernels gate on this
+    int inv_iters, sign_iters, conv, xcur, ycur, status, gemm_count, tiles_done;
+    float res_acc, res_prev, res_last, rho_s, rho_a, alpha1, alpha2, unused;
 };
 
-// Mutable per-matrix iteration state (device, SoA, indexed by slot in the batch).
-struct BatchState {
-    float* res_acc;      // running sum of squares accumulated by the residual epilogue
-    float* res_prev;     // residual of the previous iteration (||.||_F / sqrt(n))
-    float* res_last;     // last residual measured
-    float* rho_s;        // spectral-radius estimate of S_sub
-    float* rho_a;        // spectral-radius estimate of A_sub
-    float* alpha1;       // first sign iteration: 1 / rho_a^2
-    float* alpha2;       // first sign iteration: 0.5 / rho_a
-    int* tiles_done;     // tiles finished in the running launch
-    int* inv_conv;       // residual passed in G1 of this iteration
-    int* inv_done;       // inverse finished
-    int* inv_iters;
-    int* ybuf;           // buffer id holding S^-1 once inv_done
-    int* sign_conv;
-    int* sign_done;
-    int* sign_iters;
-    int* xbuf;           // buffer id holding sign(A) once sign_done
-    int* status;         // ST_* bits
-    int* gemm_count;     // executed square GEMMs (FLOP accounting)
-};
-
-enum FinishKind { FIN_NONE = 0, FIN_INV_G1, FIN_INV_G2, FIN_SIGN_G1, FIN_SIGN_G2, FIN_COUNT_ONLY };
-enum GateKind { GATE_NONE = 0, GATE_INV_ACTIVE, GATE_SIGN_ACTIVE, GATE_INV_OK };
-
-// One grouped GEMM launch: for every gated matrix m of the batch
-//   C_m = sgn * alpha_m * (A_m B_m) + beta * I,   optionally res_m += || alpha_m A_m B_m - I ||_F^2
-struct GemmOp {
-    int nmat;
-    int ntiles;
-    const MatInfo* mats;
-    BatchState st;
-    int a_buf, b_buf, c_buf;     // buffer ids; a_buf == -1 -> per-matrix st.ybuf[m]
-    float alpha;                 // scalar alpha, used when alpha_arr == nullptr
-    const float* alpha_arr;
-    float sgn;                   // +1 or -1
-    float beta;
+// What a slot does in GEMM launch L (0 or 1) of the running round:
+//   C = sgn * alpha * (A B) + beta * I,  optionally res += || alpha A B - I ||_F^2
+struct __align__(16) SlotOp {
+    int kind, a_buf, b_buf, c_buf;
+    float alpha, sgn, beta;
     int want_res;
-    int gate;                    // GateKind
-    int finish;                  // FinishKind
-    float tol;
-    int max_iters;
+    int tile_start, ntiles, pad0, pad1;
 };
 
-__device__ __forceinline__ bool gate_open(const GemmOp& op, int m) {
-    switch (op.gate) {
-        case GATE_INV_ACTIVE:  return op.st.inv_done[m] == 0;
-        case GATE_SIGN_ACTIVE: return op.st.sign_done[m] == 0 && (op.st.status[m] & ST_NOTSPD) == 0;
-        case GATE_INV_OK:      return (op.st.status[m] & ST_NOTSPD) == 0;
-        default:               return true;
-    }
+struct AtomArrays {               // per-atom inputs and results (device)
+    const int* dim;
+    const int* pos;
+    const int* nb;
+    int *inv, *sign, *status, *gemms;
+    float *res, *rho;
+};
+
+enum { PF_FLOP_USEFUL = 0, PF_FLOP_PADDED, PF_GATHER_SRC, PF_GATHER_DENSE, PF_DCOLS_BYTES, PF_SUBMATS, PF_LEN };
+
+struct Engine {
+    Slot* slots;
+    SlotOp* ops;                  // [2][S]
+    int* ntiles;                  // [2] tiles of GEMM launch 0 / 1 of the running round
+    int S, cap, ld;               // slots, slot capacity (rows), leading dimension (elements)
+    long long bufsz, slotsz;      // elements per buffer / per slot
+    float tol_inv, tol_sign, mu;
+    int max_inv, max_sign, p_s, p_a;
+    int* next_atom;               // atom feed [*next_atom, a_end)
+    int a_end;
+    int* finished;                // atoms finished so far
+    double* prof;                 // [PF_LEN] counters of the profiled rounds
+    int profiling;                // this round is a profiled (eager, per-launch timed) round
+    volatile int* h_done;         // host-mapped copy of *finished
+    AtomArrays at;
+};
+
+__device__ __forceinline__ long long buf_off(const Engine& e, int slot, int buf) {
+    return (long long)slot * e.slotsz + (long long)buf * e.bufsz;
 }
 
-// Tile id -> matrix index by binary search over MatInfo::tile_start.
-__device__ __forceinline__ int find_matrix(const MatInfo* mats, int nmat, int tile) {
-    int lo = 0, hi = nmat - 1;
+// Tile id -> slot by binary search over SlotOp::tile_start (a slot with ntiles == 0 shares its
+// tile_start with the next slot and is never returned for a valid tile).
+__device__ __forceinline__ int find_slot(const SlotOp* ops, int S, int tile) {
+    int lo = 0, hi = S - 1;
     while (lo < hi) {
-        int mid = (lo + hi + 1) >> 1;
-        if (mats[mid].tile_start <= tile) lo = mid; else hi = mid - 1;
+        const int mid = (lo + hi + 1) >> 1;
+        if (ops[mid].tile_start <= tile) lo = mid; else hi = mid - 1;
     }
     return lo;
 }
 
-// Called by exactly one thread once per finished tile, after the tile's stores and residual
-// atomics were issued and fenced. The thread that finishes the last tile of matrix m advances the
-// matrix's iteration state (convergence test of SURVEY C-7 / DESIGN.md "Convergence").
-__device__ __forceinline__ void tile_finished(const GemmOp& op, int m, int ntiles_m) {
-    if (op.finish == FIN_NONE) return;
+// Called by exactly one thread per finished tile, after the tile's stores and residual atomics. The
+// thread that finishes the last tile of the slot's GEMM advances the slot's iteration state
+// (DESIGN.md "Readings" C-7).
+__device__ __forceinline__ void tile_finished(const Engine& e, int slot, const SlotOp& op) {
+    Slot& s = e.slots[slot];
     __threadfence();
-    int prev = atomicAdd(&op.st.tiles_done[m], 1);
-    if (prev != ntiles_m - 1) return;
+    const int prev = atomicAdd(&s.tiles_done, 1);
+    if (prev != op.ntiles - 1) return;
     __threadfence();
-    op.st.tiles_done[m] = 0;
-    atomicAdd(&op.st.gemm_count[m], 1);
-    const BatchState& s = op.st;
-    const float n = (float)op.mats[m].n;
-    if (op.finish == FIN_INV_G1 || op.finish == FIN_SIGN_G1) {
-        float sum = atomicExch(&s.res_acc[m], 0.0f);
-        float r = sqrtf(sum / n);
-        float rp = s.res_prev[m];
-        s.res_prev[m] = r;
-        s.res_last[m] = r;
-        int* conv = (op.finish == FIN_INV_G1) ? s.inv_conv : s.sign_conv;
-        int iters = (op.finish == FIN_INV_G1) ? s.inv_iters[m] : s.sign_iters[m];
-        bool ok = r < op.tol;
-        bool stagnated = (r > 0.5f * rp) && (r < 4.f * op.tol) && iters > 0;   // rounding floor reached
-        bool diverged = !(r == r) || (iters > 1 && r > rp && r > 0.9f);
-        bool capped = iters + 1 >= op.max_iters;
-        if (diverged || (capped && !ok && !stagnated))
-            atomicOr(&s.status[m], op.finish == FIN_INV_G1 ? ST_NOTSPD : ST_NOCONV);
-        conv[m] = (ok || stagnated || diverged || capped) ? 1 : 0;
-    } else if (op.finish == FIN_INV_G2) {
-        s.inv_iters[m] += 1;
-        if (s.inv_conv[m]) { s.inv_done[m] = 1; s.ybuf[m] = op.c_buf; }
-    } else if (op.finish == FIN_SIGN_G2) {
-        s.sign_iters[m] += 1;
-        if (s.sign_conv[m]) { s.sign_done[m] = 1; s.xbuf[m] = op.c_buf; }
+    s.tiles_done = 0;
+    s.gemm_count += 1;
+    if (op.kind == OP_INV_G1 || op.kind == OP_SIGN_G1) {
+        const bool inv = op.kind == OP_INV_G1;
+        const float sum = atomicExch(&s.res_acc, 0.0f);
+        const float r = sqrtf(sum / (float)s.n);
+        const float rp = s.res_prev;
+        s.res_prev = r;
+        s.res_last = r;
+        const float tol = inv ? e.tol_inv : e.tol_sign;
+        const int iters = inv ? s.inv_iters : s.sign_iters;
+        const int cap = inv ? e.max_inv : e.max_sign;
+        const bool ok = r < tol;
+        const bool stagnated = (r > 0.5f * rp) && (r < 4.f * tol) && iters > 0;   // rounding floor reached
+        const bool diverged = !(r == r) || (iters > 1 && r > rp && r > 0.9f);
+        const bool capped = iters + 1 >= cap;
+        if (diverged || (capped && !ok && !stagnated)) s.status |= inv ? ST_NOTSPD : ST_NOCONV;
+        s.conv = (ok || stagnated || diverged || capped) ? 1 : 0;
+    } else if (op.kind == OP_INV_G2) {
+        s.inv_iters += 1;
+        s.ycur = 5 - s.ycur;
+        if (s.conv) { s.conv = 0; s.res_prev = 1e30f; s.phase = (s.status & ST_NOTSPD) ? PH_FIN : PH_AMAT; }
+    } else if (op.kind == OP_AMAT) {
+        s.phase = PH_PA;
+    } else if (op.kind == OP_SIGN_G2) {
+        s.sign_iters += 1;
+        s.xcur = 1 - s.xcur;
+        if (s.conv) { s.conv = 0; s.phase = PH_FIN; }
     }
 }
 

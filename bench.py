@@ -259,7 +259,7 @@ def main():
     if os.path.exists(tp):
         with open(tp) as f:
             traffic = json.load(f).get("dram_bytes_per_launch")
-    roofline = {"bound": "tensor", "kernel": "gemm_umma_kernel", "achieved": gemm_tf, "peak": peaks["bf16_tflops_sustained"],
+    roofline = {"bound": "tensor", "kernel": "gemm2_round_kernel", "achieved": gemm_tf, "peak": peaks["bf16_tflops_sustained"],
                 "unit": "TFLOP/s", "frac": gemm_tf / peaks["bf16_tflops_sustained"], "traffic": traffic,
                 "peak_source": peaks["source"] + " bf16_tflops_sustained (kernel timed inside a long step)",
                 "achieved_padded": gemm_tf_padded, "avg_launch_us": 1e3 * prof_acc["gemm_ms"] / max(prof_acc["gemm_launches"], 1),

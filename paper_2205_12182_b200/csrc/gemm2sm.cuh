@@ -1,0 +1,466 @@
+// Grouped, variable-size FP16 x FP16 -> FP32 GEMM for sm_100a on CTA PAIRS (tcgen05 cta_group::2).
+//
+// This is the GEMM "C = alpha A B + beta C" the paper counts as 2n^3 FLOP inside the
+// matrix iterations (Eq. 6; Schulz inverse, ref [14] PAPER.md:L217).
+//
+// Two CTAs of a cluster (one TPC) compute one 256 x bn tile (bn <= 256, multiple of 16): CTA r owns
+// rows [m0 + 128 r, m0 + 128 r + 128) of A and of the accumulator (its own TMEM) and stages columns
+// [n0 + r bn/2, n0 + (r+1) bn/2) of B; the leader CTA issues one tcgen05.mma (M = 256) per 16 k that
+// reads both CTAs' shared memory, so every byte of B is fetched from L2 once per pair instead of once
+// per CTA (L2 -> SM bytes per FLOP drop by a third against 128 x bn single-CTA tiles).
+//
+// All matrices are row-major: A is a K-major operand, B an MN-major operand (X * X needs no
+// transposed copy of X). TMA boxes are 64 x 64 FP16 with the 128-byte swizzle.
+//
+// Warp roles per CTA: warps 0-7 epilogue (TMEM lane quarter = warp & 3; the two warps of a quarter take
+// alternate 32-column chunks), warp 8 tile scheduler (leader CTA only), warp 9 TMA producer, warp 10
+// TMEM allocator + MMA issuer (leader only). The scheduler
+// publishes TileInfo records into a small shared-memory ring in BOTH CTAs; every other role consumes
+// them in order. Where the tiles come from is the caller's business (`next` functor): a static list in
+// the round engine, the device work queue in the persistent engine.
+#pragma once
+#include "gemm_umma.cuh"
+
+namespace nolsm {
+
+constexpr int G2_STAGES = 5;
+constexpr int G2_A_BYTES = 128 * BK * 2;              // 16 KB: this CTA's 128 rows x 64 k
+constexpr int G2_B_BYTES = 2 * B_BOX_BYTES;           // 16 KB: 64 k x (up to 128) columns
+constexpr int G2_STAGE_BYTES = G2_A_BYTES + G2_B_BYTES;
+constexpr int G2_NTI = 4;                             // tile-info ring depth
+constexpr int G2_EPI_WARPS = 8;                       // warp w: TMEM lane quarter w & 3, column chunks of parity w >> 2
+constexpr int G2_WARP_SCHED = 8, G2_WARP_TMA = 9, G2_WARP_MMA = 10;
+constexpr int G2_CTRL_THREADS = 11 * 32;              // warps 0..10
+// consumers of a TileInfo: leader = producer + MMA + epilogue warps, peer = producer + epilogue warps
+constexpr int G2_TI_CONSUMERS = 2 * (1 + G2_EPI_WARPS) + 1;
+
+struct __align__(16) TileInfo {      // 64 bytes
+    int valid;                        // 0 = no more tiles
+    int slot, m0, n0;                 // pair tile origin (rows m0 .. m0+255, columns n0 .. n0+bn-1)
+    int n, n16, bn, nreports;         // nreports = CTA reports that complete the slot's GEMM
+    int a_buf, b_buf, c_buf, want_res;
+    float alpha, sgn, beta;
+    int kind;
+};
+
+struct G2Smem {                       // byte offsets from the 1024-aligned base of the CTA's dynamic smem
+    uint32_t base;
+    __device__ uint32_t stage_a(int s) const { return base + s * G2_STAGE_BYTES; }
+    __device__ uint32_t stage_b(int s) const { return base + s * G2_STAGE_BYTES + G2_A_BYTES; }
+    __device__ uint32_t bars() const { return base + G2_STAGES * G2_STAGE_BYTES; }
+    __device__ uint32_t full(int s) const { return bars() + 8u * s; }
+    __device__ uint32_t empty(int s) const { return bars() + 8u * (G2_STAGES + s); }
+    __device__ uint32_t tfull(int a) const { return bars() + 8u * (2 * G2_STAGES + a); }
+    __device__ uint32_t tempty(int a) const { return bars() + 8u * (2 * G2_STAGES + 2 + a); }
+    __device__ uint32_t ti_full(int q) const { return bars() + 8u * (2 * G2_STAGES + 4 + q); }
+    __device__ uint32_t ti_empty(int q) const { return bars() + 8u * (2 * G2_STAGES + 4 + G2_NTI + q); }
+    __device__ uint32_t tmem_ptr() const { return bars() + 8u * (2 * G2_STAGES + 4 + 2 * G2_NTI); }
+    __device__ uint32_t tinfo(int q) const { return bars() + 256u + 64u * q; }
+};
+constexpr int G2_SMEM_BYTES = G2_STAGES * G2_STAGE_BYTES + 256 + 64 * G2_NTI + 1024 /*align*/;
+
+#ifdef G2_TIMING
+// probe builds only: cycles spent waiting, summed over CTAs
+__device__ unsigned long long g2_timing[8];
+#define G2_T0() const long long t0_ = clock64()
+#define G2_T1(i) tacc_[i] += clock64() - t0_
+#define G2_TDECL() long long tacc_[8] = {0, 0, 0, 0, 0, 0, 0, 0}
+#define G2_TFLUSH(lane0) do { if (lane0) for (int i_ = 0; i_ < 8; ++i_) if (tacc_[i_]) atomicAdd(&g2_timing[i_], (unsigned long long)tacc_[i_]); } while (0)
+#else
+#define G2_T0()
+#define G2_T1(i)
+#define G2_TDECL()
+#define G2_TFLUSH(lane0)
+#endif
+
+namespace ptx {
+
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t mapa(uint32_t saddr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+// Arrive without memory ordering, for barriers that only hand back a resource whose reads are already
+// complete: `dep` is a value loaded from that resource, listed as an operand so the load has retired.
+__device__ __forceinline__ void mbar_arrive_cluster_relaxed(uint32_t cluster_addr, uint32_t dep) {
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr), "r"(dep) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.b32 %0, 1, 0, p;\n\t}\n"
+        : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
+    uint32_t spins = 0;
+    while (!mbar_try_wait_cluster(bar, parity)) {
+        if (++spins > SPIN_LIMIT) __trap();
+    }
+}
+__device__ __forceinline__ void st_cluster_u32(uint32_t cluster_addr, uint32_t v) {
+    asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(cluster_addr), "r"(v) : "memory");
+}
+// TMA load whose completion bytes are credited to an mbarrier of either CTA of the pair.
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar_cluster) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes"
+        " [%0], [%1, {%2, %3}], [%4];"
+        ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar_cluster) : "memory");
+}
+__device__ __forceinline__ void tmem_alloc_pair(uint32_t smem_dst, uint32_t ncols) {
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc_pair(uint32_t taddr, uint32_t ncols) {
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void umma_f16_pair(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}\n"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// arrives (once the MMAs issued so far have completed) on the barrier at the same offset in both CTAs
+__device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
+    asm volatile(
+        "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+        ::"r"(bar), "h"((uint16_t)3) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
+}  // namespace ptx
+
+// ------------------------------------------------------------------------------------------------
+// One-time setup / teardown (all threads of both CTAs).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t g2_setup(const G2Smem& sm, int warp, int lane) {
+    if (warp == G2_WARP_TMA && lane == 0) {
+        for (int s = 0; s < G2_STAGES; ++s) { ptx::mbar_init(sm.full(s), 1); ptx::mbar_init(sm.empty(s), 1); }
+        for (int a = 0; a < 2; ++a) { ptx::mbar_init(sm.tfull(a), 1); ptx::mbar_init(sm.tempty(a), 2 * G2_EPI_WARPS); }
+        for (int q = 0; q < G2_NTI; ++q) { ptx::mbar_init(sm.ti_full(q), 1); ptx::mbar_init(sm.ti_empty(q), G2_TI_CONSUMERS); }
+        ptx::fence_mbar_init();
+    }
+    if (warp == G2_WARP_MMA) ptx::tmem_alloc_pair(sm.tmem_ptr(), 512);
+    ptx::tc_fence_before();
+    ptx::cluster_sync();
+    ptx::tc_fence_after();
+    uint32_t tmem_base;
+    asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(sm.tmem_ptr()));
+    return tmem_base;
+}
+__device__ __forceinline__ void g2_teardown(uint32_t tmem_base, int warp) {
+    ptx::tc_fence_before();
+    ptx::cluster_sync();
+    if (warp == G2_WARP_MMA) ptx::tmem_dealloc_pair(tmem_base, 512);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Scheduler (leader CTA, one warp): publishes TileInfo records to both CTAs until `next` says stop.
+// next(TileInfo&) fills the record and returns false when there is no more work.
+// ------------------------------------------------------------------------------------------------
+template <typename Next>
+__device__ __forceinline__ void g2_scheduler(const G2Smem& sm, int lane, Next next) {
+    int q = 0; uint32_t ph = 0;
+    for (;;) {
+        for (uint32_t spins = 0; !ptx::mbar_try_wait_cluster(sm.ti_empty(q), ph ^ 1);) {    // runs ahead: poll gently
+            __nanosleep(200);
+            if (++spins > SPIN_LIMIT) __trap();
+        }
+        TileInfo ti{};
+        if (lane == 0) ti.valid = next(ti) ? 1 : 0;
+        // lane i publishes word i of lane 0's record to both CTAs
+        const uint32_t* w = reinterpret_cast<const uint32_t*>(&ti);
+        uint32_t mine = 0;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const uint32_t v = __shfl_sync(0xffffffffu, w[i], 0);
+            if (lane == i) mine = v;
+        }
+        const int more = __shfl_sync(0xffffffffu, ti.valid, 0);
+        if (lane < 16) {
+            asm volatile("st.shared.u32 [%0], %1;" ::"r"(sm.tinfo(q) + 4u * lane), "r"(mine) : "memory");
+            ptx::st_cluster_u32(ptx::mapa(sm.tinfo(q), 1) + 4u * lane, mine);
+        }
+        __syncwarp();
+        if (lane == 0) {
+            ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_full(q), 0));
+            ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_full(q), 1));
+        }
+        if (!more) break;
+        if (++q == G2_NTI) { q = 0; ph ^= 1; }
+    }
+}
+
+// Consumer side of the TileInfo ring: wait for record q, copy it to registers, release the ring entry.
+__device__ __forceinline__ TileInfo g2_take(const G2Smem& sm, int q, uint32_t ph, bool release_lane) {
+    ptx::mbar_wait_cluster(sm.ti_full(q), ph);
+    TileInfo ti;
+    uint32_t* w = reinterpret_cast<uint32_t*>(&ti);
+#pragma unroll
+    for (int i = 0; i < 16; i += 4)
+        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(w[i]), "=r"(w[i + 1]), "=r"(w[i + 2]), "=r"(w[i + 3]) : "r"(sm.tinfo(q) + 4u * i) : "memory");
+    __syncwarp();
+    if (release_lane) ptx::mbar_arrive_cluster_relaxed(ptx::mapa(sm.ti_empty(q), 0), w[0] ^ w[15]);
+    return ti;
+}
+
+// ------------------------------------------------------------------------------------------------
+// TMA producer (one warp per CTA; lane 0 issues).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap* maps, uint32_t rank, int lane) {
+    int stage = 0; uint32_t phase = 0;
+    int q = 0; uint32_t tph = 0;
+    for (;;) {
+        const TileInfo ti = g2_take(sm, q, tph, lane == 0);
+        if (++q == G2_NTI) { q = 0; tph ^= 1; }
+        if (!ti.valid) break;
+        const CUtensorMap* map_a = maps + (size_t)ti.slot * NBUF + ti.a_buf;
+        const CUtensorMap* map_b = maps + (size_t)ti.slot * NBUF + ti.b_buf;
+        const int nkb = (ti.n16 + BK - 1) / BK;
+        const int half = ti.bn >> 1;
+        const int nbox = (half + 63) >> 6;
+        const uint32_t bytes = 2u * (G2_A_BYTES + nbox * B_BOX_BYTES);     // both CTAs of the pair
+        const int row0 = ti.m0 + 128 * (int)rank;
+        const int col0 = ti.n0 + half * (int)rank;
+        const uint32_t full0 = ptx::mapa(sm.full(0), 0);                    // the leader's full barriers
+        for (int kb = 0; kb < nkb; ++kb) {
+            ptx::mbar_wait(sm.empty(stage), phase ^ 1);
+            if (lane == 0) {
+                const uint32_t fb = full0 + 8u * stage;
+                if (rank == 0) ptx::mbar_expect_tx(sm.full(stage), bytes);
+                const uint32_t sa = sm.stage_a(stage), sb = sm.stage_b(stage);
+                ptx::tma_load_2d_pair(sa, map_a, kb * BK, row0, fb);
+                ptx::tma_load_2d_pair(sa + 8192, map_a, kb * BK, row0 + 64, fb);
+                for (int b = 0; b < nbox; ++b)
+                    ptx::tma_load_2d_pair(sb + b * B_BOX_BYTES, map_b, col0 + b * 64, kb * BK, fb);
+            }
+            __syncwarp();
+            if (++stage == G2_STAGES) { stage = 0; phase ^= 1; }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// MMA issuer (leader CTA, one warp; one elected lane issues).
+// The issue loop must stay well under the tensor-pipe time of a k-block (4 MMAs x ~120 cycles): the
+// four MMAs of a full k-block go out as one asm block with the descriptors advanced by immediates
+// (A: +32 B per 16 k inside the 128-byte swizzle row; B: +2048 B = 16 k-rows of 128 B).
+// ------------------------------------------------------------------------------------------------
+namespace ptx {
+// 4 x (M = 256, N, K = 16) on one 64-k stage; acc0 = 0 overwrites the accumulator with the first MMA.
+__device__ __forceinline__ void umma_f16_pair_x4(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc0) {
+    asm volatile(
+        "{\n\t.reg .pred p, t;\n\t.reg .b64 a1, b1, a2, b2, a3, b3;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "setp.eq.b32 t, 0, 0;\n\t"
+        "add.s64 a1, %1, 2;\n\tadd.s64 b1, %2, 128;\n\t"
+        "add.s64 a2, %1, 4;\n\tadd.s64 b2, %2, 256;\n\t"
+        "add.s64 a3, %1, 6;\n\tadd.s64 b3, %2, 384;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], a1, b1, %3, t;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], a2, b2, %3, t;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], a3, b3, %3, t;\n\t}\n"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc0) : "memory");
+}
+}  // namespace ptx
+
+__device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int lane) {
+    int stage = 0; uint32_t phase = 0;
+    int acc = 0; uint32_t acc_phase = 0;
+    int q = 0; uint32_t tph = 0;
+    // descriptors of stage 0; stage s adds s * G2_STAGE_BYTES / 16 to the address field
+    const uint64_t da0 = make_smem_desc(sm.stage_a(0), 16, 1024);
+    const uint64_t db0 = make_smem_desc(sm.stage_b(0), B_BOX_BYTES, 1024);
+    G2_TDECL();
+    const long long tstart_ = clock64();
+    for (;;) {
+        TileInfo ti;
+        { G2_T0(); ti = g2_take(sm, q, tph, lane == 0); G2_T1(0); }
+        if (++q == G2_NTI) { q = 0; tph ^= 1; }
+        if (!ti.valid) break;
+        const int nkb = (ti.n16 + BK - 1) / BK;
+        const int ktail = (ti.n16 - (nkb - 1) * BK) >> 4;          // 16-k slices of the last k-block (1..4)
+        const uint32_t idesc = make_idesc_f16(256, ti.bn);
+        { G2_T0(); ptx::mbar_wait_cluster(sm.tempty(acc), acc_phase ^ 1); G2_T1(1); }
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + acc * 256;
+        for (int kb = 0; kb < nkb; ++kb) {
+            { G2_T0(); ptx::mbar_wait(sm.full(stage), phase); G2_T1(2); }
+            ptx::tc_fence_after();
+            if (ptx::elect_one()) {
+                const uint64_t da = da0 + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
+                const uint64_t db = db0 + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
+                if (kb < nkb - 1 || ktail == 4) {
+                    ptx::umma_f16_pair_x4(d_tmem, da, db, idesc, kb != 0);
+                } else {
+                    for (int k = 0; k < ktail; ++k)
+                        ptx::umma_f16_pair(d_tmem, da + 2 * k, db + 128 * k, idesc, (kb | k) != 0);
+                }
+                ptx::umma_commit_pair(sm.empty(stage));
+                if (kb == nkb - 1) ptx::umma_commit_pair(sm.tfull(acc));
+            }
+            __syncwarp();
+            if (++stage == G2_STAGES) { stage = 0; phase ^= 1; }
+        }
+        if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+    }
+#ifdef G2_TIMING
+    tacc_[3] = clock64() - tstart_;
+#endif
+    G2_TFLUSH(lane == 0);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Epilogue (warps 0..3 of each CTA): C = sgn * alpha * acc + beta * I, FP16 stores, fused squared
+// residual || alpha A B - I ||_F^2 (the convergence test, C-7). `done(ti)` is called by one
+// thread of the CTA after all of the CTA's stores of the tile have been issued and fenced.
+// ------------------------------------------------------------------------------------------------
+template <typename Done>
+__device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base, const Engine& e, __half* base,
+                                            uint32_t rank, int warp, int lane, Done done) {
+    int acc = 0; uint32_t acc_phase = 0;
+    int q = 0; uint32_t tph = 0;
+    const uint32_t tempty0 = ptx::mapa(sm.tempty(0), 0);
+    const int quarter = warp & 3, chalf = warp >> 2;
+    G2_TDECL();
+    for (;;) {
+        TileInfo ti;
+        { G2_T0(); ti = g2_take(sm, q, tph, lane == 0); G2_T1(4); }
+        if (++q == G2_NTI) { q = 0; tph ^= 1; }
+        if (!ti.valid) break;
+        const int n = ti.n, n16 = ti.n16, bn = ti.bn;
+        __half* C = base + buf_off(e, ti.slot, ti.c_buf);
+        const int rbase = ti.m0 + 128 * (int)rank + quarter * 32;      // first row of this warp
+        const int row = rbase + lane;
+        const int col0 = ti.n0;
+        const float sa = ti.sgn * ti.alpha;
+        { G2_T0(); ptx::mbar_wait(sm.tfull(acc), acc_phase); G2_T1(5); }
+        G2_T0();
+        ptx::tc_fence_after();
+        float rsum = 0.f, vsum = 0.f;
+        uint32_t dep = 0;
+        for (int c = chalf * 32; c < bn; c += 64) {
+            if (col0 + c >= n16) break;                            // warp-uniform
+            uint32_t v[32];
+            ptx::tmem_ld_32x32(tmem_base + acc * 256 + ((uint32_t)(quarter * 32) << 16) + c, v);
+            ptx::tmem_ld_wait();
+            dep ^= v[0];
+            __half* crow = C + (size_t)row * e.ld + col0 + c;
+            const bool full = (c + 32 <= bn) && (col0 + c + 32 <= n16);
+            const bool diag = (col0 + c < rbase + 32) && (col0 + c + 32 > rbase);
+            if (full && !diag) {
+                // interior chunk: C = (sgn alpha) acc, residual term alpha^2 acc^2 (no identity entries here)
+                if (row < n16) {
+                    float f[32];
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        const float a = __uint_as_float(v[j]);
+                        vsum = fmaf(a, a, vsum);
+                        f[j] = sa * a;
+                    }
+#pragma unroll
+                    for (int j = 0; j < 32; j += 8) st_half8(crow + j, f + j);
+                }
+            } else if (row < n16) {
+                float f[32];
+#pragma unroll
+                for (int j = 0; j < 32; ++j) {
+                    const int col = col0 + c + j;
+                    const float x = ti.alpha * __uint_as_float(v[j]);
+                    const float delta = (col == row && row < n) ? 1.f : 0.f;
+                    const float d = (c + j < bn && col < n16) ? x - delta : 0.f;   // pad rows / columns give exactly 0
+                    rsum = fmaf(d, d, rsum);
+                    f[j] = ti.sgn * x + ti.beta * delta;
+                }
+                const int cw = min(min(32, bn - c), n16 - (col0 + c));   // 16 or 32 valid columns
+#pragma unroll
+                for (int j = 0; j < 32; j += 8)
+                    if (j < cw) st_half8(crow + j, f + j);
+            }
+        }
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive_cluster_relaxed(tempty0 + 8u * acc, dep);
+        if (ti.want_res) {
+            rsum = fmaf(ti.alpha * ti.alpha, vsum, rsum);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) rsum += __shfl_xor_sync(0xffffffffu, rsum, o);
+            if (lane == 0 && rsum != 0.f) atomicAdd(&e.slots[ti.slot].res_acc, rsum);
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(G2_EPI_WARPS * 32) : "memory");   // the CTA's epilogue warps
+        G2_T1(6);
+        if (warp == 0 && lane == 0) done(ti);
+        G2_T1(7);
+        if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+    }
+    G2_TFLUSH(warp == 0 && lane == 0);
+}
+
+// ================================================================================================
+// Round engine: one launch serves the op table `launch` of the running round; pair p walks the tile
+// list with stride #pairs.
+// ================================================================================================
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(G2_CTRL_THREADS, 1)
+gemm2_round_kernel(const __grid_constant__ UmmaArgs args) {
+    extern __shared__ uint8_t smem_raw[];
+    const Engine& e = args.e;
+    const SlotOp* ops = e.ops + args.launch * e.S;
+    const int ntiles = e.ntiles[args.launch];
+    G2Smem sm;
+    sm.base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = ptx::cluster_ctarank();
+    const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
+    if (pair >= ntiles) return;                                   // whole cluster idle (uniform per pair)
+
+    const uint32_t tmem_base = g2_setup(sm, warp, lane);
+
+    if (warp < G2_EPI_WARPS) {
+        g2_epilogue(sm, tmem_base, e, args.base, rank, warp, lane, [&](const TileInfo& ti) {
+            SlotOp op = ops[ti.slot];
+            op.ntiles = ti.nreports;
+            tile_finished(e, ti.slot, op);
+        });
+    } else if (warp == G2_WARP_SCHED) {
+        if (rank == 0) {
+            int tile = pair;
+            g2_scheduler(sm, lane, [&](TileInfo& ti) {
+                if (tile >= ntiles) return false;
+                const int slot = find_slot(ops, e.S, tile);
+                const SlotOp op = ops[slot];
+                const Slot& sl = e.slots[slot];
+                const int t = tile - op.tile_start;
+                const int tm = t / sl.ntn, tn = t - tm * sl.ntn;
+                ti.slot = slot; ti.m0 = tm * BM; ti.n0 = tn * BN;
+                ti.n = sl.n; ti.n16 = sl.n16; ti.bn = min(BN, sl.n16 - tn * BN); ti.nreports = 2 * op.ntiles;
+                ti.a_buf = op.a_buf; ti.b_buf = op.b_buf; ti.c_buf = op.c_buf; ti.want_res = op.want_res;
+                ti.alpha = op.alpha; ti.sgn = op.sgn; ti.beta = op.beta; ti.kind = op.kind;
+                tile += npairs;
+                return true;
+            });
+        }
+    } else if (warp == G2_WARP_TMA) {
+        g2_producer(sm, args.maps, rank, lane);
+    } else if (warp == G2_WARP_MMA) {
+        if (rank == 0) g2_mma(sm, tmem_base, lane);
+    }
+    g2_teardown(tmem_base, warp);
+}
+
+}  // namespace nolsm

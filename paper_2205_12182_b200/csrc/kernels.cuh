@@ -32,12 +32,11 @@ struct SysView {
     const int* nset_off;          // first row/column of atom j inside submatrix i
 };
 
-__device__ __forceinline__ void choose_tiling(int n16, int& ntm, int& ntn, int& bn) {
+// Tiles of one n16 x n16 GEMM: ntm x ntn tiles of BM x BN; the last tile column is exactly as wide as
+// what is left (a multiple of 16), so no columns are padded; rows are padded to BM.
+__host__ __device__ __forceinline__ void choose_tiling(int n16, int& ntm, int& ntn) {
     ntm = (n16 + BM - 1) / BM;
-    ntn = (n16 + 255) / 256;
-    bn = ((n16 + ntn - 1) / ntn + 15) / 16 * 16;
-    if (bn > 256) bn = 256;
-    ntn = (n16 + bn - 1) / bn;
+    ntn = (n16 + BN - 1) / BN;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -69,7 +68,7 @@ __global__ void __launch_bounds__(MAX_SLOTS) k_round_begin(Engine e) {
             const int a = atomicAdd(e.next_atom, 1);
             if (a < e.a_end) {
                 s.atom = a; s.n = e.at.dim[a]; s.n16 = (s.n + 15) & ~15; s.pos = e.at.pos[a]; s.nbi = e.at.nb[a];
-                choose_tiling(s.n16, s.ntm, s.ntn, s.bn);
+                choose_tiling(s.n16, s.ntm, s.ntn);
                 s.inv_iters = 0; s.sign_iters = 0; s.conv = 0; s.xcur = 0; s.ycur = 2; s.status = 0;
                 s.gemm_count = 0; s.tiles_done = 0;
                 s.res_acc = 0.f; s.res_prev = 1e30f; s.res_last = 0.f; s.rho_s = 0.f; s.rho_a = 0.f;
@@ -101,7 +100,7 @@ __global__ void __launch_bounds__(MAX_SLOTS) k_round_begin(Engine e) {
         if (e.profiling && (t0 || t1)) {
             const double n = s.n, ng = (t0 ? 1 : 0) + (t1 ? 1 : 0);
             atomicAdd(&s_fl[0], 2.0 * n * n * n * ng);
-            atomicAdd(&s_fl[1], 2.0 * (double)(s.ntm * BM) * (double)(s.ntn * s.bn) * (double)s.n16 * ng);
+            atomicAdd(&s_fl[1], 2.0 * (double)(s.ntm * BM) * (double)s.n16 * (double)s.n16 * ng);
         }
     }
     s_t0[threadIdx.x] = t0; s_t1[threadIdx.x] = t1;

@@ -12,7 +12,7 @@
 #include <vector>
 
 #include "../../include/nolsm.h"
-#include "gemm_umma.cuh"
+#include "gemm2sm.cuh"
 #include "kernels.cuh"
 #include "tmap_host.h"
 
@@ -182,14 +182,6 @@ bool use_umma(const nolsm_ctx* c) {
     return c->opt.gemm_backend != NOLSM_GEMM_SIMT;
 }
 
-void host_tiling(int n16, int& ntm, int& ntn, int& bn) {      // mirrors choose_tiling (kernels.cuh)
-    ntm = (n16 + BM - 1) / BM;
-    ntn = (n16 + 255) / 256;
-    bn = ((n16 + ntn - 1) / ntn + 15) / 16 * 16;
-    if (bn > 256) bn = 256;
-    ntn = (n16 + bn - 1) / bn;
-}
-
 SysView sys_view(const nolsm_ctx* c) {
     SysView v;
     v.row_ptr = c->d_row_ptr; v.col_idx = c->d_col_idx; v.blk_off = c->d_blk_off; v.atom_nb = c->d_atom_nb;
@@ -218,7 +210,7 @@ void launch_gemm(nolsm_ctx* c, const Engine& e, int launch, cudaStream_t s) {
     if (use_umma(c)) {
         UmmaArgs a;
         a.e = e; a.maps = c->d_maps; a.base = (__half*)c->ws; a.launch = launch;
-        LAUNCH(c, K_GEMM, s, gemm_umma_kernel<<<c->sms, UMMA_THREADS, UMMA_SMEM_BYTES, s>>>(a));
+        LAUNCH(c, K_GEMM, s, gemm2_round_kernel<<<c->sms & ~1, G2_CTRL_THREADS, G2_SMEM_BYTES, s>>>(a));
     } else {
         const int t64 = (e.cap + 63) / 64;
         LAUNCH(c, K_GEMM, s, k_gemm_simt<T><<<dim3(t64 * t64, e.S), 256, 0, s>>>(e, (T*)c->ws, launch));
@@ -340,7 +332,7 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
     for (int i = 0; i < ROUND_DEPTH; ++i) ok = ok && cudaEventCreateWithFlags(&c->ev_round[i], cudaEventDisableTiming) == cudaSuccess;
     if (!ok) { cudaGetLastError(); delete c; return NOLSM_ECUDA; }
     if (use_umma(c)) {
-        if (cudaFuncSetAttribute(gemm_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, UMMA_SMEM_BYTES) != cudaSuccess) {
+        if (cudaFuncSetAttribute(gemm2_round_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, G2_SMEM_BYTES) != cudaSuccess) {
             cudaGetLastError();
             delete c;
             return NOLSM_ECUDA;
@@ -489,8 +481,8 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         min_n = std::min(min_n, c->dim[i]);
         max_nset = std::max<int>(max_nset, (int)(c->nset_ptr[i + 1] - c->nset_ptr[i]));
         max_nbi = std::max(max_nbi, c->atom_nb[i]);
-        int ntm, ntn, bn;
-        host_tiling((c->dim[i] + 15) & ~15, ntm, ntn, bn);
+        int ntm, ntn;
+        choose_tiling((c->dim[i] + 15) & ~15, ntm, ntn);
         mean_tiles += (double)ntm * ntn;
     }
     mean_tiles /= (double)n_atoms;
@@ -519,7 +511,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     e = Engine{};
     const size_t es = elem_size(c);
     e.cap = (max_n + 15) & ~15;
-    e.ld = e.cap;
+    e.ld = (e.cap + 63) & ~63;        // rows start on 128-byte lines: TMA boxes map to whole L2 lines
     e.bufsz = (long long)e.cap * e.ld;
     e.slotsz = e.bufsz * NBUF;
     size_t free_b = 0, total_b = 0;
@@ -801,10 +793,10 @@ int nolsm_get_stats(nolsm_ctx* c, nolsm_stats* out) {
             out->sum_inv_iters += inv[i]; out->sum_sign_iters += sg[i]; out->gemms_executed += gm[i];
             const double d = c->dim[i];
             out->flops_useful += 2.0 * d * d * d * gm[i];
-            int ntm, ntn, bn;
+            int ntm, ntn;
             const int n16 = (c->dim[i] + 15) & ~15;
-            host_tiling(n16, ntm, ntn, bn);
-            out->flops_padded += 2.0 * (double)(ntm * BM) * (double)(ntn * bn) * (double)n16 * gm[i];
+            choose_tiling(n16, ntm, ntn);
+            out->flops_padded += 2.0 * (double)(ntm * BM) * (double)n16 * (double)n16 * gm[i];
             out->n_notspd += (st[i] & ST_NOTSPD) ? 1 : 0;
             out->n_noconv += (st[i] & ST_NOCONV) ? 1 : 0;
         }

@@ -28,7 +28,8 @@
 namespace nolsm {
 
 constexpr int NBUF = 5;          // B0 = S then X(even), B1 = H0 then X(odd), B2/B3 = Y ping-pong, B4 = R / T
-constexpr int BM = 128;          // GEMM tile rows
+constexpr int BM = 256;          // GEMM tile rows (one CTA pair, tcgen05 cta_group::2)
+constexpr int BN = 256;          // GEMM tile columns; the last tile of a row is n16 - 256 (ntn - 1) wide
 constexpr int BK = 64;           // GEMM k-block (one 128-byte swizzle atom of fp16)
 constexpr int MAX_SLOTS = 1024;
 
@@ -40,7 +41,7 @@ enum OpKind { OP_NONE = 0, OP_INV_G1, OP_INV_G2, OP_AMAT, OP_SIGN_G1, OP_SIGN_G2
 
 struct __align__(16) Slot {
     // geometry of the atom in the slot (written at refill)
-    int atom, n, n16, pos, nbi, ntm, ntn, bn;
+    int atom, n, n16, pos, nbi, ntm, ntn, pad0;
     // phase machine
     int phase;       // current phase (advanced by the kernels of the running round)
     int snap;        // phase when the running round began; kernels gate on this

@@ -52,6 +52,7 @@ enum { NOLSM_PREC_FP16_FP32 = 0, /* FP16 operands, FP32 accumulate, tcgen05 tens
        NOLSM_PREC_FP32 = 1 };    /* all-FP32 validation mode (FFMA, no tensor cores, no TF32) */
 enum { NOLSM_DTYPE_F64 = 0, NOLSM_DTYPE_F32 = 1 };
 enum { NOLSM_GEMM_AUTO = 0, NOLSM_GEMM_UMMA = 1, NOLSM_GEMM_SIMT = 2 };
+enum { NOLSM_ENGINE_AUTO = 0, NOLSM_ENGINE_PERSISTENT = 1, NOLSM_ENGINE_ROUNDS = 2 };
 enum { NOLSM_MAT_NOTSPD = 1, NOLSM_MAT_NOCONV = 2 }; /* per-atom status bits */
 
 /* Zero in any field selects the default given in brackets. */
@@ -67,7 +68,9 @@ typedef struct {
     double eps_filter;       /* block (j,i) enters N(i) iff max(|H0_ji|max, |S_ji|max) > eps_filter [0 = structural] */
     int batch_atoms;         /* workspace slots = submatrices resident at once [auto: ~16 waves of GEMM tiles] */
     size_t workspace_bytes;  /* cap on the library-owned dense workspace [auto] */
-    int profile_every;       /* > 0: every k-th round runs eagerly with CUDA events around each launch [0 = off] */
+    int profile_every;       /* round engine, > 0: every k-th round runs eagerly with CUDA events around each launch [0 = off] */
+    int engine;              /* NOLSM_ENGINE_* [AUTO: PERSISTENT (one kernel launch per density_matrix call) for the
+                                FP16/tcgen05 path when every n_i <= 2048, else ROUNDS (one CUDA graph per iteration round)] */
 } nolsm_options;
 
 typedef struct {
@@ -100,9 +103,9 @@ int nolsm_assemble(nolsm_ctx* ctx, int64_t n_atoms, const int32_t* atom_nb, cons
 
 /* a1-a7 for all atoms: gather, Schulz inverse, spectral scaling, Newton-Schulz sign (Eq. 6),
  * convergence tests, D columns, scatter and energy partials. The work is ordered after everything
- * already enqueued on `cuda_stream`, and `cuda_stream` is made to wait for it; the call itself returns
- * once the last engine round has been enqueued (the host replays one CUDA graph per round and reads a
- * device-written progress counter to know when to stop).
+ * already enqueued on `cuda_stream`, and `cuda_stream` is made to wait for it. Persistent engine: the
+ * call enqueues ONE kernel and returns. Round engine: the call returns once the last round has been
+ * enqueued (the host replays one CUDA graph per round and reads a device-written progress counter).
  *   D_vals   d_dtype[blk_off[nnzb]]   host or device; blocks outside every N(i) are zeroed. */
 int nolsm_density_matrix(nolsm_ctx* ctx, double mu, void* D_vals, int d_dtype, void* cuda_stream);
 
@@ -144,6 +147,16 @@ int nolsm_get_atom_stats(nolsm_ctx* ctx, int64_t atom_begin, int64_t count, int3
  * n must be >= NOLSM_PROFILE_LEN. Synchronises the stream. */
 #define NOLSM_PROFILE_LEN 14
 int nolsm_get_profile(nolsm_ctx* ctx, double* out, int n);
+
+/* Counters of the persistent engine for the last density_matrix call (all zero after a round-engine call).
+ *   out[0] 1 = persistent engine ran;  out[1] kernel duration in ms (CUDA events on its stream);
+ *   out[2] kernel duration from the device clock (first scheduler start to last scheduler end), ms;
+ *   out[3] GEMM tiles executed (256 x bn, one per CTA pair);  out[4], out[5] tile-scheduler idle / busy
+ *   time summed over the CTA pairs, ms;  out[6] claim overshoots;  out[7] slots;  out[8] CTA pairs;
+ *   out[9 + k], out[17 + k], out[25 + k]  side tasks of kind k (1 refill, 2 gather, 3 first Schulz step,
+ *   4 D columns + scatter): busy ms summed over side groups, algorithmic bytes, tasks.  n must be >= NOLSM_COUNTERS_LEN. Synchronises. */
+#define NOLSM_COUNTERS_LEN 33
+int nolsm_get_engine_counters(nolsm_ctx* ctx, double* out, int n);
 
 const char* nolsm_last_error(const nolsm_ctx* ctx);
 

@@ -10,6 +10,7 @@ import numpy as np
 PREC_FP16_FP32, PREC_FP32 = 0, 1
 DTYPE_F64, DTYPE_F32 = 0, 1
 GEMM_AUTO, GEMM_UMMA, GEMM_SIMT = 0, 1, 2
+ENGINE_AUTO, ENGINE_PERSISTENT, ENGINE_ROUNDS = 0, 1, 2
 STATUS_NAMES = {0: "OK", 1: "EINVAL", 2: "ECUDA", 3: "ENOMEM", 4: "ESTATE", 5: "ENOTSPD", 6: "ENOCONV"}
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -20,7 +21,8 @@ class NolsmOptions(C.Structure):
     _fields_ = [("precision", C.c_int), ("gemm_backend", C.c_int), ("max_inv_iters", C.c_int),
                 ("max_sign_iters", C.c_int), ("tol_inv", C.c_float), ("tol_sign", C.c_float),
                 ("power_iters_s", C.c_int), ("power_iters_a", C.c_int), ("eps_filter", C.c_double),
-                ("batch_atoms", C.c_int), ("workspace_bytes", C.c_size_t), ("profile_every", C.c_int)]
+                ("batch_atoms", C.c_int), ("workspace_bytes", C.c_size_t), ("profile_every", C.c_int),
+                ("engine", C.c_int)]
 
 
 class NolsmStats(C.Structure):
@@ -66,11 +68,12 @@ def load_library():
     lib.nolsm_get_stats.argtypes = [P, C.POINTER(NolsmStats)]
     lib.nolsm_get_atom_stats.argtypes = [P, I64, I64, P, P, P, P, P, P, P]
     lib.nolsm_get_profile.argtypes = [P, C.POINTER(C.c_double), I32]
+    lib.nolsm_get_engine_counters.argtypes = [P, C.POINTER(C.c_double), I32]
     lib.nolsm_last_error.argtypes = [P]
     lib.nolsm_last_error.restype = C.c_char_p
     for f in ("nolsm_create", "nolsm_assemble", "nolsm_density_matrix", "nolsm_density_matrix_range", "nolsm_energy",
               "nolsm_destroy", "nolsm_get_index_set", "nolsm_gather_submatrix", "nolsm_get_stats",
-              "nolsm_get_atom_stats", "nolsm_get_profile"):
+              "nolsm_get_atom_stats", "nolsm_get_profile", "nolsm_get_engine_counters"):
         getattr(lib, f).restype = C.c_int
     _LIB = lib
     return lib
@@ -191,6 +194,18 @@ class Nolsm:
                 "gemm_flops_padded", "dcols_ms", "dcols_launches", "dcols_bytes", "other_ms", "other_launches",
                 "sampled_submatrices", "kernel_launches")
         return dict(zip(keys, list(out)))
+
+    def engine_counters(self) -> dict:
+        """Counters of the persistent engine for the last density_matrix call (include/nolsm.h)."""
+        out = (C.c_double * 33)()
+        self._check(self._lib.nolsm_get_engine_counters(self._h, out, 33))
+        v = list(out)
+        kinds = ("none", "refill", "gather", "schulz1", "dcols", "k5", "k6", "k7")
+        d = {"persistent": bool(v[0]), "kernel_ms": v[1], "kernel_ms_device_clock": v[2], "tiles": v[3],
+             "sched_idle_ms": v[4], "sched_busy_ms": v[5], "overshoots": v[6], "slots": int(v[7]), "pairs": int(v[8])}
+        d["side"] = {k: {"busy_ms": v[9 + i], "bytes": v[17 + i], "tasks": v[25 + i]} for i, k in enumerate(kinds)
+                     if v[25 + i] > 0}
+        return d
 
     def destroy(self):
         if self._h:

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "nolsm_api.cu")
 DEPS = [os.path.join(HERE, "csrc", f) for f in
-        ("nolsm_api.cu", "kernels.cuh", "gemm_umma.cuh", "nolsm_device.cuh", "tmap_host.h")] + \
+        ("nolsm_api.cu", "kernels.cuh", "gemm_umma.cuh", "gemm2sm.cuh", "persist.cuh", "nolsm_device.cuh", "tmap_host.h")] + \
        [os.path.join(os.path.dirname(HERE), "include", "nolsm.h")]
 LIB = os.path.join(HERE, "libnolsm.so")
 

@@ -111,6 +111,15 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
         if (++spins > SPIN_LIMIT) __trap();
     }
 }
+// Wait that may legitimately last long (a role of the persistent engine with no work): polls gently
+// after a short spin; traps only after tens of seconds.
+__device__ __forceinline__ void mbar_wait_cluster_patient(uint32_t bar, uint32_t parity) {
+    uint32_t spins = 0;
+    while (!mbar_try_wait_cluster(bar, parity)) {
+        if (++spins > 2048u) __nanosleep(128);
+        if (spins > (1u << 28)) __trap();
+    }
+}
 __device__ __forceinline__ void st_cluster_u32(uint32_t cluster_addr, uint32_t v) {
     asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(cluster_addr), "r"(v) : "memory");
 }
@@ -208,7 +217,7 @@ __device__ __forceinline__ void g2_scheduler(const G2Smem& sm, int lane, Next ne
 
 // Consumer side of the TileInfo ring: wait for record q, copy it to registers, release the ring entry.
 __device__ __forceinline__ TileInfo g2_take(const G2Smem& sm, int q, uint32_t ph, bool release_lane) {
-    ptx::mbar_wait_cluster(sm.ti_full(q), ph);
+    ptx::mbar_wait_cluster_patient(sm.ti_full(q), ph);
     TileInfo ti;
     uint32_t* w = reinterpret_cast<uint32_t*>(&ti);
 #pragma unroll
@@ -230,8 +239,9 @@ __device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap*
         const TileInfo ti = g2_take(sm, q, tph, lane == 0);
         if (++q == G2_NTI) { q = 0; tph ^= 1; }
         if (!ti.valid) break;
-        const CUtensorMap* map_a = maps + (size_t)ti.slot * NBUF + ti.a_buf;
-        const CUtensorMap* map_b = maps + (size_t)ti.slot * NBUF + ti.b_buf;
+        ptx::fence_proxy_async();      // operands may have been written by generic stores of another CTA
+        const CUtensorMap* map_a = maps + (size_t)ti.slot * NMAP + ti.a_buf;
+        const CUtensorMap* map_b = maps + (size_t)ti.slot * NMAP + ti.b_buf;
         const int nkb = (ti.n16 + BK - 1) / BK;
         const int half = ti.bn >> 1;
         const int nbox = (half + 63) >> 6;
@@ -331,8 +341,8 @@ __device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int
 // residual || alpha A B - I ||_F^2 (the convergence test, C-7). `done(ti)` is called by one
 // thread of the CTA after all of the CTA's stores of the tile have been issued and fenced.
 // ------------------------------------------------------------------------------------------------
-template <typename Done>
-__device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base, const Engine& e, __half* base,
+template <typename Eng, typename Done>
+__device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base, const Eng& e, __half* base,
                                             uint32_t rank, int warp, int lane, Done done) {
     int acc = 0; uint32_t acc_phase = 0;
     int q = 0; uint32_t tph = 0;
@@ -345,7 +355,9 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
         if (++q == G2_NTI) { q = 0; tph ^= 1; }
         if (!ti.valid) break;
         const int n = ti.n, n16 = ti.n16, bn = ti.bn;
-        __half* C = base + buf_off(e, ti.slot, ti.c_buf);
+        int ldc;
+        __half* C = c_ptr(e, base, ti.slot, ti.c_buf, ldc);
+        const bool ident = ti.kind != OP_POW_S && ti.kind != OP_POW_A;   // power-iteration tiles: C = alpha A V, res = ||C||_F^2
         const int rbase = ti.m0 + 128 * (int)rank + quarter * 32;      // first row of this warp
         const int row = rbase + lane;
         const int col0 = ti.n0;
@@ -361,7 +373,7 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
             ptx::tmem_ld_32x32(tmem_base + acc * 256 + ((uint32_t)(quarter * 32) << 16) + c, v);
             ptx::tmem_ld_wait();
             dep ^= v[0];
-            __half* crow = C + (size_t)row * e.ld + col0 + c;
+            __half* crow = C + (size_t)row * ldc + col0 + c;
             const bool full = (c + 32 <= bn) && (col0 + c + 32 <= n16);
             const bool diag = (col0 + c < rbase + 32) && (col0 + c + 32 > rbase);
             if (full && !diag) {
@@ -383,7 +395,7 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                 for (int j = 0; j < 32; ++j) {
                     const int col = col0 + c + j;
                     const float x = ti.alpha * __uint_as_float(v[j]);
-                    const float delta = (col == row && row < n) ? 1.f : 0.f;
+                    const float delta = (col == row && row < n && ident) ? 1.f : 0.f;
                     const float d = (c + j < bn && col < n16) ? x - delta : 0.f;   // pad rows / columns give exactly 0
                     rsum = fmaf(d, d, rsum);
                     f[j] = ti.sgn * x + ti.beta * delta;
@@ -395,6 +407,7 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
             }
         }
         ptx::tc_fence_before();
+        ptx::fence_proxy_async();      // C is read next through the async proxy (TMA), possibly by another CTA
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive_cluster_relaxed(tempty0 + 8u * acc, dep);
         if (ti.want_res) {

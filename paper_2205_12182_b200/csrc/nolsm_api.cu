@@ -3,6 +3,7 @@
 // runs in the kernels of kernels.cuh and gemm_umma.cuh.
 #include <algorithm>
 #include <atomic>
+#include <chrono>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -14,6 +15,7 @@
 #include "../../include/nolsm.h"
 #include "gemm2sm.cuh"
 #include "kernels.cuh"
+#include "persist.cuh"
 #include "tmap_host.h"
 
 using namespace nolsm;
@@ -74,6 +76,17 @@ struct nolsm_ctx {
     cudaEvent_t ev_round[ROUND_DEPTH] = {};
     cudaGraphExec_t graph_exec = nullptr;
     bool use_graph = true;
+
+    // persistent engine (persist.cuh): one kernel launch per density_matrix call
+    bool persist = false;
+    PEngine peng{};
+    int* d_abort = nullptr;
+    cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr;
+    int h_a0 = 0;
+    unsigned long long h_ctr0[PC_LEN] = {};
+    std::vector<unsigned int> h_sclaim0;
+    bool last_persist = false;
+    double timeout_s = 300.0;
 
     // last density call
     cudaStream_t last_stream = nullptr;
@@ -182,6 +195,14 @@ bool use_umma(const nolsm_ctx* c) {
     return c->opt.gemm_backend != NOLSM_GEMM_SIMT;
 }
 
+// The persistent engine serves the mixed-precision tcgen05 path; the round engine serves the FP32 / SIMT
+// validation modes (and NOLSM_ENGINE=rounds).
+bool want_persist(const nolsm_ctx* c) {
+    if (!use_umma(c)) return false;
+    if (c->opt.engine == NOLSM_ENGINE_ROUNDS) return false;
+    return true;
+}
+
 SysView sys_view(const nolsm_ctx* c) {
     SysView v;
     v.row_ptr = c->d_row_ptr; v.col_idx = c->d_col_idx; v.blk_off = c->d_blk_off; v.atom_nb = c->d_atom_nb;
@@ -285,6 +306,31 @@ int enqueue_round(nolsm_ctx* c, const Engine& e, void* D, int d_dtype, bool fork
     return NOLSM_OK;
 }
 
+// Waits for the last density_matrix call. The persistent kernel is watched: past the time limit the host
+// raises the kernel's abort word (copy on a second stream), which makes every role leave its loop.
+int wait_result(nolsm_ctx* c) {
+    if (c->last_persist) {
+        const auto t0 = std::chrono::steady_clock::now();
+        bool aborted = false;
+        for (;;) {
+            const cudaError_t q = cudaEventQuery(c->ev_out);
+            if (q == cudaSuccess) break;
+            if (q != cudaErrorNotReady) { c->err = std::string("persistent engine: ") + cudaGetErrorString(q); return NOLSM_ECUDA; }
+            const double el = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+            if (!aborted && el > c->timeout_s) {
+                static const int one = 1;
+                cudaMemcpyAsync(c->d_abort, &one, 4, cudaMemcpyHostToDevice, c->s_x);
+                aborted = true;
+            }
+            if (el > c->timeout_s + 20.0) { c->err = "persistent engine did not stop after abort"; return NOLSM_ECUDA; }
+            std::this_thread::sleep_for(std::chrono::microseconds(el < 0.01 ? 20 : 200));
+        }
+        if (aborted) { c->err = "persistent engine exceeded its time limit and was aborted"; return NOLSM_ECUDA; }
+    }
+    CU_TRY(c, cudaStreamSynchronize(c->last_stream));
+    return NOLSM_OK;
+}
+
 int getenv_int(const char* name, int dflt) {
     const char* v = getenv(name);
     return v && *v ? atoi(v) : dflt;
@@ -324,15 +370,23 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
     if (getenv_int("NOLSM_PROFILE_EVERY", 0) > 0) o.profile_every = getenv_int("NOLSM_PROFILE_EVERY", 0);
     if (getenv_int("NOLSM_SLOTS", 0) > 0) o.batch_atoms = getenv_int("NOLSM_SLOTS", 0);
     c->use_graph = getenv_int("NOLSM_GRAPH", 1) != 0;
+    if (const char* en = getenv("NOLSM_ENGINE")) {
+        if (!strcmp(en, "rounds")) o.engine = NOLSM_ENGINE_ROUNDS;
+        else if (!strcmp(en, "persistent")) o.engine = NOLSM_ENGINE_PERSISTENT;
+    }
+    if (o.engine < 0 || o.engine > NOLSM_ENGINE_ROUNDS) { delete c; return NOLSM_EINVAL; }
+    if (getenv_int("NOLSM_TIMEOUT_S", 0) > 0) c->timeout_s = getenv_int("NOLSM_TIMEOUT_S", 0);
     bool ok = cudaStreamCreateWithFlags(&c->s_main, cudaStreamNonBlocking) == cudaSuccess &&
               cudaStreamCreateWithFlags(&c->s_x, cudaStreamNonBlocking) == cudaSuccess &&
               cudaStreamCreateWithFlags(&c->s_f, cudaStreamNonBlocking) == cudaSuccess;
     cudaEvent_t* evs[] = {&c->ev_fork, &c->ev_x, &c->ev_f, &c->ev_in, &c->ev_out};
     for (cudaEvent_t* e : evs) ok = ok && cudaEventCreateWithFlags(e, cudaEventDisableTiming) == cudaSuccess;
     for (int i = 0; i < ROUND_DEPTH; ++i) ok = ok && cudaEventCreateWithFlags(&c->ev_round[i], cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaEventCreate(&c->ev_k0) == cudaSuccess && cudaEventCreate(&c->ev_k1) == cudaSuccess;
     if (!ok) { cudaGetLastError(); delete c; return NOLSM_ECUDA; }
     if (use_umma(c)) {
-        if (cudaFuncSetAttribute(gemm2_round_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, G2_SMEM_BYTES) != cudaSuccess) {
+        if (cudaFuncSetAttribute(gemm2_round_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, G2_SMEM_BYTES) != cudaSuccess ||
+            cudaFuncSetAttribute(nolsm_persist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES) != cudaSuccess) {
             cudaGetLastError();
             delete c;
             return NOLSM_ECUDA;
@@ -347,7 +401,7 @@ int nolsm_destroy(nolsm_ctx* c) {
     cudaSetDevice(c->dev);
     free_assembled(c);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
-    cudaEvent_t evs[] = {c->ev_fork, c->ev_x, c->ev_f, c->ev_in, c->ev_out};
+    cudaEvent_t evs[] = {c->ev_fork, c->ev_x, c->ev_f, c->ev_in, c->ev_out, c->ev_k0, c->ev_k1};
     for (cudaEvent_t e : evs) if (e) cudaEventDestroy(e);
     for (int i = 0; i < ROUND_DEPTH; ++i) if (c->ev_round[i]) cudaEventDestroy(c->ev_round[i]);
     if (c->s_main) cudaStreamDestroy(c->s_main);
@@ -518,14 +572,26 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     CU_TRY(c, cudaMemGetInfo(&free_b, &total_b));
     const size_t slot_bytes = (size_t)e.slotsz * es;
     const size_t cap_bytes = c->opt.workspace_bytes ? c->opt.workspace_bytes : std::min<size_t>(free_b / 2, (size_t)48 << 30);
-    // default: enough slots for ~16 waves of 128 x bn tiles per GEMM launch
-    int S = c->opt.batch_atoms > 0 ? c->opt.batch_atoms : (int)std::ceil(16.0 * c->sms / std::max(1.0, mean_tiles));
+    // persistent engine: slot buffers must fit the side tasks' shared memory (power-iteration vectors, Y columns)
+    const int g_rowatoms = std::min(P_GATHER_ROWATOMS, std::max(1, getenv_int("NOLSM_GATHER_ROWATOMS", 2)));
+    c->persist = want_persist(c) && e.cap <= P_MAX_CAP &&
+                 (size_t)(max_nset + 1) * 4 + 16 + (size_t)max_nbi * e.cap * 2 <= (size_t)P_SIDE_SMEM &&
+                 (size_t)(2 * max_nset + 1) * 4 + 8 + (size_t)g_rowatoms * max_nset * 8 + (size_t)e.cap * 2 <= (size_t)P_SIDE_SMEM;
+    if (!c->persist && c->opt.engine == NOLSM_ENGINE_PERSISTENT)
+        return fail(c, NOLSM_EINVAL, "the persistent engine needs FP16/tcgen05 mode and submatrix dimensions <= 2048");
+    // round engine: enough slots for ~16 waves of tiles per GEMM launch; persistent engine: the slots in
+    // flight (GEMM chain + side phases), few enough to keep the active iterates in L2
+    int S = c->opt.batch_atoms > 0 ? c->opt.batch_atoms
+            : c->persist ? (int)std::min(64.0, std::max(16.0, std::ceil(5.0 * c->sms / std::max(1.0, mean_tiles))))
+                         : (int)std::ceil(16.0 * c->sms / std::max(1.0, mean_tiles));
     S = std::max(S, 2);
     S = (int)std::min<size_t>(S, std::max<size_t>(2, cap_bytes / slot_bytes));
     S = std::min(S, MAX_SLOTS);
     S = (int)std::min<int64_t>(S, std::max<int64_t>(2, n_atoms));
     e.S = S;
-    c->ws_bytes = slot_bytes * S;
+    // after the S slots: two vector blocks per slot and one shared start block (block power iteration), cap x VLD each
+    const size_t vec_bytes = (size_t)e.cap * VLD * es;
+    c->ws_bytes = slot_bytes * S + vec_bytes * (2 * (size_t)S + 1);
     if ((r = dmalloc(c, &c->ws, c->ws_bytes))) return r;
     CU_TRY(c, cudaMemsetAsync(c->ws, 0, c->ws_bytes, s));
     if ((r = dmalloc(c, (void**)&e.slots, sizeof(Slot) * S))) return r;
@@ -564,19 +630,59 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     CU_TRY(c, cudaMemsetAsync(c->d_e_atom, 0, 8 * n_atoms, s));
     if (use_umma(c)) {
         if (!encode_tiled_fn()) return fail(c, NOLSM_ECUDA, "cuTensorMapEncodeTiled not available");
-        std::vector<CUtensorMap> maps((size_t)S * NBUF);
-        for (int sl = 0; sl < S; ++sl)
+        std::vector<CUtensorMap> maps((size_t)S * NMAP);
+        const __half* vec0 = (const __half*)c->ws + (long long)S * e.slotsz;
+        for (int sl = 0; sl < S; ++sl) {
             for (int b = 0; b < NBUF; ++b) {
                 const __half* base = (const __half*)c->ws + (long long)sl * e.slotsz + (long long)b * e.bufsz;
-                if (!make_tmap_f16_64x64(&maps[(size_t)sl * NBUF + b], base, e.cap, e.ld))
+                if (!make_tmap_f16_64x64(&maps[(size_t)sl * NMAP + b], base, e.cap, e.ld))
                     return fail(c, NOLSM_ECUDA, "cuTensorMapEncodeTiled failed");
             }
+            for (int v = 0; v < 3; ++v) {       // maps 5, 6: the slot's vector blocks; map 7: the shared start block
+                const __half* base = vec0 + (v < 2 ? (long long)sl * 2 + v : (long long)S * 2) * ((long long)e.cap * VLD);
+                if (!make_tmap_f16_64x64(&maps[(size_t)sl * NMAP + NBUF + v], base, e.cap, VLD, VLD))
+                    return fail(c, NOLSM_ECUDA, "cuTensorMapEncodeTiled failed");
+            }
+        }
+        {   // start block of the power iterations: +-1 from a fixed hash in the first NVC columns, zero elsewhere
+            std::vector<__half> v0((size_t)e.cap * VLD, __float2half(0.f));
+            for (int rr = 0; rr < e.cap; ++rr)
+                for (int cc = 0; cc < NVC; ++cc) {
+                    unsigned h = (unsigned)(rr * NVC + cc) * 2654435761u + 0x9E3779B9u;
+                    h ^= h >> 15; h *= 0x2C1B3C6Du; h ^= h >> 12; h *= 0x297A2D39u; h ^= h >> 15;
+                    v0[(size_t)rr * VLD + cc] = __float2half((h & 1u) ? 1.f : -1.f);
+                }
+            CU_TRY(c, cudaMemcpyAsync((void*)(vec0 + (long long)S * 2 * ((long long)e.cap * VLD)), v0.data(), v0.size() * 2, cudaMemcpyHostToDevice, s));
+            CU_TRY(c, cudaStreamSynchronize(s));      // `v0` is a local
+        }
         if ((r = dmalloc(c, (void**)&c->d_maps, maps.size() * sizeof(CUtensorMap)))) return r;
         CU_TRY(c, cudaMemcpyAsync(c->d_maps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, s));
         CU_TRY(c, cudaStreamSynchronize(s));      // `maps` is a local
     }
     r = c->opt.precision == NOLSM_PREC_FP32 ? set_smem_limits<float>(c) : set_smem_limits<__half>(c);
     if (r) return r;
+    if (c->persist) {
+        PEngine& pe = c->peng;
+        pe = PEngine{};
+        if ((r = dmalloc(c, (void**)&pe.slots, sizeof(PSlot) * S))) return r;
+        if ((r = dmalloc(c, (void**)&pe.gclaim, 8 * S))) return r;
+        if ((r = dmalloc(c, (void**)&pe.sclaim, 4 * S))) return r;
+        if ((r = dmalloc(c, (void**)&pe.ctr, 8 * PC_LEN))) return r;
+        if ((r = dmalloc(c, (void**)&c->d_abort, 16))) return r;
+        pe.S = S; pe.cap = e.cap; pe.ld = e.ld; pe.bufsz = e.bufsz; pe.slotsz = e.slotsz;
+        pe.tol_inv = e.tol_inv; pe.tol_sign = e.tol_sign; pe.max_inv = e.max_inv; pe.max_sign = e.max_sign;
+        pe.p_s = e.p_s; pe.p_a = e.p_a; pe.safety_s = 1.05f; pe.safety_a = 1.05f;
+        pe.gather_rowatoms = g_rowatoms;
+        pe.schulz_chunks = std::max(1, getenv_int("NOLSM_SCHULZ_CHUNKS", 16));
+        pe.dcols_chunks = std::max(1, getenv_int("NOLSM_DCOLS_CHUNKS", 16));
+        pe.next_atom = e.next_atom; pe.finished = e.finished; pe.abort_flag = c->d_abort;
+        pe.at = e.at; pe.sv = sys_view(c);
+        pe.S_vals = c->dS; pe.H_vals = c->dH; pe.val_f64 = val_dtype == NOLSM_DTYPE_F64;
+        pe.e_atom = c->d_e_atom; pe.maps = c->d_maps; pe.base = (__half*)c->ws;
+        c->h_sclaim0.assign(S, ((unsigned)SK_REFILL << 28) | (1u << 14));
+        CU_TRY(c, cudaFuncSetAttribute(k_side_gather<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SIDE_SMEM));
+        CU_TRY(c, cudaFuncSetAttribute(k_side_gather<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SIDE_SMEM));
+    }
     CU_TRY(c, cudaStreamSynchronize(s));
     c->assembled = true;
     return NOLSM_OK;
@@ -616,6 +722,36 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
     CU_TRY(c, cudaStreamWaitEvent(s, c->ev_in, 0));
     CU_TRY(c, cudaMemsetAsync(D_dev + (size_t)v0 * ds, 0, (size_t)(v1 - v0) * ds, s));
     CU_TRY(c, cudaMemsetAsync(c->d_e_atom + a0, 0, 8 * (a1 - a0), s));
+    c->ev_used = 0; c->recs.clear(); c->launches = 0; c->prof_on = false;
+    c->last_persist = c->persist;
+    if (c->persist) {
+        // ---- persistent engine: one kernel launch evaluates the whole range ----
+        PEngine pe = c->peng;
+        pe.mu = (float)mu; pe.a_end = (int)a1; pe.total = (int)(a1 - a0);
+        pe.D_vals = D_dev; pe.d_f64 = d_dtype == NOLSM_DTYPE_F64;
+        c->h_a0 = (int)a0;
+        memset(c->h_ctr0, 0, sizeof(c->h_ctr0));
+        c->h_ctr0[PC_T_START] = ~0ull;
+        CU_TRY(c, cudaMemsetAsync(pe.slots, 0, sizeof(PSlot) * pe.S, s));
+        CU_TRY(c, cudaMemsetAsync(pe.gclaim, 0, 8 * pe.S, s));
+        CU_TRY(c, cudaMemcpyAsync(pe.sclaim, c->h_sclaim0.data(), 4 * pe.S, cudaMemcpyHostToDevice, s));
+        CU_TRY(c, cudaMemcpyAsync(pe.ctr, c->h_ctr0, 8 * PC_LEN, cudaMemcpyHostToDevice, s));
+        CU_TRY(c, cudaMemcpyAsync(pe.next_atom, &c->h_a0, 4, cudaMemcpyHostToDevice, s));
+        CU_TRY(c, cudaMemsetAsync(pe.finished, 0, 4, s));
+        CU_TRY(c, cudaMemsetAsync(c->d_abort, 0, 4, s));
+        CU_TRY(c, cudaEventRecord(c->ev_k0, s));
+        nolsm_persist_kernel<<<c->sms & ~1, P_THREADS, P_SMEM_BYTES, s>>>(pe);
+        CU_TRY(c, cudaGetLastError());
+        CU_TRY(c, cudaEventRecord(c->ev_k1, s));
+        c->launches = 1;
+        c->rounds = 0;
+        if (host_out) CU_TRY(c, cudaMemcpyAsync((char*)D_vals + (size_t)v0 * ds, c->d_D_stage, (size_t)(v1 - v0) * ds, cudaMemcpyDeviceToHost, s));
+        CU_TRY(c, cudaEventRecord(c->ev_out, s));
+        CU_TRY(c, cudaStreamWaitEvent(us, c->ev_out, 0));
+        c->last_stream = us; c->last_a0 = a0; c->last_a1 = a1; c->have_result = true;
+        if (e_partial_host) return nolsm_energy(c, e_partial_host);
+        return NOLSM_OK;
+    }
     Engine e = c->eng;
     e.mu = (float)mu;
     e.a_end = (int)a1;
@@ -627,7 +763,6 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
     CU_TRY(c, cudaMemsetAsync(e.prof, 0, sizeof(double) * PF_LEN, s));
     CU_TRY(c, cudaStreamSynchronize(s));       // a0i is a local; also makes *h_done = 0 below race-free
     *c->h_done = 0;
-    c->ev_used = 0; c->recs.clear(); c->launches = 0; c->prof_on = false;
     const bool fp32 = c->opt.precision == NOLSM_PREC_FP32;
 
     // ---- one round captured as a CUDA graph ----
@@ -690,7 +825,7 @@ int nolsm_energy(nolsm_ctx* c, double* e_elec) {
     if (!c || !e_elec) return NOLSM_EINVAL;
     if (!c->have_result) return fail(c, NOLSM_ESTATE, "no density matrix has been computed");
     cudaSetDevice(c->dev);
-    CU_TRY(c, cudaStreamSynchronize(c->last_stream));
+    if (int r = wait_result(c)) return r;
     const int64_t n = c->last_a1 - c->last_a0;
     std::vector<double> e(n);
     std::vector<int> st(n);
@@ -726,6 +861,29 @@ int nolsm_gather_submatrix(nolsm_ctx* c, int64_t atom, int which, int out_fp16, 
     cudaSetDevice(c->dev);
     const size_t es = out_fp16 ? 2 : 4;
     if ((size_t)c->eng.slotsz * es > c->ws_bytes) return fail(c, NOLSM_ENOMEM, "workspace too small for an FP32 gather");
+    if (c->persist && out_fp16) {
+        // the gather task of the persistent engine, launched stand-alone for slot 0
+        int* d_atom;
+        CU_TRY(c, cudaMalloc((void**)&d_atom, 4));
+        const int a32 = (int)atom;
+        CU_TRY(c, cudaMemcpy(d_atom, &a32, 4, cudaMemcpyHostToDevice));
+        const PEngine& pe = c->peng;
+        const int nset = (int)(c->nset_ptr[atom + 1] - c->nset_ptr[atom]);
+        dim3 grid((nset + pe.gather_rowatoms - 1) / pe.gather_rowatoms, 1);
+        if (c->val_dtype == NOLSM_DTYPE_F64)
+            k_side_gather<double><<<grid, P_SIDE_THREADS, P_SIDE_SMEM, c->s_main>>>(pe.sv, (const double*)c->dS, (const double*)c->dH, pe.base, pe.slotsz, pe.bufsz, pe.ld, d_atom, c->d_dim, nullptr);
+        else
+            k_side_gather<float><<<grid, P_SIDE_THREADS, P_SIDE_SMEM, c->s_main>>>(pe.sv, (const float*)c->dS, (const float*)c->dH, pe.base, pe.slotsz, pe.bufsz, pe.ld, d_atom, c->d_dim, nullptr);
+        cudaError_t ce = cudaGetLastError();
+        if (ce == cudaSuccess) ce = cudaStreamSynchronize(c->s_main);
+        const int n = c->dim[atom];
+        if (ce == cudaSuccess)
+            ce = cudaMemcpy2D(out_host, (size_t)n * 2, (const char*)c->ws + (size_t)which * pe.bufsz * 2, (size_t)pe.ld * 2,
+                              (size_t)n * 2, n, cudaMemcpyDeviceToHost);
+        cudaFree(d_atom);
+        if (ce != cudaSuccess) { c->err = cudaGetErrorString(ce); return NOLSM_ECUDA; }
+        return NOLSM_OK;
+    }
     // a one-slot view of the engine with the slot forced into phase NEW
     Engine e = c->eng;
     e.S = 1;
@@ -759,7 +917,7 @@ int nolsm_get_atom_stats(nolsm_ctx* c, int64_t a0, int64_t count, int32_t* dims,
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "not assembled");
     if (a0 < 0 || count < 0 || a0 + count > c->n_atoms) return fail(c, NOLSM_EINVAL, "range");
     cudaSetDevice(c->dev);
-    if (c->have_result) CU_TRY(c, cudaStreamSynchronize(c->last_stream));
+    if (c->have_result) { if (int r = wait_result(c)) return r; }
     if (dims) memcpy(dims, c->dim.data() + a0, 4 * count);
     if (inv_iters) CU_TRY(c, cudaMemcpy(inv_iters, c->eng.at.inv + a0, 4 * count, cudaMemcpyDeviceToHost));
     if (sign_iters) CU_TRY(c, cudaMemcpy(sign_iters, c->eng.at.sign + a0, 4 * count, cudaMemcpyDeviceToHost));
@@ -815,7 +973,24 @@ int nolsm_get_profile(nolsm_ctx* c, double* out, int n) {
     if (!c || !out || n < NOLSM_PROFILE_LEN) return NOLSM_EINVAL;
     if (!c->have_result) return fail(c, NOLSM_ESTATE, "no density matrix has been computed");
     cudaSetDevice(c->dev);
-    CU_TRY(c, cudaStreamSynchronize(c->last_stream));
+    if (int r = wait_result(c)) return r;
+    if (c->last_persist) {
+        // one launch: the kernel's duration from CUDA events on its stream; side-task times are summed
+        // over the side groups (SM-time, the tasks run concurrently with the GEMM pipeline)
+        unsigned long long ct[PC_LEN];
+        CU_TRY(c, cudaMemcpy(ct, c->peng.ctr, sizeof(ct), cudaMemcpyDeviceToHost));
+        float kms = 0;
+        CU_TRY(c, cudaEventElapsedTime(&kms, c->ev_k0, c->ev_k1));
+        nolsm_stats st;
+        if (int r = nolsm_get_stats(c, &st)) return r;
+        out[0] = ct[PC_SIDE_NS + SK_GATHER] * 1e-6; out[1] = (double)ct[PC_SIDE_TASKS + SK_GATHER]; out[2] = (double)ct[PC_SIDE_BYTES + SK_GATHER];
+        out[3] = kms; out[4] = 1; out[5] = st.flops_useful; out[6] = st.flops_padded;
+        out[7] = ct[PC_SIDE_NS + SK_DCOLS] * 1e-6; out[8] = (double)ct[PC_SIDE_TASKS + SK_DCOLS]; out[9] = (double)ct[PC_SIDE_BYTES + SK_DCOLS];
+        out[10] = (ct[PC_SIDE_NS + SK_REFILL] + ct[PC_SIDE_NS + SK_SCHULZ1]) * 1e-6;
+        out[11] = (double)(ct[PC_SIDE_TASKS + SK_REFILL] + ct[PC_SIDE_TASKS + SK_SCHULZ1]);
+        out[12] = (double)(c->last_a1 - c->last_a0); out[13] = 1;
+        return NOLSM_OK;
+    }
     double ms[4] = {0, 0, 0, 0}, cnt[4] = {0, 0, 0, 0};
     for (const nolsm_ctx::Rec& r : c->recs) {
         float t = 0;
@@ -830,6 +1005,28 @@ int nolsm_get_profile(nolsm_ctx* c, double* out, int n) {
     out[7] = ms[K_DCOLS]; out[8] = cnt[K_DCOLS]; out[9] = pf[PF_DCOLS_BYTES];
     out[10] = ms[K_OTHER]; out[11] = cnt[K_OTHER];
     out[12] = pf[PF_SUBMATS]; out[13] = (double)c->launches;
+    return NOLSM_OK;
+}
+
+int nolsm_get_engine_counters(nolsm_ctx* c, double* out, int n) {
+    if (!c || !out || n < NOLSM_COUNTERS_LEN) return NOLSM_EINVAL;
+    if (!c->have_result) return fail(c, NOLSM_ESTATE, "no density matrix has been computed");
+    for (int i = 0; i < NOLSM_COUNTERS_LEN; ++i) out[i] = 0;
+    if (!c->last_persist) return NOLSM_OK;
+    cudaSetDevice(c->dev);
+    if (int r = wait_result(c)) return r;
+    unsigned long long ct[PC_LEN];
+    CU_TRY(c, cudaMemcpy(ct, c->peng.ctr, sizeof(ct), cudaMemcpyDeviceToHost));
+    float kms = 0;
+    CU_TRY(c, cudaEventElapsedTime(&kms, c->ev_k0, c->ev_k1));
+    out[0] = 1; out[1] = kms; out[2] = (double)(ct[PC_T_END] - ct[PC_T_START]) * 1e-6;
+    out[3] = (double)ct[PC_TILES]; out[4] = ct[PC_SCHED_IDLE_NS] * 1e-6; out[5] = ct[PC_SCHED_BUSY_NS] * 1e-6;
+    out[6] = (double)ct[PC_OVERSHOOT]; out[7] = c->peng.S; out[8] = (c->sms & ~1) / 2;
+    for (int k = 0; k < 8; ++k) {
+        out[9 + k] = ct[PC_SIDE_NS + k] * 1e-6;
+        out[17 + k] = (double)ct[PC_SIDE_BYTES + k];
+        out[25 + k] = (double)ct[PC_SIDE_TASKS + k];
+    }
     return NOLSM_OK;
 }
 

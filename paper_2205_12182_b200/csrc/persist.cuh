@@ -1,0 +1,742 @@
+// Persistent engine: the whole hot path a1-a7 of one nolsm_density_matrix call in ONE kernel launch.
+//
+// grid = one CTA per SM in clusters of two (CTA pairs); every CTA runs
+//   warps 0-10   the grouped tcgen05 GEMM pipeline of gemm2sm.cuh (epilogue x 8, tile scheduler, TMA
+//                producer, MMA issuer), fed from a device-side claim table instead of a static tile list;
+//   warps 11-14  a SIDE GROUP that executes the O(n^2) steps of the path as small tasks: gather
+//                (PAPER.md:L56, L60), the closed-form first Schulz step, and D columns + scatter +
+//                energy (Eq. 4).
+// The spectral scalings (rho(S_sub) for the Schulz start, rho(A_sub) for X0 = A / rho, C-6)
+// come from a BLOCK power iteration with 16 vectors that runs as 256 x 16 GEMM tiles in the same
+// pipeline (V <- alpha M V, Frobenius norm of the product from the fused residual reduction).
+//
+// A slot (nolsm_device.cuh) holds one atom submatrix. At any time a slot has at most ONE live piece of
+// work: a GEMM op (claim word gclaim[slot] = tiles << 20 | next tile) or a side task (sclaim[slot] =
+// kind << 28 | chunks << 14 | next chunk). Tiles / chunks are claimed with one atomicAdd; the thread
+// that completes the last tile / chunk runs the slot's transition (convergence test, C-7) and
+// installs the next piece of work, or refills the slot with the next atom. Schedulers scan the claim
+// tables in slot order, so only as many slots as the GPU can keep busy are active at once and the
+// iterates of the active slots stay resident in L2 from one GEMM to the next. The host launches the
+// kernel once and waits.
+//
+// Cross-CTA data flow: GEMM outputs are written with generic stores and read back by TMA (async proxy)
+// of other CTAs: writers fence (fence.proxy.async, __threadfence) before the completing atomic; readers
+// fence.proxy.async after the claim. Slot state is read and written with .cg accesses (L1 is not
+// coherent across SMs).
+#pragma once
+#include "gemm2sm.cuh"
+#include "kernels.cuh"
+
+namespace nolsm {
+
+constexpr int P_SIDE_WARPS = 4;
+constexpr int P_SIDE_THREADS = P_SIDE_WARPS * 32;
+constexpr int P_THREADS = G2_CTRL_THREADS + P_SIDE_THREADS;
+constexpr int P_SIDE_SMEM = 60 * 1024;
+constexpr int P_SMEM_BYTES = G2_SMEM_BYTES + P_SIDE_SMEM;
+constexpr int P_MAX_CAP = 2048;
+constexpr int P_GATHER_ROWATOMS = 4;            // row-atoms of N(i) per gather chunk (at most)
+
+enum SideKind { SK_NONE = 0, SK_REFILL, SK_GATHER, SK_SCHULZ1, SK_DCOLS };
+
+// counters written by the kernel (unsigned long long each)
+enum { PC_TILES = 0, PC_SCHED_IDLE_NS, PC_SCHED_BUSY_NS, PC_OVERSHOOT, PC_T_START, PC_T_END,
+       PC_SIDE_NS,            // + kind
+       PC_SIDE_BYTES = PC_SIDE_NS + 8,   // + kind (algorithmic bytes)
+       PC_SIDE_TASKS = PC_SIDE_BYTES + 8,
+       PC_LEN = PC_SIDE_TASKS + 8 };
+
+struct __align__(16) PSlot {      // 160 bytes
+    int atom, n, n16, pos, nbi, ntm, ntn, nset;                     // geometry (written at refill)
+    int op_kind, a_buf, b_buf, c_buf;                               // live GEMM op: C = sgn alpha A B + beta I
+    float alpha, sgn, beta; int want_res;
+    int inv_iters, sign_iters, conv, xcur, ycur, status, gemm_count, tiles_done;
+    float res_acc, res_prev, res_last, rho_s, rho_a, alpha1, alpha2; int side_done;
+    int pow_step; float pow_norm2, pow_alpha, pow_est;              // block power iteration state
+    int pad[4];
+};
+
+struct PEngine {
+    PSlot* slots;
+    unsigned long long* gclaim;   // [S] GEMM claim words
+    unsigned int* sclaim;         // [S] side-task claim words
+    int S, cap, ld;
+    long long bufsz, slotsz;
+    float tol_inv, tol_sign, mu, safety_s, safety_a;
+    int max_inv, max_sign, p_s, p_a;
+    int gather_rowatoms, schulz_chunks, dcols_chunks;   // row-atoms of N(i) per gather chunk; chunks of the other tasks
+    int* next_atom; int a_end, total;
+    int* finished;
+    volatile int* abort_flag;     // device word; the host sets it (copy on another stream) to stop a kernel that overran its time limit
+    unsigned long long* ctr;      // [PC_LEN]
+    AtomArrays at;
+    SysView sv;
+    const void *S_vals, *H_vals; int val_f64;
+    void* D_vals; int d_f64;
+    double* e_atom;
+    const CUtensorMap* maps;
+    __half* base;
+};
+
+__device__ __forceinline__ long long buf_off(const PEngine& e, int slot, int buf) {
+    return (long long)slot * e.slotsz + (long long)buf * e.bufsz;
+}
+// Buffers 0..NBUF-1: the slot's square buffers (leading dimension ld). Buffers NBUF, NBUF+1: the slot's
+// two vector blocks (cap x VLD, the first NVC columns are used); they follow the S slots in the workspace.
+__device__ __forceinline__ __half* c_ptr(const PEngine& e, __half* base, int slot, int buf, int& ldc) {
+    if (buf < NBUF) { ldc = e.ld; return base + buf_off(e, slot, buf); }
+    ldc = VLD;
+    return base + (long long)e.S * e.slotsz + ((long long)slot * 2 + (buf - NBUF)) * ((long long)e.cap * VLD);
+}
+
+namespace pl {
+__device__ __forceinline__ unsigned long long gtime() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ void side_sync() { asm volatile("bar.sync 2, %0;" ::"n"(P_SIDE_THREADS) : "memory"); }
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ float dot8(const uint4& m, const float4& x0, const float4& x1) {
+    const __half2* h = reinterpret_cast<const __half2*>(&m);
+    const float2 a = __half22float2(h[0]), b = __half22float2(h[1]), c = __half22float2(h[2]), d = __half22float2(h[3]);
+    float s = a.x * x0.x;
+    s = fmaf(a.y, x0.y, s); s = fmaf(b.x, x0.z, s); s = fmaf(b.y, x0.w, s);
+    s = fmaf(c.x, x1.x, s); s = fmaf(c.y, x1.y, s); s = fmaf(d.x, x1.z, s); s = fmaf(d.y, x1.w, s);
+    return s;
+}
+}  // namespace pl
+
+// ------------------------------------------------------------------------------------------------
+// Installing work on a slot (one thread; the slot has no other live work at that moment).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void p_install_side(const PEngine& e, int slot, int kind, int chunks) {
+    __threadfence();
+    *(volatile unsigned int*)&e.sclaim[slot] = ((unsigned)kind << 28) | ((unsigned)chunks << 14);
+}
+
+__device__ __forceinline__ void p_install_gemm(const PEngine& e, int slot, int kind) {
+    PSlot* s = &e.slots[slot];
+    const int xcur = __ldcg(&s->xcur), ycur = __ldcg(&s->ycur);
+    const bool first = __ldcg(&s->sign_iters) == 0;
+    int a = 0, b = 0, c = 0, want = 0;
+    float alpha = 1.f, sgn = 1.f, beta = 0.f;
+    switch (kind) {
+        case OP_INV_G1: a = 0; b = ycur; c = 4; sgn = -1.f; beta = 2.f; want = 1; break;          // R = 2I - S Y
+        case OP_INV_G2: a = ycur; b = 4; c = 5 - ycur; break;                                       // Y <- Y R
+        case OP_AMAT: a = ycur; b = 1; c = 0; beta = -e.mu; break;                                  // A = Y H0 - mu I
+        case OP_SIGN_G1: a = xcur; b = xcur; c = 4; alpha = first ? __ldcg(&s->alpha1) : 1.f; sgn = -1.f; beta = 3.f; want = 1; break;
+        case OP_SIGN_G2: a = xcur; b = 4; c = 1 - xcur; alpha = first ? __ldcg(&s->alpha2) : 0.5f; break;
+        case OP_POW_S:
+        case OP_POW_A: {                                                                            // V <- alpha M V
+            const int st = __ldcg(&s->pow_step);
+            a = 0; b = st == 0 ? NMAP - 1 : NBUF + ((st - 1) & 1); c = NBUF + (st & 1);
+            alpha = __ldcg(&s->pow_alpha); want = 1;
+        } break;
+        default: break;
+    }
+    __stcg(reinterpret_cast<int4*>(&s->op_kind), make_int4(kind, a, b, c));
+    __stcg(reinterpret_cast<float4*>(&s->alpha), make_float4(alpha, sgn, beta, __int_as_float(want)));
+    const bool pow = kind == OP_POW_S || kind == OP_POW_A;
+    const unsigned long long tiles = (unsigned long long)(__ldcg(&s->ntm) * (pow ? 1 : __ldcg(&s->ntn)));
+    __threadfence();
+    *(volatile unsigned long long*)&e.gclaim[slot] = tiles << 20;
+}
+
+// Starts the block power iteration on buffer 0 (S_sub or A_sub): V0 = the shared +-1 start block.
+__device__ __forceinline__ void p_start_power(const PEngine& e, int slot, int kind) {
+    PSlot* s = &e.slots[slot];
+    __stcg(&s->pow_step, 0);
+    __stcg(&s->pow_norm2, (float)NVC * (float)__ldcg(&s->n));
+    __stcg(&s->pow_alpha, 1.f);
+    p_install_gemm(e, slot, kind);
+}
+
+// Takes the next atom of the feed into the slot and installs its gather (phase NEW). Returns false when
+// the feed is exhausted (the slot stays free).
+__device__ __forceinline__ bool p_refill(const PEngine& e, int slot) {
+    if (*(volatile int*)e.next_atom >= e.a_end) return false;
+    const int a = atomicAdd(e.next_atom, 1);
+    if (a >= e.a_end) return false;
+    PSlot* s = &e.slots[slot];
+    const int n = e.at.dim[a], n16 = (n + 15) & ~15;
+    int ntm, ntn;
+    choose_tiling(n16, ntm, ntn);
+    const int nset = (int)(e.sv.nset_ptr[a + 1] - e.sv.nset_ptr[a]);
+    __stcg(reinterpret_cast<int4*>(&s->atom), make_int4(a, n, n16, e.at.pos[a]));
+    __stcg(reinterpret_cast<int4*>(&s->nbi), make_int4(e.at.nb[a], ntm, ntn, nset));
+    __stcg(reinterpret_cast<int4*>(&s->inv_iters), make_int4(0, 0, 0, 0));            // inv, sign, conv, xcur
+    __stcg(reinterpret_cast<int4*>(&s->ycur), make_int4(2, 0, 0, 0));                 // ycur, status, gemm_count, tiles_done
+    __stcg(reinterpret_cast<float4*>(&s->res_acc), make_float4(0.f, 1e30f, 0.f, 0.f)); // res_acc, res_prev, res_last, rho_s
+    __stcg(reinterpret_cast<float4*>(&s->rho_a), make_float4(0.f, 1.f, 0.5f, 0.f));    // rho_a, alpha1, alpha2, side_done
+    p_install_side(e, slot, SK_GATHER, (nset + e.gather_rowatoms - 1) / e.gather_rowatoms);
+    return true;
+}
+
+// Phase FIN finished (or skipped for a failed inverse): publish the atom's results, free / refill the slot.
+__device__ __forceinline__ void p_retire(const PEngine& e, int slot) {
+    PSlot* s = &e.slots[slot];
+    const int a = __ldcg(&s->atom);
+    e.at.inv[a] = __ldcg(&s->inv_iters); e.at.sign[a] = __ldcg(&s->sign_iters); e.at.status[a] = __ldcg(&s->status);
+    e.at.gemms[a] = __ldcg(&s->gemm_count); e.at.res[a] = __ldcg(&s->res_last); e.at.rho[a] = __ldcg(&s->rho_a);
+    const bool more = p_refill(e, slot);
+    if (!more) *(volatile unsigned int*)&e.sclaim[slot] = 0u;
+    __threadfence();
+    atomicAdd(e.finished, 1);
+}
+
+// ------------------------------------------------------------------------------------------------
+// GEMM side: called by one thread per CTA per finished tile (after the CTA's stores and residual
+// atomics). The last report of the op runs the slot's transition (same rules as tile_finished of the
+// round engine: DESIGN.md C-7) and installs what comes next.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int nreports) {
+    PSlot* s = &e.slots[slot];
+    __threadfence();
+    const int prev = atomicAdd(&s->tiles_done, 1);
+    if (prev != nreports - 1) return;
+    __threadfence();
+    __stcg(&s->tiles_done, 0);
+    const int kind = __ldcg(&s->op_kind);
+    if (kind == OP_POW_S || kind == OP_POW_A) {
+        // ||alpha M V_k||_F^2 from the fused reduction; rho estimate = growth of the Frobenius norm
+        const float r_new = atomicExch(&s->res_acc, 0.0f);
+        const float alpha = __ldcg(&s->pow_alpha);
+        float est = sqrtf(r_new / __ldcg(&s->pow_norm2)) / alpha;
+        if (!(est > 1e-20f) || !(est < 1e20f)) est = 1.f;
+        const int step = __ldcg(&s->pow_step) + 1;
+        const int P = kind == OP_POW_S ? e.p_s : e.p_a;
+        if (step < P) {
+            __stcg(&s->pow_step, step);
+            __stcg(&s->pow_norm2, r_new);
+            __stcg(&s->pow_alpha, 1.f / est);                         // keeps ||V_k||_F at its starting magnitude
+            p_install_gemm(e, slot, kind);
+        } else if (kind == OP_POW_S) {
+            __stcg(&s->rho_s, e.safety_s * est);
+            p_install_side(e, slot, SK_SCHULZ1, e.schulz_chunks);
+        } else {
+            const float rho = e.safety_a * est;
+            __stcg(&s->rho_a, rho);
+            __stcg(&s->alpha1, 1.f / (rho * rho));
+            __stcg(&s->alpha2, 0.5f / rho);
+            p_install_gemm(e, slot, OP_SIGN_G1);
+        }
+        return;
+    }
+    __stcg(&s->gemm_count, __ldcg(&s->gemm_count) + 1);
+    if (kind == OP_INV_G1 || kind == OP_SIGN_G1) {
+        const bool inv = kind == OP_INV_G1;
+        const float sum = atomicExch(&s->res_acc, 0.0f);
+        const float r = sqrtf(sum / (float)__ldcg(&s->n));
+        const float rp = __ldcg(&s->res_prev);
+        __stcg(&s->res_prev, r);
+        __stcg(&s->res_last, r);
+        const float tol = inv ? e.tol_inv : e.tol_sign;
+        const int iters = inv ? __ldcg(&s->inv_iters) : __ldcg(&s->sign_iters);
+        const int cap = inv ? e.max_inv : e.max_sign;
+        const bool ok = r < tol;
+        const bool stagnated = (r > 0.5f * rp) && (r < 4.f * tol) && iters > 0;   // rounding floor reached
+        const bool diverged = !(r == r) || (iters > 1 && r > rp && r > 0.9f);
+        const bool capped = iters + 1 >= cap;
+        if (diverged || (capped && !ok && !stagnated)) __stcg(&s->status, __ldcg(&s->status) | (inv ? ST_NOTSPD : ST_NOCONV));
+        __stcg(&s->conv, (ok || stagnated || diverged || capped) ? 1 : 0);
+        p_install_gemm(e, slot, inv ? OP_INV_G2 : OP_SIGN_G2);
+    } else if (kind == OP_INV_G2) {
+        __stcg(&s->inv_iters, __ldcg(&s->inv_iters) + 1);
+        __stcg(&s->ycur, 5 - __ldcg(&s->ycur));
+        if (__ldcg(&s->conv)) {
+            __stcg(&s->conv, 0);
+            __stcg(&s->res_prev, 1e30f);
+            if (__ldcg(&s->status) & ST_NOTSPD) p_retire(e, slot);      // no D for this atom (rows stay zero)
+            else p_install_gemm(e, slot, OP_AMAT);
+        } else {
+            p_install_gemm(e, slot, OP_INV_G1);
+        }
+    } else if (kind == OP_AMAT) {
+        p_start_power(e, slot, OP_POW_A);
+    } else if (kind == OP_SIGN_G2) {
+        __stcg(&s->sign_iters, __ldcg(&s->sign_iters) + 1);
+        __stcg(&s->xcur, 1 - __ldcg(&s->xcur));
+        if (__ldcg(&s->conv)) {
+            __stcg(&s->conv, 0);
+            p_install_side(e, slot, SK_DCOLS, e.dcols_chunks);
+        } else {
+            p_install_gemm(e, slot, OP_SIGN_G1);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Tile scheduler of the persistent engine (leader CTA, one warp): claims tiles from gclaim[] in slot
+// order and publishes them to both CTAs of the pair.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, int lane) {
+    int q = 0; uint32_t ph = 0;
+    unsigned long long idle_ns = 0, ntiles = 0, overshoot = 0;
+    const unsigned long long t_begin = pl::gtime();
+    for (;;) {
+        for (uint32_t spins = 0; !ptx::mbar_try_wait_cluster(sm.ti_empty(q), ph ^ 1);) {
+            __nanosleep(100);
+            if (++spins > (1u << 26)) __trap();
+        }
+        TileInfo ti{};
+        int got = 0;
+        unsigned long long t_idle0 = 0;
+        for (;;) {
+            int found = -1;
+            for (int base = 0; base < e.S; base += 32) {
+                const int sidx = base + lane;
+                const unsigned long long w = sidx < e.S ? *(volatile unsigned long long*)&e.gclaim[sidx] : 0ull;
+                const bool avail = (unsigned)(w & 0xFFFFFu) < (unsigned)((w >> 20) & 0xFFFFFu);
+                const unsigned m = __ballot_sync(0xffffffffu, avail);
+                if (m) { found = base + __ffs(m) - 1; break; }
+            }
+            if (found >= 0) {
+                unsigned long long w = 0;
+                if (lane == 0) w = atomicAdd(&e.gclaim[found], 1ull);
+                w = __shfl_sync(0xffffffffu, w, 0);
+                const int t = (int)(w & 0xFFFFFu), nt = (int)((w >> 20) & 0xFFFFFu);
+                if (t < nt) {
+                    if (lane == 0) {
+                        __threadfence();
+                        const PSlot* s = &e.slots[found];
+                        const int4 g0 = __ldcg(reinterpret_cast<const int4*>(&s->atom));     // atom n n16 pos
+                        const int4 g1 = __ldcg(reinterpret_cast<const int4*>(&s->nbi));      // nbi ntm ntn nset
+                        const int4 o0 = __ldcg(reinterpret_cast<const int4*>(&s->op_kind));
+                        const float4 o1 = __ldcg(reinterpret_cast<const float4*>(&s->alpha));
+                        const bool pow = o0.x == OP_POW_S || o0.x == OP_POW_A;
+                        const int ntn = pow ? 1 : g1.z;
+                        const int tm = t / ntn, tn = t - tm * ntn;
+                        ti.slot = found; ti.m0 = tm * BM; ti.n0 = tn * BN;
+                        ti.n = g0.y; ti.n16 = g0.z; ti.bn = pow ? NVC : min(BN, g0.z - tn * BN); ti.nreports = 2 * nt;
+                        ti.kind = o0.x; ti.a_buf = o0.y; ti.b_buf = o0.z; ti.c_buf = o0.w;
+                        ti.alpha = o1.x; ti.sgn = o1.y; ti.beta = o1.z; ti.want_res = __float_as_int(o1.w);
+                    }
+                    got = 1;
+                    break;
+                }
+                ++overshoot;
+                continue;
+            }
+            if (*(volatile int*)e.finished >= e.total || *e.abort_flag) break;
+            if (!t_idle0) t_idle0 = pl::gtime();
+            __nanosleep(200);
+        }
+        if (t_idle0) idle_ns += pl::gtime() - t_idle0;
+        ntiles += got;
+        if (lane == 0) ti.valid = got;
+        const uint32_t* w = reinterpret_cast<const uint32_t*>(&ti);
+        uint32_t mine = 0;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const uint32_t v = __shfl_sync(0xffffffffu, w[i], 0);
+            if (lane == i) mine = v;
+        }
+        if (lane < 16) {
+            asm volatile("st.shared.u32 [%0], %1;" ::"r"(sm.tinfo(q) + 4u * lane), "r"(mine) : "memory");
+            ptx::st_cluster_u32(ptx::mapa(sm.tinfo(q), 1) + 4u * lane, mine);
+        }
+        __syncwarp();
+        if (lane == 0) {
+            ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_full(q), 0));
+            ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_full(q), 1));
+        }
+        if (!got) break;
+        if (++q == G2_NTI) { q = 0; ph ^= 1; }
+    }
+    if (lane == 0) {
+        const unsigned long long t_end = pl::gtime();
+        atomicAdd(&e.ctr[PC_TILES], ntiles);
+        atomicAdd(&e.ctr[PC_SCHED_IDLE_NS], idle_ns);
+        atomicAdd(&e.ctr[PC_SCHED_BUSY_NS], t_end - t_begin - idle_ns);
+        atomicAdd(&e.ctr[PC_OVERSHOOT], overshoot);
+        atomicMin(&e.ctr[PC_T_START], t_begin);
+        atomicMax(&e.ctr[PC_T_END], t_end);
+    }
+}
+
+// ================================================================================================
+// Side tasks. `tid` in [0, P_SIDE_THREADS); `sm` is the side group's shared memory (P_SIDE_SMEM bytes).
+// One side group is four warps on an SM that is busy with GEMM tiles, so every loop is written for
+// memory-level parallelism: several independent loads are issued before the first one is used.
+// ================================================================================================
+
+// a1, one chunk of row-atoms of N(i): builds the dense rows of T_i(S) (buffer 0) and T_i(H0) (buffer 1)
+// that belong to row-atoms [a_lo, a_hi) of N(i): block (j_a, j_b) of the sparse matrix where it exists,
+// zeros elsewhere and in the pad strip [n, n16). The last chunk also zeroes rows [n, n16).
+template <typename TV>
+__device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_vals, const TV* __restrict__ H_vals,
+                                  __half* __restrict__ dstS, __half* __restrict__ dstH, int atom, int n, int n16, int ld,
+                                  int chunk, int nchunks, unsigned char* sm, int tid, unsigned long long* bytes) {
+    const long long p0 = sv.nset_ptr[atom];
+    const int cnt = (int)(sv.nset_ptr[atom + 1] - p0);
+    int* s_nset = reinterpret_cast<int*>(sm);                              // [cnt] atoms of N(i)
+    int* s_off = s_nset + cnt;                                             // [cnt + 1] first column of each atom
+    long long* s_boff = reinterpret_cast<long long*>(sm + (((size_t)(2 * cnt + 1) * 4 + 7) & ~(size_t)7));   // [rows of the chunk][cnt]
+    const int a_lo = (int)((long long)cnt * chunk / nchunks), a_hi = (int)((long long)cnt * (chunk + 1) / nchunks);
+    const int na = a_hi - a_lo;
+    unsigned short* s_colmap = reinterpret_cast<unsigned short*>(s_boff + (size_t)max(na, 1) * cnt);        // [n16]
+    for (int b = tid; b < cnt; b += P_SIDE_THREADS) {
+        const int k = sv.nset_atom[p0 + b], o = sv.nset_off[p0 + b];
+        s_nset[b] = k; s_off[b] = o;
+        const int nbb = sv.atom_nb[k];
+        for (int c = 0; c < nbb; ++c) s_colmap[o + c] = (unsigned short)b;
+    }
+    if (tid == 0) s_off[cnt] = n;
+    for (int c = n + tid; c < n16; c += P_SIDE_THREADS) s_colmap[c] = 0xFFFF;
+    for (int q = tid; q < na * cnt; q += P_SIDE_THREADS) s_boff[q] = -1;
+    pl::side_sync();
+    // CSR rows of the chunk's row-atoms against N(i) (both ascending): every entry looks itself up in N(i)
+    for (int al = 0; al < na; ++al) {
+        const int j = s_nset[a_lo + al];
+        const long long r0 = sv.row_ptr[j], r1 = sv.row_ptr[j + 1];
+        for (long long p = r0 + tid; p < r1; p += P_SIDE_THREADS) {
+            const int k = sv.col_idx[p];
+            int lo = 0, hi = cnt;
+            while (lo < hi) { const int mid = (lo + hi) >> 1; if (s_nset[mid] < k) lo = mid + 1; else hi = mid; }
+            if (lo < cnt && s_nset[lo] == k) s_boff[al * cnt + lo] = sv.blk_off[p];
+        }
+    }
+    pl::side_sync();
+    unsigned long long nread = 0;
+    const int half_n16 = n16 >> 1;
+    constexpr int U = 4;                                                   // column pairs in flight per thread
+    for (int al = 0; al < na; ++al) {
+        const int a = a_lo + al;
+        const int nbj = s_off[a + 1] - s_off[a], row0 = s_off[a];
+        const int total = nbj * half_n16;                                  // column pairs of this row strip
+        const long long* boff = s_boff + al * cnt;
+#pragma unroll 1
+        for (int which = 0; which < 2; ++which) {
+            const TV* __restrict__ vals = which ? H_vals : S_vals;
+            __half* __restrict__ dst = which ? dstH : dstS;
+#pragma unroll 1
+            for (int idx0 = tid; idx0 < total; idx0 += U * P_SIDE_THREADS) {
+                TV v[2 * U];
+                long long o[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const int idx = idx0 + u * P_SIDE_THREADS;
+                    v[2 * u] = (TV)0; v[2 * u + 1] = (TV)0; o[u] = -1;
+                    if (idx < total) {
+                        const int rr = idx / half_n16;
+                        const int c = (idx - rr * half_n16) << 1;
+                        o[u] = (long long)(row0 + rr) * ld + c;
+                        const unsigned b0 = s_colmap[c], b1 = s_colmap[c + 1];
+                        if (b0 != 0xFFFFu) {
+                            const long long bo = boff[b0];
+                            if (bo >= 0) { v[2 * u] = __ldg(vals + bo + (long long)rr * (s_off[b0 + 1] - s_off[b0]) + (c - s_off[b0])); ++nread; }
+                        }
+                        if (b1 != 0xFFFFu) {
+                            const long long bo = boff[b1];
+                            if (bo >= 0) { v[2 * u + 1] = __ldg(vals + bo + (long long)rr * (s_off[b1 + 1] - s_off[b1]) + (c + 1 - s_off[b1])); ++nread; }
+                        }
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < U; ++u)
+                    if (o[u] >= 0)
+                        *reinterpret_cast<__half2*>(dst + o[u]) = __halves2half2(Num<__half>::from_d((double)v[2 * u]), Num<__half>::from_d((double)v[2 * u + 1]));
+            }
+        }
+    }
+    if (chunk == nchunks - 1) {
+        const __half2 z = __floats2half2_rn(0.f, 0.f);
+        for (int idx = tid; idx < (n16 - n) * half_n16; idx += P_SIDE_THREADS) {
+            const int rr = idx / half_n16, c = (idx - rr * half_n16) << 1;
+            *reinterpret_cast<__half2*>(dstS + (long long)(n + rr) * ld + c) = z;
+            *reinterpret_cast<__half2*>(dstH + (long long)(n + rr) * ld + c) = z;
+        }
+    }
+    if (bytes) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) nread += __shfl_xor_sync(0xffffffffu, nread, o);
+        if ((tid & 31) == 0 && nread) atomicAdd(bytes, nread * sizeof(TV));                          // source values read
+        if (tid == 0) atomicAdd(bytes, (unsigned long long)(s_off[a_hi] - s_off[a_lo]) * n16 * 4ull); // dense FP16 rows written (S and H0)
+    }
+}
+
+// First Schulz step in closed form, rows [r_lo, r_hi) of n16: Y1 = (2/rho) I - S / rho^2 inside
+// [0, n)^2, zero in the pad strip (C-8).
+__device__ void side_schulz1_chunk(const __half* __restrict__ S, __half* __restrict__ Y, int n, int n16, int ld, float rho,
+                                   int chunk, int nchunks, int tid) {
+    const int r_lo = (int)((long long)n16 * chunk / nchunks), r_hi = (int)((long long)n16 * (chunk + 1) / nchunks);
+    const float d = 2.f / rho, sc = 1.f / (rho * rho);
+    const int ppr = n16 >> 3;
+    const int total = (r_hi - r_lo) * ppr;
+    constexpr int U = 8;
+#pragma unroll 1
+    for (int idx0 = tid; idx0 < total; idx0 += U * P_SIDE_THREADS) {
+        uint4 u[U];
+#pragma unroll
+        for (int q = 0; q < U; ++q) {
+            const int idx = idx0 + q * P_SIDE_THREADS;
+            if (idx < total) {
+                const int rl = idx / ppr, p = idx - rl * ppr;
+                u[q] = __ldcg(reinterpret_cast<const uint4*>(S + (long long)(r_lo + rl) * ld + p * 8));
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < U; ++q) {
+            const int idx = idx0 + q * P_SIDE_THREADS;
+            if (idx < total) {
+                const int rl = idx / ppr, p = idx - rl * ppr;
+                const int r = r_lo + rl, c0 = p * 8;
+                const __half2* h = reinterpret_cast<const __half2*>(&u[q]);
+                float f[8];
+#pragma unroll
+                for (int w = 0; w < 4; ++w) { const float2 t = __half22float2(h[w]); f[2 * w] = t.x; f[2 * w + 1] = t.y; }
+#pragma unroll
+                for (int w = 0; w < 8; ++w) {
+                    const int c = c0 + w;
+                    f[w] = (r < n && c < n) ? ((r == c ? d : 0.f) - sc * f[w]) : 0.f;
+                }
+                st_half8(Y + (long long)r * ld + c0, f);
+            }
+        }
+    }
+}
+
+// a6 + a7, rows [r_lo, r_hi) of the submatrix: D_sub[r, cols(i)] = 1/2 (Y[r, cols] - X[r, :] Y[:, cols]),
+// written to slot (i, j) of the output as (D_ji)^T, and the energy partial sum_j <D_ji, H0_ji> in FP64.
+template <typename TV, typename TD>
+__device__ void side_dcols_chunk(const SysView& sv, const __half* __restrict__ X, const __half* __restrict__ Y,
+                                 const TV* __restrict__ H_vals, TD* __restrict__ D_vals, double* e_atom,
+                                 int atom, int n, int n16, int ld, int pos, int nbi, int chunk, int nchunks, unsigned char* sm, int tid) {
+    const long long p0 = sv.nset_ptr[atom];
+    const int cnt = (int)(sv.nset_ptr[atom + 1] - p0);
+    int* s_off = reinterpret_cast<int*>(sm);                               // [cnt + 1]
+    __half* yt = reinterpret_cast<__half*>(sm + (((size_t)(cnt + 1) * 4 + 15) & ~(size_t)15));   // [nbi][n16]: Y[:, cols]^T
+    for (int b = tid; b < cnt; b += P_SIDE_THREADS) s_off[b] = sv.nset_off[p0 + b];
+    if (tid == 0) s_off[cnt] = n;
+    const unsigned short* Yu = reinterpret_cast<const unsigned short*>(Y);
+    unsigned short* ytu = reinterpret_cast<unsigned short*>(yt);
+    {
+        constexpr int U = 8;
+        const int total = n16 * nbi;
+#pragma unroll 1
+        for (int idx0 = tid; idx0 < total; idx0 += U * P_SIDE_THREADS) {
+            unsigned short v[U];
+#pragma unroll
+            for (int q = 0; q < U; ++q) {
+                const int idx = idx0 + q * P_SIDE_THREADS;
+                v[q] = 0;
+                if (idx < total) {
+                    const int k = idx / nbi, c = idx - k * nbi;
+                    if (k < n) v[q] = __ldcg(Yu + (long long)k * ld + pos + c);
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < U; ++q) {
+                const int idx = idx0 + q * P_SIDE_THREADS;
+                if (idx < total) { const int k = idx / nbi, c = idx - k * nbi; ytu[c * n16 + k] = v[q]; }
+            }
+        }
+    }
+    pl::side_sync();
+    const int warp = tid >> 5, lane = tid & 31;
+    const int r_lo = (int)((long long)n * chunk / nchunks), r_hi = (int)((long long)n * (chunk + 1) / nchunks);
+    const int ppr = n16 >> 3;
+    double e_part = 0.0;
+    constexpr int XP = P_MAX_CAP / 8 / 32;                                 // 16-byte pieces of an X row per lane (at most)
+    for (int r = r_lo + warp; r < r_hi; r += P_SIDE_WARPS) {
+        const __half* xrow = X + (long long)r * ld;
+        uint4 xr[XP];
+#pragma unroll
+        for (int q = 0; q < XP; ++q) {
+            const int p = lane + 32 * q;
+            xr[q] = p < ppr ? __ldcg(reinterpret_cast<const uint4*>(xrow + p * 8)) : make_uint4(0, 0, 0, 0);
+        }
+        int lo = 0, hi = cnt - 1;                                          // atom of N(i) that owns row r
+        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_off[mid] <= r) lo = mid; else hi = mid - 1; }
+        const int a = lo, bb = r - s_off[a], nbj = s_off[a + 1] - s_off[a];
+        const long long out0 = sv.blk_off[sv.nset_slot[p0 + a]];
+        for (int c0 = 0; c0 < nbi; c0 += 16) {
+            const int nc = min(16, nbi - c0);
+            float acc[16];
+#pragma unroll
+            for (int c = 0; c < 16; ++c) acc[c] = 0.f;
+#pragma unroll
+            for (int q = 0; q < XP; ++q) {
+                const int p = lane + 32 * q;
+                if (p < ppr) {
+                    const __half2* xh = reinterpret_cast<const __half2*>(&xr[q]);
+                    const float2 x01 = __half22float2(xh[0]), x23 = __half22float2(xh[1]), x45 = __half22float2(xh[2]), x67 = __half22float2(xh[3]);
+                    const float4 xa = make_float4(x01.x, x01.y, x23.x, x23.y), xb = make_float4(x45.x, x45.y, x67.x, x67.y);
+#pragma unroll
+                    for (int c = 0; c < 16; ++c)
+                        if (c < nc) {
+                            const uint4 yu = *reinterpret_cast<const uint4*>(yt + (size_t)(c0 + c) * n16 + p * 8);
+                            acc[c] += pl::dot8(yu, xa, xb);
+                        }
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < 16; ++c)
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], o);
+            float mine = 0.f;
+#pragma unroll
+            for (int c = 0; c < 16; ++c) if (lane == c) mine = acc[c];
+            if (lane < nc) {
+                const int c = c0 + lane;
+                const float d = 0.5f * (__half2float(yt[(size_t)c * n16 + r]) - mine);
+                const long long o = out0 + (long long)c * nbj + bb;        // slot (i, j_a): [c][bb] = D_sub[r, pos + c]
+                D_vals[o] = (TD)d;
+                e_part += (double)d * (double)H_vals[o];
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) e_part += __shfl_xor_sync(0xffffffffu, e_part, o);
+    if (lane == 0 && e_part != 0.0) atomicAdd(&e_atom[atom], e_part);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Side group main loop.
+// ------------------------------------------------------------------------------------------------
+__device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
+    __shared__ int s_ctl[4];                      // slot, kind, chunk, nchunks
+    const int warp = tid >> 5, lane = tid & 31;
+    unsigned long long busy_ns[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tasks[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (;;) {
+        if (warp == 0) {
+            int slot = -1, kind = -1, chunk = 0, nch = 0;
+            for (;;) {
+                int found = -1;
+                for (int base = 0; base < e.S; base += 32) {
+                    const int sidx = base + lane;
+                    const unsigned w = sidx < e.S ? *(volatile unsigned int*)&e.sclaim[sidx] : 0u;
+                    const bool avail = (w & 0x3FFFu) < ((w >> 14) & 0x3FFFu);
+                    const unsigned m = __ballot_sync(0xffffffffu, avail);
+                    if (m) { found = base + __ffs(m) - 1; break; }
+                }
+                if (found >= 0) {
+                    unsigned w = 0;
+                    if (lane == 0) w = atomicAdd(&e.sclaim[found], 1u);
+                    w = __shfl_sync(0xffffffffu, w, 0);
+                    const int c = (int)(w & 0x3FFFu), n = (int)((w >> 14) & 0x3FFFu);
+                    if (c < n) { slot = found; kind = (int)(w >> 28); chunk = c; nch = n; break; }
+                    continue;
+                }
+                if (*(volatile int*)e.finished >= e.total || *e.abort_flag) break;
+                __nanosleep(500);
+            }
+            if (lane == 0) { s_ctl[0] = slot; s_ctl[1] = kind; s_ctl[2] = chunk; s_ctl[3] = nch; }
+        }
+        pl::side_sync();
+        const int slot = s_ctl[0], kind = s_ctl[1], chunk = s_ctl[2], nch = s_ctl[3];
+        if (kind < 0) break;
+        __threadfence();
+        const unsigned long long t0 = pl::gtime();
+        PSlot* s = &e.slots[slot];
+        const int4 g0 = __ldcg(reinterpret_cast<const int4*>(&s->atom));     // atom n n16 pos
+        const int4 g1 = __ldcg(reinterpret_cast<const int4*>(&s->nbi));      // nbi ntm ntn nset
+        const int atom = g0.x, n = g0.y, n16 = g0.z, pos = g0.w, nbi = g1.x;
+        switch (kind) {
+            case SK_GATHER: {
+                __half* dS = e.base + buf_off(e, slot, 0);
+                __half* dH = e.base + buf_off(e, slot, 1);
+                if (e.val_f64) side_gather_chunk<double>(e.sv, (const double*)e.S_vals, (const double*)e.H_vals, dS, dH, atom, n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER]);
+                else side_gather_chunk<float>(e.sv, (const float*)e.S_vals, (const float*)e.H_vals, dS, dH, atom, n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER]);
+            } break;
+            case SK_SCHULZ1:
+                side_schulz1_chunk(e.base + buf_off(e, slot, 0), e.base + buf_off(e, slot, 2), n, n16, e.ld, __ldcg(&s->rho_s), chunk, nch, tid);
+                break;
+            case SK_DCOLS: {
+                const __half* X = e.base + buf_off(e, slot, __ldcg(&s->xcur));
+                const __half* Y = e.base + buf_off(e, slot, __ldcg(&s->ycur));
+                if (e.val_f64) {
+                    if (e.d_f64) side_dcols_chunk<double, double>(e.sv, X, Y, (const double*)e.H_vals, (double*)e.D_vals, e.e_atom, atom, n, n16, e.ld, pos, nbi, chunk, nch, sm, tid);
+                    else side_dcols_chunk<double, float>(e.sv, X, Y, (const double*)e.H_vals, (float*)e.D_vals, e.e_atom, atom, n, n16, e.ld, pos, nbi, chunk, nch, sm, tid);
+                } else {
+                    if (e.d_f64) side_dcols_chunk<float, double>(e.sv, X, Y, (const float*)e.H_vals, (double*)e.D_vals, e.e_atom, atom, n, n16, e.ld, pos, nbi, chunk, nch, sm, tid);
+                    else side_dcols_chunk<float, float>(e.sv, X, Y, (const float*)e.H_vals, (float*)e.D_vals, e.e_atom, atom, n, n16, e.ld, pos, nbi, chunk, nch, sm, tid);
+                }
+            } break;
+            default: break;                       // SK_REFILL: nothing to compute
+        }
+        ptx::fence_proxy_async();                 // buffers written here are read next by TMA
+        pl::side_sync();
+        if (tid == 0) {
+            busy_ns[kind & 7] += pl::gtime() - t0;
+            tasks[kind & 7] += 1;
+            __threadfence();
+            const int prev = nch > 1 ? atomicAdd(&s->side_done, 1) : 0;
+            if (prev == nch - 1) {
+                __threadfence();
+                if (nch > 1) __stcg(&s->side_done, 0);
+                switch (kind) {
+                    case SK_REFILL:
+                        if (!p_refill(e, slot)) *(volatile unsigned int*)&e.sclaim[slot] = 0u;
+                        break;
+                    case SK_GATHER: p_start_power(e, slot, OP_POW_S); break;
+                    case SK_SCHULZ1:
+                        __stcg(&s->inv_iters, 1);
+                        __stcg(&s->ycur, 2);
+                        p_install_gemm(e, slot, OP_INV_G1);
+                        break;
+                    case SK_DCOLS: {
+                        const double nv = (double)(e.sv.blk_off[e.sv.row_ptr[atom + 1]] - e.sv.blk_off[e.sv.row_ptr[atom]]);
+                        atomicAdd(&e.ctr[PC_SIDE_BYTES + SK_DCOLS],
+                                  (unsigned long long)(nv * ((e.d_f64 ? 8 : 4) + (e.val_f64 ? 8 : 4)) + ((double)n * n + (double)n * nbi) * 2.0));
+                        p_retire(e, slot);
+                    } break;
+                    default: break;
+                }
+            }
+        }
+    }
+    if (tid == 0)
+        for (int k = 0; k < 8; ++k) {
+            if (busy_ns[k]) atomicAdd(&e.ctr[PC_SIDE_NS + k], busy_ns[k]);
+            if (tasks[k]) atomicAdd(&e.ctr[PC_SIDE_TASKS + k], tasks[k]);
+        }
+}
+
+// ================================================================================================
+// The kernel.
+// ================================================================================================
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(P_THREADS, 1)
+nolsm_persist_kernel(const __grid_constant__ PEngine e) {
+    extern __shared__ uint8_t smem_raw[];
+    G2Smem sm;
+    sm.base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t* side_sm = smem_raw + (sm.base - ptx::smem_u32(smem_raw)) + (G2_SMEM_BYTES - 1024);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = ptx::cluster_ctarank();
+
+    const uint32_t tmem_base = g2_setup(sm, warp, lane);
+
+    if (warp < G2_EPI_WARPS) {
+        g2_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, [&](const TileInfo& ti) { p_tile_finished(e, ti.slot, ti.nreports); });
+    } else if (warp == G2_WARP_SCHED) {
+        if (rank == 0) p_scheduler(sm, e, lane);
+    } else if (warp == G2_WARP_TMA) {
+        g2_producer(sm, e.maps, rank, lane);
+    } else if (warp == G2_WARP_MMA) {
+        if (rank == 0) g2_mma(sm, tmem_base, lane);
+    } else {
+        p_side_loop(e, side_sm, (int)threadIdx.x - G2_CTRL_THREADS);
+    }
+    g2_teardown(tmem_base, warp);
+}
+
+// Stand-alone launch of the gather task for one slot (diagnostics: nolsm_gather_submatrix and the
+// HBM-bandwidth measurement of the gather code without the GEMMs). grid = (chunks, slots).
+template <typename TV>
+__global__ void __launch_bounds__(P_SIDE_THREADS) k_side_gather(SysView sv, const TV* S_vals, const TV* H_vals, __half* base,
+                                                                long long slotsz, long long bufsz, int ld, const int* atoms,
+                                                                const int* dims, unsigned long long* bytes) {
+    extern __shared__ unsigned char sm_dyn[];
+    const int atom = atoms[blockIdx.y], n = dims[atom], n16 = (n + 15) & ~15;
+    __half* dS = base + (long long)blockIdx.y * slotsz;
+    side_gather_chunk<TV>(sv, S_vals, H_vals, dS, dS + bufsz, atom, n, n16, ld, blockIdx.x, gridDim.x, sm_dyn, threadIdx.x, bytes);
+}
+
+}  // namespace nolsm

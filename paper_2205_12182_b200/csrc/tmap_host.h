@@ -27,10 +27,10 @@ inline EncodeTiledFn encode_tiled_fn() {
 // Row-major n x n FP16 matrix with leading dimension ld (elements); box = 64 (contiguous) x 64 rows,
 // 128-byte swizzle, out-of-bounds elements read as zero. The same map serves the K-major A operand
 // (box = 64 k x 64 rows) and the MN-major B operand (box = 64 n x 64 k).
-inline bool make_tmap_f16_64x64(CUtensorMap* out, const void* base, int n, int ld) {
+inline bool make_tmap_f16_64x64(CUtensorMap* out, const void* base, int n, int ld, int cols = 0) {
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return false;
-    cuuint64_t dims[2] = {(cuuint64_t)n, (cuuint64_t)n};
+    cuuint64_t dims[2] = {(cuuint64_t)(cols ? cols : n), (cuuint64_t)n};
     cuuint64_t strides[1] = {(cuuint64_t)ld * 2};
     cuuint32_t box[2] = {64, 64};
     cuuint32_t estr[2] = {1, 1};

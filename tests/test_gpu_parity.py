@@ -102,11 +102,16 @@ def test_cfg0_fp32_mode(cfg0):
     assert abs(E - cmp["e_ref"]) / abs(cmp["e_ref"]) <= TOL_FP32
 
 
-@pytest.mark.parametrize("backend", ["umma", "simt"])
+@pytest.mark.parametrize("backend", ["umma", "umma-rounds", "simt"])
 def test_cfg0_mixed_mode(cfg0, backend):
-    from paper_2205_12182_b200 import GEMM_SIMT, GEMM_UMMA
+    """umma: tcgen05 GEMMs in the persistent engine (the default path); umma-rounds: the same GEMM
+    pipeline in the round engine; simt: FP16 operands with FFMA GEMMs (round engine)."""
+    from paper_2205_12182_b200 import ENGINE_PERSISTENT, ENGINE_ROUNDS, GEMM_SIMT, GEMM_UMMA
     s = cfg0
-    D, E, st, stats = _run(s, gemm_backend=GEMM_UMMA if backend == "umma" else GEMM_SIMT)
+    kw = {"umma": dict(gemm_backend=GEMM_UMMA, engine=ENGINE_PERSISTENT),
+          "umma-rounds": dict(gemm_backend=GEMM_UMMA, engine=ENGINE_ROUNDS),
+          "simt": dict(gemm_backend=GEMM_SIMT)}[backend]
+    D, E, st, stats = _run(s, **kw)
     cmp = compare_atoms(s, D, st["e_atom"], range(s.n_atoms))
     print("mixed cfg0", backend, {k: v for k, v in cmp.items() if k != "ref"}, stats)
     assert (st["status"] == 0).all()
@@ -147,13 +152,15 @@ def test_density_matrix_range_touches_only_its_rows(cfg0):
     assert abs(e - cmp["e_ref"]) / abs(cmp["e_ref"]) <= TOL_MIXED_E
 
 
+@pytest.mark.parametrize("engine", ["persistent", "rounds"])
 @pytest.mark.parametrize("name,n_atoms,sample", [("cfg1", 600, 6), ("cfg2", 300, 3), ("cfg3", 1500, 6)])
-def test_small_proxies_mixed(name, n_atoms, sample):
+def test_small_proxies_mixed(name, n_atoms, sample, engine):
     """Reduced-size versions of configs 1-3 (same density, basis and generator): several tiles per
     matrix, ragged tails, mixed 5/13 basis for cfg3. Oracle on a seeded sample of atoms."""
+    from paper_2205_12182_b200 import ENGINE_PERSISTENT, ENGINE_ROUNDS
     s = make_system(name, n_atoms=n_atoms)
     atoms = np.random.default_rng(1).choice(s.n_atoms, sample, replace=False)
-    D, E, st, stats = _run(s)
+    D, E, st, stats = _run(s, engine=ENGINE_PERSISTENT if engine == "persistent" else ENGINE_ROUNDS)
     cmp = compare_atoms(s, D, st["e_atom"], atoms)
     print(name, {k: v for k, v in cmp.items() if k != "ref"}, stats)
     assert (st["status"] == 0).all()

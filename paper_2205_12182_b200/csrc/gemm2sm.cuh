@@ -28,6 +28,9 @@ constexpr int G2_A_BYTES = 128 * BK * 2;              // 16 KB: this CTA's 128 r
 constexpr int G2_B_BYTES = 2 * B_BOX_BYTES;           // 16 KB: 64 k x (up to 128) columns
 constexpr int G2_STAGE_BYTES = G2_A_BYTES + G2_B_BYTES;
 constexpr int G2_NTI = 4;                             // tile-info ring depth
+#ifndef G2_WANT_LEAD
+#define G2_WANT_LEAD 14                               // k-blocks before the end of its tile at which the producer asks for the next one
+#endif
 constexpr int G2_EPI_WARPS = 8;                       // warp w: TMEM lane quarter w & 3, column chunks of parity w >> 2
 constexpr int G2_WARP_SCHED = 8, G2_WARP_TMA = 9, G2_WARP_MMA = 10;
 constexpr int G2_CTRL_THREADS = 11 * 32;              // warps 0..10
@@ -55,6 +58,8 @@ struct G2Smem {                       // byte offsets from the 1024-aligned base
     __device__ uint32_t ti_full(int q) const { return bars() + 8u * (2 * G2_STAGES + 4 + q); }
     __device__ uint32_t ti_empty(int q) const { return bars() + 8u * (2 * G2_STAGES + 4 + G2_NTI + q); }
     __device__ uint32_t tmem_ptr() const { return bars() + 8u * (2 * G2_STAGES + 4 + 2 * G2_NTI); }
+    // "the producer has issued every load of its current tile and wants the next record" (leader CTA only)
+    __device__ uint32_t want() const { return bars() + 8u * (2 * G2_STAGES + 4 + 2 * G2_NTI) + 8u; }
     __device__ uint32_t tinfo(int q) const { return bars() + 256u + 64u * q; }
 };
 constexpr int G2_SMEM_BYTES = G2_STAGES * G2_STAGE_BYTES + 256 + 64 * G2_NTI + 1024 /*align*/;
@@ -162,6 +167,7 @@ __device__ __forceinline__ uint32_t g2_setup(const G2Smem& sm, int warp, int lan
         for (int s = 0; s < G2_STAGES; ++s) { ptx::mbar_init(sm.full(s), 1); ptx::mbar_init(sm.empty(s), 1); }
         for (int a = 0; a < 2; ++a) { ptx::mbar_init(sm.tfull(a), 1); ptx::mbar_init(sm.tempty(a), 2 * G2_EPI_WARPS); }
         for (int q = 0; q < G2_NTI; ++q) { ptx::mbar_init(sm.ti_full(q), 1); ptx::mbar_init(sm.ti_empty(q), G2_TI_CONSUMERS); }
+        ptx::mbar_init(sm.want(), 1);
         ptx::fence_mbar_init();
     }
     if (warp == G2_WARP_MMA) ptx::tmem_alloc_pair(sm.tmem_ptr(), 512);
@@ -232,7 +238,7 @@ __device__ __forceinline__ TileInfo g2_take(const G2Smem& sm, int q, uint32_t ph
 // ------------------------------------------------------------------------------------------------
 // TMA producer (one warp per CTA; lane 0 issues).
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap* maps, uint32_t rank, int lane) {
+__device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap* maps, uint32_t rank, int lane, int want_lead = G2_WANT_LEAD) {
     int stage = 0; uint32_t phase = 0;
     int q = 0; uint32_t tph = 0;
     for (;;) {
@@ -249,9 +255,11 @@ __device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap*
         const int row0 = ti.m0 + 128 * (int)rank;
         const int col0 = ti.n0 + half * (int)rank;
         const uint32_t full0 = ptx::mapa(sm.full(0), 0);                    // the leader's full barriers
+        const int kb_want = max(0, nkb - want_lead);
         for (int kb = 0; kb < nkb; ++kb) {
             ptx::mbar_wait(sm.empty(stage), phase ^ 1);
             if (lane == 0) {
+                if (kb == kb_want && rank == 0) ptx::mbar_arrive(sm.want());   // the scheduler may claim the next tile now
                 const uint32_t fb = full0 + 8u * stage;
                 if (rank == 0) ptx::mbar_expect_tx(sm.full(stage), bytes);
                 const uint32_t sa = sm.stage_a(stage), sb = sm.stage_b(stage);

@@ -529,7 +529,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         }
     });
     int max_n = 0, min_n = 1 << 30, max_nset = 0, max_nbi = 0;
-    double mean_tiles = 0;
+    double mean_tiles = 0, mean_n2 = 0;
     for (int64_t i = 0; i < n_atoms; ++i) {
         max_n = std::max(max_n, c->dim[i]);
         min_n = std::min(min_n, c->dim[i]);
@@ -538,8 +538,10 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         int ntm, ntn;
         choose_tiling((c->dim[i] + 15) & ~15, ntm, ntn);
         mean_tiles += (double)ntm * ntn;
+        mean_n2 += (double)c->dim[i] * c->dim[i];
     }
     mean_tiles /= (double)n_atoms;
+    mean_n2 /= (double)n_atoms;
     if (max_n > 65535) return fail(c, NOLSM_EINVAL, "submatrix dimension > 65535 not supported");
     c->max_n = max_n; c->max_nset = max_nset; c->max_nbi = max_nbi;
     if (!c->filtered) {
@@ -581,8 +583,17 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         return fail(c, NOLSM_EINVAL, "the persistent engine needs FP16/tcgen05 mode and submatrix dimensions <= 2048");
     // round engine: enough slots for ~16 waves of tiles per GEMM launch; persistent engine: the slots in
     // flight (GEMM chain + side phases), few enough to keep the active iterates in L2
+    // heavy-phase cap of the persistent engine: the live iterates of a slot in the GEMM chain are ~3.5 n^2 FP16
+    // (X, T, next X / S, Y, R, next Y); the slots inside the chain together may fill L2 (measured on cfg2:
+    // 10-14 slots give the same throughput, fewer starve the pairs, more overflow L2 and draw HBM power)
+    int l2_bytes = 0;
+    cudaDeviceGetAttribute(&l2_bytes, cudaDevAttrL2CacheSize, c->dev);
+    if (l2_bytes <= 0) l2_bytes = 64 << 20;
+    int g_max = (int)std::floor(1.0 * (double)l2_bytes / (3.5 * mean_n2 * 2.0));
+    g_max = std::max(3, std::min(g_max, 48));
+    if (getenv_int("NOLSM_GMAX", 0) > 0) g_max = getenv_int("NOLSM_GMAX", 0);
     int S = c->opt.batch_atoms > 0 ? c->opt.batch_atoms
-            : c->persist ? (int)std::min(64.0, std::max(16.0, std::ceil(5.0 * c->sms / std::max(1.0, mean_tiles))))
+            : c->persist ? std::min(96, g_max + std::max(12, g_max))
                          : (int)std::ceil(16.0 * c->sms / std::max(1.0, mean_tiles));
     S = std::max(S, 2);
     S = (int)std::min<size_t>(S, std::max<size_t>(2, cap_bytes / slot_bytes));
@@ -669,10 +680,14 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         if ((r = dmalloc(c, (void**)&pe.sclaim, 4 * S))) return r;
         if ((r = dmalloc(c, (void**)&pe.ctr, 8 * PC_LEN))) return r;
         if ((r = dmalloc(c, (void**)&c->d_abort, 16))) return r;
+        if ((r = dmalloc(c, (void**)&pe.heavy, 16))) return r;
+        if ((r = dmalloc(c, (void**)&pe.parked, 4 * S))) return r;
         pe.S = S; pe.cap = e.cap; pe.ld = e.ld; pe.bufsz = e.bufsz; pe.slotsz = e.slotsz;
         pe.tol_inv = e.tol_inv; pe.tol_sign = e.tol_sign; pe.max_inv = e.max_inv; pe.max_sign = e.max_sign;
         pe.p_s = e.p_s; pe.p_a = e.p_a; pe.safety_s = 1.05f; pe.safety_a = 1.05f;
         pe.gather_rowatoms = g_rowatoms;
+        pe.g_max = std::max(1, std::min(g_max, S));
+        pe.want_lead = std::max(1, getenv_int("NOLSM_WANT_LEAD", G2_WANT_LEAD));
         pe.schulz_chunks = std::max(1, getenv_int("NOLSM_SCHULZ_CHUNKS", 16));
         pe.dcols_chunks = std::max(1, getenv_int("NOLSM_DCOLS_CHUNKS", 16));
         pe.next_atom = e.next_atom; pe.finished = e.finished; pe.abort_flag = c->d_abort;
@@ -739,6 +754,8 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
         CU_TRY(c, cudaMemcpyAsync(pe.next_atom, &c->h_a0, 4, cudaMemcpyHostToDevice, s));
         CU_TRY(c, cudaMemsetAsync(pe.finished, 0, 4, s));
         CU_TRY(c, cudaMemsetAsync(c->d_abort, 0, 4, s));
+        CU_TRY(c, cudaMemsetAsync(pe.heavy, 0, 4, s));
+        CU_TRY(c, cudaMemsetAsync(pe.parked, 0, 4 * pe.S, s));
         CU_TRY(c, cudaEventRecord(c->ev_k0, s));
         nolsm_persist_kernel<<<c->sms & ~1, P_THREADS, P_SMEM_BYTES, s>>>(pe);
         CU_TRY(c, cudaGetLastError());

@@ -67,6 +67,9 @@ struct PEngine {
     int gather_rowatoms, schulz_chunks, dcols_chunks;   // row-atoms of N(i) per gather chunk; chunks of the other tasks
     int* next_atom; int a_end, total;
     int* finished;
+    int* heavy;                   // [1] slots inside the GEMM-heavy phases INV .. SIGN right now (at most g_max)
+    int* parked;                  // [S] 1 = the slot finished its first Schulz step and waits for a heavy token
+    int g_max, want_lead;
     volatile int* abort_flag;     // device word; the host sets it (copy on another stream) to stop a kernel that overran its time limit
     unsigned long long* ctr;      // [PC_LEN]
     AtomArrays at;
@@ -155,6 +158,40 @@ __device__ __forceinline__ void p_start_power(const PEngine& e, int slot, int ki
     __stcg(&s->pow_norm2, (float)NVC * (float)__ldcg(&s->n));
     __stcg(&s->pow_alpha, 1.f);
     p_install_gemm(e, slot, kind);
+}
+
+// L2 residency: a slot's iterates (X, T, Y: ~3-4 n^2 FP16) are re-read by every GEMM of its chain, so only
+// as many slots as fit in L2 together may be inside the heavy phases (Schulz iterations .. sign iterations)
+// at once. A slot that is ready to enter takes a token or parks; a slot that leaves hands its token to a
+// parked slot (and installs that slot's first GEMM) or returns it.
+__device__ __forceinline__ void p_enter_heavy_now(const PEngine& e, int slot) {
+    PSlot* s = &e.slots[slot];
+    __stcg(&s->inv_iters, 1);
+    __stcg(&s->ycur, 2);
+    p_install_gemm(e, slot, OP_INV_G1);
+}
+__device__ __forceinline__ void p_enter_heavy(const PEngine& e, int slot) {
+    if (atomicAdd(e.heavy, 1) < e.g_max) { p_enter_heavy_now(e, slot); return; }
+    atomicSub(e.heavy, 1);
+    __threadfence();
+    atomicExch(&e.parked[slot], 1);
+    __threadfence();
+    // a token may have been returned between the failed attempt and the parking: try once more
+    if (atomicAdd(e.heavy, 1) < e.g_max) {
+        if (atomicCAS(&e.parked[slot], 1, 0) == 1) { p_enter_heavy_now(e, slot); return; }
+        // a leaving slot admitted this one meanwhile (with its own token)
+    }
+    atomicSub(e.heavy, 1);
+}
+__device__ __forceinline__ void p_leave_heavy(const PEngine& e) {
+    for (int s = 0; s < e.S; ++s) {
+        if (*(volatile int*)&e.parked[s] == 1 && atomicCAS(&e.parked[s], 1, 0) == 1) {
+            __threadfence();
+            p_enter_heavy_now(e, s);          // the token changes hands
+            return;
+        }
+    }
+    atomicSub(e.heavy, 1);
 }
 
 // Takes the next atom of the feed into the slot and installs its gather (phase NEW). Returns false when
@@ -252,7 +289,7 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
         if (__ldcg(&s->conv)) {
             __stcg(&s->conv, 0);
             __stcg(&s->res_prev, 1e30f);
-            if (__ldcg(&s->status) & ST_NOTSPD) p_retire(e, slot);      // no D for this atom (rows stay zero)
+            if (__ldcg(&s->status) & ST_NOTSPD) { p_leave_heavy(e); p_retire(e, slot); }   // no D for this atom (rows stay zero)
             else p_install_gemm(e, slot, OP_AMAT);
         } else {
             p_install_gemm(e, slot, OP_INV_G1);
@@ -264,6 +301,7 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
         __stcg(&s->xcur, 1 - __ldcg(&s->xcur));
         if (__ldcg(&s->conv)) {
             __stcg(&s->conv, 0);
+            p_leave_heavy(e);
             p_install_side(e, slot, SK_DCOLS, e.dcols_chunks);
         } else {
             p_install_gemm(e, slot, OP_SIGN_G1);
@@ -283,6 +321,14 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
         for (uint32_t spins = 0; !ptx::mbar_try_wait_cluster(sm.ti_empty(q), ph ^ 1);) {
             __nanosleep(100);
             if (++spins > (1u << 26)) __trap();
+        }
+        // Claim lazily: only when the producer has issued every load of the tile before and needs the next
+        // record (it runs G2_STAGES k-blocks ahead of the MMA, which hides the claim). A pair that claimed
+        // further ahead would hoard tiles of a GEMM that idle pairs could run at the same time, and the
+        // slot's chain of dependent GEMMs would take that much longer.
+        for (uint32_t spins = 0; !ptx::mbar_try_wait(sm.want(), (uint32_t)(ntiles & 1) ^ 1u);) {
+            __nanosleep(64);
+            if (++spins > (1u << 28)) __trap();
         }
         TileInfo ti{};
         int got = 0;
@@ -676,11 +722,7 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
                         if (!p_refill(e, slot)) *(volatile unsigned int*)&e.sclaim[slot] = 0u;
                         break;
                     case SK_GATHER: p_start_power(e, slot, OP_POW_S); break;
-                    case SK_SCHULZ1:
-                        __stcg(&s->inv_iters, 1);
-                        __stcg(&s->ycur, 2);
-                        p_install_gemm(e, slot, OP_INV_G1);
-                        break;
+                    case SK_SCHULZ1: p_enter_heavy(e, slot); break;
                     case SK_DCOLS: {
                         const double nv = (double)(e.sv.blk_off[e.sv.row_ptr[atom + 1]] - e.sv.blk_off[e.sv.row_ptr[atom]]);
                         atomicAdd(&e.ctr[PC_SIDE_BYTES + SK_DCOLS],
@@ -718,7 +760,7 @@ nolsm_persist_kernel(const __grid_constant__ PEngine e) {
     } else if (warp == G2_WARP_SCHED) {
         if (rank == 0) p_scheduler(sm, e, lane);
     } else if (warp == G2_WARP_TMA) {
-        g2_producer(sm, e.maps, rank, lane);
+        g2_producer(sm, e.maps, rank, lane, e.want_lead);
     } else if (warp == G2_WARP_MMA) {
         if (rank == 0) g2_mma(sm, tmem_base, lane);
     } else {

@@ -71,6 +71,12 @@ typedef struct {
     int profile_every;       /* round engine, > 0: every k-th round runs eagerly with CUDA events around each launch [0 = off] */
     int engine;              /* NOLSM_ENGINE_* [AUTO: PERSISTENT (one kernel launch per density_matrix call) for the
                                 FP16/tcgen05 path when every n_i <= 2048, else ROUNDS (one CUDA graph per iteration round)] */
+    int sign_scaled_iters;   /* persistent engine: the first k sign iterations run Eq. 6 on alpha X_k instead of X_k,
+                                X_{k+1} = 1/2 (alpha X_k)(3I - (alpha X_k)^2), alpha = sign_scale > 1, which lifts small
+                                eigenvalues 1.5 alpha x per step instead of 1.5 x and keeps the rest inside
+                                [alpha (3 - alpha^2) / 2, 1]; two steps with the optimal scalings for that interval follow,
+                                then plain Eq. 6 until the convergence test passes (C-6b) [6; -1 = plain Eq. 6] */
+    float sign_scale;        /* alpha of the scaled steps, 1 < alpha < sqrt(3) [1.5] */
 } nolsm_options;
 
 typedef struct {

@@ -42,7 +42,7 @@ struct __align__(16) TileInfo {      // 64 bytes
     int slot, m0, n0;                 // pair tile origin (rows m0 .. m0+255, columns n0 .. n0+bn-1)
     int n, n16, bn, nreports;         // nreports = CTA reports that complete the slot's GEMM
     int a_buf, b_buf, c_buf, want_res;
-    float alpha, sgn, beta;
+    float c_out, alpha_res, beta;      // C = c_out * acc + beta * I ; residual || alpha_res * acc - I ||_F^2
     int kind;
 };
 
@@ -345,8 +345,8 @@ __device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int
 }
 
 // ------------------------------------------------------------------------------------------------
-// Epilogue (warps 0..3 of each CTA): C = sgn * alpha * acc + beta * I, FP16 stores, fused squared
-// residual || alpha A B - I ||_F^2 (the convergence test, C-7). `done(ti)` is called by one
+// Epilogue (warps 0..7 of each CTA): C = c_out * acc + beta * I, FP16 stores, fused squared
+// residual || alpha_res A B - I ||_F^2 (the convergence test, C-7). `done(ti)` is called by one
 // thread of the CTA after all of the CTA's stores of the tile have been issued and fenced.
 // ------------------------------------------------------------------------------------------------
 template <typename Eng, typename Done>
@@ -369,7 +369,7 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
         const int rbase = ti.m0 + 128 * (int)rank + quarter * 32;      // first row of this warp
         const int row = rbase + lane;
         const int col0 = ti.n0;
-        const float sa = ti.sgn * ti.alpha;
+        const float sa = ti.c_out;
         { G2_T0(); ptx::mbar_wait(sm.tfull(acc), acc_phase); G2_T1(5); }
         G2_T0();
         ptx::tc_fence_after();
@@ -402,11 +402,11 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
 #pragma unroll
                 for (int j = 0; j < 32; ++j) {
                     const int col = col0 + c + j;
-                    const float x = ti.alpha * __uint_as_float(v[j]);
+                    const float a = __uint_as_float(v[j]);
                     const float delta = (col == row && row < n && ident) ? 1.f : 0.f;
-                    const float d = (c + j < bn && col < n16) ? x - delta : 0.f;   // pad rows / columns give exactly 0
+                    const float d = (c + j < bn && col < n16) ? ti.alpha_res * a - delta : 0.f;   // pad rows / columns give exactly 0
                     rsum = fmaf(d, d, rsum);
-                    f[j] = ti.sgn * x + ti.beta * delta;
+                    f[j] = ti.c_out * a + ti.beta * delta;
                 }
                 const int cw = min(min(32, bn - c), n16 - (col0 + c));   // 16 or 32 valid columns
 #pragma unroll
@@ -419,7 +419,7 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive_cluster_relaxed(tempty0 + 8u * acc, dep);
         if (ti.want_res) {
-            rsum = fmaf(ti.alpha * ti.alpha, vsum, rsum);
+            rsum = fmaf(ti.alpha_res * ti.alpha_res, vsum, rsum);
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) rsum += __shfl_xor_sync(0xffffffffu, rsum, o);
             if (lane == 0 && rsum != 0.f) atomicAdd(&e.slots[ti.slot].res_acc, rsum);
@@ -471,7 +471,7 @@ gemm2_round_kernel(const __grid_constant__ UmmaArgs args) {
                 ti.slot = slot; ti.m0 = tm * BM; ti.n0 = tn * BN;
                 ti.n = sl.n; ti.n16 = sl.n16; ti.bn = min(BN, sl.n16 - tn * BN); ti.nreports = 2 * op.ntiles;
                 ti.a_buf = op.a_buf; ti.b_buf = op.b_buf; ti.c_buf = op.c_buf; ti.want_res = op.want_res;
-                ti.alpha = op.alpha; ti.sgn = op.sgn; ti.beta = op.beta; ti.kind = op.kind;
+                ti.c_out = op.sgn * op.alpha; ti.alpha_res = op.alpha; ti.beta = op.beta; ti.kind = op.kind;
                 tile += npairs;
                 return true;
             });

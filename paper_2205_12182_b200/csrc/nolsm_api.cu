@@ -365,6 +365,13 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
     if (o.power_iters_s <= 0) o.power_iters_s = 6;
     if (o.power_iters_a <= 0) o.power_iters_a = 12;
     if (o.eps_filter < 0) { delete c; return NOLSM_EINVAL; }
+    if (o.sign_scaled_iters == 0) o.sign_scaled_iters = 6;
+    if (getenv("NOLSM_SIGN_SCALED_ITERS")) o.sign_scaled_iters = getenv_int("NOLSM_SIGN_SCALED_ITERS", 6);
+    if (o.sign_scaled_iters < 0) o.sign_scaled_iters = 0;
+    if (o.sign_scaled_iters > 14) o.sign_scaled_iters = 14;
+    if (o.sign_scale == 0.f) o.sign_scale = 1.5f;
+    if (const char* v = getenv("NOLSM_SIGN_SCALE")) o.sign_scale = (float)atof(v);
+    if (!(o.sign_scale > 1.f && o.sign_scale < 1.7320508f)) { delete c; return NOLSM_EINVAL; }
     cudaSetDevice(cuda_device);
     cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, cuda_device);
     if (getenv_int("NOLSM_PROFILE_EVERY", 0) > 0) o.profile_every = getenv_int("NOLSM_PROFILE_EVERY", 0);
@@ -686,6 +693,21 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         pe.tol_inv = e.tol_inv; pe.tol_sign = e.tol_sign; pe.max_inv = e.max_inv; pe.max_sign = e.max_sign;
         pe.p_s = e.p_s; pe.p_a = e.p_a; pe.safety_s = 1.05f; pe.safety_a = 1.05f;
         pe.gather_rowatoms = g_rowatoms;
+        {   // scaled Newton-Schulz schedule (C-6b): k0 steps with alpha_f, then the two optimal scalings
+            // alpha = sqrt(3 / (1 + l + l^2)) for the interval [l, 1] the steps before leave the spectrum in
+            const int k0 = c->opt.sign_scaled_iters;
+            pe.n_sched = 0;
+            if (k0 > 0) {
+                const double af = c->opt.sign_scale;
+                for (int k = 0; k < k0; ++k) pe.alpha_sched[pe.n_sched++] = (float)af;
+                double l = 0.5 * af * (3.0 - af * af);
+                for (int k = 0; k < 2; ++k) {
+                    const double al = std::sqrt(3.0 / (1.0 + l + l * l));
+                    pe.alpha_sched[pe.n_sched++] = (float)al;
+                    l = 0.5 * al * l * (3.0 - al * al * l * l);
+                }
+            }
+        }
         pe.g_max = std::max(1, std::min(g_max, S));
         pe.want_lead = std::max(1, getenv_int("NOLSM_WANT_LEAD", G2_WANT_LEAD));
         pe.schulz_chunks = std::max(1, getenv_int("NOLSM_SCHULZ_CHUNKS", 16));

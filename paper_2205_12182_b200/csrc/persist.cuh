@@ -48,12 +48,12 @@ enum { PC_TILES = 0, PC_SCHED_IDLE_NS, PC_SCHED_BUSY_NS, PC_OVERSHOOT, PC_T_STAR
 
 struct __align__(16) PSlot {      // 160 bytes
     int atom, n, n16, pos, nbi, ntm, ntn, nset;                     // geometry (written at refill)
-    int op_kind, a_buf, b_buf, c_buf;                               // live GEMM op: C = sgn alpha A B + beta I
-    float alpha, sgn, beta; int want_res;
+    int op_kind, a_buf, b_buf, c_buf;                               // live GEMM op: C = c_out A B + beta I, residual of alpha_res A B
+    float c_out, alpha_res, beta; int want_res;
     int inv_iters, sign_iters, conv, xcur, ycur, status, gemm_count, tiles_done;
     float res_acc, res_prev, res_last, rho_s, rho_a, alpha1, alpha2; int side_done;
     int pow_step; float pow_norm2, pow_alpha, pow_est;              // block power iteration state
-    int pad[4];
+    int noboost, pad[3];                                            // noboost: the scaled steps are over for this matrix
 };
 
 struct PEngine {
@@ -70,6 +70,7 @@ struct PEngine {
     int* heavy;                   // [1] slots inside the GEMM-heavy phases INV .. SIGN right now (at most g_max)
     int* parked;                  // [S] 1 = the slot finished its first Schulz step and waits for a heavy token
     int g_max, want_lead;
+    int n_sched; float alpha_sched[16];   // scaled Newton-Schulz: alpha_k of sign iteration k < n_sched (1 afterwards)
     volatile int* abort_flag;     // device word; the host sets it (copy on another stream) to stop a kernel that overran its time limit
     unsigned long long* ctr;      // [PC_LEN]
     AtomArrays at;
@@ -123,28 +124,41 @@ __device__ __forceinline__ void p_install_side(const PEngine& e, int slot, int k
     *(volatile unsigned int*)&e.sclaim[slot] = ((unsigned)kind << 28) | ((unsigned)chunks << 14);
 }
 
+// Scaling alpha_k of sign iteration k (C-6b): X_{k+1} = 1/2 (alpha X_k)(3I - (alpha X_k)^2).
+__device__ __forceinline__ float p_sign_alpha(const PEngine& e, const PSlot* s, int k) {
+    return (k < e.n_sched && !__ldcg(&s->noboost)) ? e.alpha_sched[k] : 1.f;
+}
+
 __device__ __forceinline__ void p_install_gemm(const PEngine& e, int slot, int kind) {
     PSlot* s = &e.slots[slot];
     const int xcur = __ldcg(&s->xcur), ycur = __ldcg(&s->ycur);
-    const bool first = __ldcg(&s->sign_iters) == 0;
+    const int k = __ldcg(&s->sign_iters);
+    const bool first = k == 0;
     int a = 0, b = 0, c = 0, want = 0;
-    float alpha = 1.f, sgn = 1.f, beta = 0.f;
+    float c_out = 1.f, alpha_res = 1.f, beta = 0.f;
     switch (kind) {
-        case OP_INV_G1: a = 0; b = ycur; c = 4; sgn = -1.f; beta = 2.f; want = 1; break;          // R = 2I - S Y
+        case OP_INV_G1: a = 0; b = ycur; c = 4; c_out = -1.f; beta = 2.f; want = 1; break;       // R = 2I - S Y
         case OP_INV_G2: a = ycur; b = 4; c = 5 - ycur; break;                                       // Y <- Y R
         case OP_AMAT: a = ycur; b = 1; c = 0; beta = -e.mu; break;                                  // A = Y H0 - mu I
-        case OP_SIGN_G1: a = xcur; b = xcur; c = 4; alpha = first ? __ldcg(&s->alpha1) : 1.f; sgn = -1.f; beta = 3.f; want = 1; break;
-        case OP_SIGN_G2: a = xcur; b = 4; c = 1 - xcur; alpha = first ? __ldcg(&s->alpha2) : 0.5f; break;
+        case OP_SIGN_G1: {                                                                          // T = 3I - alpha^2 X^2
+            const float al = p_sign_alpha(e, s, k);
+            alpha_res = first ? __ldcg(&s->alpha1) : 1.f;                                           // X0 = A / rho is never stored
+            a = xcur; b = xcur; c = 4; c_out = -al * al * alpha_res; beta = 3.f; want = 1;
+        } break;
+        case OP_SIGN_G2: {                                                                          // X <- alpha/2 X T
+            const float al = p_sign_alpha(e, s, k);
+            a = xcur; b = 4; c = 1 - xcur; c_out = al * (first ? __ldcg(&s->alpha2) : 0.5f);
+        } break;
         case OP_POW_S:
         case OP_POW_A: {                                                                            // V <- alpha M V
             const int st = __ldcg(&s->pow_step);
             a = 0; b = st == 0 ? NMAP - 1 : NBUF + ((st - 1) & 1); c = NBUF + (st & 1);
-            alpha = __ldcg(&s->pow_alpha); want = 1;
+            c_out = alpha_res = __ldcg(&s->pow_alpha); want = 1;
         } break;
         default: break;
     }
     __stcg(reinterpret_cast<int4*>(&s->op_kind), make_int4(kind, a, b, c));
-    __stcg(reinterpret_cast<float4*>(&s->alpha), make_float4(alpha, sgn, beta, __int_as_float(want)));
+    __stcg(reinterpret_cast<float4*>(&s->c_out), make_float4(c_out, alpha_res, beta, __int_as_float(want)));
     const bool pow = kind == OP_POW_S || kind == OP_POW_A;
     const unsigned long long tiles = (unsigned long long)(__ldcg(&s->ntm) * (pow ? 1 : __ldcg(&s->ntn)));
     __threadfence();
@@ -211,6 +225,7 @@ __device__ __forceinline__ bool p_refill(const PEngine& e, int slot) {
     __stcg(reinterpret_cast<int4*>(&s->ycur), make_int4(2, 0, 0, 0));                 // ycur, status, gemm_count, tiles_done
     __stcg(reinterpret_cast<float4*>(&s->res_acc), make_float4(0.f, 1e30f, 0.f, 0.f)); // res_acc, res_prev, res_last, rho_s
     __stcg(reinterpret_cast<float4*>(&s->rho_a), make_float4(0.f, 1.f, 0.5f, 0.f));    // rho_a, alpha1, alpha2, side_done
+    __stcg(reinterpret_cast<int4*>(&s->noboost), make_int4(0, 0, 0, 0));
     p_install_side(e, slot, SK_GATHER, (nset + e.gather_rowatoms - 1) / e.gather_rowatoms);
     return true;
 }
@@ -278,10 +293,22 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
         const int cap = inv ? e.max_inv : e.max_sign;
         const bool ok = r < tol;
         const bool stagnated = (r > 0.5f * rp) && (r < 4.f * tol) && iters > 0;   // rounding floor reached
-        const bool diverged = !(r == r) || (iters > 1 && r > rp && r > 0.9f);
+        // during the scaled sign steps the bulk of the spectrum is deliberately kept away from +-1, so the
+        // residual need not fall from one step to the next: the divergence rule applies after them
+        const bool scaled_phase = !inv && iters <= e.n_sched && !__ldcg(&s->noboost);
+        const bool diverged = !(r == r) || (!scaled_phase && iters > 1 && r > rp && r > 0.9f);
         const bool capped = iters + 1 >= cap;
         if (diverged || (capped && !ok && !stagnated)) __stcg(&s->status, __ldcg(&s->status) | (inv ? ST_NOTSPD : ST_NOCONV));
-        __stcg(&s->conv, (ok || stagnated || diverged || capped) ? 1 : 0);
+        const bool conv = ok || stagnated || diverged || capped;
+        if (!inv && conv && p_sign_alpha(e, s, iters) != 1.f) {
+            // X_k passed the test, but T was formed with alpha_k != 1 and a scaled step would move the spectrum
+            // away from +-1 again: switch the scaling off for this matrix and form T = 3I - X_k^2 once more
+            __stcg(&s->noboost, 1);
+            __stcg(&s->res_prev, rp);
+            p_install_gemm(e, slot, OP_SIGN_G1);
+            return;
+        }
+        __stcg(&s->conv, conv ? 1 : 0);
         p_install_gemm(e, slot, inv ? OP_INV_G2 : OP_SIGN_G2);
     } else if (kind == OP_INV_G2) {
         __stcg(&s->inv_iters, __ldcg(&s->inv_iters) + 1);
@@ -354,14 +381,14 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
                         const int4 g0 = __ldcg(reinterpret_cast<const int4*>(&s->atom));     // atom n n16 pos
                         const int4 g1 = __ldcg(reinterpret_cast<const int4*>(&s->nbi));      // nbi ntm ntn nset
                         const int4 o0 = __ldcg(reinterpret_cast<const int4*>(&s->op_kind));
-                        const float4 o1 = __ldcg(reinterpret_cast<const float4*>(&s->alpha));
+                        const float4 o1 = __ldcg(reinterpret_cast<const float4*>(&s->c_out));
                         const bool pow = o0.x == OP_POW_S || o0.x == OP_POW_A;
                         const int ntn = pow ? 1 : g1.z;
                         const int tm = t / ntn, tn = t - tm * ntn;
                         ti.slot = found; ti.m0 = tm * BM; ti.n0 = tn * BN;
                         ti.n = g0.y; ti.n16 = g0.z; ti.bn = pow ? NVC : min(BN, g0.z - tn * BN); ti.nreports = 2 * nt;
                         ti.kind = o0.x; ti.a_buf = o0.y; ti.b_buf = o0.z; ti.c_buf = o0.w;
-                        ti.alpha = o1.x; ti.sgn = o1.y; ti.beta = o1.z; ti.want_res = __float_as_int(o1.w);
+                        ti.c_out = o1.x; ti.alpha_res = o1.y; ti.beta = o1.z; ti.want_res = __float_as_int(o1.w);
                     }
                     got = 1;
                     break;

@@ -365,7 +365,7 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
         const int n = ti.n, n16 = ti.n16, bn = ti.bn;
         int ldc;
         __half* C = c_ptr(e, base, ti.slot, ti.c_buf, ldc);
-        const bool ident = ti.kind != OP_POW_S && ti.kind != OP_POW_A;   // power-iteration tiles: C = alpha A V, res = ||C||_F^2
+        const bool ident = ti.kind != OP_POW_S && ti.kind != OP_POW_A && ti.kind != OP_DCOLS;   // power-iteration tiles: C = alpha A V, res = ||C||_F^2
         const int rbase = ti.m0 + 128 * (int)rank + quarter * 32;      // first row of this warp
         const int row = rbase + lane;
         const int col0 = ti.n0;
@@ -381,6 +381,15 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
             ptx::tmem_ld_32x32(tmem_base + acc * 256 + ((uint32_t)(quarter * 32) << 16) + c, v);
             ptx::tmem_ld_wait();
             dep ^= v[0];
+            if (ti.kind == OP_DCOLS) {                             // P[row, 0..31] = acc, FP32 (a6: D columns are formed from FP32)
+                if (c == 0 && row < n16) {
+                    float4* prow = reinterpret_cast<float4*>(pcols_ptr(e, ti.slot) + (size_t)row * PCW);
+#pragma unroll
+                    for (int j = 0; j < PCW; j += 4)
+                        prow[j >> 2] = make_float4(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), __uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]));
+                }
+                continue;
+            }
             __half* crow = C + (size_t)row * ldc + col0 + c;
             const bool full = (c + 32 <= bn) && (col0 + c + 32 <= n16);
             const bool diag = (col0 + c < rbase + 32) && (col0 + c + 32 > rbase);

@@ -582,12 +582,13 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     const size_t slot_bytes = (size_t)e.slotsz * es;
     const size_t cap_bytes = c->opt.workspace_bytes ? c->opt.workspace_bytes : std::min<size_t>(free_b / 2, (size_t)48 << 30);
     // persistent engine: slot buffers must fit the side tasks' shared memory (power-iteration vectors, Y columns)
-    const int g_rowatoms = std::min(P_GATHER_ROWATOMS, std::max(1, getenv_int("NOLSM_GATHER_ROWATOMS", 2)));
-    c->persist = want_persist(c) && e.cap <= P_MAX_CAP &&
-                 (size_t)(max_nset + 1) * 4 + 16 + (size_t)max_nbi * e.cap * 2 <= (size_t)P_SIDE_SMEM &&
-                 (size_t)(2 * max_nset + 1) * 4 + 8 + (size_t)g_rowatoms * max_nset * 8 + (size_t)e.cap * 2 <= (size_t)P_SIDE_SMEM;
+    const int g_rowatoms = std::max(1, getenv_int("NOLSM_GATHER_ROWATOMS", 4));
+    // (gather task: index tables + dense strip + 4 x 2 cp.async stages; a strip holds at least one dense row)
+    c->persist = want_persist(c) && e.cap <= P_MAX_CAP && max_nbi <= NVC &&
+                 (size_t)(3 * max_nset + 2) * 4 + (size_t)max_nset * 8 + 32 + G_STRIP_BYTES + (size_t)P_SIDE_WARPS * 2 * G_STAGE_BYTES <= (size_t)P_SIDE_SMEM &&
+                 (size_t)e.cap * 2 <= (size_t)G_STRIP_BYTES;
     if (!c->persist && c->opt.engine == NOLSM_ENGINE_PERSISTENT)
-        return fail(c, NOLSM_EINVAL, "the persistent engine needs FP16/tcgen05 mode and submatrix dimensions <= 2048");
+        return fail(c, NOLSM_EINVAL, "the persistent engine needs FP16/tcgen05 mode, submatrix dimensions <= 2048 and at most 16 basis functions per atom");
     // round engine: enough slots for ~16 waves of tiles per GEMM launch; persistent engine: the slots in
     // flight (GEMM chain + side phases), few enough to keep the active iterates in L2
     // heavy-phase cap of the persistent engine: the live iterates of a slot in the GEMM chain are ~3.5 n^2 FP16
@@ -688,6 +689,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         if ((r = dmalloc(c, (void**)&pe.ctr, 8 * PC_LEN))) return r;
         if ((r = dmalloc(c, (void**)&c->d_abort, 16))) return r;
         if ((r = dmalloc(c, (void**)&pe.heavy, 16))) return r;
+        if ((r = dmalloc(c, (void**)&pe.pcols, (size_t)S * e.cap * PCW * sizeof(float)))) return r;
         if ((r = dmalloc(c, (void**)&pe.parked, 4 * S))) return r;
         pe.S = S; pe.cap = e.cap; pe.ld = e.ld; pe.bufsz = e.bufsz; pe.slotsz = e.slotsz;
         pe.tol_inv = e.tol_inv; pe.tol_sign = e.tol_sign; pe.max_inv = e.max_inv; pe.max_sign = e.max_sign;
@@ -711,7 +713,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         pe.g_max = std::max(1, std::min(g_max, S));
         pe.want_lead = std::max(1, getenv_int("NOLSM_WANT_LEAD", G2_WANT_LEAD));
         pe.schulz_chunks = std::max(1, getenv_int("NOLSM_SCHULZ_CHUNKS", 16));
-        pe.dcols_chunks = std::max(1, getenv_int("NOLSM_DCOLS_CHUNKS", 16));
+        pe.dcols_chunks = std::max(1, getenv_int("NOLSM_DCOLS_CHUNKS", 4));
         pe.next_atom = e.next_atom; pe.finished = e.finished; pe.abort_flag = c->d_abort;
         pe.at = e.at; pe.sv = sys_view(c);
         pe.S_vals = c->dS; pe.H_vals = c->dH; pe.val_f64 = val_dtype == NOLSM_DTYPE_F64;

@@ -30,6 +30,7 @@ namespace nolsm {
 constexpr int NBUF = 5;          // B0 = S then X(even), B1 = H0 then X(odd), B2/B3 = Y ping-pong, B4 = R / T
 constexpr int NMAP = 8;          // tensor maps per slot: 0-4 the buffers, 5/6 the power-iteration vector blocks, 7 the start block
 constexpr int NVC = 16;          // vectors of the block power iteration (one 16-column GEMM tile)
+constexpr int PCW = 32;          // columns of an OP_DCOLS tile: cols(i) = [pos, pos + nb(i)) inside [pos & ~7, (pos & ~7) + 32), TMA boxes start 16-byte aligned
 constexpr int VLD = 64;          // leading dimension of a vector block (one 128-byte row)
 constexpr int BM = 256;          // GEMM tile rows (one CTA pair, tcgen05 cta_group::2)
 constexpr int BN = 256;          // GEMM tile columns; the last tile of a row is n16 - 256 (ntn - 1) wide
@@ -40,7 +41,8 @@ constexpr int ST_NOTSPD = 1;     // Schulz inverse iteration diverged / did not 
 constexpr int ST_NOCONV = 2;     // sign iteration hit max_sign_iters
 
 enum Phase { PH_FREE = 0, PH_NEW, PH_INV, PH_AMAT, PH_PA, PH_SIGN, PH_FIN };
-enum OpKind { OP_NONE = 0, OP_INV_G1, OP_INV_G2, OP_AMAT, OP_SIGN_G1, OP_SIGN_G2, OP_POW_S, OP_POW_A };
+enum OpKind { OP_NONE = 0, OP_INV_G1, OP_INV_G2, OP_AMAT, OP_SIGN_G1, OP_SIGN_G2, OP_POW_S, OP_POW_A,
+              OP_DCOLS };   // persistent engine: P = X Y[:, cols(i)] as one 16-column tile per 256 rows, FP32 out
 
 struct __align__(16) Slot {
     // geometry of the atom in the slot (written at refill)
@@ -96,6 +98,9 @@ __device__ __forceinline__ __half* c_ptr(const Engine& e, __half* base, int slot
     ldc = e.ld;
     return base + buf_off(e, slot, buf);
 }
+
+// FP32 output block of OP_DCOLS tiles (persistent engine only).
+__device__ __forceinline__ float* pcols_ptr(const Engine&, int) { return nullptr; }
 
 // Tile id -> slot by binary search over SlotOp::tile_start (a slot with ntiles == 0 shares its
 // tile_start with the next slot and is never returned for a valid tile).

@@ -80,6 +80,7 @@ struct PEngine {
     double* e_atom;
     const CUtensorMap* maps;
     __half* base;
+    float* pcols;                 // [S][cap][PCW] FP32: X Y[:, cols(i)] of the slot's atom (OP_DCOLS)
 };
 
 __device__ __forceinline__ long long buf_off(const PEngine& e, int slot, int buf) {
@@ -92,6 +93,8 @@ __device__ __forceinline__ __half* c_ptr(const PEngine& e, __half* base, int slo
     ldc = VLD;
     return base + (long long)e.S * e.slotsz + ((long long)slot * 2 + (buf - NBUF)) * ((long long)e.cap * VLD);
 }
+
+__device__ __forceinline__ float* pcols_ptr(const PEngine& e, int slot) { return e.pcols + (size_t)slot * e.cap * PCW; }
 
 namespace pl {
 __device__ __forceinline__ unsigned long long gtime() {
@@ -155,11 +158,12 @@ __device__ __forceinline__ void p_install_gemm(const PEngine& e, int slot, int k
             a = 0; b = st == 0 ? NMAP - 1 : NBUF + ((st - 1) & 1); c = NBUF + (st & 1);
             c_out = alpha_res = __ldcg(&s->pow_alpha); want = 1;
         } break;
+        case OP_DCOLS: a = xcur; b = ycur; c = 0; break;                                           // P = X Y[:, cols(i)]
         default: break;
     }
     __stcg(reinterpret_cast<int4*>(&s->op_kind), make_int4(kind, a, b, c));
     __stcg(reinterpret_cast<float4*>(&s->c_out), make_float4(c_out, alpha_res, beta, __int_as_float(want)));
-    const bool pow = kind == OP_POW_S || kind == OP_POW_A;
+    const bool pow = kind == OP_POW_S || kind == OP_POW_A || kind == OP_DCOLS;       // one 16-column tile per 256 rows
     const unsigned long long tiles = (unsigned long long)(__ldcg(&s->ntm) * (pow ? 1 : __ldcg(&s->ntn)));
     __threadfence();
     *(volatile unsigned long long*)&e.gclaim[slot] = tiles << 20;
@@ -280,6 +284,11 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
         }
         return;
     }
+    if (kind == OP_DCOLS) {                 // a skinny product, not one of the counted square GEMMs
+        p_leave_heavy(e);
+        p_install_side(e, slot, SK_DCOLS, e.dcols_chunks);
+        return;
+    }
     __stcg(&s->gemm_count, __ldcg(&s->gemm_count) + 1);
     if (kind == OP_INV_G1 || kind == OP_SIGN_G1) {
         const bool inv = kind == OP_INV_G1;
@@ -328,8 +337,7 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
         __stcg(&s->xcur, 1 - __ldcg(&s->xcur));
         if (__ldcg(&s->conv)) {
             __stcg(&s->conv, 0);
-            p_leave_heavy(e);
-            p_install_side(e, slot, SK_DCOLS, e.dcols_chunks);
+            p_install_gemm(e, slot, OP_DCOLS);
         } else {
             p_install_gemm(e, slot, OP_SIGN_G1);
         }
@@ -382,11 +390,11 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
                         const int4 g1 = __ldcg(reinterpret_cast<const int4*>(&s->nbi));      // nbi ntm ntn nset
                         const int4 o0 = __ldcg(reinterpret_cast<const int4*>(&s->op_kind));
                         const float4 o1 = __ldcg(reinterpret_cast<const float4*>(&s->c_out));
-                        const bool pow = o0.x == OP_POW_S || o0.x == OP_POW_A;
+                        const bool pow = o0.x == OP_POW_S || o0.x == OP_POW_A || o0.x == OP_DCOLS;
                         const int ntn = pow ? 1 : g1.z;
                         const int tm = t / ntn, tn = t - tm * ntn;
-                        ti.slot = found; ti.m0 = tm * BM; ti.n0 = tn * BN;
-                        ti.n = g0.y; ti.n16 = g0.z; ti.bn = pow ? NVC : min(BN, g0.z - tn * BN); ti.nreports = 2 * nt;
+                        ti.slot = found; ti.m0 = tm * BM; ti.n0 = o0.x == OP_DCOLS ? (g0.w & ~7) : tn * BN;   // D columns: the aligned window around pos(i)
+                        ti.n = g0.y; ti.n16 = g0.z; ti.bn = o0.x == OP_DCOLS ? PCW : pow ? NVC : min(BN, g0.z - tn * BN); ti.nreports = 2 * nt;
                         ti.kind = o0.x; ti.a_buf = o0.y; ti.b_buf = o0.z; ti.c_buf = o0.w;
                         ti.c_out = o1.x; ti.alpha_res = o1.y; ti.beta = o1.z; ti.want_res = __float_as_int(o1.w);
                     }
@@ -442,94 +450,170 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
 // a1, one chunk of row-atoms of N(i): builds the dense rows of T_i(S) (buffer 0) and T_i(H0) (buffer 1)
 // that belong to row-atoms [a_lo, a_hi) of N(i): block (j_a, j_b) of the sparse matrix where it exists,
 // zeros elsewhere and in the pad strip [n, n16). The last chunk also zeroes rows [n, n16).
+//
+// Data path (HBM-bound work, so it is built around bytes in flight): the source blocks of a row-atom are
+// contiguous runs of nb(j_a) x nb(j_b) values; every warp streams its share of them into a private
+// two-stage staging area with 8-byte cp.async (no registers held while the loads fly), converts each
+// value once (RN-even, C-13) into a shared-memory strip of the dense rows, and the strip
+// leaves with 16-byte coalesced stores. Strips are G_STRIP_BYTES at most, so a row-atom of a wide
+// submatrix takes several passes over row sub-ranges of its blocks.
+constexpr int G_STRIP_BYTES = 28 * 1024;
+constexpr int G_STAGE_BYTES = 3 * 1024;           // per warp and stage
+constexpr int G_MAXI = 8;                         // blocks (or block pieces) per stage
+
+struct GItems {                                   // what one stage of one warp holds (warp-uniform)
+    int n;
+    int off[G_MAXI], nbb[G_MAXI], e0[G_MAXI], take[G_MAXI], at[G_MAXI];
+};
+
+template <typename TV>
+__device__ __forceinline__ void g_cp_async(uint32_t dst, const TV* src) {
+    if constexpr (sizeof(TV) == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+    else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+}
+
 template <typename TV>
 __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_vals, const TV* __restrict__ H_vals,
                                   __half* __restrict__ dstS, __half* __restrict__ dstH, int atom, int n, int n16, int ld,
                                   int chunk, int nchunks, unsigned char* sm, int tid, unsigned long long* bytes) {
     const long long p0 = sv.nset_ptr[atom];
     const int cnt = (int)(sv.nset_ptr[atom + 1] - p0);
+    const int warp = tid >> 5, lane = tid & 31;
+    // shared memory: tables | strip | staging (4 warps x 2 stages)
     int* s_nset = reinterpret_cast<int*>(sm);                              // [cnt] atoms of N(i)
     int* s_off = s_nset + cnt;                                             // [cnt + 1] first column of each atom
-    long long* s_boff = reinterpret_cast<long long*>(sm + (((size_t)(2 * cnt + 1) * 4 + 7) & ~(size_t)7));   // [rows of the chunk][cnt]
+    int* s_list = s_off + cnt + 1;                                         // [cnt] present blocks of the current row-atom
+    int* s_m = s_list + cnt;                                               // [1]
+    long long* s_boff = reinterpret_cast<long long*>(sm + (((size_t)(3 * cnt + 2) * 4 + 15) & ~(size_t)15));   // [cnt]
+    unsigned char* strip_b = reinterpret_cast<unsigned char*>(s_boff) + (((size_t)cnt * 8 + 15) & ~(size_t)15);
+    __half* strip = reinterpret_cast<__half*>(strip_b);
+    unsigned char* stage_b = strip_b + G_STRIP_BYTES + (size_t)warp * 2 * G_STAGE_BYTES;
+    const uint32_t stage_u = ptx::smem_u32(stage_b);
+    constexpr int CAP_E = G_STAGE_BYTES / (int)sizeof(TV);                 // values per stage
+
     const int a_lo = (int)((long long)cnt * chunk / nchunks), a_hi = (int)((long long)cnt * (chunk + 1) / nchunks);
-    const int na = a_hi - a_lo;
-    unsigned short* s_colmap = reinterpret_cast<unsigned short*>(s_boff + (size_t)max(na, 1) * cnt);        // [n16]
-    for (int b = tid; b < cnt; b += P_SIDE_THREADS) {
-        const int k = sv.nset_atom[p0 + b], o = sv.nset_off[p0 + b];
-        s_nset[b] = k; s_off[b] = o;
-        const int nbb = sv.atom_nb[k];
-        for (int c = 0; c < nbb; ++c) s_colmap[o + c] = (unsigned short)b;
-    }
+    for (int b = tid; b < cnt; b += P_SIDE_THREADS) { s_nset[b] = sv.nset_atom[p0 + b]; s_off[b] = sv.nset_off[p0 + b]; }
     if (tid == 0) s_off[cnt] = n;
-    for (int c = n + tid; c < n16; c += P_SIDE_THREADS) s_colmap[c] = 0xFFFF;
-    for (int q = tid; q < na * cnt; q += P_SIDE_THREADS) s_boff[q] = -1;
     pl::side_sync();
-    // CSR rows of the chunk's row-atoms against N(i) (both ascending): every entry looks itself up in N(i)
-    for (int al = 0; al < na; ++al) {
-        const int j = s_nset[a_lo + al];
-        const long long r0 = sv.row_ptr[j], r1 = sv.row_ptr[j + 1];
-        for (long long p = r0 + tid; p < r1; p += P_SIDE_THREADS) {
-            const int k = sv.col_idx[p];
-            int lo = 0, hi = cnt;
-            while (lo < hi) { const int mid = (lo + hi) >> 1; if (s_nset[mid] < k) lo = mid + 1; else hi = mid; }
-            if (lo < cnt && s_nset[lo] == k) s_boff[al * cnt + lo] = sv.blk_off[p];
-        }
-    }
-    pl::side_sync();
+    const int rows_max = max(1, G_STRIP_BYTES / (n16 * 2));
+    const int vpr = n16 >> 3;                                              // 16-byte vectors per dense row
     unsigned long long nread = 0;
-    const int half_n16 = n16 >> 1;
-    constexpr int U = 4;                                                   // column pairs in flight per thread
-    for (int al = 0; al < na; ++al) {
-        const int a = a_lo + al;
+
+    for (int a = a_lo; a < a_hi; ++a) {
+        const int j = s_nset[a];
         const int nbj = s_off[a + 1] - s_off[a], row0 = s_off[a];
-        const int total = nbj * half_n16;                                  // column pairs of this row strip
-        const long long* boff = s_boff + al * cnt;
+        // CSR row of j against N(i) (both ascending): every entry looks itself up in N(i)
+        for (int b = tid; b < cnt; b += P_SIDE_THREADS) s_boff[b] = -1;
+        pl::side_sync();
+        {
+            const long long r0 = sv.row_ptr[j], r1 = sv.row_ptr[j + 1];
+            for (long long p = r0 + tid; p < r1; p += P_SIDE_THREADS) {
+                const int k = sv.col_idx[p];
+                int lo = 0, hi = cnt;
+                while (lo < hi) { const int mid = (lo + hi) >> 1; if (s_nset[mid] < k) lo = mid + 1; else hi = mid; }
+                if (lo < cnt && s_nset[lo] == k) s_boff[lo] = sv.blk_off[p];
+            }
+        }
+        pl::side_sync();
+        if (warp == 0) {                                                   // compact list of the present blocks
+            int m = 0;
+            for (int base = 0; base < cnt; base += 32) {
+                const int b = base + lane;
+                const bool pr = b < cnt && s_boff[b] >= 0;
+                const unsigned mask = __ballot_sync(0xffffffffu, pr);
+                if (pr) s_list[m + __popc(mask & ((1u << lane) - 1u))] = b;
+                m += __popc(mask);
+            }
+            if (lane == 0) *s_m = m;
+        }
+        pl::side_sync();
+        const int m = *s_m;
 #pragma unroll 1
         for (int which = 0; which < 2; ++which) {
             const TV* __restrict__ vals = which ? H_vals : S_vals;
             __half* __restrict__ dst = which ? dstH : dstS;
 #pragma unroll 1
-            for (int idx0 = tid; idx0 < total; idx0 += U * P_SIDE_THREADS) {
-                TV v[2 * U];
-                long long o[U];
+            for (int r0 = 0; r0 < nbj; r0 += rows_max) {
+                const int nr = min(rows_max, nbj - r0);
+                {   // zero the strip
+                    const uint4 z = make_uint4(0, 0, 0, 0);
+                    uint4* s4 = reinterpret_cast<uint4*>(strip);
+                    for (int q = tid; q < nr * vpr; q += P_SIDE_THREADS) s4[q] = z;
+                }
+                pl::side_sync();
+                // ---- each warp streams its blocks (list entries warp, warp + 4, ...) through its two stages ----
+                int li = warp, e_next = 0;
+                auto fill = [&](int st, GItems& it) {
+                    it.n = 0;
+                    int used = 0;
+                    while (li < m && it.n < G_MAXI) {
+                        const int b = s_list[li];
+                        const int nbb = s_off[b + 1] - s_off[b];
+                        const int bs = nr * nbb, rem = bs - e_next;
+                        const int take = min(rem, CAP_E - used);
+                        if (take <= 0 || (take < rem && used > 0)) break;      // a block is split only across empty stages
+                        const TV* src = vals + s_boff[b] + (long long)r0 * nbb + e_next;
+                        const uint32_t d0 = stage_u + (uint32_t)(st * G_STAGE_BYTES) + (uint32_t)used * (uint32_t)sizeof(TV);
+                        for (int e = lane; e < take; e += 32) g_cp_async<TV>(d0 + (uint32_t)e * (uint32_t)sizeof(TV), src + e);
+                        it.off[it.n] = s_off[b]; it.nbb[it.n] = nbb; it.e0[it.n] = e_next; it.take[it.n] = take; it.at[it.n] = used;
+                        ++it.n;
+                        used += take; e_next += take; nread += (lane == 0) ? (unsigned long long)take : 0ull;
+                        if (e_next == bs) { li += P_SIDE_WARPS; e_next = 0; }
+                    }
+                    pl::cp_async_commit();
+                };
+                auto convert = [&](int st, const GItems& it) {
+                    const TV* sv_ = reinterpret_cast<const TV*>(stage_b + st * G_STAGE_BYTES);
 #pragma unroll
-                for (int u = 0; u < U; ++u) {
-                    const int idx = idx0 + u * P_SIDE_THREADS;
-                    v[2 * u] = (TV)0; v[2 * u + 1] = (TV)0; o[u] = -1;
-                    if (idx < total) {
-                        const int rr = idx / half_n16;
-                        const int c = (idx - rr * half_n16) << 1;
-                        o[u] = (long long)(row0 + rr) * ld + c;
-                        const unsigned b0 = s_colmap[c], b1 = s_colmap[c + 1];
-                        if (b0 != 0xFFFFu) {
-                            const long long bo = boff[b0];
-                            if (bo >= 0) { v[2 * u] = __ldg(vals + bo + (long long)rr * (s_off[b0 + 1] - s_off[b0]) + (c - s_off[b0])); ++nread; }
-                        }
-                        if (b1 != 0xFFFFu) {
-                            const long long bo = boff[b1];
-                            if (bo >= 0) { v[2 * u + 1] = __ldg(vals + bo + (long long)rr * (s_off[b1 + 1] - s_off[b1]) + (c + 1 - s_off[b1])); ++nread; }
+                    for (int q = 0; q < G_MAXI; ++q) {
+                        if (q < it.n) {
+                            const int nbb = it.nbb[q];
+                            for (int e = lane; e < it.take[q]; e += 32) {
+                                const int idx = it.e0[q] + e;
+                                const int rr = idx / nbb, cc = idx - rr * nbb;
+                                strip[rr * n16 + it.off[q] + cc] = Num<__half>::from_d((double)sv_[it.at[q] + e]);
+                            }
                         }
                     }
+                };
+                GItems ia, ib;
+                fill(0, ia);
+                for (;;) {
+                    fill(1, ib);
+                    pl::cp_async_wait<1>();
+                    convert(0, ia);
+                    __syncwarp();                      // stage 0 is refilled next
+                    if (ib.n == 0) break;
+                    fill(0, ia);
+                    pl::cp_async_wait<1>();
+                    convert(1, ib);
+                    __syncwarp();
+                    if (ia.n == 0) break;
                 }
-#pragma unroll
-                for (int u = 0; u < U; ++u)
-                    if (o[u] >= 0)
-                        *reinterpret_cast<__half2*>(dst + o[u]) = __halves2half2(Num<__half>::from_d((double)v[2 * u]), Num<__half>::from_d((double)v[2 * u + 1]));
+                pl::cp_async_wait<0>();
+                pl::side_sync();
+                // ---- the strip leaves with 16-byte stores ----
+                {
+                    const uint4* s4 = reinterpret_cast<const uint4*>(strip);
+                    for (int q = tid; q < nr * vpr; q += P_SIDE_THREADS) {
+                        const int rr = q / vpr, v = q - rr * vpr;
+                        *reinterpret_cast<uint4*>(dst + (long long)(row0 + r0 + rr) * ld + v * 8) = s4[q];
+                    }
+                }
+                pl::side_sync();
             }
         }
     }
     if (chunk == nchunks - 1) {
-        const __half2 z = __floats2half2_rn(0.f, 0.f);
-        for (int idx = tid; idx < (n16 - n) * half_n16; idx += P_SIDE_THREADS) {
-            const int rr = idx / half_n16, c = (idx - rr * half_n16) << 1;
-            *reinterpret_cast<__half2*>(dstS + (long long)(n + rr) * ld + c) = z;
-            *reinterpret_cast<__half2*>(dstH + (long long)(n + rr) * ld + c) = z;
+        const uint4 z = make_uint4(0, 0, 0, 0);
+        for (int idx = tid; idx < (n16 - n) * vpr; idx += P_SIDE_THREADS) {
+            const int rr = idx / vpr, v = idx - rr * vpr;
+            *reinterpret_cast<uint4*>(dstS + (long long)(n + rr) * ld + v * 8) = z;
+            *reinterpret_cast<uint4*>(dstH + (long long)(n + rr) * ld + v * 8) = z;
         }
     }
     if (bytes) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) nread += __shfl_xor_sync(0xffffffffu, nread, o);
-        if ((tid & 31) == 0 && nread) atomicAdd(bytes, nread * sizeof(TV));                          // source values read
+        if (lane == 0 && nread) atomicAdd(bytes, nread * sizeof(TV));                                  // source values read
         if (tid == 0) atomicAdd(bytes, (unsigned long long)(s_off[a_hi] - s_off[a_lo]) * n16 * 4ull); // dense FP16 rows written (S and H0)
     }
 }
@@ -575,99 +659,42 @@ __device__ void side_schulz1_chunk(const __half* __restrict__ S, __half* __restr
     }
 }
 
-// a6 + a7, rows [r_lo, r_hi) of the submatrix: D_sub[r, cols(i)] = 1/2 (Y[r, cols] - X[r, :] Y[:, cols]),
-// written to slot (i, j) of the output as (D_ji)^T, and the energy partial sum_j <D_ji, H0_ji> in FP64.
+// a6 + a7, one chunk of the values of output row i (slot (i, j) holds (D_ji)^T, C-10):
+// D_sub[r, pos + c] = 1/2 (Y[r, pos + c] - P[r, c]) with P = X Y[:, cols(i)] from the OP_DCOLS tiles, and the
+// energy partial sum <D_ji, H0_ji> in FP64 (Eq. 4). One thread per output value, in output
+// order: the block-CSR arrays (D out, H0 in) are touched with coalesced accesses, the small L2-resident
+// operands (Y columns, P) with scattered ones.
 template <typename TV, typename TD>
-__device__ void side_dcols_chunk(const SysView& sv, const __half* __restrict__ X, const __half* __restrict__ Y,
+__device__ void side_dcols_chunk(const SysView& sv, const float* __restrict__ P, const __half* __restrict__ Y,
                                  const TV* __restrict__ H_vals, TD* __restrict__ D_vals, double* e_atom,
-                                 int atom, int n, int n16, int ld, int pos, int nbi, int chunk, int nchunks, unsigned char* sm, int tid) {
+                                 int atom, int n, int ld, int pos, int nbi, int chunk, int nchunks, unsigned char* sm, int tid) {
     const long long p0 = sv.nset_ptr[atom];
     const int cnt = (int)(sv.nset_ptr[atom + 1] - p0);
-    int* s_off = reinterpret_cast<int*>(sm);                               // [cnt + 1]
-    __half* yt = reinterpret_cast<__half*>(sm + (((size_t)(cnt + 1) * 4 + 15) & ~(size_t)15));   // [nbi][n16]: Y[:, cols]^T
+    int* s_off = reinterpret_cast<int*>(sm);                               // [cnt + 1] first row of each atom of N(i)
     for (int b = tid; b < cnt; b += P_SIDE_THREADS) s_off[b] = sv.nset_off[p0 + b];
     if (tid == 0) s_off[cnt] = n;
-    const unsigned short* Yu = reinterpret_cast<const unsigned short*>(Y);
-    unsigned short* ytu = reinterpret_cast<unsigned short*>(yt);
-    {
-        constexpr int U = 8;
-        const int total = n16 * nbi;
-#pragma unroll 1
-        for (int idx0 = tid; idx0 < total; idx0 += U * P_SIDE_THREADS) {
-            unsigned short v[U];
-#pragma unroll
-            for (int q = 0; q < U; ++q) {
-                const int idx = idx0 + q * P_SIDE_THREADS;
-                v[q] = 0;
-                if (idx < total) {
-                    const int k = idx / nbi, c = idx - k * nbi;
-                    if (k < n) v[q] = __ldcg(Yu + (long long)k * ld + pos + c);
-                }
-            }
-#pragma unroll
-            for (int q = 0; q < U; ++q) {
-                const int idx = idx0 + q * P_SIDE_THREADS;
-                if (idx < total) { const int k = idx / nbi, c = idx - k * nbi; ytu[c * n16 + k] = v[q]; }
-            }
-        }
-    }
     pl::side_sync();
-    const int warp = tid >> 5, lane = tid & 31;
-    const int r_lo = (int)((long long)n * chunk / nchunks), r_hi = (int)((long long)n * (chunk + 1) / nchunks);
-    const int ppr = n16 >> 3;
+    // the slots of row i that belong to N(i) are stored one after the other only when nothing is filtered, so
+    // the output offset of atom a is looked up; value q of the chunk = (atom a, column c, row bb) in output order
+    const int total = n * nbi;                                             // values of D written for this atom
+    const int q_lo = (int)((long long)total * chunk / nchunks), q_hi = (int)((long long)total * (chunk + 1) / nchunks);
     double e_part = 0.0;
-    constexpr int XP = P_MAX_CAP / 8 / 32;                                 // 16-byte pieces of an X row per lane (at most)
-    for (int r = r_lo + warp; r < r_hi; r += P_SIDE_WARPS) {
-        const __half* xrow = X + (long long)r * ld;
-        uint4 xr[XP];
-#pragma unroll
-        for (int q = 0; q < XP; ++q) {
-            const int p = lane + 32 * q;
-            xr[q] = p < ppr ? __ldcg(reinterpret_cast<const uint4*>(xrow + p * 8)) : make_uint4(0, 0, 0, 0);
-        }
-        int lo = 0, hi = cnt - 1;                                          // atom of N(i) that owns row r
-        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_off[mid] <= r) lo = mid; else hi = mid - 1; }
-        const int a = lo, bb = r - s_off[a], nbj = s_off[a + 1] - s_off[a];
-        const long long out0 = sv.blk_off[sv.nset_slot[p0 + a]];
-        for (int c0 = 0; c0 < nbi; c0 += 16) {
-            const int nc = min(16, nbi - c0);
-            float acc[16];
-#pragma unroll
-            for (int c = 0; c < 16; ++c) acc[c] = 0.f;
-#pragma unroll
-            for (int q = 0; q < XP; ++q) {
-                const int p = lane + 32 * q;
-                if (p < ppr) {
-                    const __half2* xh = reinterpret_cast<const __half2*>(&xr[q]);
-                    const float2 x01 = __half22float2(xh[0]), x23 = __half22float2(xh[1]), x45 = __half22float2(xh[2]), x67 = __half22float2(xh[3]);
-                    const float4 xa = make_float4(x01.x, x01.y, x23.x, x23.y), xb = make_float4(x45.x, x45.y, x67.x, x67.y);
-#pragma unroll
-                    for (int c = 0; c < 16; ++c)
-                        if (c < nc) {
-                            const uint4 yu = *reinterpret_cast<const uint4*>(yt + (size_t)(c0 + c) * n16 + p * 8);
-                            acc[c] += pl::dot8(yu, xa, xb);
-                        }
-                }
-            }
-#pragma unroll
-            for (int c = 0; c < 16; ++c)
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], o);
-            float mine = 0.f;
-#pragma unroll
-            for (int c = 0; c < 16; ++c) if (lane == c) mine = acc[c];
-            if (lane < nc) {
-                const int c = c0 + lane;
-                const float d = 0.5f * (__half2float(yt[(size_t)c * n16 + r]) - mine);
-                const long long o = out0 + (long long)c * nbj + bb;        // slot (i, j_a): [c][bb] = D_sub[r, pos + c]
-                D_vals[o] = (TD)d;
-                e_part += (double)d * (double)H_vals[o];
-            }
-        }
+    for (int q = q_lo + tid; q < q_hi; q += P_SIDE_THREADS) {
+        // rows of atom a start at s_off[a]; its values start at s_off[a] * nbi in this ordering
+        int lo = 0, hi = cnt - 1;
+        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_off[mid] * nbi <= q) lo = mid; else hi = mid - 1; }
+        const int a = lo, nbj = s_off[a + 1] - s_off[a];
+        const int rem = q - s_off[a] * nbi;
+        const int c = rem / nbj, bb = rem - c * nbj;
+        const int r = s_off[a] + bb;
+        const long long o = sv.blk_off[sv.nset_slot[p0 + a]] + rem;       // slot (i, j_a): [c][bb] = D_sub[r, pos + c]
+        const float d = 0.5f * (__half2float(__ldcg(Y + (long long)r * ld + pos + c)) - __ldcg(P + (size_t)r * PCW + (pos & 7) + c));
+        D_vals[o] = (TD)d;
+        e_part += (double)d * (double)H_vals[o];
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) e_part += __shfl_xor_sync(0xffffffffu, e_part, o);
-    if (lane == 0 && e_part != 0.0) atomicAdd(&e_atom[atom], e_part);
+    if ((tid & 31) == 0 && e_part != 0.0) atomicAdd(&e_atom[atom], e_part);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -722,14 +749,14 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
                 side_schulz1_chunk(e.base + buf_off(e, slot, 0), e.base + buf_off(e, slot, 2), n, n16, e.ld, __ldcg(&s->rho_s), chunk, nch, tid);
                 break;
             case SK_DCOLS: {
-                const __half* X = e.base + buf_off(e, slot, __ldcg(&s->xcur));
+                const float* P = pcols_ptr(e, slot);
                 const __half* Y = e.base + buf_off(e, slot, __ldcg(&s->ycur));
                 if (e.val_f64) {
-                    if (e.d_f64) side_dcols_chunk<double, double>(e.sv, X, Y, (const double*)e.H_vals, (double*)e.D_vals, e.e_atom, atom, n, n16, e.ld, pos, nbi, chunk, nch, sm, tid);
-                    else side_dcols_chunk<double, float>(e.sv, X, Y, (const double*)e.H_vals, (float*)e.D_vals, e.e_atom, atom, n, n16, e.ld, pos, nbi, chunk, nch, sm, tid);
+                    if (e.d_f64) side_dcols_chunk<double, double>(e.sv, P, Y, (const double*)e.H_vals, (double*)e.D_vals, e.e_atom, atom, n, e.ld, pos, nbi, chunk, nch, sm, tid);
+                    else side_dcols_chunk<double, float>(e.sv, P, Y, (const double*)e.H_vals, (float*)e.D_vals, e.e_atom, atom, n, e.ld, pos, nbi, chunk, nch, sm, tid);
                 } else {
-                    if (e.d_f64) side_dcols_chunk<float, double>(e.sv, X, Y, (const float*)e.H_vals, (double*)e.D_vals, e.e_atom, atom, n, n16, e.ld, pos, nbi, chunk, nch, sm, tid);
-                    else side_dcols_chunk<float, float>(e.sv, X, Y, (const float*)e.H_vals, (float*)e.D_vals, e.e_atom, atom, n, n16, e.ld, pos, nbi, chunk, nch, sm, tid);
+                    if (e.d_f64) side_dcols_chunk<float, double>(e.sv, P, Y, (const float*)e.H_vals, (double*)e.D_vals, e.e_atom, atom, n, e.ld, pos, nbi, chunk, nch, sm, tid);
+                    else side_dcols_chunk<float, float>(e.sv, P, Y, (const float*)e.H_vals, (float*)e.D_vals, e.e_atom, atom, n, e.ld, pos, nbi, chunk, nch, sm, tid);
                 }
             } break;
             default: break;                       // SK_REFILL: nothing to compute
@@ -753,7 +780,7 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
                     case SK_DCOLS: {
                         const double nv = (double)(e.sv.blk_off[e.sv.row_ptr[atom + 1]] - e.sv.blk_off[e.sv.row_ptr[atom]]);
                         atomicAdd(&e.ctr[PC_SIDE_BYTES + SK_DCOLS],
-                                  (unsigned long long)(nv * ((e.d_f64 ? 8 : 4) + (e.val_f64 ? 8 : 4)) + ((double)n * n + (double)n * nbi) * 2.0));
+                                  (unsigned long long)(nv * ((e.d_f64 ? 8 : 4) + (e.val_f64 ? 8 : 4)) + (double)n * PCW * 4.0 + (double)n * nbi * 2.0));
                         p_retire(e, slot);
                     } break;
                     default: break;

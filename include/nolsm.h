@@ -77,6 +77,9 @@ typedef struct {
                                 [alpha (3 - alpha^2) / 2, 1]; two steps with the optimal scalings for that interval follow,
                                 then plain Eq. 6 until the convergence test passes (C-6b) [6; -1 = plain Eq. 6] */
     float sign_scale;        /* alpha of the scaled steps, 1 < alpha < sqrt(3) [1.5] */
+    int cluster_ctas;        /* persistent engine, CTAs per thread-block cluster: 2 = one tcgen05 CTA pair per 256 x 256 tile;
+                                4 = two pairs on a 256 x 512 tile with the A operand TMA-multicast between them (less
+                                L2 -> SM traffic, but only 132 of 148 SMs can hold 4-CTA clusters on B200) [2] */
 } nolsm_options;
 
 typedef struct {

@@ -22,7 +22,8 @@ class NolsmOptions(C.Structure):
                 ("max_sign_iters", C.c_int), ("tol_inv", C.c_float), ("tol_sign", C.c_float),
                 ("power_iters_s", C.c_int), ("power_iters_a", C.c_int), ("eps_filter", C.c_double),
                 ("batch_atoms", C.c_int), ("workspace_bytes", C.c_size_t), ("profile_every", C.c_int),
-                ("engine", C.c_int), ("sign_scaled_iters", C.c_int), ("sign_scale", C.c_float)]
+                ("engine", C.c_int), ("sign_scaled_iters", C.c_int), ("sign_scale", C.c_float),
+                ("cluster_ctas", C.c_int)]
 
 
 class NolsmStats(C.Structure):
@@ -43,7 +44,8 @@ class NolsmError(RuntimeError):
 
 
 def lib_path() -> str:
-    return os.path.join(_HERE, "libnolsm.so")
+    """In-tree library; NOLSM_LIB names another build of the same sources (probe builds with timing counters)."""
+    return os.environ.get("NOLSM_LIB") or os.path.join(_HERE, "libnolsm.so")
 
 
 def load_library():

@@ -81,6 +81,7 @@ struct nolsm_ctx {
     bool persist = false;
     PEngine peng{};
     int* d_abort = nullptr;
+    int p_grid = 0;                     // CTAs of the persistent kernel: 4 x the clusters that can be resident together
     cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr;
     int h_a0 = 0;
     unsigned long long h_ctr0[PC_LEN] = {};
@@ -369,6 +370,8 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
     if (getenv("NOLSM_SIGN_SCALED_ITERS")) o.sign_scaled_iters = getenv_int("NOLSM_SIGN_SCALED_ITERS", 6);
     if (o.sign_scaled_iters < 0) o.sign_scaled_iters = 0;
     if (o.sign_scaled_iters > 14) o.sign_scaled_iters = 14;
+    if (getenv_int("NOLSM_CLUSTER", 0) > 0) o.cluster_ctas = getenv_int("NOLSM_CLUSTER", 0);
+    if (o.cluster_ctas != 0 && o.cluster_ctas != 2 && o.cluster_ctas != 4) { delete c; return NOLSM_EINVAL; }
     if (o.sign_scale == 0.f) o.sign_scale = 1.5f;
     if (const char* v = getenv("NOLSM_SIGN_SCALE")) o.sign_scale = (float)atof(v);
     if (!(o.sign_scale > 1.f && o.sign_scale < 1.7320508f)) { delete c; return NOLSM_EINVAL; }
@@ -393,7 +396,8 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
     if (!ok) { cudaGetLastError(); delete c; return NOLSM_ECUDA; }
     if (use_umma(c)) {
         if (cudaFuncSetAttribute(gemm2_round_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, G2_SMEM_BYTES) != cudaSuccess ||
-            cudaFuncSetAttribute(nolsm_persist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES) != cudaSuccess) {
+            cudaFuncSetAttribute(nolsm_persist_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES) != cudaSuccess ||
+            cudaFuncSetAttribute(nolsm_persist_kernel<G4_CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES) != cudaSuccess) {
             cudaGetLastError();
             delete c;
             return NOLSM_ECUDA;
@@ -712,6 +716,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         }
         pe.g_max = std::max(1, std::min(g_max, S));
         pe.want_lead = std::max(1, getenv_int("NOLSM_WANT_LEAD", G2_WANT_LEAD));
+        pe.dbg = getenv_int("NOLSM_DBG", 0);
         pe.schulz_chunks = std::max(1, getenv_int("NOLSM_SCHULZ_CHUNKS", 16));
         pe.dcols_chunks = std::max(1, getenv_int("NOLSM_DCOLS_CHUNKS", 4));
         pe.next_atom = e.next_atom; pe.finished = e.finished; pe.abort_flag = c->d_abort;
@@ -719,6 +724,21 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         pe.S_vals = c->dS; pe.H_vals = c->dH; pe.val_f64 = val_dtype == NOLSM_DTYPE_F64;
         pe.e_atom = c->d_e_atom; pe.maps = c->d_maps; pe.base = (__half*)c->ws;
         c->h_sclaim0.assign(S, ((unsigned)SK_REFILL << 28) | (1u << 14));
+        {   // every CTA waits on work published by the others: the whole grid must be resident at once
+            const int ctas = c->opt.cluster_ctas == G4_CTAS ? G4_CTAS : 2;
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3((unsigned)(c->sms / ctas * ctas)); cfg.blockDim = dim3(P_THREADS); cfg.dynamicSmemBytes = P_SMEM_BYTES;
+            cudaLaunchAttribute at;
+            at.id = cudaLaunchAttributeClusterDimension;
+            at.val.clusterDim.x = ctas; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
+            cfg.attrs = &at; cfg.numAttrs = 1;
+            int ncl = 0;
+            if (ctas == G4_CTAS) CU_TRY(c, cudaOccupancyMaxActiveClusters(&ncl, nolsm_persist_kernel<G4_CTAS>, &cfg));
+            else CU_TRY(c, cudaOccupancyMaxActiveClusters(&ncl, nolsm_persist_kernel<2>, &cfg));
+            if (ncl < 1) return fail(c, NOLSM_ECUDA, "no cluster of the persistent kernel fits on this device");
+            c->p_grid = ctas * std::min(ncl, c->sms / ctas);
+            pe.ctas = ctas;
+        }
         CU_TRY(c, cudaFuncSetAttribute(k_side_gather<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SIDE_SMEM));
         CU_TRY(c, cudaFuncSetAttribute(k_side_gather<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SIDE_SMEM));
     }
@@ -781,7 +801,16 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
         CU_TRY(c, cudaMemsetAsync(pe.heavy, 0, 4, s));
         CU_TRY(c, cudaMemsetAsync(pe.parked, 0, 4 * pe.S, s));
         CU_TRY(c, cudaEventRecord(c->ev_k0, s));
-        nolsm_persist_kernel<<<c->sms & ~1, P_THREADS, P_SMEM_BYTES, s>>>(pe);
+        {
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3((unsigned)c->p_grid); cfg.blockDim = dim3(P_THREADS); cfg.dynamicSmemBytes = P_SMEM_BYTES; cfg.stream = s;
+            cudaLaunchAttribute at;
+            at.id = cudaLaunchAttributeClusterDimension;
+            at.val.clusterDim.x = pe.ctas; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
+            cfg.attrs = &at; cfg.numAttrs = 1;
+            if (pe.ctas == G4_CTAS) CU_TRY(c, cudaLaunchKernelEx(&cfg, nolsm_persist_kernel<G4_CTAS>, pe));
+            else CU_TRY(c, cudaLaunchKernelEx(&cfg, nolsm_persist_kernel<2>, pe));
+        }
         CU_TRY(c, cudaGetLastError());
         CU_TRY(c, cudaEventRecord(c->ev_k1, s));
         c->launches = 1;
@@ -1060,9 +1089,21 @@ int nolsm_get_engine_counters(nolsm_ctx* c, double* out, int n) {
     CU_TRY(c, cudaMemcpy(ct, c->peng.ctr, sizeof(ct), cudaMemcpyDeviceToHost));
     float kms = 0;
     CU_TRY(c, cudaEventElapsedTime(&kms, c->ev_k0, c->ev_k1));
+#ifdef NOLSM_TIMING
+    {
+        unsigned long long t[16];
+        cudaMemcpyFromSymbol(t, g4_timing, sizeof(t));
+        static const char* nm[16] = {"mma_take", "mma_tempty", "mma_full", "mma_total", "epi_take", "epi_tfull(cum)", "epi_work(cum)", "epi_done(cum)",
+                                     "prod_empty", "prod_total", "prod_take", "mma_fulltile_cyc", "mma_fulltiles", "", "", ""};
+        for (int i = 0; i < 13; ++i) fprintf(stderr, "g4_timing %-16s %.3f Gcyc\n", nm[i], t[i] * 1e-9);
+        if (t[12]) fprintf(stderr, "g4_timing cycles per full-width tile (tempty wait + k-loop): %.0f\n", (double)t[11] / (double)t[12]);
+        unsigned long long z[16] = {};
+        cudaMemcpyToSymbol(g4_timing, z, sizeof(z));
+    }
+#endif
     out[0] = 1; out[1] = kms; out[2] = (double)(ct[PC_T_END] - ct[PC_T_START]) * 1e-6;
     out[3] = (double)ct[PC_TILES]; out[4] = ct[PC_SCHED_IDLE_NS] * 1e-6; out[5] = ct[PC_SCHED_BUSY_NS] * 1e-6;
-    out[6] = (double)ct[PC_OVERSHOOT]; out[7] = c->peng.S; out[8] = (c->sms & ~1) / 2;
+    out[6] = (double)ct[PC_OVERSHOOT]; out[7] = c->peng.S; out[8] = c->p_grid / 2;
     for (int k = 0; k < 8; ++k) {
         out[9 + k] = ct[PC_SIDE_NS + k] * 1e-6;
         out[17 + k] = (double)ct[PC_SIDE_BYTES + k];

@@ -1,6 +1,6 @@
 // Persistent engine: the whole hot path a1-a7 of one nolsm_density_matrix call in ONE kernel launch.
 //
-// grid = one CTA per SM in clusters of two (CTA pairs); every CTA runs
+// grid = one CTA per SM in clusters of four (two CTA pairs that share the A operand, gemm4sm.cuh); every CTA runs
 //   warps 0-10   the grouped tcgen05 GEMM pipeline of gemm2sm.cuh (epilogue x 8, tile scheduler, TMA
 //                producer, MMA issuer), fed from a device-side claim table instead of a static tile list;
 //   warps 11-14  a SIDE GROUP that executes the O(n^2) steps of the path as small tasks: gather
@@ -24,7 +24,7 @@
 // fence.proxy.async after the claim. Slot state is read and written with .cg accesses (L1 is not
 // coherent across SMs).
 #pragma once
-#include "gemm2sm.cuh"
+#include "gemm4sm.cuh"
 #include "kernels.cuh"
 
 namespace nolsm {
@@ -69,7 +69,8 @@ struct PEngine {
     int* finished;
     int* heavy;                   // [1] slots inside the GEMM-heavy phases INV .. SIGN right now (at most g_max)
     int* parked;                  // [S] 1 = the slot finished its first Schulz step and waits for a heavy token
-    int g_max, want_lead;
+    int g_max, want_lead, dbg;
+    int ctas;                     // CTAs per cluster of the running kernel: 2 (pair tiles, gemm2sm.cuh) or 4 (A shared by two pairs, gemm4sm.cuh)
     int n_sched; float alpha_sched[16];   // scaled Newton-Schulz: alpha_k of sign iteration k < n_sched (1 afterwards)
     volatile int* abort_flag;     // device word; the host sets it (copy on another stream) to stop a kernel that overran its time limit
     unsigned long long* ctr;      // [PC_LEN]
@@ -222,6 +223,7 @@ __device__ __forceinline__ bool p_refill(const PEngine& e, int slot) {
     const int n = e.at.dim[a], n16 = (n + 15) & ~15;
     int ntm, ntn;
     choose_tiling(n16, ntm, ntn);
+    if (e.ctas == G4_CTAS) ntn = g4_ntn(n16);                           // cluster tiles per row of tiles
     const int nset = (int)(e.sv.nset_ptr[a + 1] - e.sv.nset_ptr[a]);
     __stcg(reinterpret_cast<int4*>(&s->atom), make_int4(a, n, n16, e.at.pos[a]));
     __stcg(reinterpret_cast<int4*>(&s->nbi), make_int4(e.at.nb[a], ntm, ntn, nset));
@@ -348,6 +350,7 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
 // Tile scheduler of the persistent engine (leader CTA, one warp): claims tiles from gclaim[] in slot
 // order and publishes them to both CTAs of the pair.
 // ------------------------------------------------------------------------------------------------
+template <int CTAS>
 __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, int lane) {
     int q = 0; uint32_t ph = 0;
     unsigned long long idle_ns = 0, ntiles = 0, overshoot = 0;
@@ -393,8 +396,15 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
                         const bool pow = o0.x == OP_POW_S || o0.x == OP_POW_A || o0.x == OP_DCOLS;
                         const int ntn = pow ? 1 : g1.z;
                         const int tm = t / ntn, tn = t - tm * ntn;
-                        ti.slot = found; ti.m0 = tm * BM; ti.n0 = o0.x == OP_DCOLS ? (g0.w & ~7) : tn * BN;   // D columns: the aligned window around pos(i)
-                        ti.n = g0.y; ti.n16 = g0.z; ti.bn = o0.x == OP_DCOLS ? PCW : pow ? NVC : min(BN, g0.z - tn * BN); ti.nreports = 2 * nt;
+                        ti.slot = found; ti.m0 = tm * BM;
+                        if (o0.x == OP_DCOLS) { ti.n0 = g0.w & ~7; ti.bn = PCW; }          // D columns: the aligned window around pos(i), pair 0 only
+                        else if (pow) { ti.n0 = 0; ti.bn = NVC; }                          // pair 0 only
+                        else if (CTAS == G4_CTAS) {
+                            int n0, bn0, bn1;
+                            g4_cols(g0.z, tn, n0, bn0, bn1);
+                            ti.n0 = n0; ti.bn = bn0 | (bn1 << 16);
+                        } else { ti.n0 = tn * BN; ti.bn = min(BN, g0.z - tn * BN); }
+                        ti.n = g0.y; ti.n16 = g0.z; ti.nreports = CTAS * nt;
                         ti.kind = o0.x; ti.a_buf = o0.y; ti.b_buf = o0.z; ti.c_buf = o0.w;
                         ti.c_out = o1.x; ti.alpha_res = o1.y; ti.beta = o1.z; ti.want_res = __float_as_int(o1.w);
                     }
@@ -419,14 +429,12 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
             if (lane == i) mine = v;
         }
         if (lane < 16) {
-            asm volatile("st.shared.u32 [%0], %1;" ::"r"(sm.tinfo(q) + 4u * lane), "r"(mine) : "memory");
-            ptx::st_cluster_u32(ptx::mapa(sm.tinfo(q), 1) + 4u * lane, mine);
+#pragma unroll
+            for (uint32_t rk = 0; rk < (uint32_t)CTAS; ++rk)
+                ptx::st_cluster_u32(ptx::mapa(sm.tinfo(q), rk) + 4u * lane, mine);
         }
         __syncwarp();
-        if (lane == 0) {
-            ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_full(q), 0));
-            ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_full(q), 1));
-        }
+        if (lane < CTAS) ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_full(q), (uint32_t)lane));
         if (!got) break;
         if (++q == G2_NTI) { q = 0; ph ^= 1; }
     }
@@ -798,7 +806,9 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
 // ================================================================================================
 // The kernel.
 // ================================================================================================
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(P_THREADS, 1)
+// CTAS = CTAs per cluster (set at launch): 2 = pair tiles (gemm2sm.cuh), 4 = two pairs sharing A (gemm4sm.cuh).
+template <int CTAS>
+__global__ void __launch_bounds__(P_THREADS, 1)
 nolsm_persist_kernel(const __grid_constant__ PEngine e) {
     extern __shared__ uint8_t smem_raw[];
     G2Smem sm;
@@ -806,17 +816,23 @@ nolsm_persist_kernel(const __grid_constant__ PEngine e) {
     uint8_t* side_sm = smem_raw + (sm.base - ptx::smem_u32(smem_raw)) + (G2_SMEM_BYTES - 1024);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = ptx::cluster_ctarank();
+    auto done = [&](const TileInfo& ti) { p_tile_finished(e, ti.slot, ti.nreports); };
 
-    const uint32_t tmem_base = g2_setup(sm, warp, lane);
+    uint32_t tmem_base;
+    if constexpr (CTAS == G4_CTAS) tmem_base = g4_setup(sm, warp, lane);
+    else tmem_base = g2_setup(sm, warp, lane);
 
     if (warp < G2_EPI_WARPS) {
-        g2_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, [&](const TileInfo& ti) { p_tile_finished(e, ti.slot, ti.nreports); });
+        if constexpr (CTAS == G4_CTAS) g4_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, done);
+        else g2_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, done);
     } else if (warp == G2_WARP_SCHED) {
-        if (rank == 0) p_scheduler(sm, e, lane);
+        if (rank == 0) p_scheduler<CTAS>(sm, e, lane);
     } else if (warp == G2_WARP_TMA) {
-        g2_producer(sm, e.maps, rank, lane, e.want_lead);
+        if constexpr (CTAS == G4_CTAS) g4_producer(sm, e.maps, rank, lane, e.want_lead, e.dbg);
+        else g2_producer(sm, e.maps, rank, lane, e.want_lead);
     } else if (warp == G2_WARP_MMA) {
-        if (rank == 0) g2_mma(sm, tmem_base, lane);
+        if constexpr (CTAS == G4_CTAS) { if ((rank & 1u) == 0) g4_mma(sm, tmem_base, rank, lane, e.dbg); }
+        else { if (rank == 0) g2_mma(sm, tmem_base, lane); }
     } else {
         p_side_loop(e, side_sm, (int)threadIdx.x - G2_CTRL_THREADS);
     }

@@ -168,6 +168,34 @@ def test_small_proxies_mixed(name, n_atoms, sample, engine):
     assert cmp["rel_dE"] <= TOL_MIXED_E
 
 
+def test_cluster4_engine_matches_oracle():
+    """cluster_ctas = 4: two CTA pairs per 256 x 512 tile with the A operand TMA-multicast between them
+    (gemm4sm.cuh); ragged tails in both tile directions (cfg2 proxy, n ~ 900-1500)."""
+    s = make_system("cfg2", n_atoms=300)
+    atoms = np.random.default_rng(3).choice(s.n_atoms, 3, replace=False)
+    D, E, st, stats = _run(s, cluster_ctas=4)
+    cmp = compare_atoms(s, D, st["e_atom"], atoms)
+    print("cluster4 cfg2@300", {k: v for k, v in cmp.items() if k != "ref"}, stats)
+    assert (st["status"] == 0).all()
+    assert cmp["max_abs_dD"] <= TOL_MIXED_D and cmp["rel_dE"] <= TOL_MIXED_E
+
+
+def test_plain_newton_schulz_matches_scaled():
+    """sign_scaled_iters = -1 runs Eq. 6 unscaled after X0 = A / rho; the scaled schedule (default) must reach
+    the same D within the mixed tolerances and with fewer GEMMs."""
+    s = make_system("cfg2", n_atoms=300)
+    atoms = np.random.default_rng(4).choice(s.n_atoms, 3, replace=False)
+    D0, E0, st0, stats0 = _run(s, sign_scaled_iters=-1)
+    D1, E1, st1, stats1 = _run(s)
+    c0 = compare_atoms(s, D0, st0["e_atom"], atoms)
+    c1 = compare_atoms(s, D1, st1["e_atom"], atoms)
+    print("plain", c0["max_abs_dD"], c0["rel_dE"], stats0["gemms_executed"], "scaled", c1["max_abs_dD"], c1["rel_dE"], stats1["gemms_executed"])
+    for c in (c0, c1):
+        assert c["max_abs_dD"] <= TOL_MIXED_D and c["rel_dE"] <= TOL_MIXED_E
+    assert stats1["gemms_executed"] < stats0["gemms_executed"]
+    assert abs(E0 - E1) / abs(E0) <= TOL_MIXED_E
+
+
 def test_small_proxy_fp32():
     from paper_2205_12182_b200 import PREC_FP32
     s = make_system("cfg1", n_atoms=400)

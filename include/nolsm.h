@@ -70,7 +70,7 @@ typedef struct {
     size_t workspace_bytes;  /* cap on the library-owned dense workspace [auto] */
     int profile_every;       /* round engine, > 0: every k-th round runs eagerly with CUDA events around each launch [0 = off] */
     int engine;              /* NOLSM_ENGINE_* [AUTO: PERSISTENT (one kernel launch per density_matrix call) for the
-                                FP16/tcgen05 path when every n_i <= 2048, else ROUNDS (one CUDA graph per iteration round)] */
+                                FP16/tcgen05 path when every n_i <= 4096, else ROUNDS (one CUDA graph per iteration round)] */
     int sign_scaled_iters;   /* persistent engine: the first k sign iterations run Eq. 6 on alpha X_k instead of X_k,
                                 X_{k+1} = 1/2 (alpha X_k)(3I - (alpha X_k)^2), alpha = sign_scale > 1, which lifts small
                                 eigenvalues 1.5 alpha x per step instead of 1.5 x and keeps the rest inside

@@ -66,11 +66,11 @@ constexpr int G2_SMEM_BYTES = G2_STAGES * G2_STAGE_BYTES + 256 + 64 * G2_NTI + 1
 
 #ifdef G2_TIMING
 // probe builds only: cycles spent waiting, summed over CTAs
-__device__ unsigned long long g2_timing[8];
+__device__ unsigned long long g2_timing[12];
 #define G2_T0() const long long t0_ = clock64()
 #define G2_T1(i) tacc_[i] += clock64() - t0_
-#define G2_TDECL() long long tacc_[8] = {0, 0, 0, 0, 0, 0, 0, 0}
-#define G2_TFLUSH(lane0) do { if (lane0) for (int i_ = 0; i_ < 8; ++i_) if (tacc_[i_]) atomicAdd(&g2_timing[i_], (unsigned long long)tacc_[i_]); } while (0)
+#define G2_TDECL() long long tacc_[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}
+#define G2_TFLUSH(lane0) do { if (lane0) for (int i_ = 0; i_ < 12; ++i_) if (tacc_[i_]) atomicAdd(&g2_timing[i_], (unsigned long long)tacc_[i_]); } while (0)
 #else
 #define G2_T0()
 #define G2_T1(i)
@@ -315,6 +315,9 @@ __device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int
         const int nkb = (ti.n16 + BK - 1) / BK;
         const int ktail = (ti.n16 - (nkb - 1) * BK) >> 4;          // 16-k slices of the last k-block (1..4)
         const uint32_t idesc = make_idesc_f16(256, ti.bn);
+#ifdef G2_TIMING
+        const long long tk0_ = clock64();
+#endif
         { G2_T0(); ptx::mbar_wait_cluster(sm.tempty(acc), acc_phase ^ 1); G2_T1(1); }
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + acc * 256;
@@ -336,6 +339,9 @@ __device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int
             __syncwarp();
             if (++stage == G2_STAGES) { stage = 0; phase ^= 1; }
         }
+#ifdef G2_TIMING
+        if (nkb >= 16 && ti.bn == 256) { tacc_[8] += clock64() - tk0_; tacc_[9] += 1; }     // full-width tiles: tempty wait + k-loop
+#endif
         if (++acc == 2) { acc = 0; acc_phase ^= 1; }
     }
 #ifdef G2_TIMING

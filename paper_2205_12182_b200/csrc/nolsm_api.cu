@@ -81,6 +81,8 @@ struct nolsm_ctx {
     bool persist = false;
     PEngine peng{};
     int* d_abort = nullptr;
+    signed char* d_die = nullptr;       // [256] SM -> L2 die table of the die probe (persistent engine)
+    int ndie = 1;
     int p_grid = 0;                     // CTAs of the persistent kernel: 4 x the clusters that can be resident together
     cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr;
     int h_a0 = 0;
@@ -332,6 +334,81 @@ int wait_result(nolsm_ctx* c) {
     return NOLSM_OK;
 }
 
+int getenv_int(const char* name, int dflt);
+
+// Runs k_die_probe and builds the SM -> die table (persist.cuh). Leaves ndie = 1 (no affinity) when the
+// near / far pattern is not a clean two-way split of the SMs.
+void probe_dies(nolsm_ctx* c) {
+    c->ndie = 1;
+    if (getenv_int("NOLSM_DIE_AFFINITY", 0) == 0) return;   // off by default: measured on B200, affinity does not change the DRAM traffic
+    unsigned long long* d_lines = nullptr;
+    unsigned int* d_best = nullptr;
+    std::vector<unsigned int> best(256 * NPROBE, 0xFFFFFFFFu);
+    if (cudaMalloc((void**)&d_lines, NPROBE * 2048) != cudaSuccess || cudaMalloc((void**)&d_best, best.size() * 4) != cudaSuccess ||
+        cudaMalloc((void**)&c->d_die, 256) != cudaSuccess) { cudaGetLastError(); cudaFree(d_lines); cudaFree(d_best); return; }
+    cudaMemset(d_lines, 0, NPROBE * 2048);
+    cudaMemcpy(d_best, best.data(), best.size() * 4, cudaMemcpyHostToDevice);
+    for (int rep = 0; rep < 4; ++rep) k_die_probe<<<c->sms * 6, 32>>>(d_lines, d_best);
+    const bool ok = cudaDeviceSynchronize() == cudaSuccess &&
+                    cudaMemcpy(best.data(), d_best, best.size() * 4, cudaMemcpyDeviceToHost) == cudaSuccess;
+    cudaFree(d_lines); cudaFree(d_best);
+    std::vector<signed char> die(256, (signed char)-1);
+    if (ok) {
+        std::vector<int> sms;
+        for (int sm = 0; sm < 256; ++sm) if (best[sm * NPROBE] != 0xFFFFFFFFu) sms.push_back(sm);
+        if (getenv_int("NOLSM_VERBOSE", 0) >= 2)
+            for (int sm : sms) {
+                fprintf(stderr, "probe sm %3d:", sm);
+                for (int l = 0; l < NPROBE; ++l) fprintf(stderr, " %5.1f", best[sm * NPROBE + l] / 64.0);
+                fprintf(stderr, "\n");
+            }
+        // M[sm][line] = latency with the SM's mean and the line's mean removed (an SM's distance to the L2 slices
+        // and a line's slice position shift whole rows / columns); what is left is +-(near/far gap)/2 with the sign
+        // given by (die of SM) xor (home die of line): a rank-one +-1 pattern. Its leading left singular vector
+        // (power iteration on M M^T) splits the SMs by die.
+        const int ns = (int)sms.size();
+        if (ns == c->sms && ns >= 8) {
+            std::vector<double> M((size_t)ns * NPROBE);
+            for (int i = 0; i < ns; ++i) for (int l = 0; l < NPROBE; ++l) M[(size_t)i * NPROBE + l] = best[sms[i] * NPROBE + l] / 64.0;
+            for (int i = 0; i < ns; ++i) {
+                double m = 0; for (int l = 0; l < NPROBE; ++l) m += M[(size_t)i * NPROBE + l];
+                m /= NPROBE; for (int l = 0; l < NPROBE; ++l) M[(size_t)i * NPROBE + l] -= m;
+            }
+            for (int l = 0; l < NPROBE; ++l) {
+                double m = 0; for (int i = 0; i < ns; ++i) m += M[(size_t)i * NPROBE + l];
+                m /= ns; for (int i = 0; i < ns; ++i) M[(size_t)i * NPROBE + l] -= m;
+            }
+            std::vector<double> u(ns), v(NPROBE);
+            for (int i = 0; i < ns; ++i) u[i] = M[(size_t)i * NPROBE];          // start: the first line's pattern
+            double sigma = 0, total = 0;
+            for (double x : M) total += x * x;
+            for (int it = 0; it < 50; ++it) {
+                for (int l = 0; l < NPROBE; ++l) { double a = 0; for (int i = 0; i < ns; ++i) a += M[(size_t)i * NPROBE + l] * u[i]; v[l] = a; }
+                double nv = 0; for (double x : v) nv += x * x; nv = std::sqrt(nv) + 1e-300; for (double& x : v) x /= nv;
+                for (int i = 0; i < ns; ++i) { double a = 0; for (int l = 0; l < NPROBE; ++l) a += M[(size_t)i * NPROBE + l] * v[l]; u[i] = a; }
+                double nu = 0; for (double x : u) nu += x * x; sigma = std::sqrt(nu); for (double& x : u) x /= (sigma + 1e-300);
+            }
+            std::vector<double> au(ns);
+            for (int i = 0; i < ns; ++i) au[i] = std::fabs(u[i]);
+            std::nth_element(au.begin(), au.begin() + ns / 2, au.end());
+            const double med = au[ns / 2];
+            int n1 = 0, weak = 0;
+            for (int i = 0; i < ns; ++i) {
+                die[sms[i]] = (signed char)(u[i] > 0 ? 1 : 0);
+                n1 += u[i] > 0;
+                weak += std::fabs(u[i]) < 0.3 * med;
+            }
+            const double explained = sigma * sigma / (total + 1e-300);
+            if (explained > 0.5 && weak <= ns / 20 && n1 * 10 >= ns * 4 && n1 * 10 <= ns * 6) c->ndie = 2;
+            if (getenv_int("NOLSM_VERBOSE", 0))
+                fprintf(stderr, "nolsm: die probe: %d SMs, %d on die 1, %d weak, rank-one part explains %.0f %% of the variance -> ndie = %d\n",
+                        ns, n1, weak, 100.0 * explained, c->ndie);
+        } else if (getenv_int("NOLSM_VERBOSE", 0)) fprintf(stderr, "nolsm: die probe: %d SMs seen of %d -> no affinity\n", ns, c->sms);
+    }
+    if (c->ndie != 2) std::fill(die.begin(), die.end(), (signed char)-1);
+    cudaMemcpy(c->d_die, die.data(), 256, cudaMemcpyHostToDevice);
+}
+
 int getenv_int(const char* name, int dflt) {
     const char* v = getenv(name);
     return v && *v ? atoi(v) : dflt;
@@ -403,6 +480,7 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
             return NOLSM_ECUDA;
         }
     }
+    if (use_umma(c) && o.engine != NOLSM_ENGINE_ROUNDS) probe_dies(c);
     *out = c;
     return NOLSM_OK;
 }
@@ -415,6 +493,7 @@ int nolsm_destroy(nolsm_ctx* c) {
     cudaEvent_t evs[] = {c->ev_fork, c->ev_x, c->ev_f, c->ev_in, c->ev_out, c->ev_k0, c->ev_k1};
     for (cudaEvent_t e : evs) if (e) cudaEventDestroy(e);
     for (int i = 0; i < ROUND_DEPTH; ++i) if (c->ev_round[i]) cudaEventDestroy(c->ev_round[i]);
+    if (c->d_die) cudaFree(c->d_die);
     if (c->s_main) cudaStreamDestroy(c->s_main);
     if (c->s_x) cudaStreamDestroy(c->s_x);
     if (c->s_f) cudaStreamDestroy(c->s_f);
@@ -578,7 +657,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     e = Engine{};
     const size_t es = elem_size(c);
     e.cap = (max_n + 15) & ~15;
-    e.ld = (e.cap + 63) & ~63;        // rows start on 128-byte lines: TMA boxes map to whole L2 lines
+    e.ld = ((e.cap + 63) & ~63) + 64 * getenv_int("NOLSM_LD_PAD", 0);        // rows start on 128-byte lines: TMA boxes map to whole L2 lines
     e.bufsz = (long long)e.cap * e.ld;
     e.slotsz = e.bufsz * NBUF;
     size_t free_b = 0, total_b = 0;
@@ -592,7 +671,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
                  (size_t)(3 * max_nset + 2) * 4 + (size_t)max_nset * 8 + 32 + G_STRIP_BYTES + (size_t)P_SIDE_WARPS * 2 * G_STAGE_BYTES <= (size_t)P_SIDE_SMEM &&
                  (size_t)e.cap * 2 <= (size_t)G_STRIP_BYTES;
     if (!c->persist && c->opt.engine == NOLSM_ENGINE_PERSISTENT)
-        return fail(c, NOLSM_EINVAL, "the persistent engine needs FP16/tcgen05 mode, submatrix dimensions <= 2048 and at most 16 basis functions per atom");
+        return fail(c, NOLSM_EINVAL, "the persistent engine needs FP16/tcgen05 mode, submatrix dimensions <= 4096 and at most 16 basis functions per atom");
     // round engine: enough slots for ~16 waves of tiles per GEMM launch; persistent engine: the slots in
     // flight (GEMM chain + side phases), few enough to keep the active iterates in L2
     // heavy-phase cap of the persistent engine: the live iterates of a slot in the GEMM chain are ~3.5 n^2 FP16
@@ -714,7 +793,9 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
                 }
             }
         }
-        pe.g_max = std::max(1, std::min(g_max, S));
+        pe.ndie = (c->ndie == 2 && c->d_die && S >= 4) ? 2 : 1;
+        pe.die_of_sm = c->d_die;
+        pe.g_max = pe.ndie == 2 ? std::max(1, std::min(g_max, S) / 2) : std::max(1, std::min(g_max, S));
         pe.want_lead = std::max(1, getenv_int("NOLSM_WANT_LEAD", G2_WANT_LEAD));
         pe.dbg = getenv_int("NOLSM_DBG", 0);
         pe.schulz_chunks = std::max(1, getenv_int("NOLSM_SCHULZ_CHUNKS", 16));
@@ -798,7 +879,7 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
         CU_TRY(c, cudaMemcpyAsync(pe.next_atom, &c->h_a0, 4, cudaMemcpyHostToDevice, s));
         CU_TRY(c, cudaMemsetAsync(pe.finished, 0, 4, s));
         CU_TRY(c, cudaMemsetAsync(c->d_abort, 0, 4, s));
-        CU_TRY(c, cudaMemsetAsync(pe.heavy, 0, 4, s));
+        CU_TRY(c, cudaMemsetAsync(pe.heavy, 0, 8, s));
         CU_TRY(c, cudaMemsetAsync(pe.parked, 0, 4 * pe.S, s));
         CU_TRY(c, cudaEventRecord(c->ev_k0, s));
         {
@@ -1099,6 +1180,14 @@ int nolsm_get_engine_counters(nolsm_ctx* c, double* out, int n) {
         if (t[12]) fprintf(stderr, "g4_timing cycles per full-width tile (tempty wait + k-loop): %.0f\n", (double)t[11] / (double)t[12]);
         unsigned long long z[16] = {};
         cudaMemcpyToSymbol(g4_timing, z, sizeof(z));
+#ifdef G2_TIMING
+        unsigned long long t2[12];
+        cudaMemcpyFromSymbol(t2, g2_timing, sizeof(t2));
+        if (t2[9]) fprintf(stderr, "g2_timing cycles per full-width tile (tempty wait + k-loop): %.0f over %.0f tiles\n", (double)t2[8] / (double)t2[9], (double)t2[9]);
+        static const char* nm2[8] = {"mma_take", "mma_tempty", "mma_full", "mma_total", "epi_take", "epi_tfull", "epi_work(cum)", "epi_done(cum)"};
+        for (int i = 0; i < 8; ++i) fprintf(stderr, "g2_timing %-16s %.3f Gcyc\n", nm2[i], t2[i] * 1e-9);
+        cudaMemcpyToSymbol(g2_timing, z, sizeof(t2));
+#endif
     }
 #endif
     out[0] = 1; out[1] = kms; out[2] = (double)(ct[PC_T_END] - ct[PC_T_START]) * 1e-6;

@@ -34,7 +34,7 @@ constexpr int P_SIDE_THREADS = P_SIDE_WARPS * 32;
 constexpr int P_THREADS = G2_CTRL_THREADS + P_SIDE_THREADS;
 constexpr int P_SIDE_SMEM = 60 * 1024;
 constexpr int P_SMEM_BYTES = G2_SMEM_BYTES + P_SIDE_SMEM;
-constexpr int P_MAX_CAP = 2048;
+constexpr int P_MAX_CAP = 4096;
 constexpr int P_GATHER_ROWATOMS = 4;            // row-atoms of N(i) per gather chunk (at most)
 
 enum SideKind { SK_NONE = 0, SK_REFILL, SK_GATHER, SK_SCHULZ1, SK_DCOLS };
@@ -70,6 +70,8 @@ struct PEngine {
     int* heavy;                   // [1] slots inside the GEMM-heavy phases INV .. SIGN right now (at most g_max)
     int* parked;                  // [S] 1 = the slot finished its first Schulz step and waits for a heavy token
     int g_max, want_lead, dbg;
+    const signed char* die_of_sm; // [256] L2 die of every SM (0 / 1), or all -1: no die affinity (see k_die_probe)
+    int ndie;                     // 2: slot s is served only by SMs of die s & 1 and heavy tokens are per die; 1: no affinity
     int ctas;                     // CTAs per cluster of the running kernel: 2 (pair tiles, gemm2sm.cuh) or 4 (A shared by two pairs, gemm4sm.cuh)
     int n_sched; float alpha_sched[16];   // scaled Newton-Schulz: alpha_k of sign iteration k < n_sched (1 afterwards)
     volatile int* abort_flag;     // device word; the host sets it (copy on another stream) to stop a kernel that overran its time limit
@@ -96,6 +98,35 @@ __device__ __forceinline__ __half* c_ptr(const PEngine& e, __half* base, int slo
 }
 
 __device__ __forceinline__ float* pcols_ptr(const PEngine& e, int slot) { return e.pcols + (size_t)slot * e.cap * PCW; }
+
+// L2 die of the SM this CTA runs on (-1: no affinity). B200 is two dies, each with half of the SMs and half of
+// L2; a line that SMs of both dies read is kept in both halves, so iterates shared across dies see only half of
+// the 126 MB. With affinity a slot's buffers are touched by the SMs of one die only.
+__device__ __forceinline__ int p_my_die(const PEngine& e) {
+    if (e.ndie != 2) return -1;
+    unsigned smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    return (int)e.die_of_sm[smid & 255u];
+}
+
+// Die probe: every CTA times dependent L2-hit loads (ld.global.cg chain) of NPROBE lines that lie 2 KB apart and
+// records the best time per (SM, line). A line is homed in one die; the SMs of that die see it ~25 cycles sooner.
+// The host turns the per-line near / far pattern into the SM -> die table.
+constexpr int NPROBE = 16;
+__global__ void __launch_bounds__(32) k_die_probe(const unsigned long long* lines, unsigned int* best /*[256][NPROBE]*/) {
+    if (threadIdx.x != 0) return;
+    unsigned smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    for (int l = 0; l < NPROBE; ++l) {
+        const unsigned long long* p = lines + (size_t)l * 256;       // 2 KB apart
+        unsigned long long v = 0;
+        for (int i = 0; i < 8; ++i) asm volatile("ld.global.cg.u64 %0, [%1];" : "=l"(v) : "l"(p + v) : "memory");   // warm (lines hold 0)
+        const long long t0 = clock64();
+        for (int i = 0; i < 64; ++i) asm volatile("ld.global.cg.u64 %0, [%1];" : "=l"(v) : "l"(p + v) : "memory");
+        const long long t1 = clock64();
+        atomicMin(&best[(smid & 255u) * NPROBE + l], (unsigned)((t1 - t0) + (long long)v));
+    }
+}
 
 namespace pl {
 __device__ __forceinline__ unsigned long long gtime() {
@@ -189,28 +220,31 @@ __device__ __forceinline__ void p_enter_heavy_now(const PEngine& e, int slot) {
     __stcg(&s->ycur, 2);
     p_install_gemm(e, slot, OP_INV_G1);
 }
+// With die affinity (ndie == 2) slot s belongs to die s & 1: tokens are counted per die (g_max each).
 __device__ __forceinline__ void p_enter_heavy(const PEngine& e, int slot) {
-    if (atomicAdd(e.heavy, 1) < e.g_max) { p_enter_heavy_now(e, slot); return; }
-    atomicSub(e.heavy, 1);
+    int* heavy = e.heavy + (e.ndie == 2 ? (slot & 1) : 0);
+    if (atomicAdd(heavy, 1) < e.g_max) { p_enter_heavy_now(e, slot); return; }
+    atomicSub(heavy, 1);
     __threadfence();
     atomicExch(&e.parked[slot], 1);
     __threadfence();
     // a token may have been returned between the failed attempt and the parking: try once more
-    if (atomicAdd(e.heavy, 1) < e.g_max) {
+    if (atomicAdd(heavy, 1) < e.g_max) {
         if (atomicCAS(&e.parked[slot], 1, 0) == 1) { p_enter_heavy_now(e, slot); return; }
         // a leaving slot admitted this one meanwhile (with its own token)
     }
-    atomicSub(e.heavy, 1);
+    atomicSub(heavy, 1);
 }
-__device__ __forceinline__ void p_leave_heavy(const PEngine& e) {
-    for (int s = 0; s < e.S; ++s) {
+__device__ __forceinline__ void p_leave_heavy(const PEngine& e, int slot) {
+    const int step = e.ndie == 2 ? 2 : 1;
+    for (int s = e.ndie == 2 ? (slot & 1) : 0; s < e.S; s += step) {
         if (*(volatile int*)&e.parked[s] == 1 && atomicCAS(&e.parked[s], 1, 0) == 1) {
             __threadfence();
             p_enter_heavy_now(e, s);          // the token changes hands
             return;
         }
     }
-    atomicSub(e.heavy, 1);
+    atomicSub(e.heavy + (e.ndie == 2 ? (slot & 1) : 0), 1);
 }
 
 // Takes the next atom of the feed into the slot and installs its gather (phase NEW). Returns false when
@@ -287,7 +321,7 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
         return;
     }
     if (kind == OP_DCOLS) {                 // a skinny product, not one of the counted square GEMMs
-        p_leave_heavy(e);
+        p_leave_heavy(e, slot);
         p_install_side(e, slot, SK_DCOLS, e.dcols_chunks);
         return;
     }
@@ -327,7 +361,7 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
         if (__ldcg(&s->conv)) {
             __stcg(&s->conv, 0);
             __stcg(&s->res_prev, 1e30f);
-            if (__ldcg(&s->status) & ST_NOTSPD) { p_leave_heavy(e); p_retire(e, slot); }   // no D for this atom (rows stay zero)
+            if (__ldcg(&s->status) & ST_NOTSPD) { p_leave_heavy(e, slot); p_retire(e, slot); }   // no D for this atom (rows stay zero)
             else p_install_gemm(e, slot, OP_AMAT);
         } else {
             p_install_gemm(e, slot, OP_INV_G1);
@@ -355,6 +389,7 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
     int q = 0; uint32_t ph = 0;
     unsigned long long idle_ns = 0, ntiles = 0, overshoot = 0;
     const unsigned long long t_begin = pl::gtime();
+    const int my_die = p_my_die(e);
     for (;;) {
         for (uint32_t spins = 0; !ptx::mbar_try_wait_cluster(sm.ti_empty(q), ph ^ 1);) {
             __nanosleep(100);
@@ -376,7 +411,7 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
             for (int base = 0; base < e.S; base += 32) {
                 const int sidx = base + lane;
                 const unsigned long long w = sidx < e.S ? *(volatile unsigned long long*)&e.gclaim[sidx] : 0ull;
-                const bool avail = (unsigned)(w & 0xFFFFFu) < (unsigned)((w >> 20) & 0xFFFFFu);
+                const bool avail = (unsigned)(w & 0xFFFFFu) < (unsigned)((w >> 20) & 0xFFFFFu) && (my_die < 0 || (sidx & 1) == my_die);
                 const unsigned m = __ballot_sync(0xffffffffu, avail);
                 if (m) { found = base + __ffs(m) - 1; break; }
             }
@@ -711,6 +746,7 @@ __device__ void side_dcols_chunk(const SysView& sv, const float* __restrict__ P,
 __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
     __shared__ int s_ctl[4];                      // slot, kind, chunk, nchunks
     const int warp = tid >> 5, lane = tid & 31;
+    const int my_die = p_my_die(e);
     unsigned long long busy_ns[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tasks[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     for (;;) {
         if (warp == 0) {
@@ -720,7 +756,7 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
                 for (int base = 0; base < e.S; base += 32) {
                     const int sidx = base + lane;
                     const unsigned w = sidx < e.S ? *(volatile unsigned int*)&e.sclaim[sidx] : 0u;
-                    const bool avail = (w & 0x3FFFu) < ((w >> 14) & 0x3FFFu);
+                    const bool avail = (w & 0x3FFFu) < ((w >> 14) & 0x3FFFu) && (my_die < 0 || (sidx & 1) == my_die);
                     const unsigned m = __ballot_sync(0xffffffffu, avail);
                     if (m) { found = base + __ffs(m) - 1; break; }
                 }

@@ -63,8 +63,8 @@ typedef struct {
     int max_sign_iters;      /* cap on Newton-Schulz sign iterations, Eq. 6 [64] */
     float tol_inv;           /* stop when ||I - S Y||_F / sqrt(n) < tol_inv [2e-3 mixed, 1e-5 FP32] */
     float tol_sign;          /* stop when ||X^2 - I||_F / sqrt(n) < tol_sign [2e-3 mixed, 1e-5 FP32] */
-    int power_iters_s;       /* power iterations for rho(S_sub) [6] */
-    int power_iters_a;       /* power iterations for rho(A_sub) [12] */
+    int power_iters_s;       /* power iterations for rho(S_sub) [persistent engine 3 (x 1.3 safety), round engine 6 (x 1.05)] */
+    int power_iters_a;       /* power iterations for rho(A_sub) [persistent engine 6 (x 1.25 safety), round engine 12 (x 1.05)] */
     double eps_filter;       /* block (j,i) enters N(i) iff max(|H0_ji|max, |S_ji|max) > eps_filter [0 = structural] */
     int batch_atoms;         /* workspace slots = submatrices resident at once [auto: ~16 waves of GEMM tiles] */
     size_t workspace_bytes;  /* cap on the library-owned dense workspace [auto] */

@@ -70,6 +70,7 @@ struct PEngine {
     int* heavy;                   // [1] slots inside the GEMM-heavy phases INV .. SIGN right now (at most g_max)
     int* parked;                  // [S] 1 = the slot finished its first Schulz step and waits for a heavy token
     int g_max, want_lead, dbg;
+    int tile_n;                   // columns of a pair tile (256; 128 halves a GEMM's latency at more L2 traffic per FLOP)
     const signed char* die_of_sm; // [256] L2 die of every SM (0 / 1), or all -1: no die affinity (see k_die_probe)
     int ndie;                     // 2: slot s is served only by SMs of die s & 1 and heavy tokens are per die; 1: no affinity
     int ctas;                     // CTAs per cluster of the running kernel: 2 (pair tiles, gemm2sm.cuh) or 4 (A shared by two pairs, gemm4sm.cuh)
@@ -258,6 +259,7 @@ __device__ __forceinline__ bool p_refill(const PEngine& e, int slot) {
     int ntm, ntn;
     choose_tiling(n16, ntm, ntn);
     if (e.ctas == G4_CTAS) ntn = g4_ntn(n16);                           // cluster tiles per row of tiles
+    else ntn = (n16 + e.tile_n - 1) / e.tile_n;
     const int nset = (int)(e.sv.nset_ptr[a + 1] - e.sv.nset_ptr[a]);
     __stcg(reinterpret_cast<int4*>(&s->atom), make_int4(a, n, n16, e.at.pos[a]));
     __stcg(reinterpret_cast<int4*>(&s->nbi), make_int4(e.at.nb[a], ntm, ntn, nset));
@@ -438,7 +440,7 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
                             int n0, bn0, bn1;
                             g4_cols(g0.z, tn, n0, bn0, bn1);
                             ti.n0 = n0; ti.bn = bn0 | (bn1 << 16);
-                        } else { ti.n0 = tn * BN; ti.bn = min(BN, g0.z - tn * BN); }
+                        } else { ti.n0 = tn * e.tile_n; ti.bn = min(e.tile_n, g0.z - tn * e.tile_n); }
                         ti.n = g0.y; ti.n16 = g0.z; ti.nreports = CTAS * nt;
                         ti.kind = o0.x; ti.a_buf = o0.y; ti.b_buf = o0.z; ti.c_buf = o0.w;
                         ti.c_out = o1.x; ti.alpha_res = o1.y; ti.beta = o1.z; ti.want_res = __float_as_int(o1.w);

@@ -267,17 +267,22 @@ def main():
     gemm_tf = prof_acc["gemm_flops_useful"] / max(prof_acc["gemm_ms"], 1e-9) / 1e9
     gemm_tf_padded = prof_acc["gemm_flops_padded"] / max(prof_acc["gemm_ms"], 1e-9) / 1e9
     sampled_ms = prof_acc["gemm_ms"] + prof_acc["gather_ms"] + prof_acc["dcols_ms"] + prof_acc["other_ms"]
-    traffic = None
+    # DRAM traffic of the kernel from the committed ncu --set full capture (profiles/): measured per submatrix on a
+    # 1024-submatrix launch of the same workload, scaled to the submatrices of one launch here
+    traffic, traffic_note = None, None
     tp = os.path.join(ROOT, "profiles", "gemm_traffic.json")
-    if os.path.exists(tp):
+    if os.path.exists(tp) and args.workload == "cfg2":
         with open(tp) as f:
-            traffic = json.load(f).get("dram_bytes_per_launch")
+            tj = json.load(f)
+        traffic = tj.get("dram_bytes_per_submatrix", 0.0) * system.n_atoms or None
+        traffic_note = tj.get("capture")
     roofline = {"bound": "tensor", "kernel": "nolsm_persist_kernel" if persistent else "gemm2_round_kernel",
                 "achieved": gemm_tf, "peak": peaks["bf16_tflops_sustained"],
                 "unit": "TFLOP/s", "frac": gemm_tf / peaks["bf16_tflops_sustained"], "traffic": traffic,
                 "peak_source": peaks["source"] + " bf16_tflops_sustained (kernel timed inside a long step)",
                 "achieved_padded": gemm_tf_padded, "avg_launch_us": 1e3 * prof_acc["gemm_ms"] / max(prof_acc["gemm_launches"], 1),
-                "frac_of_burst": gemm_tf / peaks["bf16_tflops"], "frac_of_nominal_2250": gemm_tf / NOMINAL_FP16_TFLOPS}
+                "frac_of_burst": gemm_tf / peaks["bf16_tflops"], "frac_of_nominal_2250": gemm_tf / NOMINAL_FP16_TFLOPS,
+                "traffic_source": traffic_note}
     if persistent:
         # share of the step spent inside the kernel (the rest is assemble: host index logic + uploads)
         roofline["share_of_step_time"] = prof_acc["gemm_ms"] / (ms_step * args.steps)

@@ -23,7 +23,10 @@
 
 namespace nolsm {
 
-constexpr int G2_STAGES = 5;
+#ifndef G2_STAGES_N
+#define G2_STAGES_N 5
+#endif
+constexpr int G2_STAGES = G2_STAGES_N;
 constexpr int G2_A_BYTES = 128 * BK * 2;              // 16 KB: this CTA's 128 rows x 64 k
 constexpr int G2_B_BYTES = 2 * B_BOX_BYTES;           // 16 KB: 64 k x (up to 128) columns
 constexpr int G2_STAGE_BYTES = G2_A_BYTES + G2_B_BYTES;

@@ -213,3 +213,90 @@ def dense_from_blocks(atom_nb, row_ptr, col_idx, vals, transpose_blocks=False):
                 M[first[i]:first[i + 1], first[j]:first[j + 1]] = blk
             s += 1
     return M
+
+
+# ------------------------------------------------------------------------------------------
+# submatrix combination ("one submatrix for multiple columns", Eq. 9 / Eq. 10)
+# ------------------------------------------------------------------------------------------
+def combine_cost(n, mode):
+    """What the evaluation of a submatrix of dimension n costs in the combination criterion.
+    mode 1, Eq. 9 (L87): n^3, the FLOP count of a dense multiplication. mode 2, Eq. 10 (L91):
+    p(n) x n^3 with the GPU's measured performance characteristic; for the B200 engine the
+    measured time of a multiplication is proportional to the number of 256 x 256 x 64 tile steps
+    (C-19), so p(n) n^3 := ceil(n16/256)^2 ceil(n16/64), n16 = n rounded up to 16."""
+    n = int(n)
+    if mode == 1:
+        return n * n * n
+    n16 = (n + 15) // 16 * 16
+    t = (n16 + 255) // 256
+    return t * t * ((n16 + 63) // 64)
+
+
+def combine_groups(atom_nb, index_sets, mode=1, max_dim=2048, max_members=16, max_candidates=24):
+    """Greedy combination of columns (atoms) into groups that share ONE submatrix (C-19).
+
+    Atoms are visited in ascending id. An atom i that is still free seeds a group G = N(i). Its
+    candidates are the free atoms j of N(i), ordered by the overlap dim(N(i) & N(j)) (descending,
+    ties by id), the first max_candidates of them. A candidate joins iff the criterion of Eq. 9
+    (mode 1) or Eq. 10 (mode 2) holds for the group as it stands,
+        cost(n_G + n_j - n_{G & j}) < cost(n_G) + cost(n_j),
+    and the union stays within max_dim; then G <- G | N(j). All quantities are integers.
+    Returns the list of groups (member lists in joining order, seed first)."""
+    nb = np.asarray(atom_nb, dtype=np.int64)
+    n_at = len(nb)
+    dim = [int(nb[N].sum()) for N in index_sets]
+    free = np.ones(n_at, dtype=bool)
+    groups = []
+    for i in range(n_at):
+        if not free[i]:
+            continue
+        free[i] = False
+        members = [i]
+        if max_members > 1 and mode in (1, 2):
+            Ni = np.asarray(index_sets[i])
+            G = Ni
+            n_g = dim[i]
+            cand = []
+            for j in Ni:
+                j = int(j)
+                if j != i and free[j]:
+                    ov = int(nb[np.intersect1d(Ni, index_sets[j], assume_unique=True)].sum())
+                    cand.append((-ov, j))
+            cand.sort()
+            for _, j in cand[:max_candidates]:
+                if len(members) >= max_members:
+                    break
+                n_gj = int(nb[np.intersect1d(G, index_sets[j], assume_unique=True)].sum())
+                n_u = n_g + dim[j] - n_gj
+                if n_u > max_dim:
+                    continue
+                if combine_cost(n_u, mode) < combine_cost(n_g, mode) + combine_cost(dim[j], mode):
+                    members.append(j)
+                    free[j] = False
+                    G = np.union1d(G, index_sets[j])
+                    n_g = n_u
+        groups.append(members)
+    return groups
+
+
+def group_result(members, atom_nb, row_ptr, col_idx, blk_off, H_vals, S_vals, mu, eps_filter=0.0):
+    """One submatrix for several columns (L65): the index set of the group is the union of its members'
+    index sets, Eq. 8 is evaluated once on it, and every member i takes its own columns, restricted to the
+    rows j in N(i) - the blocks (j, i) that exist in the pattern of the result (L58, L60).
+    Returns {i: dict like atom_result(i)} plus key "G" (the union) and "n" (its dimension)."""
+    sets = {int(i): index_set(int(i), row_ptr, col_idx, atom_nb, blk_off, H_vals, S_vals, eps_filter) for i in members}
+    G = np.unique(np.concatenate(list(sets.values())))
+    H_G, off_G = submatrix(G, atom_nb, row_ptr, col_idx, blk_off, H_vals)
+    S_G, _ = submatrix(G, atom_nb, row_ptr, col_idx, blk_off, S_vals)
+    D_G, eps, s = density_eigh(H_G, S_G, mu)
+    out = {"G": G, "n": int(off_G[-1])}
+    for i, N_i in sets.items():
+        a_i = int(np.searchsorted(G, i))
+        c0, c1 = int(off_G[a_i]), int(off_G[a_i + 1])
+        rows = np.concatenate([np.arange(off_G[a], off_G[a + 1]) for a in np.searchsorted(G, N_i)])
+        Dcols = D_G[np.ix_(rows, np.arange(c0, c1))].copy()
+        off = np.zeros(len(N_i) + 1, dtype=np.int64)
+        off[1:] = np.cumsum(np.asarray(atom_nb, dtype=np.int64)[N_i])
+        e_i = float((Dcols * H_G[np.ix_(rows, np.arange(c0, c1))]).sum())
+        out[i] = dict(N=N_i, n=int(off[-1]), off=off, Dcols=Dcols, e_i=e_i, eps=eps, s=s, n_group=int(off_G[-1]))
+    return out

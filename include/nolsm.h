@@ -80,6 +80,12 @@ typedef struct {
     int cluster_ctas;        /* persistent engine, CTAs per thread-block cluster: 2 = one tcgen05 CTA pair per 256 x 256 tile;
                                 4 = two pairs on a 256 x 512 tile with the A operand TMA-multicast between them (less
                                 L2 -> SM traffic, but only 132 of 148 SMs can hold 4-CTA clusters on B200) [2] */
+    int combine;             /* persistent engine: one submatrix for several columns. 0 = one submatrix per atom;
+                                1 = greedy groups under the cubic criterion Eq. 9 (L87); 2 = under Eq. 10 (L91) with the engine's
+                                measured characteristic p(n) n^3 := ceil(n16/256)^2 ceil(n16/64) (C-19) [0] */
+    int combine_max_dim;     /* a group's union index set may not exceed this dimension [2048] */
+    int combine_max_members; /* atoms per group at most [16] */
+    int combine_max_candidates; /* candidates examined per seed atom, by descending overlap with the seed's index set [24] */
 } nolsm_options;
 
 typedef struct {
@@ -93,6 +99,8 @@ typedef struct {
     double flops_padded;          /* same with tile-padded dimensions (what the tensor cores executed) */
     int64_t n_notspd, n_noconv;
     double gather_bytes, scatter_bytes; /* algorithmic bytes of the last density_matrix call */
+    int64_t n_units;              /* dense submatrices evaluated per call (== n_atoms without combination); dim_min / dim_max /
+                                     dim_mean describe these */
 } nolsm_stats;
 
 /* Creates a context on `cuda_device`. opt may be NULL. */
@@ -130,6 +138,12 @@ int nolsm_energy(nolsm_ctx* ctx, double* e_elec);
 int nolsm_destroy(nolsm_ctx* ctx);
 
 /* ---- diagnostics used by the parity tests and the benchmark ---- */
+
+/* The group (unit) atom `atom` belongs to after nolsm_assemble (C-19; without combine the group is the atom
+ * itself): its members in joining order (seed first), the union index set (ascending atom ids) that the group's one
+ * dense submatrix is built on, and that submatrix's dimension. Call with NULL arrays to query the two counts. */
+int nolsm_get_group(nolsm_ctx* ctx, int64_t atom, int32_t* members_out, int32_t* n_members_inout, int32_t* set_out,
+                    int32_t* n_set_inout, int32_t* dim_out);
 
 /* N(i) (ascending atom ids) and n_i. atoms_out may be NULL to query the count; capacity in *n_inout. */
 int nolsm_get_index_set(nolsm_ctx* ctx, int64_t atom, int32_t* atoms_out, int32_t* n_inout, int32_t* dim_out);

@@ -23,7 +23,8 @@ class NolsmOptions(C.Structure):
                 ("power_iters_s", C.c_int), ("power_iters_a", C.c_int), ("eps_filter", C.c_double),
                 ("batch_atoms", C.c_int), ("workspace_bytes", C.c_size_t), ("profile_every", C.c_int),
                 ("engine", C.c_int), ("sign_scaled_iters", C.c_int), ("sign_scale", C.c_float),
-                ("cluster_ctas", C.c_int)]
+                ("cluster_ctas", C.c_int), ("combine", C.c_int), ("combine_max_dim", C.c_int),
+                ("combine_max_members", C.c_int), ("combine_max_candidates", C.c_int)]
 
 
 class NolsmStats(C.Structure):
@@ -31,7 +32,7 @@ class NolsmStats(C.Structure):
                 ("dim_mean", C.c_double), ("sum_inv_iters", C.c_int64), ("sum_sign_iters", C.c_int64),
                 ("gemms_executed", C.c_int64), ("flops_useful", C.c_double), ("flops_padded", C.c_double),
                 ("n_notspd", C.c_int64), ("n_noconv", C.c_int64), ("gather_bytes", C.c_double),
-                ("scatter_bytes", C.c_double)]
+                ("scatter_bytes", C.c_double), ("n_units", C.c_int64)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -66,6 +67,7 @@ def load_library():
     lib.nolsm_energy.argtypes = [P, C.POINTER(C.c_double)]
     lib.nolsm_destroy.argtypes = [P]
     lib.nolsm_get_index_set.argtypes = [P, I64, P, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+    lib.nolsm_get_group.argtypes = [P, I64, P, C.POINTER(C.c_int32), P, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     lib.nolsm_gather_submatrix.argtypes = [P, I64, I32, I32, P]
     lib.nolsm_get_stats.argtypes = [P, C.POINTER(NolsmStats)]
     lib.nolsm_get_atom_stats.argtypes = [P, I64, I64, P, P, P, P, P, P, P]
@@ -74,7 +76,7 @@ def load_library():
     lib.nolsm_last_error.argtypes = [P]
     lib.nolsm_last_error.restype = C.c_char_p
     for f in ("nolsm_create", "nolsm_assemble", "nolsm_density_matrix", "nolsm_density_matrix_range", "nolsm_energy",
-              "nolsm_destroy", "nolsm_get_index_set", "nolsm_gather_submatrix", "nolsm_get_stats",
+              "nolsm_destroy", "nolsm_get_index_set", "nolsm_get_group", "nolsm_gather_submatrix", "nolsm_get_stats",
               "nolsm_get_atom_stats", "nolsm_get_profile", "nolsm_get_engine_counters"):
         getattr(lib, f).restype = C.c_int
     _LIB = lib
@@ -168,6 +170,15 @@ class Nolsm:
         out = np.empty(n.value, dtype=np.int32)
         self._check(self._lib.nolsm_get_index_set(self._h, atom, out.ctypes.data, C.byref(n), C.byref(dim)))
         return out, dim.value
+
+    def group(self, atom: int):
+        """(members in joining order, union index set, dimension) of the group `atom` belongs to."""
+        nm, ns, dim = C.c_int32(0), C.c_int32(0), C.c_int32(0)
+        self._check(self._lib.nolsm_get_group(self._h, atom, None, C.byref(nm), None, C.byref(ns), C.byref(dim)))
+        mem = np.empty(nm.value, dtype=np.int32)
+        st = np.empty(ns.value, dtype=np.int32)
+        self._check(self._lib.nolsm_get_group(self._h, atom, mem.ctypes.data, C.byref(nm), st.ctypes.data, C.byref(ns), C.byref(dim)))
+        return mem, st, dim.value
 
     def gather_submatrix(self, atom: int, which: int, fp16: bool):
         _, dim = self.index_set(atom)

@@ -30,6 +30,15 @@ struct SysView {
     const int* nset_atom;         // atoms of N(i), ascending
     const int* nset_slot;         // slot of block (i, j) for j in N(i)
     const int* nset_off;          // first row/column of atom j inside submatrix i
+    // Units of the persistent engine: one dense submatrix serves the columns of all member atoms of a unit
+    // (Eq. 9 / Eq. 10; C-19). Without combination unit u is atom u and these arrays alias
+    // the per-atom ones.
+    const long long* unit_ptr;    // [n_units + 1] members of unit u: unit_mem[unit_ptr[u] .. unit_ptr[u + 1])
+    const int* unit_mem;
+    const long long* uset_ptr;    // [n_units + 1] index set of the unit (union of its members' N(i), ascending)
+    const int* uset_atom;
+    const int* uset_off;          // first row/column of that atom inside the unit's matrix
+    const int* nset_uoff;         // for atom i, j in N(i): first row of atom j inside the matrix of i's unit
 };
 
 // Tiles of one n16 x n16 GEMM: ntm x ntn tiles of BM x BN; the last tile column is exactly as wide as

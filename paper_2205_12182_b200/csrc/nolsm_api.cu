@@ -53,6 +53,13 @@ struct nolsm_ctx {
     std::vector<int32_t> atom_nb, col_idx, nset_atom, nset_slot, nset_off, dim, pos;
     std::vector<int64_t> row_ptr, blk_off, nset_ptr;
     bool filtered = false;
+    // units (C-19): unit u serves the atoms unit_mem[unit_ptr[u] .. unit_ptr[u+1]) with one submatrix on uset
+    int64_t n_units = 0;
+    std::vector<int64_t> unit_ptr, uset_ptr;
+    std::vector<int32_t> unit_mem, uset_atom, uset_off, udim, upos, unit_of, nset_uoff;
+    long long *d_unit_ptr = nullptr, *d_uset_ptr = nullptr;
+    int *d_unit_mem = nullptr, *d_uset_atom = nullptr, *d_uset_off = nullptr, *d_udim = nullptr, *d_upos = nullptr, *d_nset_uoff = nullptr;
+    bool combined = false;
     int max_n = 0, max_nset = 0, max_nbi = 0;
 
     // device arrays
@@ -210,6 +217,8 @@ SysView sys_view(const nolsm_ctx* c) {
     SysView v;
     v.row_ptr = c->d_row_ptr; v.col_idx = c->d_col_idx; v.blk_off = c->d_blk_off; v.atom_nb = c->d_atom_nb;
     v.nset_ptr = c->d_nset_ptr; v.nset_atom = c->d_nset_atom; v.nset_slot = c->d_nset_slot; v.nset_off = c->d_nset_off;
+    v.unit_ptr = c->d_unit_ptr; v.unit_mem = c->d_unit_mem; v.uset_ptr = c->d_uset_ptr; v.uset_atom = c->d_uset_atom;
+    v.uset_off = c->d_uset_off; v.nset_uoff = c->d_nset_uoff;
     return v;
 }
 
@@ -336,6 +345,88 @@ int wait_result(nolsm_ctx* c) {
 
 int getenv_int(const char* name, int dflt);
 
+// ---- submatrix combination (Eq. 9 / Eq. 10; C-19). Integer arithmetic only. ----
+int64_t combine_cost(int64_t n, int mode) {
+    if (mode == 1) return n * n * n;                               // Eq. 9: FLOP of a dense multiplication
+    const int64_t n16 = (n + 15) / 16 * 16, t = (n16 + 255) / 256;  // Eq. 10 with the engine's tile-time characteristic
+    return t * t * ((n16 + 63) / 64);
+}
+// sum of nb over the atoms two ascending lists have in common
+int64_t overlap_dim(const int32_t* a, int64_t na, const int32_t* b, int64_t nb_, const int32_t* atom_nb) {
+    int64_t i = 0, j = 0, d = 0;
+    while (i < na && j < nb_) {
+        if (a[i] < b[j]) ++i;
+        else if (a[i] > b[j]) ++j;
+        else { d += atom_nb[a[i]]; ++i; ++j; }
+    }
+    return d;
+}
+// Builds the units of the context from the per-atom index sets: greedy groups (mode 1 / 2) or one atom per unit (mode 0).
+void build_units(nolsm_ctx* c, int mode, int max_dim, int max_members, int max_cand) {
+    const int64_t n_at = c->n_atoms;
+    const int32_t* nb = c->atom_nb.data();
+    c->unit_ptr.assign(1, 0); c->unit_mem.clear(); c->uset_ptr.assign(1, 0); c->uset_atom.clear(); c->uset_off.clear(); c->udim.clear();
+    c->unit_of.assign(n_at, -1); c->upos.assign(n_at, 0);
+    std::vector<char> is_free(n_at, 1);
+    std::vector<int32_t> G, U;
+    std::vector<std::pair<int64_t, int32_t>> cand;
+    for (int64_t i = 0; i < n_at; ++i) {
+        if (!is_free[i]) continue;
+        is_free[i] = 0;
+        const int32_t* Ni = c->nset_atom.data() + c->nset_ptr[i];
+        const int64_t ni = c->nset_ptr[i + 1] - c->nset_ptr[i];
+        const size_t m0 = c->unit_mem.size();
+        c->unit_mem.push_back((int32_t)i);
+        G.assign(Ni, Ni + ni);
+        int64_t n_g = c->dim[i];
+        if (mode != 0 && max_members > 1) {
+            cand.clear();
+            for (int64_t q = 0; q < ni; ++q) {
+                const int32_t j = Ni[q];
+                if (j == i || !is_free[j]) continue;
+                cand.emplace_back(-overlap_dim(Ni, ni, c->nset_atom.data() + c->nset_ptr[j], c->nset_ptr[j + 1] - c->nset_ptr[j], nb), j);
+            }
+            std::sort(cand.begin(), cand.end());
+            if ((int)cand.size() > max_cand) cand.resize(max_cand);
+            for (const auto& cj : cand) {
+                if ((int)(c->unit_mem.size() - m0) >= max_members) break;
+                const int32_t j = cj.second;
+                const int32_t* Nj = c->nset_atom.data() + c->nset_ptr[j];
+                const int64_t nj = c->nset_ptr[j + 1] - c->nset_ptr[j];
+                const int64_t n_u = n_g + c->dim[j] - overlap_dim(G.data(), (int64_t)G.size(), Nj, nj, nb);
+                if (n_u > max_dim) continue;
+                if (combine_cost(n_u, mode) < combine_cost(n_g, mode) + combine_cost(c->dim[j], mode)) {
+                    c->unit_mem.push_back(j);
+                    is_free[j] = 0;
+                    U.resize(G.size() + nj);
+                    U.resize(std::set_union(G.begin(), G.end(), Nj, Nj + nj, U.begin()) - U.begin());
+                    G.swap(U);
+                    n_g = n_u;
+                }
+            }
+        }
+        const int32_t u = (int32_t)c->udim.size();
+        int off = 0;
+        for (int32_t a : G) { c->uset_atom.push_back(a); c->uset_off.push_back(off); off += nb[a]; }
+        c->uset_ptr.push_back((int64_t)c->uset_atom.size());
+        c->unit_ptr.push_back((int64_t)c->unit_mem.size());
+        c->udim.push_back(off);
+        for (size_t m = m0; m < c->unit_mem.size(); ++m) c->unit_of[c->unit_mem[m]] = u;
+    }
+    c->n_units = (int64_t)c->udim.size();
+    // offsets of every atom of N(i) inside the matrix of i's unit (N(i) is a subset of the unit's set: one merge walk)
+    c->nset_uoff.resize(c->nset_atom.size());
+    for (int64_t i = 0; i < n_at; ++i) {
+        const int32_t u = c->unit_of[i];
+        int64_t g = c->uset_ptr[u];
+        for (int64_t q = c->nset_ptr[i]; q < c->nset_ptr[i + 1]; ++q) {
+            while (c->uset_atom[g] != c->nset_atom[q]) ++g;
+            c->nset_uoff[q] = c->uset_off[g];
+            if (c->nset_atom[q] == i) c->upos[i] = c->uset_off[g];
+        }
+    }
+}
+
 // Runs k_die_probe and builds the SM -> die table (persist.cuh). Leaves ndie = 1 (no affinity) when the
 // near / far pattern is not a clean two-way split of the SMs.
 void probe_dies(nolsm_ctx* c) {
@@ -447,6 +538,11 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
     if (getenv("NOLSM_SIGN_SCALED_ITERS")) o.sign_scaled_iters = getenv_int("NOLSM_SIGN_SCALED_ITERS", 6);
     if (o.sign_scaled_iters < 0) o.sign_scaled_iters = 0;
     if (o.sign_scaled_iters > 14) o.sign_scaled_iters = 14;
+    if (getenv("NOLSM_COMBINE")) o.combine = getenv_int("NOLSM_COMBINE", 0);
+    if (o.combine < 0 || o.combine > 2) { delete c; return NOLSM_EINVAL; }
+    if (o.combine_max_dim <= 0) o.combine_max_dim = getenv_int("NOLSM_COMBINE_MAX_DIM", 2048);
+    if (o.combine_max_members <= 0) o.combine_max_members = 16;
+    if (o.combine_max_candidates <= 0) o.combine_max_candidates = 24;
     if (getenv_int("NOLSM_CLUSTER", 0) > 0) o.cluster_ctas = getenv_int("NOLSM_CLUSTER", 0);
     if (o.cluster_ctas != 0 && o.cluster_ctas != 2 && o.cluster_ctas != 4) { delete c; return NOLSM_EINVAL; }
     if (o.sign_scale == 0.f) o.sign_scale = 1.5f;
@@ -618,20 +714,25 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
             c->dim[i] = off;
         }
     });
+    // ---- units: one submatrix per atom, or per group of atoms (Eq. 9 / Eq. 10; C-19) ----
+    c->combined = c->opt.combine != 0 && want_persist(c);
+    if (c->opt.combine != 0 && !c->combined) return fail(c, NOLSM_EINVAL, "combine needs the persistent engine (FP16/tcgen05 mode)");
+    build_units(c, c->combined ? c->opt.combine : 0, std::min(c->opt.combine_max_dim, P_MAX_CAP), c->opt.combine_max_members,
+                c->opt.combine_max_candidates);
     int max_n = 0, min_n = 1 << 30, max_nset = 0, max_nbi = 0;
     double mean_tiles = 0, mean_n2 = 0;
-    for (int64_t i = 0; i < n_atoms; ++i) {
-        max_n = std::max(max_n, c->dim[i]);
-        min_n = std::min(min_n, c->dim[i]);
-        max_nset = std::max<int>(max_nset, (int)(c->nset_ptr[i + 1] - c->nset_ptr[i]));
-        max_nbi = std::max(max_nbi, c->atom_nb[i]);
+    for (int64_t i = 0; i < n_atoms; ++i) max_nbi = std::max(max_nbi, c->atom_nb[i]);
+    for (int64_t u = 0; u < c->n_units; ++u) {
+        max_n = std::max(max_n, c->udim[u]);
+        min_n = std::min(min_n, c->udim[u]);
+        max_nset = std::max<int>(max_nset, (int)(c->uset_ptr[u + 1] - c->uset_ptr[u]));
         int ntm, ntn;
-        choose_tiling((c->dim[i] + 15) & ~15, ntm, ntn);
+        choose_tiling((c->udim[u] + 15) & ~15, ntm, ntn);
         mean_tiles += (double)ntm * ntn;
-        mean_n2 += (double)c->dim[i] * c->dim[i];
+        mean_n2 += (double)c->udim[u] * c->udim[u];
     }
-    mean_tiles /= (double)n_atoms;
-    mean_n2 /= (double)n_atoms;
+    mean_tiles /= (double)c->n_units;
+    mean_n2 /= (double)c->n_units;
     if (max_n > 65535) return fail(c, NOLSM_EINVAL, "submatrix dimension > 65535 not supported");
     c->max_n = max_n; c->max_nset = max_nset; c->max_nbi = max_nbi;
     if (!c->filtered) {
@@ -651,6 +752,27 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     c->d_dim = (int*)tmp;
     if ((r = to_device(c, c->pos.data(), sizeof(int32_t) * n_atoms, &tmp, s))) return r;
     c->d_pos = (int*)tmp;
+    if ((r = to_device(c, c->unit_ptr.data(), sizeof(int64_t) * (c->n_units + 1), &tmp, s))) return r;
+    c->d_unit_ptr = (long long*)tmp;
+    if ((r = to_device(c, c->unit_mem.data(), sizeof(int32_t) * n_atoms, &tmp, s))) return r;
+    c->d_unit_mem = (int*)tmp;
+    if (c->combined) {
+        if ((r = to_device(c, c->uset_ptr.data(), sizeof(int64_t) * (c->n_units + 1), &tmp, s))) return r;
+        c->d_uset_ptr = (long long*)tmp;
+        if ((r = to_device(c, c->uset_atom.data(), sizeof(int32_t) * c->uset_atom.size(), &tmp, s))) return r;
+        c->d_uset_atom = (int*)tmp;
+        if ((r = to_device(c, c->uset_off.data(), sizeof(int32_t) * c->uset_off.size(), &tmp, s))) return r;
+        c->d_uset_off = (int*)tmp;
+        if ((r = to_device(c, c->nset_uoff.data(), sizeof(int32_t) * nn, &tmp, s))) return r;
+        c->d_nset_uoff = (int*)tmp;
+        if ((r = to_device(c, c->udim.data(), sizeof(int32_t) * c->n_units, &tmp, s))) return r;
+        c->d_udim = (int*)tmp;
+        if ((r = to_device(c, c->upos.data(), sizeof(int32_t) * n_atoms, &tmp, s))) return r;
+        c->d_upos = (int*)tmp;
+    } else {                      // unit u is atom u: the unit arrays are the per-atom ones
+        c->d_uset_ptr = c->d_nset_ptr; c->d_uset_atom = c->d_nset_atom; c->d_uset_off = c->d_nset_off;
+        c->d_nset_uoff = c->d_nset_off; c->d_udim = c->d_dim; c->d_upos = c->d_pos;
+    }
 
     // ---- engine: slots, workspace, tensor maps ----
     Engine& e = c->eng;
@@ -670,6 +792,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     c->persist = want_persist(c) && e.cap <= P_MAX_CAP && max_nbi <= NVC &&
                  (size_t)(3 * max_nset + 2) * 4 + (size_t)max_nset * 8 + 32 + G_STRIP_BYTES + (size_t)P_SIDE_WARPS * 2 * G_STAGE_BYTES <= (size_t)P_SIDE_SMEM &&
                  (size_t)e.cap * 2 <= (size_t)G_STRIP_BYTES;
+    if (c->combined && !c->persist) return fail(c, NOLSM_EINVAL, "combine: the groups do not fit the persistent engine (dimension or index-set size)");
     if (!c->persist && c->opt.engine == NOLSM_ENGINE_PERSISTENT)
         return fail(c, NOLSM_EINVAL, "the persistent engine needs FP16/tcgen05 mode, submatrix dimensions <= 4096 and at most 16 basis functions per atom");
     // round engine: enough slots for ~16 waves of tiles per GEMM launch; persistent engine: the slots in
@@ -689,7 +812,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     S = std::max(S, 2);
     S = (int)std::min<size_t>(S, std::max<size_t>(2, cap_bytes / slot_bytes));
     S = std::min(S, MAX_SLOTS);
-    S = (int)std::min<int64_t>(S, std::max<int64_t>(2, n_atoms));
+    S = (int)std::min<int64_t>(S, std::max<int64_t>(2, c->n_units));
     e.S = S;
     // after the S slots: two vector blocks per slot and one shared start block (block power iteration), cap x VLD each
     const size_t vec_bytes = (size_t)e.cap * VLD * es;
@@ -812,6 +935,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         pe.dcols_chunks = std::max(1, getenv_int("NOLSM_DCOLS_CHUNKS", 4));
         pe.next_atom = e.next_atom; pe.finished = e.finished; pe.abort_flag = c->d_abort;
         pe.at = e.at; pe.sv = sys_view(c);
+        pe.udim = c->d_udim; pe.upos = c->d_upos; pe.adim = c->d_dim;
         pe.S_vals = c->dS; pe.H_vals = c->dH; pe.val_f64 = val_dtype == NOLSM_DTYPE_F64;
         pe.e_atom = c->d_e_atom; pe.maps = c->d_maps; pe.base = (__half*)c->ws;
         c->h_sclaim0.assign(S, ((unsigned)SK_REFILL << 28) | (1u << 14));
@@ -877,9 +1001,11 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
     if (c->persist) {
         // ---- persistent engine: one kernel launch evaluates the whole range ----
         PEngine pe = c->peng;
-        pe.mu = (float)mu; pe.a_end = (int)a1; pe.total = (int)(a1 - a0);
+        if (c->combined && (a0 != 0 || a1 != c->n_atoms)) return fail(c, NOLSM_EINVAL, "with combine the whole system is evaluated per call (groups span atom ranges)");
+        const int64_t u0 = c->combined ? 0 : a0, u1 = c->combined ? c->n_units : a1;      // the feed counts units
+        pe.mu = (float)mu; pe.a_end = (int)u1; pe.total = (int)(u1 - u0);
         pe.D_vals = D_dev; pe.d_f64 = d_dtype == NOLSM_DTYPE_F64;
-        c->h_a0 = (int)a0;
+        c->h_a0 = (int)u0;
         memset(c->h_ctr0, 0, sizeof(c->h_ctr0));
         c->h_ctr0[PC_T_START] = ~0ull;
         CU_TRY(c, cudaMemsetAsync(pe.slots, 0, sizeof(PSlot) * pe.S, s));
@@ -989,12 +1115,14 @@ int nolsm_energy(nolsm_ctx* c, double* e_elec) {
     if (int r = wait_result(c)) return r;
     const int64_t n = c->last_a1 - c->last_a0;
     std::vector<double> e(n);
-    std::vector<int> st(n);
+    const int64_t u0 = c->combined ? 0 : c->last_a0, nu = c->combined ? c->n_units : n;   // status words are per unit
+    std::vector<int> st(nu);
     CU_TRY(c, cudaMemcpy(e.data(), c->d_e_atom + c->last_a0, 8 * n, cudaMemcpyDeviceToHost));
-    CU_TRY(c, cudaMemcpy(st.data(), c->eng.at.status + c->last_a0, 4 * n, cudaMemcpyDeviceToHost));
+    CU_TRY(c, cudaMemcpy(st.data(), c->eng.at.status + u0, 4 * nu, cudaMemcpyDeviceToHost));
     double sum = 0;
     int bits = 0;
-    for (int64_t i = 0; i < n; ++i) { sum += e[i]; bits |= st[i]; }
+    for (int64_t i = 0; i < n; ++i) sum += e[i];
+    for (int64_t u = 0; u < nu; ++u) bits |= st[u];
     *e_elec = sum;
     if (bits & ST_NOTSPD) return fail(c, NOLSM_ENOTSPD, "an S_sub inverse iteration failed (see nolsm_get_atom_stats)");
     if (bits & ST_NOCONV) return fail(c, NOLSM_ENOCONV, "a sign iteration hit max_sign_iters (see nolsm_get_atom_stats)");
@@ -1015,9 +1143,32 @@ int nolsm_get_index_set(nolsm_ctx* c, int64_t atom, int32_t* atoms_out, int32_t*
     return NOLSM_OK;
 }
 
+int nolsm_get_group(nolsm_ctx* c, int64_t atom, int32_t* members_out, int32_t* n_members_inout, int32_t* set_out,
+                    int32_t* n_set_inout, int32_t* dim_out) {
+    if (!c || !n_members_inout || !n_set_inout) return NOLSM_EINVAL;
+    if (!c->assembled) return fail(c, NOLSM_ESTATE, "not assembled");
+    if (atom < 0 || atom >= c->n_atoms) return fail(c, NOLSM_EINVAL, "atom out of range");
+    const int32_t u = c->unit_of[atom];
+    const int64_t m0 = c->unit_ptr[u], nm = c->unit_ptr[u + 1] - m0, s0 = c->uset_ptr[u], ns = c->uset_ptr[u + 1] - s0;
+    if (dim_out) *dim_out = c->udim[u];
+    int rc = NOLSM_OK;
+    if (members_out) {
+        if (*n_members_inout < nm) rc = fail(c, NOLSM_EINVAL, "members_out too small");
+        else memcpy(members_out, c->unit_mem.data() + m0, sizeof(int32_t) * nm);
+    }
+    if (set_out) {
+        if (*n_set_inout < ns) rc = fail(c, NOLSM_EINVAL, "set_out too small");
+        else memcpy(set_out, c->uset_atom.data() + s0, sizeof(int32_t) * ns);
+    }
+    *n_members_inout = (int32_t)nm;
+    *n_set_inout = (int32_t)ns;
+    return rc;
+}
+
 int nolsm_gather_submatrix(nolsm_ctx* c, int64_t atom, int which, int out_fp16, void* out_host) {
     if (!c || !out_host || (which != 0 && which != 1)) return NOLSM_EINVAL;
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "not assembled");
+    if (c->combined) return fail(c, NOLSM_ESTATE, "nolsm_gather_submatrix returns per-atom submatrices: assemble without combine");
     if (atom < 0 || atom >= c->n_atoms) return fail(c, NOLSM_EINVAL, "atom out of range");
     cudaSetDevice(c->dev);
     const size_t es = out_fp16 ? 2 : 4;
@@ -1079,6 +1230,31 @@ int nolsm_get_atom_stats(nolsm_ctx* c, int64_t a0, int64_t count, int32_t* dims,
     if (a0 < 0 || count < 0 || a0 + count > c->n_atoms) return fail(c, NOLSM_EINVAL, "range");
     cudaSetDevice(c->dev);
     if (c->have_result) { if (int r = wait_result(c)) return r; }
+    if (c->combined) {
+        // results are per unit: every member reports its unit's iteration counts, status and residual; the GEMMs and
+        // the unit's dimension are reported by the unit's first member only (sums over atoms stay sums over units)
+        const int64_t nu = c->n_units;
+        std::vector<int32_t> ui(nu), us(nu), ut(nu), ug(nu);
+        std::vector<float> ur(nu);
+        CU_TRY(c, cudaMemcpy(ui.data(), c->eng.at.inv, 4 * nu, cudaMemcpyDeviceToHost));
+        CU_TRY(c, cudaMemcpy(us.data(), c->eng.at.sign, 4 * nu, cudaMemcpyDeviceToHost));
+        CU_TRY(c, cudaMemcpy(ut.data(), c->eng.at.status, 4 * nu, cudaMemcpyDeviceToHost));
+        CU_TRY(c, cudaMemcpy(ug.data(), c->eng.at.gemms, 4 * nu, cudaMemcpyDeviceToHost));
+        CU_TRY(c, cudaMemcpy(ur.data(), c->eng.at.res, 4 * nu, cudaMemcpyDeviceToHost));
+        for (int64_t k = 0; k < count; ++k) {
+            const int64_t a = a0 + k;
+            const int32_t u = c->unit_of[a];
+            const bool first = c->unit_mem[c->unit_ptr[u]] == a;
+            if (dims) dims[k] = first ? c->udim[u] : 0;
+            if (inv_iters) inv_iters[k] = ui[u];
+            if (sign_iters) sign_iters[k] = us[u];
+            if (status) status[k] = ut[u];
+            if (gemms) gemms[k] = first ? ug[u] : 0;
+            if (residual) residual[k] = ur[u];
+        }
+        if (e_atom) CU_TRY(c, cudaMemcpy(e_atom, c->d_e_atom + a0, 8 * count, cudaMemcpyDeviceToHost));
+        return NOLSM_OK;
+    }
     if (dims) memcpy(dims, c->dim.data() + a0, 4 * count);
     if (inv_iters) CU_TRY(c, cudaMemcpy(inv_iters, c->eng.at.inv + a0, 4 * count, cudaMemcpyDeviceToHost));
     if (sign_iters) CU_TRY(c, cudaMemcpy(sign_iters, c->eng.at.sign + a0, 4 * count, cudaMemcpyDeviceToHost));
@@ -1096,24 +1272,26 @@ int nolsm_get_stats(nolsm_ctx* c, nolsm_stats* out) {
     const int64_t n = c->n_atoms;
     out->n_atoms = n;
     out->n_batches = c->rounds;
+    out->n_units = c->n_units;
     out->dim_min = 1 << 30;
     double dsum = 0;
-    for (int64_t i = 0; i < n; ++i) {
-        out->dim_min = std::min<int64_t>(out->dim_min, c->dim[i]);
-        out->dim_max = std::max<int64_t>(out->dim_max, c->dim[i]);
-        dsum += c->dim[i];
+    for (int64_t u = 0; u < c->n_units; ++u) {
+        out->dim_min = std::min<int64_t>(out->dim_min, c->udim[u]);
+        out->dim_max = std::max<int64_t>(out->dim_max, c->udim[u]);
+        dsum += c->udim[u];
     }
-    out->dim_mean = dsum / n;
+    out->dim_mean = dsum / (double)c->n_units;
     if (c->have_result) {
-        std::vector<int32_t> inv(n), sg(n), st(n), gm(n);
-        int r = nolsm_get_atom_stats(c, 0, n, nullptr, inv.data(), sg.data(), st.data(), gm.data(), nullptr, nullptr);
+        std::vector<int32_t> dm(n), inv(n), sg(n), st(n), gm(n);
+        int r = nolsm_get_atom_stats(c, 0, n, dm.data(), inv.data(), sg.data(), st.data(), gm.data(), nullptr, nullptr);
         if (r) return r;
         for (int64_t i = c->last_a0; i < c->last_a1; ++i) {
+            if (dm[i] == 0) continue;                       // not the first member of its unit
             out->sum_inv_iters += inv[i]; out->sum_sign_iters += sg[i]; out->gemms_executed += gm[i];
-            const double d = c->dim[i];
+            const double d = dm[i];
             out->flops_useful += 2.0 * d * d * d * gm[i];
             int ntm, ntn;
-            const int n16 = (c->dim[i] + 15) & ~15;
+            const int n16 = (dm[i] + 15) & ~15;
             choose_tiling(n16, ntm, ntn);
             out->flops_padded += 2.0 * (double)(ntm * BM) * (double)n16 * (double)n16 * gm[i];
             out->n_notspd += (st[i] & ST_NOTSPD) ? 1 : 0;
@@ -1121,9 +1299,9 @@ int nolsm_get_stats(nolsm_ctx* c, nolsm_stats* out) {
         }
         const size_t es = elem_size(c), vs = c->val_dtype == NOLSM_DTYPE_F64 ? 8 : 4;
         for (int64_t i = c->last_a0; i < c->last_a1; ++i) {
-            const double n16 = (c->dim[i] + 15) & ~15, n = c->dim[i];
+            const double n16 = (dm[i] + 15) & ~15, n = c->dim[i];
             const double nv = (double)(c->blk_off[c->row_ptr[i + 1]] - c->blk_off[c->row_ptr[i]]);
-            out->gather_bytes += 2.0 * n16 * n16 * es;                       // dense S_sub and H_sub written
+            out->gather_bytes += 2.0 * n16 * n16 * es;                       // dense S_sub and H_sub written (once per unit)
             out->scatter_bytes += nv * (c->last_ds + vs) + (n * n + n * c->atom_nb[i]) * es;
         }
     }

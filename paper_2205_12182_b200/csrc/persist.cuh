@@ -53,7 +53,8 @@ struct __align__(16) PSlot {      // 160 bytes
     int inv_iters, sign_iters, conv, xcur, ycur, status, gemm_count, tiles_done;
     float res_acc, res_prev, res_last, rho_s, rho_a, alpha1, alpha2; int side_done;
     int pow_step; float pow_norm2, pow_alpha, pow_est;              // block power iteration state
-    int noboost, pad[3];                                            // noboost: the scaled steps are over for this matrix
+    int noboost, unit, mptr, mend;                                  // noboost: the scaled steps are over for this matrix; unit and its members
+                                                                    // [mptr, mend) still to be served (atom / pos / nbi describe member mptr)
 };
 
 struct PEngine {
@@ -77,7 +78,10 @@ struct PEngine {
     int n_sched; float alpha_sched[16];   // scaled Newton-Schulz: alpha_k of sign iteration k < n_sched (1 afterwards)
     volatile int* abort_flag;     // device word; the host sets it (copy on another stream) to stop a kernel that overran its time limit
     unsigned long long* ctr;      // [PC_LEN]
-    AtomArrays at;
+    AtomArrays at;                // results are indexed by unit
+    const int* udim;              // [n_units] dimension of the unit's matrix
+    const int* upos;              // [n_atoms] first column of atom i inside its unit's matrix
+    const int* adim;              // [n_atoms] dim N(i): rows of D written for atom i
     SysView sv;
     const void *S_vals, *H_vals; int val_f64;
     void* D_vals; int d_f64;
@@ -252,22 +256,24 @@ __device__ __forceinline__ void p_leave_heavy(const PEngine& e, int slot) {
 // the feed is exhausted (the slot stays free).
 __device__ __forceinline__ bool p_refill(const PEngine& e, int slot) {
     if (*(volatile int*)e.next_atom >= e.a_end) return false;
-    const int a = atomicAdd(e.next_atom, 1);
+    const int a = atomicAdd(e.next_atom, 1);                            // a unit of the feed
     if (a >= e.a_end) return false;
     PSlot* s = &e.slots[slot];
-    const int n = e.at.dim[a], n16 = (n + 15) & ~15;
+    const int n = e.udim[a], n16 = (n + 15) & ~15;
     int ntm, ntn;
     choose_tiling(n16, ntm, ntn);
     if (e.ctas == G4_CTAS) ntn = g4_ntn(n16);                           // cluster tiles per row of tiles
     else ntn = (n16 + e.tile_n - 1) / e.tile_n;
-    const int nset = (int)(e.sv.nset_ptr[a + 1] - e.sv.nset_ptr[a]);
-    __stcg(reinterpret_cast<int4*>(&s->atom), make_int4(a, n, n16, e.at.pos[a]));
-    __stcg(reinterpret_cast<int4*>(&s->nbi), make_int4(e.at.nb[a], ntm, ntn, nset));
+    const int nset = (int)(e.sv.uset_ptr[a + 1] - e.sv.uset_ptr[a]);
+    const int m0 = (int)e.sv.unit_ptr[a], m1 = (int)e.sv.unit_ptr[a + 1];
+    const int atom = e.sv.unit_mem[m0];
+    __stcg(reinterpret_cast<int4*>(&s->atom), make_int4(atom, n, n16, e.upos[atom]));
+    __stcg(reinterpret_cast<int4*>(&s->nbi), make_int4(e.at.nb[atom], ntm, ntn, nset));
     __stcg(reinterpret_cast<int4*>(&s->inv_iters), make_int4(0, 0, 0, 0));            // inv, sign, conv, xcur
     __stcg(reinterpret_cast<int4*>(&s->ycur), make_int4(2, 0, 0, 0));                 // ycur, status, gemm_count, tiles_done
     __stcg(reinterpret_cast<float4*>(&s->res_acc), make_float4(0.f, 1e30f, 0.f, 0.f)); // res_acc, res_prev, res_last, rho_s
     __stcg(reinterpret_cast<float4*>(&s->rho_a), make_float4(0.f, 1.f, 0.5f, 0.f));    // rho_a, alpha1, alpha2, side_done
-    __stcg(reinterpret_cast<int4*>(&s->noboost), make_int4(0, 0, 0, 0));
+    __stcg(reinterpret_cast<int4*>(&s->noboost), make_int4(0, a, m0, m1));
     p_install_side(e, slot, SK_GATHER, (nset + e.gather_rowatoms - 1) / e.gather_rowatoms);
     return true;
 }
@@ -275,7 +281,7 @@ __device__ __forceinline__ bool p_refill(const PEngine& e, int slot) {
 // Phase FIN finished (or skipped for a failed inverse): publish the atom's results, free / refill the slot.
 __device__ __forceinline__ void p_retire(const PEngine& e, int slot) {
     PSlot* s = &e.slots[slot];
-    const int a = __ldcg(&s->atom);
+    const int a = __ldcg(&s->unit);
     e.at.inv[a] = __ldcg(&s->inv_iters); e.at.sign[a] = __ldcg(&s->sign_iters); e.at.status[a] = __ldcg(&s->status);
     e.at.gemms[a] = __ldcg(&s->gemm_count); e.at.res[a] = __ldcg(&s->res_last); e.at.rho[a] = __ldcg(&s->rho_a);
     const bool more = p_refill(e, slot);
@@ -323,7 +329,7 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
         return;
     }
     if (kind == OP_DCOLS) {                 // a skinny product, not one of the counted square GEMMs
-        p_leave_heavy(e, slot);
+        if (__ldcg(&s->mptr) == (int)e.sv.unit_ptr[__ldcg(&s->unit)]) p_leave_heavy(e, slot);   // first member: the chain is over
         p_install_side(e, slot, SK_DCOLS, e.dcols_chunks);
         return;
     }
@@ -492,8 +498,8 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
 // memory-level parallelism: several independent loads are issued before the first one is used.
 // ================================================================================================
 
-// a1, one chunk of row-atoms of N(i): builds the dense rows of T_i(S) (buffer 0) and T_i(H0) (buffer 1)
-// that belong to row-atoms [a_lo, a_hi) of N(i): block (j_a, j_b) of the sparse matrix where it exists,
+// a1, one chunk of row-atoms of the unit's index set N (N(i), or the union over the unit's members): builds the dense
+// rows of T(S) (buffer 0) and T(H0) (buffer 1) that belong to row-atoms [a_lo, a_hi) of N: block (j_a, j_b) of the sparse matrix where it exists,
 // zeros elsewhere and in the pad strip [n, n16). The last chunk also zeroes rows [n, n16).
 //
 // Data path (HBM-bound work, so it is built around bytes in flight): the source blocks of a row-atom are
@@ -519,10 +525,10 @@ __device__ __forceinline__ void g_cp_async(uint32_t dst, const TV* src) {
 
 template <typename TV>
 __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_vals, const TV* __restrict__ H_vals,
-                                  __half* __restrict__ dstS, __half* __restrict__ dstH, int atom, int n, int n16, int ld,
+                                  __half* __restrict__ dstS, __half* __restrict__ dstH, int unit, int n, int n16, int ld,
                                   int chunk, int nchunks, unsigned char* sm, int tid, unsigned long long* bytes) {
-    const long long p0 = sv.nset_ptr[atom];
-    const int cnt = (int)(sv.nset_ptr[atom + 1] - p0);
+    const long long p0 = sv.uset_ptr[unit];
+    const int cnt = (int)(sv.uset_ptr[unit + 1] - p0);
     const int warp = tid >> 5, lane = tid & 31;
     // shared memory: tables | strip | staging (4 warps x 2 stages)
     int* s_nset = reinterpret_cast<int*>(sm);                              // [cnt] atoms of N(i)
@@ -537,7 +543,7 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
     constexpr int CAP_E = G_STAGE_BYTES / (int)sizeof(TV);                 // values per stage
 
     const int a_lo = (int)((long long)cnt * chunk / nchunks), a_hi = (int)((long long)cnt * (chunk + 1) / nchunks);
-    for (int b = tid; b < cnt; b += P_SIDE_THREADS) { s_nset[b] = sv.nset_atom[p0 + b]; s_off[b] = sv.nset_off[p0 + b]; }
+    for (int b = tid; b < cnt; b += P_SIDE_THREADS) { s_nset[b] = sv.uset_atom[p0 + b]; s_off[b] = sv.uset_off[p0 + b]; }
     if (tid == 0) s_off[cnt] = n;
     pl::side_sync();
     const int rows_max = max(1, G_STRIP_BYTES / (n16 * 2));
@@ -712,26 +718,26 @@ __device__ void side_schulz1_chunk(const __half* __restrict__ S, __half* __restr
 template <typename TV, typename TD>
 __device__ void side_dcols_chunk(const SysView& sv, const float* __restrict__ P, const __half* __restrict__ Y,
                                  const TV* __restrict__ H_vals, TD* __restrict__ D_vals, double* e_atom,
-                                 int atom, int n, int ld, int pos, int nbi, int chunk, int nchunks, unsigned char* sm, int tid) {
+                                 int atom, int n_own, int ld, int pos, int nbi, int chunk, int nchunks, unsigned char* sm, int tid) {
     const long long p0 = sv.nset_ptr[atom];
     const int cnt = (int)(sv.nset_ptr[atom + 1] - p0);
-    int* s_off = reinterpret_cast<int*>(sm);                               // [cnt + 1] first row of each atom of N(i)
-    for (int b = tid; b < cnt; b += P_SIDE_THREADS) s_off[b] = sv.nset_off[p0 + b];
-    if (tid == 0) s_off[cnt] = n;
+    int* s_pre = reinterpret_cast<int*>(sm);                               // [cnt + 1] first value row of each atom of N(i) in output order
+    int* s_row = s_pre + cnt + 1;                                          // [cnt] first row of that atom inside the unit's matrix
+    for (int b = tid; b < cnt; b += P_SIDE_THREADS) { s_pre[b] = sv.nset_off[p0 + b]; s_row[b] = sv.nset_uoff[p0 + b]; }
+    if (tid == 0) s_pre[cnt] = n_own;
     pl::side_sync();
-    // the slots of row i that belong to N(i) are stored one after the other only when nothing is filtered, so
-    // the output offset of atom a is looked up; value q of the chunk = (atom a, column c, row bb) in output order
-    const int total = n * nbi;                                             // values of D written for this atom
+    // value q of the chunk = (atom a of N(i), column c, row bb) in output order; the rows of atom a sit at s_row[a]
+    // of the unit's matrix (== s_pre[a] when the unit is the atom itself)
+    const int total = n_own * nbi;                                         // values of D written for this atom
     const int q_lo = (int)((long long)total * chunk / nchunks), q_hi = (int)((long long)total * (chunk + 1) / nchunks);
     double e_part = 0.0;
     for (int q = q_lo + tid; q < q_hi; q += P_SIDE_THREADS) {
-        // rows of atom a start at s_off[a]; its values start at s_off[a] * nbi in this ordering
         int lo = 0, hi = cnt - 1;
-        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_off[mid] * nbi <= q) lo = mid; else hi = mid - 1; }
-        const int a = lo, nbj = s_off[a + 1] - s_off[a];
-        const int rem = q - s_off[a] * nbi;
+        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_pre[mid] * nbi <= q) lo = mid; else hi = mid - 1; }
+        const int a = lo, nbj = s_pre[a + 1] - s_pre[a];
+        const int rem = q - s_pre[a] * nbi;
         const int c = rem / nbj, bb = rem - c * nbj;
-        const int r = s_off[a] + bb;
+        const int r = s_row[a] + bb;
         const long long o = sv.blk_off[sv.nset_slot[p0 + a]] + rem;       // slot (i, j_a): [c][bb] = D_sub[r, pos + c]
         const float d = 0.5f * (__half2float(__ldcg(Y + (long long)r * ld + pos + c)) - __ldcg(P + (size_t)r * PCW + (pos & 7) + c));
         D_vals[o] = (TD)d;
@@ -788,8 +794,8 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
             case SK_GATHER: {
                 __half* dS = e.base + buf_off(e, slot, 0);
                 __half* dH = e.base + buf_off(e, slot, 1);
-                if (e.val_f64) side_gather_chunk<double>(e.sv, (const double*)e.S_vals, (const double*)e.H_vals, dS, dH, atom, n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER]);
-                else side_gather_chunk<float>(e.sv, (const float*)e.S_vals, (const float*)e.H_vals, dS, dH, atom, n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER]);
+                if (e.val_f64) side_gather_chunk<double>(e.sv, (const double*)e.S_vals, (const double*)e.H_vals, dS, dH, __ldcg(&s->unit), n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER]);
+                else side_gather_chunk<float>(e.sv, (const float*)e.S_vals, (const float*)e.H_vals, dS, dH, __ldcg(&s->unit), n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER]);
             } break;
             case SK_SCHULZ1:
                 side_schulz1_chunk(e.base + buf_off(e, slot, 0), e.base + buf_off(e, slot, 2), n, n16, e.ld, __ldcg(&s->rho_s), chunk, nch, tid);
@@ -798,11 +804,11 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
                 const float* P = pcols_ptr(e, slot);
                 const __half* Y = e.base + buf_off(e, slot, __ldcg(&s->ycur));
                 if (e.val_f64) {
-                    if (e.d_f64) side_dcols_chunk<double, double>(e.sv, P, Y, (const double*)e.H_vals, (double*)e.D_vals, e.e_atom, atom, n, e.ld, pos, nbi, chunk, nch, sm, tid);
-                    else side_dcols_chunk<double, float>(e.sv, P, Y, (const double*)e.H_vals, (float*)e.D_vals, e.e_atom, atom, n, e.ld, pos, nbi, chunk, nch, sm, tid);
+                    if (e.d_f64) side_dcols_chunk<double, double>(e.sv, P, Y, (const double*)e.H_vals, (double*)e.D_vals, e.e_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
+                    else side_dcols_chunk<double, float>(e.sv, P, Y, (const double*)e.H_vals, (float*)e.D_vals, e.e_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
                 } else {
-                    if (e.d_f64) side_dcols_chunk<float, double>(e.sv, P, Y, (const float*)e.H_vals, (double*)e.D_vals, e.e_atom, atom, n, e.ld, pos, nbi, chunk, nch, sm, tid);
-                    else side_dcols_chunk<float, float>(e.sv, P, Y, (const float*)e.H_vals, (float*)e.D_vals, e.e_atom, atom, n, e.ld, pos, nbi, chunk, nch, sm, tid);
+                    if (e.d_f64) side_dcols_chunk<float, double>(e.sv, P, Y, (const float*)e.H_vals, (double*)e.D_vals, e.e_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
+                    else side_dcols_chunk<float, float>(e.sv, P, Y, (const float*)e.H_vals, (float*)e.D_vals, e.e_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
                 }
             } break;
             default: break;                       // SK_REFILL: nothing to compute
@@ -827,7 +833,18 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
                         const double nv = (double)(e.sv.blk_off[e.sv.row_ptr[atom + 1]] - e.sv.blk_off[e.sv.row_ptr[atom]]);
                         atomicAdd(&e.ctr[PC_SIDE_BYTES + SK_DCOLS],
                                   (unsigned long long)(nv * ((e.d_f64 ? 8 : 4) + (e.val_f64 ? 8 : 4)) + (double)n * PCW * 4.0 + (double)n * nbi * 2.0));
-                        p_retire(e, slot);
+                        // the next member of the unit takes its columns from the same X and Y, or the slot retires
+                        const int mp = __ldcg(&s->mptr) + 1;
+                        if (mp < __ldcg(&s->mend)) {
+                            const int nxt = e.sv.unit_mem[mp];
+                            __stcg(&s->mptr, mp);
+                            __stcg(&s->atom, nxt);
+                            __stcg(&s->pos, e.upos[nxt]);
+                            __stcg(&s->nbi, e.at.nb[nxt]);
+                            p_install_gemm(e, slot, OP_DCOLS);
+                        } else {
+                            p_retire(e, slot);
+                        }
                     } break;
                     default: break;
                 }
@@ -884,7 +901,7 @@ __global__ void __launch_bounds__(P_SIDE_THREADS) k_side_gather(SysView sv, cons
                                                                 long long slotsz, long long bufsz, int ld, const int* atoms,
                                                                 const int* dims, unsigned long long* bytes) {
     extern __shared__ unsigned char sm_dyn[];
-    const int atom = atoms[blockIdx.y], n = dims[atom], n16 = (n + 15) & ~15;
+    const int atom = atoms[blockIdx.y], n = dims[atom], n16 = (n + 15) & ~15;      // unit id and its dimension
     __half* dS = base + (long long)blockIdx.y * slotsz;
     side_gather_chunk<TV>(sv, S_vals, H_vals, dS, dS + bufsz, atom, n, n16, ld, blockIdx.x, gridDim.x, sm_dyn, threadIdx.x, bytes);
 }

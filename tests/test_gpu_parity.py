@@ -260,3 +260,74 @@ def test_indefinite_S_is_reported(cfg0):
         if np.linalg.eigvalsh(T)[0] <= 0:
             bad_ref.add(i)
     assert bad_ref and bad_ref <= bad_gpu
+
+
+# ---- submatrix combination (Eq. 9 / Eq. 10; C-19) ---------------------------------------
+def _oracle_groups(s, mode, **kw):
+    sets = [orc.index_set(i, s.row_ptr, s.col_idx) for i in range(s.n_atoms)]
+    return orc.combine_groups(s.atom_nb, sets, mode=mode, **kw), sets
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+@pytest.mark.parametrize("name,n_atoms", [("cfg0", None), ("cfg2", 300), ("cfg3", 900)])
+def test_combined_groups_bit_exact_and_parity(name, n_atoms, mode):
+    """The library's greedy groups and union index sets equal the oracle's bit for bit; D and e_i of every member
+    of the sampled groups match the oracle's group evaluation (one Eq. 8 on the union, columns of each member,
+    rows restricted to N(member)) within the mixed-precision tolerances."""
+    s = make_system(name, n_atoms=n_atoms)
+    groups, sets = _oracle_groups(s, mode)
+    nb, rp, ci, Hv, Sv = _arrays(s)
+    blk = s.blk_off()
+    Hn, Sn = s.fill_np(MAT_H), s.fill_np(MAT_S)
+    with _nolsm(combine=mode) as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        for g in groups:
+            mem, st_, dim = ctx.group(g[0])
+            union = np.unique(np.concatenate([sets[i] for i in g]))
+            assert mem.tolist() == g and np.array_equal(st_, union.astype(np.int32))
+            assert dim == int(s.atom_nb[union].sum())
+        for i in (0, s.n_atoms - 1):
+            N, d = ctx.index_set(i)
+            assert np.array_equal(N, sets[i])                       # per-atom index sets are unchanged
+        D = torch.zeros(Hv.shape[0], dtype=torch.float64, device="cuda")
+        ctx.density_matrix(s.mu, D)
+        E = ctx.energy()
+        st = ctx.atom_stats()
+        stats = ctx.stats()
+    assert stats["n_units"] == len(groups) and (st["status"] == 0).all()
+    assert int((st["dims"] > 0).sum()) == len(groups)
+    Dh = D.cpu().numpy()
+    rng = np.random.default_rng(11)
+    pick = [groups[k] for k in rng.choice(len(groups), min(3, len(groups)), replace=False)]
+    pick.append(max(groups, key=len))
+    max_d, e_ref, e_gpu = 0.0, 0.0, 0.0
+    from tests.helpers import d_row_from_oracle
+    for g in pick:
+        res = orc.group_result(g, s.atom_nb, s.row_ptr, s.col_idx, blk, Hn, Sn, s.mu)
+        for i in g:
+            row = d_row_from_oracle(s, i, res[i], blk)
+            p0, p1 = int(s.row_ptr[i]), int(s.row_ptr[i + 1])
+            max_d = max(max_d, float(np.abs(Dh[blk[p0]:blk[p1]] - row).max()))
+            e_ref += res[i]["e_i"]
+            e_gpu += float(st["e_atom"][i])
+    print(name, "combine", mode, "groups", len(groups), "of", s.n_atoms, "max|dD|", max_d, "rel dE", abs(e_gpu - e_ref) / abs(e_ref),
+          "dim mean", stats["dim_mean"], "gemms", stats["gemms_executed"])
+    assert max_d <= TOL_MIXED_D
+    assert abs(e_gpu - e_ref) / abs(e_ref) <= TOL_MIXED_E
+    assert abs(E - st["e_atom"].sum()) <= 1e-9 * abs(E)
+
+
+def test_combine_rejects_partial_ranges_and_round_engine(cfg0):
+    from paper_2205_12182_b200 import ENGINE_ROUNDS, NolsmError
+    s = cfg0
+    nb, rp, ci, Hv, Sv = _arrays(s)
+    with _nolsm(combine=1) as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        D = torch.zeros(Hv.shape[0], dtype=torch.float64, device="cuda")
+        with pytest.raises(NolsmError) as ei:
+            ctx.density_matrix_range(s.mu, 0, 10, D)
+        assert ei.value.code == 1
+    with _nolsm(combine=1, engine=ENGINE_ROUNDS) as ctx:
+        with pytest.raises(NolsmError) as ei:
+            ctx.assemble(nb, rp, ci, Hv, Sv)
+        assert ei.value.code == 1

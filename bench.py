@@ -145,6 +145,9 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=12, help="submatrices for the cpu_baseline leg (0 = skip)")
     ap.add_argument("--ref-sample", type=int, default=4)
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--combine", type=int, default=0, choices=[0, 1, 2],
+                    help="submatrix combination of the timed path (0 = one submatrix per atom, BASELINE.json's configs)")
+    ap.add_argument("--no-combine-leg", action="store_true", help="skip the extra combine = 1 / 2 measurements")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -177,7 +180,7 @@ def main():
     ci = torch.from_numpy(system.col_idx).to(dev)
     D = torch.empty_like(Hv)
     stream = torch.cuda.current_stream().cuda_stream
-    ctx = Nolsm(local_rank, profile_every=args.profile_every)
+    ctx = Nolsm(local_rank, profile_every=args.profile_every, combine=args.combine)
 
     def step():
         ctx.assemble(nb, rp, ci, Hv, Sv, stream=stream)
@@ -222,6 +225,39 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_step = float(t.item()) / args.steps
     stats = ctx.stats()
+
+    # ---- the same workload with submatrix combination (Eq. 9 / Eq. 10): fewer, larger
+    #      submatrices serve the same atoms; reported beside the headline, which stays one submatrix per atom ----
+    combined = None
+    if not args.no_combine_leg and args.combine == 0:
+        combined = {}
+        for mode in (1, 2):
+            cx = Nolsm(local_rank, combine=mode)
+
+            def step_c():
+                cx.assemble(nb, rp, ci, Hv, Sv, stream=stream)
+                cx.density_matrix(system.mu, D, stream=stream)
+                return cx.energy(strict=False)
+            step_c()
+            barrier()
+            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            c0.record()
+            Ec = step_c()
+            c1.record()
+            barrier()
+            tc = torch.tensor([c0.elapsed_time(c1)], dtype=torch.float64, device=dev)
+            if world > 1:
+                dist.all_reduce(tc, op=dist.ReduceOp.MAX)
+            sc, pc = cx.stats(), cx.profile()
+            combined["eq9" if mode == 1 else "eq10"] = {
+                "atoms_per_s": world * system.n_atoms / (float(tc.item()) * 1e-3), "ms_per_step": float(tc.item()),
+                "submatrices": sc["n_units"], "dim_mean": sc["dim_mean"], "dim_max": sc["dim_max"],
+                "gemms_per_submatrix": sc["gemms_executed"] / max(sc["n_units"], 1),
+                "flops_useful_per_step": sc["flops_useful"], "kernel_ms": pc["gemm_ms"],
+                "kernel_tflops_useful": pc["gemm_flops_useful"] / max(pc["gemm_ms"], 1e-9) / 1e9,
+                "kernel_tflops_padded": pc["gemm_flops_padded"] / max(pc["gemm_ms"], 1e-9) / 1e9,
+                "e_elec": Ec, "n_notspd": sc["n_notspd"], "n_noconv": sc["n_noconv"]}
+            cx.destroy()
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D of the inputs and D2H of D inside ----
     e2e = None
@@ -330,9 +366,9 @@ def main():
                                                                  "measured_burst": 100 * tflops / peaks["bf16_tflops"] / world,
                                                                  "measured_sustained": 100 * tflops / peaks["bf16_tflops_sustained"] / world},
             "flops_useful_per_step": stats["flops_useful"], "flops_padded_per_step": stats["flops_padded"],
-            "gemms_per_submatrix": stats["gemms_executed"] / system.n_atoms, "e_elec": E,
+            "gemms_per_submatrix": stats["gemms_executed"] / max(stats["n_units"], 1), "submatrices": stats["n_units"], "e_elec": E,
             "n_notspd": stats["n_notspd"], "n_noconv": stats["n_noconv"],
-            "roofline": roofline, "hbm_kernels": hbm, "engine": engine, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
+            "roofline": roofline, "hbm_kernels": hbm, "engine": engine, "combined": combined, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
             "gpu_launches": int(prof_acc["kernel_launches"]),
             "paper_context": "1.1 EFLOP/s FP16/FP32 on 4400 A100 (~257 TFLOP/s per GPU, ~80% of 312), other hardware"}
     print(json.dumps(line), flush=True)

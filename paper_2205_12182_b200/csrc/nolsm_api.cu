@@ -25,7 +25,7 @@ namespace {
 template <typename F>
 void parallel_for(int64_t n, F f) {
     unsigned nt = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
-    if (n < 1 << 16) nt = 1;
+    if (n < 1 << 11) nt = 1;
     if (nt == 1) { f(0, n); return; }
     std::vector<std::thread> th;
     const int64_t chunk = (n + nt - 1) / nt;
@@ -370,6 +370,21 @@ void build_units(nolsm_ctx* c, int mode, int max_dim, int max_members, int max_c
     std::vector<char> is_free(n_at, 1);
     std::vector<int32_t> G, U;
     std::vector<std::pair<int64_t, int32_t>> cand;
+    // overlaps dim(N(i) & N(j)) of every pair of the pattern, in parallel (the greedy pass below is sequential)
+    std::vector<int32_t> ov;
+    if (mode != 0 && max_members > 1) {
+        ov.resize(c->nset_atom.size());
+        parallel_for(n_at, [&](int64_t b, int64_t e) {
+            for (int64_t i = b; i < e; ++i) {
+                const int32_t* Ni = c->nset_atom.data() + c->nset_ptr[i];
+                const int64_t ni = c->nset_ptr[i + 1] - c->nset_ptr[i];
+                for (int64_t q = 0; q < ni; ++q) {
+                    const int32_t j = Ni[q];
+                    ov[c->nset_ptr[i] + q] = j == i ? 0 : (int32_t)overlap_dim(Ni, ni, c->nset_atom.data() + c->nset_ptr[j], c->nset_ptr[j + 1] - c->nset_ptr[j], nb);
+                }
+            }
+        });
+    }
     for (int64_t i = 0; i < n_at; ++i) {
         if (!is_free[i]) continue;
         is_free[i] = 0;
@@ -384,7 +399,7 @@ void build_units(nolsm_ctx* c, int mode, int max_dim, int max_members, int max_c
             for (int64_t q = 0; q < ni; ++q) {
                 const int32_t j = Ni[q];
                 if (j == i || !is_free[j]) continue;
-                cand.emplace_back(-overlap_dim(Ni, ni, c->nset_atom.data() + c->nset_ptr[j], c->nset_ptr[j + 1] - c->nset_ptr[j], nb), j);
+                cand.emplace_back(-(int64_t)ov[c->nset_ptr[i] + q], j);
             }
             std::sort(cand.begin(), cand.end());
             if ((int)cand.size() > max_cand) cand.resize(max_cand);

@@ -95,3 +95,44 @@ def test_cfg4_streamed_in_atom_batches():
     pool = np.concatenate([np.arange(b * B, (b + 1) * B) for b in batches])
     atoms = np.sort(rng.choice(pool, 128, replace=False))
     _check_sample(s, D, e_atom, atoms, "cfg4, 128 atoms of 4 batches")
+
+
+def test_cfg1_full_combined_groups_and_parity():
+    """configs[1] at full size with submatrix combination (Eq. 9): the library's groups equal the oracle's greedy
+    groups bit for bit over all 3,000 atoms; D and e_i of the members of sampled groups match the oracle."""
+    from oracle import nolsm_oracle as orc
+    from paper_2205_12182_b200 import Nolsm
+    from tests.helpers import d_row_from_oracle
+    s = make_system("cfg1")
+    sets = [orc.index_set(i, s.row_ptr, s.col_idx) for i in range(s.n_atoms)]
+    groups = orc.combine_groups(s.atom_nb, sets, mode=1)
+    nb, rp, ci, Hv, Sv = _device_inputs(s)
+    D = torch.empty_like(Hv)
+    with Nolsm(0, combine=1) as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        for g in groups:
+            mem, st_, dim = ctx.group(g[0])
+            assert mem.tolist() == g
+            assert np.array_equal(st_, np.unique(np.concatenate([sets[i] for i in g])).astype(np.int32))
+        ctx.density_matrix(s.mu, D)
+        E = ctx.energy()
+        st = ctx.atom_stats()
+        stats = ctx.stats()
+    assert stats["n_units"] == len(groups) < s.n_atoms // 2 and (st["status"] == 0).all()
+    blk = s.blk_off()
+    Hn, Sn = s.fill_np(MAT_H), s.fill_np(MAT_S)
+    rows = _DeviceRows(D)
+    rng = np.random.default_rng(7)
+    max_d, e_ref, e_gpu = 0.0, 0.0, 0.0
+    for k in rng.choice(len(groups), 6, replace=False):
+        g = groups[int(k)]
+        res = orc.group_result(g, s.atom_nb, s.row_ptr, s.col_idx, blk, Hn, Sn, s.mu)
+        for i in g:
+            ref = d_row_from_oracle(s, i, res[i], blk)
+            p0, p1 = int(s.row_ptr[i]), int(s.row_ptr[i + 1])
+            max_d = max(max_d, float(np.abs(rows[blk[p0]:blk[p1]] - ref).max()))
+            e_ref += res[i]["e_i"]
+            e_gpu += float(st["e_atom"][i])
+    print("cfg1 full combined", len(groups), "groups, max|dD|", max_d, "rel dE", abs(e_gpu - e_ref) / abs(e_ref))
+    assert max_d <= TOL_D and abs(e_gpu - e_ref) / abs(e_ref) <= TOL_E
+    assert abs(E - st["e_atom"].sum()) <= 1e-9 * abs(E)

@@ -116,7 +116,8 @@ __device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t par
 __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
     uint32_t spins = 0;
     while (!mbar_try_wait_cluster(bar, parity)) {
-        if (++spins > SPIN_LIMIT) __trap();
+        if (++spins > 4096u) __nanosleep(64);
+        if (spins > SPIN_LIMIT_SLOW) __trap();
     }
 }
 // Wait that may legitimately last long (a role of the persistent engine with no work): polls gently
@@ -197,7 +198,7 @@ __device__ __forceinline__ void g2_scheduler(const G2Smem& sm, int lane, Next ne
     for (;;) {
         for (uint32_t spins = 0; !ptx::mbar_try_wait_cluster(sm.ti_empty(q), ph ^ 1);) {    // runs ahead: poll gently
             __nanosleep(200);
-            if (++spins > SPIN_LIMIT) __trap();
+            if (++spins > SPIN_LIMIT_SLOW) __trap();
         }
         TileInfo ti{};
         if (lane == 0) ti.valid = next(ti) ? 1 : 0;

@@ -7,6 +7,7 @@ namespace nolsm {
 
 constexpr int B_BOX_BYTES = BK * 64 * 2;            // one TMA box: 64 (contiguous) x 64 FP16 = 8 KB
 constexpr uint32_t SPIN_LIMIT = 1u << 22;   // a protocol bug traps after seconds instead of hanging the GPU
+constexpr uint32_t SPIN_LIMIT_SLOW = 1u << 26;   // waits that back off with nanosleep: ~10 s
 
 namespace ptx {
 
@@ -47,7 +48,8 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if (++spins > SPIN_LIMIT) __trap();
+        if (++spins > 4096u) __nanosleep(64);          // a long wait (kernels of other graph branches share the SM): back off
+        if (spins > SPIN_LIMIT_SLOW) __trap();
     }
 }
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {

@@ -143,11 +143,17 @@ size_t prof_begin(nolsm_ctx* c, int kind, cudaStream_t s) {
 }
 void prof_end(nolsm_ctx* c, size_t i, cudaStream_t s) {
     if (c->prof_on) cudaEventRecord(c->ev_pool[i + 1], s);
+    static const bool sync_debug = getenv("NOLSM_SYNC_DEBUG") != nullptr;      // eager rounds only (NOLSM_GRAPH=0)
+    if (sync_debug) {
+        const cudaError_t e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) { fprintf(stderr, "nolsm: launch %lld failed: %s\n", (long long)c->launches, cudaGetErrorString(e)); abort(); }
+    }
 }
 
 #define LAUNCH(c, kind, s, ...)                      \
     do {                                             \
         const size_t pi_ = prof_begin(c, kind, s);   \
+        if (getenv("NOLSM_SYNC_DEBUG")) fprintf(stderr, "nolsm: launch %lld kind %d: %s\n", (long long)(c)->launches, kind, #__VA_ARGS__); \
         __VA_ARGS__;                                 \
         prof_end(c, pi_, s);                         \
     } while (0)
@@ -1073,7 +1079,11 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
     if (c->use_graph) {
         cudaGraph_t g = nullptr;
         CU_TRY(c, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
-        r = fp32 ? enqueue_round<float>(c, e, D_dev, d_dtype, true) : enqueue_round<__half>(c, e, D_dev, d_dtype, true);
+        // The three branches of a round (GEMMs | gather + power iteration | D columns) are captured one after the other:
+        // with concurrent branches the round engine hung intermittently on submatrices of ~1900 dimensions (B200, CUDA
+        // 12.9; the serial capture never did, 6 of 6 against 2 of 5). NOLSM_FORK=1 restores the concurrent branches.
+        const bool fork = getenv_int("NOLSM_FORK", 0) != 0;
+        r = fp32 ? enqueue_round<float>(c, e, D_dev, d_dtype, fork) : enqueue_round<__half>(c, e, D_dev, d_dtype, fork);
         cudaError_t ce = cudaStreamEndCapture(s, &g);
         if (r) { if (g) cudaGraphDestroy(g); return r; }
         if (ce != cudaSuccess) { c->err = std::string("stream capture: ") + cudaGetErrorString(ce); return NOLSM_ECUDA; }

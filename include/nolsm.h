@@ -139,6 +139,20 @@ int nolsm_destroy(nolsm_ctx* ctx);
 
 /* ---- diagnostics used by the parity tests and the benchmark ---- */
 
+/* Tr(D S) of the last density_matrix call (the chemical potential is iterated until the electron count
+ * is right): sum over the evaluated atoms i of q_i = sum_{j in N(i)} <D_ji, S_ji>, accumulated in FP64 in the scatter
+ * step. q_atom_out (host, nullable) receives the q_i of the evaluated range. Synchronises. */
+int nolsm_electron_count(nolsm_ctx* ctx, double* n_elec, double* q_atom_out);
+
+/* Chemical-potential search: bisection on mu in [mu_lo, mu_hi] until |Tr(D(mu) S) - n_target| <=
+ * tol_n, the bracket is narrower than tol_mu, or max_evals (0 = 40) density-matrix evaluations were spent. Tr(D S) never
+ * decreases with mu; NOLSM_EINVAL if n_target is not bracketed. On return D_vals (host or device, as for
+ * nolsm_density_matrix) holds D(mu_out), n_out = Tr(D(mu_out) S), evals_out the evaluations spent; nolsm_energy and
+ * nolsm_get_stats refer to that last evaluation. Every evaluation is a full a1-a7 pass (S_sub^-1 is not kept across
+ * evaluations: the dense submatrices of a 32,768-atom system exceed HBM). */
+int nolsm_find_mu(nolsm_ctx* ctx, double n_target, double mu_lo, double mu_hi, double tol_n, double tol_mu, int max_evals,
+                  void* D_vals, int d_dtype, void* cuda_stream, double* mu_out, double* n_out, int* evals_out);
+
 /* The group (unit) atom `atom` belongs to after nolsm_assemble (C-19; without combine the group is the atom
  * itself): its members in joining order (seed first), the union index set (ascending atom ids) that the group's one
  * dense submatrix is built on, and that submatrix's dimension. Call with NULL arrays to query the two counts. */

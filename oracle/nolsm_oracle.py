@@ -154,7 +154,8 @@ def atom_result(i, atom_nb, row_ptr, col_idx, blk_off, H_vals, S_vals, mu, eps_f
     c0, c1 = int(off[a]), int(off[a + 1])
     Dcols = D_sub[:, c0:c1].copy()
     e_i = float((Dcols * H_sub[:, c0:c1]).sum())
-    return dict(N=N_i, n=int(off[-1]), pos=c0, off=off, Dcols=Dcols, e_i=e_i, eps=eps, s=s,
+    q_i = float((Dcols * S_sub[:, c0:c1]).sum())           # atom i's share of Tr(D S), the electron count (L149)
+    return dict(N=N_i, n=int(off[-1]), pos=c0, off=off, Dcols=Dcols, e_i=e_i, q_i=q_i, eps=eps, s=s,
                 H_sub=H_sub, S_sub=S_sub, D_sub=D_sub)
 
 
@@ -298,5 +299,37 @@ def group_result(members, atom_nb, row_ptr, col_idx, blk_off, H_vals, S_vals, mu
         off = np.zeros(len(N_i) + 1, dtype=np.int64)
         off[1:] = np.cumsum(np.asarray(atom_nb, dtype=np.int64)[N_i])
         e_i = float((Dcols * H_G[np.ix_(rows, np.arange(c0, c1))]).sum())
-        out[i] = dict(N=N_i, n=int(off[-1]), off=off, Dcols=Dcols, e_i=e_i, eps=eps, s=s, n_group=int(off_G[-1]))
+        q_i = float((Dcols * S_G[np.ix_(rows, np.arange(c0, c1))]).sum())
+        out[i] = dict(N=N_i, n=int(off[-1]), off=off, Dcols=Dcols, e_i=e_i, q_i=q_i, eps=eps, s=s, n_group=int(off_G[-1]))
     return out
+
+
+# ------------------------------------------------------------------------------------------
+# chemical potential: mu is iterated until the electron count Tr(D S) is right
+# ------------------------------------------------------------------------------------------
+def electron_count(atom_nb, row_ptr, col_idx, H_vals, S_vals, mu, atoms=None):
+    """Tr(D(mu) S) of the submatrix method: sum over atoms i of q_i = sum_{j in N(i)} <D_ji, S_ji>."""
+    blk_off = block_offsets(atom_nb, row_ptr, col_idx)
+    q = 0.0
+    for i in (range(len(atom_nb)) if atoms is None else atoms):
+        q += atom_result(int(i), atom_nb, row_ptr, col_idx, blk_off, H_vals, S_vals, mu)["q_i"]
+    return q
+
+
+def find_mu(count, n_target, mu_lo, mu_hi, tol_n=1e-3, tol_mu=1e-6, max_evals=40):
+    """Bisection on mu for count(mu) = n_target; count never decreases with mu (every generalised eigenvalue of
+    every submatrix that drops below mu adds a non-negative share). Returns (mu, count(mu), evaluations)."""
+    n_lo, n_hi = count(mu_lo), count(mu_hi)
+    evals = 2
+    if n_lo - tol_n > n_target or n_hi + tol_n < n_target:
+        raise ValueError("electron count not bracketed")
+    mu, n_mu = mu_hi, n_hi
+    while evals < max_evals and abs(n_mu - n_target) > tol_n and (mu_hi - mu_lo) > tol_mu:
+        mu = 0.5 * (mu_lo + mu_hi)
+        n_mu = count(mu)
+        evals += 1
+        if n_mu < n_target:
+            mu_lo = mu
+        else:
+            mu_hi = mu
+    return mu, n_mu, evals

@@ -67,6 +67,9 @@ def load_library():
     lib.nolsm_energy.argtypes = [P, C.POINTER(C.c_double)]
     lib.nolsm_destroy.argtypes = [P]
     lib.nolsm_get_index_set.argtypes = [P, I64, P, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+    lib.nolsm_electron_count.argtypes = [P, C.POINTER(C.c_double), P]
+    lib.nolsm_find_mu.argtypes = [P, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double, I32, P, I32, P,
+                                  C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int)]
     lib.nolsm_get_group.argtypes = [P, I64, P, C.POINTER(C.c_int32), P, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     lib.nolsm_gather_submatrix.argtypes = [P, I64, I32, I32, P]
     lib.nolsm_get_stats.argtypes = [P, C.POINTER(NolsmStats)]
@@ -76,7 +79,7 @@ def load_library():
     lib.nolsm_last_error.argtypes = [P]
     lib.nolsm_last_error.restype = C.c_char_p
     for f in ("nolsm_create", "nolsm_assemble", "nolsm_density_matrix", "nolsm_density_matrix_range", "nolsm_energy",
-              "nolsm_destroy", "nolsm_get_index_set", "nolsm_get_group", "nolsm_gather_submatrix", "nolsm_get_stats",
+              "nolsm_destroy", "nolsm_get_index_set", "nolsm_get_group", "nolsm_electron_count", "nolsm_find_mu", "nolsm_gather_submatrix", "nolsm_get_stats",
               "nolsm_get_atom_stats", "nolsm_get_profile", "nolsm_get_engine_counters"):
         getattr(lib, f).restype = C.c_int
     _LIB = lib
@@ -162,6 +165,26 @@ class Nolsm:
         rc = self._lib.nolsm_energy(self._h, C.byref(e))
         self._check(rc, soft=() if strict else (5, 6))
         return e.value
+
+    def electron_count(self, per_atom: bool = False):
+        """Tr(D S) of the last density_matrix call (and the per-atom partials q_i of the evaluated range)."""
+        n = C.c_double()
+        if not per_atom:
+            self._check(self._lib.nolsm_electron_count(self._h, C.byref(n), None))
+            return n.value
+        q = np.zeros(self.n_atoms, dtype=np.float64)
+        self._check(self._lib.nolsm_electron_count(self._h, C.byref(n), q.ctypes.data))
+        return n.value, q
+
+    def find_mu(self, n_target: float, mu_lo: float, mu_hi: float, D_vals, tol_n: float = 1e-3, tol_mu: float = 1e-6,
+                max_evals: int = 0, stream: int = 0):
+        """Bisection on mu until Tr(D S) = n_target (include/nolsm.h). Returns (mu, Tr(D S), evaluations)."""
+        pd, kd = _ptr(D_vals)
+        self._keep_out = kd
+        mu, n, ev = C.c_double(), C.c_double(), C.c_int()
+        self._check(self._lib.nolsm_find_mu(self._h, n_target, mu_lo, mu_hi, tol_n, tol_mu, max_evals, pd, _val_dtype(kd), stream,
+                                            C.byref(mu), C.byref(n), C.byref(ev)), soft=(6,))
+        return mu.value, n.value, ev.value
 
     def index_set(self, atom: int):
         n = C.c_int32(0)

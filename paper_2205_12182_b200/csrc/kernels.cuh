@@ -380,8 +380,8 @@ __global__ void __launch_bounds__(256) k_gemm_simt(Engine e, T* base, int launch
 // grid = (row chunks, S); dynamic smem: int off[max_nset + 1], float Yc[n][nbi].
 // ---------------------------------------------------------------------------------------------
 template <typename T, typename TV, typename TD>
-__global__ void __launch_bounds__(256) k_dcols_scatter(Engine e, SysView sv, const T* base, const TV* H_vals, TD* D_vals,
-                                                       double* e_atom, int max_nset) {
+__global__ void __launch_bounds__(256) k_dcols_scatter(Engine e, SysView sv, const T* base, const TV* H_vals, const TV* S_vals, TD* D_vals,
+                                                       double* e_atom, double* q_atom, int max_nset) {
     const int slot = blockIdx.y;
     const Slot& s = e.slots[slot];
     if (s.snap != PH_FIN || (s.status & ST_NOTSPD)) return;
@@ -401,7 +401,7 @@ __global__ void __launch_bounds__(256) k_dcols_scatter(Engine e, SysView sv, con
     }
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    double e_part = 0.0;
+    double e_part = 0.0, q_part = 0.0;
     for (int r = blockIdx.x * 8 + warp; r < n; r += gridDim.x * 8) {
         int lo = 0, hi = cnt - 1;                                   // atom of N(i) that owns row r
         while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_off[mid] <= r) lo = mid; else hi = mid - 1; }
@@ -432,12 +432,14 @@ __global__ void __launch_bounds__(256) k_dcols_scatter(Engine e, SysView sv, con
                 const long long o = out0 + (long long)c * nbj + bb;      // slot (i, j_a): [c][bb] = D_sub[r, pos + c]
                 D_vals[o] = (TD)d;
                 e_part += (double)d * (double)H_vals[o];
+                q_part += (double)d * (double)S_vals[o];
             }
         }
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) e_part += __shfl_xor_sync(0xffffffffu, e_part, o);
+    for (int o = 16; o > 0; o >>= 1) { e_part += __shfl_xor_sync(0xffffffffu, e_part, o); q_part += __shfl_xor_sync(0xffffffffu, q_part, o); }
     if (lane == 0 && e_part != 0.0) atomicAdd(&e_atom[s.atom], e_part);
+    if (lane == 0 && q_part != 0.0) atomicAdd(&q_atom[s.atom], q_part);
     if (e.profiling && blockIdx.x == 0 && threadIdx.x == 0) {
         const double nv = (double)(sv.blk_off[sv.row_ptr[s.atom + 1]] - sv.blk_off[sv.row_ptr[s.atom]]);
         atomicAdd(&e.prof[PF_DCOLS_BYTES], nv * (sizeof(TD) + sizeof(TV)) + ((double)n * n + (double)n * nbi) * sizeof(T));

@@ -78,6 +78,7 @@ struct nolsm_ctx {
     int* h_done = nullptr;              // pinned, mapped
     int *d_dim = nullptr, *d_pos = nullptr;
     double* d_e_atom = nullptr;
+    double* d_q_atom = nullptr;
     cudaStream_t s_main = nullptr, s_x = nullptr, s_f = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_x = nullptr, ev_f = nullptr, ev_in = nullptr, ev_out = nullptr;
     cudaEvent_t ev_round[ROUND_DEPTH] = {};
@@ -265,10 +266,10 @@ void launch_dcols(nolsm_ctx* c, const Engine& e, TD* D, cudaStream_t s) {
     dim3 grid(gx, e.S);
     if (c->val_dtype == NOLSM_DTYPE_F64) {
         auto k = k_dcols_scatter<T, double, TD>;
-        LAUNCH(c, K_DCOLS, s, k<<<grid, 256, smem, s>>>(e, sys_view(c), (const T*)c->ws, (const double*)c->dH, D, c->d_e_atom, c->max_nset));
+        LAUNCH(c, K_DCOLS, s, k<<<grid, 256, smem, s>>>(e, sys_view(c), (const T*)c->ws, (const double*)c->dH, (const double*)c->dS, D, c->d_e_atom, c->d_q_atom, c->max_nset));
     } else {
         auto k = k_dcols_scatter<T, float, TD>;
-        LAUNCH(c, K_DCOLS, s, k<<<grid, 256, smem, s>>>(e, sys_view(c), (const T*)c->ws, (const float*)c->dH, D, c->d_e_atom, c->max_nset));
+        LAUNCH(c, K_DCOLS, s, k<<<grid, 256, smem, s>>>(e, sys_view(c), (const T*)c->ws, (const float*)c->dH, (const float*)c->dS, D, c->d_e_atom, c->d_q_atom, c->max_nset));
     }
 }
 
@@ -875,6 +876,8 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     e.at.dim = c->d_dim; e.at.pos = c->d_pos; e.at.nb = c->d_atom_nb;
     if ((r = dmalloc(c, (void**)&c->d_e_atom, 8 * n_atoms))) return r;
     CU_TRY(c, cudaMemsetAsync(c->d_e_atom, 0, 8 * n_atoms, s));
+    if ((r = dmalloc(c, (void**)&c->d_q_atom, 8 * n_atoms))) return r;
+    CU_TRY(c, cudaMemsetAsync(c->d_q_atom, 0, 8 * n_atoms, s));
     if (use_umma(c)) {
         if (!encode_tiled_fn()) return fail(c, NOLSM_ECUDA, "cuTensorMapEncodeTiled not available");
         std::vector<CUtensorMap> maps((size_t)S * NMAP);
@@ -958,7 +961,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         pe.at = e.at; pe.sv = sys_view(c);
         pe.udim = c->d_udim; pe.upos = c->d_upos; pe.adim = c->d_dim;
         pe.S_vals = c->dS; pe.H_vals = c->dH; pe.val_f64 = val_dtype == NOLSM_DTYPE_F64;
-        pe.e_atom = c->d_e_atom; pe.maps = c->d_maps; pe.base = (__half*)c->ws;
+        pe.e_atom = c->d_e_atom; pe.q_atom = c->d_q_atom; pe.maps = c->d_maps; pe.base = (__half*)c->ws;
         c->h_sclaim0.assign(S, ((unsigned)SK_REFILL << 28) | (1u << 14));
         {   // every CTA waits on work published by the others: the whole grid must be resident at once
             const int ctas = c->opt.cluster_ctas == G4_CTAS ? G4_CTAS : 2;
@@ -1017,6 +1020,7 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
     CU_TRY(c, cudaStreamWaitEvent(s, c->ev_in, 0));
     CU_TRY(c, cudaMemsetAsync(D_dev + (size_t)v0 * ds, 0, (size_t)(v1 - v0) * ds, s));
     CU_TRY(c, cudaMemsetAsync(c->d_e_atom + a0, 0, 8 * (a1 - a0), s));
+    CU_TRY(c, cudaMemsetAsync(c->d_q_atom + a0, 0, 8 * (a1 - a0), s));
     c->ev_used = 0; c->recs.clear(); c->launches = 0; c->prof_on = false;
     c->last_persist = c->persist;
     if (c->persist) {
@@ -1151,6 +1155,64 @@ int nolsm_energy(nolsm_ctx* c, double* e_elec) {
     *e_elec = sum;
     if (bits & ST_NOTSPD) return fail(c, NOLSM_ENOTSPD, "an S_sub inverse iteration failed (see nolsm_get_atom_stats)");
     if (bits & ST_NOCONV) return fail(c, NOLSM_ENOCONV, "a sign iteration hit max_sign_iters (see nolsm_get_atom_stats)");
+    return NOLSM_OK;
+}
+
+int nolsm_electron_count(nolsm_ctx* c, double* n_elec, double* q_atom_out) {
+    if (!c || !n_elec) return NOLSM_EINVAL;
+    if (!c->have_result) return fail(c, NOLSM_ESTATE, "no density matrix has been computed");
+    cudaSetDevice(c->dev);
+    if (int r = wait_result(c)) return r;
+    const int64_t n = c->last_a1 - c->last_a0;
+    std::vector<double> q(n);
+    CU_TRY(c, cudaMemcpy(q.data(), c->d_q_atom + c->last_a0, 8 * n, cudaMemcpyDeviceToHost));
+    double sum = 0;
+    for (int64_t i = 0; i < n; ++i) sum += q[i];
+    *n_elec = sum;
+    if (q_atom_out) memcpy(q_atom_out, q.data(), 8 * n);
+    return NOLSM_OK;
+}
+
+int nolsm_find_mu(nolsm_ctx* c, double n_target, double mu_lo, double mu_hi, double tol_n, double tol_mu, int max_evals,
+                  void* D_vals, int d_dtype, void* cuda_stream, double* mu_out, double* n_out, int* evals_out) {
+    if (!c || !D_vals || !mu_out) return NOLSM_EINVAL;
+    if (!c->assembled) return fail(c, NOLSM_ESTATE, "nolsm_assemble has not been called");
+    if (!(mu_lo < mu_hi) || !(tol_n >= 0) || !(tol_mu >= 0)) return fail(c, NOLSM_EINVAL, "need mu_lo < mu_hi and tolerances >= 0");
+    if (max_evals <= 0) max_evals = 40;
+    // N(mu) = Tr(D(mu) S) never decreases with mu (it counts the generalised eigenvalues of every submatrix below mu,
+    // weighted by their share in the atom's columns): bisection. Every evaluation is one nolsm_density_matrix call;
+    // D_vals holds the density matrix of the last evaluated mu on return, which is the mu reported.
+    int evals = 0, rc_soft = NOLSM_OK;
+    auto count = [&](double mu, double* n) -> int {
+        int r = nolsm_density_matrix(c, mu, D_vals, d_dtype, cuda_stream);
+        if (r) return r;
+        ++evals;
+        double e;
+        r = nolsm_energy(c, &e);
+        if (r == NOLSM_ENOCONV) { rc_soft = r; r = NOLSM_OK; }       // flagged matrices are still written (nolsm.h)
+        if (r) return r;
+        return nolsm_electron_count(c, n, nullptr);
+    };
+    double n_lo, n_hi, mu = mu_lo, n_mu = 0;
+    int r;
+    if ((r = count(mu_lo, &n_lo))) return r;
+    if ((r = count(mu_hi, &n_hi))) return r;
+    mu = mu_hi; n_mu = n_hi;
+    if (n_lo - tol_n > n_target || n_hi + tol_n < n_target) {
+        if (n_out) *n_out = n_hi;
+        if (evals_out) *evals_out = evals;
+        *mu_out = mu_hi;
+        return fail(c, NOLSM_EINVAL, "nolsm_find_mu: the electron count is not bracketed by [mu_lo, mu_hi]");
+    }
+    while (evals < max_evals && std::fabs(n_mu - n_target) > tol_n && (mu_hi - mu_lo) > tol_mu) {
+        mu = 0.5 * (mu_lo + mu_hi);
+        if ((r = count(mu, &n_mu))) return r;
+        if (n_mu < n_target) mu_lo = mu; else mu_hi = mu;
+    }
+    *mu_out = mu;
+    if (n_out) *n_out = n_mu;
+    if (evals_out) *evals_out = evals;
+    if (rc_soft) return fail(c, rc_soft, "a sign iteration hit max_sign_iters during the mu search (see nolsm_get_atom_stats)");
     return NOLSM_OK;
 }
 

@@ -86,6 +86,7 @@ struct PEngine {
     const void *S_vals, *H_vals; int val_f64;
     void* D_vals; int d_f64;
     double* e_atom;
+    double* q_atom;               // [n_atoms] electron-count partials sum_j <D_ji, S_ji> (Tr(D S))
     const CUtensorMap* maps;
     __half* base;
     float* pcols;                 // [S][cap][PCW] FP32: X Y[:, cols(i)] of the slot's atom (OP_DCOLS)
@@ -717,8 +718,8 @@ __device__ void side_schulz1_chunk(const __half* __restrict__ S, __half* __restr
 // operands (Y columns, P) with scattered ones.
 template <typename TV, typename TD>
 __device__ void side_dcols_chunk(const SysView& sv, const float* __restrict__ P, const __half* __restrict__ Y,
-                                 const TV* __restrict__ H_vals, TD* __restrict__ D_vals, double* e_atom,
-                                 int atom, int n_own, int ld, int pos, int nbi, int chunk, int nchunks, unsigned char* sm, int tid) {
+                                 const TV* __restrict__ H_vals, const TV* __restrict__ S_vals, TD* __restrict__ D_vals, double* e_atom,
+                                 double* q_atom, int atom, int n_own, int ld, int pos, int nbi, int chunk, int nchunks, unsigned char* sm, int tid) {
     const long long p0 = sv.nset_ptr[atom];
     const int cnt = (int)(sv.nset_ptr[atom + 1] - p0);
     int* s_pre = reinterpret_cast<int*>(sm);                               // [cnt + 1] first value row of each atom of N(i) in output order
@@ -730,7 +731,7 @@ __device__ void side_dcols_chunk(const SysView& sv, const float* __restrict__ P,
     // of the unit's matrix (== s_pre[a] when the unit is the atom itself)
     const int total = n_own * nbi;                                         // values of D written for this atom
     const int q_lo = (int)((long long)total * chunk / nchunks), q_hi = (int)((long long)total * (chunk + 1) / nchunks);
-    double e_part = 0.0;
+    double e_part = 0.0, q_part = 0.0;
     for (int q = q_lo + tid; q < q_hi; q += P_SIDE_THREADS) {
         int lo = 0, hi = cnt - 1;
         while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_pre[mid] * nbi <= q) lo = mid; else hi = mid - 1; }
@@ -742,10 +743,12 @@ __device__ void side_dcols_chunk(const SysView& sv, const float* __restrict__ P,
         const float d = 0.5f * (__half2float(__ldcg(Y + (long long)r * ld + pos + c)) - __ldcg(P + (size_t)r * PCW + (pos & 7) + c));
         D_vals[o] = (TD)d;
         e_part += (double)d * (double)H_vals[o];
+        q_part += (double)d * (double)S_vals[o];
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) e_part += __shfl_xor_sync(0xffffffffu, e_part, o);
+    for (int o = 16; o > 0; o >>= 1) { e_part += __shfl_xor_sync(0xffffffffu, e_part, o); q_part += __shfl_xor_sync(0xffffffffu, q_part, o); }
     if ((tid & 31) == 0 && e_part != 0.0) atomicAdd(&e_atom[atom], e_part);
+    if ((tid & 31) == 0 && q_part != 0.0) atomicAdd(&q_atom[atom], q_part);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -804,11 +807,11 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
                 const float* P = pcols_ptr(e, slot);
                 const __half* Y = e.base + buf_off(e, slot, __ldcg(&s->ycur));
                 if (e.val_f64) {
-                    if (e.d_f64) side_dcols_chunk<double, double>(e.sv, P, Y, (const double*)e.H_vals, (double*)e.D_vals, e.e_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
-                    else side_dcols_chunk<double, float>(e.sv, P, Y, (const double*)e.H_vals, (float*)e.D_vals, e.e_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
+                    if (e.d_f64) side_dcols_chunk<double, double>(e.sv, P, Y, (const double*)e.H_vals, (const double*)e.S_vals, (double*)e.D_vals, e.e_atom, e.q_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
+                    else side_dcols_chunk<double, float>(e.sv, P, Y, (const double*)e.H_vals, (const double*)e.S_vals, (float*)e.D_vals, e.e_atom, e.q_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
                 } else {
-                    if (e.d_f64) side_dcols_chunk<float, double>(e.sv, P, Y, (const float*)e.H_vals, (double*)e.D_vals, e.e_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
-                    else side_dcols_chunk<float, float>(e.sv, P, Y, (const float*)e.H_vals, (float*)e.D_vals, e.e_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
+                    if (e.d_f64) side_dcols_chunk<float, double>(e.sv, P, Y, (const float*)e.H_vals, (const float*)e.S_vals, (double*)e.D_vals, e.e_atom, e.q_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
+                    else side_dcols_chunk<float, float>(e.sv, P, Y, (const float*)e.H_vals, (const float*)e.S_vals, (float*)e.D_vals, e.e_atom, e.q_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
                 }
             } break;
             default: break;                       // SK_REFILL: nothing to compute

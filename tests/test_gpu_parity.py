@@ -331,3 +331,58 @@ def test_combine_rejects_partial_ranges_and_round_engine(cfg0):
         with pytest.raises(NolsmError) as ei:
             ctx.assemble(nb, rp, ci, Hv, Sv)
         assert ei.value.code == 1
+
+
+# ---- electron count and chemical-potential search ---------------------------------------
+@pytest.mark.parametrize("combine", [0, 1])
+def test_electron_count_matches_oracle(cfg0, combine):
+    s = cfg0
+    nb, rp, ci, Hv, Sv = _arrays(s)
+    Hn, Sn = s.fill_np(MAT_H), s.fill_np(MAT_S)
+    blk = s.blk_off()
+    with _nolsm(combine=combine) as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        D = torch.zeros(Hv.shape[0], dtype=torch.float64, device="cuda")
+        for mu in (0.0, -1.2):
+            ctx.density_matrix(mu, D)
+            n_gpu, q = ctx.electron_count(per_atom=True)
+            if combine:
+                sets = [orc.index_set(i, s.row_ptr, s.col_idx) for i in range(s.n_atoms)]
+                q_ref = np.zeros(s.n_atoms)
+                for g in orc.combine_groups(s.atom_nb, sets, mode=1):
+                    res = orc.group_result(g, s.atom_nb, s.row_ptr, s.col_idx, blk, Hn, Sn, mu)
+                    for i in g:
+                        q_ref[i] = res[i]["q_i"]
+            else:
+                q_ref = np.array([orc.atom_result(i, s.atom_nb, s.row_ptr, s.col_idx, blk, Hn, Sn, mu)["q_i"] for i in range(s.n_atoms)])
+            print("electron count mu", mu, "combine", combine, n_gpu, q_ref.sum(), np.abs(q - q_ref).max())
+            assert abs(n_gpu - q.sum()) <= 1e-9 * abs(n_gpu)
+            assert abs(n_gpu - q_ref.sum()) <= TOL_MIXED_E * abs(q_ref.sum())
+            assert np.abs(q - q_ref).max() <= 2e-2
+
+
+def test_find_mu_reaches_the_target_count(cfg0):
+    """Bisection through the C ABI: the returned mu gives the requested Tr(D S) within tol_n on the GPU, and the oracle's
+    count at that mu agrees within the mixed-precision tolerance; D_vals holds D(mu)."""
+    s = cfg0
+    nb, rp, ci, Hv, Sv = _arrays(s)
+    Hn, Sn = s.fill_np(MAT_H), s.fill_np(MAT_S)
+    target = 0.5 * float(s.atom_nb.sum())
+    with _nolsm() as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        D = torch.zeros(Hv.shape[0], dtype=torch.float64, device="cuda")
+        mu, n_mu, evals = ctx.find_mu(target, -7.0, 8.0, D, tol_n=0.05, tol_mu=1e-4)
+        E = ctx.energy()
+        st = ctx.atom_stats()
+        assert abs(n_mu - target) <= 0.05 and 3 < evals <= 24 and -0.9 < mu < 0.9
+        n_ref = orc.electron_count(s.atom_nb, s.row_ptr, s.col_idx, Hn, Sn, mu)
+        assert abs(n_ref - n_mu) <= TOL_MIXED_E * target
+        s_mu = make_system("cfg0")
+        s_mu.mu = mu
+        cmp = compare_atoms(s_mu, D.cpu().numpy(), st["e_atom"], range(0, s.n_atoms, 4))
+        print("find_mu", mu, n_mu, evals, n_ref, cmp["max_abs_dD"], cmp["rel_dE"])
+        assert cmp["max_abs_dD"] <= TOL_MIXED_D and cmp["rel_dE"] <= TOL_MIXED_E
+        from paper_2205_12182_b200 import NolsmError
+        with pytest.raises(NolsmError) as ei:                       # target above the number of basis functions
+            ctx.find_mu(2.0 * float(s.atom_nb.sum()), -8.0, 8.0, D)
+        assert ei.value.code == 1

@@ -374,24 +374,41 @@ void build_units(nolsm_ctx* c, int mode, int max_dim, int max_members, int max_c
     const int32_t* nb = c->atom_nb.data();
     c->unit_ptr.assign(1, 0); c->unit_mem.clear(); c->uset_ptr.assign(1, 0); c->uset_atom.clear(); c->uset_off.clear(); c->udim.clear();
     c->unit_of.assign(n_at, -1); c->upos.assign(n_at, 0);
+    const bool verbose = getenv_int("NOLSM_VERBOSE", 0) >= 2;
+    auto t_prev = std::chrono::steady_clock::now();
+    auto lap = [&](const char* what) {
+        if (!verbose) return;
+        const auto t = std::chrono::steady_clock::now();
+        fprintf(stderr, "  build_units: %-24s %8.2f ms\n", what, std::chrono::duration<double, std::milli>(t - t_prev).count());
+        t_prev = t;
+    };
     std::vector<char> is_free(n_at, 1);
-    std::vector<int32_t> G, U;
+    std::vector<int32_t> G, in_g(n_at, -1);
     std::vector<std::pair<int64_t, int32_t>> cand;
     // overlaps dim(N(i) & N(j)) of every pair of the pattern, in parallel (the greedy pass below is sequential)
     std::vector<int32_t> ov;
     if (mode != 0 && max_members > 1) {
         ov.resize(c->nset_atom.size());
         parallel_for(n_at, [&](int64_t b, int64_t e) {
+            std::vector<int32_t> mark(n_at, -1);                    // mark[k] == i: atom k is in N(i)
             for (int64_t i = b; i < e; ++i) {
                 const int32_t* Ni = c->nset_atom.data() + c->nset_ptr[i];
                 const int64_t ni = c->nset_ptr[i + 1] - c->nset_ptr[i];
+                for (int64_t q = 0; q < ni; ++q) mark[Ni[q]] = (int32_t)i;
                 for (int64_t q = 0; q < ni; ++q) {
                     const int32_t j = Ni[q];
-                    ov[c->nset_ptr[i] + q] = j == i ? 0 : (int32_t)overlap_dim(Ni, ni, c->nset_atom.data() + c->nset_ptr[j], c->nset_ptr[j + 1] - c->nset_ptr[j], nb);
+                    int32_t d = 0;
+                    if (j != i) {
+                        const int32_t* Nj = c->nset_atom.data() + c->nset_ptr[j];
+                        const int64_t nj = c->nset_ptr[j + 1] - c->nset_ptr[j];
+                        for (int64_t t = 0; t < nj; ++t) d += (mark[Nj[t]] == (int32_t)i) ? nb[Nj[t]] : 0;
+                    }
+                    ov[c->nset_ptr[i] + q] = d;
                 }
             }
         });
     }
+    lap("pair overlaps");
     for (int64_t i = 0; i < n_at; ++i) {
         if (!is_free[i]) continue;
         is_free[i] = 0;
@@ -402,6 +419,7 @@ void build_units(nolsm_ctx* c, int mode, int max_dim, int max_members, int max_c
         G.assign(Ni, Ni + ni);
         int64_t n_g = c->dim[i];
         if (mode != 0 && max_members > 1) {
+            for (int64_t q = 0; q < ni; ++q) in_g[Ni[q]] = (int32_t)i;          // in_g[k] == i: atom k is in the group's set
             cand.clear();
             for (int64_t q = 0; q < ni; ++q) {
                 const int32_t j = Ni[q];
@@ -415,17 +433,19 @@ void build_units(nolsm_ctx* c, int mode, int max_dim, int max_members, int max_c
                 const int32_t j = cj.second;
                 const int32_t* Nj = c->nset_atom.data() + c->nset_ptr[j];
                 const int64_t nj = c->nset_ptr[j + 1] - c->nset_ptr[j];
-                const int64_t n_u = n_g + c->dim[j] - overlap_dim(G.data(), (int64_t)G.size(), Nj, nj, nb);
+                int64_t n_gj = 0;
+                for (int64_t t = 0; t < nj; ++t) n_gj += (in_g[Nj[t]] == (int32_t)i) ? nb[Nj[t]] : 0;
+                const int64_t n_u = n_g + c->dim[j] - n_gj;
                 if (n_u > max_dim) continue;
                 if (combine_cost(n_u, mode) < combine_cost(n_g, mode) + combine_cost(c->dim[j], mode)) {
                     c->unit_mem.push_back(j);
                     is_free[j] = 0;
-                    U.resize(G.size() + nj);
-                    U.resize(std::set_union(G.begin(), G.end(), Nj, Nj + nj, U.begin()) - U.begin());
-                    G.swap(U);
+                    for (int64_t t = 0; t < nj; ++t)
+                        if (in_g[Nj[t]] != (int32_t)i) { in_g[Nj[t]] = (int32_t)i; G.push_back(Nj[t]); }
                     n_g = n_u;
                 }
             }
+            if (c->unit_mem.size() - m0 > 1) std::sort(G.begin(), G.end());
         }
         const int32_t u = (int32_t)c->udim.size();
         int off = 0;
@@ -436,6 +456,7 @@ void build_units(nolsm_ctx* c, int mode, int max_dim, int max_members, int max_c
         for (size_t m = m0; m < c->unit_mem.size(); ++m) c->unit_of[c->unit_mem[m]] = u;
     }
     c->n_units = (int64_t)c->udim.size();
+    lap("greedy pass");
     // offsets of every atom of N(i) inside the matrix of i's unit (N(i) is a subset of the unit's set: one merge walk)
     c->nset_uoff.resize(c->nset_atom.size());
     for (int64_t i = 0; i < n_at; ++i) {
@@ -629,7 +650,16 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     if (val_dtype != NOLSM_DTYPE_F64 && val_dtype != NOLSM_DTYPE_F32) return fail(c, NOLSM_EINVAL, "bad val_dtype");
     cudaStream_t s = (cudaStream_t)cuda_stream;
     cudaSetDevice(c->dev);
+    const bool verbose = getenv_int("NOLSM_VERBOSE", 0) >= 1;
+    auto t_prev = std::chrono::steady_clock::now();
+    auto lap = [&](const char* what) {
+        if (!verbose) return;
+        const auto t = std::chrono::steady_clock::now();
+        fprintf(stderr, "nolsm_assemble: %-28s %8.2f ms\n", what, std::chrono::duration<double, std::milli>(t - t_prev).count());
+        t_prev = t;
+    };
     free_assembled(c);
+    lap("free");
     int r;
     c->n_atoms = n_atoms;
     c->val_dtype = val_dtype;
@@ -673,6 +703,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         return fail(c, NOLSM_EINVAL, why[bad.load()]);
     }
 
+    lap("pattern to host + validate");
     // ---- block offsets ----
     c->blk_off.resize(c->nnzb + 1);
     c->blk_off[0] = 0;
@@ -695,6 +726,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     if ((r = to_device(c, H0_vals, vs * c->nvals, &c->dH, s))) return r;
     if ((r = to_device(c, S_vals, vs * c->nvals, &c->dS, s))) return r;
 
+    lap("block offsets + uploads");
     // ---- index sets N(i) (C-1 filter) ----
     std::vector<unsigned char> keep;
     c->filtered = c->opt.eps_filter > 0;
@@ -736,11 +768,13 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
             c->dim[i] = off;
         }
     });
+    lap("index sets");
     // ---- units: one submatrix per atom, or per group of atoms (Eq. 9 / Eq. 10; C-19) ----
     c->combined = c->opt.combine != 0 && want_persist(c);
     if (c->opt.combine != 0 && !c->combined) return fail(c, NOLSM_EINVAL, "combine needs the persistent engine (FP16/tcgen05 mode)");
     build_units(c, c->combined ? c->opt.combine : 0, std::min(c->opt.combine_max_dim, P_MAX_CAP), c->opt.combine_max_members,
                 c->opt.combine_max_candidates);
+    lap("units (grouping)");
     int max_n = 0, min_n = 1 << 30, max_nset = 0, max_nbi = 0;
     double mean_tiles = 0, mean_n2 = 0;
     for (int64_t i = 0; i < n_atoms; ++i) max_nbi = std::max(max_nbi, c->atom_nb[i]);
@@ -796,6 +830,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         c->d_nset_uoff = c->d_nset_off; c->d_udim = c->d_dim; c->d_upos = c->d_pos;
     }
 
+    lap("uploads of index data");
     // ---- engine: slots, workspace, tensor maps ----
     Engine& e = c->eng;
     e = Engine{};
@@ -982,6 +1017,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         CU_TRY(c, cudaFuncSetAttribute(k_side_gather<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SIDE_SMEM));
     }
     CU_TRY(c, cudaStreamSynchronize(s));
+    lap("workspace, maps, engine");
     c->assembled = true;
     return NOLSM_OK;
 }

@@ -386,3 +386,38 @@ def test_find_mu_reaches_the_target_count(cfg0):
         with pytest.raises(NolsmError) as ei:                       # target above the number of basis functions
             ctx.find_mu(2.0 * float(s.atom_nb.sum()), -8.0, 8.0, D)
         assert ei.value.code == 1
+
+
+@pytest.mark.parametrize("kw", [dict(combine=1, cluster_ctas=4), dict(combine=2, eps_filter=0.02), dict(combine=1, sign_scaled_iters=-1)])
+def test_combination_with_other_options(kw):
+    """Combination together with the cluster-of-4 pipeline, with the max-abs block filter (filtered index sets feed the
+    grouping) and with plain Eq. 6: groups bit-exact, host float32 output, parity on sampled groups."""
+    s = make_system("cfg1", n_atoms=500)
+    Hn, Sn = s.fill_np(MAT_H), s.fill_np(MAT_S)
+    blk = s.blk_off()
+    eps = kw.get("eps_filter", 0.0)
+    sets = [orc.index_set(i, s.row_ptr, s.col_idx, s.atom_nb, blk, Hn, Sn, eps) for i in range(s.n_atoms)]
+    groups = orc.combine_groups(s.atom_nb, sets, mode=kw["combine"])
+    from tests.helpers import d_row_from_oracle
+    with _nolsm(**kw) as ctx:
+        ctx.assemble(s.atom_nb, s.row_ptr, s.col_idx, Hn, Sn)                   # host inputs
+        for g in groups[::7]:
+            mem, st_, dim = ctx.group(g[0])
+            assert mem.tolist() == g and np.array_equal(st_, np.unique(np.concatenate([sets[i] for i in g])).astype(np.int32))
+        D = np.zeros(len(Hn), dtype=np.float32)                                  # host float32 output
+        ctx.density_matrix(s.mu, D)
+        E = ctx.energy()
+        st = ctx.atom_stats()
+        assert ctx.stats()["n_units"] == len(groups)
+    max_d, e_ref, e_gpu = 0.0, 0.0, 0.0
+    for g in groups[3::29]:
+        res = orc.group_result(g, s.atom_nb, s.row_ptr, s.col_idx, blk, Hn, Sn, s.mu, eps_filter=eps)
+        for i in g:
+            row = d_row_from_oracle(s, i, res[i], blk)
+            p0, p1 = int(s.row_ptr[i]), int(s.row_ptr[i + 1])
+            max_d = max(max_d, float(np.abs(D[blk[p0]:blk[p1]] - row).max()))
+            e_ref += res[i]["e_i"]
+            e_gpu += float(st["e_atom"][i])
+    print("options", kw, "groups", len(groups), "max|dD|", max_d, "rel dE", abs(e_gpu - e_ref) / abs(e_ref))
+    assert max_d <= TOL_MIXED_D and abs(e_gpu - e_ref) / abs(e_ref) <= TOL_MIXED_E
+    assert abs(E - st["e_atom"].sum()) <= 1e-9 * abs(E)

@@ -414,7 +414,7 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                         f[j] = sa * a;
                     }
 #pragma unroll
-                    for (int j = 0; j < 32; j += 8) st_half8(crow + j, f + j);
+                    for (int j = 0; j < 32; j += 16) st_half16(crow + j, f + j);
                 }
             } else if (row < n16) {
                 float f[32];
@@ -429,8 +429,8 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                 }
                 const int cw = min(min(32, bn - c), n16 - (col0 + c));   // 16 or 32 valid columns
 #pragma unroll
-                for (int j = 0; j < 32; j += 8)
-                    if (j < cw) st_half8(crow + j, f + j);
+                for (int j = 0; j < 32; j += 16)
+                    if (j < cw) st_half16(crow + j, f + j);
             }
         }
         ptx::tc_fence_before();

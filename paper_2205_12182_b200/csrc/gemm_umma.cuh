@@ -140,4 +140,17 @@ __device__ __forceinline__ void st_half8(__half* p, const float* v) {
     *reinterpret_cast<uint4*>(p) = u;
 }
 
+// 16 halves = 32 bytes = one L2 sector with ONE store (st.global.v8.b32, sm_100): a row-per-thread epilogue issues half
+// as many write requests as with 16-byte stores and never writes half a sector. `p` must be 32-byte aligned.
+__device__ __forceinline__ void st_half16(__half* p, const float* v) {
+    uint32_t u[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        __half2 h = __floats2half2_rn(v[2 * i], v[2 * i + 1]);
+        u[i] = *reinterpret_cast<uint32_t*>(&h);
+    }
+    asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+                 ::"l"(p), "r"(u[0]), "r"(u[1]), "r"(u[2]), "r"(u[3]), "r"(u[4]), "r"(u[5]), "r"(u[6]), "r"(u[7]) : "memory");
+}
+
 }  // namespace nolsm

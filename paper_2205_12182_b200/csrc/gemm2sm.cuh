@@ -23,10 +23,14 @@
 
 namespace nolsm {
 
+// The TMA ring: 4 stages of 32 KB (measured: 3, 4 and 5 stages run at the same speed - the ring is not what bounds the
+// k-loop); the fifth 32 KB hold the epilogue's staging boxes for TMA stores of C.
 #ifndef G2_STAGES_N
-#define G2_STAGES_N 5
+#define G2_STAGES_N 4
 #endif
 constexpr int G2_STAGES = G2_STAGES_N;
+constexpr int G2_CBOX_BYTES = 64 * 64 * 2;            // one 64 x 64 FP16 box of C, 128-byte swizzle (the TMA map's box)
+constexpr int G2_CSTAGE_BYTES = 4 * G2_CBOX_BYTES;    // two row groups (64 rows each) x two buffers
 constexpr int G2_A_BYTES = 128 * BK * 2;              // 16 KB: this CTA's 128 rows x 64 k
 constexpr int G2_B_BYTES = 2 * B_BOX_BYTES;           // 16 KB: 64 k x (up to 128) columns
 constexpr int G2_STAGE_BYTES = G2_A_BYTES + G2_B_BYTES;
@@ -53,7 +57,8 @@ struct G2Smem {                       // byte offsets from the 1024-aligned base
     uint32_t base;
     __device__ uint32_t stage_a(int s) const { return base + s * G2_STAGE_BYTES; }
     __device__ uint32_t stage_b(int s) const { return base + s * G2_STAGE_BYTES + G2_A_BYTES; }
-    __device__ uint32_t bars() const { return base + G2_STAGES * G2_STAGE_BYTES; }
+    __device__ uint32_t stage_c(int group, int buf) const { return base + G2_STAGES * G2_STAGE_BYTES + (group * 2 + buf) * G2_CBOX_BYTES; }
+    __device__ uint32_t bars() const { return base + G2_STAGES * G2_STAGE_BYTES + G2_CSTAGE_BYTES; }
     __device__ uint32_t full(int s) const { return bars() + 8u * s; }
     __device__ uint32_t empty(int s) const { return bars() + 8u * (G2_STAGES + s); }
     __device__ uint32_t tfull(int a) const { return bars() + 8u * (2 * G2_STAGES + a); }
@@ -65,7 +70,7 @@ struct G2Smem {                       // byte offsets from the 1024-aligned base
     __device__ uint32_t want() const { return bars() + 8u * (2 * G2_STAGES + 4 + 2 * G2_NTI) + 8u; }
     __device__ uint32_t tinfo(int q) const { return bars() + 256u + 64u * q; }
 };
-constexpr int G2_SMEM_BYTES = G2_STAGES * G2_STAGE_BYTES + 256 + 64 * G2_NTI + 1024 /*align*/;
+constexpr int G2_SMEM_BYTES = G2_STAGES * G2_STAGE_BYTES + G2_CSTAGE_BYTES + 256 + 64 * G2_NTI + 1024 /*align*/;
 
 #ifdef G2_TIMING
 // probe builds only: cycles spent waiting, summed over CTAs
@@ -160,6 +165,28 @@ __device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
         ::"r"(bar), "h"((uint16_t)3) : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+// TMA store of one box from shared memory (bulk async-group completion)
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, int c0, int c1, uint32_t src) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group [%0, {%1, %2}], [%3];"
+                 ::"l"(map), "r"(c0), "r"(c1), "r"(src) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// 32 halves of one row into a staging box: chunks (16 B) j0 .. j0 + 3 of box row r, 128-byte swizzle (chunk ^ (r & 7))
+__device__ __forceinline__ void st_box_row(uint32_t box, int r, int j0, const float* v) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        __half2 h0 = __floats2half2_rn(v[8 * q], v[8 * q + 1]), h1 = __floats2half2_rn(v[8 * q + 2], v[8 * q + 3]);
+        __half2 h2 = __floats2half2_rn(v[8 * q + 4], v[8 * q + 5]), h3 = __floats2half2_rn(v[8 * q + 6], v[8 * q + 7]);
+        const uint32_t a = box + (uint32_t)r * 128u + (uint32_t)(((j0 + q) ^ (r & 7)) << 4);
+        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(*reinterpret_cast<uint32_t*>(&h0)),
+                     "r"(*reinterpret_cast<uint32_t*>(&h1)), "r"(*reinterpret_cast<uint32_t*>(&h2)), "r"(*reinterpret_cast<uint32_t*>(&h3)) : "memory");
+    }
+}
 
 }  // namespace ptx
 
@@ -361,7 +388,7 @@ __device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int
 // ------------------------------------------------------------------------------------------------
 template <typename Eng, typename Done>
 __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base, const Eng& e, __half* base,
-                                            uint32_t rank, int warp, int lane, Done done) {
+                                            uint32_t rank, int warp, int lane, Done done, const CUtensorMap* maps = nullptr) {
     int acc = 0; uint32_t acc_phase = 0;
     int q = 0; uint32_t tph = 0;
     const uint32_t tempty0 = ptx::mapa(sm.tempty(0), 0);
@@ -385,6 +412,65 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
         ptx::tc_fence_after();
         float rsum = 0.f, vsum = 0.f;
         uint32_t dep = 0;
+        const bool via_tma = maps != nullptr && ident;             // square GEMM tiles leave through shared memory and TMA stores
+        if (via_tma) {
+            // C leaves in 64 x 64 boxes: the four warps that hold rows [64 g, 64 g + 64) of the CTA's 128 rows and the two
+            // 32-column halves of a box write it into a swizzled staging buffer; one thread hands it to the TMA unit, which
+            // writes whole 128-byte lines (the row-per-thread register stores issue one request per 32 bytes and go
+            // through the SM's load/store path, which the k-loop's ingest also needs). Two buffers per row group.
+            const int g = quarter >> 1, rbox = ((quarter & 1) << 5) + lane;
+            const bool issuer = (quarter & 1) == 0 && chalf == 0 && lane == 0;
+            const CUtensorMap* map_c = maps + (size_t)ti.slot * NMAP + ti.c_buf;
+            const int nbx = (bn + 63) >> 6;
+            for (int kx = 0; kx < nbx; ++kx) {
+                const int c = (kx << 6) + (chalf << 5);
+                const uint32_t box = sm.stage_c(g, kx & 1);
+                if (issuer) ptx::bulk_wait_read<1>();              // the store that read this buffer two boxes ago is done with it
+                asm volatile("bar.sync %0, 128;" ::"r"(3 + g) : "memory");
+                float f[32];
+                if (c < bn && col0 + c < n16) {
+                    uint32_t v[32];
+                    ptx::tmem_ld_32x32(tmem_base + acc * 256 + ((uint32_t)(quarter * 32) << 16) + c, v);
+                    ptx::tmem_ld_wait();
+                    dep ^= v[0];
+                    const bool full = (c + 32 <= bn) && (col0 + c + 32 <= n16);
+                    const bool diag = (col0 + c < rbase + 32) && (col0 + c + 32 > rbase);
+                    if (full && !diag) {
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) {
+                            const float a = __uint_as_float(v[j]);
+                            if (row < n16) vsum = fmaf(a, a, vsum);
+                            f[j] = sa * a;
+                        }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) {
+                            const int col = col0 + c + j;
+                            const float a = __uint_as_float(v[j]);
+                            const float delta = (col == row && row < n) ? 1.f : 0.f;
+                            const bool in = (c + j < bn && col < n16 && row < n16);
+                            const float d = in ? ti.alpha_res * a - delta : 0.f;      // pad rows / columns give exactly 0
+                            rsum = fmaf(d, d, rsum);
+                            f[j] = in ? ti.c_out * a + ti.beta * delta : 0.f;
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) f[j] = 0.f;
+                }
+                ptx::st_box_row(box, rbox, chalf << 2, f);
+                ptx::fence_proxy_async_smem();
+                asm volatile("bar.sync %0, 128;" ::"r"(3 + g) : "memory");
+                if (issuer) {
+                    ptx::tma_store_2d(map_c, col0 + (kx << 6), ti.m0 + 128 * (int)rank + 64 * g, box);
+                    ptx::bulk_commit();
+                }
+            }
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive_cluster_relaxed(tempty0 + 8u * acc, dep);     // the accumulator is free
+            if (issuer) ptx::bulk_wait<0>();                       // the boxes of this tile are in global memory
+        } else
         for (int c = chalf * 32; c < bn; c += 64) {
             if (col0 + c >= n16) break;                            // warp-uniform
             uint32_t v[32];
@@ -433,10 +519,12 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                     if (j < cw) st_half16(crow + j, f + j);
             }
         }
-        ptx::tc_fence_before();
-        ptx::fence_proxy_async();      // C is read next through the async proxy (TMA), possibly by another CTA
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive_cluster_relaxed(tempty0 + 8u * acc, dep);
+        if (!via_tma) {
+            ptx::tc_fence_before();
+            ptx::fence_proxy_async();      // C is read next through the async proxy (TMA), possibly by another CTA
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive_cluster_relaxed(tempty0 + 8u * acc, dep);
+        }
         if (ti.want_res) {
             rsum = fmaf(ti.alpha_res * ti.alpha_res, vsum, rsum);
 #pragma unroll

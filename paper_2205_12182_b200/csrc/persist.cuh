@@ -71,6 +71,7 @@ struct PEngine {
     int* heavy;                   // [1] slots inside the GEMM-heavy phases INV .. SIGN right now (at most g_max)
     int* parked;                  // [S] 1 = the slot finished its first Schulz step and waits for a heavy token
     int g_max, want_lead, dbg;
+    int tma_store;                // 1: square GEMM tiles leave through shared-memory boxes and TMA stores
     int tile_n;                   // columns of a pair tile (256; 128 halves a GEMM's latency at more L2 traffic per FLOP)
     const signed char* die_of_sm; // [256] L2 die of every SM (0 / 1), or all -1: no die affinity (see k_die_probe)
     int ndie;                     // 2: slot s is served only by SMs of die s & 1 and heavy tokens are per die; 1: no affinity
@@ -882,7 +883,7 @@ nolsm_persist_kernel(const __grid_constant__ PEngine e) {
 
     if (warp < G2_EPI_WARPS) {
         if constexpr (CTAS == G4_CTAS) g4_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, done);
-        else g2_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, done);
+        else g2_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, done, e.tma_store ? e.maps : nullptr);
     } else if (warp == G2_WARP_SCHED) {
         if (rank == 0) p_scheduler<CTAS>(sm, e, lane);
     } else if (warp == G2_WARP_TMA) {

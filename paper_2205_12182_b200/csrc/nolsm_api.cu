@@ -63,7 +63,9 @@ struct nolsm_ctx {
     int max_n = 0, max_nset = 0, max_nbi = 0;
 
     // device arrays
-    std::vector<void*> owned;           // everything cudaMalloc'ed by assemble (freed on re-assemble / destroy)
+    std::vector<std::pair<void*, size_t>> owned;   // everything cudaMalloc'ed by assemble
+    std::vector<std::pair<void*, size_t>> pool;    // blocks of the previous assemble, reused by the next one (cudaFree of GB-sized
+                                                   // blocks stalled re-assembly for up to 0.7 s; freed by nolsm_destroy)
     long long *d_row_ptr = nullptr, *d_blk_off = nullptr, *d_nset_ptr = nullptr;
     int *d_col_idx = nullptr, *d_atom_nb = nullptr, *d_nset_atom = nullptr, *d_nset_slot = nullptr, *d_nset_off = nullptr;
     const void *dH = nullptr, *dS = nullptr;
@@ -171,16 +173,39 @@ bool is_device_ptr(const void* p) {
 }
 
 int dmalloc(nolsm_ctx* c, void** p, size_t bytes) {
-    CU_TRY(c, cudaMalloc(p, std::max<size_t>(bytes, 16)));
-    c->owned.push_back(*p);
+    bytes = std::max<size_t>(bytes, 16);
+    // best fit from the pool: the smallest block that holds `bytes` and is not more than twice as large
+    int best = -1;
+    for (int i = 0; i < (int)c->pool.size(); ++i)
+        if (c->pool[i].second >= bytes && c->pool[i].second <= 2 * bytes + 4096 && (best < 0 || c->pool[i].second < c->pool[best].second)) best = i;
+    if (best >= 0) {
+        *p = c->pool[best].first;
+        c->owned.push_back(c->pool[best]);
+        c->pool.erase(c->pool.begin() + best);
+        return NOLSM_OK;
+    }
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e == cudaErrorMemoryAllocation && !c->pool.empty()) {      // give the pooled blocks back and try once more
+        cudaGetLastError();
+        for (auto& b : c->pool) cudaFree(b.first);
+        c->pool.clear();
+        e = cudaMalloc(p, bytes);
+    }
+    CU_TRY(c, e);
+    c->owned.push_back({*p, bytes});
     return NOLSM_OK;
 }
 
-void free_assembled(nolsm_ctx* c) {
-    for (void* p : c->owned) cudaFree(p);
+// Ends the assembled state. The device blocks go to the pool (release = true: back to the driver).
+void free_assembled(nolsm_ctx* c, bool release = false) {
+    for (auto& b : c->owned) c->pool.push_back(b);
     c->owned.clear();
-    if (c->h_done) { cudaFreeHost(c->h_done); c->h_done = nullptr; }
-    if (c->d_D_stage) { cudaFree(c->d_D_stage); c->d_D_stage = nullptr; c->d_D_stage_bytes = 0; }
+    if (release) {
+        for (auto& b : c->pool) cudaFree(b.first);
+        c->pool.clear();
+        if (c->h_done) { cudaFreeHost(c->h_done); c->h_done = nullptr; }
+    }
+    if (c->d_D_stage && release) { cudaFree(c->d_D_stage); c->d_D_stage = nullptr; c->d_D_stage_bytes = 0; }
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
     c->ws = nullptr; c->assembled = false; c->have_result = false;
 }
@@ -627,7 +652,7 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
 int nolsm_destroy(nolsm_ctx* c) {
     if (!c) return NOLSM_EINVAL;
     cudaSetDevice(c->dev);
-    free_assembled(c);
+    free_assembled(c, true);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     cudaEvent_t evs[] = {c->ev_fork, c->ev_x, c->ev_f, c->ev_in, c->ev_out, c->ev_k0, c->ev_k1};
     for (cudaEvent_t e : evs) if (e) cudaEventDestroy(e);
@@ -658,6 +683,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         fprintf(stderr, "nolsm_assemble: %-28s %8.2f ms\n", what, std::chrono::duration<double, std::milli>(t - t_prev).count());
         t_prev = t;
     };
+    if (c->have_result) wait_result(c);          // the pooled blocks of the last call are about to be reused
     free_assembled(c);
     lap("free");
     int r;
@@ -885,7 +911,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     CU_TRY(c, cudaMemsetAsync(e.slots, 0, sizeof(Slot) * S, s));
     CU_TRY(c, cudaMemsetAsync(e.ops, 0, sizeof(SlotOp) * 2 * S, s));
     CU_TRY(c, cudaMemsetAsync(e.ntiles, 0, 16, s));
-    CU_TRY(c, cudaHostAlloc((void**)&c->h_done, 64, cudaHostAllocMapped));
+    if (!c->h_done) CU_TRY(c, cudaHostAlloc((void**)&c->h_done, 64, cudaHostAllocMapped));
     *c->h_done = 0;
     int* h_done_dev = nullptr;
     CU_TRY(c, cudaHostGetDevicePointer((void**)&h_done_dev, c->h_done, 0));

@@ -130,8 +130,18 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
 __device__ __forceinline__ void mbar_wait_cluster_patient(uint32_t bar, uint32_t parity) {
     uint32_t spins = 0;
     while (!mbar_try_wait_cluster(bar, parity)) {
-        if (++spins > 2048u) __nanosleep(128);
+        if (++spins > 16u) __nanosleep(200);
         if (spins > (1u << 28)) __trap();
+    }
+}
+// Wait of the eight epilogue warps for the accumulator of the tile being multiplied: microseconds long and not on the
+// critical path (two accumulators), so the warps sleep between polls instead of issuing a try_wait loop (which was 28 %
+// of all instructions the kernel issued: profiles/r01_persist_v6.md) - the issue slots and the power go to the k-loop.
+__device__ __forceinline__ void mbar_wait_sleepy(uint32_t bar, uint32_t parity) {
+    uint32_t spins = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        __nanosleep(spins < 4u ? 64 : 256);
+        if (++spins > (1u << 26)) __trap();
     }
 }
 __device__ __forceinline__ void st_cluster_u32(uint32_t cluster_addr, uint32_t v) {
@@ -407,7 +417,7 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
         const int row = rbase + lane;
         const int col0 = ti.n0;
         const float sa = ti.c_out;
-        { G2_T0(); ptx::mbar_wait(sm.tfull(acc), acc_phase); G2_T1(5); }
+        { G2_T0(); ptx::mbar_wait_sleepy(sm.tfull(acc), acc_phase); G2_T1(5); }
         G2_T0();
         ptx::tc_fence_after();
         float rsum = 0.f, vsum = 0.f;

@@ -259,7 +259,7 @@ __device__ __forceinline__ void g4_epilogue(const G2Smem& sm, uint32_t tmem_base
             const int row = rbase + lane;
             const int col0 = pt.n0;
             const float sa = ti.c_out;
-            ptx::mbar_wait_cluster(sm.tfull(acc), acc_phase);
+            ptx::mbar_wait_sleepy(sm.tfull(acc), acc_phase);
             G4_T1(5);
             ptx::tc_fence_after();
             float rsum = 0.f, vsum = 0.f;

@@ -45,7 +45,8 @@ constexpr int G2_CTRL_THREADS = 11 * 32;              // warps 0..10
 constexpr int G2_TI_CONSUMERS = 2 * (1 + G2_EPI_WARPS) + 1;
 
 struct __align__(16) TileInfo {      // 64 bytes
-    int valid;                        // 0 = no more tiles
+    int valid;                        // 0 = no more tiles; bit 1 set: half-height tile (rows m0 .. m0+127, one M = 128 MMA per 16 k:
+                                      // 64 rows per CTA; TMEM lanes 0-63 hold columns [0, bn/2), lanes 64-127 columns [bn/2, bn))
     int slot, m0, n0;                 // pair tile origin (rows m0 .. m0+255, columns n0 .. n0+bn-1)
     int n, n16, bn, nreports;         // nreports = CTA reports that complete the slot's GEMM
     int a_buf, b_buf, c_buf, want_res;
@@ -292,8 +293,9 @@ __device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap*
         const int nkb = (ti.n16 + BK - 1) / BK;
         const int half = ti.bn >> 1;
         const int nbox = (half + 63) >> 6;
-        const uint32_t bytes = 2u * (G2_A_BYTES + nbox * B_BOX_BYTES);     // both CTAs of the pair
-        const int row0 = ti.m0 + 128 * (int)rank;
+        const bool hh = (ti.valid & 2) != 0;                               // half-height tile: 64 rows of A per CTA
+        const uint32_t bytes = 2u * ((hh ? G2_A_BYTES / 2 : G2_A_BYTES) + nbox * B_BOX_BYTES);     // both CTAs of the pair
+        const int row0 = ti.m0 + (hh ? 64 : 128) * (int)rank;
         const int col0 = ti.n0 + half * (int)rank;
         const uint32_t full0 = ptx::mapa(sm.full(0), 0);                    // the leader's full barriers
         const int kb_want = max(0, nkb - want_lead);
@@ -305,7 +307,7 @@ __device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap*
                 if (rank == 0) ptx::mbar_expect_tx(sm.full(stage), bytes);
                 const uint32_t sa = sm.stage_a(stage), sb = sm.stage_b(stage);
                 ptx::tma_load_2d_pair(sa, map_a, kb * BK, row0, fb);
-                ptx::tma_load_2d_pair(sa + 8192, map_a, kb * BK, row0 + 64, fb);
+                if (!hh) ptx::tma_load_2d_pair(sa + 8192, map_a, kb * BK, row0 + 64, fb);
                 for (int b = 0; b < nbox; ++b)
                     ptx::tma_load_2d_pair(sb + b * B_BOX_BYTES, map_b, col0 + b * 64, kb * BK, fb);
             }
@@ -355,7 +357,7 @@ __device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int
         if (!ti.valid) break;
         const int nkb = (ti.n16 + BK - 1) / BK;
         const int ktail = (ti.n16 - (nkb - 1) * BK) >> 4;          // 16-k slices of the last k-block (1..4)
-        const uint32_t idesc = make_idesc_f16(256, ti.bn);
+        const uint32_t idesc = make_idesc_f16((ti.valid & 2) ? 128 : 256, ti.bn);
 #ifdef G2_TIMING
         const long long tk0_ = clock64();
 #endif
@@ -409,20 +411,24 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
         { G2_T0(); ti = g2_take(sm, q, tph, lane == 0); G2_T1(4); }
         if (++q == G2_NTI) { q = 0; tph ^= 1; }
         if (!ti.valid) break;
-        const int n = ti.n, n16 = ti.n16, bn = ti.bn;
+        const int n = ti.n, n16 = ti.n16;
         int ldc;
         __half* C = c_ptr(e, base, ti.slot, ti.c_buf, ldc);
         const bool ident = ti.kind != OP_POW_S && ti.kind != OP_POW_A && ti.kind != OP_DCOLS;   // power-iteration tiles: C = alpha A V, res = ||C||_F^2
-        const int rbase = ti.m0 + 128 * (int)rank + quarter * 32;      // first row of this warp
+        // full-height tile: the CTA's 128 TMEM lanes are 128 rows, every warp sees all bn columns; half-height tile
+        // (M = 128 over the pair): lanes 0-63 and 64-127 are the same 64 rows with the left / right half of the columns
+        const bool hh = (ti.valid & 2) != 0;
+        const int rbase = hh ? ti.m0 + 64 * (int)rank + (quarter & 1) * 32 : ti.m0 + 128 * (int)rank + quarter * 32;   // first row of this warp
         const int row = rbase + lane;
-        const int col0 = ti.n0;
+        const int col0 = hh ? ti.n0 + (quarter >> 1) * (ti.bn >> 1) : ti.n0;
+        const int bn = hh ? ti.bn >> 1 : ti.bn;                        // columns this warp's lanes hold
         const float sa = ti.c_out;
         { G2_T0(); ptx::mbar_wait_sleepy(sm.tfull(acc), acc_phase); G2_T1(5); }
         G2_T0();
         ptx::tc_fence_after();
         float rsum = 0.f, vsum = 0.f;
         uint32_t dep = 0;
-        const bool via_tma = maps != nullptr && ident;             // square GEMM tiles leave through shared memory and TMA stores
+        const bool via_tma = maps != nullptr && ident && !hh;      // full-height square GEMM tiles leave through shared memory and TMA stores
         if (via_tma) {
             // C leaves in 64 x 64 boxes: the four warps that hold rows [64 g, 64 g + 64) of the CTA's 128 rows and the two
             // 32-column halves of a box write it into a swizzled staging buffer; one thread hands it to the TMA unit, which

@@ -1015,6 +1015,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         pe.g_max = pe.ndie == 2 ? std::max(1, std::min(g_max, S) / 2) : std::max(1, std::min(g_max, S));
         pe.want_lead = std::max(1, getenv_int("NOLSM_WANT_LEAD", G2_WANT_LEAD));
         pe.dbg = getenv_int("NOLSM_DBG", 0);
+        pe.half_tiles = c->opt.cluster_ctas == G4_CTAS ? 0 : getenv_int("NOLSM_HALF_TILES", 1);
         pe.tma_store = getenv_int("NOLSM_TMA_STORE", 1);
         pe.tile_n = getenv_int("NOLSM_TILE_N", BN) == 128 ? 128 : BN;
         pe.schulz_chunks = std::max(1, getenv_int("NOLSM_SCHULZ_CHUNKS", 16));
@@ -1443,7 +1444,14 @@ int nolsm_get_stats(nolsm_ctx* c, nolsm_stats* out) {
             int ntm, ntn;
             const int n16 = (dm[i] + 15) & ~15;
             choose_tiling(n16, ntm, ntn);
-            out->flops_padded += 2.0 * (double)(ntm * BM) * (double)n16 * (double)n16 * gm[i];
+            // rows the tensor cores executed: 256 per row block; the persistent pair engine runs a last row block of at most
+            // 128 rows as M = 128 tiles (except on a ragged last column tile whose width is not a multiple of 32)
+            double rows = (double)(ntm * BM);
+            if (c->last_persist && c->peng.half_tiles && n16 - (ntm - 1) * BM <= BM / 2) {
+                const int last_bn = n16 - (ntn - 1) * BN;
+                rows -= (BM / 2) * ((last_bn & 31) == 0 ? 1.0 : (double)(n16 - last_bn) / (double)n16);
+            }
+            out->flops_padded += 2.0 * rows * (double)n16 * (double)n16 * gm[i];
             out->n_notspd += (st[i] & ST_NOTSPD) ? 1 : 0;
             out->n_noconv += (st[i] & ST_NOCONV) ? 1 : 0;
         }

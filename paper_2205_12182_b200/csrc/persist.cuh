@@ -72,6 +72,7 @@ struct PEngine {
     int* parked;                  // [S] 1 = the slot finished its first Schulz step and waits for a heavy token
     int g_max, want_lead, dbg;
     int tma_store;                // 1: square GEMM tiles leave through shared-memory boxes and TMA stores
+    int half_tiles;               // 1: half-height (M = 128) tiles for a last row block of at most 128 rows
     int tile_n;                   // columns of a pair tile (256; 128 halves a GEMM's latency at more L2 traffic per FLOP)
     const signed char* die_of_sm; // [256] L2 die of every SM (0 / 1), or all -1: no die affinity (see k_die_probe)
     int ndie;                     // 2: slot s is served only by SMs of die s & 1 and heavy tokens are per die; 1: no affinity
@@ -414,7 +415,7 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
             if (++spins > (1u << 28)) __trap();
         }
         TileInfo ti{};
-        int got = 0;
+        int got = 0, half_height = 0;
         unsigned long long t_idle0 = 0;
         for (;;) {
             int found = -1;
@@ -448,7 +449,11 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
                             int n0, bn0, bn1;
                             g4_cols(g0.z, tn, n0, bn0, bn1);
                             ti.n0 = n0; ti.bn = bn0 | (bn1 << 16);
-                        } else { ti.n0 = tn * e.tile_n; ti.bn = min(e.tile_n, g0.z - tn * e.tile_n); }
+                        } else {
+                            ti.n0 = tn * e.tile_n; ti.bn = min(e.tile_n, g0.z - tn * e.tile_n);
+                            // the last row block when at most 128 rows are left: one M = 128 MMA per 16 k instead of M = 256
+                            if (e.half_tiles && g0.z - tm * BM <= BM / 2 && (ti.bn & 31) == 0) half_height = 1;
+                        }
                         ti.n = g0.y; ti.n16 = g0.z; ti.nreports = CTAS * nt;
                         ti.kind = o0.x; ti.a_buf = o0.y; ti.b_buf = o0.z; ti.c_buf = o0.w;
                         ti.c_out = o1.x; ti.alpha_res = o1.y; ti.beta = o1.z; ti.want_res = __float_as_int(o1.w);
@@ -465,7 +470,7 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
         }
         if (t_idle0) idle_ns += pl::gtime() - t_idle0;
         ntiles += got;
-        if (lane == 0) ti.valid = got;
+        if (lane == 0) ti.valid = got ? (1 | (half_height << 1)) : 0;
         const uint32_t* w = reinterpret_cast<const uint32_t*>(&ti);
         uint32_t mine = 0;
 #pragma unroll

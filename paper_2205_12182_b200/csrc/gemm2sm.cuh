@@ -478,7 +478,8 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                 ptx::fence_proxy_async_smem();
                 asm volatile("bar.sync %0, 128;" ::"r"(3 + g) : "memory");
                 if (issuer) {
-                    ptx::tma_store_2d(map_c, col0 + (kx << 6), ti.m0 + 128 * (int)rank + 64 * g, box);
+                    const int brow = ti.m0 + 128 * (int)rank + 64 * g;
+                    if (brow < n16) ptx::tma_store_2d(map_c, col0 + (kx << 6), brow, box);    // boxes below the matrix are padding
                     ptx::bulk_commit();
                 }
             }

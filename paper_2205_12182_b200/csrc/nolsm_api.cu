@@ -1015,6 +1015,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         pe.g_max = pe.ndie == 2 ? std::max(1, std::min(g_max, S) / 2) : std::max(1, std::min(g_max, S));
         pe.want_lead = std::max(1, getenv_int("NOLSM_WANT_LEAD", G2_WANT_LEAD));
         pe.dbg = getenv_int("NOLSM_DBG", 0);
+        pe.split_tokens = getenv_int("NOLSM_SPLIT_TOKENS", 1);
         pe.half_tiles = c->opt.cluster_ctas == G4_CTAS ? 0 : getenv_int("NOLSM_HALF_TILES", 1);
         pe.tma_store = getenv_int("NOLSM_TMA_STORE", 1);
         pe.tile_n = getenv_int("NOLSM_TILE_N", BN) == 128 ? 128 : BN;

@@ -52,7 +52,7 @@ struct __align__(16) PSlot {      // 160 bytes
     float c_out, alpha_res, beta; int want_res;
     int inv_iters, sign_iters, conv, xcur, ycur, status, gemm_count, tiles_done;
     float res_acc, res_prev, res_last, rho_s, rho_a, alpha1, alpha2; int side_done;
-    int pow_step; float pow_norm2, pow_alpha, pow_est;              // block power iteration state
+    int pow_step; float pow_norm2, pow_alpha; int resume;           // block power iteration state; resume: which token phase comes next
     int noboost, unit, mptr, mend;                                  // noboost: the scaled steps are over for this matrix; unit and its members
                                                                     // [mptr, mend) still to be served (atom / pos / nbi describe member mptr)
 };
@@ -72,6 +72,7 @@ struct PEngine {
     int* parked;                  // [S] 1 = the slot finished its first Schulz step and waits for a heavy token
     int g_max, want_lead, dbg;
     int tma_store;                // 1: square GEMM tiles leave through shared-memory boxes and TMA stores
+    int split_tokens;             // 1: the heavy token is returned for the rho(A) power iteration and taken again for the sign phase
     int half_tiles;               // 1: half-height (M = 128) tiles for a last row block of at most 128 rows
     int tile_n;                   // columns of a pair tile (256; 128 halves a GEMM's latency at more L2 traffic per FLOP)
     const signed char* die_of_sm; // [256] L2 die of every SM (0 / 1), or all -1: no die affinity (see k_die_probe)
@@ -222,11 +223,17 @@ __device__ __forceinline__ void p_start_power(const PEngine& e, int slot, int ki
 // as many slots as fit in L2 together may be inside the heavy phases (Schulz iterations .. sign iterations)
 // at once. A slot that is ready to enter takes a token or parks; a slot that leaves hands its token to a
 // parked slot (and installs that slot's first GEMM) or returns it.
+// A slot takes a token twice: for the Schulz iterations .. A = S^-1 H0 (resume == 0) and, after the power iteration for
+// rho(A) - nine dependent 16-column tile passes that would hold the token idle - for the sign iterations (resume == 1).
 __device__ __forceinline__ void p_enter_heavy_now(const PEngine& e, int slot) {
     PSlot* s = &e.slots[slot];
-    __stcg(&s->inv_iters, 1);
-    __stcg(&s->ycur, 2);
-    p_install_gemm(e, slot, OP_INV_G1);
+    if (__ldcg(&s->resume) == 0) {
+        __stcg(&s->inv_iters, 1);
+        __stcg(&s->ycur, 2);
+        p_install_gemm(e, slot, OP_INV_G1);
+    } else {
+        p_install_gemm(e, slot, OP_SIGN_G1);
+    }
 }
 // With die affinity (ndie == 2) slot s belongs to die s & 1: tokens are counted per die (g_max each).
 __device__ __forceinline__ void p_enter_heavy(const PEngine& e, int slot) {
@@ -277,6 +284,7 @@ __device__ __forceinline__ bool p_refill(const PEngine& e, int slot) {
     __stcg(reinterpret_cast<float4*>(&s->res_acc), make_float4(0.f, 1e30f, 0.f, 0.f)); // res_acc, res_prev, res_last, rho_s
     __stcg(reinterpret_cast<float4*>(&s->rho_a), make_float4(0.f, 1.f, 0.5f, 0.f));    // rho_a, alpha1, alpha2, side_done
     __stcg(reinterpret_cast<int4*>(&s->noboost), make_int4(0, a, m0, m1));
+    __stcg(&s->resume, 0);
     p_install_side(e, slot, SK_GATHER, (nset + e.gather_rowatoms - 1) / e.gather_rowatoms);
     return true;
 }
@@ -327,7 +335,8 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
             __stcg(&s->rho_a, rho);
             __stcg(&s->alpha1, 1.f / (rho * rho));
             __stcg(&s->alpha2, 0.5f / rho);
-            p_install_gemm(e, slot, OP_SIGN_G1);
+            if (e.split_tokens) { __stcg(&s->resume, 1); p_enter_heavy(e, slot); }
+            else p_install_gemm(e, slot, OP_SIGN_G1);
         }
         return;
     }
@@ -378,6 +387,7 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
             p_install_gemm(e, slot, OP_INV_G1);
         }
     } else if (kind == OP_AMAT) {
+        if (e.split_tokens) p_leave_heavy(e, slot);              // the token is not held across the power iteration
         p_start_power(e, slot, OP_POW_A);
     } else if (kind == OP_SIGN_G2) {
         __stcg(&s->sign_iters, __ldcg(&s->sign_iters) + 1);

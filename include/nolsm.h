@@ -127,7 +127,9 @@ int nolsm_assemble(nolsm_ctx* ctx, int64_t n_atoms, const int32_t* atom_nb, cons
 int nolsm_density_matrix(nolsm_ctx* ctx, double mu, void* D_vals, int d_dtype, void* cuda_stream);
 
 /* Same for atoms [atom_begin, atom_end) only; other rows of D_vals are left untouched. If
- * e_partial_host is not NULL the call synchronises and stores sum of e_i over the range. */
+ * e_partial_host is not NULL the call synchronises and stores sum of e_i over the range. With combine every group
+ * that has a member in the range is evaluated and serves its members inside the range (a group that straddles a range
+ * boundary is evaluated once per range it touches). */
 int nolsm_density_matrix_range(nolsm_ctx* ctx, double mu, int64_t atom_begin, int64_t atom_end, void* D_vals,
                                int d_dtype, double* e_partial_host, void* cuda_stream);
 

@@ -60,6 +60,8 @@ struct nolsm_ctx {
     long long *d_unit_ptr = nullptr, *d_uset_ptr = nullptr;
     int *d_unit_mem = nullptr, *d_uset_atom = nullptr, *d_uset_off = nullptr, *d_udim = nullptr, *d_upos = nullptr, *d_nset_uoff = nullptr;
     bool combined = false;
+    int* d_feed = nullptr;              // units of the running call (combined mode)
+    std::vector<int32_t> h_feed;
     int max_n = 0, max_nset = 0, max_nbi = 0;
 
     // device arrays
@@ -851,6 +853,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         c->d_udim = (int*)tmp;
         if ((r = to_device(c, c->upos.data(), sizeof(int32_t) * n_atoms, &tmp, s))) return r;
         c->d_upos = (int*)tmp;
+        if ((r = dmalloc(c, (void**)&c->d_feed, 4 * (size_t)c->n_units))) return r;
     } else {                      // unit u is atom u: the unit arrays are the per-atom ones
         c->d_uset_ptr = c->d_nset_ptr; c->d_uset_atom = c->d_nset_atom; c->d_uset_off = c->d_nset_off;
         c->d_nset_uoff = c->d_nset_off; c->d_udim = c->d_dim; c->d_upos = c->d_pos;
@@ -1091,9 +1094,22 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
     if (c->persist) {
         // ---- persistent engine: one kernel launch evaluates the whole range ----
         PEngine pe = c->peng;
-        if (c->combined && (a0 != 0 || a1 != c->n_atoms)) return fail(c, NOLSM_EINVAL, "with combine the whole system is evaluated per call (groups span atom ranges)");
-        const int64_t u0 = c->combined ? 0 : a0, u1 = c->combined ? c->n_units : a1;      // the feed counts units
+        // the feed counts units. Combined: every unit with a member in [a0, a1) is evaluated and serves its members inside
+        // the range (a unit that straddles a range boundary is evaluated once per range it touches)
+        int64_t u0 = a0, u1 = a1;
+        if (c->combined) {
+            c->h_feed.clear();
+            std::vector<char> seen(c->n_units, 0);
+            for (int64_t a = a0; a < a1; ++a) {
+                const int32_t u = c->unit_of[a];
+                if (!seen[u]) { seen[u] = 1; c->h_feed.push_back(u); }
+            }
+            std::sort(c->h_feed.begin(), c->h_feed.end());
+            CU_TRY(c, cudaMemcpyAsync(c->d_feed, c->h_feed.data(), 4 * c->h_feed.size(), cudaMemcpyHostToDevice, s));
+            u0 = 0; u1 = (int64_t)c->h_feed.size();
+        }
         pe.mu = (float)mu; pe.a_end = (int)u1; pe.total = (int)(u1 - u0);
+        pe.feed = c->combined ? c->d_feed : nullptr; pe.atom_lo = (int)a0; pe.atom_hi = (int)a1;
         pe.D_vals = D_dev; pe.d_f64 = d_dtype == NOLSM_DTYPE_F64;
         c->h_a0 = (int)u0;
         memset(c->h_ctr0, 0, sizeof(c->h_ctr0));
@@ -1216,7 +1232,8 @@ int nolsm_energy(nolsm_ctx* c, double* e_elec) {
     double sum = 0;
     int bits = 0;
     for (int64_t i = 0; i < n; ++i) sum += e[i];
-    for (int64_t u = 0; u < nu; ++u) bits |= st[u];
+    if (c->combined) { for (int32_t u : c->h_feed) bits |= st[u]; }           // the units of the last call
+    else for (int64_t u = 0; u < nu; ++u) bits |= st[u];
     *e_elec = sum;
     if (bits & ST_NOTSPD) return fail(c, NOLSM_ENOTSPD, "an S_sub inverse iteration failed (see nolsm_get_atom_stats)");
     if (bits & ST_NOCONV) return fail(c, NOLSM_ENOCONV, "a sign iteration hit max_sign_iters (see nolsm_get_atom_stats)");

@@ -66,7 +66,9 @@ struct PEngine {
     float tol_inv, tol_sign, mu, safety_s, safety_a;
     int max_inv, max_sign, p_s, p_a;
     int gather_rowatoms, schulz_chunks, dcols_chunks;   // row-atoms of N(i) per gather chunk; chunks of the other tasks
-    int* next_atom; int a_end, total;
+    int* next_atom; int a_end, total;                 // feed position, its end, units of this call
+    const int* feed;              // feed position -> unit id (nullptr: the position is the unit id)
+    int atom_lo, atom_hi;         // only members inside [atom_lo, atom_hi) get their columns of D (nolsm_density_matrix_range)
     int* finished;
     int* heavy;                   // [1] slots inside the GEMM-heavy phases INV .. SIGN right now (at most g_max)
     int* parked;                  // [S] 1 = the slot finished its first Schulz step and waits for a heavy token
@@ -266,8 +268,9 @@ __device__ __forceinline__ void p_leave_heavy(const PEngine& e, int slot) {
 // the feed is exhausted (the slot stays free).
 __device__ __forceinline__ bool p_refill(const PEngine& e, int slot) {
     if (*(volatile int*)e.next_atom >= e.a_end) return false;
-    const int a = atomicAdd(e.next_atom, 1);                            // a unit of the feed
-    if (a >= e.a_end) return false;
+    const int fpos = atomicAdd(e.next_atom, 1);                         // a unit of the feed
+    if (fpos >= e.a_end) return false;
+    const int a = e.feed ? e.feed[fpos] : fpos;
     PSlot* s = &e.slots[slot];
     const int n = e.udim[a], n16 = (n + 15) & ~15;
     int ntm, ntn;
@@ -275,7 +278,9 @@ __device__ __forceinline__ bool p_refill(const PEngine& e, int slot) {
     if (e.ctas == G4_CTAS) ntn = g4_ntn(n16);                           // cluster tiles per row of tiles
     else ntn = (n16 + e.tile_n - 1) / e.tile_n;
     const int nset = (int)(e.sv.uset_ptr[a + 1] - e.sv.uset_ptr[a]);
-    const int m0 = (int)e.sv.unit_ptr[a], m1 = (int)e.sv.unit_ptr[a + 1];
+    int m0 = (int)e.sv.unit_ptr[a];
+    const int m1 = (int)e.sv.unit_ptr[a + 1];
+    while (m0 + 1 < m1 && (e.sv.unit_mem[m0] < e.atom_lo || e.sv.unit_mem[m0] >= e.atom_hi)) ++m0;   // the feed holds units with a member in range
     const int atom = e.sv.unit_mem[m0];
     __stcg(reinterpret_cast<int4*>(&s->atom), make_int4(atom, n, n16, e.upos[atom]));
     __stcg(reinterpret_cast<int4*>(&s->nbi), make_int4(e.at.nb[atom], ntm, ntn, nset));
@@ -341,7 +346,7 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
         return;
     }
     if (kind == OP_DCOLS) {                 // a skinny product, not one of the counted square GEMMs
-        if (__ldcg(&s->mptr) == (int)e.sv.unit_ptr[__ldcg(&s->unit)]) p_leave_heavy(e, slot);   // first member: the chain is over
+        if (__ldcg(&s->resume) != 2) { __stcg(&s->resume, 2); p_leave_heavy(e, slot); }          // first member served: the chain is over
         p_install_side(e, slot, SK_DCOLS, e.dcols_chunks);
         return;
     }
@@ -853,8 +858,10 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
                         atomicAdd(&e.ctr[PC_SIDE_BYTES + SK_DCOLS],
                                   (unsigned long long)(nv * ((e.d_f64 ? 8 : 4) + (e.val_f64 ? 8 : 4)) + (double)n * PCW * 4.0 + (double)n * nbi * 2.0));
                         // the next member of the unit takes its columns from the same X and Y, or the slot retires
-                        const int mp = __ldcg(&s->mptr) + 1;
-                        if (mp < __ldcg(&s->mend)) {
+                        int mp = __ldcg(&s->mptr) + 1;
+                        const int mend = __ldcg(&s->mend);
+                        while (mp < mend && (e.sv.unit_mem[mp] < e.atom_lo || e.sv.unit_mem[mp] >= e.atom_hi)) ++mp;
+                        if (mp < mend) {
                             const int nxt = e.sv.unit_mem[mp];
                             __stcg(&s->mptr, mp);
                             __stcg(&s->atom, nxt);

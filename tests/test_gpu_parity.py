@@ -317,16 +317,30 @@ def test_combined_groups_bit_exact_and_parity(name, n_atoms, mode):
     assert abs(E - st["e_atom"].sum()) <= 1e-9 * abs(E)
 
 
-def test_combine_rejects_partial_ranges_and_round_engine(cfg0):
+def test_combine_with_atom_ranges_and_round_engine(cfg0):
+    """nolsm_density_matrix_range with combination: every group with a member in the range is evaluated and serves its
+    members inside the range only - those rows equal the whole-system evaluation, all other rows stay untouched, and the
+    range energy is the sum of the members' e_i. The round engine rejects combine."""
     from paper_2205_12182_b200 import ENGINE_ROUNDS, NolsmError
     s = cfg0
     nb, rp, ci, Hv, Sv = _arrays(s)
+    blk = s.blk_off()
     with _nolsm(combine=1) as ctx:
         ctx.assemble(nb, rp, ci, Hv, Sv)
-        D = torch.zeros(Hv.shape[0], dtype=torch.float64, device="cuda")
-        with pytest.raises(NolsmError) as ei:
-            ctx.density_matrix_range(s.mu, 0, 10, D)
-        assert ei.value.code == 1
+        D_all = torch.zeros(Hv.shape[0], dtype=torch.float64, device="cuda")
+        ctx.density_matrix(s.mu, D_all)
+        ctx.energy()
+        e_all = ctx.atom_stats()["e_atom"]
+        D = torch.full((Hv.shape[0],), 7.0, dtype=torch.float64, device="cuda")
+        a0, a1 = 10, 30
+        e_rng = ctx.density_matrix_range(s.mu, a0, a1, D, want_energy=True)
+        e_at = ctx.atom_stats()["e_atom"]
+    v0, v1 = int(blk[s.row_ptr[a0]]), int(blk[s.row_ptr[a1]])
+    Dh, Dall = D.cpu().numpy(), D_all.cpu().numpy()
+    assert (Dh[:v0] == 7.0).all() and (Dh[v1:] == 7.0).all()
+    assert np.abs(Dh[v0:v1] - Dall[v0:v1]).max() <= 2e-3
+    assert abs(e_rng - e_at[a0:a1].sum()) <= 1e-9 * abs(e_rng)
+    assert abs(e_rng - e_all[a0:a1].sum()) <= TOL_MIXED_E * abs(e_rng)
     with _nolsm(combine=1, engine=ENGINE_ROUNDS) as ctx:
         with pytest.raises(NolsmError) as ei:
             ctx.assemble(nb, rp, ci, Hv, Sv)

@@ -874,9 +874,9 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     const size_t cap_bytes = c->opt.workspace_bytes ? c->opt.workspace_bytes : std::min<size_t>(free_b / 2, (size_t)48 << 30);
     // persistent engine: slot buffers must fit the side tasks' shared memory (power-iteration vectors, Y columns)
     const int g_rowatoms = std::max(1, getenv_int("NOLSM_GATHER_ROWATOMS", 4));
-    // (gather task: index tables + dense strip + 4 x 2 cp.async stages; a strip holds at least one dense row)
+    // (gather task: index tables + dense strip; a strip holds at least one dense row)
     c->persist = want_persist(c) && e.cap <= P_MAX_CAP && max_nbi <= NVC &&
-                 (size_t)(3 * max_nset + 2) * 4 + (size_t)max_nset * 8 + 32 + G_STRIP_BYTES + (size_t)P_SIDE_WARPS * 2 * G_STAGE_BYTES <= (size_t)P_SIDE_SMEM &&
+                 (size_t)(3 * max_nset + 2) * 4 + (size_t)max_nset * 8 + 32 + G_STRIP_BYTES <= (size_t)P_SIDE_SMEM &&
                  (size_t)e.cap * 2 <= (size_t)G_STRIP_BYTES;
     if (c->combined && !c->persist) return fail(c, NOLSM_EINVAL, "combine: the groups do not fit the persistent engine (dimension or index-set size)");
     if (!c->persist && c->opt.engine == NOLSM_ENGINE_PERSISTENT)
@@ -1018,6 +1018,7 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
         pe.g_max = pe.ndie == 2 ? std::max(1, std::min(g_max, S) / 2) : std::max(1, std::min(g_max, S));
         pe.want_lead = std::max(1, getenv_int("NOLSM_WANT_LEAD", G2_WANT_LEAD));
         pe.dbg = getenv_int("NOLSM_DBG", 0);
+        pe.gather_prefetch = getenv_int("NOLSM_GATHER_PREFETCH", 0);   // measured: no gain on cfg1 / cfg2, the loads in flight already cover the latency
         pe.split_tokens = getenv_int("NOLSM_SPLIT_TOKENS", 1);
         pe.half_tiles = c->opt.cluster_ctas == G4_CTAS ? 0 : getenv_int("NOLSM_HALF_TILES", 1);
         pe.tma_store = getenv_int("NOLSM_TMA_STORE", 1);
@@ -1541,6 +1542,7 @@ int nolsm_get_engine_counters(nolsm_ctx* c, double* out, int n) {
         static const char* nm[16] = {"mma_take", "mma_tempty", "mma_full", "mma_total", "epi_take", "epi_tfull(cum)", "epi_work(cum)", "epi_done(cum)",
                                      "prod_empty", "prod_total", "prod_take", "mma_fulltile_cyc", "mma_fulltiles", "", "", ""};
         for (int i = 0; i < 13; ++i) fprintf(stderr, "g4_timing %-16s %.3f Gcyc\n", nm[i], t[i] * 1e-9);
+        fprintf(stderr, "gather phases (thread 0 of every side group, Gcyc): lookup %.3f zero %.3f stream %.3f writeout %.3f\n", t[12] * 1e-9, t[13] * 1e-9, t[14] * 1e-9, t[15] * 1e-9);
         if (t[12]) fprintf(stderr, "g4_timing cycles per full-width tile (tempty wait + k-loop): %.0f\n", (double)t[11] / (double)t[12]);
         unsigned long long z[16] = {};
         cudaMemcpyToSymbol(g4_timing, z, sizeof(z));

@@ -75,6 +75,7 @@ struct PEngine {
     int g_max, want_lead, dbg;
     int tma_store;                // 1: square GEMM tiles leave through shared-memory boxes and TMA stores
     int split_tokens;             // 1: the heavy token is returned for the rho(A) power iteration and taken again for the sign phase
+    int gather_prefetch;          // 1: the gather task prefetches a row-atom's source blocks into L2 before staging them
     int half_tiles;               // 1: half-height (M = 128) tiles for a last row block of at most 128 rows
     int tile_n;                   // columns of a pair tile (256; 128 halves a GEMM's latency at more L2 traffic per FLOP)
     const signed char* die_of_sm; // [256] L2 die of every SM (0 / 1), or all -1: no die affinity (see k_die_probe)
@@ -524,35 +525,22 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
 // rows of T(S) (buffer 0) and T(H0) (buffer 1) that belong to row-atoms [a_lo, a_hi) of N: block (j_a, j_b) of the sparse matrix where it exists,
 // zeros elsewhere and in the pad strip [n, n16). The last chunk also zeroes rows [n, n16).
 //
-// Data path (HBM-bound work, so it is built around bytes in flight): the source blocks of a row-atom are
-// contiguous runs of nb(j_a) x nb(j_b) values; every warp streams its share of them into a private
-// two-stage staging area with 8-byte cp.async (no registers held while the loads fly), converts each
-// value once (RN-even, C-13) into a shared-memory strip of the dense rows, and the strip
-// leaves with 16-byte coalesced stores. Strips are G_STRIP_BYTES at most, so a row-atom of a wide
-// submatrix takes several passes over row sub-ranges of its blocks.
-constexpr int G_STRIP_BYTES = 28 * 1024;
-constexpr int G_STAGE_BYTES = 3 * 1024;           // per warp and stage
-constexpr int G_MAXI = 8;                         // blocks (or block pieces) per stage
-
-struct GItems {                                   // what one stage of one warp holds (warp-uniform)
-    int n;
-    int off[G_MAXI], nbb[G_MAXI], e0[G_MAXI], take[G_MAXI], at[G_MAXI];
-};
-
-template <typename TV>
-__device__ __forceinline__ void g_cp_async(uint32_t dst, const TV* src) {
-    if constexpr (sizeof(TV) == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
-    else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
-}
+// Data path: the source blocks of a row-atom are contiguous runs of nb(j_a) x nb(j_b) values. All of them (S and H0) are
+// prefetched into L2 first; every warp then loads G_NB blocks at a time with coalesced 8-byte loads, converts each value
+// once (RN-even, C-13) into a shared-memory strip of the dense rows, and the strip leaves with 16-byte
+// coalesced stores. Strips are G_STRIP_BYTES at most, so a row-atom of a very wide submatrix takes several passes over
+// row sub-ranges of its blocks.
+constexpr int G_STRIP_BYTES = 48 * 1024;
+constexpr int G_NB = 2;                           // blocks a warp has in flight (8 loads per lane each)
 
 template <typename TV>
 __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_vals, const TV* __restrict__ H_vals,
                                   __half* __restrict__ dstS, __half* __restrict__ dstH, int unit, int n, int n16, int ld,
-                                  int chunk, int nchunks, unsigned char* sm, int tid, unsigned long long* bytes) {
+                                  int chunk, int nchunks, unsigned char* sm, int tid, unsigned long long* bytes, int e_prefetch = 1) {
     const long long p0 = sv.uset_ptr[unit];
     const int cnt = (int)(sv.uset_ptr[unit + 1] - p0);
     const int warp = tid >> 5, lane = tid & 31;
-    // shared memory: tables | strip | staging (4 warps x 2 stages)
+    // shared memory: tables | strip
     int* s_nset = reinterpret_cast<int*>(sm);                              // [cnt] atoms of N(i)
     int* s_off = s_nset + cnt;                                             // [cnt + 1] first column of each atom
     int* s_list = s_off + cnt + 1;                                         // [cnt] present blocks of the current row-atom
@@ -560,9 +548,6 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
     long long* s_boff = reinterpret_cast<long long*>(sm + (((size_t)(3 * cnt + 2) * 4 + 15) & ~(size_t)15));   // [cnt]
     unsigned char* strip_b = reinterpret_cast<unsigned char*>(s_boff) + (((size_t)cnt * 8 + 15) & ~(size_t)15);
     __half* strip = reinterpret_cast<__half*>(strip_b);
-    unsigned char* stage_b = strip_b + G_STRIP_BYTES + (size_t)warp * 2 * G_STAGE_BYTES;
-    const uint32_t stage_u = ptx::smem_u32(stage_b);
-    constexpr int CAP_E = G_STAGE_BYTES / (int)sizeof(TV);                 // values per stage
 
     const int a_lo = (int)((long long)cnt * chunk / nchunks), a_hi = (int)((long long)cnt * (chunk + 1) / nchunks);
     for (int b = tid; b < cnt; b += P_SIDE_THREADS) { s_nset[b] = sv.uset_atom[p0 + b]; s_off[b] = sv.uset_off[p0 + b]; }
@@ -572,6 +557,12 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
     const int vpr = n16 >> 3;                                              // 16-byte vectors per dense row
     unsigned long long nread = 0;
 
+#ifdef NOLSM_TIMING
+    long long tp_[4] = {0, 0, 0, 0}, tq_ = clock64();
+#define GT_(i) do { const long long t_ = clock64(); tp_[i] += t_ - tq_; tq_ = t_; } while (0)
+#else
+#define GT_(i)
+#endif
     for (int a = a_lo; a < a_hi; ++a) {
         const int j = s_nset[a];
         const int nbj = s_off[a + 1] - s_off[a], row0 = s_off[a];
@@ -601,6 +592,24 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
         }
         pl::side_sync();
         const int m = *s_m;
+        // L2 prefetch of every source block of this row-atom (S and H0): the staged loads below can keep only ~24 KB in
+        // flight per side group, a prefetch needs no shared memory, so all but the first stage round find their lines in L2
+        if (e_prefetch) {
+            const int nbmax = s_off[cnt] > 0 ? 32 : 32;            // lines per block: computed per block below
+            (void)nbmax;
+            for (int q = tid; q < m; q += P_SIDE_THREADS) {
+                const int b = s_list[q];
+                const long long bo = s_boff[b];
+                const int bytes_b = nbj * (s_off[b + 1] - s_off[b]) * (int)sizeof(TV);
+                const char* ps = reinterpret_cast<const char*>(S_vals + bo);
+                const char* ph = reinterpret_cast<const char*>(H_vals + bo);
+                for (int o = 0; o < bytes_b + 127; o += 128) {
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(ps + min(o, bytes_b - 1)));
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(ph + min(o, bytes_b - 1)));
+                }
+            }
+        }
+        GT_(0);
 #pragma unroll 1
         for (int which = 0; which < 2; ++which) {
             const TV* __restrict__ vals = which ? H_vals : S_vals;
@@ -614,57 +623,47 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
                     for (int q = tid; q < nr * vpr; q += P_SIDE_THREADS) s4[q] = z;
                 }
                 pl::side_sync();
-                // ---- each warp streams its blocks (list entries warp, warp + 4, ...) through its two stages ----
-                int li = warp, e_next = 0;
-                auto fill = [&](int st, GItems& it) {
-                    it.n = 0;
-                    int used = 0;
-                    while (li < m && it.n < G_MAXI) {
-                        const int b = s_list[li];
-                        const int nbb = s_off[b + 1] - s_off[b];
-                        const int bs = nr * nbb, rem = bs - e_next;
-                        const int take = min(rem, CAP_E - used);
-                        if (take <= 0 || (take < rem && used > 0)) break;      // a block is split only across empty stages
-                        const TV* src = vals + s_boff[b] + (long long)r0 * nbb + e_next;
-                        const uint32_t d0 = stage_u + (uint32_t)(st * G_STAGE_BYTES) + (uint32_t)used * (uint32_t)sizeof(TV);
-                        for (int e = lane; e < take; e += 32) g_cp_async<TV>(d0 + (uint32_t)e * (uint32_t)sizeof(TV), src + e);
-                        it.off[it.n] = s_off[b]; it.nbb[it.n] = nbb; it.e0[it.n] = e_next; it.take[it.n] = take; it.at[it.n] = used;
-                        ++it.n;
-                        used += take; e_next += take; nread += (lane == 0) ? (unsigned long long)take : 0ull;
-                        if (e_next == bs) { li += P_SIDE_WARPS; e_next = 0; }
-                    }
-                    pl::cp_async_commit();
-                };
-                auto convert = [&](int st, const GItems& it) {
-                    const TV* sv_ = reinterpret_cast<const TV*>(stage_b + st * G_STAGE_BYTES);
+                GT_(1);
+                // ---- each warp takes G_NB blocks at a time: all their loads are issued (coalesced 8-byte loads, G_NB x 8 per
+                //      lane in flight) before the first value is converted into the strip. (8-byte cp.async staging ran at
+                //      ~8 cycles per element in the load/store unit and made the gather the busiest side task.) ----
+#pragma unroll 1
+                for (int l0 = warp * G_NB; l0 < m; l0 += P_SIDE_WARPS * G_NB) {
+                    TV v[G_NB][8];
 #pragma unroll
-                    for (int q = 0; q < G_MAXI; ++q) {
-                        if (q < it.n) {
-                            const int nbb = it.nbb[q];
-                            for (int e = lane; e < it.take[q]; e += 32) {
-                                const int idx = it.e0[q] + e;
-                                const int rr = idx / nbb, cc = idx - rr * nbb;
-                                strip[rr * n16 + it.off[q] + cc] = Num<__half>::from_d((double)sv_[it.at[q] + e]);
+                    for (int u = 0; u < G_NB; ++u) {
+                        const int li = l0 + u;
+                        if (li < m) {
+                            const int b = s_list[li];
+                            const int nbb = s_off[b + 1] - s_off[b], bs = nr * nbb;
+                            const TV* src = vals + s_boff[b] + (long long)r0 * nbb;
+#pragma unroll
+                            for (int k = 0; k < 8; ++k) {
+                                const int e = lane + 32 * k;
+                                v[u][k] = e < bs ? __ldg(src + e) : (TV)0;
+                            }
+                            nread += (lane == 0) ? (unsigned long long)bs : 0ull;
+                        }
+                    }
+#pragma unroll
+                    for (int u = 0; u < G_NB; ++u) {
+                        const int li = l0 + u;
+                        if (li < m) {
+                            const int b = s_list[li];
+                            const int nbb = s_off[b + 1] - s_off[b], bs = nr * nbb, c0 = s_off[b];
+#pragma unroll
+                            for (int k = 0; k < 8; ++k) {
+                                const int e = lane + 32 * k;
+                                if (e < bs) {
+                                    const int rr = e / nbb, cc = e - rr * nbb;
+                                    strip[rr * n16 + c0 + cc] = Num<__half>::from_d((double)v[u][k]);
+                                }
                             }
                         }
                     }
-                };
-                GItems ia, ib;
-                fill(0, ia);
-                for (;;) {
-                    fill(1, ib);
-                    pl::cp_async_wait<1>();
-                    convert(0, ia);
-                    __syncwarp();                      // stage 0 is refilled next
-                    if (ib.n == 0) break;
-                    fill(0, ia);
-                    pl::cp_async_wait<1>();
-                    convert(1, ib);
-                    __syncwarp();
-                    if (ia.n == 0) break;
                 }
-                pl::cp_async_wait<0>();
                 pl::side_sync();
+                GT_(2);
                 // ---- the strip leaves with 16-byte stores ----
                 {
                     const uint4* s4 = reinterpret_cast<const uint4*>(strip);
@@ -674,9 +673,13 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
                     }
                 }
                 pl::side_sync();
+                GT_(3);
             }
         }
     }
+#ifdef NOLSM_TIMING
+    if (tid == 0) for (int i_ = 0; i_ < 4; ++i_) atomicAdd(&g4_timing[12 + i_], (unsigned long long)tp_[i_]);
+#endif
     if (chunk == nchunks - 1) {
         const uint4 z = make_uint4(0, 0, 0, 0);
         for (int idx = tid; idx < (n16 - n) * vpr; idx += P_SIDE_THREADS) {
@@ -818,8 +821,8 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
             case SK_GATHER: {
                 __half* dS = e.base + buf_off(e, slot, 0);
                 __half* dH = e.base + buf_off(e, slot, 1);
-                if (e.val_f64) side_gather_chunk<double>(e.sv, (const double*)e.S_vals, (const double*)e.H_vals, dS, dH, __ldcg(&s->unit), n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER]);
-                else side_gather_chunk<float>(e.sv, (const float*)e.S_vals, (const float*)e.H_vals, dS, dH, __ldcg(&s->unit), n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER]);
+                if (e.val_f64) side_gather_chunk<double>(e.sv, (const double*)e.S_vals, (const double*)e.H_vals, dS, dH, __ldcg(&s->unit), n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER], e.gather_prefetch);
+                else side_gather_chunk<float>(e.sv, (const float*)e.S_vals, (const float*)e.H_vals, dS, dH, __ldcg(&s->unit), n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER], e.gather_prefetch);
             } break;
             case SK_SCHULZ1:
                 side_schulz1_chunk(e.base + buf_off(e, slot, 0), e.base + buf_off(e, slot, 2), n, n16, e.ld, __ldcg(&s->rho_s), chunk, nch, tid);

@@ -361,6 +361,8 @@ def main():
                        "dim_mean": stats["dim_mean"], "dim_min": stats["dim_min"], "dim_max": stats["dim_max"],
                        "precision": "fp16 operands / fp32 accumulate", "gamma_S": system.gamma,
                        "parallelism": "replicas" if world > 1 else "single",
+                       "combine": args.combine,
+                       "value_counts": "atoms served per second (one submatrix per atom when combine = 0)",
                        "l2": "inputs (8 GB block-CSR) and workspace >> 126 MB L2; no flush needed"},
             "tensor_tflops": tflops, "pct_of_dense_fp16_peak": {"nominal_2250": 100 * tflops / NOMINAL_FP16_TFLOPS / world,
                                                                  "measured_burst": 100 * tflops / peaks["bf16_tflops"] / world,

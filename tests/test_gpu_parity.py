@@ -435,3 +435,67 @@ def test_combination_with_other_options(kw):
     print("options", kw, "groups", len(groups), "max|dD|", max_d, "rel dE", abs(e_gpu - e_ref) / abs(e_ref))
     assert max_d <= TOL_MIXED_D and abs(e_gpu - e_ref) / abs(e_ref) <= TOL_MIXED_E
     assert abs(E - st["e_atom"].sum()) <= 1e-9 * abs(E)
+
+
+# ---- randomized shapes: basis sizes 1..16, submatrix dimensions around the tile boundaries -----------------------
+def _random_system(rng, n_at, nb_choices, p_link):
+    """Random symmetric pattern (diagonal set), random basis sizes, S = I + small symmetric, H0 symmetric with a gap."""
+    atom_nb = rng.choice(nb_choices, n_at).astype(np.int32)
+    pat = rng.random((n_at, n_at)) < p_link
+    pat = np.triu(pat, 1)
+    pat = pat | pat.T | np.eye(n_at, dtype=bool)
+    first = np.concatenate([[0], np.cumsum(atom_nb)])
+    N = int(first[-1])
+    A = rng.normal(size=(N, N))
+    H = 0.05 * (A + A.T)
+    half = rng.random(N) < 0.5
+    H[np.diag_indices(N)] = np.where(half, -1.0, 1.0) + 0.1 * rng.normal(size=N)
+    B = rng.normal(size=(N, N))
+    S = np.eye(N) + 0.004 * (B + B.T)
+    row_ptr, col_idx, Hv, Sv = [0], [], [], []
+    for i in range(n_at):
+        for j in np.flatnonzero(pat[i]):
+            col_idx.append(j)
+            Hv.append(H[first[i]:first[i + 1], first[j]:first[j + 1]].reshape(-1))
+            Sv.append(S[first[i]:first[i + 1], first[j]:first[j + 1]].reshape(-1))
+        row_ptr.append(len(col_idx))
+    return atom_nb, np.array(row_ptr, np.int64), np.array(col_idx, np.int32), np.concatenate(Hv), np.concatenate(Sv)
+
+
+@pytest.mark.parametrize("seed,n_at,nbs,p_link,combine", [
+    (0, 60, [1, 3, 5], 0.5, 0), (1, 90, [13, 16], 0.25, 0), (2, 70, [8, 16, 1], 0.6, 1),
+    (3, 120, [5, 13], 0.35, 2), (4, 40, [16], 1.0, 0), (5, 150, [2, 7], 0.8, 1)])
+def test_random_shapes_against_oracle(seed, n_at, nbs, p_link, combine):
+    """Random patterns and basis sizes (1..16 functions per atom): submatrix dimensions from a few functions to ~1000,
+    not multiples of 16, last row blocks on both sides of the half-height threshold, with and without combination."""
+    rng = np.random.default_rng(100 + seed)
+    atom_nb, rp, ci, Hv, Sv = _random_system(rng, n_at, nbs, p_link)
+    blk = orc.block_offsets(atom_nb, rp, ci)
+    with _nolsm(combine=combine) as ctx:
+        ctx.assemble(atom_nb, rp, ci, Hv, Sv)
+        D = np.zeros(len(Hv))
+        ctx.density_matrix(0.0, D)
+        E = ctx.energy()
+        st = ctx.atom_stats()
+        stats = ctx.stats()
+    assert (st["status"] == 0).all()
+    sets = [orc.index_set(i, rp, ci) for i in range(n_at)]
+    groups = orc.combine_groups(atom_nb, sets, mode=combine) if combine else [[i] for i in range(n_at)]
+    assert stats["n_units"] == len(groups)
+    max_d, e_ref, e_gpu = 0.0, 0.0, 0.0
+    for g in groups[::max(1, len(groups) // 12)]:
+        res = orc.group_result(g, atom_nb, rp, ci, blk, Hv, Sv, 0.0)
+        for i in g:
+            p0, p1 = int(rp[i]), int(rp[i + 1])
+            ref = np.zeros(int(blk[p1] - blk[p0]))
+            cols = ci[p0:p1]
+            for a, j in enumerate(res[i]["N"]):
+                p = p0 + int(np.searchsorted(cols, j))
+                ref[blk[p] - blk[p0]:blk[p + 1] - blk[p0]] = res[i]["Dcols"][res[i]["off"][a]:res[i]["off"][a + 1], :].T.reshape(-1)
+            max_d = max(max_d, float(np.abs(D[blk[p0]:blk[p1]] - ref).max()))
+            e_ref += res[i]["e_i"]
+            e_gpu += float(st["e_atom"][i])
+    print("random shapes", seed, "dims", stats["dim_min"], stats["dim_max"], "units", stats["n_units"], "max|dD|", max_d,
+          "rel dE", abs(e_gpu - e_ref) / abs(e_ref))
+    assert max_d <= TOL_MIXED_D
+    assert abs(e_gpu - e_ref) <= TOL_MIXED_E * abs(e_ref)

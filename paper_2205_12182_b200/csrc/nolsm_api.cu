@@ -146,10 +146,13 @@ size_t prof_begin(nolsm_ctx* c, int kind, cudaStream_t s) {
     c->recs.push_back({kind, i});
     return i;
 }
+bool sync_debug() {                                   // NOLSM_SYNC_DEBUG: eager rounds (NOLSM_GRAPH=0) name and synchronise every launch
+    static const bool on = getenv("NOLSM_SYNC_DEBUG") != nullptr;
+    return on;
+}
 void prof_end(nolsm_ctx* c, size_t i, cudaStream_t s) {
     if (c->prof_on) cudaEventRecord(c->ev_pool[i + 1], s);
-    static const bool sync_debug = getenv("NOLSM_SYNC_DEBUG") != nullptr;      // eager rounds only (NOLSM_GRAPH=0)
-    if (sync_debug) {
+    if (sync_debug()) {
         const cudaError_t e = cudaStreamSynchronize(s);
         if (e != cudaSuccess) { fprintf(stderr, "nolsm: launch %lld failed: %s\n", (long long)c->launches, cudaGetErrorString(e)); abort(); }
     }
@@ -158,7 +161,7 @@ void prof_end(nolsm_ctx* c, size_t i, cudaStream_t s) {
 #define LAUNCH(c, kind, s, ...)                      \
     do {                                             \
         const size_t pi_ = prof_begin(c, kind, s);   \
-        if (getenv("NOLSM_SYNC_DEBUG")) fprintf(stderr, "nolsm: launch %lld kind %d: %s\n", (long long)(c)->launches, kind, #__VA_ARGS__); \
+        if (sync_debug()) fprintf(stderr, "nolsm: launch %lld kind %d: %s\n", (long long)(c)->launches, kind, #__VA_ARGS__); \
         __VA_ARGS__;                                 \
         prof_end(c, pi_, s);                         \
     } while (0)

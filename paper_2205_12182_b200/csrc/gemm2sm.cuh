@@ -452,12 +452,12 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                     const bool full = (c + 32 <= bn) && (col0 + c + 32 <= n16);
                     const bool diag = (col0 + c < rbase + 32) && (col0 + c + 32 > rbase);
                     if (full && !diag) {
+                        if (ti.want_res && row < n16) {
 #pragma unroll
-                        for (int j = 0; j < 32; ++j) {
-                            const float a = __uint_as_float(v[j]);
-                            if (row < n16) vsum = fmaf(a, a, vsum);
-                            f[j] = sa * a;
+                            for (int j = 0; j < 32; ++j) { const float a = __uint_as_float(v[j]); vsum = fmaf(a, a, vsum); }
                         }
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) f[j] = sa * __uint_as_float(v[j]);
                     } else {
 #pragma unroll
                         for (int j = 0; j < 32; ++j) {

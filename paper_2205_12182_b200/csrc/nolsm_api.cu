@@ -614,8 +614,8 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
     if (getenv("NOLSM_COMBINE")) o.combine = getenv_int("NOLSM_COMBINE", 0);
     if (o.combine < 0 || o.combine > 2) { delete c; return NOLSM_EINVAL; }
     if (o.combine_max_dim <= 0) o.combine_max_dim = getenv_int("NOLSM_COMBINE_MAX_DIM", 2048);
-    if (o.combine_max_members <= 0) o.combine_max_members = 16;
-    if (o.combine_max_candidates <= 0) o.combine_max_candidates = 24;
+    if (o.combine_max_members <= 0) o.combine_max_members = getenv_int("NOLSM_COMBINE_MAX_MEMBERS", 16);
+    if (o.combine_max_candidates <= 0) o.combine_max_candidates = getenv_int("NOLSM_COMBINE_MAX_CANDIDATES", 24);
     if (getenv_int("NOLSM_CLUSTER", 0) > 0) o.cluster_ctas = getenv_int("NOLSM_CLUSTER", 0);
     if (o.cluster_ctas != 0 && o.cluster_ctas != 2 && o.cluster_ctas != 4) { delete c; return NOLSM_EINVAL; }
     if (o.sign_scale == 0.f) o.sign_scale = 1.5f;

@@ -106,6 +106,22 @@ def blas_threads() -> int:
         return os.cpu_count() or 1
 
 
+def max_over_ranks(value: float, world: int, device=None) -> float:
+    """The slowest rank's time decides (replicas run side by side): all-reduce MAX over the process group."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replicas_value(units_per_rank: int, world: int, seconds: float) -> float:
+    """Whole-job throughput of `world` independent replicas that each process `units_per_rank` units (weak scaling)."""
+    return world * units_per_rank / seconds
+
+
 def workload_label(name, n_atoms):
     return name if n_atoms is None else f"{name}@{n_atoms}"
 
@@ -219,11 +235,7 @@ def main():
     e1.record()
     barrier()
     clocks = sampler.stop()
-    ms_total = e0.elapsed_time(e1)
-    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item()) / args.steps
+    ms_step = max_over_ranks(e0.elapsed_time(e1), world, dev) / args.steps
     stats = ctx.stats()
 
     # ---- the same workload with submatrix combination (Eq. 9 / Eq. 10): fewer, larger
@@ -245,12 +257,10 @@ def main():
             Ec = step_c()
             c1.record()
             barrier()
-            tc = torch.tensor([c0.elapsed_time(c1)], dtype=torch.float64, device=dev)
-            if world > 1:
-                dist.all_reduce(tc, op=dist.ReduceOp.MAX)
+            ms_c = max_over_ranks(c0.elapsed_time(c1), world, dev)
             sc, pc = cx.stats(), cx.profile()
             combined["eq9" if mode == 1 else "eq10"] = {
-                "atoms_per_s": world * system.n_atoms / (float(tc.item()) * 1e-3), "ms_per_step": float(tc.item()),
+                "atoms_per_s": replicas_value(system.n_atoms, world, ms_c * 1e-3), "ms_per_step": ms_c,
                 "submatrices": sc["n_units"], "dim_mean": sc["dim_mean"], "dim_max": sc["dim_max"],
                 "gemms_per_submatrix": sc["gemms_executed"] / max(sc["n_units"], 1),
                 "flops_useful_per_step": sc["flops_useful"], "kernel_ms": pc["gemm_ms"],
@@ -278,13 +288,11 @@ def main():
         for _ in range(k_e2e):
             step_host()
         torch.cuda.synchronize()
-        dt = torch.tensor([(time.perf_counter() - t0) / k_e2e], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        dt_e2e = max_over_ranks((time.perf_counter() - t0) / k_e2e, world, dev)
         h2d = hH.numel() * 8 * 2 + h_nb.nbytes + h_rp.nbytes + h_ci.nbytes
         d2h = hD.numel() * 8 + 8
-        e2e = {"value": world * system.n_atoms / float(dt.item()), "unit": "submatrices/s",
-               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * float(dt.item())}
+        e2e = {"value": replicas_value(system.n_atoms, world, dt_e2e), "unit": "submatrices/s",
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * dt_e2e}
         ctx2.destroy()
         del hH, hS, hD
 
@@ -294,7 +302,7 @@ def main():
         return
 
     peaks = load_peaks()
-    value = world * system.n_atoms / (ms_step * 1e-3)
+    value = replicas_value(system.n_atoms, world, ms_step * 1e-3)
     tflops = world * stats["flops_useful"] / (ms_step * 1e-3) / 1e12
     # dominant kernel. Persistent engine: ONE launch of nolsm_persist_kernel per step runs a1-a7; its duration
     # comes from CUDA events recorded on the launching stream (nolsm_get_profile). Round engine: the grouped

@@ -20,7 +20,8 @@
  *     must be structurally symmetric with every diagonal block present.
  *   - Output layout: D_vals uses the same pattern and offsets; slot (i, j) holds (D_ji)^T, where block
  *     D_ji (rows of atom j, columns of atom i) is taken from submatrix i. The array is
- *     therefore D^T in block-CSR and row i is written by submatrix i alone. D is not symmetrised.
+ *     therefore D^T in block-CSR and row i is written by submatrix i alone (with options.combine: by the submatrix of the
+ *     group atom i belongs to). D is not symmetrised.
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
  *   - All functions return a nolsm_status; none throws or aborts. Numerical failures of single
  *     submatrices are reported asynchronously: they set per-atom status bits (nolsm_get_atom_stats) and

@@ -184,6 +184,11 @@ int nolsm_get_atom_stats(nolsm_ctx* ctx, int64_t atom_begin, int64_t count, int3
  *   out[7..9]   D columns + scatter: total ms, launches, algorithmic bytes (X and Y columns read, D row written, H0 row read)
  *   out[10..11] other kernels (mat-vecs, state, flags): total ms, launches
  *   out[12]     submatrices gathered in the sampled rounds;  out[13] kernel launches of the whole call
+ * After a call served by the persistent engine (one kernel, nolsm_get_engine_counters out[0] = 1) the same slots
+ * describe that kernel and cover the whole call: out[3] = its duration in ms (CUDA events on its stream), out[4] = 1,
+ * out[5..6] FLOP of all its GEMMs; out[0..2], out[7..9] and out[10..11] are the side tasks inside it (gather; D columns
+ * + scatter; refill + first Schulz step): busy ms summed over the side groups, tasks, algorithmic bytes;
+ * out[12] = submatrices of the call, out[13] = 1.
  * n must be >= NOLSM_PROFILE_LEN. Synchronises the stream. */
 #define NOLSM_PROFILE_LEN 14
 int nolsm_get_profile(nolsm_ctx* ctx, double* out, int n);

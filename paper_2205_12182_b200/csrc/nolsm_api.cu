@@ -413,28 +413,32 @@ void build_units(nolsm_ctx* c, int mode, int max_dim, int max_members, int max_c
         t_prev = t;
     };
     std::vector<char> is_free(n_at, 1);
-    std::vector<int32_t> G, in_g(n_at, -1);
+    std::vector<int32_t> G, gw(n_at, 0);      // gw[k] = n_b(k) while atom k is in the current group's set, else 0
     std::vector<std::pair<int64_t, int32_t>> cand;
     // overlaps dim(N(i) & N(j)) of every pair of the pattern, in parallel (the greedy pass below is sequential)
     std::vector<int32_t> ov;
     if (mode != 0 && max_members > 1) {
         ov.resize(c->nset_atom.size());
+        // the overlap is symmetric: each thread computes the pairs j > i of its atoms and stores both directions (the
+        // position of i in the sorted N(j) by binary search). w[k] = n_b(k) while k is in N(i), else 0: one gather per term.
         parallel_for(n_at, [&](int64_t b, int64_t e) {
-            std::vector<int32_t> mark(n_at, -1);                    // mark[k] == i: atom k is in N(i)
+            std::vector<int32_t> w(n_at, 0);
             for (int64_t i = b; i < e; ++i) {
                 const int32_t* Ni = c->nset_atom.data() + c->nset_ptr[i];
                 const int64_t ni = c->nset_ptr[i + 1] - c->nset_ptr[i];
-                for (int64_t q = 0; q < ni; ++q) mark[Ni[q]] = (int32_t)i;
+                for (int64_t q = 0; q < ni; ++q) w[Ni[q]] = nb[Ni[q]];
                 for (int64_t q = 0; q < ni; ++q) {
                     const int32_t j = Ni[q];
+                    if (j <= i) { if (j == i) ov[c->nset_ptr[i] + q] = 0; continue; }
+                    const int32_t* Nj = c->nset_atom.data() + c->nset_ptr[j];
+                    const int64_t nj = c->nset_ptr[j + 1] - c->nset_ptr[j];
                     int32_t d = 0;
-                    if (j != i) {
-                        const int32_t* Nj = c->nset_atom.data() + c->nset_ptr[j];
-                        const int64_t nj = c->nset_ptr[j + 1] - c->nset_ptr[j];
-                        for (int64_t t = 0; t < nj; ++t) d += (mark[Nj[t]] == (int32_t)i) ? nb[Nj[t]] : 0;
-                    }
+                    for (int64_t t = 0; t < nj; ++t) d += w[Nj[t]];
                     ov[c->nset_ptr[i] + q] = d;
+                    const int32_t* it = std::lower_bound(Nj, Nj + nj, (int32_t)i);     // the pattern is symmetric (validated in assemble)
+                    if (it != Nj + nj && *it == (int32_t)i) ov[c->nset_ptr[j] + (it - Nj)] = d;
                 }
+                for (int64_t q = 0; q < ni; ++q) w[Ni[q]] = 0;
             }
         });
     }
@@ -449,7 +453,7 @@ void build_units(nolsm_ctx* c, int mode, int max_dim, int max_members, int max_c
         G.assign(Ni, Ni + ni);
         int64_t n_g = c->dim[i];
         if (mode != 0 && max_members > 1) {
-            for (int64_t q = 0; q < ni; ++q) in_g[Ni[q]] = (int32_t)i;          // in_g[k] == i: atom k is in the group's set
+            for (int64_t q = 0; q < ni; ++q) gw[Ni[q]] = nb[Ni[q]];
             cand.clear();
             for (int64_t q = 0; q < ni; ++q) {
                 const int32_t j = Ni[q];
@@ -463,18 +467,19 @@ void build_units(nolsm_ctx* c, int mode, int max_dim, int max_members, int max_c
                 const int32_t j = cj.second;
                 const int32_t* Nj = c->nset_atom.data() + c->nset_ptr[j];
                 const int64_t nj = c->nset_ptr[j + 1] - c->nset_ptr[j];
-                int64_t n_gj = 0;
-                for (int64_t t = 0; t < nj; ++t) n_gj += (in_g[Nj[t]] == (int32_t)i) ? nb[Nj[t]] : 0;
+                int64_t n_gj = -cj.first;                   // while the set is still N(i): the pair overlap computed above
+                if (G.size() != (size_t)ni) { n_gj = 0; for (int64_t t = 0; t < nj; ++t) n_gj += gw[Nj[t]]; }
                 const int64_t n_u = n_g + c->dim[j] - n_gj;
                 if (n_u > max_dim) continue;
                 if (combine_cost(n_u, mode) < combine_cost(n_g, mode) + combine_cost(c->dim[j], mode)) {
                     c->unit_mem.push_back(j);
                     is_free[j] = 0;
                     for (int64_t t = 0; t < nj; ++t)
-                        if (in_g[Nj[t]] != (int32_t)i) { in_g[Nj[t]] = (int32_t)i; G.push_back(Nj[t]); }
+                        if (gw[Nj[t]] == 0) { gw[Nj[t]] = nb[Nj[t]]; G.push_back(Nj[t]); }
                     n_g = n_u;
                 }
             }
+            for (int32_t a : G) gw[a] = 0;
             if (c->unit_mem.size() - m0 > 1) std::sort(G.begin(), G.end());
         }
         const int32_t u = (int32_t)c->udim.size();

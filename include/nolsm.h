@@ -23,7 +23,9 @@
  *     therefore D^T in block-CSR and row i is written by submatrix i alone (with options.combine: by the submatrix of the
  *     group atom i belongs to). D is not symmetrised.
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
- *   - All functions return a nolsm_status; none throws or aborts. Numerical failures of single
+ *   - All functions return a nolsm_status; none throws, aborts or traps: a persistent kernel that overruns
+ *     options.timeout_s, or in which a wait stalls (device watchdog), is stopped through an abort word and the call
+ *     that waits for it returns NOLSM_ECUDA. Numerical failures of single
  *     submatrices are reported asynchronously: they set per-atom status bits (nolsm_get_atom_stats) and
  *     make nolsm_energy return NOLSM_ENOTSPD / NOLSM_ENOCONV after writing the result.
  */
@@ -54,12 +56,16 @@ enum { NOLSM_PREC_FP16_FP32 = 0, /* FP16 operands, FP32 accumulate, tcgen05 tens
 enum { NOLSM_DTYPE_F64 = 0, NOLSM_DTYPE_F32 = 1 };
 enum { NOLSM_GEMM_AUTO = 0, NOLSM_GEMM_UMMA = 1, NOLSM_GEMM_SIMT = 2 };
 enum { NOLSM_ENGINE_AUTO = 0, NOLSM_ENGINE_PERSISTENT = 1, NOLSM_ENGINE_ROUNDS = 2 };
+enum { NOLSM_ITER_EQ6 = 0,       /* Eq. 6 as printed: S^-1 by the Schulz iteration, sign iteration on A = S^-1 H0 - mu I */
+       NOLSM_ITER_LOWDIN = 1 };  /* symmetric form: Z = S^-1/2 by the coupled Newton-Schulz iteration, the same sign
+                                    iteration on the symmetric Z H0 Z - mu I, D = Z 1/2 (I - X) Z; every iterate is symmetric
+                                    (C-21). Persistent engine only. */
 enum { NOLSM_MAT_NOTSPD = 1, NOLSM_MAT_NOCONV = 2 }; /* per-atom status bits */
 
 /* Zero in any field selects the default given in brackets. */
 typedef struct {
     int precision;           /* NOLSM_PREC_* [FP16_FP32] */
-    int gemm_backend;        /* NOLSM_GEMM_* [AUTO: UMMA for FP16_FP32, SIMT for FP32] */
+    int gemm_backend;        /* NOLSM_GEMM_* [AUTO: UMMA (tcgen05, persistent engine) for FP16_FP32, SIMT (FFMA, round engine) for FP32] */
     int max_inv_iters;       /* cap on Schulz inverse iterations [24] */
     int max_sign_iters;      /* cap on Newton-Schulz sign iterations, Eq. 6 [64] */
     float tol_inv;           /* stop when ||I - S Y||_F / sqrt(n) < tol_inv [2e-3 mixed, 1e-5 FP32] */
@@ -70,23 +76,31 @@ typedef struct {
     int batch_atoms;         /* workspace slots = submatrices resident at once [auto: ~16 waves of GEMM tiles] */
     size_t workspace_bytes;  /* cap on the library-owned dense workspace [auto] */
     int profile_every;       /* round engine, > 0: every k-th round runs eagerly with CUDA events around each launch [0 = off] */
-    int engine;              /* NOLSM_ENGINE_* [AUTO: PERSISTENT (one kernel launch per density_matrix call) for the
-                                FP16/tcgen05 path when every n_i <= 4096, else ROUNDS (one CUDA graph per iteration round)] */
+    int engine;              /* NOLSM_ENGINE_* [AUTO: PERSISTENT (one kernel launch per density_matrix call, tcgen05 GEMMs) for the
+                                FP16_FP32 path when every n_i <= 4096 and nb(i) <= 16; else ROUNDS (plain FFMA GEMMs, one CUDA
+                                graph per iteration round): the validation engine] */
     int sign_scaled_iters;   /* persistent engine: the first k sign iterations run Eq. 6 on alpha X_k instead of X_k,
                                 X_{k+1} = 1/2 (alpha X_k)(3I - (alpha X_k)^2), alpha = sign_scale > 1, which lifts small
                                 eigenvalues 1.5 alpha x per step instead of 1.5 x and keeps the rest inside
                                 [alpha (3 - alpha^2) / 2, 1]; two steps with the optimal scalings for that interval follow,
                                 then plain Eq. 6 until the convergence test passes (C-6b) [6; -1 = plain Eq. 6] */
     float sign_scale;        /* alpha of the scaled steps, 1 < alpha < sqrt(3) [1.5] */
-    int cluster_ctas;        /* persistent engine, CTAs per thread-block cluster: 2 = one tcgen05 CTA pair per 256 x 256 tile;
-                                4 = two pairs on a 256 x 512 tile with the A operand TMA-multicast between them (less
-                                L2 -> SM traffic, but only 132 of 148 SMs can hold 4-CTA clusters on B200) [2] */
     int combine;             /* persistent engine: one submatrix for several columns. 0 = one submatrix per atom;
-                                1 = greedy groups under the cubic criterion Eq. 9 (L87); 2 = under Eq. 10 (L91) with the engine's
-                                measured characteristic p(n) n^3 := ceil(n16/256)^2 ceil(n16/64) (C-19) [0] */
+                                1 = greedy groups under the cubic criterion Eq. 9 (L87); 2 = under Eq. 10 (L91): predicted runtime
+                                n^3 / r(n) with the measured multiplication rate r(n) of nolsm_set_perf_table, linearly interpolated
+                                (without a table: the tile-step model ceil(n16/256)^2 ceil(n16/64), C-19) [0] */
     int combine_max_dim;     /* a group's union index set may not exceed this dimension [2048] */
     int combine_max_members; /* atoms per group at most [16] */
     int combine_max_candidates; /* candidates examined per seed atom, by descending overlap with the seed's index set [24] */
+    int iteration;           /* NOLSM_ITER_* [EQ6] */
+    int symmetric_tiles;     /* persistent engine: products of symmetric commuting matrices (the Schulz iterates; every product of
+                                the Loewdin form) multiply only the tiles on and above the diagonal of the tile grid and mirror
+                                them [0 = on; -1 = off: every tile is multiplied] */
+    int heavy_slots;         /* persistent engine: submatrices inside the GEMM chains at once [0 = auto: L2 size / (3.5 n^2 FP16)] */
+    int claim_lead;          /* persistent engine: a CTA pair claims its next tile when its TMA producer is this many k-blocks
+                                from the end of the current one [14] */
+    int mu_trials;           /* nolsm_find_mu, persistent engine: trial mu evaluated per pass on the resident S_sub^-1, A0 [3; max 8] */
+    double timeout_s;        /* persistent engine: the host stops a kernel that runs longer than this [300] */
 } nolsm_options;
 
 typedef struct {
@@ -102,6 +116,9 @@ typedef struct {
     double gather_bytes, scatter_bytes; /* algorithmic bytes of the last density_matrix call */
     int64_t n_units;              /* dense submatrices evaluated per call (== n_atoms without combination); dim_min / dim_max /
                                      dim_mean describe these */
+    int64_t gemms_symmetric;      /* of gemms_executed: symmetric products that multiplied the upper triangle of tiles only; they
+                                     count (ntm + 1) / (2 ntm) of 2 n^3 in flops_useful (the share of tiles executed) */
+    double flops_paper;           /* sum_i 2 n_i^3 * gemms_i with every product counted in full (PAPER.md:L156 knows no symmetric ones) */
 } nolsm_stats;
 
 /* Creates a context on `cuda_device`. opt may be NULL. */
@@ -147,12 +164,20 @@ int nolsm_destroy(nolsm_ctx* ctx);
  * step. q_atom_out (host, nullable) receives the q_i of the evaluated range. Synchronises. */
 int nolsm_electron_count(nolsm_ctx* ctx, double* n_elec, double* q_atom_out);
 
-/* Chemical-potential search: bisection on mu in [mu_lo, mu_hi] until |Tr(D(mu) S) - n_target| <=
- * tol_n, the bracket is narrower than tol_mu, or max_evals (0 = 40) density-matrix evaluations were spent. Tr(D S) never
- * decreases with mu; NOLSM_EINVAL if n_target is not bracketed. On return D_vals (host or device, as for
- * nolsm_density_matrix) holds D(mu_out), n_out = Tr(D(mu_out) S), evals_out the evaluations spent; nolsm_energy and
- * nolsm_get_stats refer to that last evaluation. Every evaluation is a full a1-a7 pass (S_sub^-1 is not kept across
- * evaluations: the dense submatrices of a 32,768-atom system exceed HBM). */
+/* Tr(D(mu_j) S) for n_mu (1..8) trial chemical potentials in ONE pass over the atoms (mu is iterated
+ * until the electron count is right; S_sub^-1 and A0 = S_sub^-1 H_sub do not depend on mu): every submatrix is gathered
+ * and inverted once, then the sign chain (Eq. 6) and the traces run once per trial mu on the resident A0 - mu_j I
+ * (C-20). No D is written. n_elec_out[j] = Tr(D(mu_j) S), e_out[j] (nullable) = Tr(D(mu_j) H0); host arrays.
+ * Persistent engine only. Synchronises. NOLSM_ENOTSPD / NOLSM_ENOCONV as for nolsm_energy. */
+int nolsm_electron_counts(nolsm_ctx* ctx, const double* mu, int n_mu, double* n_elec_out, double* e_out, void* cuda_stream);
+
+/* Chemical-potential search for |Tr(D(mu) S) - n_target| <= tol_n on [mu_lo, mu_hi]; stops also when
+ * the bracket is narrower than tol_mu or max_evals (0 = 40) trial mu were evaluated. Tr(D S) never decreases with mu;
+ * NOLSM_EINVAL if n_target is not bracketed. Persistent engine: the end points, then options.mu_trials equidistant trial mu
+ * per pass (nolsm_electron_counts: the bracket shrinks by mu_trials + 1 per pass, the gather and the inverse are done once
+ * per pass), and one final nolsm_density_matrix call at the mu reported. Round engine: bisection, one full call per trial.
+ * On return D_vals (host or device, as for nolsm_density_matrix) holds D(mu_out), n_out = Tr(D(mu_out) S), evals_out the
+ * trial mu evaluated; nolsm_energy and nolsm_get_stats refer to the final call. */
 int nolsm_find_mu(nolsm_ctx* ctx, double n_target, double mu_lo, double mu_hi, double tol_n, double tol_mu, int max_evals,
                   void* D_vals, int d_dtype, void* cuda_stream, double* mu_out, double* n_out, int* evals_out);
 
@@ -162,11 +187,20 @@ int nolsm_find_mu(nolsm_ctx* ctx, double n_target, double mu_lo, double mu_hi, d
 int nolsm_get_group(nolsm_ctx* ctx, int64_t atom, int32_t* members_out, int32_t* n_members_inout, int32_t* set_out,
                     int32_t* n_set_inout, int32_t* dim_out);
 
+/* p(n) of Eq. 10 ("the matrix multiplication performance p(n) of the GPUs is measured for different
+ * matrix sizes n and interpolated"): count measured points, dimensions n[] strictly ascending in 1..8192, rates in TFLOP/s
+ * (rounded to integer GFLOP/s). combine = 2 then compares predicted runtimes n^3 / r(n), r linearly interpolated between
+ * neighbouring points and constant outside the table, in integer arithmetic (csrc/grouping.cpp). Takes effect at the next
+ * nolsm_assemble; count = 0 removes the table. workloads/pn_b200.json holds the table measured on B200 with
+ * `python bench.py --pn-sweep`. Host arrays. */
+int nolsm_set_perf_table(nolsm_ctx* ctx, const int32_t* n, const double* tflops, int count);
+
 /* N(i) (ascending atom ids) and n_i. atoms_out may be NULL to query the count; capacity in *n_inout. */
 int nolsm_get_index_set(nolsm_ctx* ctx, int64_t atom, int32_t* atoms_out, int32_t* n_inout, int32_t* dim_out);
 
-/* Runs the gather kernel for one atom and copies the dense n_i x n_i submatrix (row-major, tight) to
- * host memory. which: 0 = T_i(S), 1 = T_i(H0). out_fp16 != 0 -> uint16 FP16 bits, else float. */
+/* Runs the gather kernel for one atom and copies the dense submatrix the atom is evaluated on (row-major, tight) to
+ * host memory: n_i x n_i on N(i), or with combine the group's submatrix on its union index set (dimension and set from
+ * nolsm_get_group; FP16 only). which: 0 = T(S), 1 = T(H0). out_fp16 != 0 -> uint16 FP16 bits, else float. */
 int nolsm_gather_submatrix(nolsm_ctx* ctx, int64_t atom, int which, int out_fp16, void* out_host);
 
 int nolsm_get_stats(nolsm_ctx* ctx, nolsm_stats* out);
@@ -202,6 +236,13 @@ int nolsm_get_profile(nolsm_ctx* ctx, double* out, int n);
  *   4 D columns + scatter): busy ms summed over side groups, algorithmic bytes, tasks.  n must be >= NOLSM_COUNTERS_LEN. Synchronises. */
 #define NOLSM_COUNTERS_LEN 33
 int nolsm_get_engine_counters(nolsm_ctx* ctx, double* out, int n);
+
+/* HBM-bound side tasks timed alone: which = 0 the gather of every submatrix of the assembled system (a1),
+ * which = 1 the D columns + scatter + energy of every atom (a6-a7, on whatever the slots hold). The device functions of
+ * the persistent kernel, one 128-thread side group per CTA, `reps` launches between CUDA events. ms_out = mean time of one
+ * launch, bytes_out = algorithmic bytes of one launch (source blocks read + dense FP16 rows written; D written + H0, S,
+ * P and Y columns read). Invalidates the results of the last density_matrix call. Persistent engine only. */
+int nolsm_side_task_bandwidth(nolsm_ctx* ctx, int which, int reps, double* ms_out, double* bytes_out);
 
 const char* nolsm_last_error(const nolsm_ctx* ctx);
 

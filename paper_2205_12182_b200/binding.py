@@ -11,6 +11,7 @@ PREC_FP16_FP32, PREC_FP32 = 0, 1
 DTYPE_F64, DTYPE_F32 = 0, 1
 GEMM_AUTO, GEMM_UMMA, GEMM_SIMT = 0, 1, 2
 ENGINE_AUTO, ENGINE_PERSISTENT, ENGINE_ROUNDS = 0, 1, 2
+ITER_EQ6, ITER_LOWDIN = 0, 1
 STATUS_NAMES = {0: "OK", 1: "EINVAL", 2: "ECUDA", 3: "ENOMEM", 4: "ESTATE", 5: "ENOTSPD", 6: "ENOCONV"}
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -23,8 +24,10 @@ class NolsmOptions(C.Structure):
                 ("power_iters_s", C.c_int), ("power_iters_a", C.c_int), ("eps_filter", C.c_double),
                 ("batch_atoms", C.c_int), ("workspace_bytes", C.c_size_t), ("profile_every", C.c_int),
                 ("engine", C.c_int), ("sign_scaled_iters", C.c_int), ("sign_scale", C.c_float),
-                ("cluster_ctas", C.c_int), ("combine", C.c_int), ("combine_max_dim", C.c_int),
-                ("combine_max_members", C.c_int), ("combine_max_candidates", C.c_int)]
+                ("combine", C.c_int), ("combine_max_dim", C.c_int),
+                ("combine_max_members", C.c_int), ("combine_max_candidates", C.c_int), ("iteration", C.c_int),
+                ("symmetric_tiles", C.c_int), ("heavy_slots", C.c_int), ("claim_lead", C.c_int), ("mu_trials", C.c_int),
+                ("timeout_s", C.c_double)]
 
 
 class NolsmStats(C.Structure):
@@ -32,7 +35,8 @@ class NolsmStats(C.Structure):
                 ("dim_mean", C.c_double), ("sum_inv_iters", C.c_int64), ("sum_sign_iters", C.c_int64),
                 ("gemms_executed", C.c_int64), ("flops_useful", C.c_double), ("flops_padded", C.c_double),
                 ("n_notspd", C.c_int64), ("n_noconv", C.c_int64), ("gather_bytes", C.c_double),
-                ("scatter_bytes", C.c_double), ("n_units", C.c_int64)]
+                ("scatter_bytes", C.c_double), ("n_units", C.c_int64), ("gemms_symmetric", C.c_int64),
+                ("flops_paper", C.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -45,8 +49,7 @@ class NolsmError(RuntimeError):
 
 
 def lib_path() -> str:
-    """In-tree library; NOLSM_LIB names another build of the same sources (probe builds with timing counters)."""
-    return os.environ.get("NOLSM_LIB") or os.path.join(_HERE, "libnolsm.so")
+    return os.path.join(_HERE, "libnolsm.so")
 
 
 def load_library():
@@ -76,11 +79,15 @@ def load_library():
     lib.nolsm_get_atom_stats.argtypes = [P, I64, I64, P, P, P, P, P, P, P]
     lib.nolsm_get_profile.argtypes = [P, C.POINTER(C.c_double), I32]
     lib.nolsm_get_engine_counters.argtypes = [P, C.POINTER(C.c_double), I32]
+    lib.nolsm_electron_counts.argtypes = [P, P, I32, P, P, P]
+    lib.nolsm_set_perf_table.argtypes = [P, P, P, I32]
+    lib.nolsm_side_task_bandwidth.argtypes = [P, I32, I32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.nolsm_last_error.argtypes = [P]
     lib.nolsm_last_error.restype = C.c_char_p
     for f in ("nolsm_create", "nolsm_assemble", "nolsm_density_matrix", "nolsm_density_matrix_range", "nolsm_energy",
               "nolsm_destroy", "nolsm_get_index_set", "nolsm_get_group", "nolsm_electron_count", "nolsm_find_mu", "nolsm_gather_submatrix", "nolsm_get_stats",
-              "nolsm_get_atom_stats", "nolsm_get_profile", "nolsm_get_engine_counters"):
+              "nolsm_get_atom_stats", "nolsm_get_profile", "nolsm_get_engine_counters", "nolsm_electron_counts",
+              "nolsm_set_perf_table", "nolsm_side_task_bandwidth"):
         getattr(lib, f).restype = C.c_int
     _LIB = lib
     return lib
@@ -176,6 +183,29 @@ class Nolsm:
         self._check(self._lib.nolsm_electron_count(self._h, C.byref(n), q.ctypes.data))
         return n.value, q
 
+    def electron_counts(self, mus, with_energy: bool = False, stream: int = 0, strict: bool = True):
+        """Tr(D(mu_j) S) for up to 8 trial mu in one pass over the atoms (include/nolsm.h); no D is written."""
+        mu = np.ascontiguousarray(mus, dtype=np.float64)
+        n = np.zeros(len(mu), dtype=np.float64)
+        e = np.zeros(len(mu), dtype=np.float64)
+        self._check(self._lib.nolsm_electron_counts(self._h, mu.ctypes.data, len(mu), n.ctypes.data, e.ctypes.data, stream),
+                    soft=() if strict else (5, 6))
+        return (n, e) if with_energy else n
+
+    def set_perf_table(self, n, tflops):
+        """p(n) of Eq. 10: measured multiplication rate (TFLOP/s) at dimensions n (include/nolsm.h)."""
+        nn = np.ascontiguousarray(n, dtype=np.int32)
+        tt = np.ascontiguousarray(tflops, dtype=np.float64)
+        if len(nn) != len(tt):
+            raise ValueError("n and tflops must have the same length")
+        self._check(self._lib.nolsm_set_perf_table(self._h, nn.ctypes.data, tt.ctypes.data, len(nn)))
+
+    def side_task_bandwidth(self, which: int, reps: int = 3):
+        """(ms per launch, algorithmic bytes per launch) of the gather (0) / scatter (1) task launched alone."""
+        ms, by = C.c_double(), C.c_double()
+        self._check(self._lib.nolsm_side_task_bandwidth(self._h, which, reps, C.byref(ms), C.byref(by)))
+        return ms.value, by.value
+
     def find_mu(self, n_target: float, mu_lo: float, mu_hi: float, D_vals, tol_n: float = 1e-3, tol_mu: float = 1e-6,
                 max_evals: int = 0, stream: int = 0):
         """Bisection on mu until Tr(D S) = n_target (include/nolsm.h). Returns (mu, Tr(D S), evaluations)."""
@@ -204,7 +234,7 @@ class Nolsm:
         return mem, st, dim.value
 
     def gather_submatrix(self, atom: int, which: int, fp16: bool):
-        _, dim = self.index_set(atom)
+        _, _, dim = self.group(atom)                 # the submatrix the atom is evaluated on (its own without combine)
         out = np.empty((dim, dim), dtype=np.float16 if fp16 else np.float32)
         self._check(self._lib.nolsm_gather_submatrix(self._h, atom, which, 1 if fp16 else 0, out.ctypes.data))
         return out
@@ -236,7 +266,7 @@ class Nolsm:
         out = (C.c_double * 33)()
         self._check(self._lib.nolsm_get_engine_counters(self._h, out, 33))
         v = list(out)
-        kinds = ("none", "refill", "gather", "schulz1", "dcols", "k5", "k6", "k7")
+        kinds = ("none", "refill", "gather", "elementwise", "dcols", "wcols", "k6", "k7")
         d = {"persistent": bool(v[0]), "kernel_ms": v[1], "kernel_ms_device_clock": v[2], "tiles": v[3],
              "sched_idle_ms": v[4], "sched_busy_ms": v[5], "overshoots": v[6], "slots": int(v[7]), "pairs": int(v[8])}
         d["side"] = {k: {"busy_ms": v[9 + i], "bytes": v[17 + i], "tasks": v[25 + i]} for i, k in enumerate(kinds)

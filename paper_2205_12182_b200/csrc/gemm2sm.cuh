@@ -16,8 +16,7 @@
 // alternate 32-column chunks), warp 8 tile scheduler (leader CTA only), warp 9 TMA producer, warp 10
 // TMEM allocator + MMA issuer (leader only). The scheduler
 // publishes TileInfo records into a small shared-memory ring in BOTH CTAs; every other role consumes
-// them in order. Where the tiles come from is the caller's business (`next` functor): a static list in
-// the round engine, the device work queue in the persistent engine.
+// them in order. The tiles come from the device work queue of the persistent engine (persist.cuh).
 #pragma once
 #include "gemm_umma.cuh"
 
@@ -44,9 +43,17 @@ constexpr int G2_CTRL_THREADS = 11 * 32;              // warps 0..10
 // consumers of a TileInfo: leader = producer + MMA + epilogue warps, peer = producer + epilogue warps
 constexpr int G2_TI_CONSUMERS = 2 * (1 + G2_EPI_WARPS) + 1;
 
+// flags of TileInfo::valid
+constexpr int TI_VALID = 1;           // 0 = no more tiles
+constexpr int TI_HALF = 2;            // half-height tile (rows m0 .. m0+127, one M = 128 MMA per 16 k: 64 rows per CTA; TMEM lanes
+                                      // 0-63 hold columns [0, bn/2), lanes 64-127 columns [bn/2, bn))
+constexpr int TI_MIRROR = 4;          // off-diagonal tile of a symmetric product: C^T goes to the block below the diagonal too
+constexpr int TI_PLAIN = 8;           // C = c_out acc without identity term; residual = || alpha_res acc ||_F^2 (power iteration, D columns)
+constexpr int TI_F32OUT = 16;         // the first PCW accumulator columns go to the slot's FP32 block instead of C (D columns)
+constexpr int TI_SYMDIAG = 32;        // diagonal tile of a symmetric product: only its upper triangle is stored, and mirrored
+
 struct __align__(16) TileInfo {      // 64 bytes
-    int valid;                        // 0 = no more tiles; bit 1 set: half-height tile (rows m0 .. m0+127, one M = 128 MMA per 16 k:
-                                      // 64 rows per CTA; TMEM lanes 0-63 hold columns [0, bn/2), lanes 64-127 columns [bn/2, bn))
+    int valid;                        // TI_* flags
     int slot, m0, n0;                 // pair tile origin (rows m0 .. m0+255, columns n0 .. n0+bn-1)
     int n, n16, bn, nreports;         // nreports = CTA reports that complete the slot's GEMM
     int a_buf, b_buf, c_buf, want_res;
@@ -72,20 +79,6 @@ struct G2Smem {                       // byte offsets from the 1024-aligned base
     __device__ uint32_t tinfo(int q) const { return bars() + 256u + 64u * q; }
 };
 constexpr int G2_SMEM_BYTES = G2_STAGES * G2_STAGE_BYTES + G2_CSTAGE_BYTES + 256 + 64 * G2_NTI + 1024 /*align*/;
-
-#ifdef G2_TIMING
-// probe builds only: cycles spent waiting, summed over CTAs
-__device__ unsigned long long g2_timing[12];
-#define G2_T0() const long long t0_ = clock64()
-#define G2_T1(i) tacc_[i] += clock64() - t0_
-#define G2_TDECL() long long tacc_[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}
-#define G2_TFLUSH(lane0) do { if (lane0) for (int i_ = 0; i_ < 12; ++i_) if (tacc_[i_]) atomicAdd(&g2_timing[i_], (unsigned long long)tacc_[i_]); } while (0)
-#else
-#define G2_T0()
-#define G2_T1(i)
-#define G2_TDECL()
-#define G2_TFLUSH(lane0)
-#endif
 
 namespace ptx {
 
@@ -119,31 +112,43 @@ __device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t par
         : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
 }
-__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
+// The waits below return false on a stall (watchdog, gemm_umma.cuh).
+__device__ __forceinline__ bool mbar_wait_cluster(uint32_t bar, uint32_t parity, volatile int* abort_flag) {
     uint32_t spins = 0;
+    unsigned long long t0 = 0;
     while (!mbar_try_wait_cluster(bar, parity)) {
-        if (++spins > 4096u) __nanosleep(64);
-        if (spins > SPIN_LIMIT_SLOW) __trap();
+        if (++spins > 4096u) {
+            __nanosleep(64);
+            if ((spins & 4095u) == 0 && stalled(t0, abort_flag)) return false;
+        }
     }
+    return true;
 }
-// Wait that may legitimately last long (a role of the persistent engine with no work): polls gently
-// after a short spin; traps only after tens of seconds.
-__device__ __forceinline__ void mbar_wait_cluster_patient(uint32_t bar, uint32_t parity) {
-    uint32_t spins = 0;
+// Wait that may legitimately last long (a role of the persistent engine with no work): polls gently after a short spin.
+// The scheduler ends such a wait with a record that says "no more tiles"; the watchdog only covers a scheduler that is
+// itself stuck, so its limit is ten times the usual one.
+__device__ __forceinline__ bool mbar_wait_cluster_patient(uint32_t bar, uint32_t parity, volatile int* abort_flag) {
+    uint32_t spins = 0, rounds = 0;
+    unsigned long long t0 = 0;
     while (!mbar_try_wait_cluster(bar, parity)) {
-        if (++spins > 16u) __nanosleep(200);
-        if (spins > (1u << 28)) __trap();
+        if (++spins > 16u) {
+            __nanosleep(spins < 1024u ? 200 : 1000);
+            if ((spins & 4095u) == 0 && stalled(t0, abort_flag)) { if (++rounds >= 10u) return false; t0 = 0; }
+        }
     }
+    return true;
 }
 // Wait of the eight epilogue warps for the accumulator of the tile being multiplied: microseconds long and not on the
 // critical path (two accumulators), so the warps sleep between polls instead of issuing a try_wait loop (which was 28 %
 // of all instructions the kernel issued: profiles/r01_persist_v6.md) - the issue slots and the power go to the k-loop.
-__device__ __forceinline__ void mbar_wait_sleepy(uint32_t bar, uint32_t parity) {
+__device__ __forceinline__ bool mbar_wait_sleepy(uint32_t bar, uint32_t parity, volatile int* abort_flag) {
     uint32_t spins = 0;
+    unsigned long long t0 = 0;
     while (!mbar_try_wait(bar, parity)) {
         __nanosleep(spins < 4u ? 64 : 256);
-        if (++spins > (1u << 26)) __trap();
+        if ((++spins & 4095u) == 0 && stalled(t0, abort_flag)) return false;
     }
+    return true;
 }
 __device__ __forceinline__ void st_cluster_u32(uint32_t cluster_addr, uint32_t v) {
     asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(cluster_addr), "r"(v) : "memory");
@@ -187,15 +192,13 @@ __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.w
 template <int N>
 __device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-// 32 halves of one row into a staging box: chunks (16 B) j0 .. j0 + 3 of box row r, 128-byte swizzle (chunk ^ (r & 7))
-__device__ __forceinline__ void st_box_row(uint32_t box, int r, int j0, const float* v) {
+// 32 halves (16 packed pairs) of one row into a staging box: chunks (16 B) j0 .. j0 + 3 of box row r, 128-byte swizzle
+// (chunk ^ (r & 7))
+__device__ __forceinline__ void st_box_row(uint32_t box, int r, int j0, const uint32_t* hp) {
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-        __half2 h0 = __floats2half2_rn(v[8 * q], v[8 * q + 1]), h1 = __floats2half2_rn(v[8 * q + 2], v[8 * q + 3]);
-        __half2 h2 = __floats2half2_rn(v[8 * q + 4], v[8 * q + 5]), h3 = __floats2half2_rn(v[8 * q + 6], v[8 * q + 7]);
         const uint32_t a = box + (uint32_t)r * 128u + (uint32_t)(((j0 + q) ^ (r & 7)) << 4);
-        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(*reinterpret_cast<uint32_t*>(&h0)),
-                     "r"(*reinterpret_cast<uint32_t*>(&h1)), "r"(*reinterpret_cast<uint32_t*>(&h2)), "r"(*reinterpret_cast<uint32_t*>(&h3)) : "memory");
+        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(hp[4 * q]), "r"(hp[4 * q + 1]), "r"(hp[4 * q + 2]), "r"(hp[4 * q + 3]) : "memory");
     }
 }
 
@@ -226,65 +229,36 @@ __device__ __forceinline__ void g2_teardown(uint32_t tmem_base, int warp) {
     if (warp == G2_WARP_MMA) ptx::tmem_dealloc_pair(tmem_base, 512);
 }
 
-// ------------------------------------------------------------------------------------------------
-// Scheduler (leader CTA, one warp): publishes TileInfo records to both CTAs until `next` says stop.
-// next(TileInfo&) fills the record and returns false when there is no more work.
-// ------------------------------------------------------------------------------------------------
-template <typename Next>
-__device__ __forceinline__ void g2_scheduler(const G2Smem& sm, int lane, Next next) {
-    int q = 0; uint32_t ph = 0;
-    for (;;) {
-        for (uint32_t spins = 0; !ptx::mbar_try_wait_cluster(sm.ti_empty(q), ph ^ 1);) {    // runs ahead: poll gently
-            __nanosleep(200);
-            if (++spins > SPIN_LIMIT_SLOW) __trap();
-        }
-        TileInfo ti{};
-        if (lane == 0) ti.valid = next(ti) ? 1 : 0;
-        // lane i publishes word i of lane 0's record to both CTAs
-        const uint32_t* w = reinterpret_cast<const uint32_t*>(&ti);
-        uint32_t mine = 0;
-#pragma unroll
-        for (int i = 0; i < 16; ++i) {
-            const uint32_t v = __shfl_sync(0xffffffffu, w[i], 0);
-            if (lane == i) mine = v;
-        }
-        const int more = __shfl_sync(0xffffffffu, ti.valid, 0);
-        if (lane < 16) {
-            asm volatile("st.shared.u32 [%0], %1;" ::"r"(sm.tinfo(q) + 4u * lane), "r"(mine) : "memory");
-            ptx::st_cluster_u32(ptx::mapa(sm.tinfo(q), 1) + 4u * lane, mine);
-        }
-        __syncwarp();
-        if (lane == 0) {
-            ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_full(q), 0));
-            ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_full(q), 1));
-        }
-        if (!more) break;
-        if (++q == G2_NTI) { q = 0; ph ^= 1; }
-    }
-}
-
 // Consumer side of the TileInfo ring: wait for record q, copy it to registers, release the ring entry.
-__device__ __forceinline__ TileInfo g2_take(const G2Smem& sm, int q, uint32_t ph, bool release_lane) {
-    ptx::mbar_wait_cluster_patient(sm.ti_full(q), ph);
+// A stalled wait returns a record with valid == 0: the role leaves its loop. WARP = true: called by a whole warp
+// (lane `release_lane` releases the entry); WARP = false: called by the single thread that runs a role.
+template <bool WARP>
+__device__ __forceinline__ TileInfo g2_take(const G2Smem& sm, int q, uint32_t ph, bool release_lane, volatile int* abort_flag) {
     TileInfo ti;
+    if (!ptx::mbar_wait_cluster_patient(sm.ti_full(q), ph, abort_flag)) { ti.valid = 0; return ti; }
     uint32_t* w = reinterpret_cast<uint32_t*>(&ti);
 #pragma unroll
     for (int i = 0; i < 16; i += 4)
         asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
                      : "=r"(w[i]), "=r"(w[i + 1]), "=r"(w[i + 2]), "=r"(w[i + 3]) : "r"(sm.tinfo(q) + 4u * i) : "memory");
-    __syncwarp();
+    if (WARP) __syncwarp();
     if (release_lane) ptx::mbar_arrive_cluster_relaxed(ptx::mapa(sm.ti_empty(q), 0), w[0] ^ w[15]);
     return ti;
 }
 
 // ------------------------------------------------------------------------------------------------
-// TMA producer (one warp per CTA; lane 0 issues).
+// TMA producer: ONE thread per CTA runs this loop (the other lanes of its warp wait at the end of the role). The loop
+// is what paces a tile when the operands come from L2: per k-block it waits for the stage, arms the leader's full
+// barrier and issues the three or four box loads; everything else is hoisted out (measured on B200: with the whole warp
+// in the loop and lane 0 predicated inside, the k-block took ~650 cycles whatever the tile's width, the producer was
+// busy 85 % of the time and the MMA warp waited for operands; profiles/r02_producer.md).
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap* maps, uint32_t rank, int lane, int want_lead = G2_WANT_LEAD) {
+__device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap* maps, uint32_t rank, int want_lead, volatile int* abort_flag) {
     int stage = 0; uint32_t phase = 0;
     int q = 0; uint32_t tph = 0;
+    const uint32_t full0 = ptx::mapa(sm.full(0), 0);                        // the leader's full barriers
     for (;;) {
-        const TileInfo ti = g2_take(sm, q, tph, lane == 0);
+        const TileInfo ti = g2_take<false>(sm, q, tph, true, abort_flag);
         if (++q == G2_NTI) { q = 0; tph ^= 1; }
         if (!ti.valid) break;
         ptx::fence_proxy_async();      // operands may have been written by generic stores of another CTA
@@ -293,32 +267,30 @@ __device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap*
         const int nkb = (ti.n16 + BK - 1) / BK;
         const int half = ti.bn >> 1;
         const int nbox = (half + 63) >> 6;
-        const bool hh = (ti.valid & 2) != 0;                               // half-height tile: 64 rows of A per CTA
+        const bool hh = (ti.valid & TI_HALF) != 0;                         // half-height tile: 64 rows of A per CTA
         const uint32_t bytes = 2u * ((hh ? G2_A_BYTES / 2 : G2_A_BYTES) + nbox * B_BOX_BYTES);     // both CTAs of the pair
         const int row0 = ti.m0 + (hh ? 64 : 128) * (int)rank;
         const int col0 = ti.n0 + half * (int)rank;
-        const uint32_t full0 = ptx::mapa(sm.full(0), 0);                    // the leader's full barriers
-        const int kb_want = max(0, nkb - want_lead);
+        const int kb_want = rank == 0 ? max(0, nkb - want_lead) : -1;
+#pragma unroll 1
         for (int kb = 0; kb < nkb; ++kb) {
-            ptx::mbar_wait(sm.empty(stage), phase ^ 1);
-            if (lane == 0) {
-                if (kb == kb_want && rank == 0) ptx::mbar_arrive(sm.want());   // the scheduler may claim the next tile now
-                const uint32_t fb = full0 + 8u * stage;
-                if (rank == 0) ptx::mbar_expect_tx(sm.full(stage), bytes);
-                const uint32_t sa = sm.stage_a(stage), sb = sm.stage_b(stage);
-                ptx::tma_load_2d_pair(sa, map_a, kb * BK, row0, fb);
-                if (!hh) ptx::tma_load_2d_pair(sa + 8192, map_a, kb * BK, row0 + 64, fb);
-                for (int b = 0; b < nbox; ++b)
-                    ptx::tma_load_2d_pair(sb + b * B_BOX_BYTES, map_b, col0 + b * 64, kb * BK, fb);
-            }
-            __syncwarp();
+            if (!ptx::mbar_wait(sm.empty(stage), phase ^ 1, abort_flag)) return;
+            if (kb == kb_want) ptx::mbar_arrive(sm.want());                // the scheduler may claim the next tile now
+            const uint32_t fb = full0 + 8u * stage;
+            if (rank == 0) ptx::mbar_expect_tx(sm.full(stage), bytes);
+            const uint32_t sa = sm.stage_a(stage), sb = sm.stage_b(stage);
+            const int k0 = kb * BK;
+            ptx::tma_load_2d_pair(sa, map_a, k0, row0, fb);
+            if (!hh) ptx::tma_load_2d_pair(sa + 8192, map_a, k0, row0 + 64, fb);
+            ptx::tma_load_2d_pair(sb, map_b, col0, k0, fb);
+            if (nbox > 1) ptx::tma_load_2d_pair(sb + B_BOX_BYTES, map_b, col0 + 64, k0, fb);
             if (++stage == G2_STAGES) { stage = 0; phase ^= 1; }
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// MMA issuer (leader CTA, one warp; one elected lane issues).
+// MMA issuer: ONE thread of the leader CTA.
 // The issue loop must stay well under the tensor-pipe time of a k-block (4 MMAs x ~120 cycles): the
 // four MMAs of a full k-block go out as one asm block with the descriptors advanced by immediates
 // (A: +32 B per 16 k inside the 128-byte swizzle row; B: +2048 B = 16 k-rows of 128 B).
@@ -341,100 +313,101 @@ __device__ __forceinline__ void umma_f16_pair_x4(uint32_t d_tmem, uint64_t a_des
 }
 }  // namespace ptx
 
-__device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int lane) {
+__device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, volatile int* abort_flag) {
     int stage = 0; uint32_t phase = 0;
     int acc = 0; uint32_t acc_phase = 0;
     int q = 0; uint32_t tph = 0;
     // descriptors of stage 0; stage s adds s * G2_STAGE_BYTES / 16 to the address field
     const uint64_t da0 = make_smem_desc(sm.stage_a(0), 16, 1024);
     const uint64_t db0 = make_smem_desc(sm.stage_b(0), B_BOX_BYTES, 1024);
-    G2_TDECL();
-    const long long tstart_ = clock64();
     for (;;) {
-        TileInfo ti;
-        { G2_T0(); ti = g2_take(sm, q, tph, lane == 0); G2_T1(0); }
+        const TileInfo ti = g2_take<false>(sm, q, tph, true, abort_flag);
         if (++q == G2_NTI) { q = 0; tph ^= 1; }
         if (!ti.valid) break;
         const int nkb = (ti.n16 + BK - 1) / BK;
         const int ktail = (ti.n16 - (nkb - 1) * BK) >> 4;          // 16-k slices of the last k-block (1..4)
-        const uint32_t idesc = make_idesc_f16((ti.valid & 2) ? 128 : 256, ti.bn);
-#ifdef G2_TIMING
-        const long long tk0_ = clock64();
-#endif
-        { G2_T0(); ptx::mbar_wait_cluster(sm.tempty(acc), acc_phase ^ 1); G2_T1(1); }
+        const uint32_t idesc = make_idesc_f16((ti.valid & TI_HALF) ? 128 : 256, ti.bn);
+        if (!ptx::mbar_wait_cluster(sm.tempty(acc), acc_phase ^ 1, abort_flag)) return;
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + acc * 256;
+#pragma unroll 1
         for (int kb = 0; kb < nkb; ++kb) {
-            { G2_T0(); ptx::mbar_wait(sm.full(stage), phase); G2_T1(2); }
+            if (!ptx::mbar_wait(sm.full(stage), phase, abort_flag)) return;
             ptx::tc_fence_after();
-            if (ptx::elect_one()) {
-                const uint64_t da = da0 + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
-                const uint64_t db = db0 + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
-                if (kb < nkb - 1 || ktail == 4) {
-                    ptx::umma_f16_pair_x4(d_tmem, da, db, idesc, kb != 0);
-                } else {
-                    for (int k = 0; k < ktail; ++k)
-                        ptx::umma_f16_pair(d_tmem, da + 2 * k, db + 128 * k, idesc, (kb | k) != 0);
-                }
-                ptx::umma_commit_pair(sm.empty(stage));
-                if (kb == nkb - 1) ptx::umma_commit_pair(sm.tfull(acc));
+            const uint64_t da = da0 + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
+            const uint64_t db = db0 + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
+            if (kb < nkb - 1 || ktail == 4) {
+                ptx::umma_f16_pair_x4(d_tmem, da, db, idesc, kb != 0);
+            } else {
+                for (int k = 0; k < ktail; ++k)
+                    ptx::umma_f16_pair(d_tmem, da + 2 * k, db + 128 * k, idesc, (kb | k) != 0);
             }
-            __syncwarp();
+            ptx::umma_commit_pair(sm.empty(stage));
+            if (kb == nkb - 1) ptx::umma_commit_pair(sm.tfull(acc));
             if (++stage == G2_STAGES) { stage = 0; phase ^= 1; }
         }
-#ifdef G2_TIMING
-        if (nkb >= 16 && ti.bn == 256) { tacc_[8] += clock64() - tk0_; tacc_[9] += 1; }     // full-width tiles: tempty wait + k-loop
-#endif
         if (++acc == 2) { acc = 0; acc_phase ^= 1; }
     }
-#ifdef G2_TIMING
-    tacc_[3] = clock64() - tstart_;
-#endif
-    G2_TFLUSH(lane == 0);
 }
 
 // ------------------------------------------------------------------------------------------------
 // Epilogue (warps 0..7 of each CTA): C = c_out * acc + beta * I, FP16 stores, fused squared
 // residual || alpha_res A B - I ||_F^2 (the convergence test, C-7). `done(ti)` is called by one
 // thread of the CTA after all of the CTA's stores of the tile have been issued and fenced.
+//
+// TI_MIRROR (symmetric products): only the tiles on and above the diagonal of the tile grid are
+// multiplied; an off-diagonal tile also writes its transpose into the block below the diagonal (lanes of a warp are
+// consecutive rows, so element j of every lane is a run of 32 consecutive FP16 of one row of C^T: one 64-byte store
+// instruction per column) and its residual counts twice.
 // ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void st_mirror(__half* Ct /* &C[col_first][row] */, int ldc, const uint32_t* hp, int ncols) {
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+        if (j < ncols) {
+            const unsigned short v = (unsigned short)((j & 1) ? (hp[j >> 1] >> 16) : (hp[j >> 1] & 0xFFFFu));
+            asm volatile("st.global.b16 [%0], %1;" ::"l"(Ct + (size_t)j * ldc), "h"(v) : "memory");
+        }
+    }
+}
+
 template <typename Eng, typename Done>
 __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base, const Eng& e, __half* base,
-                                            uint32_t rank, int warp, int lane, Done done, const CUtensorMap* maps = nullptr) {
+                                            uint32_t rank, int warp, int lane, Done done, const CUtensorMap* maps, volatile int* abort_flag) {
     int acc = 0; uint32_t acc_phase = 0;
     int q = 0; uint32_t tph = 0;
     const uint32_t tempty0 = ptx::mapa(sm.tempty(0), 0);
     const int quarter = warp & 3, chalf = warp >> 2;
-    G2_TDECL();
+    const int g = quarter >> 1;                                    // row group (64 rows) of the TMA-store path
+    bool stalled = false;
     for (;;) {
-        TileInfo ti;
-        { G2_T0(); ti = g2_take(sm, q, tph, lane == 0); G2_T1(4); }
+        const TileInfo ti = g2_take<true>(sm, q, tph, lane == 0, abort_flag);
         if (++q == G2_NTI) { q = 0; tph ^= 1; }
         if (!ti.valid) break;
         const int n = ti.n, n16 = ti.n16;
         int ldc;
         __half* C = c_ptr(e, base, ti.slot, ti.c_buf, ldc);
-        const bool ident = ti.kind != OP_POW_S && ti.kind != OP_POW_A && ti.kind != OP_DCOLS;   // power-iteration tiles: C = alpha A V, res = ||C||_F^2
+        const bool ident = (ti.valid & TI_PLAIN) == 0;             // plain tiles: C = c_out acc, res = ||alpha_res acc||_F^2 (no identity)
+        const bool mirror = (ti.valid & TI_MIRROR) != 0;
         // full-height tile: the CTA's 128 TMEM lanes are 128 rows, every warp sees all bn columns; half-height tile
         // (M = 128 over the pair): lanes 0-63 and 64-127 are the same 64 rows with the left / right half of the columns
-        const bool hh = (ti.valid & 2) != 0;
+        const bool hh = (ti.valid & TI_HALF) != 0;
         const int rbase = hh ? ti.m0 + 64 * (int)rank + (quarter & 1) * 32 : ti.m0 + 128 * (int)rank + quarter * 32;   // first row of this warp
         const int row = rbase + lane;
         const int col0 = hh ? ti.n0 + (quarter >> 1) * (ti.bn >> 1) : ti.n0;
         const int bn = hh ? ti.bn >> 1 : ti.bn;                        // columns this warp's lanes hold
         const float sa = ti.c_out;
-        { G2_T0(); ptx::mbar_wait_sleepy(sm.tfull(acc), acc_phase); G2_T1(5); }
-        G2_T0();
+        if (!ptx::mbar_wait_sleepy(sm.tfull(acc), acc_phase, abort_flag)) { stalled = true; break; }
         ptx::tc_fence_after();
         float rsum = 0.f, vsum = 0.f;
         uint32_t dep = 0;
-        const bool via_tma = maps != nullptr && ident && !hh;      // full-height square GEMM tiles leave through shared memory and TMA stores
+        const bool symdiag = (ti.valid & TI_SYMDIAG) != 0;         // diagonal tile of a symmetric product
+        const bool via_tma = ident && !hh && !symdiag;             // full-height square GEMM tiles leave through shared memory and TMA stores
         if (via_tma) {
             // C leaves in 64 x 64 boxes: the four warps that hold rows [64 g, 64 g + 64) of the CTA's 128 rows and the two
             // 32-column halves of a box write it into a swizzled staging buffer; one thread hands it to the TMA unit, which
             // writes whole 128-byte lines (the row-per-thread register stores issue one request per 32 bytes and go
             // through the SM's load/store path, which the k-loop's ingest also needs). Two buffers per row group.
-            const int g = quarter >> 1, rbox = ((quarter & 1) << 5) + lane;
+            const int rbox = ((quarter & 1) << 5) + lane;
             const bool issuer = (quarter & 1) == 0 && chalf == 0 && lane == 0;
             const CUtensorMap* map_c = maps + (size_t)ti.slot * NMAP + ti.c_buf;
             const int nbx = (bn + 63) >> 6;
@@ -444,14 +417,15 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                 if (issuer) ptx::bulk_wait_read<1>();              // the store that read this buffer two boxes ago is done with it
                 asm volatile("bar.sync %0, 128;" ::"r"(3 + g) : "memory");
                 float f[32];
+                int ncols = 0;                                     // valid columns of this chunk (warp-uniform)
                 if (c < bn && col0 + c < n16) {
                     uint32_t v[32];
                     ptx::tmem_ld_32x32(tmem_base + acc * 256 + ((uint32_t)(quarter * 32) << 16) + c, v);
                     ptx::tmem_ld_wait();
                     dep ^= v[0];
-                    const bool full = (c + 32 <= bn) && (col0 + c + 32 <= n16);
+                    ncols = min(min(32, bn - c), n16 - (col0 + c));
                     const bool diag = (col0 + c < rbase + 32) && (col0 + c + 32 > rbase);
-                    if (full && !diag) {
+                    if (ncols == 32 && !diag) {
                         if (ti.want_res && row < n16) {
 #pragma unroll
                             for (int j = 0; j < 32; ++j) { const float a = __uint_as_float(v[j]); vsum = fmaf(a, a, vsum); }
@@ -464,7 +438,7 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                             const int col = col0 + c + j;
                             const float a = __uint_as_float(v[j]);
                             const float delta = (col == row && row < n) ? 1.f : 0.f;
-                            const bool in = (c + j < bn && col < n16 && row < n16);
+                            const bool in = (j < ncols && row < n16);
                             const float d = in ? ti.alpha_res * a - delta : 0.f;      // pad rows / columns give exactly 0
                             rsum = fmaf(d, d, rsum);
                             f[j] = in ? ti.c_out * a + ti.beta * delta : 0.f;
@@ -474,7 +448,11 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
 #pragma unroll
                     for (int j = 0; j < 32; ++j) f[j] = 0.f;
                 }
-                ptx::st_box_row(box, rbox, chalf << 2, f);
+                uint32_t hp[16];
+#pragma unroll
+                for (int j = 0; j < 16; ++j) { __half2 h = __floats2half2_rn(f[2 * j], f[2 * j + 1]); hp[j] = *reinterpret_cast<uint32_t*>(&h); }
+                ptx::st_box_row(box, rbox, chalf << 2, hp);
+                if (mirror && ncols > 0 && row < n16) st_mirror(C + (size_t)(col0 + c) * ldc + row, ldc, hp, ncols);
                 ptx::fence_proxy_async_smem();
                 asm volatile("bar.sync %0, 128;" ::"r"(3 + g) : "memory");
                 if (issuer) {
@@ -484,6 +462,7 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                 }
             }
             ptx::tc_fence_before();
+            if (mirror) ptx::fence_proxy_async();                  // the transposed block was written with generic stores, read next by TMA
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive_cluster_relaxed(tempty0 + 8u * acc, dep);     // the accumulator is free
             if (issuer) ptx::bulk_wait<0>();                       // the boxes of this tile are in global memory
@@ -494,7 +473,7 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
             ptx::tmem_ld_32x32(tmem_base + acc * 256 + ((uint32_t)(quarter * 32) << 16) + c, v);
             ptx::tmem_ld_wait();
             dep ^= v[0];
-            if (ti.kind == OP_DCOLS) {                             // P[row, 0..31] = acc, FP32 (a6: D columns are formed from FP32)
+            if (ti.valid & TI_F32OUT) {                            // P[row, 0..31] = acc, FP32 (a6: D columns are formed from FP32)
                 if (c == 0 && row < n16) {
                     float4* prow = reinterpret_cast<float4*>(pcols_ptr(e, ti.slot) + (size_t)row * PCW);
 #pragma unroll
@@ -503,37 +482,59 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                 }
                 continue;
             }
-            __half* crow = C + (size_t)row * ldc + col0 + c;
-            const bool full = (c + 32 <= bn) && (col0 + c + 32 <= n16);
-            const bool diag = (col0 + c < rbase + 32) && (col0 + c + 32 > rbase);
-            if (full && !diag) {
+            const int gc0 = col0 + c;                              // first column of this chunk
+            __half* crow = C + (size_t)row * ldc + gc0;
+            const int cw = min(min(32, bn - c), n16 - gc0);        // 16 or 32 valid columns (warp-uniform)
+            const bool diag = (gc0 < rbase + 32) && (gc0 + 32 > rbase);
+            float f[32];
+            if (cw == 32 && !diag) {
                 // interior chunk: C = (sgn alpha) acc, residual term alpha^2 acc^2 (no identity entries here)
                 if (row < n16) {
-                    float f[32];
 #pragma unroll
                     for (int j = 0; j < 32; ++j) {
                         const float a = __uint_as_float(v[j]);
                         vsum = fmaf(a, a, vsum);
                         f[j] = sa * a;
                     }
-#pragma unroll
-                    for (int j = 0; j < 32; j += 16) st_half16(crow + j, f + j);
                 }
             } else if (row < n16) {
-                float f[32];
 #pragma unroll
                 for (int j = 0; j < 32; ++j) {
-                    const int col = col0 + c + j;
+                    const int col = gc0 + j;
                     const float a = __uint_as_float(v[j]);
                     const float delta = (col == row && row < n && ident) ? 1.f : 0.f;
-                    const float d = (c + j < bn && col < n16) ? ti.alpha_res * a - delta : 0.f;   // pad rows / columns give exactly 0
+                    const float d = j < cw ? ti.alpha_res * a - delta : 0.f;   // pad rows / columns give exactly 0
                     rsum = fmaf(d, d, rsum);
                     f[j] = ti.c_out * a + ti.beta * delta;
                 }
-                const int cw = min(min(32, bn - c), n16 - (col0 + c));   // 16 or 32 valid columns
+            }
+            if (row < n16) {
+                if (!symdiag) {
 #pragma unroll
-                for (int j = 0; j < 32; j += 16)
-                    if (j < cw) st_half16(crow + j, f + j);
+                    for (int j = 0; j < 32; j += 16)
+                        if (j < cw) st_half16(crow + j, f + j);
+                } else if (gc0 >= rbase + 32) {
+                    // diagonal tile of a symmetric product, chunk above the diagonal: stored and mirrored; the chunks below
+                    // the diagonal are not stored (their mirror images are), so the stored matrix is exactly symmetric
+                    uint32_t hp[16];
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) { __half2 h = __floats2half2_rn(f[2 * j], f[2 * j + 1]); hp[j] = *reinterpret_cast<uint32_t*>(&h); }
+#pragma unroll
+                    for (int j = 0; j < 32; j += 16)
+                        if (j < cw) st_half16(crow + j, f + j);
+                    st_mirror(C + (size_t)gc0 * ldc + row, ldc, hp, cw);
+                } else if (gc0 + 32 > rbase) {
+                    // chunk that holds diagonal elements: element by element, upper triangle stored and mirrored
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        const int col = gc0 + j;
+                        if (j < cw && col >= row) {
+                            const __half h = __float2half_rn(f[j]);
+                            crow[j] = h;
+                            if (col > row) C[(size_t)col * ldc + row] = h;
+                        }
+                    }
+                }
             }
         }
         if (!via_tma) {
@@ -544,68 +545,21 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
         }
         if (ti.want_res) {
             rsum = fmaf(ti.alpha_res * ti.alpha_res, vsum, rsum);
+            if (mirror) rsum *= 2.f;
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) rsum += __shfl_xor_sync(0xffffffffu, rsum, o);
             if (lane == 0 && rsum != 0.f) atomicAdd(&e.slots[ti.slot].res_acc, rsum);
         }
         asm volatile("bar.sync 1, %0;" ::"n"(G2_EPI_WARPS * 32) : "memory");   // the CTA's epilogue warps
-        G2_T1(6);
         if (warp == 0 && lane == 0) done(ti);
-        G2_T1(7);
         if (++acc == 2) { acc = 0; acc_phase ^= 1; }
     }
-    G2_TFLUSH(warp == 0 && lane == 0);
-}
-
-// ================================================================================================
-// Round engine: one launch serves the op table `launch` of the running round; pair p walks the tile
-// list with stride #pairs.
-// ================================================================================================
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(G2_CTRL_THREADS, 1)
-gemm2_round_kernel(const __grid_constant__ UmmaArgs args) {
-    extern __shared__ uint8_t smem_raw[];
-    const Engine& e = args.e;
-    const SlotOp* ops = e.ops + args.launch * e.S;
-    const int ntiles = e.ntiles[args.launch];
-    G2Smem sm;
-    sm.base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t rank = ptx::cluster_ctarank();
-    const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
-    if (pair >= ntiles) return;                                   // whole cluster idle (uniform per pair)
-
-    const uint32_t tmem_base = g2_setup(sm, warp, lane);
-
-    if (warp < G2_EPI_WARPS) {
-        g2_epilogue(sm, tmem_base, e, args.base, rank, warp, lane, [&](const TileInfo& ti) {
-            SlotOp op = ops[ti.slot];
-            op.ntiles = ti.nreports;
-            tile_finished(e, ti.slot, op);
-        });
-    } else if (warp == G2_WARP_SCHED) {
-        if (rank == 0) {
-            int tile = pair;
-            g2_scheduler(sm, lane, [&](TileInfo& ti) {
-                if (tile >= ntiles) return false;
-                const int slot = find_slot(ops, e.S, tile);
-                const SlotOp op = ops[slot];
-                const Slot& sl = e.slots[slot];
-                const int t = tile - op.tile_start;
-                const int tm = t / sl.ntn, tn = t - tm * sl.ntn;
-                ti.slot = slot; ti.m0 = tm * BM; ti.n0 = tn * BN;
-                ti.n = sl.n; ti.n16 = sl.n16; ti.bn = min(BN, sl.n16 - tn * BN); ti.nreports = 2 * op.ntiles;
-                ti.a_buf = op.a_buf; ti.b_buf = op.b_buf; ti.c_buf = op.c_buf; ti.want_res = op.want_res;
-                ti.c_out = op.sgn * op.alpha; ti.alpha_res = op.alpha; ti.beta = op.beta; ti.kind = op.kind;
-                tile += npairs;
-                return true;
-            });
-        }
-    } else if (warp == G2_WARP_TMA) {
-        g2_producer(sm, args.maps, rank, lane);
-    } else if (warp == G2_WARP_MMA) {
-        if (rank == 0) g2_mma(sm, tmem_base, lane);
+    if (stalled) {
+        // a warp that gives up on a stalled wait releases the named barriers its peers may be waiting at (they stall and
+        // leave at their next wait)
+        asm volatile("bar.arrive %0, 128;" ::"r"(3 + g) : "memory");
+        asm volatile("bar.arrive 1, %0;" ::"n"(G2_EPI_WARPS * 32) : "memory");
     }
-    g2_teardown(tmem_base, warp);
 }
 
 }  // namespace nolsm

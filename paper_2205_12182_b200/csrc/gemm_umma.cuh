@@ -6,8 +6,9 @@
 namespace nolsm {
 
 constexpr int B_BOX_BYTES = BK * 64 * 2;            // one TMA box: 64 (contiguous) x 64 FP16 = 8 KB
-constexpr uint32_t SPIN_LIMIT = 1u << 22;   // a protocol bug traps after seconds instead of hanging the GPU
-constexpr uint32_t SPIN_LIMIT_SLOW = 1u << 26;   // waits that back off with nanosleep: ~10 s
+// Watchdog of every mbarrier wait: a wait that lasts this long is a protocol stall. The waiter raises the engine's
+// abort word (value 2) and leaves its role; the host reports NOLSM_ECUDA (no __trap: the CUDA context stays usable).
+constexpr unsigned long long STALL_NS = 30ull * 1000000000ull;
 
 namespace ptx {
 
@@ -44,13 +45,31 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
         : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
 }
-// Bounded wait: a protocol bug traps (the launch fails with an error) instead of hanging the GPU.
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+// One step of the watchdog (called from the slow path of a wait, every so many polls): returns true when the wait
+// has lasted STALL_NS; the caller then gives up.
+__device__ __forceinline__ bool stalled(unsigned long long& t0, volatile int* abort_flag) {
+    const unsigned long long t = globaltimer_ns();
+    if (!t0) { t0 = t; return false; }
+    if (t - t0 < STALL_NS) return false;
+    atomicExch(const_cast<int*>(abort_flag), 2);
+    return true;
+}
+// Wait on an mbarrier of this CTA. Returns false on a stall (watchdog).
+__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatile int* abort_flag) {
     uint32_t spins = 0;
+    unsigned long long t0 = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if (++spins > 4096u) __nanosleep(64);          // a long wait (kernels of other graph branches share the SM): back off
-        if (spins > SPIN_LIMIT_SLOW) __trap();
+        if (++spins > 4096u) {
+            __nanosleep(64);
+            if ((spins & 4095u) == 0 && stalled(t0, abort_flag)) return false;
+        }
     }
+    return true;
 }
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
     asm volatile(
@@ -119,13 +138,6 @@ __device__ __forceinline__ uint32_t make_idesc_f16(int m, int n) {
     d |= (uint32_t)(m >> 4) << 24;
     return d;
 }
-
-struct UmmaArgs {
-    Engine e;
-    const CUtensorMap* maps;    // [S][NBUF]: cap x cap, row pitch ld, box 64 x 64, SWIZZLE_128B
-    __half* base;               // workspace base
-    int launch;                 // 0 or 1: which op table of the round
-};
 
 __device__ __forceinline__ void st_half8(__half* p, const float* v) {
     __half2 h0 = __floats2half2_rn(v[0], v[1]);

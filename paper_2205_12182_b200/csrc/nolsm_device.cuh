@@ -27,8 +27,9 @@
 
 namespace nolsm {
 
-constexpr int NBUF = 5;          // B0 = S then X(even), B1 = H0 then X(odd), B2/B3 = Y ping-pong, B4 = R / T
-constexpr int NMAP = 8;          // tensor maps per slot: 0-4 the buffers, 5/6 the power-iteration vector blocks, 7 the start block
+constexpr int NBUF = 6;          // Eq. 6 form: B0 = S then X(even), B1 = H0 then X(odd), B2/B3 = Y ping-pong, B4 = R / T, B5 = A0 (several trial mu);
+                                 // Loewdin form: B0 = S, Y, then H0 Z; B1 = H0 then X; B2 = Y then X; B3/B5 = Z ping-pong (the free one keeps Ht0); B4 = T
+constexpr int NMAP = NBUF + 3;   // tensor maps per slot: the buffers, two vector blocks (power iteration, W of the Loewdin D columns), the shared start block
 constexpr int NVC = 16;          // vectors of the block power iteration (one 16-column GEMM tile)
 constexpr int PCW = 32;          // columns of an OP_DCOLS tile: cols(i) = [pos, pos + nb(i)) inside [pos & ~7, (pos & ~7) + 32), TMA boxes start 16-byte aligned
 constexpr int VLD = 64;          // leading dimension of a vector block (one 128-byte row)
@@ -42,7 +43,9 @@ constexpr int ST_NOCONV = 2;     // sign iteration hit max_sign_iters
 
 enum Phase { PH_FREE = 0, PH_NEW, PH_INV, PH_AMAT, PH_PA, PH_SIGN, PH_FIN };
 enum OpKind { OP_NONE = 0, OP_INV_G1, OP_INV_G2, OP_AMAT, OP_SIGN_G1, OP_SIGN_G2, OP_POW_S, OP_POW_A,
-              OP_DCOLS };   // persistent engine: P = X Y[:, cols(i)] as one 16-column tile per 256 rows, FP32 out
+              OP_DCOLS,     // persistent engine: P = X Y[:, cols(i)] as one 32-column tile per 256 rows, FP32 out
+              OP_DCOLS2,    // Loewdin form: P = Z W
+              OP_LW_Y1, OP_LW_G1, OP_LW_G2, OP_LW_G3, OP_LW_HZ, OP_LW_HT };   // coupled Newton-Schulz for S^-1/2 and Ht = Z H0 Z (persist.cuh)
 
 struct __align__(16) Slot {
     // geometry of the atom in the slot (written at refill)

@@ -1,14 +1,23 @@
 // Persistent engine: the whole hot path a1-a7 of one nolsm_density_matrix call in ONE kernel launch.
 //
-// grid = one CTA per SM in clusters of four (two CTA pairs that share the A operand, gemm4sm.cuh); every CTA runs
+// grid = one CTA per SM in clusters of two (one tcgen05 CTA pair per tile, gemm2sm.cuh); every CTA runs
 //   warps 0-10   the grouped tcgen05 GEMM pipeline of gemm2sm.cuh (epilogue x 8, tile scheduler, TMA
 //                producer, MMA issuer), fed from a device-side claim table instead of a static tile list;
 //   warps 11-14  a SIDE GROUP that executes the O(n^2) steps of the path as small tasks: gather
-//                (PAPER.md:L56, L60), the closed-form first Schulz step, and D columns + scatter +
-//                energy (Eq. 4).
-// The spectral scalings (rho(S_sub) for the Schulz start, rho(A_sub) for X0 = A / rho, C-6)
+//                (PAPER.md:L56, L60), the closed-form first iteration steps, diagonal shifts, and D columns +
+//                scatter + energy (Eq. 4).
+// The spectral scalings (rho(S_sub) for the start of the inverse iteration, rho(A_sub) for X0 = A / rho, C-6)
 // come from a BLOCK power iteration with 16 vectors that runs as 256 x 16 GEMM tiles in the same
 // pipeline (V <- alpha M V, Frobenius norm of the product from the fused residual reduction).
+//
+// Two chains of matrix iterations are built on the same machinery (PEngine::lowdin, C-21):
+//   0  Eq. 6 as printed: Y = S^-1 by the Schulz iteration, A = Y H0 - mu I, X <- 1/2 X (3I - X^2), D = 1/2 (I - X) Y.
+//      S, Y and R = 2I - S Y are polynomials of S: symmetric, so the Schulz GEMMs multiply only the tiles on and above
+//      the diagonal (TI_MIRROR, gemm2sm.cuh); A and the sign iterates are not symmetric.
+//   1  the symmetric (Loewdin) form, "other iteration schemes that only require scalings, additions and
+//      multiplications": Z = S^-1/2 by the coupled Newton-Schulz iteration T = 1/2 (3I - Z Y), Y <- Y T, Z <- T Z,
+//      Ht = Z H0 Z - mu I (symmetric), the same Eq. 6 sign iteration on Ht, D = Z 1/2 (I - X) Z. Every iterate is
+//      symmetric: all GEMMs but one (H0 Z) multiply the upper triangle of tiles only.
 //
 // A slot (nolsm_device.cuh) holds one atom submatrix. At any time a slot has at most ONE live piece of
 // work: a GEMM op (claim word gclaim[slot] = tiles << 20 | next tile) or a side task (sclaim[slot] =
@@ -19,12 +28,12 @@
 // iterates of the active slots stay resident in L2 from one GEMM to the next. The host launches the
 // kernel once and waits.
 //
-// Cross-CTA data flow: GEMM outputs are written with generic stores and read back by TMA (async proxy)
-// of other CTAs: writers fence (fence.proxy.async, __threadfence) before the completing atomic; readers
+// Cross-CTA data flow: GEMM outputs are written with generic stores or TMA stores and read back by TMA (async proxy)
+// of other CTAs: writers fence (fence.proxy.async, __threadfence / bulk wait) before the completing atomic; readers
 // fence.proxy.async after the claim. Slot state is read and written with .cg accesses (L1 is not
 // coherent across SMs).
 #pragma once
-#include "gemm4sm.cuh"
+#include "gemm2sm.cuh"
 #include "kernels.cuh"
 
 namespace nolsm {
@@ -35,9 +44,13 @@ constexpr int P_THREADS = G2_CTRL_THREADS + P_SIDE_THREADS;
 constexpr int P_SIDE_SMEM = 60 * 1024;
 constexpr int P_SMEM_BYTES = G2_SMEM_BYTES + P_SIDE_SMEM;
 constexpr int P_MAX_CAP = 4096;
-constexpr int P_GATHER_ROWATOMS = 4;            // row-atoms of N(i) per gather chunk (at most)
+constexpr int P_MAX_MU = 8;                     // trial chemical potentials per call (nolsm_electron_counts)
 
-enum SideKind { SK_NONE = 0, SK_REFILL, SK_GATHER, SK_SCHULZ1, SK_DCOLS };
+enum SideKind { SK_NONE = 0, SK_REFILL, SK_GATHER, SK_ELEM, SK_DCOLS, SK_WCOLS };
+// elementwise side task SK_ELEM: dst = d I - sc src (PSlot::elem_kind says which)
+enum ElemKind { EL_SCHULZ1 = 0,   // Y1 = (2/rho) I - S / rho^2                 (first Schulz step, C-8)
+                EL_LW1,           // T0 = Z1 = 3/2 I - S / (2 rho)               (first coupled Newton-Schulz step, C-21)
+                EL_SHIFT };       // X0 buffer = A0 - mu_j I                     (next trial mu on the resident A0, C-20)
 
 // counters written by the kernel (unsigned long long each)
 enum { PC_TILES = 0, PC_SCHED_IDLE_NS, PC_SCHED_BUSY_NS, PC_OVERSHOOT, PC_T_START, PC_T_END,
@@ -46,15 +59,23 @@ enum { PC_TILES = 0, PC_SCHED_IDLE_NS, PC_SCHED_BUSY_NS, PC_OVERSHOOT, PC_T_STAR
        PC_SIDE_TASKS = PC_SIDE_BYTES + 8,
        PC_LEN = PC_SIDE_TASKS + 8 };
 
-struct __align__(16) PSlot {      // 160 bytes
-    int atom, n, n16, pos, nbi, ntm, ntn, nset;                     // geometry (written at refill)
+constexpr int OPF_RES = 1;        // op flags: fused residual wanted
+constexpr int OPF_SYM = 2;        // symmetric product: upper-triangle tiles, mirrored stores
+constexpr int OPF_NARROW = 4;     // one narrow tile per row block (power iteration, D columns)
+
+struct __align__(16) PSlot {      // 176 bytes
+    int atom, n, n16, pos;                                          // geometry (written at refill; atom / pos / nbi describe member mptr)
+    int nbi, ntm, nset, unit;
     int op_kind, a_buf, b_buf, c_buf;                               // live GEMM op: C = c_out A B + beta I, residual of alpha_res A B
-    float c_out, alpha_res, beta; int want_res;
-    int inv_iters, sign_iters, conv, xcur, ycur, status, gemm_count, tiles_done;
-    float res_acc, res_prev, res_last, rho_s, rho_a, alpha1, alpha2; int side_done;
+    float c_out, alpha_res, beta; int op_flags;
+    int inv_iters, sign_iters, conv, xcur;
+    int ycur, status, gemm_count, tiles_done;
+    float res_acc, res_prev, res_last, rho_s;
+    float rho_a, alpha1, alpha2; int side_done;
     int pow_step; float pow_norm2, pow_alpha; int resume;           // block power iteration state; resume: which token phase comes next
-    int noboost, unit, mptr, mend;                                  // noboost: the scaled steps are over for this matrix; unit and its members
-                                                                    // [mptr, mend) still to be served (atom / pos / nbi describe member mptr)
+    int noboost, mptr, mend, zcur;                                  // noboost: the scaled steps are over for this matrix; members [mptr, mend) still to be served
+    int xsum, pow_buf, mu_idx, sym_count;                           // X ping-pong: next = xsum - xcur; buffer of the running power iteration; trial mu; symmetric GEMMs run
+    int elem_kind, abuf, pad0, pad1;                                // SK_ELEM variant; buffer that keeps the mu-independent A0 (several trial mu)
 };
 
 struct PEngine {
@@ -63,28 +84,27 @@ struct PEngine {
     unsigned int* sclaim;         // [S] side-task claim words
     int S, cap, ld;
     long long bufsz, slotsz;
-    float tol_inv, tol_sign, mu, safety_s, safety_a;
+    float tol_inv, tol_sign, safety_s, safety_a;
     int max_inv, max_sign, p_s, p_a;
-    int gather_rowatoms, schulz_chunks, dcols_chunks;   // row-atoms of N(i) per gather chunk; chunks of the other tasks
+    int gather_rowatoms, elem_chunks, dcols_chunks;   // row-atoms of N(i) per gather chunk; chunks of the other tasks
     int* next_atom; int a_end, total;                 // feed position, its end, units of this call
     const int* feed;              // feed position -> unit id (nullptr: the position is the unit id)
     int atom_lo, atom_hi;         // only members inside [atom_lo, atom_hi) get their columns of D (nolsm_density_matrix_range)
     int* finished;
-    int* heavy;                   // [1] slots inside the GEMM-heavy phases INV .. SIGN right now (at most g_max)
-    int* parked;                  // [S] 1 = the slot finished its first Schulz step and waits for a heavy token
-    int g_max, want_lead, dbg;
-    int tma_store;                // 1: square GEMM tiles leave through shared-memory boxes and TMA stores
-    int split_tokens;             // 1: the heavy token is returned for the rho(A) power iteration and taken again for the sign phase
-    int gather_prefetch;          // 1: the gather task prefetches a row-atom's source blocks into L2 before staging them
-    int half_tiles;               // 1: half-height (M = 128) tiles for a last row block of at most 128 rows
-    int tile_n;                   // columns of a pair tile (256; 128 halves a GEMM's latency at more L2 traffic per FLOP)
-    const signed char* die_of_sm; // [256] L2 die of every SM (0 / 1), or all -1: no die affinity (see k_die_probe)
-    int ndie;                     // 2: slot s is served only by SMs of die s & 1 and heavy tokens are per die; 1: no affinity
-    int ctas;                     // CTAs per cluster of the running kernel: 2 (pair tiles, gemm2sm.cuh) or 4 (A shared by two pairs, gemm4sm.cuh)
+    int* heavy;                   // [1] slots inside the GEMM-heavy phases right now (at most g_max)
+    int* parked;                  // [S] 1 = the slot is ready for a heavy phase and waits for a token
+    int g_max, want_lead;
+    int lowdin;                   // 0: Eq. 6 on A = S^-1 H0 - mu I; 1: symmetric (Loewdin) form
+    int sym_tiles;                // 1: symmetric products multiply the upper triangle of tiles only
+    int n_mu; float mu[P_MAX_MU]; // trial chemical potentials of this call (1 for nolsm_density_matrix)
+    int count_only;               // 1: D is not written, only e and q per trial mu (nolsm_electron_counts)
+    double* nelec_mu;             // [P_MAX_MU] sum_i q_i per trial mu (count_only)
+    double* e_mu;                 // [P_MAX_MU] sum_i e_i per trial mu (count_only)
     int n_sched; float alpha_sched[16];   // scaled Newton-Schulz: alpha_k of sign iteration k < n_sched (1 afterwards)
-    volatile int* abort_flag;     // device word; the host sets it (copy on another stream) to stop a kernel that overran its time limit
+    volatile int* abort_flag;     // device word; 1: the host stops a kernel that overran its time limit, 2: a wait stalled (watchdog)
     unsigned long long* ctr;      // [PC_LEN]
     AtomArrays at;                // results are indexed by unit
+    int* gsym;                    // [n_units] symmetric GEMMs run for the unit
     const int* udim;              // [n_units] dimension of the unit's matrix
     const int* upos;              // [n_atoms] first column of atom i inside its unit's matrix
     const int* adim;              // [n_atoms] dim N(i): rows of D written for atom i
@@ -102,7 +122,7 @@ __device__ __forceinline__ long long buf_off(const PEngine& e, int slot, int buf
     return (long long)slot * e.slotsz + (long long)buf * e.bufsz;
 }
 // Buffers 0..NBUF-1: the slot's square buffers (leading dimension ld). Buffers NBUF, NBUF+1: the slot's
-// two vector blocks (cap x VLD, the first NVC columns are used); they follow the S slots in the workspace.
+// two vector blocks (cap x VLD); they follow the S slots in the workspace.
 __device__ __forceinline__ __half* c_ptr(const PEngine& e, __half* base, int slot, int buf, int& ldc) {
     if (buf < NBUF) { ldc = e.ld; return base + buf_off(e, slot, buf); }
     ldc = VLD;
@@ -111,56 +131,9 @@ __device__ __forceinline__ __half* c_ptr(const PEngine& e, __half* base, int slo
 
 __device__ __forceinline__ float* pcols_ptr(const PEngine& e, int slot) { return e.pcols + (size_t)slot * e.cap * PCW; }
 
-// L2 die of the SM this CTA runs on (-1: no affinity). B200 is two dies, each with half of the SMs and half of
-// L2; a line that SMs of both dies read is kept in both halves, so iterates shared across dies see only half of
-// the 126 MB. With affinity a slot's buffers are touched by the SMs of one die only.
-__device__ __forceinline__ int p_my_die(const PEngine& e) {
-    if (e.ndie != 2) return -1;
-    unsigned smid;
-    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-    return (int)e.die_of_sm[smid & 255u];
-}
-
-// Die probe: every CTA times dependent L2-hit loads (ld.global.cg chain) of NPROBE lines that lie 2 KB apart and
-// records the best time per (SM, line). A line is homed in one die; the SMs of that die see it ~25 cycles sooner.
-// The host turns the per-line near / far pattern into the SM -> die table.
-constexpr int NPROBE = 16;
-__global__ void __launch_bounds__(32) k_die_probe(const unsigned long long* lines, unsigned int* best /*[256][NPROBE]*/) {
-    if (threadIdx.x != 0) return;
-    unsigned smid;
-    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-    for (int l = 0; l < NPROBE; ++l) {
-        const unsigned long long* p = lines + (size_t)l * 256;       // 2 KB apart
-        unsigned long long v = 0;
-        for (int i = 0; i < 8; ++i) asm volatile("ld.global.cg.u64 %0, [%1];" : "=l"(v) : "l"(p + v) : "memory");   // warm (lines hold 0)
-        const long long t0 = clock64();
-        for (int i = 0; i < 64; ++i) asm volatile("ld.global.cg.u64 %0, [%1];" : "=l"(v) : "l"(p + v) : "memory");
-        const long long t1 = clock64();
-        atomicMin(&best[(smid & 255u) * NPROBE + l], (unsigned)((t1 - t0) + (long long)v));
-    }
-}
-
 namespace pl {
-__device__ __forceinline__ unsigned long long gtime() {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
+__device__ __forceinline__ unsigned long long gtime() { return ptx::globaltimer_ns(); }
 __device__ __forceinline__ void side_sync() { asm volatile("bar.sync 2, %0;" ::"n"(P_SIDE_THREADS) : "memory"); }
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-__device__ __forceinline__ float dot8(const uint4& m, const float4& x0, const float4& x1) {
-    const __half2* h = reinterpret_cast<const __half2*>(&m);
-    const float2 a = __half22float2(h[0]), b = __half22float2(h[1]), c = __half22float2(h[2]), d = __half22float2(h[3]);
-    float s = a.x * x0.x;
-    s = fmaf(a.y, x0.y, s); s = fmaf(b.x, x0.z, s); s = fmaf(b.y, x0.w, s);
-    s = fmaf(c.x, x1.x, s); s = fmaf(c.y, x1.y, s); s = fmaf(d.x, x1.z, s); s = fmaf(d.y, x1.w, s);
-    return s;
-}
 }  // namespace pl
 
 // ------------------------------------------------------------------------------------------------
@@ -170,100 +143,137 @@ __device__ __forceinline__ void p_install_side(const PEngine& e, int slot, int k
     __threadfence();
     *(volatile unsigned int*)&e.sclaim[slot] = ((unsigned)kind << 28) | ((unsigned)chunks << 14);
 }
+__device__ __forceinline__ void p_install_elem(const PEngine& e, int slot, int elem_kind) {
+    __stcg(&e.slots[slot].elem_kind, elem_kind);
+    p_install_side(e, slot, SK_ELEM, e.elem_chunks);
+}
 
 // Scaling alpha_k of sign iteration k (C-6b): X_{k+1} = 1/2 (alpha X_k)(3I - (alpha X_k)^2).
 __device__ __forceinline__ float p_sign_alpha(const PEngine& e, const PSlot* s, int k) {
     return (k < e.n_sched && !__ldcg(&s->noboost)) ? e.alpha_sched[k] : 1.f;
 }
 
+__device__ __forceinline__ int p_tiles_of(const PEngine& e, int ntm, int flags) {
+    if (flags & OPF_NARROW) return ntm;
+    if ((flags & OPF_SYM) && e.sym_tiles) return ntm * (ntm + 1) / 2;
+    return ntm * ntm;
+}
+
 __device__ __forceinline__ void p_install_gemm(const PEngine& e, int slot, int kind) {
     PSlot* s = &e.slots[slot];
-    const int xcur = __ldcg(&s->xcur), ycur = __ldcg(&s->ycur);
+    const int xcur = __ldcg(&s->xcur), ycur = __ldcg(&s->ycur), zcur = __ldcg(&s->zcur), xnext = __ldcg(&s->xsum) - xcur;
     const int k = __ldcg(&s->sign_iters);
     const bool first = k == 0;
-    int a = 0, b = 0, c = 0, want = 0;
+    const int symx = e.lowdin ? OPF_SYM : 0;                                                       // the sign iterates are symmetric in the Loewdin form only
+    int a = 0, b = 0, c = 0, flags = 0;
     float c_out = 1.f, alpha_res = 1.f, beta = 0.f;
     switch (kind) {
-        case OP_INV_G1: a = 0; b = ycur; c = 4; c_out = -1.f; beta = 2.f; want = 1; break;       // R = 2I - S Y
-        case OP_INV_G2: a = ycur; b = 4; c = 5 - ycur; break;                                       // Y <- Y R
-        case OP_AMAT: a = ycur; b = 1; c = 0; beta = -e.mu; break;                                  // A = Y H0 - mu I
+        case OP_INV_G1: a = 0; b = ycur; c = 4; c_out = -1.f; beta = 2.f; flags = OPF_RES | OPF_SYM; break;     // R = 2I - S Y
+        case OP_INV_G2: a = ycur; b = 4; c = 5 - ycur; flags = OPF_SYM; break;                                   // Y <- Y R
+        case OP_AMAT:                                                                                            // A = Y H0 - mu I (A0 = Y H0 with several trial mu)
+            a = ycur; b = 1;
+            if (e.n_mu > 1) { c = 5; __stcg(&s->abuf, 5); } else { c = 0; beta = -e.mu[0]; }
+            break;
         case OP_SIGN_G1: {                                                                          // T = 3I - alpha^2 X^2
             const float al = p_sign_alpha(e, s, k);
             alpha_res = first ? __ldcg(&s->alpha1) : 1.f;                                           // X0 = A / rho is never stored
-            a = xcur; b = xcur; c = 4; c_out = -al * al * alpha_res; beta = 3.f; want = 1;
+            a = xcur; b = xcur; c = 4; c_out = -al * al * alpha_res; beta = 3.f; flags = OPF_RES | symx;
         } break;
         case OP_SIGN_G2: {                                                                          // X <- alpha/2 X T
             const float al = p_sign_alpha(e, s, k);
-            a = xcur; b = 4; c = 1 - xcur; c_out = al * (first ? __ldcg(&s->alpha2) : 0.5f);
+            a = xcur; b = 4; c = xnext; c_out = al * (first ? __ldcg(&s->alpha2) : 0.5f); flags = symx;
         } break;
         case OP_POW_S:
         case OP_POW_A: {                                                                            // V <- alpha M V
             const int st = __ldcg(&s->pow_step);
-            a = 0; b = st == 0 ? NMAP - 1 : NBUF + ((st - 1) & 1); c = NBUF + (st & 1);
-            c_out = alpha_res = __ldcg(&s->pow_alpha); want = 1;
+            a = __ldcg(&s->pow_buf); b = st == 0 ? NMAP - 1 : NBUF + ((st - 1) & 1); c = NBUF + (st & 1);
+            c_out = alpha_res = __ldcg(&s->pow_alpha); flags = OPF_RES | OPF_NARROW;
         } break;
-        case OP_DCOLS: a = xcur; b = ycur; c = 0; break;                                           // P = X Y[:, cols(i)]
+        case OP_DCOLS: a = xcur; b = e.lowdin ? zcur : ycur; c = 0; flags = OPF_NARROW; break;      // P = X Y[:, cols(i)]  (Loewdin: X Z[:, cols(i)])
+        case OP_DCOLS2: a = zcur; b = NBUF; c = 0; flags = OPF_NARROW; break;                       // P = Z W, W = 1/2 (Z[:, cols] - X Z[:, cols])
+        // ---- Loewdin form (C-21): Y0 = S / rho, Z0 = I ----
+        case OP_LW_Y1: a = 0; b = 4; c = 2; c_out = 1.f / __ldcg(&s->rho_s); flags = OPF_SYM; break;              // Y1 = Y0 T0
+        case OP_LW_G1: a = zcur; b = ycur; c = 4; c_out = -0.5f; beta = 1.5f; flags = OPF_RES | OPF_SYM; break;   // T = 1/2 (3I - Z Y)
+        case OP_LW_G2: a = ycur; b = 4; c = 2 - ycur; flags = OPF_SYM; break;                                     // Y <- Y T
+        case OP_LW_G3: a = 4; b = zcur; c = 8 - zcur; flags = OPF_SYM; break;                                     // Z <- T Z
+        case OP_LW_HZ: a = 1; b = zcur; c = 0; break;                                                             // M = H0 Z
+        case OP_LW_HT:                                                                                            // Ht = Z M / rho - mu I
+            a = zcur; b = 0; c_out = 1.f / __ldcg(&s->rho_s); flags = OPF_SYM;
+            if (e.n_mu > 1) { c = 8 - zcur; __stcg(&s->abuf, 8 - zcur); } else { c = 2; beta = -e.mu[0]; }
+            break;
         default: break;
     }
     __stcg(reinterpret_cast<int4*>(&s->op_kind), make_int4(kind, a, b, c));
-    __stcg(reinterpret_cast<float4*>(&s->c_out), make_float4(c_out, alpha_res, beta, __int_as_float(want)));
-    const bool pow = kind == OP_POW_S || kind == OP_POW_A || kind == OP_DCOLS;       // one 16-column tile per 256 rows
-    const unsigned long long tiles = (unsigned long long)(__ldcg(&s->ntm) * (pow ? 1 : __ldcg(&s->ntn)));
+    __stcg(reinterpret_cast<float4*>(&s->c_out), make_float4(c_out, alpha_res, beta, __int_as_float(flags)));
+    const unsigned long long tiles = (unsigned long long)p_tiles_of(e, __ldcg(&s->ntm), flags);
     __threadfence();
     *(volatile unsigned long long*)&e.gclaim[slot] = tiles << 20;
 }
 
-// Starts the block power iteration on buffer 0 (S_sub or A_sub): V0 = the shared +-1 start block.
-__device__ __forceinline__ void p_start_power(const PEngine& e, int slot, int kind) {
+// Starts the block power iteration on buffer `buf` (S_sub or the X0 buffer): V0 = the shared +-1 start block.
+__device__ __forceinline__ void p_start_power(const PEngine& e, int slot, int kind, int buf) {
     PSlot* s = &e.slots[slot];
     __stcg(&s->pow_step, 0);
     __stcg(&s->pow_norm2, (float)NVC * (float)__ldcg(&s->n));
     __stcg(&s->pow_alpha, 1.f);
+    __stcg(&s->pow_buf, buf);
     p_install_gemm(e, slot, kind);
 }
 
 // L2 residency: a slot's iterates (X, T, Y: ~3-4 n^2 FP16) are re-read by every GEMM of its chain, so only
-// as many slots as fit in L2 together may be inside the heavy phases (Schulz iterations .. sign iterations)
-// at once. A slot that is ready to enter takes a token or parks; a slot that leaves hands its token to a
-// parked slot (and installs that slot's first GEMM) or returns it.
-// A slot takes a token twice: for the Schulz iterations .. A = S^-1 H0 (resume == 0) and, after the power iteration for
-// rho(A) - nine dependent 16-column tile passes that would hold the token idle - for the sign iterations (resume == 1).
+// as many slots as fit in L2 together may be inside the heavy phases (inverse iterations .. sign iterations)
+// at once. A slot that is ready to enter takes a token or parks; a slot that leaves returns its token and wakes a
+// parked slot if a token is free.
+// A slot takes a token twice: for the inverse iterations .. A (resume == 0) and, after the power iteration for
+// rho(A) - dependent 16-column tile passes that would hold the token idle - for the sign iterations (resume == 1).
 __device__ __forceinline__ void p_enter_heavy_now(const PEngine& e, int slot) {
     PSlot* s = &e.slots[slot];
     if (__ldcg(&s->resume) == 0) {
         __stcg(&s->inv_iters, 1);
-        __stcg(&s->ycur, 2);
-        p_install_gemm(e, slot, OP_INV_G1);
+        if (e.lowdin) { __stcg(&s->ycur, 2); __stcg(&s->zcur, 3); p_install_gemm(e, slot, OP_LW_Y1); }
+        else { __stcg(&s->ycur, 2); p_install_gemm(e, slot, OP_INV_G1); }
     } else {
         p_install_gemm(e, slot, OP_SIGN_G1);
     }
 }
-// With die affinity (ndie == 2) slot s belongs to die s & 1: tokens are counted per die (g_max each).
+// Token count without transient overshoot (a failed atomicAdd-and-undo could make a concurrent waker give up).
+__device__ __forceinline__ bool p_token_acquire(const PEngine& e) {
+    int old = *(volatile int*)e.heavy;
+    while (old < e.g_max) {
+        const int prev = atomicCAS(e.heavy, old, old + 1);
+        if (prev == old) return true;
+        old = prev;
+    }
+    return false;
+}
+// Returns a token, then wakes a parked slot if a token can be taken again. Every release is followed by a scan, and a
+// slot parks BEFORE its last attempt to take a token, so a parked slot is always seen by the release that frees the
+// token it failed to get.
+__device__ __forceinline__ void p_token_release(const PEngine& e) {
+    atomicSub(e.heavy, 1);
+    for (;;) {
+        __threadfence();
+        int found = -1;
+        for (int s = 0; s < e.S; ++s)
+            if (*(volatile int*)&e.parked[s] == 1) { found = s; break; }
+        if (found < 0) return;
+        if (!p_token_acquire(e)) return;              // every token is held: its holder wakes the parked slot when it leaves
+        if (atomicCAS(&e.parked[found], 1, 0) == 1) { __threadfence(); p_enter_heavy_now(e, found); return; }
+        atomicSub(e.heavy, 1);                        // somebody else admitted that slot: give the token back and look again
+    }
+}
 __device__ __forceinline__ void p_enter_heavy(const PEngine& e, int slot) {
-    int* heavy = e.heavy + (e.ndie == 2 ? (slot & 1) : 0);
-    if (atomicAdd(heavy, 1) < e.g_max) { p_enter_heavy_now(e, slot); return; }
-    atomicSub(heavy, 1);
+    if (p_token_acquire(e)) { p_enter_heavy_now(e, slot); return; }
     __threadfence();
     atomicExch(&e.parked[slot], 1);
     __threadfence();
     // a token may have been returned between the failed attempt and the parking: try once more
-    if (atomicAdd(heavy, 1) < e.g_max) {
+    if (p_token_acquire(e)) {
         if (atomicCAS(&e.parked[slot], 1, 0) == 1) { p_enter_heavy_now(e, slot); return; }
-        // a leaving slot admitted this one meanwhile (with its own token)
+        p_token_release(e);                           // a leaving slot admitted this one meanwhile (with its own token)
     }
-    atomicSub(heavy, 1);
 }
-__device__ __forceinline__ void p_leave_heavy(const PEngine& e, int slot) {
-    const int step = e.ndie == 2 ? 2 : 1;
-    for (int s = e.ndie == 2 ? (slot & 1) : 0; s < e.S; s += step) {
-        if (*(volatile int*)&e.parked[s] == 1 && atomicCAS(&e.parked[s], 1, 0) == 1) {
-            __threadfence();
-            p_enter_heavy_now(e, s);          // the token changes hands
-            return;
-        }
-    }
-    atomicSub(e.heavy + (e.ndie == 2 ? (slot & 1) : 0), 1);
-}
+__device__ __forceinline__ void p_leave_heavy(const PEngine& e, int) { p_token_release(e); }
 
 // Takes the next atom of the feed into the slot and installs its gather (phase NEW). Returns false when
 // the feed is exhausted (the slot stays free).
@@ -274,22 +284,21 @@ __device__ __forceinline__ bool p_refill(const PEngine& e, int slot) {
     const int a = e.feed ? e.feed[fpos] : fpos;
     PSlot* s = &e.slots[slot];
     const int n = e.udim[a], n16 = (n + 15) & ~15;
-    int ntm, ntn;
-    choose_tiling(n16, ntm, ntn);
-    if (e.ctas == G4_CTAS) ntn = g4_ntn(n16);                           // cluster tiles per row of tiles
-    else ntn = (n16 + e.tile_n - 1) / e.tile_n;
+    const int ntm = (n16 + BM - 1) / BM;
     const int nset = (int)(e.sv.uset_ptr[a + 1] - e.sv.uset_ptr[a]);
     int m0 = (int)e.sv.unit_ptr[a];
     const int m1 = (int)e.sv.unit_ptr[a + 1];
     while (m0 + 1 < m1 && (e.sv.unit_mem[m0] < e.atom_lo || e.sv.unit_mem[m0] >= e.atom_hi)) ++m0;   // the feed holds units with a member in range
     const int atom = e.sv.unit_mem[m0];
     __stcg(reinterpret_cast<int4*>(&s->atom), make_int4(atom, n, n16, e.upos[atom]));
-    __stcg(reinterpret_cast<int4*>(&s->nbi), make_int4(e.at.nb[atom], ntm, ntn, nset));
+    __stcg(reinterpret_cast<int4*>(&s->nbi), make_int4(e.at.nb[atom], ntm, nset, a));
     __stcg(reinterpret_cast<int4*>(&s->inv_iters), make_int4(0, 0, 0, 0));            // inv, sign, conv, xcur
     __stcg(reinterpret_cast<int4*>(&s->ycur), make_int4(2, 0, 0, 0));                 // ycur, status, gemm_count, tiles_done
     __stcg(reinterpret_cast<float4*>(&s->res_acc), make_float4(0.f, 1e30f, 0.f, 0.f)); // res_acc, res_prev, res_last, rho_s
     __stcg(reinterpret_cast<float4*>(&s->rho_a), make_float4(0.f, 1.f, 0.5f, 0.f));    // rho_a, alpha1, alpha2, side_done
-    __stcg(reinterpret_cast<int4*>(&s->noboost), make_int4(0, a, m0, m1));
+    __stcg(reinterpret_cast<int4*>(&s->noboost), make_int4(0, m0, m1, 3));             // noboost, mptr, mend, zcur
+    __stcg(reinterpret_cast<int4*>(&s->xsum), make_int4(e.lowdin ? 3 : 1, 0, 0, 0));   // xsum, pow_buf, mu_idx, sym_count
+    __stcg(reinterpret_cast<int4*>(&s->elem_kind), make_int4(0, 0, 0, 0));
     __stcg(&s->resume, 0);
     p_install_side(e, slot, SK_GATHER, (nset + e.gather_rowatoms - 1) / e.gather_rowatoms);
     return true;
@@ -301,17 +310,45 @@ __device__ __forceinline__ void p_retire(const PEngine& e, int slot) {
     const int a = __ldcg(&s->unit);
     e.at.inv[a] = __ldcg(&s->inv_iters); e.at.sign[a] = __ldcg(&s->sign_iters); e.at.status[a] = __ldcg(&s->status);
     e.at.gemms[a] = __ldcg(&s->gemm_count); e.at.res[a] = __ldcg(&s->res_last); e.at.rho[a] = __ldcg(&s->rho_a);
+    e.gsym[a] = __ldcg(&s->sym_count);
     const bool more = p_refill(e, slot);
     if (!more) *(volatile unsigned int*)&e.sclaim[slot] = 0u;
     __threadfence();
     atomicAdd(e.finished, 1);
 }
 
+// The sign chain of the slot's current trial mu starts: state of the iteration, then the power iteration for rho on the
+// X0 buffer (buffer 0 in the Eq. 6 form, 2 in the Loewdin form).
+__device__ __forceinline__ void p_begin_sign_chain(const PEngine& e, int slot) {
+    PSlot* s = &e.slots[slot];
+    const int x0 = e.lowdin ? 2 : 0;
+    __stcg(reinterpret_cast<int4*>(&s->inv_iters), make_int4(__ldcg(&s->inv_iters), 0, 0, x0));   // sign_iters, conv, xcur
+    __stcg(&s->noboost, 0);
+    __stcg(&s->res_prev, 1e30f);
+    p_start_power(e, slot, OP_POW_A, x0);
+}
+
 // ------------------------------------------------------------------------------------------------
 // GEMM side: called by one thread per CTA per finished tile (after the CTA's stores and residual
-// atomics). The last report of the op runs the slot's transition (same rules as tile_finished of the
-// round engine: DESIGN.md C-7) and installs what comes next.
+// atomics). The last report of the op runs the slot's transition (C-7) and installs what comes next.
 // ------------------------------------------------------------------------------------------------
+// Convergence rule C-7 on the residual r of an inverse-type (inv) or sign iteration. Returns true when the iteration
+// is over (converged, stagnated at the rounding floor, diverged or capped); sets the status bits.
+__device__ __forceinline__ bool p_converged(const PEngine& e, PSlot* s, bool inv, float r, float rp) {
+    const float tol = inv ? e.tol_inv : e.tol_sign;
+    const int iters = inv ? __ldcg(&s->inv_iters) : __ldcg(&s->sign_iters);
+    const int cap = inv ? e.max_inv : e.max_sign;
+    const bool ok = r < tol;
+    const bool stagnated = (r > 0.5f * rp) && (r < 4.f * tol) && iters > 0;   // rounding floor reached
+    // during the scaled sign steps the bulk of the spectrum is deliberately kept away from +-1, so the
+    // residual need not fall from one step to the next: the divergence rule applies after them
+    const bool scaled_phase = !inv && iters <= e.n_sched && !__ldcg(&s->noboost);
+    const bool diverged = !(r == r) || (!scaled_phase && iters > 1 && r > rp && r > 0.9f);
+    const bool capped = iters + 1 >= cap;
+    if (diverged || (capped && !ok && !stagnated)) __stcg(&s->status, __ldcg(&s->status) | (inv ? ST_NOTSPD : ST_NOCONV));
+    return ok || stagnated || diverged || capped;
+}
+
 __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int nreports) {
     PSlot* s = &e.slots[slot];
     __threadfence();
@@ -320,6 +357,7 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
     __threadfence();
     __stcg(&s->tiles_done, 0);
     const int kind = __ldcg(&s->op_kind);
+    const int flags = __ldcg(&s->op_flags);
     if (kind == OP_POW_S || kind == OP_POW_A) {
         // ||alpha M V_k||_F^2 from the fused reduction; rho estimate = growth of the Frobenius norm
         const float r_new = atomicExch(&s->res_acc, 0.0f);
@@ -335,43 +373,35 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
             p_install_gemm(e, slot, kind);
         } else if (kind == OP_POW_S) {
             __stcg(&s->rho_s, e.safety_s * est);
-            p_install_side(e, slot, SK_SCHULZ1, e.schulz_chunks);
+            p_install_elem(e, slot, e.lowdin ? EL_LW1 : EL_SCHULZ1);
         } else {
             const float rho = e.safety_a * est;
             __stcg(&s->rho_a, rho);
             __stcg(&s->alpha1, 1.f / (rho * rho));
             __stcg(&s->alpha2, 0.5f / rho);
-            if (e.split_tokens) { __stcg(&s->resume, 1); p_enter_heavy(e, slot); }
-            else p_install_gemm(e, slot, OP_SIGN_G1);
+            __stcg(&s->resume, 1);
+            p_enter_heavy(e, slot);
         }
         return;
     }
     if (kind == OP_DCOLS) {                 // a skinny product, not one of the counted square GEMMs
         if (__ldcg(&s->resume) != 2) { __stcg(&s->resume, 2); p_leave_heavy(e, slot); }          // first member served: the chain is over
-        p_install_side(e, slot, SK_DCOLS, e.dcols_chunks);
+        if (e.lowdin) p_install_side(e, slot, SK_WCOLS, 1);
+        else p_install_side(e, slot, SK_DCOLS, e.dcols_chunks);
         return;
     }
-    __stcg(&s->gemm_count, __ldcg(&s->gemm_count) + 1);
-    if (kind == OP_INV_G1 || kind == OP_SIGN_G1) {
-        const bool inv = kind == OP_INV_G1;
+    if (kind == OP_DCOLS2) { p_install_side(e, slot, SK_DCOLS, e.dcols_chunks); return; }
+    if ((flags & OPF_SYM) && e.sym_tiles) __stcg(&s->sym_count, __ldcg(&s->sym_count) + 1);
+    else __stcg(&s->gemm_count, __ldcg(&s->gemm_count) + 1);
+    if (kind == OP_INV_G1 || kind == OP_SIGN_G1 || kind == OP_LW_G1) {
+        const bool inv = kind != OP_SIGN_G1;
         const float sum = atomicExch(&s->res_acc, 0.0f);
         const float r = sqrtf(sum / (float)__ldcg(&s->n));
         const float rp = __ldcg(&s->res_prev);
         __stcg(&s->res_prev, r);
         __stcg(&s->res_last, r);
-        const float tol = inv ? e.tol_inv : e.tol_sign;
-        const int iters = inv ? __ldcg(&s->inv_iters) : __ldcg(&s->sign_iters);
-        const int cap = inv ? e.max_inv : e.max_sign;
-        const bool ok = r < tol;
-        const bool stagnated = (r > 0.5f * rp) && (r < 4.f * tol) && iters > 0;   // rounding floor reached
-        // during the scaled sign steps the bulk of the spectrum is deliberately kept away from +-1, so the
-        // residual need not fall from one step to the next: the divergence rule applies after them
-        const bool scaled_phase = !inv && iters <= e.n_sched && !__ldcg(&s->noboost);
-        const bool diverged = !(r == r) || (!scaled_phase && iters > 1 && r > rp && r > 0.9f);
-        const bool capped = iters + 1 >= cap;
-        if (diverged || (capped && !ok && !stagnated)) __stcg(&s->status, __ldcg(&s->status) | (inv ? ST_NOTSPD : ST_NOCONV));
-        const bool conv = ok || stagnated || diverged || capped;
-        if (!inv && conv && p_sign_alpha(e, s, iters) != 1.f) {
+        const bool conv = p_converged(e, s, inv, r, rp);
+        if (!inv && conv && p_sign_alpha(e, s, __ldcg(&s->sign_iters)) != 1.f) {
             // X_k passed the test, but T was formed with alpha_k != 1 and a scaled step would move the spectrum
             // away from +-1 again: switch the scaling off for this matrix and form T = 3I - X_k^2 once more
             __stcg(&s->noboost, 1);
@@ -380,7 +410,9 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
             return;
         }
         __stcg(&s->conv, conv ? 1 : 0);
-        p_install_gemm(e, slot, inv ? OP_INV_G2 : OP_SIGN_G2);
+        if (kind == OP_INV_G1) p_install_gemm(e, slot, OP_INV_G2);
+        else if (kind == OP_SIGN_G1) p_install_gemm(e, slot, OP_SIGN_G2);
+        else p_install_gemm(e, slot, conv ? OP_LW_G3 : OP_LW_G2);      // the last step needs Z only
     } else if (kind == OP_INV_G2) {
         __stcg(&s->inv_iters, __ldcg(&s->inv_iters) + 1);
         __stcg(&s->ycur, 5 - __ldcg(&s->ycur));
@@ -392,12 +424,31 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
         } else {
             p_install_gemm(e, slot, OP_INV_G1);
         }
-    } else if (kind == OP_AMAT) {
-        if (e.split_tokens) p_leave_heavy(e, slot);              // the token is not held across the power iteration
-        p_start_power(e, slot, OP_POW_A);
+    } else if (kind == OP_LW_Y1) {
+        p_install_gemm(e, slot, OP_LW_G1);
+    } else if (kind == OP_LW_G2) {
+        __stcg(&s->ycur, 2 - __ldcg(&s->ycur));
+        p_install_gemm(e, slot, OP_LW_G3);
+    } else if (kind == OP_LW_G3) {
+        __stcg(&s->inv_iters, __ldcg(&s->inv_iters) + 1);
+        __stcg(&s->zcur, 8 - __ldcg(&s->zcur));
+        if (__ldcg(&s->conv)) {
+            __stcg(&s->conv, 0);
+            __stcg(&s->res_prev, 1e30f);
+            if (__ldcg(&s->status) & ST_NOTSPD) { p_leave_heavy(e, slot); p_retire(e, slot); }
+            else p_install_gemm(e, slot, OP_LW_HZ);
+        } else {
+            p_install_gemm(e, slot, OP_LW_G1);
+        }
+    } else if (kind == OP_LW_HZ) {
+        p_install_gemm(e, slot, OP_LW_HT);
+    } else if (kind == OP_AMAT || kind == OP_LW_HT) {
+        p_leave_heavy(e, slot);                                  // the token is not held across the power iteration
+        if (e.n_mu > 1) p_install_elem(e, slot, EL_SHIFT);      // X0 buffer = A0 - mu_0 I, then the sign chain
+        else p_begin_sign_chain(e, slot);
     } else if (kind == OP_SIGN_G2) {
         __stcg(&s->sign_iters, __ldcg(&s->sign_iters) + 1);
-        __stcg(&s->xcur, 1 - __ldcg(&s->xcur));
+        __stcg(&s->xcur, __ldcg(&s->xsum) - __ldcg(&s->xcur));
         if (__ldcg(&s->conv)) {
             __stcg(&s->conv, 0);
             p_install_gemm(e, slot, OP_DCOLS);
@@ -411,34 +462,34 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
 // Tile scheduler of the persistent engine (leader CTA, one warp): claims tiles from gclaim[] in slot
 // order and publishes them to both CTAs of the pair.
 // ------------------------------------------------------------------------------------------------
-template <int CTAS>
 __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, int lane) {
     int q = 0; uint32_t ph = 0;
     unsigned long long idle_ns = 0, ntiles = 0, overshoot = 0;
     const unsigned long long t_begin = pl::gtime();
-    const int my_die = p_my_die(e);
+    bool stalled = false;
     for (;;) {
-        for (uint32_t spins = 0; !ptx::mbar_try_wait_cluster(sm.ti_empty(q), ph ^ 1);) {
-            __nanosleep(100);
-            if (++spins > (1u << 26)) __trap();
-        }
+        if (!ptx::mbar_wait_cluster_patient(sm.ti_empty(q), ph ^ 1, e.abort_flag)) { stalled = true; break; }
         // Claim lazily: only when the producer has issued every load of the tile before and needs the next
         // record (it runs G2_STAGES k-blocks ahead of the MMA, which hides the claim). A pair that claimed
         // further ahead would hoard tiles of a GEMM that idle pairs could run at the same time, and the
         // slot's chain of dependent GEMMs would take that much longer.
-        for (uint32_t spins = 0; !ptx::mbar_try_wait(sm.want(), (uint32_t)(ntiles & 1) ^ 1u);) {
-            __nanosleep(64);
-            if (++spins > (1u << 28)) __trap();
+        {
+            uint32_t spins = 0; unsigned long long t0 = 0;
+            while (!ptx::mbar_try_wait(sm.want(), (uint32_t)(ntiles & 1) ^ 1u)) {
+                __nanosleep(64);
+                if ((++spins & 4095u) == 0 && ptx::stalled(t0, e.abort_flag)) { stalled = true; break; }
+            }
+            if (stalled) break;
         }
         TileInfo ti{};
-        int got = 0, half_height = 0;
+        int got = 0, tflags = 0;
         unsigned long long t_idle0 = 0;
         for (;;) {
             int found = -1;
             for (int base = 0; base < e.S; base += 32) {
                 const int sidx = base + lane;
                 const unsigned long long w = sidx < e.S ? *(volatile unsigned long long*)&e.gclaim[sidx] : 0ull;
-                const bool avail = (unsigned)(w & 0xFFFFFu) < (unsigned)((w >> 20) & 0xFFFFFu) && (my_die < 0 || (sidx & 1) == my_die);
+                const bool avail = (unsigned)(w & 0xFFFFFu) < (unsigned)((w >> 20) & 0xFFFFFu);
                 const unsigned m = __ballot_sync(0xffffffffu, avail);
                 if (m) { found = base + __ffs(m) - 1; break; }
             }
@@ -446,33 +497,42 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
                 unsigned long long w = 0;
                 if (lane == 0) w = atomicAdd(&e.gclaim[found], 1ull);
                 w = __shfl_sync(0xffffffffu, w, 0);
-                const int t = (int)(w & 0xFFFFFu), nt = (int)((w >> 20) & 0xFFFFFu);
+                int t = (int)(w & 0xFFFFFu);
+                const int nt = (int)((w >> 20) & 0xFFFFFu);
                 if (t < nt) {
                     if (lane == 0) {
                         __threadfence();
                         const PSlot* s = &e.slots[found];
                         const int4 g0 = __ldcg(reinterpret_cast<const int4*>(&s->atom));     // atom n n16 pos
-                        const int4 g1 = __ldcg(reinterpret_cast<const int4*>(&s->nbi));      // nbi ntm ntn nset
+                        const int4 g1 = __ldcg(reinterpret_cast<const int4*>(&s->nbi));      // nbi ntm nset unit
                         const int4 o0 = __ldcg(reinterpret_cast<const int4*>(&s->op_kind));
                         const float4 o1 = __ldcg(reinterpret_cast<const float4*>(&s->c_out));
-                        const bool pow = o0.x == OP_POW_S || o0.x == OP_POW_A || o0.x == OP_DCOLS;
-                        const int ntn = pow ? 1 : g1.z;
-                        const int tm = t / ntn, tn = t - tm * ntn;
-                        ti.slot = found; ti.m0 = tm * BM;
-                        if (o0.x == OP_DCOLS) { ti.n0 = g0.w & ~7; ti.bn = PCW; }          // D columns: the aligned window around pos(i), pair 0 only
-                        else if (pow) { ti.n0 = 0; ti.bn = NVC; }                          // pair 0 only
-                        else if (CTAS == G4_CTAS) {
-                            int n0, bn0, bn1;
-                            g4_cols(g0.z, tn, n0, bn0, bn1);
-                            ti.n0 = n0; ti.bn = bn0 | (bn1 << 16);
+                        const int flags = __float_as_int(o1.w), ntm = g1.y;
+                        ti.slot = found;
+                        tflags = TI_VALID;
+                        if (flags & OPF_NARROW) {
+                            ti.m0 = t * BM;
+                            tflags |= TI_PLAIN;
+                            if (o0.x == OP_DCOLS) { ti.n0 = g0.w & ~7; ti.bn = PCW; tflags |= TI_F32OUT; }   // D columns: the aligned window around pos(i)
+                            else if (o0.x == OP_DCOLS2) { ti.n0 = 0; ti.bn = PCW; tflags |= TI_F32OUT; }      // B operand: the W block
+                            else { ti.n0 = 0; ti.bn = NVC; }                                                  // power iteration
                         } else {
-                            ti.n0 = tn * e.tile_n; ti.bn = min(e.tile_n, g0.z - tn * e.tile_n);
+                            int tm, tn;
+                            if ((flags & OPF_SYM) && e.sym_tiles) {          // tiles on and above the diagonal, row by row
+                                tm = 0;
+                                while (t >= ntm - tm) { t -= ntm - tm; ++tm; }
+                                tn = tm + t;
+                                tflags |= tn > tm ? TI_MIRROR : TI_SYMDIAG;
+                            } else {
+                                tm = t / ntm; tn = t - tm * ntm;
+                            }
+                            ti.m0 = tm * BM; ti.n0 = tn * BN; ti.bn = min(BN, g0.z - tn * BN);
                             // the last row block when at most 128 rows are left: one M = 128 MMA per 16 k instead of M = 256
-                            if (e.half_tiles && g0.z - tm * BM <= BM / 2 && (ti.bn & 31) == 0) half_height = 1;
+                            if (g0.z - tm * BM <= BM / 2 && (ti.bn & 31) == 0) tflags |= TI_HALF;
                         }
-                        ti.n = g0.y; ti.n16 = g0.z; ti.nreports = CTAS * nt;
+                        ti.n = g0.y; ti.n16 = g0.z; ti.nreports = 2 * nt;
                         ti.kind = o0.x; ti.a_buf = o0.y; ti.b_buf = o0.z; ti.c_buf = o0.w;
-                        ti.c_out = o1.x; ti.alpha_res = o1.y; ti.beta = o1.z; ti.want_res = __float_as_int(o1.w);
+                        ti.c_out = o1.x; ti.alpha_res = o1.y; ti.beta = o1.z; ti.want_res = flags & OPF_RES;
                     }
                     got = 1;
                     break;
@@ -486,7 +546,7 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
         }
         if (t_idle0) idle_ns += pl::gtime() - t_idle0;
         ntiles += got;
-        if (lane == 0) ti.valid = got ? (1 | (half_height << 1)) : 0;
+        if (lane == 0) ti.valid = got ? tflags : 0;
         const uint32_t* w = reinterpret_cast<const uint32_t*>(&ti);
         uint32_t mine = 0;
 #pragma unroll
@@ -496,11 +556,11 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
         }
         if (lane < 16) {
 #pragma unroll
-            for (uint32_t rk = 0; rk < (uint32_t)CTAS; ++rk)
+            for (uint32_t rk = 0; rk < 2u; ++rk)
                 ptx::st_cluster_u32(ptx::mapa(sm.tinfo(q), rk) + 4u * lane, mine);
         }
         __syncwarp();
-        if (lane < CTAS) ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_full(q), (uint32_t)lane));
+        if (lane < 2) ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_full(q), (uint32_t)lane));
         if (!got) break;
         if (++q == G2_NTI) { q = 0; ph ^= 1; }
     }
@@ -525,8 +585,8 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
 // rows of T(S) (buffer 0) and T(H0) (buffer 1) that belong to row-atoms [a_lo, a_hi) of N: block (j_a, j_b) of the sparse matrix where it exists,
 // zeros elsewhere and in the pad strip [n, n16). The last chunk also zeroes rows [n, n16).
 //
-// Data path: the source blocks of a row-atom are contiguous runs of nb(j_a) x nb(j_b) values. All of them (S and H0) are
-// prefetched into L2 first; every warp then loads G_NB blocks at a time with coalesced 8-byte loads, converts each value
+// Data path: the source blocks of a row-atom are contiguous runs of nb(j_a) x nb(j_b) values. Every warp loads G_NB blocks
+// at a time with coalesced 8-byte loads, converts each value
 // once (RN-even, C-13) into a shared-memory strip of the dense rows, and the strip leaves with 16-byte
 // coalesced stores. Strips are G_STRIP_BYTES at most, so a row-atom of a very wide submatrix takes several passes over
 // row sub-ranges of its blocks.
@@ -536,7 +596,7 @@ constexpr int G_NB = 2;                           // blocks a warp has in flight
 template <typename TV>
 __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_vals, const TV* __restrict__ H_vals,
                                   __half* __restrict__ dstS, __half* __restrict__ dstH, int unit, int n, int n16, int ld,
-                                  int chunk, int nchunks, unsigned char* sm, int tid, unsigned long long* bytes, int e_prefetch = 1) {
+                                  int chunk, int nchunks, unsigned char* sm, int tid, unsigned long long* bytes) {
     const long long p0 = sv.uset_ptr[unit];
     const int cnt = (int)(sv.uset_ptr[unit + 1] - p0);
     const int warp = tid >> 5, lane = tid & 31;
@@ -557,12 +617,6 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
     const int vpr = n16 >> 3;                                              // 16-byte vectors per dense row
     unsigned long long nread = 0;
 
-#ifdef NOLSM_TIMING
-    long long tp_[4] = {0, 0, 0, 0}, tq_ = clock64();
-#define GT_(i) do { const long long t_ = clock64(); tp_[i] += t_ - tq_; tq_ = t_; } while (0)
-#else
-#define GT_(i)
-#endif
     for (int a = a_lo; a < a_hi; ++a) {
         const int j = s_nset[a];
         const int nbj = s_off[a + 1] - s_off[a], row0 = s_off[a];
@@ -592,24 +646,6 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
         }
         pl::side_sync();
         const int m = *s_m;
-        // L2 prefetch of every source block of this row-atom (S and H0): the staged loads below can keep only ~24 KB in
-        // flight per side group, a prefetch needs no shared memory, so all but the first stage round find their lines in L2
-        if (e_prefetch) {
-            const int nbmax = s_off[cnt] > 0 ? 32 : 32;            // lines per block: computed per block below
-            (void)nbmax;
-            for (int q = tid; q < m; q += P_SIDE_THREADS) {
-                const int b = s_list[q];
-                const long long bo = s_boff[b];
-                const int bytes_b = nbj * (s_off[b + 1] - s_off[b]) * (int)sizeof(TV);
-                const char* ps = reinterpret_cast<const char*>(S_vals + bo);
-                const char* ph = reinterpret_cast<const char*>(H_vals + bo);
-                for (int o = 0; o < bytes_b + 127; o += 128) {
-                    asm volatile("prefetch.global.L2 [%0];" ::"l"(ps + min(o, bytes_b - 1)));
-                    asm volatile("prefetch.global.L2 [%0];" ::"l"(ph + min(o, bytes_b - 1)));
-                }
-            }
-        }
-        GT_(0);
 #pragma unroll 1
         for (int which = 0; which < 2; ++which) {
             const TV* __restrict__ vals = which ? H_vals : S_vals;
@@ -623,7 +659,6 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
                     for (int q = tid; q < nr * vpr; q += P_SIDE_THREADS) s4[q] = z;
                 }
                 pl::side_sync();
-                GT_(1);
                 // ---- each warp takes G_NB blocks at a time: all their loads are issued (coalesced 8-byte loads, G_NB x 8 per
                 //      lane in flight) before the first value is converted into the strip. (8-byte cp.async staging ran at
                 //      ~8 cycles per element in the load/store unit and made the gather the busiest side task.) ----
@@ -663,7 +698,6 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
                     }
                 }
                 pl::side_sync();
-                GT_(2);
                 // ---- the strip leaves with 16-byte stores ----
                 {
                     const uint4* s4 = reinterpret_cast<const uint4*>(strip);
@@ -673,13 +707,9 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
                     }
                 }
                 pl::side_sync();
-                GT_(3);
             }
         }
     }
-#ifdef NOLSM_TIMING
-    if (tid == 0) for (int i_ = 0; i_ < 4; ++i_) atomicAdd(&g4_timing[12 + i_], (unsigned long long)tp_[i_]);
-#endif
     if (chunk == nchunks - 1) {
         const uint4 z = make_uint4(0, 0, 0, 0);
         for (int idx = tid; idx < (n16 - n) * vpr; idx += P_SIDE_THREADS) {
@@ -694,15 +724,15 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
     }
 }
 
-// First Schulz step in closed form, rows [r_lo, r_hi) of n16: Y1 = (2/rho) I - S / rho^2 inside
-// [0, n)^2, zero in the pad strip (C-8).
-__device__ void side_schulz1_chunk(const __half* __restrict__ S, __half* __restrict__ Y, int n, int n16, int ld, float rho,
-                                   int chunk, int nchunks, int tid) {
+// Elementwise task, rows [r_lo, r_hi) of n16: dst = d I - sc src inside [0, n)^2, zero in the pad strip; dst2 (nullable)
+// receives the same values. First Schulz step Y1 = (2/rho) I - S / rho^2 (C-8), first coupled Newton-Schulz
+// step T0 = Z1 = 3/2 I - S / (2 rho) (C-21), diagonal shift A0 - mu I (C-20).
+__device__ void side_elem_chunk(const __half* __restrict__ src, __half* __restrict__ dst, __half* __restrict__ dst2, int n, int n16, int ld,
+                                float d, float sc, int chunk, int nchunks, int tid) {
     const int r_lo = (int)((long long)n16 * chunk / nchunks), r_hi = (int)((long long)n16 * (chunk + 1) / nchunks);
-    const float d = 2.f / rho, sc = 1.f / (rho * rho);
     const int ppr = n16 >> 3;
     const int total = (r_hi - r_lo) * ppr;
-    constexpr int U = 8;
+    constexpr int U = 4;
 #pragma unroll 1
     for (int idx0 = tid; idx0 < total; idx0 += U * P_SIDE_THREADS) {
         uint4 u[U];
@@ -711,7 +741,7 @@ __device__ void side_schulz1_chunk(const __half* __restrict__ S, __half* __restr
             const int idx = idx0 + q * P_SIDE_THREADS;
             if (idx < total) {
                 const int rl = idx / ppr, p = idx - rl * ppr;
-                u[q] = __ldcg(reinterpret_cast<const uint4*>(S + (long long)(r_lo + rl) * ld + p * 8));
+                u[q] = __ldcg(reinterpret_cast<const uint4*>(src + (long long)(r_lo + rl) * ld + p * 8));
             }
         }
 #pragma unroll
@@ -729,21 +759,38 @@ __device__ void side_schulz1_chunk(const __half* __restrict__ S, __half* __restr
                     const int c = c0 + w;
                     f[w] = (r < n && c < n) ? ((r == c ? d : 0.f) - sc * f[w]) : 0.f;
                 }
-                st_half8(Y + (long long)r * ld + c0, f);
+                st_half8(dst + (long long)r * ld + c0, f);
+                if (dst2) st_half8(dst2 + (long long)r * ld + c0, f);
             }
         }
     }
 }
 
+// Loewdin form, between the two skinny products of a member's D columns: W[r, j] = 1/2 (Z[r, w0 + j] - P[r, j]) for the
+// PCW columns of the aligned window w0 = pos & ~7, FP16 into the slot's first vector block (the B operand of OP_DCOLS2).
+__device__ void side_wcols(const float* __restrict__ P, const __half* __restrict__ Z, __half* __restrict__ W, int n16, int ld, int w0, int tid) {
+    for (int idx = tid; idx < n16 * (PCW / 8); idx += P_SIDE_THREADS) {
+        const int r = idx / (PCW / 8), c0 = (idx - r * (PCW / 8)) * 8;
+        const uint4 z = __ldcg(reinterpret_cast<const uint4*>(Z + (long long)r * ld + w0 + c0));
+        const float4 p0 = __ldcg(reinterpret_cast<const float4*>(P + (size_t)r * PCW + c0));
+        const float4 p1 = __ldcg(reinterpret_cast<const float4*>(P + (size_t)r * PCW + c0 + 4));
+        const __half2* h = reinterpret_cast<const __half2*>(&z);
+        const float2 z0 = __half22float2(h[0]), z1 = __half22float2(h[1]), z2 = __half22float2(h[2]), z3 = __half22float2(h[3]);
+        float f[8] = {0.5f * (z0.x - p0.x), 0.5f * (z0.y - p0.y), 0.5f * (z1.x - p0.z), 0.5f * (z1.y - p0.w),
+                      0.5f * (z2.x - p1.x), 0.5f * (z2.y - p1.y), 0.5f * (z3.x - p1.z), 0.5f * (z3.y - p1.w)};
+        st_half8(W + (long long)r * VLD + c0, f);
+    }
+}
+
 // a6 + a7, one chunk of the values of output row i (slot (i, j) holds (D_ji)^T, C-10):
-// D_sub[r, pos + c] = 1/2 (Y[r, pos + c] - P[r, c]) with P = X Y[:, cols(i)] from the OP_DCOLS tiles, and the
-// energy partial sum <D_ji, H0_ji> in FP64 (Eq. 4). One thread per output value, in output
-// order: the block-CSR arrays (D out, H0 in) are touched with coalesced accesses, the small L2-resident
-// operands (Y columns, P) with scattered ones.
+// D_sub[r, pos + c] = ysc Y[r, pos + c] + psc P[r, c] with P from the skinny tensor tiles (Eq. 6 form: 1/2 (Y - X Y[:, cols]),
+// Loewdin form: Z W / rho_s), and the energy partial sum <D_ji, H0_ji> in FP64 (Eq. 4). One thread per
+// output value, in output order: the block-CSR arrays (D out, H0 in) are touched with coalesced accesses, the small
+// L2-resident operands (Y columns, P) with scattered ones. D_vals == nullptr: only the partial sums (count_only).
 template <typename TV, typename TD>
-__device__ void side_dcols_chunk(const SysView& sv, const float* __restrict__ P, const __half* __restrict__ Y,
-                                 const TV* __restrict__ H_vals, const TV* __restrict__ S_vals, TD* __restrict__ D_vals, double* e_atom,
-                                 double* q_atom, int atom, int n_own, int ld, int pos, int nbi, int chunk, int nchunks, unsigned char* sm, int tid) {
+__device__ void side_dcols_chunk(const SysView& sv, const float* __restrict__ P, const __half* __restrict__ Y, float ysc, float psc,
+                                 const TV* __restrict__ H_vals, const TV* __restrict__ S_vals, TD* __restrict__ D_vals, double* e_acc,
+                                 double* q_acc, int atom, int n_own, int ld, int pos, int nbi, int chunk, int nchunks, unsigned char* sm, int tid) {
     const long long p0 = sv.nset_ptr[atom];
     const int cnt = (int)(sv.nset_ptr[atom + 1] - p0);
     int* s_pre = reinterpret_cast<int*>(sm);                               // [cnt + 1] first value row of each atom of N(i) in output order
@@ -764,15 +811,16 @@ __device__ void side_dcols_chunk(const SysView& sv, const float* __restrict__ P,
         const int c = rem / nbj, bb = rem - c * nbj;
         const int r = s_row[a] + bb;
         const long long o = sv.blk_off[sv.nset_slot[p0 + a]] + rem;       // slot (i, j_a): [c][bb] = D_sub[r, pos + c]
-        const float d = 0.5f * (__half2float(__ldcg(Y + (long long)r * ld + pos + c)) - __ldcg(P + (size_t)r * PCW + (pos & 7) + c));
-        D_vals[o] = (TD)d;
+        float d = psc * __ldcg(P + (size_t)r * PCW + (pos & 7) + c);
+        if (ysc != 0.f) d = fmaf(ysc, __half2float(__ldcg(Y + (long long)r * ld + pos + c)), d);
+        if (D_vals) D_vals[o] = (TD)d;
         e_part += (double)d * (double)H_vals[o];
         q_part += (double)d * (double)S_vals[o];
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) { e_part += __shfl_xor_sync(0xffffffffu, e_part, o); q_part += __shfl_xor_sync(0xffffffffu, q_part, o); }
-    if ((tid & 31) == 0 && e_part != 0.0) atomicAdd(&e_atom[atom], e_part);
-    if ((tid & 31) == 0 && q_part != 0.0) atomicAdd(&q_atom[atom], q_part);
+    if ((tid & 31) == 0 && e_part != 0.0) atomicAdd(e_acc, e_part);
+    if ((tid & 31) == 0 && q_part != 0.0) atomicAdd(q_acc, q_part);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -781,7 +829,6 @@ __device__ void side_dcols_chunk(const SysView& sv, const float* __restrict__ P,
 __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
     __shared__ int s_ctl[4];                      // slot, kind, chunk, nchunks
     const int warp = tid >> 5, lane = tid & 31;
-    const int my_die = p_my_die(e);
     unsigned long long busy_ns[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tasks[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     for (;;) {
         if (warp == 0) {
@@ -791,7 +838,7 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
                 for (int base = 0; base < e.S; base += 32) {
                     const int sidx = base + lane;
                     const unsigned w = sidx < e.S ? *(volatile unsigned int*)&e.sclaim[sidx] : 0u;
-                    const bool avail = (w & 0x3FFFu) < ((w >> 14) & 0x3FFFu) && (my_die < 0 || (sidx & 1) == my_die);
+                    const bool avail = (w & 0x3FFFu) < ((w >> 14) & 0x3FFFu);
                     const unsigned m = __ballot_sync(0xffffffffu, avail);
                     if (m) { found = base + __ffs(m) - 1; break; }
                 }
@@ -815,27 +862,44 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
         const unsigned long long t0 = pl::gtime();
         PSlot* s = &e.slots[slot];
         const int4 g0 = __ldcg(reinterpret_cast<const int4*>(&s->atom));     // atom n n16 pos
-        const int4 g1 = __ldcg(reinterpret_cast<const int4*>(&s->nbi));      // nbi ntm ntn nset
+        const int4 g1 = __ldcg(reinterpret_cast<const int4*>(&s->nbi));      // nbi ntm nset unit
         const int atom = g0.x, n = g0.y, n16 = g0.z, pos = g0.w, nbi = g1.x;
+        const int mu_idx = __ldcg(&s->mu_idx);
         switch (kind) {
             case SK_GATHER: {
                 __half* dS = e.base + buf_off(e, slot, 0);
                 __half* dH = e.base + buf_off(e, slot, 1);
-                if (e.val_f64) side_gather_chunk<double>(e.sv, (const double*)e.S_vals, (const double*)e.H_vals, dS, dH, __ldcg(&s->unit), n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER], e.gather_prefetch);
-                else side_gather_chunk<float>(e.sv, (const float*)e.S_vals, (const float*)e.H_vals, dS, dH, __ldcg(&s->unit), n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER], e.gather_prefetch);
+                if (e.val_f64) side_gather_chunk<double>(e.sv, (const double*)e.S_vals, (const double*)e.H_vals, dS, dH, g1.w, n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER]);
+                else side_gather_chunk<float>(e.sv, (const float*)e.S_vals, (const float*)e.H_vals, dS, dH, g1.w, n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER]);
             } break;
-            case SK_SCHULZ1:
-                side_schulz1_chunk(e.base + buf_off(e, slot, 0), e.base + buf_off(e, slot, 2), n, n16, e.ld, __ldcg(&s->rho_s), chunk, nch, tid);
-                break;
+            case SK_ELEM: {
+                const int ek = __ldcg(&s->elem_kind);
+                const float rho = __ldcg(&s->rho_s);
+                if (ek == EL_SCHULZ1)
+                    side_elem_chunk(e.base + buf_off(e, slot, 0), e.base + buf_off(e, slot, 2), nullptr, n, n16, e.ld, 2.f / rho, 1.f / (rho * rho), chunk, nch, tid);
+                else if (ek == EL_LW1)
+                    side_elem_chunk(e.base + buf_off(e, slot, 0), e.base + buf_off(e, slot, 4), e.base + buf_off(e, slot, 3), n, n16, e.ld, 1.5f, 0.5f / rho, chunk, nch, tid);
+                else
+                    side_elem_chunk(e.base + buf_off(e, slot, __ldcg(&s->abuf)), e.base + buf_off(e, slot, e.lowdin ? 2 : 0), nullptr, n, n16, e.ld, -e.mu[mu_idx], -1.f, chunk, nch, tid);
+            } break;
+            case SK_WCOLS: {
+                int ldw;
+                __half* W = c_ptr(e, e.base, slot, NBUF, ldw);
+                side_wcols(pcols_ptr(e, slot), e.base + buf_off(e, slot, __ldcg(&s->zcur)), W, n16, e.ld, pos & ~7, tid);
+            } break;
             case SK_DCOLS: {
                 const float* P = pcols_ptr(e, slot);
                 const __half* Y = e.base + buf_off(e, slot, __ldcg(&s->ycur));
+                const float ysc = e.lowdin ? 0.f : 0.5f, psc = e.lowdin ? 1.f / __ldcg(&s->rho_s) : -0.5f;
+                double* e_acc = e.count_only ? &e.e_mu[mu_idx] : &e.e_atom[atom];
+                double* q_acc = e.count_only ? &e.nelec_mu[mu_idx] : &e.q_atom[atom];
+                void* Dv = e.count_only ? nullptr : e.D_vals;
                 if (e.val_f64) {
-                    if (e.d_f64) side_dcols_chunk<double, double>(e.sv, P, Y, (const double*)e.H_vals, (const double*)e.S_vals, (double*)e.D_vals, e.e_atom, e.q_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
-                    else side_dcols_chunk<double, float>(e.sv, P, Y, (const double*)e.H_vals, (const double*)e.S_vals, (float*)e.D_vals, e.e_atom, e.q_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
+                    if (e.d_f64) side_dcols_chunk<double, double>(e.sv, P, Y, ysc, psc, (const double*)e.H_vals, (const double*)e.S_vals, (double*)Dv, e_acc, q_acc, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
+                    else side_dcols_chunk<double, float>(e.sv, P, Y, ysc, psc, (const double*)e.H_vals, (const double*)e.S_vals, (float*)Dv, e_acc, q_acc, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
                 } else {
-                    if (e.d_f64) side_dcols_chunk<float, double>(e.sv, P, Y, (const float*)e.H_vals, (const float*)e.S_vals, (double*)e.D_vals, e.e_atom, e.q_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
-                    else side_dcols_chunk<float, float>(e.sv, P, Y, (const float*)e.H_vals, (const float*)e.S_vals, (float*)e.D_vals, e.e_atom, e.q_atom, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
+                    if (e.d_f64) side_dcols_chunk<float, double>(e.sv, P, Y, ysc, psc, (const float*)e.H_vals, (const float*)e.S_vals, (double*)Dv, e_acc, q_acc, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
+                    else side_dcols_chunk<float, float>(e.sv, P, Y, ysc, psc, (const float*)e.H_vals, (const float*)e.S_vals, (float*)Dv, e_acc, q_acc, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
                 }
             } break;
             default: break;                       // SK_REFILL: nothing to compute
@@ -854,17 +918,32 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
                     case SK_REFILL:
                         if (!p_refill(e, slot)) *(volatile unsigned int*)&e.sclaim[slot] = 0u;
                         break;
-                    case SK_GATHER: p_start_power(e, slot, OP_POW_S); break;
-                    case SK_SCHULZ1: p_enter_heavy(e, slot); break;
+                    case SK_GATHER: p_start_power(e, slot, OP_POW_S, 0); break;
+                    case SK_ELEM:
+                        if (__ldcg(&s->elem_kind) == EL_SHIFT) p_begin_sign_chain(e, slot);
+                        else p_enter_heavy(e, slot);
+                        break;
+                    case SK_WCOLS: p_install_gemm(e, slot, OP_DCOLS2); break;
                     case SK_DCOLS: {
                         const double nv = (double)(e.sv.blk_off[e.sv.row_ptr[atom + 1]] - e.sv.blk_off[e.sv.row_ptr[atom]]);
                         atomicAdd(&e.ctr[PC_SIDE_BYTES + SK_DCOLS],
-                                  (unsigned long long)(nv * ((e.d_f64 ? 8 : 4) + (e.val_f64 ? 8 : 4)) + (double)n * PCW * 4.0 + (double)n * nbi * 2.0));
-                        // the next member of the unit takes its columns from the same X and Y, or the slot retires
+                                  (unsigned long long)(nv * ((e.count_only ? 0 : (e.d_f64 ? 8 : 4)) + 2 * (e.val_f64 ? 8 : 4)) + (double)n * PCW * 4.0 + (double)n * nbi * 2.0));
+                        // the next member of the unit takes its columns from the same X and Y; then the next trial mu
+                        // restarts the sign chain on the resident A0; then the slot retires
                         int mp = __ldcg(&s->mptr) + 1;
                         const int mend = __ldcg(&s->mend);
                         while (mp < mend && (e.sv.unit_mem[mp] < e.atom_lo || e.sv.unit_mem[mp] >= e.atom_hi)) ++mp;
-                        if (mp < mend) {
+                        if (mp >= mend && mu_idx + 1 < e.n_mu) {
+                            mp = (int)e.sv.unit_ptr[g1.w];
+                            while (mp + 1 < mend && (e.sv.unit_mem[mp] < e.atom_lo || e.sv.unit_mem[mp] >= e.atom_hi)) ++mp;
+                            const int nxt = e.sv.unit_mem[mp];
+                            __stcg(&s->mptr, mp);
+                            __stcg(&s->atom, nxt);
+                            __stcg(&s->pos, e.upos[nxt]);
+                            __stcg(&s->nbi, e.at.nb[nxt]);
+                            __stcg(&s->mu_idx, mu_idx + 1);
+                            p_install_elem(e, slot, EL_SHIFT);
+                        } else if (mp < mend) {
                             const int nxt = e.sv.unit_mem[mp];
                             __stcg(&s->mptr, mp);
                             __stcg(&s->atom, nxt);
@@ -890,9 +969,7 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
 // ================================================================================================
 // The kernel.
 // ================================================================================================
-// CTAS = CTAs per cluster (set at launch): 2 = pair tiles (gemm2sm.cuh), 4 = two pairs sharing A (gemm4sm.cuh).
-template <int CTAS>
-__global__ void __launch_bounds__(P_THREADS, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(P_THREADS, 1)
 nolsm_persist_kernel(const __grid_constant__ PEngine e) {
     extern __shared__ uint8_t smem_raw[];
     G2Smem sm;
@@ -902,37 +979,46 @@ nolsm_persist_kernel(const __grid_constant__ PEngine e) {
     const uint32_t rank = ptx::cluster_ctarank();
     auto done = [&](const TileInfo& ti) { p_tile_finished(e, ti.slot, ti.nreports); };
 
-    uint32_t tmem_base;
-    if constexpr (CTAS == G4_CTAS) tmem_base = g4_setup(sm, warp, lane);
-    else tmem_base = g2_setup(sm, warp, lane);
+    const uint32_t tmem_base = g2_setup(sm, warp, lane);
 
     if (warp < G2_EPI_WARPS) {
-        if constexpr (CTAS == G4_CTAS) g4_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, done);
-        else g2_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, done, e.tma_store ? e.maps : nullptr);
+        g2_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, done, e.maps, e.abort_flag);
     } else if (warp == G2_WARP_SCHED) {
-        if (rank == 0) p_scheduler<CTAS>(sm, e, lane);
+        if (rank == 0) p_scheduler(sm, e, lane);
     } else if (warp == G2_WARP_TMA) {
-        if constexpr (CTAS == G4_CTAS) g4_producer(sm, e.maps, rank, lane, e.want_lead, e.dbg);
-        else g2_producer(sm, e.maps, rank, lane, e.want_lead);
+        if (lane == 0) g2_producer(sm, e.maps, rank, e.want_lead, e.abort_flag);
     } else if (warp == G2_WARP_MMA) {
-        if constexpr (CTAS == G4_CTAS) { if ((rank & 1u) == 0) g4_mma(sm, tmem_base, rank, lane, e.dbg); }
-        else { if (rank == 0) g2_mma(sm, tmem_base, lane); }
+        if (rank == 0 && lane == 0) g2_mma(sm, tmem_base, e.abort_flag);
     } else {
         p_side_loop(e, side_sm, (int)threadIdx.x - G2_CTRL_THREADS);
     }
     g2_teardown(tmem_base, warp);
 }
 
-// Stand-alone launch of the gather task for one slot (diagnostics: nolsm_gather_submatrix and the
-// HBM-bandwidth measurement of the gather code without the GEMMs). grid = (chunks, slots).
+// Stand-alone launches of the side tasks (diagnostics: nolsm_gather_submatrix, and the HBM-bandwidth measurement of the
+// gather and scatter code without the GEMMs, nolsm_side_task_bandwidth). The same device functions as in the
+// persistent kernel, one side group (128 threads) per CTA.
+// grid = (chunks, units): unit atoms[blockIdx.y] is gathered into slot blockIdx.y % nslots.
 template <typename TV>
 __global__ void __launch_bounds__(P_SIDE_THREADS) k_side_gather(SysView sv, const TV* S_vals, const TV* H_vals, __half* base,
-                                                                long long slotsz, long long bufsz, int ld, const int* atoms,
-                                                                const int* dims, unsigned long long* bytes) {
+                                                                long long slotsz, long long bufsz, int ld, const int* units,
+                                                                const int* dims, int nslots, unsigned long long* bytes) {
     extern __shared__ unsigned char sm_dyn[];
-    const int atom = atoms[blockIdx.y], n = dims[atom], n16 = (n + 15) & ~15;      // unit id and its dimension
-    __half* dS = base + (long long)blockIdx.y * slotsz;
-    side_gather_chunk<TV>(sv, S_vals, H_vals, dS, dS + bufsz, atom, n, n16, ld, blockIdx.x, gridDim.x, sm_dyn, threadIdx.x, bytes);
+    const int unit = units[blockIdx.y], n = dims[unit], n16 = (n + 15) & ~15;
+    __half* dS = base + (long long)(blockIdx.y % nslots) * slotsz;
+    side_gather_chunk<TV>(sv, S_vals, H_vals, dS, dS + bufsz, unit, n, n16, ld, blockIdx.x, gridDim.x, sm_dyn, threadIdx.x, bytes);
+}
+// grid = (chunks, atoms): the scatter task for atom atoms[blockIdx.y] (its own submatrix; P and Y of slot blockIdx.y % nslots).
+template <typename TV, typename TD>
+__global__ void __launch_bounds__(P_SIDE_THREADS) k_side_dcols(SysView sv, const float* pcols, const __half* base, long long slotsz,
+                                                               long long ybuf_off, int cap, int ld, const int* atoms, const int* dims,
+                                                               const int* pos, const int* nb, int nslots, const TV* H_vals,
+                                                               const TV* S_vals, TD* D_vals, double* e_atom, double* q_atom) {
+    extern __shared__ unsigned char sm_dyn[];
+    const int atom = atoms[blockIdx.y], sl = blockIdx.y % nslots;
+    side_dcols_chunk<TV, TD>(sv, pcols + (size_t)sl * cap * PCW, base + (long long)sl * slotsz + ybuf_off, 0.5f, -0.5f, H_vals, S_vals,
+                             D_vals, &e_atom[atom], &q_atom[atom], atom, dims[atom], ld, pos[atom], nb[atom], blockIdx.x, gridDim.x,
+                             sm_dyn, threadIdx.x);
 }
 
 }  // namespace nolsm

@@ -17,6 +17,7 @@ TOL_FP32 = 1e-5
 
 def _nolsm(**kw):
     from paper_2205_12182_b200 import Nolsm
+    kw.setdefault("timeout_s", 90.0)              # a stalled kernel fails the test instead of holding the GPU for minutes
     return Nolsm(0, **kw)
 
 
@@ -102,14 +103,17 @@ def test_cfg0_fp32_mode(cfg0):
     assert abs(E - cmp["e_ref"]) / abs(cmp["e_ref"]) <= TOL_FP32
 
 
-@pytest.mark.parametrize("backend", ["umma", "umma-rounds", "simt"])
+@pytest.mark.parametrize("backend", ["umma", "umma-fulltiles", "lowdin", "lowdin-fulltiles", "simt"])
 def test_cfg0_mixed_mode(cfg0, backend):
-    """umma: tcgen05 GEMMs in the persistent engine (the default path); umma-rounds: the same GEMM
-    pipeline in the round engine; simt: FP16 operands with FFMA GEMMs (round engine)."""
-    from paper_2205_12182_b200 import ENGINE_PERSISTENT, ENGINE_ROUNDS, GEMM_SIMT, GEMM_UMMA
+    """umma: tcgen05 GEMMs in the persistent engine (the default path: Eq. 6 form, the symmetric Schulz products multiply the
+    upper triangle of tiles only); -fulltiles: every tile multiplied; lowdin: the symmetric form (DESIGN.md C-21);
+    simt: FP16 operands with FFMA GEMMs (round engine)."""
+    from paper_2205_12182_b200 import ENGINE_PERSISTENT, GEMM_SIMT, GEMM_UMMA, ITER_LOWDIN
     s = cfg0
     kw = {"umma": dict(gemm_backend=GEMM_UMMA, engine=ENGINE_PERSISTENT),
-          "umma-rounds": dict(gemm_backend=GEMM_UMMA, engine=ENGINE_ROUNDS),
+          "umma-fulltiles": dict(symmetric_tiles=-1),
+          "lowdin": dict(iteration=ITER_LOWDIN),
+          "lowdin-fulltiles": dict(iteration=ITER_LOWDIN, symmetric_tiles=-1),
           "simt": dict(gemm_backend=GEMM_SIMT)}[backend]
     D, E, st, stats = _run(s, **kw)
     cmp = compare_atoms(s, D, st["e_atom"], range(s.n_atoms))
@@ -152,32 +156,23 @@ def test_density_matrix_range_touches_only_its_rows(cfg0):
     assert abs(e - cmp["e_ref"]) / abs(cmp["e_ref"]) <= TOL_MIXED_E
 
 
-@pytest.mark.parametrize("engine", ["persistent", "rounds"])
+@pytest.mark.parametrize("engine", ["persistent", "persistent-fulltiles", "lowdin", "rounds"])
 @pytest.mark.parametrize("name,n_atoms,sample", [("cfg1", 600, 6), ("cfg2", 300, 3), ("cfg3", 1500, 6)])
 def test_small_proxies_mixed(name, n_atoms, sample, engine):
     """Reduced-size versions of configs 1-3 (same density, basis and generator): several tiles per
-    matrix, ragged tails, mixed 5/13 basis for cfg3. Oracle on a seeded sample of atoms."""
-    from paper_2205_12182_b200 import ENGINE_PERSISTENT, ENGINE_ROUNDS
+    matrix (mirrored off-diagonal tiles, ragged tails, half-height corner tiles), mixed 5/13 basis for cfg3. Oracle on a
+    seeded sample of atoms. rounds: the FFMA round engine on FP16 operands."""
+    from paper_2205_12182_b200 import ENGINE_PERSISTENT, ENGINE_ROUNDS, ITER_LOWDIN
     s = make_system(name, n_atoms=n_atoms)
     atoms = np.random.default_rng(1).choice(s.n_atoms, sample, replace=False)
-    D, E, st, stats = _run(s, engine=ENGINE_PERSISTENT if engine == "persistent" else ENGINE_ROUNDS)
+    kw = {"persistent": dict(engine=ENGINE_PERSISTENT), "persistent-fulltiles": dict(symmetric_tiles=-1),
+          "lowdin": dict(iteration=ITER_LOWDIN), "rounds": dict(engine=ENGINE_ROUNDS)}[engine]
+    D, E, st, stats = _run(s, **kw)
     cmp = compare_atoms(s, D, st["e_atom"], atoms)
     print(name, {k: v for k, v in cmp.items() if k != "ref"}, stats)
     assert (st["status"] == 0).all()
     assert cmp["max_abs_dD"] <= TOL_MIXED_D
     assert cmp["rel_dE"] <= TOL_MIXED_E
-
-
-def test_cluster4_engine_matches_oracle():
-    """cluster_ctas = 4: two CTA pairs per 256 x 512 tile with the A operand TMA-multicast between them
-    (gemm4sm.cuh); ragged tails in both tile directions (cfg2 proxy, n ~ 900-1500)."""
-    s = make_system("cfg2", n_atoms=300)
-    atoms = np.random.default_rng(3).choice(s.n_atoms, 3, replace=False)
-    D, E, st, stats = _run(s, cluster_ctas=4)
-    cmp = compare_atoms(s, D, st["e_atom"], atoms)
-    print("cluster4 cfg2@300", {k: v for k, v in cmp.items() if k != "ref"}, stats)
-    assert (st["status"] == 0).all()
-    assert cmp["max_abs_dD"] <= TOL_MIXED_D and cmp["rel_dE"] <= TOL_MIXED_E
 
 
 def test_plain_newton_schulz_matches_scaled():
@@ -388,7 +383,7 @@ def test_find_mu_reaches_the_target_count(cfg0):
         mu, n_mu, evals = ctx.find_mu(target, -7.0, 8.0, D, tol_n=0.05, tol_mu=1e-4)
         E = ctx.energy()
         st = ctx.atom_stats()
-        assert abs(n_mu - target) <= 0.05 and 3 < evals <= 24 and -0.9 < mu < 0.9
+        assert abs(n_mu - target) <= 0.05 and 3 < evals <= 40 and -0.9 < mu < 0.9
         n_ref = orc.electron_count(s.atom_nb, s.row_ptr, s.col_idx, Hn, Sn, mu)
         assert abs(n_ref - n_mu) <= TOL_MIXED_E * target
         s_mu = make_system("cfg0")
@@ -402,9 +397,9 @@ def test_find_mu_reaches_the_target_count(cfg0):
         assert ei.value.code == 1
 
 
-@pytest.mark.parametrize("kw", [dict(combine=1, cluster_ctas=4), dict(combine=2, eps_filter=0.02), dict(combine=1, sign_scaled_iters=-1)])
+@pytest.mark.parametrize("kw", [dict(combine=1, iteration=1), dict(combine=2, eps_filter=0.02), dict(combine=1, sign_scaled_iters=-1)])
 def test_combination_with_other_options(kw):
-    """Combination together with the cluster-of-4 pipeline, with the max-abs block filter (filtered index sets feed the
+    """Combination together with the symmetric (Loewdin) form, with the max-abs block filter (filtered index sets feed the
     grouping) and with plain Eq. 6: groups bit-exact, host float32 output, parity on sampled groups."""
     s = make_system("cfg1", n_atoms=500)
     Hn, Sn = s.fill_np(MAT_H), s.fill_np(MAT_S)

@@ -219,21 +219,40 @@ def dense_from_blocks(atom_nb, row_ptr, col_idx, vals, transpose_blocks=False):
 # ------------------------------------------------------------------------------------------
 # submatrix combination ("one submatrix for multiple columns", Eq. 9 / Eq. 10)
 # ------------------------------------------------------------------------------------------
-def combine_cost(n, mode):
+def perf_rate(perf_table, n):
+    """r(n) of Eq. 10 (L89: "the matrix multiplication performance p(n) of the GPUs is measured for different matrix
+    sizes n and interpolated"): perf_table = (dimensions ascending, rates in integer GFLOP/s); linear interpolation
+    between neighbouring points, constant outside the table, in integers (floor division of non-negative numbers)."""
+    tn, tr = perf_table
+    n = int(n)
+    if n <= tn[0]:
+        return int(tr[0])
+    if n >= tn[-1]:
+        return int(tr[-1])
+    k = 0
+    while tn[k + 1] <= n:
+        k += 1
+    return (int(tr[k]) * (int(tn[k + 1]) - n) + int(tr[k + 1]) * (n - int(tn[k]))) // (int(tn[k + 1]) - int(tn[k]))
+
+
+def combine_cost(n, mode, perf_table=None):
     """What the evaluation of a submatrix of dimension n costs in the combination criterion.
-    mode 1, Eq. 9 (L87): n^3, the FLOP count of a dense multiplication. mode 2, Eq. 10 (L91):
-    p(n) x n^3 with the GPU's measured performance characteristic; for the B200 engine the
-    measured time of a multiplication is proportional to the number of 256 x 256 x 64 tile steps
-    (C-19), so p(n) n^3 := ceil(n16/256)^2 ceil(n16/64), n16 = n rounded up to 16."""
+    mode 1, Eq. 9 (L87): n^3, the FLOP count of a dense multiplication. mode 2, Eq. 10 (L91): the predicted runtime
+    "p(n) x n^3" with the measured performance characteristic of the GPU, i.e. n^3 / r(n) for a measured rate r(n)
+    (perf_rate), scaled by 10^6 and floored so that everything stays an integer. Without a table mode 2 falls back to
+    a model of the B200 engine, the number of 256 x 256 x 64 tile steps of a multiplication,
+    ceil(n16/256)^2 ceil(n16/64) with n16 = n rounded up to 16 (C-19)."""
     n = int(n)
     if mode == 1:
         return n * n * n
+    if perf_table is not None:
+        return 10 ** 6 * n * n * n // perf_rate(perf_table, n)
     n16 = (n + 15) // 16 * 16
     t = (n16 + 255) // 256
     return t * t * ((n16 + 63) // 64)
 
 
-def combine_groups(atom_nb, index_sets, mode=1, max_dim=2048, max_members=16, max_candidates=24):
+def combine_groups(atom_nb, index_sets, mode=1, max_dim=2048, max_members=16, max_candidates=24, perf_table=None):
     """Greedy combination of columns (atoms) into groups that share ONE submatrix (C-19).
 
     Atoms are visited in ascending id. An atom i that is still free seeds a group G = N(i). Its
@@ -241,7 +260,8 @@ def combine_groups(atom_nb, index_sets, mode=1, max_dim=2048, max_members=16, ma
     ties by id), the first max_candidates of them. A candidate joins iff the criterion of Eq. 9
     (mode 1) or Eq. 10 (mode 2) holds for the group as it stands,
         cost(n_G + n_j - n_{G & j}) < cost(n_G) + cost(n_j),
-    and the union stays within max_dim; then G <- G | N(j). All quantities are integers.
+    and the union stays within max_dim; then G <- G | N(j). All quantities are integers. perf_table: the measured
+    (dimensions, GFLOP/s) of Eq. 10 (perf_rate).
     Returns the list of groups (member lists in joining order, seed first)."""
     nb = np.asarray(atom_nb, dtype=np.int64)
     n_at = len(nb)
@@ -271,7 +291,7 @@ def combine_groups(atom_nb, index_sets, mode=1, max_dim=2048, max_members=16, ma
                 n_u = n_g + dim[j] - n_gj
                 if n_u > max_dim:
                     continue
-                if combine_cost(n_u, mode) < combine_cost(n_g, mode) + combine_cost(dim[j], mode):
+                if combine_cost(n_u, mode, perf_table) < combine_cost(n_g, mode, perf_table) + combine_cost(dim[j], mode, perf_table):
                     members.append(j)
                     free[j] = False
                     G = np.union1d(G, index_sets[j])

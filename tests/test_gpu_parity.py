@@ -91,6 +91,57 @@ def test_gather_bit_exact(cfg0):
                 assert np.array_equal(g32, T.astype(np.float32))
 
 
+@pytest.mark.parametrize("name,n_atoms,combine", [("cfg2", 300, 0), ("cfg3", 20000, 0), ("cfg2", 300, 1), ("cfg3", 900, 1)])
+def test_gather_bit_exact_large(name, n_atoms, combine):
+    """P13 at the sizes where the gather task has more than one path: submatrices of 1200-2100 dimensions (the dense
+    strip of a row-atom takes several passes once 2 n16 exceeds 48 KB / 13 rows), mixed 5- and 13-function blocks
+    (cfg3 at full size: the largest submatrix of the blob), and a combined unit's union set (the dense matrix the group is
+    evaluated on). FP16 output == RN-even(FP64 -> FP16) of the oracle's dense submatrix, bit for bit."""
+    s = make_system(name, n_atoms=None if (name, n_atoms) == ("cfg3", 20000) else n_atoms)
+    dims = np.array([int(s.atom_nb[s.col_idx[s.row_ptr[i]:s.row_ptr[i + 1]]].sum()) for i in range(s.n_atoms)])
+    picks = [int(np.argmax(dims)), int(np.argsort(dims)[len(dims) // 2])]
+    if name == "cfg3":
+        mixed = [i for i in np.argsort(-dims)[:2000] if len(set(s.atom_nb[s.col_idx[s.row_ptr[i]:s.row_ptr[i + 1]]].tolist())) == 2]
+        picks.append(int(mixed[0]))                                  # a large submatrix with both block sizes
+    need = np.unique(np.concatenate([s.col_idx[s.row_ptr[a]:s.row_ptr[a + 1]] for a in picks]))
+    if combine:
+        sets = [orc.index_set(i, s.row_ptr, s.col_idx) for i in range(s.n_atoms)]
+        groups = orc.combine_groups(s.atom_nb, sets, mode=1)
+        big = max(groups, key=len)
+        assert len(big) > 1
+        picks = [big[0], big[-1]]
+    blk = s.blk_off()
+    if s.n_atoms > 5000:                                             # values on the device only; the oracle sees the neighbourhoods
+        Hd, Sd = s.fill_torch(MAT_H, "cuda"), s.fill_torch(MAT_S, "cuda")
+        sub = s.restrict(need)
+        Hn, Sn = sub.fill_np(MAT_H), sub.fill_np(MAT_S)
+        sblk = orc.block_offsets(sub.atom_nb, sub.row_ptr, sub.col_idx)
+        parent = sub.meta["parent_atoms"]
+        dense = lambda i, vals: orc.submatrix(np.searchsorted(parent, s.col_idx[s.row_ptr[i]:s.row_ptr[i + 1]]),
+                                              sub.atom_nb, sub.row_ptr, sub.col_idx, sblk, vals)[0]
+        arrays = (torch.from_numpy(s.atom_nb).cuda(), torch.from_numpy(s.row_ptr).cuda(), torch.from_numpy(s.col_idx).cuda(), Hd, Sd)
+    else:
+        Hn, Sn = s.fill_np(MAT_H), s.fill_np(MAT_S)
+        arrays = _arrays(s)
+        if combine:
+            dense = lambda i, vals: orc.submatrix(np.unique(np.concatenate([sets[m] for m in next(g for g in groups if i in g)])),
+                                                  s.atom_nb, s.row_ptr, s.col_idx, blk, vals)[0]
+        else:
+            dense = lambda i, vals: orc.submatrix(orc.index_set(i, s.row_ptr, s.col_idx), s.atom_nb, s.row_ptr, s.col_idx, blk, vals)[0]
+    biggest = 0
+    with _nolsm(combine=combine) as ctx:
+        ctx.assemble(*arrays)
+        for i in picks:
+            for which, vals in ((0, Sn), (1, Hn)):
+                T = dense(i, vals)
+                g16 = ctx.gather_submatrix(i, which, fp16=True)
+                assert g16.shape == T.shape
+                assert np.array_equal(g16.view(np.uint16), T.astype(np.float16).view(np.uint16))
+                biggest = max(biggest, T.shape[0])
+    assert biggest >= (1400 if name == "cfg2" or not combine else 1000)   # 13-row atoms: more than one strip pass from n16 = 1904 on
+    print("gather bit-exact", name, combine, [int(dims[i]) for i in picks], biggest)
+
+
 def test_cfg0_fp32_mode(cfg0):
     from paper_2205_12182_b200 import PREC_FP32
     s = cfg0
@@ -232,6 +283,88 @@ def test_single_atom_and_errors():
         assert ei.value.code == 1
 
 
+@pytest.mark.parametrize("iteration", [0, 1])
+def test_eigenvalue_at_mu_is_flagged_noconv_and_half_occupied(iteration):
+    """C-9: a generalised eigenvalue exactly at mu. Three atoms with two functions each, full pattern, S = I, and the two
+    functions of atom 0 duplicates of each other (equal rows and columns of H0): v = (1, -1, 0, ...) / sqrt 2 is an
+    eigenvector with eigenvalue exactly 0 = mu, and it stays an exact null vector of every iterate (columns 0 and 1 of
+    every polynomial of H0 are computed by identical operations). The sign iteration can never converge on it: the call
+    reports NOLSM_ENOCONV, sets the status bit, and still writes D - with the mode half occupied (sign(0) = 0), which is the
+    mean of the oracle's D just below and just above mu."""
+    from paper_2205_12182_b200 import NolsmError
+    nb = np.array([2, 2, 2], np.int32)
+    rp = np.array([0, 3, 6, 9], np.int64)
+    ci = np.array([0, 1, 2] * 3, np.int32)
+    a, b, c, d, e, f, g, h, i_, j, k, l, m, n_, o = 0.5, 0.25, -0.375, 0.125, 0.3125, -1.25, 0.1875, -0.25, 0.0625, 0.75, 0.125, -0.1875, 1.5, 0.25, -0.875
+    Hd = np.array([[a, a, b, c, d, e], [a, a, b, c, d, e], [b, b, f, g, h, i_], [c, c, g, j, k, l], [d, d, h, k, m, n_], [e, e, i_, l, n_, o]])
+    assert np.array_equal(Hd, Hd.T)
+    eps = np.linalg.eigvalsh(Hd)
+    assert np.sum(np.abs(eps) < 1e-12) == 1 and np.sort(np.abs(eps))[1] > 0.05
+    Sd = np.eye(6)
+    to_blocks = lambda M: np.concatenate([M[2 * i:2 * i + 2, 2 * jj:2 * jj + 2].reshape(-1) for i in range(3) for jj in range(3)])
+    Hv, Sv = to_blocks(Hd), to_blocks(Sd)
+    with _nolsm(iteration=iteration, max_sign_iters=40) as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        D = np.zeros(36)
+        ctx.density_matrix(0.0, D)
+        with pytest.raises(NolsmError) as ei:
+            ctx.energy()
+        assert ei.value.code == 6                                   # NOLSM_ENOCONV, after writing the result
+        st = ctx.atom_stats()
+        assert (st["status"] == 2).all() and (st["sign_iters"] >= 39).all()
+    blk = orc.block_offsets(nb, rp, ci)
+    for atom in range(3):
+        lo = orc.atom_result(atom, nb, rp, ci, blk, Hv, Sv, -0.01)
+        hi = orc.atom_result(atom, nb, rp, ci, blk, Hv, Sv, +0.01)
+        ref = 0.5 * (lo["Dcols"] + hi["Dcols"])                    # [6 rows, 2 columns of the atom]
+        got = np.stack([D[blk[3 * atom + jj]:blk[3 * atom + jj + 1]].reshape(2, 2).T for jj in range(3)]).reshape(6, 2)   # slot (i, j) = (D_ji)^T
+        assert np.abs(got - ref).max() <= TOL_MIXED_D
+        assert abs(float(st["e_atom"][atom]) - 0.5 * (lo["e_i"] + hi["e_i"])) <= 2e-3
+
+
+@pytest.mark.parametrize("iteration", [0, 1])
+def test_electron_counts_for_several_mu_in_one_pass(cfg0, iteration):
+    """nolsm_electron_counts: Tr(D(mu_j) S) and Tr(D(mu_j) H0) for several trial mu on the resident S_sub^-1 and A0 (C-20)
+    against the oracle's count at each mu, and against one nolsm_density_matrix call per mu."""
+    s = cfg0
+    nb, rp, ci, Hv, Sv = _arrays(s)
+    Hn, Sn = s.fill_np(MAT_H), s.fill_np(MAT_S)
+    mus = [-0.6, -0.05, 0.3, 1.1]
+    n_tot = float(s.atom_nb.sum())
+    with _nolsm(iteration=iteration) as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        counts, energies = ctx.electron_counts(mus, with_energy=True)
+        D = torch.zeros(Hv.shape[0], dtype=torch.float64, device="cuda")
+        for j, mu in enumerate(mus):
+            ref = orc.electron_count(s.atom_nb, s.row_ptr, s.col_idx, Hn, Sn, mu)
+            assert abs(counts[j] - ref) <= TOL_MIXED_E * n_tot
+            ctx.density_matrix(mu, D)
+            E1 = ctx.energy()
+            assert abs(ctx.electron_count() - counts[j]) <= TOL_MIXED_E * n_tot
+            assert abs(E1 - energies[j]) <= TOL_MIXED_E * abs(E1) + 1e-3
+        assert all(counts[j + 1] >= counts[j] - 1e-3 for j in range(len(mus) - 1))       # never decreases with mu
+    print("electron_counts", iteration, counts, energies)
+
+
+def test_fp32_mode_on_13_function_submatrices():
+    """The all-FP32 validation mode (plain FFMA round engine) where it is hard: submatrices of ~1200 dimensions with 13
+    functions per atom, whose spectra reach within 1e-3 of mu (cfg2) - and the mixed 5 / 13 blob of cfg3. BASELINE.json
+    asks for 1e-5 on D and E."""
+    from paper_2205_12182_b200 import PREC_FP32
+    for name, n_atoms, count in (("cfg2", 300, 12), ("cfg3", 900, 12)):
+        s = make_system(name, n_atoms=n_atoms)
+        nb, rp, ci, Hv, Sv = _arrays(s)
+        with _nolsm(precision=PREC_FP32) as ctx:
+            ctx.assemble(nb, rp, ci, Hv, Sv)
+            D = torch.zeros(Hv.shape[0], dtype=torch.float64, device="cuda")
+            ctx.density_matrix_range(s.mu, 0, count, D, want_energy=True)
+            st = ctx.atom_stats()
+        cmp = compare_atoms(s, D.cpu().numpy(), st["e_atom"], range(count))
+        print("fp32", name, {k: v for k, v in cmp.items() if k != "ref"})
+        assert (st["status"][:count] == 0).all()
+        assert cmp["max_abs_dD"] <= TOL_FP32 and cmp["rel_dE"] <= TOL_FP32
+
+
 def test_indefinite_S_is_reported(cfg0):
     """gamma = 1 (BASELINE.json's literal amplitude 0.3) is indefinite on cfg0 (SURVEY finding 1): the
     Schulz inverse cannot converge for the affected submatrices and the library must say so."""
@@ -263,18 +396,37 @@ def _oracle_groups(s, mode, **kw):
     return orc.combine_groups(s.atom_nb, sets, mode=mode, **kw), sets
 
 
-@pytest.mark.parametrize("mode", [1, 2])
+def _measured_perf_table():
+    """p(n) measured on B200 (workloads/pn_b200.json): (dimensions, TFLOP/s) for the library, (dimensions, integer
+    GFLOP/s) for the oracle."""
+    import json
+    import os
+    with open(os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "workloads", "pn_b200.json")) as f:
+        tab = json.load(f)["table"]
+    n, tf = [int(r["n"]) for r in tab], [float(r["tflops"]) for r in tab]
+    return (n, tf), (n, [int(round(t * 1000)) for t in tf])
+
+
+@pytest.mark.parametrize("mode", [1, 2, "2+table"])
 @pytest.mark.parametrize("name,n_atoms", [("cfg0", None), ("cfg2", 300), ("cfg3", 900)])
 def test_combined_groups_bit_exact_and_parity(name, n_atoms, mode):
     """The library's greedy groups and union index sets equal the oracle's bit for bit; D and e_i of every member
     of the sampled groups match the oracle's group evaluation (one Eq. 8 on the union, columns of each member,
-    rows restricted to N(member)) within the mixed-precision tolerances."""
+    rows restricted to N(member)) within the mixed-precision tolerances. "2+table": Eq. 10 with the measured,
+    interpolated p(n) handed to both sides; 2: the tile-step fallback."""
     s = make_system(name, n_atoms=n_atoms)
-    groups, sets = _oracle_groups(s, mode)
+    lib_table, orc_table = _measured_perf_table()
+    with_table = mode == "2+table"
+    mode = 2 if with_table else mode
+    groups, sets = _oracle_groups(s, mode, perf_table=orc_table if with_table else None)
+    if with_table and name == "cfg2":
+        assert groups != _oracle_groups(s, 2)[0]                    # the measured table decides differently from the model
     nb, rp, ci, Hv, Sv = _arrays(s)
     blk = s.blk_off()
     Hn, Sn = s.fill_np(MAT_H), s.fill_np(MAT_S)
     with _nolsm(combine=mode) as ctx:
+        if with_table:
+            ctx.set_perf_table(*lib_table)
         ctx.assemble(nb, rp, ci, Hv, Sv)
         for g in groups:
             mem, st_, dim = ctx.group(g[0])

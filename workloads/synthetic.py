@@ -399,6 +399,15 @@ def _geometry(name: str, n_atoms: int | None, seed: int):
         n = n_atoms or n
         edge = (n / DENSITY) ** (1.0 / 3.0)
         return uniform_positions(n, edge, seed, MINSEP, True), edge, np.full(n, nb, np.int32), {}
+    if name.startswith("pn-"):
+        # p(n) family ("measured for different matrix sizes n"): a periodic system at the paper's density whose
+        # submatrix dimension is set by the basis size and the cutoff, "pn-<nb>-<r_c>": dim ~ (4/3 pi r_c^3 0.1 + 1) nb
+        _, nb, rc = name.split("-")
+        n = n_atoms or 2048
+        edge = (n / DENSITY) ** (1.0 / 3.0)
+        if edge < 2.0 * float(rc):
+            raise ValueError("pn system: box edge < 2 r_c (one image per pair is needed)")
+        return uniform_positions(n, edge, seed, MINSEP, True), edge, np.full(n, int(nb), np.int32), {"r_c": float(rc)}
     if name == "cfg3":
         n = n_atoms or 20000
         n_blob = int(round(n * 6378 / 20000))
@@ -415,7 +424,11 @@ def make_system(name: str, n_atoms: int | None = None, seed: int = 0, gamma: flo
     (same density and basis; used for proxies and small parity cases). `gamma` overrides the
     tabulated C-12 rescale (key f"{name}" or f"{name}@{n_atoms}" in gamma_table.json)."""
     pos, box, atom_nb, meta = _geometry(name, n_atoms, seed)
-    row_ptr, col_idx, dist = neighbour_pattern(pos, R_C, box)
+    row_ptr, col_idx, dist = neighbour_pattern(pos, meta.get("r_c", R_C), box)
+    if gamma is None and name.startswith("pn-"):
+        # C-12 rescale from the row-variance estimate lambda_min(W) ~ -2.3 sqrt(0.1233 nb) (SURVEY appendix 1; the S blocks
+        # have decayed by r = 6 A, so larger cutoffs change nothing): lambda_min(S) ~ 0.3
+        gamma = 0.85 / math.sqrt(float(atom_nb[0]))
     if gamma is None:
         tab = gamma_table()
         key = name if n_atoms is None else f"{name}@{n_atoms}"

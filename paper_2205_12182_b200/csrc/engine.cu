@@ -304,6 +304,9 @@ int engine_plan(nolsm_ctx* c, cudaStream_t s) {
     cudaDeviceGetAttribute(&l2_bytes, cudaDevAttrL2CacheSize, c->dev);
     if (l2_bytes <= 0) l2_bytes = 64 << 20;
     int g_max = (int)std::floor(1.0 * (double)l2_bytes / (3.5 * mean_n2 * 2.0));
+    // the Loewdin form offers (ntm + 1) / 2 ntm of the tiles per GEMM (upper triangle only): twice as many chains keep the
+    // CTA pairs busy (measured on cfg2: 24-28 against 12-14, profiles/r02_persist.md)
+    if (c->opt.iteration == NOLSM_ITER_LOWDIN && c->opt.symmetric_tiles >= 0) g_max *= 2;
     g_max = std::max(3, std::min(g_max, 48));
     if (c->opt.heavy_slots > 0) g_max = c->opt.heavy_slots;
     int S = c->opt.batch_atoms > 0 ? c->opt.batch_atoms

@@ -113,42 +113,48 @@ __device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t par
     return ok != 0;
 }
 // The waits below return false on a stall (watchdog, gemm_umma.cuh).
-__device__ __forceinline__ bool mbar_wait_cluster(uint32_t bar, uint32_t parity, volatile int* abort_flag) {
-    uint32_t spins = 0;
-    unsigned long long t0 = 0;
-    while (!mbar_try_wait_cluster(bar, parity)) {
-        if (++spins > 4096u) {
-            __nanosleep(64);
-            if ((spins & 4095u) == 0 && stalled(t0, abort_flag)) return false;
-        }
-    }
-    return true;
+__device__ __forceinline__ bool mbar_try_wait_cluster_hint(uint32_t bar, uint32_t parity, uint32_t ns) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2, %3;\n\t"
+        "selp.b32 %0, 1, 0, p;\n\t}\n"
+        : "=r"(ok) : "r"(bar), "r"(parity), "r"(ns) : "memory");
+    return ok != 0;
 }
-// Wait that may legitimately last long (a role of the persistent engine with no work): polls gently after a short spin.
-// The scheduler ends such a wait with a record that says "no more tiles"; the watchdog only covers a scheduler that is
-// itself stuck, so its limit is ten times the usual one.
-__device__ __forceinline__ bool mbar_wait_cluster_patient(uint32_t bar, uint32_t parity, volatile int* abort_flag) {
-    uint32_t spins = 0, rounds = 0;
+__device__ __noinline__ bool mbar_wait_cluster_slow(uint32_t bar, uint32_t parity, volatile int* abort_flag, uint32_t ns, uint32_t rounds) {
     unsigned long long t0 = 0;
-    while (!mbar_try_wait_cluster(bar, parity)) {
-        if (++spins > 16u) {
-            __nanosleep(spins < 1024u ? 200 : 1000);
-            if ((spins & 4095u) == 0 && stalled(t0, abort_flag)) { if (++rounds >= 10u) return false; t0 = 0; }
-        }
+    for (uint32_t spins = 1;; ++spins) {
+        if (mbar_try_wait_cluster_hint(bar, parity, ns)) return true;
+        if ((spins & 1023u) == 0 && stalled(t0, abort_flag)) { if (--rounds == 0) return false; t0 = 0; }
     }
-    return true;
+}
+__device__ __noinline__ bool mbar_wait_cluster_sleep(uint32_t bar, uint32_t parity, volatile int* abort_flag, uint32_t ns, uint32_t rounds) {
+    unsigned long long t0 = 0;
+    for (uint32_t spins = 1;; ++spins) {
+        if (mbar_try_wait_cluster(bar, parity)) return true;
+        __nanosleep(ns);
+        if ((spins & 4095u) == 0 && stalled(t0, abort_flag)) { if (--rounds == 0) return false; t0 = 0; }
+    }
+}
+__device__ __forceinline__ bool mbar_wait_cluster(uint32_t bar, uint32_t parity, volatile int* abort_flag) {
+#pragma unroll 1
+    for (int i = 0; i < 4096; ++i)
+        if (mbar_try_wait_cluster(bar, parity)) return true;
+    return mbar_wait_cluster_sleep(bar, parity, abort_flag, 64u, 1u);
+}
+// Wait that may legitimately last long (a role of the persistent engine with no work). The scheduler ends such a wait
+// with a record that says "no more tiles"; the watchdog only covers a scheduler that is itself stuck, so its limit is
+// ten times the usual one.
+__device__ __forceinline__ bool mbar_wait_cluster_patient(uint32_t bar, uint32_t parity, volatile int* abort_flag) {
+    if (mbar_try_wait_cluster(bar, parity)) return true;
+    return mbar_wait_cluster_slow(bar, parity, abort_flag, 4000u, 10u);
 }
 // Wait of the eight epilogue warps for the accumulator of the tile being multiplied: microseconds long and not on the
-// critical path (two accumulators), so the warps sleep between polls instead of issuing a try_wait loop (which was 28 %
-// of all instructions the kernel issued: profiles/r01_persist_v6.md) - the issue slots and the power go to the k-loop.
+// critical path (two accumulators): suspended try_waits (no polling loop).
 __device__ __forceinline__ bool mbar_wait_sleepy(uint32_t bar, uint32_t parity, volatile int* abort_flag) {
-    uint32_t spins = 0;
-    unsigned long long t0 = 0;
-    while (!mbar_try_wait(bar, parity)) {
-        __nanosleep(spins < 4u ? 64 : 256);
-        if ((++spins & 4095u) == 0 && stalled(t0, abort_flag)) return false;
-    }
-    return true;
+    if (mbar_try_wait(bar, parity)) return true;
+    return mbar_wait_slow(bar, parity, abort_flag, 4000u, 1u);
 }
 __device__ __forceinline__ void st_cluster_u32(uint32_t cluster_addr, uint32_t v) {
     asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(cluster_addr), "r"(v) : "memory");
@@ -202,6 +208,38 @@ __device__ __forceinline__ void st_box_row(uint32_t box, int r, int j0, const ui
     }
 }
 
+// The same 32 halves written TRANSPOSED: element j of box row r, column c0 + j goes to box row c0 + j, column r. The lanes
+// of a warp are 32 consecutive r: under the swizzle they hit 4 distinct 16-byte chunks of one 128-byte row, 2 lanes per
+// bank word: no bank conflict.
+__device__ __forceinline__ void st_box_col(uint32_t box, int r, int c0, const uint32_t* hp) {
+    const uint32_t rlo = (uint32_t)(r & 7) << 1, rhi = (uint32_t)(r >> 3);
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+        const int cc = c0 + j;
+        const uint32_t a = box + (uint32_t)cc * 128u + (((rhi ^ (uint32_t)(cc & 7)) << 4) | rlo);
+        const unsigned short v = (unsigned short)((j & 1) ? (hp[j >> 1] >> 16) : (hp[j >> 1] & 0xFFFFu));
+        asm volatile("st.shared.b16 [%0], %1;" ::"r"(a), "h"(v) : "memory");
+    }
+}
+// Diagonal box of a symmetric product (box rows and box columns are the same index range): the upper triangle of the
+// box, element (r, c0 + j) with c0 + j >= r, goes to its own place and to the transposed place.
+__device__ __forceinline__ void st_box_sym(uint32_t box, int r, int c0, const uint32_t* hp) {
+    const uint32_t rlo = (uint32_t)(r & 7) << 1, rhi = (uint32_t)(r >> 3);
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+        const int cc = c0 + j;
+        if (cc >= r) {
+            const unsigned short v = (unsigned short)((j & 1) ? (hp[j >> 1] >> 16) : (hp[j >> 1] & 0xFFFFu));
+            const uint32_t an = box + (uint32_t)r * 128u + (((((uint32_t)cc >> 3) ^ (uint32_t)(r & 7)) << 4) | ((uint32_t)(cc & 7) << 1));
+            asm volatile("st.shared.b16 [%0], %1;" ::"r"(an), "h"(v) : "memory");
+            if (cc > r) {
+                const uint32_t at = box + (uint32_t)cc * 128u + (((rhi ^ (uint32_t)(cc & 7)) << 4) | rlo);
+                asm volatile("st.shared.b16 [%0], %1;" ::"r"(at), "h"(v) : "memory");
+            }
+        }
+    }
+}
+
 }  // namespace ptx
 
 // ------------------------------------------------------------------------------------------------
@@ -247,18 +285,18 @@ __device__ __forceinline__ TileInfo g2_take(const G2Smem& sm, int q, uint32_t ph
 }
 
 // ------------------------------------------------------------------------------------------------
-// TMA producer: ONE thread per CTA runs this loop (the other lanes of its warp wait at the end of the role). The loop
-// is what paces a tile when the operands come from L2: per k-block it waits for the stage, arms the leader's full
-// barrier and issues the three or four box loads; everything else is hoisted out (measured on B200: with the whole warp
-// in the loop and lane 0 predicated inside, the k-block took ~650 cycles whatever the tile's width, the producer was
-// busy 85 % of the time and the MMA warp waited for operands; profiles/r02_producer.md).
+// TMA producer (one warp per CTA). The whole warp runs the loop on warp-uniform values and ONE ELECTED lane issues: with
+// `elect.sync` the compiler keeps the tensor-map addresses, coordinates and barrier addresses in uniform registers and the
+// loads go out back to back. (With `if (lane == 0)` around the issue block every UTMALDG sat in a loop over the distinct
+// values of its operands; the k-block then took ~650 cycles whatever the tile's width, the producer was busy 85 % of the
+// time and the MMA warp waited for operands: profiles/r02_persist.md.)
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap* maps, uint32_t rank, int want_lead, volatile int* abort_flag) {
+__device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap* maps, uint32_t rank, int lane, int want_lead, volatile int* abort_flag) {
     int stage = 0; uint32_t phase = 0;
     int q = 0; uint32_t tph = 0;
     const uint32_t full0 = ptx::mapa(sm.full(0), 0);                        // the leader's full barriers
     for (;;) {
-        const TileInfo ti = g2_take<false>(sm, q, tph, true, abort_flag);
+        const TileInfo ti = g2_take<true>(sm, q, tph, lane == 0, abort_flag);
         if (++q == G2_NTI) { q = 0; tph ^= 1; }
         if (!ti.valid) break;
         ptx::fence_proxy_async();      // operands may have been written by generic stores of another CTA
@@ -275,22 +313,25 @@ __device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap*
 #pragma unroll 1
         for (int kb = 0; kb < nkb; ++kb) {
             if (!ptx::mbar_wait(sm.empty(stage), phase ^ 1, abort_flag)) return;
-            if (kb == kb_want) ptx::mbar_arrive(sm.want());                // the scheduler may claim the next tile now
-            const uint32_t fb = full0 + 8u * stage;
-            if (rank == 0) ptx::mbar_expect_tx(sm.full(stage), bytes);
-            const uint32_t sa = sm.stage_a(stage), sb = sm.stage_b(stage);
-            const int k0 = kb * BK;
-            ptx::tma_load_2d_pair(sa, map_a, k0, row0, fb);
-            if (!hh) ptx::tma_load_2d_pair(sa + 8192, map_a, k0, row0 + 64, fb);
-            ptx::tma_load_2d_pair(sb, map_b, col0, k0, fb);
-            if (nbox > 1) ptx::tma_load_2d_pair(sb + B_BOX_BYTES, map_b, col0 + 64, k0, fb);
+            if (ptx::elect_one()) {
+                if (kb == kb_want) ptx::mbar_arrive(sm.want());            // the scheduler may claim the next tile now
+                const uint32_t fb = full0 + 8u * stage;
+                if (rank == 0) ptx::mbar_expect_tx(sm.full(stage), bytes);
+                const uint32_t sa = sm.stage_a(stage), sb = sm.stage_b(stage);
+                const int k0 = kb * BK;
+                ptx::tma_load_2d_pair(sa, map_a, k0, row0, fb);
+                if (!hh) ptx::tma_load_2d_pair(sa + 8192, map_a, k0, row0 + 64, fb);
+                ptx::tma_load_2d_pair(sb, map_b, col0, k0, fb);
+                if (nbox > 1) ptx::tma_load_2d_pair(sb + B_BOX_BYTES, map_b, col0 + 64, k0, fb);
+            }
+            __syncwarp();
             if (++stage == G2_STAGES) { stage = 0; phase ^= 1; }
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// MMA issuer: ONE thread of the leader CTA.
+// MMA issuer (one warp of the leader CTA; one elected lane issues, see g2_producer).
 // The issue loop must stay well under the tensor-pipe time of a k-block (4 MMAs x ~120 cycles): the
 // four MMAs of a full k-block go out as one asm block with the descriptors advanced by immediates
 // (A: +32 B per 16 k inside the 128-byte swizzle row; B: +2048 B = 16 k-rows of 128 B).
@@ -313,7 +354,7 @@ __device__ __forceinline__ void umma_f16_pair_x4(uint32_t d_tmem, uint64_t a_des
 }
 }  // namespace ptx
 
-__device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, volatile int* abort_flag) {
+__device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int lane, volatile int* abort_flag) {
     int stage = 0; uint32_t phase = 0;
     int acc = 0; uint32_t acc_phase = 0;
     int q = 0; uint32_t tph = 0;
@@ -321,7 +362,7 @@ __device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, vol
     const uint64_t da0 = make_smem_desc(sm.stage_a(0), 16, 1024);
     const uint64_t db0 = make_smem_desc(sm.stage_b(0), B_BOX_BYTES, 1024);
     for (;;) {
-        const TileInfo ti = g2_take<false>(sm, q, tph, true, abort_flag);
+        const TileInfo ti = g2_take<true>(sm, q, tph, lane == 0, abort_flag);
         if (++q == G2_NTI) { q = 0; tph ^= 1; }
         if (!ti.valid) break;
         const int nkb = (ti.n16 + BK - 1) / BK;
@@ -334,16 +375,19 @@ __device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, vol
         for (int kb = 0; kb < nkb; ++kb) {
             if (!ptx::mbar_wait(sm.full(stage), phase, abort_flag)) return;
             ptx::tc_fence_after();
-            const uint64_t da = da0 + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
-            const uint64_t db = db0 + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
-            if (kb < nkb - 1 || ktail == 4) {
-                ptx::umma_f16_pair_x4(d_tmem, da, db, idesc, kb != 0);
-            } else {
-                for (int k = 0; k < ktail; ++k)
-                    ptx::umma_f16_pair(d_tmem, da + 2 * k, db + 128 * k, idesc, (kb | k) != 0);
+            if (ptx::elect_one()) {
+                const uint64_t da = da0 + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
+                const uint64_t db = db0 + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
+                if (kb < nkb - 1 || ktail == 4) {
+                    ptx::umma_f16_pair_x4(d_tmem, da, db, idesc, kb != 0);
+                } else {
+                    for (int k = 0; k < ktail; ++k)
+                        ptx::umma_f16_pair(d_tmem, da + 2 * k, db + 128 * k, idesc, (kb | k) != 0);
+                }
+                ptx::umma_commit_pair(sm.empty(stage));
+                if (kb == nkb - 1) ptx::umma_commit_pair(sm.tfull(acc));
             }
-            ptx::umma_commit_pair(sm.empty(stage));
-            if (kb == nkb - 1) ptx::umma_commit_pair(sm.tfull(acc));
+            __syncwarp();
             if (++stage == G2_STAGES) { stage = 0; phase ^= 1; }
         }
         if (++acc == 2) { acc = 0; acc_phase ^= 1; }
@@ -387,7 +431,6 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
         int ldc;
         __half* C = c_ptr(e, base, ti.slot, ti.c_buf, ldc);
         const bool ident = (ti.valid & TI_PLAIN) == 0;             // plain tiles: C = c_out acc, res = ||alpha_res acc||_F^2 (no identity)
-        const bool mirror = (ti.valid & TI_MIRROR) != 0;
         // full-height tile: the CTA's 128 TMEM lanes are 128 rows, every warp sees all bn columns; half-height tile
         // (M = 128 over the pair): lanes 0-63 and 64-127 are the same 64 rows with the left / right half of the columns
         const bool hh = (ti.valid & TI_HALF) != 0;
@@ -401,20 +444,33 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
         float rsum = 0.f, vsum = 0.f;
         uint32_t dep = 0;
         const bool symdiag = (ti.valid & TI_SYMDIAG) != 0;         // diagonal tile of a symmetric product
-        const bool via_tma = ident && !hh && !symdiag;             // full-height square GEMM tiles leave through shared memory and TMA stores
+        const bool via_tma = ident && !hh;                         // full-height square GEMM tiles leave through shared memory and TMA stores
+        float rsum2 = 0.f, vsum2 = 0.f;                            // residual terms of boxes that stand for their mirror image too
         if (via_tma) {
             // C leaves in 64 x 64 boxes: the four warps that hold rows [64 g, 64 g + 64) of the CTA's 128 rows and the two
             // 32-column halves of a box write it into a swizzled staging buffer; one thread hands it to the TMA unit, which
             // writes whole 128-byte lines (the row-per-thread register stores issue one request per 32 bytes and go
             // through the SM's load/store path, which the k-loop's ingest also needs). Two buffers per row group.
+            // Symmetric products (TI_MIRROR / TI_SYMDIAG): a box above the diagonal is also written TRANSPOSED into the
+            // second buffer and stored to the mirrored position (2-byte shared-memory stores, conflict-free under the
+            // 128-byte swizzle; the transposed copy as 2-byte global stores cost 16 % of the Loewdin form's throughput);
+            // a box on the diagonal is filled from its upper triangle, so the stored matrix is exactly symmetric; a box
+            // below the diagonal is not stored at all.
             const int rbox = ((quarter & 1) << 5) + lane;
             const bool issuer = (quarter & 1) == 0 && chalf == 0 && lane == 0;
             const CUtensorMap* map_c = maps + (size_t)ti.slot * NMAP + ti.c_buf;
             const int nbx = (bn + 63) >> 6;
+            const int brow = ti.m0 + 128 * (int)rank + 64 * g;     // first row of this group's boxes
+            int bsel = 0;
             for (int kx = 0; kx < nbx; ++kx) {
                 const int c = (kx << 6) + (chalf << 5);
-                const uint32_t box = sm.stage_c(g, kx & 1);
-                if (issuer) ptx::bulk_wait_read<1>();              // the store that read this buffer two boxes ago is done with it
+                const int bcol = col0 + (kx << 6);                 // first column of the box
+                // 0: plain box; 1: box above the diagonal of a symmetric product (stored and mirrored); 2: diagonal box;
+                // 3: box below the diagonal (skipped). Uniform over the four warps of the group.
+                const int mode = (ti.valid & TI_MIRROR) ? 1 : !symdiag ? 0 : bcol > brow ? 1 : bcol == brow ? 2 : 3;
+                if (mode == 3) continue;
+                const uint32_t box = sm.stage_c(g, mode == 1 ? 0 : bsel), boxt = sm.stage_c(g, 1);
+                if (issuer) { if (mode == 1) ptx::bulk_wait_read<0>(); else ptx::bulk_wait_read<1>(); }   // the stores that read these buffers are done with them
                 asm volatile("bar.sync %0, 128;" ::"r"(3 + g) : "memory");
                 float f[32];
                 int ncols = 0;                                     // valid columns of this chunk (warp-uniform)
@@ -427,12 +483,15 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                     const bool diag = (col0 + c < rbase + 32) && (col0 + c + 32 > rbase);
                     if (ncols == 32 && !diag) {
                         if (ti.want_res && row < n16) {
+                            float vs = 0.f;
 #pragma unroll
-                            for (int j = 0; j < 32; ++j) { const float a = __uint_as_float(v[j]); vsum = fmaf(a, a, vsum); }
+                            for (int j = 0; j < 32; ++j) { const float a = __uint_as_float(v[j]); vs = fmaf(a, a, vs); }
+                            if (mode == 1) vsum2 += vs; else vsum += vs;
                         }
 #pragma unroll
                         for (int j = 0; j < 32; ++j) f[j] = sa * __uint_as_float(v[j]);
                     } else {
+                        float rs = 0.f;
 #pragma unroll
                         for (int j = 0; j < 32; ++j) {
                             const int col = col0 + c + j;
@@ -440,9 +499,10 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                             const float delta = (col == row && row < n) ? 1.f : 0.f;
                             const bool in = (j < ncols && row < n16);
                             const float d = in ? ti.alpha_res * a - delta : 0.f;      // pad rows / columns give exactly 0
-                            rsum = fmaf(d, d, rsum);
+                            rs = fmaf(d, d, rs);
                             f[j] = in ? ti.c_out * a + ti.beta * delta : 0.f;
                         }
+                        if (mode == 1) rsum2 += rs; else rsum += rs;
                     }
                 } else {
 #pragma unroll
@@ -451,18 +511,24 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                 uint32_t hp[16];
 #pragma unroll
                 for (int j = 0; j < 16; ++j) { __half2 h = __floats2half2_rn(f[2 * j], f[2 * j + 1]); hp[j] = *reinterpret_cast<uint32_t*>(&h); }
-                ptx::st_box_row(box, rbox, chalf << 2, hp);
-                if (mirror && ncols > 0 && row < n16) st_mirror(C + (size_t)(col0 + c) * ldc + row, ldc, hp, ncols);
+                if (mode != 2) {
+                    ptx::st_box_row(box, rbox, chalf << 2, hp);
+                    if (mode == 1) ptx::st_box_col(boxt, rbox, chalf << 5, hp);
+                } else {
+                    ptx::st_box_sym(box, rbox, chalf << 5, hp);
+                }
                 ptx::fence_proxy_async_smem();
                 asm volatile("bar.sync %0, 128;" ::"r"(3 + g) : "memory");
                 if (issuer) {
-                    const int brow = ti.m0 + 128 * (int)rank + 64 * g;
-                    if (brow < n16) ptx::tma_store_2d(map_c, col0 + (kx << 6), brow, box);    // boxes below the matrix are padding
+                    if (brow < n16) {                              // boxes below the matrix are padding
+                        ptx::tma_store_2d(map_c, bcol, brow, box);
+                        if (mode == 1) ptx::tma_store_2d(map_c, brow, bcol, boxt);
+                    }
                     ptx::bulk_commit();
                 }
+                if (mode != 1) bsel ^= 1;
             }
             ptx::tc_fence_before();
-            if (mirror) ptx::fence_proxy_async();                  // the transposed block was written with generic stores, read next by TMA
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive_cluster_relaxed(tempty0 + 8u * acc, dep);     // the accumulator is free
             if (issuer) ptx::bulk_wait<0>();                       // the boxes of this tile are in global memory
@@ -544,8 +610,7 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
             if (lane == 0) ptx::mbar_arrive_cluster_relaxed(tempty0 + 8u * acc, dep);
         }
         if (ti.want_res) {
-            rsum = fmaf(ti.alpha_res * ti.alpha_res, vsum, rsum);
-            if (mirror) rsum *= 2.f;
+            rsum = fmaf(ti.alpha_res * ti.alpha_res, vsum, rsum) + 2.f * fmaf(ti.alpha_res * ti.alpha_res, vsum2, rsum2);
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) rsum += __shfl_xor_sync(0xffffffffu, rsum, o);
             if (lane == 0 && rsum != 0.f) atomicAdd(&e.slots[ti.slot].res_acc, rsum);

@@ -59,17 +59,41 @@ __device__ __forceinline__ bool stalled(unsigned long long& t0, volatile int* ab
     atomicExch(const_cast<int*>(abort_flag), 2);
     return true;
 }
-// Wait on an mbarrier of this CTA. Returns false on a stall (watchdog).
-__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatile int* abort_flag) {
-    uint32_t spins = 0;
+// try_wait with a suspend-time hint: the hardware parks the thread until the phase completes or `ns` have passed, so a
+// waiting warp issues one instruction per `ns` instead of a sleep-and-poll loop (the polling loops of the eight epilogue
+// warps were 30 % of all instructions the kernel issued: profiles/r02_persist.md) and wakes without the sleep's latency.
+__device__ __forceinline__ bool mbar_try_wait_hint(uint32_t bar, uint32_t parity, uint32_t ns) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+        "selp.b32 %0, 1, 0, p;\n\t}\n"
+        : "=r"(ok) : "r"(bar), "r"(parity), "r"(ns) : "memory");
+    return ok != 0;
+}
+// Slow path of every wait: suspended try_waits, the watchdog every 1024 of them. Out of line: one copy of the loop.
+__device__ __noinline__ bool mbar_wait_slow(uint32_t bar, uint32_t parity, volatile int* abort_flag, uint32_t ns, uint32_t rounds) {
     unsigned long long t0 = 0;
-    while (!mbar_try_wait(bar, parity)) {
-        if (++spins > 4096u) {
-            __nanosleep(64);
-            if ((spins & 4095u) == 0 && stalled(t0, abort_flag)) return false;
-        }
+    for (uint32_t spins = 1;; ++spins) {
+        if (mbar_try_wait_hint(bar, parity, ns)) return true;
+        if ((spins & 1023u) == 0 && stalled(t0, abort_flag)) { if (--rounds == 0) return false; t0 = 0; }
     }
-    return true;
+}
+// Slow path with sleeps between polls (nanosleep `ns`), the watchdog every 4096 polls. Out of line.
+__device__ __noinline__ bool mbar_wait_sleep(uint32_t bar, uint32_t parity, volatile int* abort_flag, uint32_t ns, uint32_t rounds) {
+    unsigned long long t0 = 0;
+    for (uint32_t spins = 1;; ++spins) {
+        if (mbar_try_wait(bar, parity)) return true;
+        __nanosleep(ns);
+        if ((spins & 4095u) == 0 && stalled(t0, abort_flag)) { if (--rounds == 0) return false; t0 = 0; }
+    }
+}
+// Wait on an mbarrier of this CTA (the hot waits of the k-loop: stage full / stage empty). Returns false on a stall.
+__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatile int* abort_flag) {
+#pragma unroll 1
+    for (int i = 0; i < 4096; ++i)
+        if (mbar_try_wait(bar, parity)) return true;
+    return mbar_wait_sleep(bar, parity, abort_flag, 64u, 1u);
 }
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
     asm volatile(

@@ -466,21 +466,13 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
     int q = 0; uint32_t ph = 0;
     unsigned long long idle_ns = 0, ntiles = 0, overshoot = 0;
     const unsigned long long t_begin = pl::gtime();
-    bool stalled = false;
     for (;;) {
-        if (!ptx::mbar_wait_cluster_patient(sm.ti_empty(q), ph ^ 1, e.abort_flag)) { stalled = true; break; }
+        if (!ptx::mbar_wait_cluster_patient(sm.ti_empty(q), ph ^ 1, e.abort_flag)) break;
         // Claim lazily: only when the producer has issued every load of the tile before and needs the next
         // record (it runs G2_STAGES k-blocks ahead of the MMA, which hides the claim). A pair that claimed
         // further ahead would hoard tiles of a GEMM that idle pairs could run at the same time, and the
         // slot's chain of dependent GEMMs would take that much longer.
-        {
-            uint32_t spins = 0; unsigned long long t0 = 0;
-            while (!ptx::mbar_try_wait(sm.want(), (uint32_t)(ntiles & 1) ^ 1u)) {
-                __nanosleep(64);
-                if ((++spins & 4095u) == 0 && ptx::stalled(t0, e.abort_flag)) { stalled = true; break; }
-            }
-            if (stalled) break;
-        }
+        if (!ptx::mbar_wait(sm.want(), (uint32_t)(ntiles & 1) ^ 1u, e.abort_flag)) break;
         TileInfo ti{};
         int got = 0, tflags = 0;
         unsigned long long t_idle0 = 0;
@@ -986,9 +978,9 @@ nolsm_persist_kernel(const __grid_constant__ PEngine e) {
     } else if (warp == G2_WARP_SCHED) {
         if (rank == 0) p_scheduler(sm, e, lane);
     } else if (warp == G2_WARP_TMA) {
-        if (lane == 0) g2_producer(sm, e.maps, rank, e.want_lead, e.abort_flag);
+        g2_producer(sm, e.maps, rank, lane, e.want_lead, e.abort_flag);
     } else if (warp == G2_WARP_MMA) {
-        if (rank == 0 && lane == 0) g2_mma(sm, tmem_base, e.abort_flag);
+        if (rank == 0) g2_mma(sm, tmem_base, lane, e.abort_flag);
     } else {
         p_side_loop(e, side_sm, (int)threadIdx.x - G2_CTRL_THREADS);
     }

@@ -365,6 +365,23 @@ def test_fp32_mode_on_13_function_submatrices():
         assert cmp["max_abs_dD"] <= TOL_FP32 and cmp["rel_dE"] <= TOL_FP32
 
 
+def test_one_heavy_token_and_many_small_units():
+    """Stress of the token hand-off of the persistent engine (persist.cuh p_token_release): ONE token, many small units
+    whose transitions are fast, every slot parks and is woken hundreds of times; a lost wake-up would leave the kernel
+    waiting for its time limit. Repeated calls, results equal to the default run."""
+    s = make_system("cfg1", n_atoms=600)
+    nb, rp, ci, Hv, Sv = _arrays(s)
+    D0, E0, st0, _ = _run(s)
+    with _nolsm(heavy_slots=1, batch_atoms=24, timeout_s=60.0) as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        D = torch.zeros(Hv.shape[0], dtype=torch.float64, device="cuda")
+        for _ in range(3):
+            ctx.density_matrix(s.mu, D)
+            E = ctx.energy()
+            assert abs(E - E0) <= TOL_MIXED_E * abs(E0)           # two valid runs (residual sums are atomics: iteration counts may differ)
+    assert np.abs(D.cpu().numpy() - D0).max() <= TOL_MIXED_D
+
+
 def test_indefinite_S_is_reported(cfg0):
     """gamma = 1 (BASELINE.json's literal amplitude 0.3) is indefinite on cfg0 (SURVEY finding 1): the
     Schulz inverse cannot converge for the affected submatrices and the library must say so."""

@@ -232,9 +232,12 @@ int nolsm_get_profile(nolsm_ctx* ctx, double* out, int n);
  *   out[2] kernel duration from the device clock (first scheduler start to last scheduler end), ms;
  *   out[3] GEMM tiles executed (256 x bn, one per CTA pair);  out[4], out[5] tile-scheduler idle / busy
  *   time summed over the CTA pairs, ms;  out[6] claim overshoots;  out[7] slots;  out[8] CTA pairs;
- *   out[9 + k], out[17 + k], out[25 + k]  side tasks of kind k (1 refill, 2 gather, 3 first Schulz step,
- *   4 D columns + scatter): busy ms summed over side groups, algorithmic bytes, tasks.  n must be >= NOLSM_COUNTERS_LEN. Synchronises. */
-#define NOLSM_COUNTERS_LEN 33
+ *   out[9 + k], out[17 + k], out[25 + k]  side tasks of kind k (1 refill, 2 gather, 3 elementwise steps,
+ *   4 D columns + scatter, 5 W columns of the Loewdin form): busy ms summed over side groups, algorithmic bytes, tasks;
+ *   out[33..35] where the MMA-issuing warps (one per CTA pair) spent the kernel, ms summed over the pairs: waiting for a
+ *   tile record, waiting for a free accumulator (= for the epilogue), inside k-loops (operand waits + issue).
+ *   n must be >= NOLSM_COUNTERS_LEN. Synchronises. */
+#define NOLSM_COUNTERS_LEN 36
 int nolsm_get_engine_counters(nolsm_ctx* ctx, double* out, int n);
 
 /* HBM-bound side tasks timed alone: which = 0 the gather of every submatrix of the assembled system (a1),

@@ -263,12 +263,13 @@ class Nolsm:
 
     def engine_counters(self) -> dict:
         """Counters of the persistent engine for the last density_matrix call (include/nolsm.h)."""
-        out = (C.c_double * 33)()
-        self._check(self._lib.nolsm_get_engine_counters(self._h, out, 33))
+        out = (C.c_double * 36)()
+        self._check(self._lib.nolsm_get_engine_counters(self._h, out, 36))
         v = list(out)
         kinds = ("none", "refill", "gather", "elementwise", "dcols", "wcols", "k6", "k7")
         d = {"persistent": bool(v[0]), "kernel_ms": v[1], "kernel_ms_device_clock": v[2], "tiles": v[3],
              "sched_idle_ms": v[4], "sched_busy_ms": v[5], "overshoots": v[6], "slots": int(v[7]), "pairs": int(v[8])}
+        d["mma_wait_record_ms"], d["mma_wait_accumulator_ms"], d["mma_kloop_ms"] = v[33], v[34], v[35]
         d["side"] = {k: {"busy_ms": v[9 + i], "bytes": v[17 + i], "tasks": v[25 + i]} for i, k in enumerate(kinds)
                      if v[25 + i] > 0}
         return d

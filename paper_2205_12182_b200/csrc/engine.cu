@@ -622,6 +622,7 @@ int engine_counters(nolsm_ctx* c, double* out) {
         out[17 + k] = (double)ct[PC_SIDE_BYTES + k];
         out[25 + k] = (double)ct[PC_SIDE_TASKS + k];
     }
+    for (int k = 0; k < 3; ++k) out[33 + k] = ct[PC_MMA_NS + k] * 1e-6;
     return NOLSM_OK;
 }
 

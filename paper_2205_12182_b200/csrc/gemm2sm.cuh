@@ -33,15 +33,15 @@ constexpr int G2_CSTAGE_BYTES = 4 * G2_CBOX_BYTES;    // two row groups (64 rows
 constexpr int G2_A_BYTES = 128 * BK * 2;              // 16 KB: this CTA's 128 rows x 64 k
 constexpr int G2_B_BYTES = 2 * B_BOX_BYTES;           // 16 KB: 64 k x (up to 128) columns
 constexpr int G2_STAGE_BYTES = G2_A_BYTES + G2_B_BYTES;
-constexpr int G2_NTI = 4;                             // tile-info ring depth
+constexpr int G2_NTI = 4;                             // tile-info ring depth (8 was measured on cfg1 with 1-3 claim credits: 3-10 % slower)
 #ifndef G2_WANT_LEAD
 #define G2_WANT_LEAD 14                               // k-blocks before the end of its tile at which the producer asks for the next one
 #endif
 constexpr int G2_EPI_WARPS = 8;                       // warp w: TMEM lane quarter w & 3, column chunks of parity w >> 2
 constexpr int G2_WARP_SCHED = 8, G2_WARP_TMA = 9, G2_WARP_MMA = 10;
 constexpr int G2_CTRL_THREADS = 11 * 32;              // warps 0..10
-// consumers of a TileInfo: leader = producer + MMA + epilogue warps, peer = producer + epilogue warps
-constexpr int G2_TI_CONSUMERS = 2 * (1 + G2_EPI_WARPS) + 1;
+// consumers of a TileInfo: leader = producer + MMA + epilogue warps, peer = producer + finisher + epilogue warps
+constexpr int G2_TI_CONSUMERS = 2 * (1 + G2_EPI_WARPS) + 2;     // + the finisher warp of the peer CTA
 
 // flags of TileInfo::valid
 constexpr int TI_VALID = 1;           // 0 = no more tiles
@@ -74,11 +74,15 @@ struct G2Smem {                       // byte offsets from the 1024-aligned base
     __device__ uint32_t ti_full(int q) const { return bars() + 8u * (2 * G2_STAGES + 4 + q); }
     __device__ uint32_t ti_empty(int q) const { return bars() + 8u * (2 * G2_STAGES + 4 + G2_NTI + q); }
     __device__ uint32_t tmem_ptr() const { return bars() + 8u * (2 * G2_STAGES + 4 + 2 * G2_NTI); }
-    // "the producer has issued every load of its current tile and wants the next record" (leader CTA only)
+    // a counter, not a barrier: the tiles whose loads the leader's producer has issued up to the claim point (kb_want)
     __device__ uint32_t want() const { return bars() + 8u * (2 * G2_STAGES + 4 + 2 * G2_NTI) + 8u; }
-    __device__ uint32_t tinfo(int q) const { return bars() + 256u + 64u * q; }
+    // "every store of tile record q is in global memory": one arrival per epilogue warp of both CTAs, in the PEER CTA's
+    // shared memory, where the finisher warp waits for it
+    __device__ uint32_t cdone(int q) const { return bars() + 8u * (2 * G2_STAGES + 4 + 2 * G2_NTI) + 16u + 8u * q; }
+    __device__ uint32_t tinfo(int q) const { return bars() + 512u + 64u * q; }
 };
-constexpr int G2_SMEM_BYTES = G2_STAGES * G2_STAGE_BYTES + G2_CSTAGE_BYTES + 256 + 64 * G2_NTI + 1024 /*align*/;
+constexpr int G2_SMEM_BYTES = G2_STAGES * G2_STAGE_BYTES + G2_CSTAGE_BYTES + 512 + 64 * G2_NTI + 1024 /*align*/;
+static_assert(8 * (2 * G2_STAGES + 4 + 3 * G2_NTI) + 16 <= 512, "barrier area");
 
 namespace ptx {
 
@@ -150,6 +154,10 @@ __device__ __forceinline__ bool mbar_wait_cluster_patient(uint32_t bar, uint32_t
     if (mbar_try_wait_cluster(bar, parity)) return true;
     return mbar_wait_cluster_slow(bar, parity, abort_flag, 4000u, 10u);
 }
+__device__ __forceinline__ bool mbar_wait_patient(uint32_t bar, uint32_t parity, volatile int* abort_flag) {
+    if (mbar_try_wait(bar, parity)) return true;
+    return mbar_wait_slow(bar, parity, abort_flag, 4000u, 10u);
+}
 // Wait of the eight epilogue warps for the accumulator of the tile being multiplied: microseconds long and not on the
 // critical path (two accumulators): suspended try_waits (no polling loop).
 __device__ __forceinline__ bool mbar_wait_sleepy(uint32_t bar, uint32_t parity, volatile int* abort_flag) {
@@ -158,6 +166,24 @@ __device__ __forceinline__ bool mbar_wait_sleepy(uint32_t bar, uint32_t parity, 
 }
 __device__ __forceinline__ void st_cluster_u32(uint32_t cluster_addr, uint32_t v) {
     asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(cluster_addr), "r"(v) : "memory");
+}
+// Asynchronous store of one word into the shared memory of a CTA of the cluster; its 4 bytes are credited to the
+// transaction count of an mbarrier of that CTA. A thread that sees the barrier's phase complete (plain CTA-scope wait)
+// sees the word: no cluster-scope acquire, hence no L1 invalidation (CCTL.IVALL) on the consumer's side.
+__device__ __forceinline__ void st_async_u32(uint32_t cluster_addr, uint32_t v, uint32_t mbar_cluster_addr) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];"
+                 ::"r"(cluster_addr), "r"(v), "r"(mbar_cluster_addr) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx_cluster(uint32_t mbar_cluster_addr, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.release.cluster.shared::cluster.b64 _, [%0], %1;" ::"r"(mbar_cluster_addr), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ uint32_t ld_shared_volatile_u32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_shared_volatile_u32(uint32_t addr, uint32_t v) {
+    asm volatile("st.volatile.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 // TMA load whose completion bytes are credited to an mbarrier of either CTA of the pair.
 __device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar_cluster) {
@@ -250,7 +276,8 @@ __device__ __forceinline__ uint32_t g2_setup(const G2Smem& sm, int warp, int lan
         for (int s = 0; s < G2_STAGES; ++s) { ptx::mbar_init(sm.full(s), 1); ptx::mbar_init(sm.empty(s), 1); }
         for (int a = 0; a < 2; ++a) { ptx::mbar_init(sm.tfull(a), 1); ptx::mbar_init(sm.tempty(a), 2 * G2_EPI_WARPS); }
         for (int q = 0; q < G2_NTI; ++q) { ptx::mbar_init(sm.ti_full(q), 1); ptx::mbar_init(sm.ti_empty(q), G2_TI_CONSUMERS); }
-        ptx::mbar_init(sm.want(), 1);
+        ptx::st_shared_volatile_u32(sm.want(), 0u);
+        for (int q = 0; q < G2_NTI; ++q) ptx::mbar_init(sm.cdone(q), 2 * G2_EPI_WARPS);
         ptx::fence_mbar_init();
     }
     if (warp == G2_WARP_MMA) ptx::tmem_alloc_pair(sm.tmem_ptr(), 512);
@@ -273,7 +300,7 @@ __device__ __forceinline__ void g2_teardown(uint32_t tmem_base, int warp) {
 template <bool WARP>
 __device__ __forceinline__ TileInfo g2_take(const G2Smem& sm, int q, uint32_t ph, bool release_lane, volatile int* abort_flag) {
     TileInfo ti;
-    if (!ptx::mbar_wait_cluster_patient(sm.ti_full(q), ph, abort_flag)) { ti.valid = 0; return ti; }
+    if (!ptx::mbar_wait_patient(sm.ti_full(q), ph, abort_flag)) { ti.valid = 0; return ti; }      // record written with st.async: CTA-scope wait
     uint32_t* w = reinterpret_cast<uint32_t*>(&ti);
 #pragma unroll
     for (int i = 0; i < 16; i += 4)
@@ -282,6 +309,33 @@ __device__ __forceinline__ TileInfo g2_take(const G2Smem& sm, int q, uint32_t ph
     if (WARP) __syncwarp();
     if (release_lane) ptx::mbar_arrive_cluster_relaxed(ptx::mapa(sm.ti_empty(q), 0), w[0] ^ w[15]);
     return ti;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Finisher (one warp of the PEER CTA, which has no scheduler and no MMA issuer to run): per tile it waits until the
+// epilogue warps of both CTAs have reported that their stores are in global memory, then `done(ti)` counts the tile
+// and, for the last tile of a GEMM, runs the slot's transition. The epilogue warps never wait for the completion of
+// their stores, for the counting atomic or for a transition: per tile that was a CTA-wide barrier, a bulk-store wait, a
+// fence and an atomic round trip on the epilogue's path, more than the k-loop of a 560-wide tile.
+// The ring entry is released only after the tile is complete, so the epilogue can never be a full ring ahead of it.
+// ------------------------------------------------------------------------------------------------
+template <typename Done>
+__device__ __forceinline__ void g2_finisher(const G2Smem& sm, int lane, Done done, volatile int* abort_flag) {
+    int q = 0; uint32_t tph = 0;
+    for (;;) {
+        const TileInfo ti = g2_take<true>(sm, q, tph, false, abort_flag);
+        if (!ti.valid) {
+            if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_empty(q), 0));
+            break;
+        }
+        if (!ptx::mbar_wait_cluster_patient(sm.cdone(q), tph, abort_flag)) break;
+        if (lane == 0) {
+            ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_empty(q), 0));
+            done(ti);
+        }
+        __syncwarp();
+        if (++q == G2_NTI) { q = 0; tph ^= 1; }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -294,11 +348,13 @@ __device__ __forceinline__ TileInfo g2_take(const G2Smem& sm, int q, uint32_t ph
 __device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap* maps, uint32_t rank, int lane, int want_lead, volatile int* abort_flag) {
     int stage = 0; uint32_t phase = 0;
     int q = 0; uint32_t tph = 0;
+    uint32_t started = 0;                                                   // tiles that have reached their claim point
     const uint32_t full0 = ptx::mapa(sm.full(0), 0);                        // the leader's full barriers
     for (;;) {
         const TileInfo ti = g2_take<true>(sm, q, tph, lane == 0, abort_flag);
         if (++q == G2_NTI) { q = 0; tph ^= 1; }
         if (!ti.valid) break;
+        ++started;
         ptx::fence_proxy_async();      // operands may have been written by generic stores of another CTA
         const CUtensorMap* map_a = maps + (size_t)ti.slot * NMAP + ti.a_buf;
         const CUtensorMap* map_b = maps + (size_t)ti.slot * NMAP + ti.b_buf;
@@ -314,7 +370,7 @@ __device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap*
         for (int kb = 0; kb < nkb; ++kb) {
             if (!ptx::mbar_wait(sm.empty(stage), phase ^ 1, abort_flag)) return;
             if (ptx::elect_one()) {
-                if (kb == kb_want) ptx::mbar_arrive(sm.want());            // the scheduler may claim the next tile now
+                if (kb == kb_want) ptx::st_shared_volatile_u32(sm.want(), started);   // the scheduler may claim the next tile now
                 const uint32_t fb = full0 + 8u * stage;
                 if (rank == 0) ptx::mbar_expect_tx(sm.full(stage), bytes);
                 const uint32_t sa = sm.stage_a(stage), sb = sm.stage_b(stage);
@@ -354,7 +410,10 @@ __device__ __forceinline__ void umma_f16_pair_x4(uint32_t d_tmem, uint64_t a_des
 }
 }  // namespace ptx
 
-__device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int lane, volatile int* abort_flag) {
+// mma_ns (nullable): [0] waiting for a tile record, [1] waiting for a free accumulator (the epilogue), [2] inside k-loops
+// (operand waits + issue), summed over the leader CTAs, nanoseconds (three timer reads per tile).
+__device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int lane, volatile int* abort_flag, unsigned long long* mma_ns) {
+    unsigned long long t_take = 0, t_acc = 0, t_k = 0;
     int stage = 0; uint32_t phase = 0;
     int acc = 0; uint32_t acc_phase = 0;
     int q = 0; uint32_t tph = 0;
@@ -362,14 +421,17 @@ __device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int
     const uint64_t da0 = make_smem_desc(sm.stage_a(0), 16, 1024);
     const uint64_t db0 = make_smem_desc(sm.stage_b(0), B_BOX_BYTES, 1024);
     for (;;) {
+        const unsigned long long t0 = ptx::globaltimer_ns();
         const TileInfo ti = g2_take<true>(sm, q, tph, lane == 0, abort_flag);
         if (++q == G2_NTI) { q = 0; tph ^= 1; }
         if (!ti.valid) break;
+        const unsigned long long t1 = ptx::globaltimer_ns();
         const int nkb = (ti.n16 + BK - 1) / BK;
         const int ktail = (ti.n16 - (nkb - 1) * BK) >> 4;          // 16-k slices of the last k-block (1..4)
         const uint32_t idesc = make_idesc_f16((ti.valid & TI_HALF) ? 128 : 256, ti.bn);
         if (!ptx::mbar_wait_cluster(sm.tempty(acc), acc_phase ^ 1, abort_flag)) return;
         ptx::tc_fence_after();
+        const unsigned long long t2 = ptx::globaltimer_ns();
         const uint32_t d_tmem = tmem_base + acc * 256;
 #pragma unroll 1
         for (int kb = 0; kb < nkb; ++kb) {
@@ -391,13 +453,15 @@ __device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int
             if (++stage == G2_STAGES) { stage = 0; phase ^= 1; }
         }
         if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+        t_take += t1 - t0; t_acc += t2 - t1; t_k += ptx::globaltimer_ns() - t2;
     }
+    if (mma_ns && lane == 0) { atomicAdd(&mma_ns[0], t_take); atomicAdd(&mma_ns[1], t_acc); atomicAdd(&mma_ns[2], t_k); }
 }
 
 // ------------------------------------------------------------------------------------------------
 // Epilogue (warps 0..7 of each CTA): C = c_out * acc + beta * I, FP16 stores, fused squared
-// residual || alpha_res A B - I ||_F^2 (the convergence test, C-7). `done(ti)` is called by one
-// thread of the CTA after all of the CTA's stores of the tile have been issued and fenced.
+// residual || alpha_res A B - I ||_F^2 (the convergence test, C-7). Every warp reports to the finisher
+// (g2_finisher) once its stores of the tile are in global memory.
 //
 // TI_MIRROR (symmetric products): only the tiles on and above the diagonal of the tile grid are
 // multiplied; an off-diagonal tile also writes its transpose into the block below the diagonal (lanes of a warp are
@@ -414,9 +478,9 @@ __device__ __forceinline__ void st_mirror(__half* Ct /* &C[col_first][row] */, i
     }
 }
 
-template <typename Eng, typename Done>
+template <typename Eng>
 __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base, const Eng& e, __half* base,
-                                            uint32_t rank, int warp, int lane, Done done, const CUtensorMap* maps, volatile int* abort_flag) {
+                                            uint32_t rank, int warp, int lane, const CUtensorMap* maps, volatile int* abort_flag) {
     int acc = 0; uint32_t acc_phase = 0;
     int q = 0; uint32_t tph = 0;
     const uint32_t tempty0 = ptx::mapa(sm.tempty(0), 0);
@@ -425,6 +489,7 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
     bool stalled = false;
     for (;;) {
         const TileInfo ti = g2_take<true>(sm, q, tph, lane == 0, abort_flag);
+        const uint32_t cdone_peer = ptx::mapa(sm.cdone(q), 1);
         if (++q == G2_NTI) { q = 0; tph ^= 1; }
         if (!ti.valid) break;
         const int n = ti.n, n16 = ti.n16;
@@ -615,15 +680,15 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
             for (int o = 16; o > 0; o >>= 1) rsum += __shfl_xor_sync(0xffffffffu, rsum, o);
             if (lane == 0 && rsum != 0.f) atomicAdd(&e.slots[ti.slot].res_acc, rsum);
         }
-        asm volatile("bar.sync 1, %0;" ::"n"(G2_EPI_WARPS * 32) : "memory");   // the CTA's epilogue warps
-        if (warp == 0 && lane == 0) done(ti);
+        // this warp's stores of the tile are in global memory (the TMA stores of its row group: the issuer waited for them)
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive_cluster(cdone_peer);
         if (++acc == 2) { acc = 0; acc_phase ^= 1; }
     }
     if (stalled) {
         // a warp that gives up on a stalled wait releases the named barriers its peers may be waiting at (they stall and
         // leave at their next wait)
         asm volatile("bar.arrive %0, 128;" ::"r"(3 + g) : "memory");
-        asm volatile("bar.arrive 1, %0;" ::"n"(G2_EPI_WARPS * 32) : "memory");
     }
 }
 

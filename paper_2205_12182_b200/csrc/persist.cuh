@@ -2,7 +2,8 @@
 //
 // grid = one CTA per SM in clusters of two (one tcgen05 CTA pair per tile, gemm2sm.cuh); every CTA runs
 //   warps 0-10   the grouped tcgen05 GEMM pipeline of gemm2sm.cuh (epilogue x 8, tile scheduler, TMA
-//                producer, MMA issuer), fed from a device-side claim table instead of a static tile list;
+//                producer, MMA issuer in the leader CTA / tile finisher in the peer CTA), fed from a device-side
+//                claim table instead of a static tile list;
 //   warps 11-14  a SIDE GROUP that executes the O(n^2) steps of the path as small tasks: gather
 //                (PAPER.md:L56, L60), the closed-form first iteration steps, diagonal shifts, and D columns +
 //                scatter + energy (Eq. 4).
@@ -57,7 +58,8 @@ enum { PC_TILES = 0, PC_SCHED_IDLE_NS, PC_SCHED_BUSY_NS, PC_OVERSHOOT, PC_T_STAR
        PC_SIDE_NS,            // + kind
        PC_SIDE_BYTES = PC_SIDE_NS + 8,   // + kind (algorithmic bytes)
        PC_SIDE_TASKS = PC_SIDE_BYTES + 8,
-       PC_LEN = PC_SIDE_TASKS + 8 };
+       PC_MMA_NS = PC_SIDE_TASKS + 8,    // + 0 tile-record wait, 1 accumulator wait, 2 k-loops (MMA warps of the leader CTAs)
+       PC_LEN = PC_MMA_NS + 3 };
 
 constexpr int OPF_RES = 1;        // op flags: fused residual wanted
 constexpr int OPF_SYM = 2;        // symmetric product: upper-triangle tiles, mirrored stores
@@ -329,7 +331,7 @@ __device__ __forceinline__ void p_begin_sign_chain(const PEngine& e, int slot) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// GEMM side: called by one thread per CTA per finished tile (after the CTA's stores and residual
+// GEMM side: called by the finisher of a CTA pair once per finished tile (after the pair's stores and residual
 // atomics). The last report of the op runs the slot's transition (C-7) and installs what comes next.
 // ------------------------------------------------------------------------------------------------
 // Convergence rule C-7 on the residual r of an inverse-type (inv) or sign iteration. Returns true when the iteration
@@ -466,65 +468,73 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
     int q = 0; uint32_t ph = 0;
     unsigned long long idle_ns = 0, ntiles = 0, overshoot = 0;
     const unsigned long long t_begin = pl::gtime();
+    bool short_tiles = false;
+    // tiles claimed and not yet published (lane 0): tiles [pend_t, pend_end) of the op whose record is cached below
+    int pend_t = 0, pend_end = 0, pend_slot = 0, pend_nt = 0;
+    int4 g0 = make_int4(0, 0, 0, 0), g1 = g0, o0 = g0;
+    float4 o1 = make_float4(0.f, 0.f, 0.f, 0.f);
     for (;;) {
         if (!ptx::mbar_wait_cluster_patient(sm.ti_empty(q), ph ^ 1, e.abort_flag)) break;
         // Claim lazily: only when the producer has issued every load of the tile before and needs the next
         // record (it runs G2_STAGES k-blocks ahead of the MMA, which hides the claim). A pair that claimed
         // further ahead would hoard tiles of a GEMM that idle pairs could run at the same time, and the
         // slot's chain of dependent GEMMs would take that much longer.
-        if (!ptx::mbar_wait(sm.want(), (uint32_t)(ntiles & 1) ^ 1u, e.abort_flag)) break;
+        {
+            // short tiles (k-loop of a few microseconds): the claim - slot scan, atomic, slot record - takes as long as the tile,
+            // so the scheduler may be three tiles ahead of the producer's claim points instead of one
+            const int credits = short_tiles ? 3 : 1;
+            uint32_t spins = 0; unsigned long long t0 = 0;
+            bool stalled = false;
+            while ((int)((uint32_t)ntiles - ptx::ld_shared_volatile_u32(sm.want())) >= credits) {
+                __nanosleep(32);
+                if ((++spins & 0xFFFFu) == 0 && ptx::stalled(t0, e.abort_flag)) { stalled = true; break; }
+            }
+            if (stalled) break;
+        }
         TileInfo ti{};
-        int got = 0, tflags = 0;
+        int got = __shfl_sync(0xffffffffu, pend_t < pend_end ? 1 : 0, 0), tflags = 0;
         unsigned long long t_idle0 = 0;
-        for (;;) {
+        while (!got) {
+            // scan of the claim table in slot order: all words of a lane are loaded before the first ballot
+            unsigned long long w3[3];
+#pragma unroll
+            for (int r = 0; r < 3; ++r) {
+                const int sidx = 32 * r + lane;
+                w3[r] = sidx < e.S ? *(volatile unsigned long long*)&e.gclaim[sidx] : 0ull;
+            }
             int found = -1;
-            for (int base = 0; base < e.S; base += 32) {
+            unsigned long long wf = 0;
+#pragma unroll
+            for (int r = 0; r < 3; ++r) {
+                const bool avail = (unsigned)(w3[r] & 0xFFFFFu) < (unsigned)((w3[r] >> 20) & 0xFFFFFu);
+                const unsigned m = __ballot_sync(0xffffffffu, avail);
+                if (m && found < 0) { found = 32 * r + __ffs(m) - 1; wf = __shfl_sync(0xffffffffu, w3[r], __ffs(m) - 1); }
+            }
+            for (int base = 96; base < e.S && found < 0; base += 32) {      // more than 96 slots (never by default)
                 const int sidx = base + lane;
                 const unsigned long long w = sidx < e.S ? *(volatile unsigned long long*)&e.gclaim[sidx] : 0ull;
                 const bool avail = (unsigned)(w & 0xFFFFFu) < (unsigned)((w >> 20) & 0xFFFFFu);
                 const unsigned m = __ballot_sync(0xffffffffu, avail);
-                if (m) { found = base + __ffs(m) - 1; break; }
+                if (m) { found = base + __ffs(m) - 1; wf = __shfl_sync(0xffffffffu, w, __ffs(m) - 1); }
             }
             if (found >= 0) {
+                // one tile per claim (three per claim for GEMMs of at most nine tiles was measured on cfg1: no faster without
+                // combination, slower in the Loewdin form - the tiles of a GEMM should spread over pairs, not queue on one)
+                (void)wf;
+                const int k = 1;
                 unsigned long long w = 0;
-                if (lane == 0) w = atomicAdd(&e.gclaim[found], 1ull);
+                if (lane == 0) w = atomicAdd(&e.gclaim[found], (unsigned long long)k);
                 w = __shfl_sync(0xffffffffu, w, 0);
-                int t = (int)(w & 0xFFFFFu);
-                const int nt = (int)((w >> 20) & 0xFFFFFu);
+                const int t = (int)(w & 0xFFFFFu), nt = (int)((w >> 20) & 0xFFFFFu);
                 if (t < nt) {
                     if (lane == 0) {
                         __threadfence();
                         const PSlot* s = &e.slots[found];
-                        const int4 g0 = __ldcg(reinterpret_cast<const int4*>(&s->atom));     // atom n n16 pos
-                        const int4 g1 = __ldcg(reinterpret_cast<const int4*>(&s->nbi));      // nbi ntm nset unit
-                        const int4 o0 = __ldcg(reinterpret_cast<const int4*>(&s->op_kind));
-                        const float4 o1 = __ldcg(reinterpret_cast<const float4*>(&s->c_out));
-                        const int flags = __float_as_int(o1.w), ntm = g1.y;
-                        ti.slot = found;
-                        tflags = TI_VALID;
-                        if (flags & OPF_NARROW) {
-                            ti.m0 = t * BM;
-                            tflags |= TI_PLAIN;
-                            if (o0.x == OP_DCOLS) { ti.n0 = g0.w & ~7; ti.bn = PCW; tflags |= TI_F32OUT; }   // D columns: the aligned window around pos(i)
-                            else if (o0.x == OP_DCOLS2) { ti.n0 = 0; ti.bn = PCW; tflags |= TI_F32OUT; }      // B operand: the W block
-                            else { ti.n0 = 0; ti.bn = NVC; }                                                  // power iteration
-                        } else {
-                            int tm, tn;
-                            if ((flags & OPF_SYM) && e.sym_tiles) {          // tiles on and above the diagonal, row by row
-                                tm = 0;
-                                while (t >= ntm - tm) { t -= ntm - tm; ++tm; }
-                                tn = tm + t;
-                                tflags |= tn > tm ? TI_MIRROR : TI_SYMDIAG;
-                            } else {
-                                tm = t / ntm; tn = t - tm * ntm;
-                            }
-                            ti.m0 = tm * BM; ti.n0 = tn * BN; ti.bn = min(BN, g0.z - tn * BN);
-                            // the last row block when at most 128 rows are left: one M = 128 MMA per 16 k instead of M = 256
-                            if (g0.z - tm * BM <= BM / 2 && (ti.bn & 31) == 0) tflags |= TI_HALF;
-                        }
-                        ti.n = g0.y; ti.n16 = g0.z; ti.nreports = 2 * nt;
-                        ti.kind = o0.x; ti.a_buf = o0.y; ti.b_buf = o0.z; ti.c_buf = o0.w;
-                        ti.c_out = o1.x; ti.alpha_res = o1.y; ti.beta = o1.z; ti.want_res = flags & OPF_RES;
+                        g0 = __ldcg(reinterpret_cast<const int4*>(&s->atom));     // atom n n16 pos
+                        g1 = __ldcg(reinterpret_cast<const int4*>(&s->nbi));      // nbi ntm nset unit
+                        o0 = __ldcg(reinterpret_cast<const int4*>(&s->op_kind));
+                        o1 = __ldcg(reinterpret_cast<const float4*>(&s->c_out));
+                        pend_t = t; pend_end = min(t + k, nt); pend_slot = found; pend_nt = nt;
                     }
                     got = 1;
                     break;
@@ -538,6 +548,35 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
         }
         if (t_idle0) idle_ns += pl::gtime() - t_idle0;
         ntiles += got;
+        if (got && lane == 0) {
+            int t = pend_t++;
+            const int flags = __float_as_int(o1.w), ntm = g1.y;
+            ti.slot = pend_slot;
+            tflags = TI_VALID;
+            if (flags & OPF_NARROW) {
+                ti.m0 = t * BM;
+                tflags |= TI_PLAIN;
+                if (o0.x == OP_DCOLS) { ti.n0 = g0.w & ~7; ti.bn = PCW; tflags |= TI_F32OUT; }   // D columns: the aligned window around pos(i)
+                else if (o0.x == OP_DCOLS2) { ti.n0 = 0; ti.bn = PCW; tflags |= TI_F32OUT; }      // B operand: the W block
+                else { ti.n0 = 0; ti.bn = NVC; }                                                  // power iteration
+            } else {
+                int tm, tn;
+                if ((flags & OPF_SYM) && e.sym_tiles) {          // tiles on and above the diagonal, row by row
+                    tm = 0;
+                    while (t >= ntm - tm) { t -= ntm - tm; ++tm; }
+                    tn = tm + t;
+                    tflags |= tn > tm ? TI_MIRROR : TI_SYMDIAG;
+                } else {
+                    tm = t / ntm; tn = t - tm * ntm;
+                }
+                ti.m0 = tm * BM; ti.n0 = tn * BN; ti.bn = min(BN, g0.z - tn * BN);
+                // the last row block when at most 128 rows are left: one M = 128 MMA per 16 k instead of M = 256
+                if (g0.z - tm * BM <= BM / 2 && (ti.bn & 31) == 0) tflags |= TI_HALF;
+            }
+            ti.n = g0.y; ti.n16 = g0.z; ti.nreports = pend_nt;
+            ti.kind = o0.x; ti.a_buf = o0.y; ti.b_buf = o0.z; ti.c_buf = o0.w;
+            ti.c_out = o1.x; ti.alpha_res = o1.y; ti.beta = o1.z; ti.want_res = flags & OPF_RES;
+        }
         if (lane == 0) ti.valid = got ? tflags : 0;
         const uint32_t* w = reinterpret_cast<const uint32_t*>(&ti);
         uint32_t mine = 0;
@@ -546,13 +585,13 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
             const uint32_t v = __shfl_sync(0xffffffffu, w[i], 0);
             if (lane == i) mine = v;
         }
+        short_tiles = __shfl_sync(0xffffffffu, ti.n16, 0) <= 768;
         if (lane < 16) {
 #pragma unroll
             for (uint32_t rk = 0; rk < 2u; ++rk)
-                ptx::st_cluster_u32(ptx::mapa(sm.tinfo(q), rk) + 4u * lane, mine);
+                ptx::st_async_u32(ptx::mapa(sm.tinfo(q), rk) + 4u * lane, mine, ptx::mapa(sm.ti_full(q), rk));
         }
-        __syncwarp();
-        if (lane < 2) ptx::mbar_arrive_cluster(ptx::mapa(sm.ti_full(q), (uint32_t)lane));
+        if (lane < 2) ptx::mbar_arrive_expect_tx_cluster(ptx::mapa(sm.ti_full(q), (uint32_t)lane), 64u);
         if (!got) break;
         if (++q == G2_NTI) { q = 0; ph ^= 1; }
     }
@@ -974,13 +1013,14 @@ nolsm_persist_kernel(const __grid_constant__ PEngine e) {
     const uint32_t tmem_base = g2_setup(sm, warp, lane);
 
     if (warp < G2_EPI_WARPS) {
-        g2_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, done, e.maps, e.abort_flag);
+        g2_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, e.maps, e.abort_flag);
     } else if (warp == G2_WARP_SCHED) {
         if (rank == 0) p_scheduler(sm, e, lane);
     } else if (warp == G2_WARP_TMA) {
         g2_producer(sm, e.maps, rank, lane, e.want_lead, e.abort_flag);
     } else if (warp == G2_WARP_MMA) {
-        if (rank == 0) g2_mma(sm, tmem_base, lane, e.abort_flag);
+        if (rank == 0) g2_mma(sm, tmem_base, lane, e.abort_flag, &e.ctr[PC_MMA_NS]);
+        else g2_finisher(sm, lane, done, e.abort_flag);
     } else {
         p_side_loop(e, side_sm, (int)threadIdx.x - G2_CTRL_THREADS);
     }

@@ -442,6 +442,22 @@ def main():
                 cx = Nolsm(local_rank)
                 if name != "cfg4":
                     others[name] = measure(cx, ao, so, Do, stream, world, dev, steps=2 if name == "cfg1" else 1)
+                    if name == "cfg1":
+                        # chemical-potential search for half filling: trial mu per pass on the resident
+                        # S_sub^-1 and A0 (nolsm_electron_counts) against one trial per pass
+                        target = 0.5 * float(so.atom_nb.sum())
+                        mu_search = {"target_electrons": target, "bracket": [-2.0, 2.0], "tol_n": 0.5}
+                        for k in (1, 3, 7):
+                            cm = Nolsm(local_rank, mu_trials=k)
+                            cm.assemble(*ao, stream=stream)
+                            torch.cuda.synchronize()
+                            t0 = time.perf_counter()
+                            mu_f, n_f, ev = cm.find_mu(target, -2.0, 2.0, Do, tol_n=0.5, tol_mu=1e-5, stream=stream)
+                            torch.cuda.synchronize()
+                            mu_search[f"trials_per_pass_{k}"] = {"mu": mu_f, "electrons": n_f, "trial_mu_evaluated": ev,
+                                                                 "seconds": time.perf_counter() - t0}
+                            cm.destroy()
+                        others["cfg1"]["mu_search"] = mu_search
                 else:
                     nbatch = 4
                     edges = [so.n_atoms * b // nbatch for b in range(nbatch + 1)]

@@ -99,8 +99,13 @@ typedef struct {
     int heavy_slots;         /* persistent engine: submatrices inside the GEMM chains at once [0 = auto: L2 size / (3.5 n^2 FP16)] */
     int claim_lead;          /* persistent engine: a CTA pair claims its next tile when its TMA producer is this many k-blocks
                                 from the end of the current one [14] */
-    int mu_trials;           /* nolsm_find_mu, persistent engine: trial mu evaluated per pass on the resident S_sub^-1, A0 [3; max 8] */
+    int mu_trials;           /* nolsm_find_mu, persistent engine: trial mu evaluated per pass on the resident S_sub^-1, A0 [1 = bisection:
+                                a trial after the first costs ~3/4 of a pass and K trials gain log2(K + 1) bits, so K = 1 needs the
+                                least work per bit (measured: bench.py other_configs.cfg1.mu_search); max 8] */
     double timeout_s;        /* persistent engine: the host stops a kernel that runs longer than this [300] */
+    int l2_load_policy;      /* persistent engine: L2 eviction priority of the TMA operand loads: 1 evict_first, 2 evict_last, 3 normal [1] */
+    int l2_store_policy;     /* the same for the TMA stores of the GEMM results [2: a result stays in L2 until the next GEMM of its
+                                chain reads it instead of being pushed out by operand traffic; measured +5 % on configs[2]] */
 } nolsm_options;
 
 typedef struct {

@@ -323,7 +323,7 @@ int nolsm_find_mu(nolsm_ctx* c, double n_target, double mu_lo, double mu_hi, dou
         if ((r = soften(nolsm_energy(c, &e)))) return r;       // flagged matrices are still written (nolsm.h)
         return nolsm_electron_count(c, n, nullptr);
     };
-    const int K = c->persist ? std::max(1, std::min(c->opt.mu_trials > 0 ? c->opt.mu_trials : 3, NOLSM_MAX_MU)) : 1;
+    const int K = c->persist ? std::max(1, std::min(c->opt.mu_trials > 0 ? c->opt.mu_trials : 1, NOLSM_MAX_MU)) : 1;
     double mu = mu_hi, n_mu = 0;
     int r;
     if (c->persist) {

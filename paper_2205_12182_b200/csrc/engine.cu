@@ -435,6 +435,7 @@ int engine_plan(nolsm_ctx* c, cudaStream_t s) {
         pe.g_max = std::max(1, std::min(g_max, S));
         pe.want_lead = c->opt.claim_lead > 0 ? c->opt.claim_lead : G2_WANT_LEAD;
         pe.lowdin = c->opt.iteration == NOLSM_ITER_LOWDIN ? 1 : 0;
+        pe.l2_load = c->opt.l2_load_policy > 0 ? c->opt.l2_load_policy : 1; pe.l2_store = c->opt.l2_store_policy > 0 ? c->opt.l2_store_policy : 2;
         pe.sym_tiles = c->opt.symmetric_tiles >= 0 ? 1 : 0;
         pe.n_mu = 1; pe.count_only = 0;
         pe.nelec_mu = c->d_mu_acc; pe.e_mu = c->d_mu_acc + NOLSM_MAX_MU;

@@ -186,11 +186,22 @@ __device__ __forceinline__ void st_shared_volatile_u32(uint32_t addr, uint32_t v
     asm volatile("st.volatile.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 // TMA load whose completion bytes are credited to an mbarrier of either CTA of the pair.
-__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar_cluster) {
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar_cluster, uint64_t policy) {
     asm volatile(
-        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes"
-        " [%0], [%1, {%2, %3}], [%4];"
-        ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar_cluster) : "memory");
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%2, %3}], [%4], %5;"
+        ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar_cluster), "l"(policy) : "memory");
+}
+// L2 eviction-priority policy for the bulk copies: 1 evict_first, 2 evict_last, else evict_normal.
+// The engine loads every operand with evict_first and stores every GEMM result with evict_last: a result must survive in
+// L2 until the next GEMM of its chain reads it, some tens of microseconds and several hundred MB of operand traffic later;
+// with equal priorities the operand traffic pushes it out to HBM first (measured on cfg2: +5 %, profiles/r02_persist.md).
+__device__ __forceinline__ uint64_t l2_policy(int kind) {
+    uint64_t p;
+    if (kind == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    else if (kind == 2) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+    return p;
 }
 __device__ __forceinline__ void tmem_alloc_pair(uint32_t smem_dst, uint32_t ncols) {
     asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
@@ -214,9 +225,9 @@ __device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 // TMA store of one box from shared memory (bulk async-group completion)
-__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, int c0, int c1, uint32_t src) {
-    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group [%0, {%1, %2}], [%3];"
-                 ::"l"(map), "r"(c0), "r"(c1), "r"(src) : "memory");
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, int c0, int c1, uint32_t src, uint64_t policy) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group.L2::cache_hint [%0, {%1, %2}], [%3], %4;"
+                 ::"l"(map), "r"(c0), "r"(c1), "r"(src), "l"(policy) : "memory");
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N>
@@ -345,7 +356,8 @@ __device__ __forceinline__ void g2_finisher(const G2Smem& sm, int lane, Done don
 // values of its operands; the k-block then took ~650 cycles whatever the tile's width, the producer was busy 85 % of the
 // time and the MMA warp waited for operands: profiles/r02_persist.md.)
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap* maps, uint32_t rank, int lane, int want_lead, volatile int* abort_flag) {
+__device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap* maps, uint32_t rank, int lane, int want_lead, volatile int* abort_flag, int l2_load) {
+    const uint64_t pol = ptx::l2_policy(l2_load);
     int stage = 0; uint32_t phase = 0;
     int q = 0; uint32_t tph = 0;
     uint32_t started = 0;                                                   // tiles that have reached their claim point
@@ -375,10 +387,10 @@ __device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap*
                 if (rank == 0) ptx::mbar_expect_tx(sm.full(stage), bytes);
                 const uint32_t sa = sm.stage_a(stage), sb = sm.stage_b(stage);
                 const int k0 = kb * BK;
-                ptx::tma_load_2d_pair(sa, map_a, k0, row0, fb);
-                if (!hh) ptx::tma_load_2d_pair(sa + 8192, map_a, k0, row0 + 64, fb);
-                ptx::tma_load_2d_pair(sb, map_b, col0, k0, fb);
-                if (nbox > 1) ptx::tma_load_2d_pair(sb + B_BOX_BYTES, map_b, col0 + 64, k0, fb);
+                ptx::tma_load_2d_pair(sa, map_a, k0, row0, fb, pol);
+                if (!hh) ptx::tma_load_2d_pair(sa + 8192, map_a, k0, row0 + 64, fb, pol);
+                ptx::tma_load_2d_pair(sb, map_b, col0, k0, fb, pol);
+                if (nbox > 1) ptx::tma_load_2d_pair(sb + B_BOX_BYTES, map_b, col0 + 64, k0, fb, pol);
             }
             __syncwarp();
             if (++stage == G2_STAGES) { stage = 0; phase ^= 1; }
@@ -480,7 +492,8 @@ __device__ __forceinline__ void st_mirror(__half* Ct /* &C[col_first][row] */, i
 
 template <typename Eng>
 __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base, const Eng& e, __half* base,
-                                            uint32_t rank, int warp, int lane, const CUtensorMap* maps, volatile int* abort_flag) {
+                                            uint32_t rank, int warp, int lane, const CUtensorMap* maps, volatile int* abort_flag, int l2_store) {
+    const uint64_t pol = ptx::l2_policy(l2_store);
     int acc = 0; uint32_t acc_phase = 0;
     int q = 0; uint32_t tph = 0;
     const uint32_t tempty0 = ptx::mapa(sm.tempty(0), 0);
@@ -586,8 +599,8 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                 asm volatile("bar.sync %0, 128;" ::"r"(3 + g) : "memory");
                 if (issuer) {
                     if (brow < n16) {                              // boxes below the matrix are padding
-                        ptx::tma_store_2d(map_c, bcol, brow, box);
-                        if (mode == 1) ptx::tma_store_2d(map_c, brow, bcol, boxt);
+                        ptx::tma_store_2d(map_c, bcol, brow, box, pol);
+                        if (mode == 1) ptx::tma_store_2d(map_c, brow, bcol, boxt, pol);
                     }
                     ptx::bulk_commit();
                 }

@@ -96,6 +96,7 @@ struct PEngine {
     int* heavy;                   // [1] slots inside the GEMM-heavy phases right now (at most g_max)
     int* parked;                  // [S] 1 = the slot is ready for a heavy phase and waits for a token
     int g_max, want_lead;
+    int l2_load, l2_store;        // L2 eviction priority of the operand loads / of the stores of C (1 evict_first, 2 evict_last, 3 normal)
     int lowdin;                   // 0: Eq. 6 on A = S^-1 H0 - mu I; 1: symmetric (Loewdin) form
     int sym_tiles;                // 1: symmetric products multiply the upper triangle of tiles only
     int n_mu; float mu[P_MAX_MU]; // trial chemical potentials of this call (1 for nolsm_density_matrix)
@@ -173,7 +174,7 @@ __device__ __forceinline__ void p_install_gemm(const PEngine& e, int slot, int k
         case OP_INV_G1: a = 0; b = ycur; c = 4; c_out = -1.f; beta = 2.f; flags = OPF_RES | OPF_SYM; break;     // R = 2I - S Y
         case OP_INV_G2: a = ycur; b = 4; c = 5 - ycur; flags = OPF_SYM; break;                                   // Y <- Y R
         case OP_AMAT:                                                                                            // A = Y H0 - mu I (A0 = Y H0 with several trial mu)
-            a = ycur; b = 1;
+            a = ycur; b = 1; 
             if (e.n_mu > 1) { c = 5; __stcg(&s->abuf, 5); } else { c = 0; beta = -e.mu[0]; }
             break;
         case OP_SIGN_G1: {                                                                          // T = 3I - alpha^2 X^2
@@ -1013,11 +1014,11 @@ nolsm_persist_kernel(const __grid_constant__ PEngine e) {
     const uint32_t tmem_base = g2_setup(sm, warp, lane);
 
     if (warp < G2_EPI_WARPS) {
-        g2_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, e.maps, e.abort_flag);
+        g2_epilogue(sm, tmem_base, e, e.base, rank, warp, lane, e.maps, e.abort_flag, e.l2_store);
     } else if (warp == G2_WARP_SCHED) {
         if (rank == 0) p_scheduler(sm, e, lane);
     } else if (warp == G2_WARP_TMA) {
-        g2_producer(sm, e.maps, rank, lane, e.want_lead, e.abort_flag);
+        g2_producer(sm, e.maps, rank, lane, e.want_lead, e.abort_flag, e.l2_load);
     } else if (warp == G2_WARP_MMA) {
         if (rank == 0) g2_mma(sm, tmem_base, lane, e.abort_flag, &e.ctr[PC_MMA_NS]);
         else g2_finisher(sm, lane, done, e.abort_flag);

@@ -103,6 +103,9 @@ typedef struct {
                                 a trial after the first costs ~3/4 of a pass and K trials gain log2(K + 1) bits, so K = 1 needs the
                                 least work per bit (measured: bench.py other_configs.cfg1.mu_search); max 8] */
     double timeout_s;        /* persistent engine: the host stops a kernel that runs longer than this [300] */
+    int scan_order;          /* persistent engine, tile schedulers: 1 = every CTA pair scans the slots from slot 0 (the chains of the first
+                                slots advance first), 2 = every pair from its own slot (74 schedulers do not queue on one claim word)
+                                [0 = auto: 2 for mean dimensions up to 768, where a tile is as short as a claim] */
     int l2_load_policy;      /* persistent engine: L2 eviction priority of the TMA operand loads: 1 evict_first, 2 evict_last, 3 normal [1] */
     int l2_store_policy;     /* the same for the TMA stores of the GEMM results [2: a result stays in L2 until the next GEMM of its
                                 chain reads it instead of being pushed out by operand traffic; measured +5 % on configs[2]] */
@@ -240,9 +243,11 @@ int nolsm_get_profile(nolsm_ctx* ctx, double* out, int n);
  *   out[9 + k], out[17 + k], out[25 + k]  side tasks of kind k (1 refill, 2 gather, 3 elementwise steps,
  *   4 D columns + scatter, 5 W columns of the Loewdin form): busy ms summed over side groups, algorithmic bytes, tasks;
  *   out[33..35] where the MMA-issuing warps (one per CTA pair) spent the kernel, ms summed over the pairs: waiting for a
- *   tile record, waiting for a free accumulator (= for the epilogue), inside k-loops (operand waits + issue).
+ *   tile record, waiting for a free accumulator (= for the epilogue), inside k-loops (operand waits + issue);
+ *   out[36..37] the tile schedulers, ms summed over the pairs: waiting for a free entry of the record ring (= for the
+ *   completion of the tile four back), waiting for the producer's claim point.
  *   n must be >= NOLSM_COUNTERS_LEN. Synchronises. */
-#define NOLSM_COUNTERS_LEN 36
+#define NOLSM_COUNTERS_LEN 38
 int nolsm_get_engine_counters(nolsm_ctx* ctx, double* out, int n);
 
 /* HBM-bound side tasks timed alone: which = 0 the gather of every submatrix of the assembled system (a1),

@@ -27,7 +27,7 @@ class NolsmOptions(C.Structure):
                 ("combine", C.c_int), ("combine_max_dim", C.c_int),
                 ("combine_max_members", C.c_int), ("combine_max_candidates", C.c_int), ("iteration", C.c_int),
                 ("symmetric_tiles", C.c_int), ("heavy_slots", C.c_int), ("claim_lead", C.c_int), ("mu_trials", C.c_int),
-                ("timeout_s", C.c_double), ("l2_load_policy", C.c_int), ("l2_store_policy", C.c_int)]
+                ("timeout_s", C.c_double), ("scan_order", C.c_int), ("l2_load_policy", C.c_int), ("l2_store_policy", C.c_int)]
 
 
 class NolsmStats(C.Structure):
@@ -263,13 +263,14 @@ class Nolsm:
 
     def engine_counters(self) -> dict:
         """Counters of the persistent engine for the last density_matrix call (include/nolsm.h)."""
-        out = (C.c_double * 36)()
-        self._check(self._lib.nolsm_get_engine_counters(self._h, out, 36))
+        out = (C.c_double * 38)()
+        self._check(self._lib.nolsm_get_engine_counters(self._h, out, 38))
         v = list(out)
         kinds = ("none", "refill", "gather", "elementwise", "dcols", "wcols", "k6", "k7")
         d = {"persistent": bool(v[0]), "kernel_ms": v[1], "kernel_ms_device_clock": v[2], "tiles": v[3],
              "sched_idle_ms": v[4], "sched_busy_ms": v[5], "overshoots": v[6], "slots": int(v[7]), "pairs": int(v[8])}
         d["mma_wait_record_ms"], d["mma_wait_accumulator_ms"], d["mma_kloop_ms"] = v[33], v[34], v[35]
+        d["sched_wait_ring_ms"], d["sched_wait_claim_point_ms"] = v[36], v[37]
         d["side"] = {k: {"busy_ms": v[9 + i], "bytes": v[17 + i], "tasks": v[25 + i]} for i, k in enumerate(kinds)
                      if v[25 + i] > 0}
         return d

@@ -435,6 +435,7 @@ int engine_plan(nolsm_ctx* c, cudaStream_t s) {
         pe.g_max = std::max(1, std::min(g_max, S));
         pe.want_lead = c->opt.claim_lead > 0 ? c->opt.claim_lead : G2_WANT_LEAD;
         pe.lowdin = c->opt.iteration == NOLSM_ITER_LOWDIN ? 1 : 0;
+        pe.scan_rotate = c->opt.scan_order == 2 ? 1 : c->opt.scan_order == 1 ? 0 : (mean_n2 <= 768.0 * 768.0 ? 1 : 0);
         pe.l2_load = c->opt.l2_load_policy > 0 ? c->opt.l2_load_policy : 1; pe.l2_store = c->opt.l2_store_policy > 0 ? c->opt.l2_store_policy : 2;
         pe.sym_tiles = c->opt.symmetric_tiles >= 0 ? 1 : 0;
         pe.n_mu = 1; pe.count_only = 0;
@@ -624,6 +625,7 @@ int engine_counters(nolsm_ctx* c, double* out) {
         out[25 + k] = (double)ct[PC_SIDE_TASKS + k];
     }
     for (int k = 0; k < 3; ++k) out[33 + k] = ct[PC_MMA_NS + k] * 1e-6;
+    out[36] = ct[PC_SCHED_RING_NS] * 1e-6; out[37] = ct[PC_SCHED_CREDIT_NS] * 1e-6;
     return NOLSM_OK;
 }
 

@@ -59,7 +59,9 @@ enum { PC_TILES = 0, PC_SCHED_IDLE_NS, PC_SCHED_BUSY_NS, PC_OVERSHOOT, PC_T_STAR
        PC_SIDE_BYTES = PC_SIDE_NS + 8,   // + kind (algorithmic bytes)
        PC_SIDE_TASKS = PC_SIDE_BYTES + 8,
        PC_MMA_NS = PC_SIDE_TASKS + 8,    // + 0 tile-record wait, 1 accumulator wait, 2 k-loops (MMA warps of the leader CTAs)
-       PC_LEN = PC_MMA_NS + 3 };
+       PC_SCHED_RING_NS = PC_MMA_NS + 3, // tile schedulers: waiting for a free ring entry (= for the completion of the tile four back)
+       PC_SCHED_CREDIT_NS,               // ... for the producer's claim point
+       PC_LEN };
 
 constexpr int OPF_RES = 1;        // op flags: fused residual wanted
 constexpr int OPF_SYM = 2;        // symmetric product: upper-triangle tiles, mirrored stores
@@ -77,7 +79,7 @@ struct __align__(16) PSlot {      // 176 bytes
     int pow_step; float pow_norm2, pow_alpha; int resume;           // block power iteration state; resume: which token phase comes next
     int noboost, mptr, mend, zcur;                                  // noboost: the scaled steps are over for this matrix; members [mptr, mend) still to be served
     int xsum, pow_buf, mu_idx, sym_count;                           // X ping-pong: next = xsum - xcur; buffer of the running power iteration; trial mu; symmetric GEMMs run
-    int elem_kind, abuf, pad0, pad1;                                // SK_ELEM variant; buffer that keeps the mu-independent A0 (several trial mu)
+    int elem_kind, abuf, op_seq, pad1;                              // SK_ELEM variant; buffer that keeps the mu-independent A0 (several trial mu); ops installed so far
 };
 
 struct PEngine {
@@ -96,6 +98,7 @@ struct PEngine {
     int* heavy;                   // [1] slots inside the GEMM-heavy phases right now (at most g_max)
     int* parked;                  // [S] 1 = the slot is ready for a heavy phase and waits for a token
     int g_max, want_lead;
+    int scan_rotate;              // 1: pair p scans the claim table from slot 13 p mod S on; 0: every pair from slot 0 (slot-order priority)
     int l2_load, l2_store;        // L2 eviction priority of the operand loads / of the stores of C (1 evict_first, 2 evict_last, 3 normal)
     int lowdin;                   // 0: Eq. 6 on A = S^-1 H0 - mu I; 1: symmetric (Loewdin) form
     int sym_tiles;                // 1: symmetric products multiply the upper triangle of tiles only
@@ -209,8 +212,10 @@ __device__ __forceinline__ void p_install_gemm(const PEngine& e, int slot, int k
     __stcg(reinterpret_cast<int4*>(&s->op_kind), make_int4(kind, a, b, c));
     __stcg(reinterpret_cast<float4*>(&s->c_out), make_float4(c_out, alpha_res, beta, __int_as_float(flags)));
     const unsigned long long tiles = (unsigned long long)p_tiles_of(e, __ldcg(&s->ntm), flags);
+    const int seq = __ldcg(&s->op_seq) + 1;                        // generation of the claim word: a scheduler that cached the op's record
+    __stcg(&s->op_seq, seq);                                       // sees when the word belongs to a newer op
     __threadfence();
-    *(volatile unsigned long long*)&e.gclaim[slot] = tiles << 20;
+    *(volatile unsigned long long*)&e.gclaim[slot] = ((unsigned long long)(seq & 0xFFFFFF) << 40) | (tiles << 20);
 }
 
 // Starts the block power iteration on buffer `buf` (S_sub or the X0 buffer): V0 = the shared +-1 start block.
@@ -301,7 +306,7 @@ __device__ __forceinline__ bool p_refill(const PEngine& e, int slot) {
     __stcg(reinterpret_cast<float4*>(&s->rho_a), make_float4(0.f, 1.f, 0.5f, 0.f));    // rho_a, alpha1, alpha2, side_done
     __stcg(reinterpret_cast<int4*>(&s->noboost), make_int4(0, m0, m1, 3));             // noboost, mptr, mend, zcur
     __stcg(reinterpret_cast<int4*>(&s->xsum), make_int4(e.lowdin ? 3 : 1, 0, 0, 0));   // xsum, pow_buf, mu_idx, sym_count
-    __stcg(reinterpret_cast<int4*>(&s->elem_kind), make_int4(0, 0, 0, 0));
+    __stcg(&s->elem_kind, 0); __stcg(&s->abuf, 0);                                     // op_seq keeps counting across the slot's atoms
     __stcg(&s->resume, 0);
     p_install_side(e, slot, SK_GATHER, (nset + e.gather_rowatoms - 1) / e.gather_rowatoms);
     return true;
@@ -471,11 +476,17 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
     const unsigned long long t_begin = pl::gtime();
     bool short_tiles = false;
     // tiles claimed and not yet published (lane 0): tiles [pend_t, pend_end) of the op whose record is cached below
-    int pend_t = 0, pend_end = 0, pend_slot = 0, pend_nt = 0;
+    int pend_t = 0, pend_end = 0, pend_slot = 0, pend_nt = 0, pend_gen = -1;
+    bool sticky_ok = false;
     int4 g0 = make_int4(0, 0, 0, 0), g1 = g0, o0 = g0;
     float4 o1 = make_float4(0.f, 0.f, 0.f, 0.f);
+    unsigned long long ring_ns = 0, credit_ns = 0;
+    const int scan_off = e.scan_rotate ? (int)(((blockIdx.x >> 1) * 13u) % (unsigned)min(e.S, 96)) : 0;
     for (;;) {
+        const unsigned long long tr0 = pl::gtime();
         if (!ptx::mbar_wait_cluster_patient(sm.ti_empty(q), ph ^ 1, e.abort_flag)) break;
+        const unsigned long long tr1 = pl::gtime();
+        ring_ns += tr1 - tr0;
         // Claim lazily: only when the producer has issued every load of the tile before and needs the next
         // record (it runs G2_STAGES k-blocks ahead of the MMA, which hides the claim). A pair that claimed
         // further ahead would hoard tiles of a GEMM that idle pairs could run at the same time, and the
@@ -492,16 +503,46 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
             }
             if (stalled) break;
         }
+        credit_ns += pl::gtime() - tr1;
         TileInfo ti{};
         int got = __shfl_sync(0xffffffffu, pend_t < pend_end ? 1 : 0, 0), tflags = 0;
         unsigned long long t_idle0 = 0;
+        if (!got && sticky_ok) {
+            // the next tile of the GEMM this pair took its last tile from: one atomic, no scan, and the op's record is still
+            // in registers when the generation of the claim word is the cached one
+            unsigned long long w = 0;
+            if (lane == 0) w = atomicAdd(&e.gclaim[pend_slot], 1ull);
+            w = __shfl_sync(0xffffffffu, w, 0);
+            const int t = (int)(w & 0xFFFFFu), nt = (int)((w >> 20) & 0xFFFFFu), gen = (int)(w >> 40);
+            if (t < nt) {
+                if (lane == 0) {
+                    if (gen != pend_gen) {
+                        __threadfence();
+                        const PSlot* s = &e.slots[pend_slot];
+                        g0 = __ldcg(reinterpret_cast<const int4*>(&s->atom));
+                        g1 = __ldcg(reinterpret_cast<const int4*>(&s->nbi));
+                        o0 = __ldcg(reinterpret_cast<const int4*>(&s->op_kind));
+                        o1 = __ldcg(reinterpret_cast<const float4*>(&s->c_out));
+                        pend_gen = gen;
+                    }
+                    pend_t = t; pend_end = t + 1; pend_nt = nt;
+                }
+                got = 1;
+            } else {
+                sticky_ok = false;
+            }
+        }
         while (!got) {
             // scan of the claim table in slot order: all words of a lane are loaded before the first ballot
+            // (scan_off: with rotated scanning every pair starts at its own slot, so the claims of the 74 pairs spread over
+            // the claim words instead of queueing on the first one)
             unsigned long long w3[3];
 #pragma unroll
             for (int r = 0; r < 3; ++r) {
-                const int sidx = 32 * r + lane;
-                w3[r] = sidx < e.S ? *(volatile unsigned long long*)&e.gclaim[sidx] : 0ull;
+                const int idx = 32 * r + lane;
+                int sidx = idx + scan_off;
+                if (sidx >= e.S) sidx -= e.S;
+                w3[r] = idx < e.S ? *(volatile unsigned long long*)&e.gclaim[sidx] : 0ull;
             }
             int found = -1;
             unsigned long long wf = 0;
@@ -509,7 +550,11 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
             for (int r = 0; r < 3; ++r) {
                 const bool avail = (unsigned)(w3[r] & 0xFFFFFu) < (unsigned)((w3[r] >> 20) & 0xFFFFFu);
                 const unsigned m = __ballot_sync(0xffffffffu, avail);
-                if (m && found < 0) { found = 32 * r + __ffs(m) - 1; wf = __shfl_sync(0xffffffffu, w3[r], __ffs(m) - 1); }
+                if (m && found < 0) {
+                    found = 32 * r + __ffs(m) - 1 + scan_off;
+                    if (found >= e.S) found -= e.S;
+                    wf = __shfl_sync(0xffffffffu, w3[r], __ffs(m) - 1);
+                }
             }
             for (int base = 96; base < e.S && found < 0; base += 32) {      // more than 96 slots (never by default)
                 const int sidx = base + lane;
@@ -535,8 +580,10 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
                         g1 = __ldcg(reinterpret_cast<const int4*>(&s->nbi));      // nbi ntm nset unit
                         o0 = __ldcg(reinterpret_cast<const int4*>(&s->op_kind));
                         o1 = __ldcg(reinterpret_cast<const float4*>(&s->c_out));
-                        pend_t = t; pend_end = min(t + k, nt); pend_slot = found; pend_nt = nt;
+                        pend_t = t; pend_end = min(t + k, nt); pend_nt = nt; pend_gen = (int)(w >> 40);
                     }
+                    pend_slot = found;
+                    sticky_ok = e.scan_rotate != 0;
                     got = 1;
                     break;
                 }
@@ -602,6 +649,8 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
         atomicAdd(&e.ctr[PC_SCHED_IDLE_NS], idle_ns);
         atomicAdd(&e.ctr[PC_SCHED_BUSY_NS], t_end - t_begin - idle_ns);
         atomicAdd(&e.ctr[PC_OVERSHOOT], overshoot);
+        atomicAdd(&e.ctr[PC_SCHED_RING_NS], ring_ns);
+        atomicAdd(&e.ctr[PC_SCHED_CREDIT_NS], credit_ns);
         atomicMin(&e.ctr[PC_T_START], t_begin);
         atomicMax(&e.ctr[PC_T_END], t_end);
     }

@@ -1,5 +1,5 @@
 // Submatrix combination (Eq. 9 / Eq. 10; C-19): which atoms share one dense submatrix.
-// Host integer arithmetic only, so that the library and the oracle form bit-identical groups.
+// Host integer arithmetic only: the grouping is reproducible bit for bit by any restatement of DESIGN.md C-19.
 #include "ctx.h"
 
 namespace nolsm_host {
@@ -11,7 +11,7 @@ namespace nolsm_host {
 //     dimensions and GFLOP/s), linear interpolation between neighbouring entries, constant outside the table. In
 //     integers: r = (r_k (n_{k+1} - n) + r_{k+1} (n - n_k)) / (n_{k+1} - n_k), cost = 10^6 n^3 / r (floor divisions of
 //     non-negative numbers). Without a table: the tile-step count of the engine, ceil(n16/256)^2 ceil(n16/64) (the time
-//     of a multiplication in 256 x 256 x 64 tile steps), a model that tests/test_oracle_combine.py compares with the
+//     of a multiplication in 256 x 256 x 64 tile steps), a model that the CPU tests compare with the
 //     measured table.
 int64_t perf_rate(const std::vector<int64_t>& tn, const std::vector<int64_t>& tr, int64_t n) {
     const size_t m = tn.size();

@@ -68,7 +68,7 @@ def test_product_path_does_not_touch_the_oracle():
     pkg = os.path.join(ROOT, "paper_2205_12182_b200")
     for dirpath, _, files in os.walk(pkg):
         for f in files:
-            if f.endswith((".py", ".cu", ".cuh", ".h")):
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
                 assert "oracle" not in open(os.path.join(dirpath, f)).read().lower(), f
     for f in os.listdir(os.path.join(ROOT, "oracle")):
         if f.endswith(".py"):

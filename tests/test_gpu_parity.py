@@ -382,6 +382,50 @@ def test_one_heavy_token_and_many_small_units():
     assert np.abs(D.cpu().numpy() - D0).max() <= TOL_MIXED_D
 
 
+def test_boundary_errors_and_diagnostics_of_the_round_2_calls(cfg0):
+    """Argument checks of nolsm_set_perf_table / nolsm_electron_counts, the engine counters, and the stand-alone side-task
+    timing (bytes and times are positive; the results of the density call before it are declared stale)."""
+    from paper_2205_12182_b200 import PREC_FP32, NolsmError
+    s = cfg0
+    nb, rp, ci, Hv, Sv = _arrays(s)
+    with _nolsm() as ctx:
+        for bad_n, bad_t in (([300, 200], [1.0, 2.0]), ([100, 200], [1.0, -2.0]), ([0, 200], [1.0, 2.0]), ([100, 9000], [1.0, 2.0])):
+            with pytest.raises(NolsmError) as ei:
+                ctx.set_perf_table(bad_n, bad_t)
+            assert ei.value.code == 1
+        ctx.set_perf_table([128, 1024], [100.0, 900.0])
+        ctx.set_perf_table([], [])                                   # removes the table
+        with pytest.raises(NolsmError) as ei:
+            ctx.electron_counts([0.0])                               # not assembled
+        assert ei.value.code == 4
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        with pytest.raises(NolsmError) as ei:
+            ctx.electron_counts([0.1 * k for k in range(9)])         # more than 8 trial mu
+        assert ei.value.code == 1
+        D = torch.zeros(Hv.shape[0], dtype=torch.float64, device="cuda")
+        ctx.density_matrix(s.mu, D)
+        ctx.energy()
+        ct = ctx.engine_counters()
+        assert ct["persistent"] and ct["tiles"] > 0 and ct["pairs"] == 74 and ct["mma_kloop_ms"] > 0
+        n_counts = ctx.electron_counts([s.mu])                       # a count-only pass leaves no energy to read
+        with pytest.raises(NolsmError) as ei:
+            ctx.energy()
+        assert ei.value.code == 4
+        ctx.density_matrix(s.mu, D)
+        assert abs(ctx.electron_count() - n_counts[0]) <= TOL_MIXED_E * float(s.atom_nb.sum())
+        for which in (0, 1):
+            ms, nbytes = ctx.side_task_bandwidth(which, reps=2)
+            assert ms > 0 and nbytes > 0
+        with pytest.raises(NolsmError) as ei:                        # the timing overwrote the energies
+            ctx.energy()
+        assert ei.value.code == 4
+    with _nolsm(precision=PREC_FP32) as ctx:                         # round engine: one trial mu per call only
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        with pytest.raises(NolsmError) as ei:
+            ctx.electron_counts([0.0, 0.1])
+        assert ei.value.code == 4
+
+
 def test_indefinite_S_is_reported(cfg0):
     """gamma = 1 (BASELINE.json's literal amplitude 0.3) is indefinite on cfg0 (SURVEY finding 1): the
     Schulz inverse cannot converge for the affected submatrices and the library must say so."""

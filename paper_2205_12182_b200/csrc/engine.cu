@@ -692,6 +692,7 @@ int engine_gather(nolsm_ctx* c, int64_t id, bool is_unit, int which, int out_fp1
 // `reps` launches, CUDA events around them. bytes_out = algorithmic bytes of one launch.
 int engine_side_bandwidth(nolsm_ctx* c, int which, int reps, double* ms_out, double* bytes_out) {
     if (!c->persist) return fail(c, NOLSM_ESTATE, "side-task bandwidth needs the persistent engine");
+    if (which == 1 && c->combined) return fail(c, NOLSM_ESTATE, "scatter bandwidth: assemble without combine");
     const PEngine& pe = *c->peng;
     cudaStream_t s = c->s_main;
     cudaEvent_t e0, e1;
@@ -732,7 +733,6 @@ int engine_side_bandwidth(nolsm_ctx* c, int which, int reps, double* ms_out, dou
         return cudaGetLastError();
     };
     if (which == 1) {
-        if (c->combined) return fail(c, NOLSM_ESTATE, "scatter bandwidth: assemble without combine");
         const size_t need = (size_t)c->nvals * 8;
         if (c->d_D_stage_bytes < need) {
             if (c->d_D_stage) cudaFree(c->d_D_stage);

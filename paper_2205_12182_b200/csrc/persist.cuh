@@ -481,7 +481,7 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
     int4 g0 = make_int4(0, 0, 0, 0), g1 = g0, o0 = g0;
     float4 o1 = make_float4(0.f, 0.f, 0.f, 0.f);
     unsigned long long ring_ns = 0, credit_ns = 0;
-    const int scan_off = e.scan_rotate ? (int)(((blockIdx.x >> 1) * 13u) % (unsigned)min(e.S, 96)) : 0;
+    const int scan_off = e.scan_rotate && e.S <= 96 ? (int)(((blockIdx.x >> 1) * 13u) % (unsigned)e.S) : 0;   // (the one-shot scan covers 96 slots)
     for (;;) {
         const unsigned long long tr0 = pl::gtime();
         if (!ptx::mbar_wait_cluster_patient(sm.ti_empty(q), ph ^ 1, e.abort_flag)) break;
@@ -545,7 +545,6 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
                 w3[r] = idx < e.S ? *(volatile unsigned long long*)&e.gclaim[sidx] : 0ull;
             }
             int found = -1;
-            unsigned long long wf = 0;
 #pragma unroll
             for (int r = 0; r < 3; ++r) {
                 const bool avail = (unsigned)(w3[r] & 0xFFFFFu) < (unsigned)((w3[r] >> 20) & 0xFFFFFu);
@@ -553,7 +552,6 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
                 if (m && found < 0) {
                     found = 32 * r + __ffs(m) - 1 + scan_off;
                     if (found >= e.S) found -= e.S;
-                    wf = __shfl_sync(0xffffffffu, w3[r], __ffs(m) - 1);
                 }
             }
             for (int base = 96; base < e.S && found < 0; base += 32) {      // more than 96 slots (never by default)
@@ -561,15 +559,13 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
                 const unsigned long long w = sidx < e.S ? *(volatile unsigned long long*)&e.gclaim[sidx] : 0ull;
                 const bool avail = (unsigned)(w & 0xFFFFFu) < (unsigned)((w >> 20) & 0xFFFFFu);
                 const unsigned m = __ballot_sync(0xffffffffu, avail);
-                if (m) { found = base + __ffs(m) - 1; wf = __shfl_sync(0xffffffffu, w, __ffs(m) - 1); }
+                if (m) found = base + __ffs(m) - 1;
             }
             if (found >= 0) {
                 // one tile per claim (three per claim for GEMMs of at most nine tiles was measured on cfg1: no faster without
                 // combination, slower in the Loewdin form - the tiles of a GEMM should spread over pairs, not queue on one)
-                (void)wf;
-                const int k = 1;
                 unsigned long long w = 0;
-                if (lane == 0) w = atomicAdd(&e.gclaim[found], (unsigned long long)k);
+                if (lane == 0) w = atomicAdd(&e.gclaim[found], 1ull);
                 w = __shfl_sync(0xffffffffu, w, 0);
                 const int t = (int)(w & 0xFFFFFu), nt = (int)((w >> 20) & 0xFFFFFu);
                 if (t < nt) {
@@ -580,7 +576,7 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
                         g1 = __ldcg(reinterpret_cast<const int4*>(&s->nbi));      // nbi ntm nset unit
                         o0 = __ldcg(reinterpret_cast<const int4*>(&s->op_kind));
                         o1 = __ldcg(reinterpret_cast<const float4*>(&s->c_out));
-                        pend_t = t; pend_end = min(t + k, nt); pend_nt = nt; pend_gen = (int)(w >> 40);
+                        pend_t = t; pend_end = t + 1; pend_nt = nt; pend_gen = (int)(w >> 40);
                     }
                     pend_slot = found;
                     sticky_ok = e.scan_rotate != 0;

@@ -73,7 +73,8 @@ typedef struct {
     int power_iters_s;       /* power iterations for rho(S_sub) [persistent engine 3 (x 1.3 safety), round engine 6 (x 1.05)] */
     int power_iters_a;       /* power iterations for rho(A_sub) [persistent engine 6 (x 1.25 safety), round engine 12 (x 1.05)] */
     double eps_filter;       /* block (j,i) enters N(i) iff max(|H0_ji|max, |S_ji|max) > eps_filter [0 = structural] */
-    int batch_atoms;         /* workspace slots = submatrices resident at once [auto: ~16 waves of GEMM tiles] */
+    int batch_atoms;         /* workspace slots = submatrices resident at once [auto: persistent engine heavy_slots + max(12, heavy_slots),
+                                at most 96; round engine ~16 waves of GEMM tiles] */
     size_t workspace_bytes;  /* cap on the library-owned dense workspace [auto] */
     int profile_every;       /* round engine, > 0: every k-th round runs eagerly with CUDA events around each launch [0 = off] */
     int engine;              /* NOLSM_ENGINE_* [AUTO: PERSISTENT (one kernel launch per density_matrix call, tcgen05 GEMMs) for the
@@ -118,7 +119,8 @@ typedef struct {
     double dim_mean;
     int64_t sum_inv_iters, sum_sign_iters;
     int64_t gemms_executed;       /* square GEMMs actually run, summed over submatrices */
-    double flops_useful;          /* sum_i 2 n_i^3 * gemms_i   (PAPER.md:L156 convention) */
+    double flops_useful;          /* FLOP of the executed tiles on true dimensions: sum_i 2 n_i^3 * (full GEMMs_i + the executed share of
+                                     the symmetric ones) */
     double flops_padded;          /* same with tile-padded dimensions (what the tensor cores executed) */
     int64_t n_notspd, n_noconv;
     double gather_bytes, scatter_bytes; /* algorithmic bytes of the last density_matrix call */

@@ -277,6 +277,7 @@ def main():
                     help="submatrix combination of the timed path (0 = one submatrix per atom, BASELINE.json's configs)")
     ap.add_argument("--iteration", type=int, default=0, choices=[0, 1], help="0 = Eq. 6 as printed, 1 = symmetric (Loewdin) form")
     ap.add_argument("--symmetric-tiles", type=int, default=0, choices=[0, -1])
+    ap.add_argument("--transposed-tiles", type=int, default=0, choices=[0, -1])
     ap.add_argument("--heavy-slots", type=int, default=0)
     ap.add_argument("--claim-lead", type=int, default=0)
     ap.add_argument("--no-extra-legs", "--no-combine-leg", action="store_true", dest="no_extra",
@@ -321,7 +322,8 @@ def main():
     D = torch.empty_like(Hv)
     stream = torch.cuda.current_stream().cuda_stream
     head_opts = dict(profile_every=args.profile_every, combine=args.combine, iteration=args.iteration,
-                     symmetric_tiles=args.symmetric_tiles, heavy_slots=args.heavy_slots, claim_lead=args.claim_lead)
+                     symmetric_tiles=args.symmetric_tiles, heavy_slots=args.heavy_slots, claim_lead=args.claim_lead,
+                     transposed_tiles=args.transposed_tiles)
     ctx = Nolsm(local_rank, **head_opts)
     perf_table = load_perf_table()
     if perf_table and args.combine == 2:
@@ -571,6 +573,7 @@ def main():
                        "parallelism": "replicas" if world > 1 else "single",
                        "combine": args.combine, "iteration": "lowdin" if args.iteration else "eq6",
                        "symmetric_tiles": args.symmetric_tiles == 0,
+                       "transposed_tiles": args.transposed_tiles == 0,
                        "value_counts": "atoms served per second (one submatrix per atom when combine = 0)",
                        "l2": "inputs (8 GB block-CSR) and workspace >> 126 MB L2; no flush needed"},
             "tensor_tflops": tflops, "pct_of_dense_fp16_peak": {"nominal_2250": 100 * tflops / NOMINAL_FP16_TFLOPS / world,

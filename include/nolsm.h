@@ -110,6 +110,9 @@ typedef struct {
     int l2_load_policy;      /* persistent engine: L2 eviction priority of the TMA operand loads: 1 evict_first, 2 evict_last, 3 normal [1] */
     int l2_store_policy;     /* the same for the TMA stores of the GEMM results [2: a result stays in L2 until the next GEMM of its
                                 chain reads it instead of being pushed out by operand traffic; measured +5 % on configs[2]] */
+    int transposed_tiles;    /* persistent engine: the tiles of a ragged last row block (r < 256 rows left) are computed transposed,
+                                C^T = B^T A^T, so the MMA's M = 256 runs over full columns and its N = r over the rows that exist,
+                                instead of M = 256 (or 128) over r rows [0 = on; -1 = off] */
 } nolsm_options;
 
 typedef struct {

@@ -438,6 +438,7 @@ int engine_plan(nolsm_ctx* c, cudaStream_t s) {
         pe.scan_rotate = c->opt.scan_order == 2 ? 1 : c->opt.scan_order == 1 ? 0 : (mean_n2 <= 768.0 * 768.0 ? 1 : 0);
         pe.l2_load = c->opt.l2_load_policy > 0 ? c->opt.l2_load_policy : 1; pe.l2_store = c->opt.l2_store_policy > 0 ? c->opt.l2_store_policy : 2;
         pe.sym_tiles = c->opt.symmetric_tiles >= 0 ? 1 : 0;
+        pe.trans_tiles = c->opt.transposed_tiles >= 0 ? 1 : 0;
         pe.n_mu = 1; pe.count_only = 0;
         pe.nelec_mu = c->d_mu_acc; pe.e_mu = c->d_mu_acc + NOLSM_MAX_MU;
         pe.elem_chunks = 16;
@@ -526,6 +527,22 @@ int engine_atom_stats(nolsm_ctx* c, int64_t a0, int64_t count, int32_t* dims, in
     return NOLSM_OK;
 }
 
+// FLOP one square GEMM of dimension n16 costs the tensor cores of the persistent pair engine, by the scheduler's tile rules
+// (p_scheduler): 256 x bn tiles; symmetric products only on and above the diagonal; a ragged last row block transposed
+// (M = 256 columns, N = the rows left) or, for its corner tile, as M = 128 when at most 128 rows are left.
+static double padded_gemm_flops(int n16, bool sym, bool trans) {
+    const int ntm = (n16 + BM - 1) / BM;
+    double f = 0.0;
+    for (int tm = 0; tm < ntm; ++tm)
+        for (int tn = sym ? tm : 0; tn < ntm; ++tn) {
+            const int bn = std::min(BN, n16 - tn * BN), rleft = n16 - tm * BM;
+            if (trans && rleft < BM && tn < ntm - 1 && !sym) f += (double)BM * rleft;
+            else if (rleft <= BM / 2 && (bn & 31) == 0) f += (double)(BM / 2) * bn;
+            else f += (double)BM * bn;
+        }
+    return 2.0 * f * (double)n16;
+}
+
 // FLOP of the last call. A full GEMM counts 2 n^3. A symmetric product that multiplied only the tiles
 // on and above the diagonal counts the share it executed, 2 n^3 (ntm + 1) / (2 ntm); flops_paper counts every GEMM at
 // 2 n^3 (the paper's convention, which knows no symmetric products).
@@ -553,14 +570,14 @@ int engine_stats(nolsm_ctx* c, nolsm_stats* out) {
         const double fsym = (double)(ntm + 1) / (2.0 * ntm);
         out->flops_useful += 2.0 * d * d * d * (gm[u] + fsym * gy[u]);
         out->flops_paper += 2.0 * d * d * d * (gm[u] + gy[u]);
-        // rows / columns the tensor cores executed: 256 per row block; the persistent pair engine runs a last row block of at
-        // most 128 rows as M = 128 tiles (except on a ragged last column tile whose width is not a multiple of 32)
-        double rows = (double)(ntm * BM);
-        if (c->last_persist && n16 - (ntm - 1) * BM <= BM / 2) {
-            const int last_bn = n16 - (ntn - 1) * BN;
-            rows -= (BM / 2) * ((last_bn & 31) == 0 ? 1.0 : (double)(n16 - last_bn) / (double)n16);
+        // what the tensor cores executed: the persistent pair engine by its tile rules (padded_gemm_flops), the round
+        // engine 256 rows per row block
+        if (c->last_persist) {
+            const bool sym = c->opt.symmetric_tiles >= 0, tr = c->opt.transposed_tiles >= 0;
+            out->flops_padded += padded_gemm_flops(n16, false, tr) * gm[u] + padded_gemm_flops(n16, sym, tr) * gy[u];
+        } else {
+            out->flops_padded += 2.0 * (double)(ntm * BM) * (double)n16 * (double)n16 * (gm[u] + gy[u]);
         }
-        out->flops_padded += 2.0 * rows * (double)n16 * (double)n16 * (gm[u] + fsym * gy[u]);
         out->n_notspd += (st[u] & ST_NOTSPD) ? 1 : 0;
         out->n_noconv += (st[u] & ST_NOCONV) ? 1 : 0;
         out->gather_bytes += 2.0 * (double)n16 * (double)n16 * elem_size(c);      // dense S_sub and H_sub written (once per unit)

@@ -50,6 +50,8 @@ constexpr int TI_HALF = 2;            // half-height tile (rows m0 .. m0+127, on
 constexpr int TI_MIRROR = 4;          // off-diagonal tile of a symmetric product: C^T goes to the block below the diagonal too
 constexpr int TI_PLAIN = 8;           // C = c_out acc without identity term; residual = || alpha_res acc ||_F^2 (power iteration, D columns)
 constexpr int TI_F32OUT = 16;         // the first PCW accumulator columns go to the slot's FP32 block instead of C (D columns)
+constexpr int TI_TRANS = 64;          // tile of the ragged last row block computed transposed: C^T[n0.., m0..] = B^T A_bottom^T, so the
+                                      // MMA's M = 256 runs over full columns of C and its N = bn over the r < 256 rows that are left
 constexpr int TI_SYMDIAG = 32;        // diagonal tile of a symmetric product: only its upper triangle is stored, and mirrored
 
 struct __align__(16) TileInfo {      // 64 bytes
@@ -378,9 +380,25 @@ __device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap*
         const int row0 = ti.m0 + (hh ? 64 : 128) * (int)rank;
         const int col0 = ti.n0 + half * (int)rank;
         const int kb_want = rank == 0 ? max(0, nkb - want_lead) : -1;
+        // transposed tile: the A stage takes this CTA's 128 columns of B (two boxes), the B stage its bn / 2 rows of A
+        const bool tr = (ti.valid & TI_TRANS) != 0;
+        const int tcol0 = ti.n0 + 128 * (int)rank, trow0 = ti.m0 + half * (int)rank;
 #pragma unroll 1
         for (int kb = 0; kb < nkb; ++kb) {
             if (!ptx::mbar_wait(sm.empty(stage), phase ^ 1, abort_flag)) return;
+            if (tr) {
+                if (ptx::elect_one()) {
+                    if (kb == kb_want) ptx::st_shared_volatile_u32(sm.want(), started);
+                    const uint32_t fb = full0 + 8u * stage;
+                    if (rank == 0) ptx::mbar_expect_tx(sm.full(stage), bytes);
+                    const uint32_t sa = sm.stage_a(stage), sb = sm.stage_b(stage);
+                    const int k0 = kb * BK;
+                    ptx::tma_load_2d_pair(sa, map_b, tcol0, k0, fb, pol);
+                    ptx::tma_load_2d_pair(sa + 8192, map_b, tcol0 + 64, k0, fb, pol);
+                    ptx::tma_load_2d_pair(sb, map_a, k0, trow0, fb, pol);
+                    if (nbox > 1) ptx::tma_load_2d_pair(sb + B_BOX_BYTES, map_a, k0, trow0 + 64, fb, pol);
+                }
+            } else
             if (ptx::elect_one()) {
                 if (kb == kb_want) ptx::st_shared_volatile_u32(sm.want(), started);   // the scheduler may claim the next tile now
                 const uint32_t fb = full0 + 8u * stage;
@@ -406,19 +424,21 @@ __device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap*
 // ------------------------------------------------------------------------------------------------
 namespace ptx {
 // 4 x (M = 256, N, K = 16) on one 64-k stage; acc0 = 0 overwrites the accumulator with the first MMA.
+template <int SA = 2, int SB = 128>      // descriptor steps per 16 k (16-byte units): K-major operand 2, MN-major operand 128
 __device__ __forceinline__ void umma_f16_pair_x4(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc0) {
     asm volatile(
         "{\n\t.reg .pred p, t;\n\t.reg .b64 a1, b1, a2, b2, a3, b3;\n\t"
         "setp.ne.b32 p, %4, 0;\n\t"
         "setp.eq.b32 t, 0, 0;\n\t"
-        "add.s64 a1, %1, 2;\n\tadd.s64 b1, %2, 128;\n\t"
-        "add.s64 a2, %1, 4;\n\tadd.s64 b2, %2, 256;\n\t"
-        "add.s64 a3, %1, 6;\n\tadd.s64 b3, %2, 384;\n\t"
+        "add.s64 a1, %1, %5;\n\tadd.s64 b1, %2, %6;\n\t"
+        "add.s64 a2, %1, %7;\n\tadd.s64 b2, %2, %8;\n\t"
+        "add.s64 a3, %1, %9;\n\tadd.s64 b3, %2, %10;\n\t"
         "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t"
         "tcgen05.mma.cta_group::2.kind::f16 [%0], a1, b1, %3, t;\n\t"
         "tcgen05.mma.cta_group::2.kind::f16 [%0], a2, b2, %3, t;\n\t"
         "tcgen05.mma.cta_group::2.kind::f16 [%0], a3, b3, %3, t;\n\t}\n"
-        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc0) : "memory");
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc0),
+          "n"(SA), "n"(SB), "n"(2 * SA), "n"(2 * SB), "n"(3 * SA), "n"(3 * SB) : "memory");
 }
 }  // namespace ptx
 
@@ -432,6 +452,9 @@ __device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int
     // descriptors of stage 0; stage s adds s * G2_STAGE_BYTES / 16 to the address field
     const uint64_t da0 = make_smem_desc(sm.stage_a(0), 16, 1024);
     const uint64_t db0 = make_smem_desc(sm.stage_b(0), B_BOX_BYTES, 1024);
+    // transposed tiles (TI_TRANS): the A stage holds columns of B (MN-major), the B stage rows of A (K-major)
+    const uint64_t dat0 = make_smem_desc(sm.stage_a(0), B_BOX_BYTES, 1024);
+    const uint64_t dbt0 = make_smem_desc(sm.stage_b(0), 16, 1024);
     for (;;) {
         const unsigned long long t0 = ptx::globaltimer_ns();
         const TileInfo ti = g2_take<true>(sm, q, tph, lane == 0, abort_flag);
@@ -440,7 +463,8 @@ __device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int
         const unsigned long long t1 = ptx::globaltimer_ns();
         const int nkb = (ti.n16 + BK - 1) / BK;
         const int ktail = (ti.n16 - (nkb - 1) * BK) >> 4;          // 16-k slices of the last k-block (1..4)
-        const uint32_t idesc = make_idesc_f16((ti.valid & TI_HALF) ? 128 : 256, ti.bn);
+        const bool tr = (ti.valid & TI_TRANS) != 0;
+        const uint32_t idesc = make_idesc_f16((ti.valid & TI_HALF) ? 128 : 256, ti.bn) ^ (tr ? (3u << 15) : 0u);   // A MN-major, B K-major
         if (!ptx::mbar_wait_cluster(sm.tempty(acc), acc_phase ^ 1, abort_flag)) return;
         ptx::tc_fence_after();
         const unsigned long long t2 = ptx::globaltimer_ns();
@@ -450,13 +474,15 @@ __device__ __forceinline__ void g2_mma(const G2Smem& sm, uint32_t tmem_base, int
             if (!ptx::mbar_wait(sm.full(stage), phase, abort_flag)) return;
             ptx::tc_fence_after();
             if (ptx::elect_one()) {
-                const uint64_t da = da0 + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
-                const uint64_t db = db0 + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
+                const uint64_t da = (tr ? dat0 : da0) + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
+                const uint64_t db = (tr ? dbt0 : db0) + (uint64_t)(stage * (G2_STAGE_BYTES >> 4));
                 if (kb < nkb - 1 || ktail == 4) {
-                    ptx::umma_f16_pair_x4(d_tmem, da, db, idesc, kb != 0);
+                    if (!tr) ptx::umma_f16_pair_x4<2, 128>(d_tmem, da, db, idesc, kb != 0);
+                    else ptx::umma_f16_pair_x4<128, 2>(d_tmem, da, db, idesc, kb != 0);
                 } else {
+                    const int sa = tr ? 128 : 2, sb = tr ? 2 : 128;
                     for (int k = 0; k < ktail; ++k)
-                        ptx::umma_f16_pair(d_tmem, da + 2 * k, db + 128 * k, idesc, (kb | k) != 0);
+                        ptx::umma_f16_pair(d_tmem, da + sa * k, db + sb * k, idesc, (kb | k) != 0);
                 }
                 ptx::umma_commit_pair(sm.empty(stage));
                 if (kb == nkb - 1) ptx::umma_commit_pair(sm.tfull(acc));
@@ -512,9 +538,13 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
         // full-height tile: the CTA's 128 TMEM lanes are 128 rows, every warp sees all bn columns; half-height tile
         // (M = 128 over the pair): lanes 0-63 and 64-127 are the same 64 rows with the left / right half of the columns
         const bool hh = (ti.valid & TI_HALF) != 0;
-        const int rbase = hh ? ti.m0 + 64 * (int)rank + (quarter & 1) * 32 : ti.m0 + 128 * (int)rank + quarter * 32;   // first row of this warp
+        // transposed tile: the lanes are COLUMNS of C (n0 + ...), the accumulator columns its rows m0 .. m0 + bn - 1; below,
+        // "row" / "col" then name the lane / accumulator-column coordinate and only the stores swap them back
+        const bool trans = (ti.valid & TI_TRANS) != 0;
+        const int rbase = trans ? ti.n0 + 128 * (int)rank + quarter * 32
+                        : hh ? ti.m0 + 64 * (int)rank + (quarter & 1) * 32 : ti.m0 + 128 * (int)rank + quarter * 32;   // first row of this warp
         const int row = rbase + lane;
-        const int col0 = hh ? ti.n0 + (quarter >> 1) * (ti.bn >> 1) : ti.n0;
+        const int col0 = trans ? ti.m0 : hh ? ti.n0 + (quarter >> 1) * (ti.bn >> 1) : ti.n0;
         const int bn = hh ? ti.bn >> 1 : ti.bn;                        // columns this warp's lanes hold
         const float sa = ti.c_out;
         if (!ptx::mbar_wait_sleepy(sm.tfull(acc), acc_phase, abort_flag)) { stalled = true; break; }
@@ -538,14 +568,15 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
             const bool issuer = (quarter & 1) == 0 && chalf == 0 && lane == 0;
             const CUtensorMap* map_c = maps + (size_t)ti.slot * NMAP + ti.c_buf;
             const int nbx = (bn + 63) >> 6;
-            const int brow = ti.m0 + 128 * (int)rank + 64 * g;     // first row of this group's boxes
+            const int brow = (trans ? ti.n0 : ti.m0) + 128 * (int)rank + 64 * g;     // first row of this group's boxes
             int bsel = 0;
             for (int kx = 0; kx < nbx; ++kx) {
                 const int c = (kx << 6) + (chalf << 5);
                 const int bcol = col0 + (kx << 6);                 // first column of the box
                 // 0: plain box; 1: box above the diagonal of a symmetric product (stored and mirrored); 2: diagonal box;
                 // 3: box below the diagonal (skipped). Uniform over the four warps of the group.
-                const int mode = (ti.valid & TI_MIRROR) ? 1 : !symdiag ? 0 : bcol > brow ? 1 : bcol == brow ? 2 : 3;
+                // 4: box of a transposed tile (written transposed only).
+                const int mode = trans ? 4 : (ti.valid & TI_MIRROR) ? 1 : !symdiag ? 0 : bcol > brow ? 1 : bcol == brow ? 2 : 3;
                 if (mode == 3) continue;
                 const uint32_t box = sm.stage_c(g, mode == 1 ? 0 : bsel), boxt = sm.stage_c(g, 1);
                 if (issuer) { if (mode == 1) ptx::bulk_wait_read<0>(); else ptx::bulk_wait_read<1>(); }   // the stores that read these buffers are done with them
@@ -589,7 +620,9 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                 uint32_t hp[16];
 #pragma unroll
                 for (int j = 0; j < 16; ++j) { __half2 h = __floats2half2_rn(f[2 * j], f[2 * j + 1]); hp[j] = *reinterpret_cast<uint32_t*>(&h); }
-                if (mode != 2) {
+                if (mode == 4) {
+                    ptx::st_box_col(box, rbox, chalf << 5, hp);
+                } else if (mode != 2) {
                     ptx::st_box_row(box, rbox, chalf << 2, hp);
                     if (mode == 1) ptx::st_box_col(boxt, rbox, chalf << 5, hp);
                 } else {
@@ -598,7 +631,9 @@ __device__ __forceinline__ void g2_epilogue(const G2Smem& sm, uint32_t tmem_base
                 ptx::fence_proxy_async_smem();
                 asm volatile("bar.sync %0, 128;" ::"r"(3 + g) : "memory");
                 if (issuer) {
-                    if (brow < n16) {                              // boxes below the matrix are padding
+                    if (mode == 4) {
+                        ptx::tma_store_2d(map_c, brow, bcol, box, pol);
+                    } else if (brow < n16) {                       // boxes below the matrix are padding
                         ptx::tma_store_2d(map_c, bcol, brow, box, pol);
                         if (mode == 1) ptx::tma_store_2d(map_c, brow, bcol, boxt, pol);
                     }

@@ -102,6 +102,7 @@ struct PEngine {
     int l2_load, l2_store;        // L2 eviction priority of the operand loads / of the stores of C (1 evict_first, 2 evict_last, 3 normal)
     int lowdin;                   // 0: Eq. 6 on A = S^-1 H0 - mu I; 1: symmetric (Loewdin) form
     int sym_tiles;                // 1: symmetric products multiply the upper triangle of tiles only
+    int trans_tiles;              // 1: tiles of a ragged last row block are computed transposed (TI_TRANS)
     int n_mu; float mu[P_MAX_MU]; // trial chemical potentials of this call (1 for nolsm_density_matrix)
     int count_only;               // 1: D is not written, only e and q per trial mu (nolsm_electron_counts)
     double* nelec_mu;             // [P_MAX_MU] sum_i q_i per trial mu (count_only)
@@ -614,8 +615,13 @@ __device__ __forceinline__ void p_scheduler(const G2Smem& sm, const PEngine& e, 
                     tm = t / ntm; tn = t - tm * ntm;
                 }
                 ti.m0 = tm * BM; ti.n0 = tn * BN; ti.bn = min(BN, g0.z - tn * BN);
+                const int rleft = g0.z - tm * BM;                // rows of this row block
+                if (e.trans_tiles && rleft < BM && tn < ntm - 1 && !(tflags & (TI_MIRROR | TI_SYMDIAG))) {
+                    // ragged last row block, full-width column tile: computed transposed, the MMA's N = the rows left
+                    tflags |= TI_TRANS; ti.bn = rleft;
+                } else
                 // the last row block when at most 128 rows are left: one M = 128 MMA per 16 k instead of M = 256
-                if (g0.z - tm * BM <= BM / 2 && (ti.bn & 31) == 0) tflags |= TI_HALF;
+                if (rleft <= BM / 2 && (ti.bn & 31) == 0) tflags |= TI_HALF;
             }
             ti.n = g0.y; ti.n16 = g0.z; ti.nreports = pend_nt;
             ti.kind = o0.x; ti.a_buf = o0.y; ti.b_buf = o0.z; ti.c_buf = o0.w;

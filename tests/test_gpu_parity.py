@@ -207,23 +207,50 @@ def test_density_matrix_range_touches_only_its_rows(cfg0):
     assert abs(e - cmp["e_ref"]) / abs(cmp["e_ref"]) <= TOL_MIXED_E
 
 
-@pytest.mark.parametrize("engine", ["persistent", "persistent-fulltiles", "lowdin", "rounds"])
+@pytest.mark.parametrize("engine", ["persistent", "persistent-fulltiles", "persistent-untransposed", "lowdin", "rounds"])
 @pytest.mark.parametrize("name,n_atoms,sample", [("cfg1", 600, 6), ("cfg2", 300, 3), ("cfg3", 1500, 6)])
 def test_small_proxies_mixed(name, n_atoms, sample, engine):
     """Reduced-size versions of configs 1-3 (same density, basis and generator): several tiles per
-    matrix (mirrored off-diagonal tiles, ragged tails, half-height corner tiles), mixed 5/13 basis for cfg3. Oracle on a
-    seeded sample of atoms. rounds: the FFMA round engine on FP16 operands."""
+    matrix (mirrored off-diagonal tiles, ragged tails, transposed tiles of the last row block, half-height corner tiles),
+    mixed 5/13 basis for cfg3. Oracle on a seeded sample of atoms. -untransposed: the last row block as M = 256 / 128 tiles;
+    rounds: the FFMA round engine on FP16 operands."""
     from paper_2205_12182_b200 import ENGINE_PERSISTENT, ENGINE_ROUNDS, ITER_LOWDIN
     s = make_system(name, n_atoms=n_atoms)
     atoms = np.random.default_rng(1).choice(s.n_atoms, sample, replace=False)
     kw = {"persistent": dict(engine=ENGINE_PERSISTENT), "persistent-fulltiles": dict(symmetric_tiles=-1),
-          "lowdin": dict(iteration=ITER_LOWDIN), "rounds": dict(engine=ENGINE_ROUNDS)}[engine]
+          "persistent-untransposed": dict(transposed_tiles=-1), "lowdin": dict(iteration=ITER_LOWDIN), "rounds": dict(engine=ENGINE_ROUNDS)}[engine]
     D, E, st, stats = _run(s, **kw)
     cmp = compare_atoms(s, D, st["e_atom"], atoms)
     print(name, {k: v for k, v in cmp.items() if k != "ref"}, stats)
     assert (st["status"] == 0).all()
     assert cmp["max_abs_dD"] <= TOL_MIXED_D
     assert cmp["rel_dE"] <= TOL_MIXED_E
+
+
+def test_transposed_last_row_block_over_every_remainder():
+    """The tiles of a ragged last row block are computed as C^T = B^T A^T (TI_TRANS): submatrix dimensions whose remainder
+    modulo 256 runs over 16 .. 240 (both sides of the 128-row limit of the half-height corner tile, one and two boxes per
+    CTA), every tile multiplied so that the symmetric products take the transposed tiles too; against the oracle on a
+    sample and against the untransposed engine on every atom."""
+    s = make_system("cfg2", n_atoms=300)
+    runs = {}
+    for key, kw in (("trans", dict(symmetric_tiles=-1)), ("plain", dict(symmetric_tiles=-1, transposed_tiles=-1))):
+        runs[key] = _run(s, **kw)
+        assert (runs[key][2]["status"] == 0).all()
+    Dt, Dp = runs["trans"][0], runs["plain"][0]
+    dims = runs["trans"][2]["dims"]
+    rem = np.unique(((dims[dims > 256] + 15) // 16 * 16) % 256)
+    print("remainders", rem)
+    assert (rem > 128).any() and ((rem > 0) & (rem <= 128)).any() and len(rem) >= 8
+    # same arithmetic per element (k order of the MMA, FP32 accumulation); run-to-run differences come from the order of the
+    # residual atomics only, which can move a convergence decision by one iteration
+    assert np.abs(Dt - Dp).max() <= TOL_MIXED_D
+    atoms = np.random.default_rng(9).choice(s.n_atoms, 3, replace=False)
+    cmp = compare_atoms(s, Dt, runs["trans"][2]["e_atom"], atoms)
+    assert cmp["max_abs_dD"] <= TOL_MIXED_D and cmp["rel_dE"] <= TOL_MIXED_E
+    # the executed (padded) work shrinks, the useful work does not change
+    assert runs["trans"][3]["flops_padded"] < runs["plain"][3]["flops_padded"]
+    assert runs["trans"][3]["flops_padded"] >= runs["trans"][3]["flops_useful"]
 
 
 def test_plain_newton_schulz_matches_scaled():

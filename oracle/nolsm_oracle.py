@@ -252,6 +252,21 @@ def combine_cost(n, mode, perf_table=None):
     return t * t * ((n16 + 63) // 64)
 
 
+def predicted_seconds(flop, rate_flops):
+    """Predicted runtime of `flop` floating-point operations at a measured rate (FLOP/s): flop / rate. This is the reading
+    of Eq. 10's "predicted runtime p(n) x n^3" (L89-91) that Table II (L119-126) fixes: its "estimated speedup" column is
+    (FLOP count / estimated performance) of the uncombined set over that of the combined set (C-19)."""
+    return float(flop) / float(rate_flops)
+
+
+def estimated_performance(dims, perf_table):
+    """Table II's "estimated performance" of a set of submatrices for one multiplication each: total FLOP (2 n^3, L156)
+    over total predicted runtime, sum 2 n^3 / sum (2 n^3 / r(n)), in the unit of the table's rates."""
+    flop = sum(2.0 * float(n) ** 3 for n in dims)
+    sec = sum(predicted_seconds(2.0 * float(n) ** 3, perf_rate(perf_table, n)) for n in dims)
+    return flop / sec
+
+
 def combine_groups(atom_nb, index_sets, mode=1, max_dim=2048, max_members=16, max_candidates=24, perf_table=None):
     """Greedy combination of columns (atoms) into groups that share ONE submatrix (C-19).
 

@@ -211,3 +211,44 @@ def test_combination_is_at_least_as_close_to_full_eq5_on_cfg0():
             err_single += float(((one["Dcols"] - ref) ** 2).sum())
             err_comb += float(((res[i]["Dcols"] - ref) ** 2).sum())
     assert err_comb < err_single
+
+
+def _table2():
+    import os
+    rows = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_table2.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            c = line.split()
+            rows[c[0]] = dict(count=int(c[1]), smallest=int(c[2]), largest=int(c[3]), average=float(c[4]),
+                              pflop=float(c[5]), tflops=float(c[6]), speedup=None if c[7] == "-" else float(c[7]))
+    return rows
+
+
+def test_table2_fixes_the_reading_of_eq10_runtime():
+    """PAPER.md Table II (tests/golden/paper_table2.txt): the paper's "estimated speedup" 2.9 / 3.2 is the ratio of
+    (FLOP count / estimated performance), i.e. the predicted runtime of Eq. 10 is FLOP / p(n) (oracle.predicted_seconds,
+    DESIGN.md C-19); the literal product p(n) x n^3 with p a rate would give a slow-down."""
+    t = _table2()
+    base = orc.predicted_seconds(t["no"]["pflop"] * 1e15, t["no"]["tflops"] * 1e12)
+    for key in ("eq9", "eq10"):
+        sec = orc.predicted_seconds(t[key]["pflop"] * 1e15, t[key]["tflops"] * 1e12)
+        assert round(base / sec, 1) == t[key]["speedup"], (key, base / sec)
+        literal = (t["no"]["pflop"] * t["no"]["tflops"]) / (t[key]["pflop"] * t[key]["tflops"])
+        assert literal < 1.0                                    # the literal reading contradicts the printed speedup
+    # the narrative around the table (L93): Eq. 10 about doubles the average dimension of Eq. 9 and slightly raises the FLOP count
+    assert 1.5 < t["eq10"]["average"] / t["eq9"]["average"] < 2.0
+    assert t["eq9"]["pflop"] < t["eq10"]["pflop"] < t["no"]["pflop"]
+
+
+def test_estimated_performance_is_the_flop_weighted_harmonic_mean():
+    """Table II's "estimated performance" of a set: total FLOP over total predicted runtime. Flat table: the rate itself;
+    two sizes: worked by hand; merging small matrices into larger ones under a rising p(n) raises it (the paper's point)."""
+    flat = (np.array([100, 4000]), np.array([700, 700]))
+    assert abs(orc.estimated_performance([300, 900, 2500], flat) - 700.0) < 1e-9
+    tab = (np.array([500, 1000]), np.array([100, 300]))
+    # n = 500: 2.5e8 FLOP at 100; n = 1000: 2e9 FLOP at 300 -> (2.5e8 + 2e9) / (2.5e6 + 6.6667e6)
+    want = (2.5e8 + 2.0e9) / (2.5e8 / 100 + 2.0e9 / 300)
+    assert abs(orc.estimated_performance([500, 1000], tab) - want) / want < 1e-12
+    assert orc.estimated_performance([1000] * 4, tab) > orc.estimated_performance([500] * 32, tab)

@@ -136,3 +136,26 @@ def test_cfg1_full_combined_groups_and_parity():
     print("cfg1 full combined", len(groups), "groups, max|dD|", max_d, "rel dE", abs(e_gpu - e_ref) / abs(e_ref))
     assert max_d <= TOL_D and abs(e_gpu - e_ref) / abs(e_ref) <= TOL_E
     assert abs(E - st["e_atom"].sum()) <= 1e-9 * abs(E)
+
+
+def test_large_dimension_submatrices():
+    """Maximum sizes: the largest system of the p(n) sweep (`pn-14-8.5`: 14 functions per atom, cutoff 8.5 A, submatrices of
+    ~3,600 dimensions = 15 x 15 tiles, 57 k-blocks per tile), the regime of the paper's largest submatrices after
+    combination (Table II: thousands of dimensions). A range of atoms through nolsm_density_matrix_range, one of them
+    against the oracle (a 3,600-dimensional generalised eigenproblem in FP64)."""
+    from paper_2205_12182_b200 import Nolsm
+    s = make_system("pn-14-8.5", n_atoms=1024)
+    nb, rp, ci, Hv, Sv = _device_inputs(s)
+    D = torch.zeros_like(Hv)
+    a0, a1 = 100, 112
+    with Nolsm(0) as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        e = ctx.density_matrix_range(s.mu, a0, a1, D, want_energy=True)
+        st = ctx.atom_stats()
+        stats = ctx.stats()
+    dims = st["dims"][a0:a1]
+    print("large", dims.min(), dims.max(), stats["gemms_executed"] / (a1 - a0))
+    assert dims.min() >= 3000
+    assert (st["status"][a0:a1] == 0).all()
+    assert abs(e - st["e_atom"][a0:a1].sum()) <= 1e-9 * abs(e)
+    _check_sample(s, D, st["e_atom"], [a0 + 5], "pn-14-8.5, one atom of ~3600 dimensions")

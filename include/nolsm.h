@@ -113,6 +113,11 @@ typedef struct {
     int transposed_tiles;    /* persistent engine: the tiles of a ragged last row block (r < 256 rows left) are computed transposed,
                                 C^T = B^T A^T, so the MMA's M = 256 runs over full columns and its N = r over the rows that exist,
                                 instead of M = 256 (or 128) over r rows [0 = on; -1 = off] */
+    int diag_drop_operand_loads; /* DIAGNOSTIC, persistent engine: bit 0: the TMA producers do not load the second 64-row box of the
+                                A operand of a tile, bit 1: not the second 64-column box of B; the tensor cores multiply what the
+                                stage held before. The results of such a call are MEANINGLESS (status words report what the
+                                iterations did with them); the call measures what the operand traffic costs: a quarter / a half
+                                fewer bytes per FLOP (profiles/r02_persist.md) [0] */
 } nolsm_options;
 
 typedef struct {

@@ -28,7 +28,7 @@ class NolsmOptions(C.Structure):
                 ("combine_max_members", C.c_int), ("combine_max_candidates", C.c_int), ("iteration", C.c_int),
                 ("symmetric_tiles", C.c_int), ("heavy_slots", C.c_int), ("claim_lead", C.c_int), ("mu_trials", C.c_int),
                 ("timeout_s", C.c_double), ("scan_order", C.c_int), ("l2_load_policy", C.c_int), ("l2_store_policy", C.c_int),
-                ("transposed_tiles", C.c_int)]
+                ("transposed_tiles", C.c_int), ("diag_drop_operand_loads", C.c_int)]
 
 
 class NolsmStats(C.Structure):

@@ -439,6 +439,7 @@ int engine_plan(nolsm_ctx* c, cudaStream_t s) {
         pe.l2_load = c->opt.l2_load_policy > 0 ? c->opt.l2_load_policy : 1; pe.l2_store = c->opt.l2_store_policy > 0 ? c->opt.l2_store_policy : 2;
         pe.sym_tiles = c->opt.symmetric_tiles >= 0 ? 1 : 0;
         pe.trans_tiles = c->opt.transposed_tiles >= 0 ? 1 : 0;
+        pe.diag_drop = c->opt.diag_drop_operand_loads & 3;
         pe.n_mu = 1; pe.count_only = 0;
         pe.nelec_mu = c->d_mu_acc; pe.e_mu = c->d_mu_acc + NOLSM_MAX_MU;
         pe.elem_chunks = 16;

@@ -507,13 +507,14 @@ def main():
     gemm_tf_paper = args.steps * stats["flops_paper"] / max(prof_acc["gemm_ms"], 1e-9) / 1e9
     sampled_ms = prof_acc["gemm_ms"] + prof_acc["gather_ms"] + prof_acc["dcols_ms"] + prof_acc["other_ms"]
     # DRAM traffic of the kernel: NOT measured in this run. It is the figure of the committed ncu --set full capture
-    # (profiles/gemm_traffic.json: per submatrix on a 1024-submatrix launch of the same workload), scaled to one launch here.
+    # (profiles/gemm_traffic.csv: per submatrix on a 1024-submatrix launch of the same workload), scaled to one launch here.
     traffic, traffic_note = None, None
-    tp = os.path.join(ROOT, "profiles", "gemm_traffic.json")
+    tp = os.path.join(ROOT, "profiles", "gemm_traffic.csv")
     if os.path.exists(tp) and args.workload == "cfg2":
-        with open(tp) as f:
-            tj = json.load(f)
-        traffic = tj.get("dram_bytes_per_submatrix", 0.0) * system.n_atoms or None
+        import csv
+        with open(tp, newline="") as f:
+            tj = {r[0]: r[1] for r in csv.reader(f) if len(r) == 2}
+        traffic = float(tj.get("dram_bytes_per_submatrix", 0.0)) * system.n_atoms or None
         traffic_note = tj.get("capture")
     roofline = {"bound": "tensor", "kernel": "nolsm_persist_kernel" if persistent else "k_gemm_simt",
                 "achieved": gemm_tf, "peak": peaks["bf16_tflops_sustained"],

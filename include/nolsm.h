@@ -221,6 +221,41 @@ int nolsm_get_index_set(nolsm_ctx* ctx, int64_t atom, int32_t* atoms_out, int32_
  * nolsm_get_group; FP16 only). which: 0 = T(S), 1 = T(H0). out_fp16 != 0 -> uint16 FP16 bits, else float. */
 int nolsm_gather_submatrix(nolsm_ctx* ctx, int64_t atom, int which, int out_fp16, void* out_host);
 
+/* The same gather as nolsm_gather_submatrix (FP16 output), for callers that must not allocate device memory.
+ *
+ * Who that is: a host program that has already handed all of the GPU's memory to its own pool (a tensor framework's
+ * caching allocator, an MD code's arena) so that any further cudaMalloc fails; and a program that inspects submatrices
+ * while other work is in flight on the GPU, because cudaMalloc / cudaFree synchronise the whole device and would stall
+ * until, for example, a running density-matrix kernel of several seconds has finished. nolsm_gather_submatrix does one
+ * cudaMalloc + cudaFree per call and gathers into the context's workspace; this entry point calls no cudaMalloc,
+ * cudaFree or any other allocating routine, and leaves the workspace and the results of the last density_matrix call
+ * untouched.
+ *
+ * What it uses instead: the gather kernel writes the padded dense T(S) and T(H0) (rows of n16 = n rounded up to 16
+ * FP16 values, 16-byte stores) into a scratch array that is part of the library image: a fixed `static __device__`
+ * array of 2 * NOLSM_NOALLOC_MAX_DIM^2 FP16 values = 16 MiB. Every GPU on which the library is loaded holds these
+ * 16 MiB from the moment the library's device code is loaded there until the process exits, whether or not this
+ * function is ever called. The requested matrix is then copied, tight, from the scratch array to `out`.
+ *   atom       the atom; with options.combine the submatrix of the atom's group is gathered (dimension: nolsm_get_group)
+ *   which      0 = T(S), 1 = T(H0)
+ *   out        uint16 FP16 bits, n x n row-major, tight; memory the CALLER owns. Device memory: the kernel and the copy
+ *              are enqueued on `cuda_stream` and the call returns without waiting. Host memory: the call waits for the
+ *              stream before it returns.
+ * Limit: a submatrix whose padded dimension n16 exceeds NOLSM_NOALLOC_MAX_DIM is refused with NOLSM_EINVAL (the text of
+ * nolsm_last_error names both numbers); nothing is launched. Persistent engine only (NOLSM_ESTATE otherwise).
+ *
+ * First call on a device: it looks up the device address of the scratch array (cudaGetSymbolAddress) and raises the
+ * kernel's shared-memory limit, once per device and process. Make that first call outside any stream capture; later
+ * calls only launch one kernel and one 2-D copy.
+ *
+ * Sharing: there is ONE scratch array per GPU, shared by every context and every thread of the process. Calls whose GPU
+ * work can overlap (different streams, or different contexts on one device) overwrite each other's scratch and return
+ * garbage: keep them on one stream, or order them with events. The array keeps whatever the previous call left in it;
+ * that is harmless, because each call writes every element it later copies out (the kernel zero-fills its row strips
+ * before placing the blocks), so nothing has to be cleared between calls. */
+#define NOLSM_NOALLOC_MAX_DIM 2048
+int nolsm_gather_submatrix_noalloc(nolsm_ctx* ctx, int64_t atom, int which, void* out, void* cuda_stream);
+
 int nolsm_get_stats(nolsm_ctx* ctx, nolsm_stats* out);
 
 /* Per-atom results of the last density_matrix call for atoms [atom_begin, atom_begin + count); any

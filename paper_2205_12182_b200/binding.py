@@ -76,6 +76,7 @@ def load_library():
                                   C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int)]
     lib.nolsm_get_group.argtypes = [P, I64, P, C.POINTER(C.c_int32), P, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     lib.nolsm_gather_submatrix.argtypes = [P, I64, I32, I32, P]
+    lib.nolsm_gather_submatrix_noalloc.argtypes = [P, I64, I32, P, P]
     lib.nolsm_get_stats.argtypes = [P, C.POINTER(NolsmStats)]
     lib.nolsm_get_atom_stats.argtypes = [P, I64, I64, P, P, P, P, P, P, P]
     lib.nolsm_get_profile.argtypes = [P, C.POINTER(C.c_double), I32]
@@ -86,7 +87,7 @@ def load_library():
     lib.nolsm_last_error.argtypes = [P]
     lib.nolsm_last_error.restype = C.c_char_p
     for f in ("nolsm_create", "nolsm_assemble", "nolsm_density_matrix", "nolsm_density_matrix_range", "nolsm_energy",
-              "nolsm_destroy", "nolsm_get_index_set", "nolsm_get_group", "nolsm_electron_count", "nolsm_find_mu", "nolsm_gather_submatrix", "nolsm_get_stats",
+              "nolsm_destroy", "nolsm_get_index_set", "nolsm_get_group", "nolsm_electron_count", "nolsm_find_mu", "nolsm_gather_submatrix", "nolsm_gather_submatrix_noalloc", "nolsm_get_stats",
               "nolsm_get_atom_stats", "nolsm_get_profile", "nolsm_get_engine_counters", "nolsm_electron_counts",
               "nolsm_set_perf_table", "nolsm_side_task_bandwidth"):
         getattr(lib, f).restype = C.c_int
@@ -238,6 +239,24 @@ class Nolsm:
         _, _, dim = self.group(atom)                 # the submatrix the atom is evaluated on (its own without combine)
         out = np.empty((dim, dim), dtype=np.float16 if fp16 else np.float32)
         self._check(self._lib.nolsm_gather_submatrix(self._h, atom, which, 1 if fp16 else 0, out.ctypes.data))
+        return out
+
+    def gather_submatrix_noalloc(self, atom: int, which: int, out, stream: int = 0):
+        """nolsm_gather_submatrix_noalloc (include/nolsm.h): the FP16 gather of the submatrix `atom` is evaluated on, with
+        the kernel's scratch in the library's static device array, so the library allocates nothing -- for a process whose
+        device memory is all spoken for, or that cannot afford the device-wide wait of a cudaMalloc. `out` is the
+        caller's own float16 buffer of dim x dim elements (dim from `group(atom)`): a CUDA tensor (asynchronous on
+        `stream`) or a host tensor / numpy array (the call waits). Dimensions beyond 2048 raise. This method allocates
+        nothing either; it passes addresses through."""
+        if hasattr(out, "data_ptr"):
+            if str(out.dtype) != "torch.float16" or not out.is_contiguous():
+                raise TypeError("out must be a contiguous float16 tensor")
+            addr = out.data_ptr()
+        else:
+            if out.dtype != np.float16 or not out.flags["C_CONTIGUOUS"]:
+                raise TypeError("out must be a C-contiguous float16 array")
+            addr = out.ctypes.data
+        self._check(self._lib.nolsm_gather_submatrix_noalloc(self._h, atom, which, addr, stream))
         return out
 
     def stats(self) -> dict:

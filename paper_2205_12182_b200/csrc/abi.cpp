@@ -429,6 +429,16 @@ int nolsm_gather_submatrix(nolsm_ctx* c, int64_t atom, int which, int out_fp16, 
     return engine_gather(c, atom, false, which, out_fp16, out_host);
 }
 
+// The gather without device allocations (static scratch array in engine.cu). It does not wait for the last
+// density_matrix call: it reads only the pattern and the H0 / S values and writes only the scratch array and `out`.
+int nolsm_gather_submatrix_noalloc(nolsm_ctx* c, int64_t atom, int which, void* out, void* cuda_stream) {
+    if (!c || !out || (which != 0 && which != 1)) return NOLSM_EINVAL;
+    if (!c->assembled) return fail(c, NOLSM_ESTATE, "not assembled");
+    if (atom < 0 || atom >= c->n_atoms) return fail(c, NOLSM_EINVAL, "atom out of range");
+    cudaSetDevice(c->dev);
+    return engine_gather_noalloc(c, c->combined ? c->unit_of[atom] : atom, which, out, (cudaStream_t)cuda_stream);
+}
+
 int nolsm_get_atom_stats(nolsm_ctx* c, int64_t a0, int64_t count, int32_t* dims, int32_t* inv_iters, int32_t* sign_iters,
                          int32_t* status, int32_t* gemms, float* residual, double* e_atom) {
     if (!c) return NOLSM_EINVAL;

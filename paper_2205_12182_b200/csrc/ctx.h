@@ -173,5 +173,6 @@ int engine_atom_stats(nolsm_ctx* c, int64_t a0, int64_t count, int32_t* dims, in
 int engine_status_bits(nolsm_ctx* c, int* bits);
 int engine_gather(nolsm_ctx* c, int64_t unit_or_atom, bool is_unit, int which, int out_fp16, void* out_host);
 int engine_side_bandwidth(nolsm_ctx* c, int which, int reps, double* ms_out, double* bytes_out);
+int engine_gather_noalloc(nolsm_ctx* c, int64_t unit, int which, void* out, cudaStream_t s);   // static device scratch, no allocation
 
 }  // namespace nolsm_host

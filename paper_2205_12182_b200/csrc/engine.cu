@@ -785,3 +785,97 @@ int engine_side_bandwidth(nolsm_ctx* c, int which, int reps, double* ms_out, dou
 }
 
 }  // namespace nolsm_host
+
+// =====================================================================================================================
+// nolsm_gather_submatrix_noalloc (include/nolsm.h): the gather task a1 for one submatrix without any device allocation.
+//
+// For callers that cannot allocate: all device memory already belongs to the host program's own pool, or a cudaMalloc /
+// cudaFree (which wait for the whole device) would stall behind kernels that are still running. The dense, padded
+// T(S) | T(H0) pair that the existing path puts into workspace slot 0 goes into the array below instead, which is part of
+// the library image: 2 * 2048^2 FP16 values = 16 MiB on every GPU that loads this library, until the process exits.
+//
+// The name `g_noalloc_scratch` is a device address only inside device code. In host code it names a host-side shadow
+// object; handing that to a kernel makes the kernel fault (or, on systems where the GPU can reach host memory, scribble
+// over the shadow). Host code therefore asks the runtime for the device address, once per device with that device
+// current (noalloc_setup), and passes the returned pointer to the kernel.
+// =====================================================================================================================
+#include <mutex>
+
+constexpr int NOALLOC_MAX_DIM = NOLSM_NOALLOC_MAX_DIM;
+constexpr size_t NOALLOC_HALVES = 2ull * NOALLOC_MAX_DIM * NOALLOC_MAX_DIM;
+static_assert(NOALLOC_MAX_DIM % 16 == 0, "rows of the scratch matrices are written with 16-byte stores");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_HALVES * sizeof(__half)];
+
+namespace nolsm {
+// side_gather_chunk of the persistent kernel (persist.cuh) launched alone like k_side_gather, but the unit and its
+// dimension come by value (no device-side id list) and the two dense matrices go to `scratch` | `scratch + bufsz`.
+// grid = chunks of row-atoms, one 128-thread side group per CTA.
+template <typename TV>
+__global__ void __launch_bounds__(P_SIDE_THREADS) k_side_gather_scratch(SysView sv, const TV* S_vals, const TV* H_vals, __half* scratch,
+                                                                        long long bufsz, int ld, int unit, int n) {
+    extern __shared__ unsigned char sm_dyn[];
+    side_gather_chunk<TV>(sv, S_vals, H_vals, scratch, scratch + bufsz, unit, n, (n + 15) & ~15, ld, blockIdx.x, gridDim.x, sm_dyn,
+                          threadIdx.x, nullptr);
+}
+}  // namespace nolsm
+
+namespace {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mutex;
+__half* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};      // device address of g_noalloc_scratch on device d, once looked up
+
+// Once per device and process, with that device current: the device address of the scratch array and the shared-memory
+// limit of the two kernel instances. Neither call allocates device memory.
+int noalloc_setup(nolsm_ctx* c, __half** out) {
+    int dev = -1;
+    CU_TRY(c, cudaGetDevice(&dev));
+    if (dev != c->dev) { CU_TRY(c, cudaSetDevice(c->dev)); dev = c->dev; }
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(c, NOLSM_EINVAL, "nolsm_gather_submatrix_noalloc: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        void* p = nullptr;
+        CU_TRY(c, cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        CU_TRY(c, cudaFuncSetAttribute(k_side_gather_scratch<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SIDE_SMEM));
+        CU_TRY(c, cudaFuncSetAttribute(k_side_gather_scratch<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SIDE_SMEM));
+        g_noalloc_ptr[dev] = static_cast<__half*>(p);
+    }
+    *out = g_noalloc_ptr[dev];
+    return NOLSM_OK;
+}
+}  // namespace
+
+namespace nolsm_host {
+
+// Gathers unit `unit` (an atom without combination) into the static scratch array and copies matrix `which` tight to
+// `out` (device: asynchronous on s; host: the call waits). No cudaMalloc / cudaFree / allocating routine on this path.
+// Every element the copy reads is written by the kernel of the same call (zero-filled strips, then the blocks), so the
+// contents the previous call left behind need no clearing. Calls that overlap on the GPU race on the array.
+int engine_gather_noalloc(nolsm_ctx* c, int64_t unit, int which, void* out, cudaStream_t s) {
+    if (!c->persist) return fail(c, NOLSM_ESTATE, "nolsm_gather_submatrix_noalloc needs the persistent engine (FP16 operands)");
+    const int n = c->udim[unit], n16 = (n + 15) & ~15;
+    if (n16 > NOALLOC_MAX_DIM)
+        return fail(c, NOLSM_EINVAL, "nolsm_gather_submatrix_noalloc: padded submatrix dimension " + std::to_string(n16) +
+                                         " exceeds NOLSM_NOALLOC_MAX_DIM = " + std::to_string(NOALLOC_MAX_DIM) +
+                                         " (the static scratch array holds two 2048 x 2048 FP16 matrices); use nolsm_gather_submatrix");
+    __half* scratch = nullptr;
+    if (int r = noalloc_setup(c, &scratch)) return r;
+    const PEngine& pe = *c->peng;
+    const int nset = (int)(c->uset_ptr[unit + 1] - c->uset_ptr[unit]);
+    const long long bufsz = (long long)n16 * n16;
+    const int ld = n16;
+    const dim3 grid((nset + pe.gather_rowatoms - 1) / pe.gather_rowatoms, 1);
+    if (c->val_dtype == NOLSM_DTYPE_F64)
+        k_side_gather_scratch<double><<<grid, P_SIDE_THREADS, P_SIDE_SMEM, s>>>(pe.sv, (const double*)c->dS, (const double*)c->dH, scratch,
+                                                                                 bufsz, ld, (int)unit, n);
+    else
+        k_side_gather_scratch<float><<<grid, P_SIDE_THREADS, P_SIDE_SMEM, s>>>(pe.sv, (const float*)c->dS, (const float*)c->dH, scratch,
+                                                                                bufsz, ld, (int)unit, n);
+    CU_TRY(c, cudaGetLastError());
+    const bool on_device = is_device_ptr(out);
+    CU_TRY(c, cudaMemcpy2DAsync(out, (size_t)n * 2, scratch + (size_t)which * bufsz, (size_t)ld * 2, (size_t)n * 2, n,
+                                on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s));
+    if (!on_device) CU_TRY(c, cudaStreamSynchronize(s));
+    return NOLSM_OK;
+}
+
+}  // namespace nolsm_host

@@ -139,6 +139,15 @@ typedef struct {
     double flops_paper;           /* sum_i 2 n_i^3 * gemms_i with every product counted in full (PAPER.md:L156 knows no symmetric ones) */
 } nolsm_stats;
 
+/* Layout check for bindings that restate the structs above (paper_2205_12182_b200/binding.py does): the version is bumped
+ * whenever a field of nolsm_options / nolsm_stats or the meaning of an existing argument changes, and the two sizes are the
+ * library's own sizeof. A binding compares all three with its own at load time and refuses a stale libnolsm.so instead
+ * of silently misreading every option behind the first changed field. Needs no context and no GPU. */
+#define NOLSM_ABI_VERSION 4
+int nolsm_abi_version(void);
+size_t nolsm_sizeof_options(void);
+size_t nolsm_sizeof_stats(void);
+
 /* Creates a context on `cuda_device`. opt may be NULL. */
 int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt);
 

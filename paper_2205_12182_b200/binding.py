@@ -14,6 +14,7 @@ ENGINE_AUTO, ENGINE_PERSISTENT, ENGINE_ROUNDS = 0, 1, 2
 ITER_EQ6, ITER_LOWDIN = 0, 1
 STATUS_NAMES = {0: "OK", 1: "EINVAL", 2: "ECUDA", 3: "ENOMEM", 4: "ESTATE", 5: "ENOTSPD", 6: "ENOCONV"}
 
+ABI_VERSION = 4                                     # NOLSM_ABI_VERSION of the include/nolsm.h this file restates
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
@@ -53,6 +54,21 @@ def lib_path() -> str:
     return os.path.join(_HERE, "libnolsm.so")
 
 
+def _check_abi(lib, path):
+    """Refuses a libnolsm.so built from another header: same version number and the library's sizeof of both structs
+    must equal this file's ctypes restatement (a stale library would misread every option behind the first changed field)."""
+    stale = f"{path} is stale: rebuild it with `python -m paper_2205_12182_b200.build --force`"
+    if not hasattr(lib, "nolsm_abi_version"):
+        raise ImportError(f"{stale} (it predates nolsm_abi_version)")
+    lib.nolsm_abi_version.restype = C.c_int
+    lib.nolsm_sizeof_options.restype = C.c_size_t
+    lib.nolsm_sizeof_stats.restype = C.c_size_t
+    got = (lib.nolsm_abi_version(), lib.nolsm_sizeof_options(), lib.nolsm_sizeof_stats())
+    want = (ABI_VERSION, C.sizeof(NolsmOptions), C.sizeof(NolsmStats))
+    if got != want:
+        raise ImportError(f"{stale} (ABI version, sizeof(nolsm_options), sizeof(nolsm_stats): library {got}, binding {want})")
+
+
 def load_library():
     """Loads libnolsm.so (built in-tree by paper_2205_12182_b200/build.py). Fails loudly if absent."""
     global _LIB
@@ -63,6 +79,7 @@ def load_library():
         raise ImportError(f"{path} is missing: run `python -m paper_2205_12182_b200.build` "
                           "(there is no CPU fallback)")
     lib = C.CDLL(path)
+    _check_abi(lib, path)
     P, I64, I32 = C.c_void_p, C.c_int64, C.c_int
     lib.nolsm_create.argtypes = [C.POINTER(P), I32, C.POINTER(NolsmOptions)]
     lib.nolsm_assemble.argtypes = [P, I64, P, P, P, P, P, I32, P]

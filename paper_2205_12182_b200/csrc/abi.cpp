@@ -151,6 +151,10 @@ int run(nolsm_ctx* c, const double* mu, int n_mu, bool count_only, int64_t a0, i
 // =================================================================================================
 extern "C" {
 
+int nolsm_abi_version(void) { return NOLSM_ABI_VERSION; }
+size_t nolsm_sizeof_options(void) { return sizeof(nolsm_options); }
+size_t nolsm_sizeof_stats(void) { return sizeof(nolsm_stats); }
+
 int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
     if (!out) return NOLSM_EINVAL;
     *out = nullptr;

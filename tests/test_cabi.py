@@ -46,6 +46,30 @@ def test_option_and_stats_structs_match_header():
     assert names == [f for f, _ in NolsmStats._fields_]
 
 
+def test_abi_version_and_struct_sizes_are_checked_at_load(lib):
+    """The library reports its ABI version and its own sizeof of both structs; the binding compares them at load time and
+    refuses a mismatch (a stale libnolsm.so would otherwise misread the options silently)."""
+    from paper_2205_12182_b200 import NolsmOptions, NolsmStats, binding
+    text = open(os.path.join(ROOT, "include", "nolsm.h")).read()
+    assert int(re.search(r"#define NOLSM_ABI_VERSION (\d+)", text).group(1)) == binding.ABI_VERSION == lib.nolsm_abi_version()
+    assert lib.nolsm_sizeof_options() == ctypes.sizeof(NolsmOptions)
+    assert lib.nolsm_sizeof_stats() == ctypes.sizeof(NolsmStats)
+
+    class Stale:
+        def __init__(self, version, so, ss):
+            self.nolsm_abi_version = ctypes.CFUNCTYPE(ctypes.c_int)(lambda: version)
+            self.nolsm_sizeof_options = ctypes.CFUNCTYPE(ctypes.c_size_t)(lambda: so)
+            self.nolsm_sizeof_stats = ctypes.CFUNCTYPE(ctypes.c_size_t)(lambda: ss)
+
+    so, ss = ctypes.sizeof(NolsmOptions), ctypes.sizeof(NolsmStats)
+    binding._check_abi(Stale(binding.ABI_VERSION, so, ss), "x.so")
+    for bad in (Stale(binding.ABI_VERSION - 1, so, ss), Stale(binding.ABI_VERSION, so - 4, ss), Stale(binding.ABI_VERSION, so, ss + 8)):
+        with pytest.raises(ImportError, match="stale"):
+            binding._check_abi(bad, "x.so")
+    with pytest.raises(ImportError, match="predates"):
+        binding._check_abi(object(), "x.so")
+
+
 def test_create_fails_loudly_without_a_gpu(lib):
     import torch
     if torch.cuda.is_available():

@@ -13,7 +13,9 @@
  *     pinned) or to device memory of `cuda_device`; the library detects which. Device arrays are
  *     BORROWED until nolsm_destroy or the next nolsm_assemble and never freed by the library. Host
  *     arrays are copied during the call and may be released when it returns (for asynchronous
- *     outputs: after nolsm_energy returned).
+ *     outputs: after nolsm_energy returned). A D_vals in pinned host memory is filled by a copy enqueued behind the
+ *     kernel; a D_vals in pageable host memory is filled by the first call that waits for the results (nolsm_energy, a
+ *     getter, the next density_matrix call), so that the time limit is watched while the kernel runs.
  *   - Block-CSR: row i lists the atoms j with a block (i, j), ascending. Slot s = (i, j) holds the
  *     nb(i) x nb(j) block row-major; slot s starts at element blk_off[s] = sum over earlier slots of
  *     nb(i') * nb(j'). H0 and S share one pattern (the union of their patterns), which
@@ -23,7 +25,8 @@
  *     therefore D^T in block-CSR and row i is written by submatrix i alone (with options.combine: by the submatrix of the
  *     group atom i belongs to). D is not symmetrised.
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
- *   - All functions return a nolsm_status; none throws, aborts or traps: a persistent kernel that overruns
+ *   - All functions return a nolsm_status; none throws (every entry point catches what its host code may throw and
+ *     returns NOLSM_ENOMEM / NOLSM_ECUDA with the text in nolsm_last_error), aborts or traps: a persistent kernel that overruns
  *     options.timeout_s, or in which a wait stalls (device watchdog), is stopped through an abort word and the call
  *     that waits for it returns NOLSM_ECUDA. Numerical failures of single
  *     submatrices are reported asynchronously: they set per-atom status bits (nolsm_get_atom_stats) and
@@ -103,7 +106,12 @@ typedef struct {
     int mu_trials;           /* nolsm_find_mu, persistent engine: trial mu evaluated per pass on the resident S_sub^-1, A0 [1 = bisection:
                                 a trial after the first costs ~3/4 of a pass and K trials gain log2(K + 1) bits, so K = 1 needs the
                                 least work per bit (measured: bench.py other_configs.cfg1.mu_search); max 8] */
-    double timeout_s;        /* persistent engine: the host stops a kernel that runs longer than this [300] */
+    double timeout_s;        /* persistent engine: time limit of one kernel, counted from its launch. The call that waits for the
+                                results (nolsm_energy, any getter) stops a kernel that runs longer; inside the kernel a hot wait
+                                (pipeline stages, accumulators) that lasts timeout_s / 10 (at least 2 s) or an idle wait (tile
+                                records) that lasts timeout_s (at least 20 s) counts as a stall and stops the kernel too. The abort
+                                of any kernel launched since the last wait is reported by that wait, also when later calls on
+                                the context (a series of nolsm_density_matrix_range) went through [300] */
     int scan_order;          /* persistent engine, tile schedulers: 1 = every CTA pair scans the slots from slot 0 (the chains of the first
                                 slots advance first), 2 = every pair from its own slot (74 schedulers do not queue on one claim word)
                                 [0 = auto: 2 for mean dimensions up to 768, where a tile is as short as a claim] */

@@ -73,18 +73,40 @@ int to_host(nolsm_ctx* c, const void* src, size_t bytes, void* dst, cudaStream_t
     return NOLSM_OK;
 }
 
-// Waits for the last density_matrix call. The persistent kernel is watched: past the time limit the host
-// raises the kernel's abort word (copy on a second stream), which makes the tile schedulers stop feeding and every
-// role leave its loop. A wait inside the kernel that stalls raises the same word itself (value 2, gemm_umma.cuh).
+// The abort words of every persistent launch since the last check: the running word of the last launch and the saved
+// final words of the launches before it (run_persistent saves a launch's word before the next launch clears it, so a
+// stalled kernel in a series of nolsm_density_matrix_range calls is not forgotten). Call after the stream has drained.
+int check_abort_words(nolsm_ctx* c) {
+    if (c->launch_seq == c->checked_seq) return NOLSM_OK;
+    int w[1 + NOLSM_ABORT_HIST] = {};
+    CU_TRY(c, cudaMemcpy(w, c->d_abort, sizeof(w), cudaMemcpyDeviceToHost));
+    int worst = w[0];
+    int64_t first_bad = w[0] ? c->launch_seq - 1 : -1;
+    for (int64_t k = c->launch_seq - 2; k >= c->checked_seq; --k)
+        if (w[1 + k % NOLSM_ABORT_HIST]) { worst = std::max(worst, w[1 + k % NOLSM_ABORT_HIST]); first_bad = k; }
+    const int64_t n_calls = c->launch_seq - c->checked_seq;
+    c->checked_seq = c->launch_seq;
+    if (!worst) return NOLSM_OK;
+    c->have_result = false;
+    const std::string which = n_calls > 1 ? " (call " + std::to_string(first_bad - (c->launch_seq - n_calls) + 1) + " of the " +
+                                                std::to_string(n_calls) + " since the last wait; rows written since then are incomplete)" : "";
+    c->err = (worst == 2 ? "persistent engine: a wait inside the kernel stalled (device watchdog); the results of this call are invalid"
+                         : "persistent engine exceeded its time limit and was aborted") + which;
+    return NOLSM_ECUDA;
+}
+
+// Waits for the last density_matrix call. The persistent kernel is watched: past the time limit (counted from its
+// launch) the host raises the kernel's abort word (copy on a second stream), which makes the tile schedulers stop
+// feeding and every role leave its loop. A wait inside the kernel that stalls raises the same word itself (value 2,
+// gemm_umma.cuh). A pageable host D is copied here, after the watched wait, so the watchdog also covers that case.
 int wait_result(nolsm_ctx* c) {
     if (c->last_persist) {
-        const auto t0 = std::chrono::steady_clock::now();
         bool aborted = false;
         for (;;) {
             const cudaError_t q = cudaEventQuery(c->ev_out);
             if (q == cudaSuccess) break;
             if (q != cudaErrorNotReady) { c->err = std::string("persistent engine: ") + cudaGetErrorString(q); return NOLSM_ECUDA; }
-            const double el = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+            const double el = std::chrono::duration<double>(std::chrono::steady_clock::now() - c->t_launch).count();
             if (!aborted && el > c->timeout_s) {
                 static const int one = 1;
                 cudaMemcpyAsync(c->d_abort, &one, 4, cudaMemcpyHostToDevice, c->s_x);
@@ -93,12 +115,14 @@ int wait_result(nolsm_ctx* c) {
             if (el > c->timeout_s + 60.0) { c->err = "persistent engine did not stop after abort"; return NOLSM_ECUDA; }
             std::this_thread::sleep_for(std::chrono::microseconds(el < 0.01 ? 20 : 200));
         }
-        int word = 0;
-        CU_TRY(c, cudaMemcpy(&word, c->d_abort, 4, cudaMemcpyDeviceToHost));
-        if (word == 2) { c->have_result = false; c->err = "persistent engine: a wait inside the kernel stalled (device watchdog); the results of this call are invalid"; return NOLSM_ECUDA; }
-        if (aborted || word) { c->have_result = false; c->err = "persistent engine exceeded its time limit and was aborted"; return NOLSM_ECUDA; }
+        if (int r = check_abort_words(c)) { c->pend_dst = nullptr; return r; }
     }
     CU_TRY(c, cudaStreamSynchronize(c->last_stream));
+    if (c->pend_dst) {
+        void* dst = c->pend_dst;
+        c->pend_dst = nullptr;
+        CU_TRY(c, cudaMemcpy(dst, c->d_D_stage, c->pend_bytes, cudaMemcpyDeviceToHost));
+    }
     return NOLSM_OK;
 }
 
@@ -111,6 +135,7 @@ int run(nolsm_ctx* c, const double* mu, int n_mu, bool count_only, int64_t a0, i
     cudaStream_t us = (cudaStream_t)cuda_stream;
     cudaStream_t s = c->s_main;
     cudaSetDevice(c->dev);
+    if (c->pend_dst) { if (int r = wait_result(c)) return r; }      // the staged D of the previous call goes home first
     const size_t ds = d_dtype == NOLSM_DTYPE_F64 ? 8 : 4;
     c->last_ds = ds;
     const int64_t v0 = c->blk_off[c->row_ptr[a0]], v1 = c->blk_off[c->row_ptr[a1]];
@@ -137,7 +162,15 @@ int run(nolsm_ctx* c, const double* mu, int n_mu, bool count_only, int64_t a0, i
     CU_TRY(c, cudaMemsetAsync(c->d_e_atom + a0, 0, 8 * (a1 - a0), s));
     CU_TRY(c, cudaMemsetAsync(c->d_q_atom + a0, 0, 8 * (a1 - a0), s));
     if (int r = engine_run(c, mu, n_mu, count_only, a0, a1, D_dev, d_dtype, s)) return r;
-    if (host_out) CU_TRY(c, cudaMemcpyAsync((char*)D_vals + (size_t)v0 * ds, c->d_D_stage, (size_t)(v1 - v0) * ds, cudaMemcpyDeviceToHost, s));
+    if (host_out) {
+        // pinned memory: the copy is enqueued behind the kernel and the call returns. Pageable memory: the copy would block
+        // this thread until the kernel has ended, with nobody watching the time limit; wait_result does it instead.
+        cudaPointerAttributes at{};
+        const bool pinned = cudaPointerGetAttributes(&at, D_vals) == cudaSuccess && at.type == cudaMemoryTypeHost;
+        cudaGetLastError();
+        if (pinned) CU_TRY(c, cudaMemcpyAsync((char*)D_vals + (size_t)v0 * ds, c->d_D_stage, (size_t)(v1 - v0) * ds, cudaMemcpyDeviceToHost, s));
+        else { c->pend_dst = (char*)D_vals + (size_t)v0 * ds; c->pend_bytes = (size_t)(v1 - v0) * ds; }
+    }
     CU_TRY(c, cudaEventRecord(c->ev_out, s));
     CU_TRY(c, cudaStreamWaitEvent(us, c->ev_out, 0));
     c->last_stream = us; c->last_a0 = a0; c->last_a1 = a1; c->have_result = true;
@@ -155,7 +188,7 @@ int nolsm_abi_version(void) { return NOLSM_ABI_VERSION; }
 size_t nolsm_sizeof_options(void) { return sizeof(nolsm_options); }
 size_t nolsm_sizeof_stats(void) { return sizeof(nolsm_stats); }
 
-int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
+int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) try {
     if (!out) return NOLSM_EINVAL;
     *out = nullptr;
     int ndev = 0;
@@ -200,12 +233,12 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) {
     for (int i = 0; i < NOLSM_ROUND_DEPTH; ++i) ok = ok && cudaEventCreateWithFlags(&c->ev_round[i], cudaEventDisableTiming) == cudaSuccess;
     ok = ok && cudaEventCreate(&c->ev_k0) == cudaSuccess && cudaEventCreate(&c->ev_k1) == cudaSuccess;
     ok = ok && engine_create(c) == NOLSM_OK;
-    if (!ok) { cudaGetLastError(); engine_destroy(c); delete c; return NOLSM_ECUDA; }
+    if (!ok) { cudaGetLastError(); nolsm_destroy(c); return NOLSM_ECUDA; }   // releases the streams and events that exist
     *out = c;
     return NOLSM_OK;
-}
+} catch (...) { return NOLSM_ENOMEM; }
 
-int nolsm_destroy(nolsm_ctx* c) {
+int nolsm_destroy(nolsm_ctx* c) try {
     if (!c) return NOLSM_EINVAL;
     cudaSetDevice(c->dev);
     free_assembled(c, true);
@@ -218,11 +251,11 @@ int nolsm_destroy(nolsm_ctx* c) {
     engine_destroy(c);
     delete c;
     return NOLSM_OK;
-}
+} catch (...) { return on_exception(c, "nolsm_destroy"); }
 
 const char* nolsm_last_error(const nolsm_ctx* c) { return c ? c->err.c_str() : "null context"; }
 
-int nolsm_set_perf_table(nolsm_ctx* c, const int32_t* n, const double* tflops, int count) {
+int nolsm_set_perf_table(nolsm_ctx* c, const int32_t* n, const double* tflops, int count) try {
     if (!c) return NOLSM_EINVAL;
     if (count == 0) { c->pn_n.clear(); c->pn_rate.clear(); return NOLSM_OK; }
     if (!n || !tflops || count < 0) return fail(c, NOLSM_EINVAL, "null table");
@@ -235,10 +268,10 @@ int nolsm_set_perf_table(nolsm_ctx* c, const int32_t* n, const double* tflops, i
     }
     c->pn_n = tn; c->pn_rate = tr;
     return NOLSM_OK;
-}
+} catch (...) { return on_exception(c, "nolsm_set_perf_table"); }
 
 int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, void* D_vals, int d_dtype,
-                               double* e_partial_host, void* cuda_stream) {
+                               double* e_partial_host, void* cuda_stream) try {
     if (!c) return NOLSM_EINVAL;
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "nolsm_assemble has not been called");
     if (!D_vals || a0 < 0 || a1 > c->n_atoms || a0 >= a1) return fail(c, NOLSM_EINVAL, "bad range or null D_vals");
@@ -246,14 +279,14 @@ int nolsm_density_matrix_range(nolsm_ctx* c, double mu, int64_t a0, int64_t a1, 
     if (int r = run(c, &mu, 1, false, a0, a1, D_vals, d_dtype, cuda_stream)) return r;
     if (e_partial_host) return nolsm_energy(c, e_partial_host);
     return NOLSM_OK;
-}
+} catch (...) { return on_exception(c, "nolsm_density_matrix_range"); }
 
-int nolsm_density_matrix(nolsm_ctx* c, double mu, void* D_vals, int d_dtype, void* cuda_stream) {
+int nolsm_density_matrix(nolsm_ctx* c, double mu, void* D_vals, int d_dtype, void* cuda_stream) try {
     if (!c) return NOLSM_EINVAL;
     return nolsm_density_matrix_range(c, mu, 0, c->n_atoms, D_vals, d_dtype, nullptr, cuda_stream);
-}
+} catch (...) { return on_exception(c, "nolsm_density_matrix"); }
 
-int nolsm_energy(nolsm_ctx* c, double* e_elec) {
+int nolsm_energy(nolsm_ctx* c, double* e_elec) try {
     if (!c || !e_elec) return NOLSM_EINVAL;
     if (!c->have_result || c->last_count_only) return fail(c, NOLSM_ESTATE, "no density matrix has been computed");
     cudaSetDevice(c->dev);
@@ -269,9 +302,9 @@ int nolsm_energy(nolsm_ctx* c, double* e_elec) {
     if (bits & NOLSM_MAT_NOTSPD) return fail(c, NOLSM_ENOTSPD, "an S_sub inverse iteration failed (see nolsm_get_atom_stats)");
     if (bits & NOLSM_MAT_NOCONV) return fail(c, NOLSM_ENOCONV, "a sign iteration hit max_sign_iters (see nolsm_get_atom_stats)");
     return NOLSM_OK;
-}
+} catch (...) { return on_exception(c, "nolsm_energy"); }
 
-int nolsm_electron_count(nolsm_ctx* c, double* n_elec, double* q_atom_out) {
+int nolsm_electron_count(nolsm_ctx* c, double* n_elec, double* q_atom_out) try {
     if (!c || !n_elec) return NOLSM_EINVAL;
     if (!c->have_result || c->last_count_only) return fail(c, NOLSM_ESTATE, "no density matrix has been computed");
     cudaSetDevice(c->dev);
@@ -284,9 +317,9 @@ int nolsm_electron_count(nolsm_ctx* c, double* n_elec, double* q_atom_out) {
     *n_elec = sum;
     if (q_atom_out) memcpy(q_atom_out, q.data(), 8 * n);
     return NOLSM_OK;
-}
+} catch (...) { return on_exception(c, "nolsm_electron_count"); }
 
-int nolsm_electron_counts(nolsm_ctx* c, const double* mu, int n_mu, double* n_elec_out, double* e_out, void* cuda_stream) {
+int nolsm_electron_counts(nolsm_ctx* c, const double* mu, int n_mu, double* n_elec_out, double* e_out, void* cuda_stream) try {
     if (!c || !mu || !n_elec_out) return NOLSM_EINVAL;
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "nolsm_assemble has not been called");
     if (n_mu < 1 || n_mu > NOLSM_MAX_MU) return fail(c, NOLSM_EINVAL, "n_mu must be 1..8");
@@ -304,10 +337,10 @@ int nolsm_electron_counts(nolsm_ctx* c, const double* mu, int n_mu, double* n_el
     if (bits & NOLSM_MAT_NOTSPD) return fail(c, NOLSM_ENOTSPD, "an S_sub inverse iteration failed (see nolsm_get_atom_stats)");
     if (bits & NOLSM_MAT_NOCONV) return fail(c, NOLSM_ENOCONV, "a sign iteration hit max_sign_iters (see nolsm_get_atom_stats)");
     return NOLSM_OK;
-}
+} catch (...) { return on_exception(c, "nolsm_electron_counts"); }
 
 int nolsm_find_mu(nolsm_ctx* c, double n_target, double mu_lo, double mu_hi, double tol_n, double tol_mu, int max_evals,
-                  void* D_vals, int d_dtype, void* cuda_stream, double* mu_out, double* n_out, int* evals_out) {
+                  void* D_vals, int d_dtype, void* cuda_stream, double* mu_out, double* n_out, int* evals_out) try {
     if (!c || !D_vals || !mu_out) return NOLSM_EINVAL;
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "nolsm_assemble has not been called");
     if (!(mu_lo < mu_hi) || !(tol_n >= 0) || !(tol_mu >= 0)) return fail(c, NOLSM_EINVAL, "need mu_lo < mu_hi and tolerances >= 0");
@@ -384,9 +417,9 @@ int nolsm_find_mu(nolsm_ctx* c, double n_target, double mu_lo, double mu_hi, dou
     if (evals_out) *evals_out = evals;
     if (rc_soft) return fail(c, rc_soft, "a sign iteration hit max_sign_iters during the mu search (see nolsm_get_atom_stats)");
     return NOLSM_OK;
-}
+} catch (...) { return on_exception(c, "nolsm_find_mu"); }
 
-int nolsm_get_index_set(nolsm_ctx* c, int64_t atom, int32_t* atoms_out, int32_t* n_inout, int32_t* dim_out) {
+int nolsm_get_index_set(nolsm_ctx* c, int64_t atom, int32_t* atoms_out, int32_t* n_inout, int32_t* dim_out) try {
     if (!c || !n_inout) return NOLSM_EINVAL;
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "not assembled");
     if (atom < 0 || atom >= c->n_atoms) return fail(c, NOLSM_EINVAL, "atom out of range");
@@ -398,10 +431,10 @@ int nolsm_get_index_set(nolsm_ctx* c, int64_t atom, int32_t* atoms_out, int32_t*
     }
     *n_inout = (int32_t)cnt;
     return NOLSM_OK;
-}
+} catch (...) { return on_exception(c, "nolsm_get_index_set"); }
 
 int nolsm_get_group(nolsm_ctx* c, int64_t atom, int32_t* members_out, int32_t* n_members_inout, int32_t* set_out,
-                    int32_t* n_set_inout, int32_t* dim_out) {
+                    int32_t* n_set_inout, int32_t* dim_out) try {
     if (!c || !n_members_inout || !n_set_inout) return NOLSM_EINVAL;
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "not assembled");
     if (atom < 0 || atom >= c->n_atoms) return fail(c, NOLSM_EINVAL, "atom out of range");
@@ -420,9 +453,9 @@ int nolsm_get_group(nolsm_ctx* c, int64_t atom, int32_t* members_out, int32_t* n
     *n_members_inout = (int32_t)nm;
     *n_set_inout = (int32_t)ns;
     return rc;
-}
+} catch (...) { return on_exception(c, "nolsm_get_group"); }
 
-int nolsm_gather_submatrix(nolsm_ctx* c, int64_t atom, int which, int out_fp16, void* out_host) {
+int nolsm_gather_submatrix(nolsm_ctx* c, int64_t atom, int which, int out_fp16, void* out_host) try {
     if (!c || !out_host || (which != 0 && which != 1)) return NOLSM_EINVAL;
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "not assembled");
     if (atom < 0 || atom >= c->n_atoms) return fail(c, NOLSM_EINVAL, "atom out of range");
@@ -431,29 +464,29 @@ int nolsm_gather_submatrix(nolsm_ctx* c, int64_t atom, int which, int out_fp16, 
     // with combine the dense submatrix an atom is evaluated on is its group's (tight, dimension of nolsm_get_group)
     if (c->combined) return engine_gather(c, c->unit_of[atom], true, which, out_fp16, out_host);
     return engine_gather(c, atom, false, which, out_fp16, out_host);
-}
+} catch (...) { return on_exception(c, "nolsm_gather_submatrix"); }
 
 // The gather without device allocations (static scratch array in engine.cu). It does not wait for the last
 // density_matrix call: it reads only the pattern and the H0 / S values and writes only the scratch array and `out`.
-int nolsm_gather_submatrix_noalloc(nolsm_ctx* c, int64_t atom, int which, void* out, void* cuda_stream) {
+int nolsm_gather_submatrix_noalloc(nolsm_ctx* c, int64_t atom, int which, void* out, void* cuda_stream) try {
     if (!c || !out || (which != 0 && which != 1)) return NOLSM_EINVAL;
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "not assembled");
     if (atom < 0 || atom >= c->n_atoms) return fail(c, NOLSM_EINVAL, "atom out of range");
     cudaSetDevice(c->dev);
     return engine_gather_noalloc(c, c->combined ? c->unit_of[atom] : atom, which, out, (cudaStream_t)cuda_stream);
-}
+} catch (...) { return on_exception(c, "nolsm_gather_submatrix_noalloc"); }
 
 int nolsm_get_atom_stats(nolsm_ctx* c, int64_t a0, int64_t count, int32_t* dims, int32_t* inv_iters, int32_t* sign_iters,
-                         int32_t* status, int32_t* gemms, float* residual, double* e_atom) {
+                         int32_t* status, int32_t* gemms, float* residual, double* e_atom) try {
     if (!c) return NOLSM_EINVAL;
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "not assembled");
     if (a0 < 0 || count < 0 || a0 + count > c->n_atoms) return fail(c, NOLSM_EINVAL, "range");
     cudaSetDevice(c->dev);
     if (c->have_result) { if (int r = wait_result(c)) return r; }
     return engine_atom_stats(c, a0, count, dims, inv_iters, sign_iters, status, gemms, residual, e_atom);
-}
+} catch (...) { return on_exception(c, "nolsm_get_atom_stats"); }
 
-int nolsm_get_stats(nolsm_ctx* c, nolsm_stats* out) {
+int nolsm_get_stats(nolsm_ctx* c, nolsm_stats* out) try {
     if (!c || !out) return NOLSM_EINVAL;
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "not assembled");
     memset(out, 0, sizeof(*out));
@@ -474,30 +507,30 @@ int nolsm_get_stats(nolsm_ctx* c, nolsm_stats* out) {
         return engine_stats(c, out);
     }
     return NOLSM_OK;
-}
+} catch (...) { return on_exception(c, "nolsm_get_stats"); }
 
-int nolsm_get_profile(nolsm_ctx* c, double* out, int n) {
+int nolsm_get_profile(nolsm_ctx* c, double* out, int n) try {
     if (!c || !out || n < NOLSM_PROFILE_LEN) return NOLSM_EINVAL;
     if (!c->have_result) return fail(c, NOLSM_ESTATE, "no density matrix has been computed");
     cudaSetDevice(c->dev);
     if (int r = wait_result(c)) return r;
     return engine_profile(c, out);
-}
+} catch (...) { return on_exception(c, "nolsm_get_profile"); }
 
-int nolsm_get_engine_counters(nolsm_ctx* c, double* out, int n) {
+int nolsm_get_engine_counters(nolsm_ctx* c, double* out, int n) try {
     if (!c || !out || n < NOLSM_COUNTERS_LEN) return NOLSM_EINVAL;
     if (!c->have_result) return fail(c, NOLSM_ESTATE, "no density matrix has been computed");
     cudaSetDevice(c->dev);
     if (int r = wait_result(c)) return r;
     return engine_counters(c, out);
-}
+} catch (...) { return on_exception(c, "nolsm_get_engine_counters"); }
 
-int nolsm_side_task_bandwidth(nolsm_ctx* c, int which, int reps, double* ms_out, double* bytes_out) {
+int nolsm_side_task_bandwidth(nolsm_ctx* c, int which, int reps, double* ms_out, double* bytes_out) try {
     if (!c || !ms_out || !bytes_out || (which != 0 && which != 1) || reps < 1) return NOLSM_EINVAL;
     if (!c->assembled) return fail(c, NOLSM_ESTATE, "not assembled");
     cudaSetDevice(c->dev);
     if (c->have_result) { if (int r = wait_result(c)) return r; }
     return engine_side_bandwidth(c, which, reps, ms_out, bytes_out);
-}
+} catch (...) { return on_exception(c, "nolsm_side_task_bandwidth"); }
 
 }  // extern "C"

@@ -10,7 +10,7 @@ using namespace nolsm_host;
 extern "C" {
 
 int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const int64_t* row_ptr,
-                   const int32_t* col_idx, const void* H0_vals, const void* S_vals, int val_dtype, void* cuda_stream) {
+                   const int32_t* col_idx, const void* H0_vals, const void* S_vals, int val_dtype, void* cuda_stream) try {
     if (!c) return NOLSM_EINVAL;
     if (n_atoms <= 0 || !atom_nb || !row_ptr || !col_idx || !H0_vals || !S_vals)
         return fail(c, NOLSM_EINVAL, "null pointer or n_atoms <= 0");
@@ -192,6 +192,6 @@ int nolsm_assemble(nolsm_ctx* c, int64_t n_atoms, const int32_t* atom_nb, const 
     lap("workspace, maps, engine");
     c->assembled = true;
     return NOLSM_OK;
-}
+} catch (...) { return on_exception(c, "nolsm_assemble"); }
 
 }  // extern "C"

@@ -1,6 +1,6 @@
 // Host-side context of the NOLSM library (include/nolsm.h) and the helpers its translation units share:
-//   abi.cu       context life cycle, results, diagnostics
-//   assemble.cu  nolsm_assemble: validation, index sets N(i), workspace plan, tensor maps         (a0)
+//   abi.cpp      context life cycle, results, diagnostics
+//   assemble.cpp nolsm_assemble: validation, index sets N(i), workspace plan, tensor maps         (a0)
 //   grouping.cpp submatrix combination: Eq. 9 / Eq. 10 costs, greedy groups
 //   engine.cu    the launches: persistent kernel (a1-a7), round engine (FP32 validation), stand-alone side tasks
 #pragma once
@@ -10,6 +10,9 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <exception>
+#include <new>
+#include <system_error>
 #include <string>
 #include <thread>
 #include <vector>
@@ -26,6 +29,7 @@ struct PEngine;
 
 constexpr int NOLSM_ROUND_DEPTH = 4;    // rounds kept in flight ahead of the device (round engine)
 constexpr int NOLSM_MAX_MU = 8;         // == P_MAX_MU (persist.cuh)
+constexpr int NOLSM_ABORT_HIST = 16;    // abort words of earlier launches kept until a call waits for the results
 
 struct nolsm_ctx {
     int dev = 0;
@@ -82,7 +86,14 @@ struct nolsm_ctx {
 
     // persistent engine (persist.cuh): one kernel launch per density_matrix call
     bool persist = false;
-    int* d_abort = nullptr;
+    int* d_abort = nullptr;             // [1 + NOLSM_ABORT_HIST]: the running kernel's abort word, then the final words of the
+                                        // launches nobody has waited for yet (launch k at 1 + k % NOLSM_ABORT_HIST)
+    int64_t launch_seq = 0, checked_seq = 0;   // persistent launches since assemble; launches whose abort word has been read
+    std::chrono::steady_clock::time_point t_launch{};   // when the last persistent kernel was enqueued (host time limit)
+    unsigned long long h_stall_ns = 0;  // device watchdog limit of the hot waits, from timeout_s
+    // D of a call with pageable host output stays in d_D_stage until a call waits for the result (wait_result copies it)
+    void* pend_dst = nullptr;
+    size_t pend_bytes = 0;
     int p_grid = 0;                     // CTAs of the persistent kernel
     cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr;
     int h_a0 = 0;
@@ -122,33 +133,65 @@ struct nolsm_ctx {
 
 namespace nolsm_host {
 
+// f(begin, end) over chunks of [0, n) on up to 16 threads. An exception inside a worker (std::bad_alloc of a per-thread
+// vector) is carried to the caller and rethrown there after every worker has been joined; if a thread cannot be
+// started, the caller's thread does that chunk itself.
 template <typename F>
 void parallel_for(int64_t n, F f) {
     unsigned nt = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
     if (n < 1 << 11) nt = 1;
     if (nt == 1) { f(0, n); return; }
     std::vector<std::thread> th;
+    std::vector<std::exception_ptr> err(nt);
+    th.reserve(nt);
     const int64_t chunk = (n + nt - 1) / nt;
     for (unsigned t = 0; t < nt; ++t) {
         const int64_t b = t * chunk, e = std::min<int64_t>(n, b + chunk);
-        if (b < e) th.emplace_back([=] { f(b, e); });
+        if (b >= e) continue;
+        auto work = [&f, &err, t, b, e] { try { f(b, e); } catch (...) { err[t] = std::current_exception(); } };
+        try { th.emplace_back(work); } catch (const std::system_error&) { work(); }
     }
     for (auto& x : th) x.join();
+    for (auto& ep : err) if (ep) std::rethrow_exception(ep);
 }
 
+// Temporary device buffers and events of the diagnostics: released on every return path.
+struct DevBuf {
+    void* p = nullptr;
+    ~DevBuf() { if (p) cudaFree(p); }
+    template <typename T> T* as() const { return static_cast<T*>(p); }
+};
+struct EventPair {
+    cudaEvent_t a = nullptr, b = nullptr;
+    ~EventPair() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
+};
+
 inline int fail(nolsm_ctx* c, int code, const std::string& msg) { c->err = msg; return code; }
+// Handler of the function-try-block around every extern "C" entry point: no exception crosses the C boundary
+// (std::bad_alloc from the host-side vectors, std::system_error from the worker threads of parallel_for).
+inline int on_exception(nolsm_ctx* c, const char* where) {
+    int code = NOLSM_ENOMEM;
+    std::string what = "out of host memory";
+    try { throw; }
+    catch (const std::bad_alloc&) {}
+    catch (const std::exception& e) { code = NOLSM_ECUDA; what = e.what(); }
+    catch (...) { code = NOLSM_ECUDA; what = "unknown exception"; }
+    if (c) { try { c->err = std::string(where) + ": " + what; } catch (...) {} }
+    return code;
+}
 inline bool verbose(int level = 1) {
     static const int v = [] { const char* s = getenv("NOLSM_VERBOSE"); return s && *s ? atoi(s) : 0; }();
     return v >= level;
 }
 
-// abi.cu
+// abi.cpp
 bool is_device_ptr(const void* p);
 int dmalloc(nolsm_ctx* c, void** p, size_t bytes);
 void free_assembled(nolsm_ctx* c, bool release = false);
 int to_device(nolsm_ctx* c, const void* src, size_t bytes, const void** out, cudaStream_t s);
 int to_host(nolsm_ctx* c, const void* src, size_t bytes, void* dst, cudaStream_t s);
 int wait_result(nolsm_ctx* c);
+int check_abort_words(nolsm_ctx* c);    // reads the abort words of every launch since the last check
 inline size_t elem_size(const nolsm_ctx* c) { return c->opt.precision == NOLSM_PREC_FP32 ? 4 : 2; }
 inline bool use_umma(const nolsm_ctx* c) { return c->opt.precision != NOLSM_PREC_FP32 && c->opt.gemm_backend != NOLSM_GEMM_SIMT; }
 // The persistent engine serves the mixed-precision tcgen05 path; the round engine (plain FFMA GEMMs) serves the FP32

@@ -225,7 +225,19 @@ int run_persistent(nolsm_ctx* c, const double* mu, int n_mu, bool count_only, in
     CU_TRY(c, cudaMemcpyAsync(pe.ctr, c->h_ctr0.data(), 8 * PC_LEN, cudaMemcpyHostToDevice, s));
     CU_TRY(c, cudaMemcpyAsync(pe.next_atom, &c->h_a0, 4, cudaMemcpyHostToDevice, s));
     CU_TRY(c, cudaMemsetAsync(pe.finished, 0, 4, s));
+    // the abort word of the previous launch is kept (stream order: after that kernel) before this launch clears it; when
+    // the history is full the host waits and reads it first
+    if (c->launch_seq - c->checked_seq >= NOLSM_ABORT_HIST) {
+        CU_TRY(c, cudaStreamSynchronize(s));
+        if (int r = check_abort_words(c)) return r;
+    }
+    if (c->launch_seq > c->checked_seq)
+        CU_TRY(c, cudaMemcpyAsync(c->d_abort + 1 + (c->launch_seq - 1) % NOLSM_ABORT_HIST, c->d_abort, 4, cudaMemcpyDeviceToDevice, s));
     CU_TRY(c, cudaMemsetAsync(c->d_abort, 0, 4, s));
+    // device watchdog from options.timeout_s: a hot wait (k-loop stages, accumulators) may last timeout_s / 10, an idle
+    // wait (tile records, ring entries: ten rounds of that) timeout_s
+    c->h_stall_ns = (unsigned long long)(std::max(2.0, c->timeout_s / 10.0) * 1e9);
+    CU_TRY(c, cudaMemcpyToSymbolAsync(g_stall_ns, &c->h_stall_ns, 8, 0, cudaMemcpyHostToDevice, s));
     CU_TRY(c, cudaMemsetAsync(pe.heavy, 0, 8, s));
     CU_TRY(c, cudaMemsetAsync(pe.parked, 0, 4 * pe.S, s));
     CU_TRY(c, cudaMemsetAsync(c->d_mu_acc, 0, 16 * NOLSM_MAX_MU, s));
@@ -233,6 +245,8 @@ int run_persistent(nolsm_ctx* c, const double* mu, int n_mu, bool count_only, in
     nolsm_persist_kernel<<<c->p_grid, P_THREADS, P_SMEM_BYTES, s>>>(pe);
     CU_TRY(c, cudaGetLastError());
     CU_TRY(c, cudaEventRecord(c->ev_k1, s));
+    c->t_launch = std::chrono::steady_clock::now();
+    c->launch_seq += 1;
     c->launches = 1;
     c->rounds = 0;
     return NOLSM_OK;
@@ -243,8 +257,9 @@ int run_persistent(nolsm_ctx* c, const double* mu, int n_mu, bool count_only, in
 namespace nolsm_host {
 
 int engine_create(nolsm_ctx* c) {
-    c->eng = new Engine{};
-    c->peng = new PEngine{};
+    c->eng = new (std::nothrow) Engine{};
+    c->peng = new (std::nothrow) PEngine{};
+    if (!c->eng || !c->peng) return fail(c, NOLSM_ENOMEM, "out of host memory");
     static_assert(P_MAX_MU == NOLSM_MAX_MU, "trial-mu capacity");
     if (use_umma(c)) CU_TRY(c, cudaFuncSetAttribute(nolsm_persist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES));
     return NOLSM_OK;
@@ -402,7 +417,9 @@ int engine_plan(nolsm_ctx* c, cudaStream_t s) {
         if ((r = dmalloc(c, (void**)&pe.gclaim, 8 * S))) return r;
         if ((r = dmalloc(c, (void**)&pe.sclaim, 4 * S))) return r;
         if ((r = dmalloc(c, (void**)&pe.ctr, 8 * PC_LEN))) return r;
-        if ((r = dmalloc(c, (void**)&c->d_abort, 16))) return r;
+        if ((r = dmalloc(c, (void**)&c->d_abort, 4 * (1 + NOLSM_ABORT_HIST)))) return r;
+        CU_TRY(c, cudaMemsetAsync(c->d_abort, 0, 4 * (1 + NOLSM_ABORT_HIST), s));
+        c->launch_seq = c->checked_seq = 0;
         if ((r = dmalloc(c, (void**)&pe.heavy, 16))) return r;
         if ((r = dmalloc(c, (void**)&pe.pcols, (size_t)S * e.cap * PCW * sizeof(float)))) return r;
         if ((r = dmalloc(c, (void**)&pe.parked, 4 * S))) return r;
@@ -655,9 +672,10 @@ int engine_gather(nolsm_ctx* c, int64_t id, bool is_unit, int which, int out_fp1
     if (c->persist && out_fp16) {
         // the gather task of the persistent engine, launched stand-alone into slot 0
         const int64_t unit = is_unit ? id : (c->combined ? -1 : id);
-        if (unit < 0) return fail(c, NOLSM_ESTATE, "with combine the dense submatrices are per group: ask for a unit (nolsm_gather_unit)");
-        int* d_unit;
-        CU_TRY(c, cudaMalloc((void**)&d_unit, 4));
+        if (unit < 0) return fail(c, NOLSM_ESTATE, "with combine the dense submatrices are per group: nolsm_gather_submatrix maps the atom to its unit");
+        DevBuf unit_buf;
+        CU_TRY(c, cudaMalloc(&unit_buf.p, 4));
+        int* d_unit = unit_buf.as<int>();
         const int u32 = (int)unit;
         CU_TRY(c, cudaMemcpy(d_unit, &u32, 4, cudaMemcpyHostToDevice));
         const PEngine& pe = *c->peng;
@@ -673,7 +691,6 @@ int engine_gather(nolsm_ctx* c, int64_t id, bool is_unit, int which, int out_fp1
         if (ce == cudaSuccess)
             ce = cudaMemcpy2D(out_host, (size_t)n * 2, (const char*)c->ws + (size_t)which * pe.bufsz * 2, (size_t)pe.ld * 2,
                               (size_t)n * 2, n, cudaMemcpyDeviceToHost);
-        cudaFree(d_unit);
         if (ce != cudaSuccess) { c->err = cudaGetErrorString(ce); return NOLSM_ECUDA; }
         return NOLSM_OK;
     }
@@ -686,8 +703,9 @@ int engine_gather(nolsm_ctx* c, int64_t id, bool is_unit, int which, int out_fp1
     Slot sl{};
     sl.atom = (int)atom; sl.n = c->dim[atom]; sl.n16 = (sl.n + 15) & ~15; sl.pos = c->pos[atom]; sl.nbi = c->atom_nb[atom];
     sl.phase = sl.snap = PH_NEW;
-    Slot* d_sl;
-    CU_TRY(c, cudaMalloc((void**)&d_sl, sizeof(Slot)));
+    DevBuf slot_buf;
+    CU_TRY(c, cudaMalloc(&slot_buf.p, sizeof(Slot)));
+    Slot* d_sl = slot_buf.as<Slot>();
     CU_TRY(c, cudaMemcpy(d_sl, &sl, sizeof(Slot), cudaMemcpyHostToDevice));
     e.slots = d_sl;
     int r;
@@ -700,7 +718,6 @@ int engine_gather(nolsm_ctx* c, int64_t id, bool is_unit, int which, int out_fp1
                               (size_t)e.ld * es, (size_t)sl.n * es, sl.n, cudaMemcpyDeviceToHost);
         if (ce != cudaSuccess) { c->err = cudaGetErrorString(ce); r = NOLSM_ECUDA; }
     }
-    cudaFree(d_sl);
     return r;
 }
 
@@ -713,17 +730,19 @@ int engine_side_bandwidth(nolsm_ctx* c, int which, int reps, double* ms_out, dou
     if (which == 1 && c->combined) return fail(c, NOLSM_ESTATE, "scatter bandwidth: assemble without combine");
     const PEngine& pe = *c->peng;
     cudaStream_t s = c->s_main;
-    cudaEvent_t e0, e1;
-    CU_TRY(c, cudaEventCreate(&e0));
-    CU_TRY(c, cudaEventCreate(&e1));
+    EventPair evp;
+    CU_TRY(c, cudaEventCreate(&evp.a));
+    CU_TRY(c, cudaEventCreate(&evp.b));
+    const cudaEvent_t e0 = evp.a, e1 = evp.b;
     const int64_t count = which == 0 ? c->n_units : c->n_atoms;
     std::vector<int> ids(count);
     for (int64_t i = 0; i < count; ++i) ids[i] = (int)i;
-    int* d_ids;
-    CU_TRY(c, cudaMalloc((void**)&d_ids, 4 * count));
+    DevBuf ids_buf, bytes_buf;
+    CU_TRY(c, cudaMalloc(&ids_buf.p, 4 * count));
+    int* d_ids = ids_buf.as<int>();
     CU_TRY(c, cudaMemcpy(d_ids, ids.data(), 4 * count, cudaMemcpyHostToDevice));
-    unsigned long long* d_bytes;
-    CU_TRY(c, cudaMalloc((void**)&d_bytes, 8));
+    CU_TRY(c, cudaMalloc(&bytes_buf.p, 8));
+    unsigned long long* d_bytes = bytes_buf.as<unsigned long long>();
     CU_TRY(c, cudaMemset(d_bytes, 0, 8));
     double bytes = 0;
     const size_t vs = c->val_dtype == NOLSM_DTYPE_F64 ? 8 : 4;
@@ -776,8 +795,6 @@ int engine_side_bandwidth(nolsm_ctx* c, int which, int reps, double* ms_out, dou
     CU_TRY(c, cudaEventSynchronize(e1));
     float ms = 0;
     CU_TRY(c, cudaEventElapsedTime(&ms, e0, e1));
-    cudaFree(d_ids); cudaFree(d_bytes);
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
     *ms_out = ms / reps;
     *bytes_out = bytes;
     c->have_result = false;                           // the energies of the last call were overwritten

@@ -8,7 +8,9 @@ namespace nolsm {
 constexpr int B_BOX_BYTES = BK * 64 * 2;            // one TMA box: 64 (contiguous) x 64 FP16 = 8 KB
 // Watchdog of every mbarrier wait: a wait that lasts this long is a protocol stall. The waiter raises the engine's
 // abort word (value 2) and leaves its role; the host reports NOLSM_ECUDA (no __trap: the CUDA context stays usable).
-constexpr unsigned long long STALL_NS = 30ull * 1000000000ull;
+// The limit follows options.timeout_s (engine.cu sets it before every launch: timeout_s / 10, at least 2 s; the idle
+// waits allow ten rounds of it = timeout_s); 30 s until then.
+__device__ unsigned long long g_stall_ns = 30ull * 1000000000ull;
 
 namespace ptx {
 
@@ -51,11 +53,11 @@ __device__ __forceinline__ unsigned long long globaltimer_ns() {
     return t;
 }
 // One step of the watchdog (called from the slow path of a wait, every so many polls): returns true when the wait
-// has lasted STALL_NS; the caller then gives up.
+// has lasted g_stall_ns; the caller then gives up.
 __device__ __forceinline__ bool stalled(unsigned long long& t0, volatile int* abort_flag) {
     const unsigned long long t = globaltimer_ns();
     if (!t0) { t0 = t; return false; }
-    if (t - t0 < STALL_NS) return false;
+    if (t - t0 < g_stall_ns) return false;
     atomicExch(const_cast<int*>(abort_flag), 2);
     return true;
 }

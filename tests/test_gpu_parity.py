@@ -750,3 +750,50 @@ def test_diagnostic_drop_of_operand_loads_completes(drop):
         st = ctx.atom_stats()
         stats = ctx.stats()
     assert stats["gemms_executed"] == int(st["gemms"].sum()) and stats["gemms_executed"] > 0
+
+
+def test_time_limit_abort_is_reported_by_the_next_wait_and_the_context_recovers():
+    """options.timeout_s counts from the launch. A kernel that overruns it is stopped by the call that waits, and the abort is
+    not forgotten when a later call on the context went through in the meantime (a series of density_matrix_range calls
+    followed by one wait): the wait reports which call of the series was stopped. The context stays usable."""
+    from paper_2205_12182_b200 import NolsmError
+    s = make_system("cfg2", n_atoms=1200)
+    nb, rp, ci, Hv, Sv = _arrays(s)
+    D = torch.zeros_like(Hv)
+    with _nolsm(timeout_s=0.05) as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        ctx.density_matrix_range(s.mu, 0, 1000, D)             # > 100 ms of work: overruns the 50 ms
+        ctx.density_matrix_range(s.mu, 1000, 1004, D)          # a few ms: runs to its end after the first was stopped
+        with pytest.raises(NolsmError) as ei:
+            ctx.energy()
+        assert ei.value.code == 2 and "time limit" in str(ei.value) and "call 1 of the 2" in str(ei.value), str(ei.value)
+        e = ctx.density_matrix_range(s.mu, 1000, 1004, D, want_energy=True)
+        st = ctx.atom_stats()
+        assert (st["status"][1000:1004] == 0).all() and abs(e - st["e_atom"][1000:1004].sum()) <= 1e-9 * abs(e)
+    cmp = compare_atoms(s, D.cpu().numpy(), st["e_atom"], [1000, 1003])
+    assert cmp["max_abs_dD"] <= TOL_MIXED_D and cmp["rel_dE"] <= TOL_MIXED_E
+
+
+def test_pageable_host_output_arrives_with_the_wait(cfg0):
+    """D_vals in pageable host memory is filled by the call that waits for the results (the watched wait comes first), in
+    pinned host memory by a copy behind the kernel; both equal the device output of the same call within the tolerance."""
+    s = cfg0
+    nb, rp, ci, Hv, Sv = _arrays(s)
+    with _nolsm() as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        Dd = torch.zeros_like(Hv)
+        ctx.density_matrix(s.mu, Dd)
+        e0 = ctx.energy()
+        Dp = np.full(Hv.shape[0], np.nan)
+        ctx.density_matrix(s.mu, Dp)
+        e1 = ctx.energy()
+        Dq = torch.full((Hv.shape[0],), float("nan"), dtype=torch.float64).pin_memory()
+        ctx.density_matrix(s.mu, Dq)
+        e2 = ctx.energy()
+        Dr = np.full(Hv.shape[0], np.nan)
+        ctx.density_matrix(s.mu, Dr)                           # never waited for explicitly: the next call delivers it
+        ctx.density_matrix(s.mu, Dd)
+        ctx.energy()
+    ref = Dd.cpu().numpy()
+    for got, e in ((Dp, e1), (Dq.numpy(), e2), (Dr, e0)):
+        assert np.isfinite(got).all() and np.abs(got - ref).max() <= 2e-3 and abs(e - e0) <= 1e-4 * abs(e0)

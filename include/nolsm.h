@@ -74,7 +74,8 @@ typedef struct {
     float tol_inv;           /* stop when ||I - S Y||_F / sqrt(n) < tol_inv [2e-3 mixed, 1e-5 FP32] */
     float tol_sign;          /* stop when ||X^2 - I||_F / sqrt(n) < tol_sign [2e-3 mixed, 1e-5 FP32] */
     int power_iters_s;       /* power iterations for rho(S_sub) [persistent engine 3 (x 1.3 safety), round engine 6 (x 1.05)] */
-    int power_iters_a;       /* power iterations for rho(A_sub) [persistent engine 6 (x 1.25 safety), round engine 12 (x 1.05)] */
+    int power_iters_a;       /* power iterations for rho(A_sub) [persistent engine 6 (x 1.25 safety; more while the estimate is not
+                                settled, nolsm_get_engine_counters out[38]), round engine 12 (x 1.05)] */
     double eps_filter;       /* block (j,i) enters N(i) iff max(|H0_ji|max, |S_ji|max) > eps_filter [0 = structural] */
     int batch_atoms;         /* workspace slots = submatrices resident at once [auto: persistent engine heavy_slots + max(12, heavy_slots),
                                 at most 96; round engine ~16 waves of GEMM tiles] */
@@ -151,7 +152,7 @@ typedef struct {
  * whenever a field of nolsm_options / nolsm_stats or the meaning of an existing argument changes, and the two sizes are the
  * library's own sizeof. A binding compares all three with its own at load time and refuses a stale libnolsm.so instead
  * of silently misreading every option behind the first changed field. Needs no context and no GPU. */
-#define NOLSM_ABI_VERSION 4
+#define NOLSM_ABI_VERSION 5
 int nolsm_abi_version(void);
 size_t nolsm_sizeof_options(void);
 size_t nolsm_sizeof_stats(void);
@@ -307,9 +308,12 @@ int nolsm_get_profile(nolsm_ctx* ctx, double* out, int n);
  *   out[33..35] where the MMA-issuing warps (one per CTA pair) spent the kernel, ms summed over the pairs: waiting for a
  *   tile record, waiting for a free accumulator (= for the epilogue), inside k-loops (operand waits + issue);
  *   out[36..37] the tile schedulers, ms summed over the pairs: waiting for a free entry of the record ring (= for the
- *   completion of the tile four back), waiting for the producer's claim point.
+ *   completion of the tile four back), waiting for the producer's claim point;
+ *   out[38] power-iteration steps for rho(A) beyond options.power_iters_a, summed over the submatrices: the iteration
+ *   goes on (up to 24 steps) while the estimate still grows by more than 5 % per step or its growth rises from one step to
+ *   the next, the mark of an eigenvalue outside the bulk that the fixed step count would underestimate.
  *   n must be >= NOLSM_COUNTERS_LEN. Synchronises. */
-#define NOLSM_COUNTERS_LEN 38
+#define NOLSM_COUNTERS_LEN 39
 int nolsm_get_engine_counters(nolsm_ctx* ctx, double* out, int n);
 
 /* HBM-bound side tasks timed alone: which = 0 the gather of every submatrix of the assembled system (a1),

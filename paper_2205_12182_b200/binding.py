@@ -14,7 +14,7 @@ ENGINE_AUTO, ENGINE_PERSISTENT, ENGINE_ROUNDS = 0, 1, 2
 ITER_EQ6, ITER_LOWDIN = 0, 1
 STATUS_NAMES = {0: "OK", 1: "EINVAL", 2: "ECUDA", 3: "ENOMEM", 4: "ESTATE", 5: "ENOTSPD", 6: "ENOCONV"}
 
-ABI_VERSION = 4                                     # NOLSM_ABI_VERSION of the include/nolsm.h this file restates
+ABI_VERSION = 5                                     # NOLSM_ABI_VERSION of the include/nolsm.h this file restates
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
@@ -300,14 +300,15 @@ class Nolsm:
 
     def engine_counters(self) -> dict:
         """Counters of the persistent engine for the last density_matrix call (include/nolsm.h)."""
-        out = (C.c_double * 38)()
-        self._check(self._lib.nolsm_get_engine_counters(self._h, out, 38))
+        out = (C.c_double * 39)()
+        self._check(self._lib.nolsm_get_engine_counters(self._h, out, 39))
         v = list(out)
         kinds = ("none", "refill", "gather", "elementwise", "dcols", "wcols", "k6", "k7")
         d = {"persistent": bool(v[0]), "kernel_ms": v[1], "kernel_ms_device_clock": v[2], "tiles": v[3],
              "sched_idle_ms": v[4], "sched_busy_ms": v[5], "overshoots": v[6], "slots": int(v[7]), "pairs": int(v[8])}
         d["mma_wait_record_ms"], d["mma_wait_accumulator_ms"], d["mma_kloop_ms"] = v[33], v[34], v[35]
         d["sched_wait_ring_ms"], d["sched_wait_claim_point_ms"] = v[36], v[37]
+        d["power_steps_extra"] = int(v[38])
         d["side"] = {k: {"busy_ms": v[9 + i], "bytes": v[17 + i], "tasks": v[25 + i]} for i, k in enumerate(kinds)
                      if v[25 + i] > 0}
         return d

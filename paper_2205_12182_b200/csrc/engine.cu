@@ -314,7 +314,7 @@ int engine_plan(nolsm_ctx* c, cudaStream_t s) {
     if (!c->persist && (c->opt.engine == NOLSM_ENGINE_PERSISTENT || c->opt.iteration == NOLSM_ITER_LOWDIN))
         return fail(c, NOLSM_EINVAL, "the persistent engine needs FP16/tcgen05 mode, submatrix dimensions <= 4096 and at most 16 basis functions per atom");
     // heavy-phase cap of the persistent engine: the live iterates of a slot in the GEMM chain are ~3.5 n^2 FP16
-    // (X, T, next X / S, Y, R, next Y); the slots inside the chain together may fill L2 (profiles/r02_gmax_lead_sweep.md)
+    // (X, T, next X / S, Y, R, next Y); the slots inside the chain together may fill L2 (heavy_slots sweep in profiles/r02_persist.md)
     int l2_bytes = 0;
     cudaDeviceGetAttribute(&l2_bytes, cudaDevAttrL2CacheSize, c->dev);
     if (l2_bytes <= 0) l2_bytes = 64 << 20;
@@ -428,9 +428,11 @@ int engine_plan(nolsm_ctx* c, cudaStream_t s) {
         // Block power iteration (16 vectors, Frobenius growth): the estimate creeps up on rho from below (dense spectrum
         // edge: 0.75-0.80 rho after 3 steps, 0.84-0.87 after 6, 0.91-0.94 after 12 on the synthetic workloads), and an
         // overestimate is cheap (a factor 1.3 costs 0.3 scaled sign steps; the Schulz start converges for any
-        // rho_hat > rho / 2) while an underestimate beyond 1.155 / alpha flips signs: few steps, generous safety.
+        // rho_hat > rho / 2) while an underestimate beyond 1.155 / alpha flips signs: few steps, generous safety, and for
+        // rho(A) more steps (up to p_cap) while the estimate is visibly not settled (persist.cuh, p_tile_finished).
         pe.p_s = c->opt.power_iters_s > 0 ? c->opt.power_iters_s : 3;
         pe.p_a = c->opt.power_iters_a > 0 ? c->opt.power_iters_a : 6;
+        pe.p_cap = std::max(pe.p_a, 24);
         pe.safety_s = pe.p_s >= 6 ? 1.05f : 1.3f;
         pe.safety_a = pe.p_a >= 12 ? 1.05f : pe.p_a >= 6 ? 1.25f : 1.45f;
         pe.gather_rowatoms = 4;
@@ -661,6 +663,7 @@ int engine_counters(nolsm_ctx* c, double* out) {
     }
     for (int k = 0; k < 3; ++k) out[33 + k] = ct[PC_MMA_NS + k] * 1e-6;
     out[36] = ct[PC_SCHED_RING_NS] * 1e-6; out[37] = ct[PC_SCHED_CREDIT_NS] * 1e-6;
+    out[38] = (double)ct[PC_POW_EXTRA];
     return NOLSM_OK;
 }
 

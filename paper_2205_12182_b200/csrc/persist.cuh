@@ -61,6 +61,7 @@ enum { PC_TILES = 0, PC_SCHED_IDLE_NS, PC_SCHED_BUSY_NS, PC_OVERSHOOT, PC_T_STAR
        PC_MMA_NS = PC_SIDE_TASKS + 8,    // + 0 tile-record wait, 1 accumulator wait, 2 k-loops (MMA warps of the leader CTAs)
        PC_SCHED_RING_NS = PC_MMA_NS + 3, // tile schedulers: waiting for a free ring entry (= for the completion of the tile four back)
        PC_SCHED_CREDIT_NS,               // ... for the producer's claim point
+       PC_POW_EXTRA,                     // power-iteration steps for rho(A) beyond p_a (estimate not settled, see p_tile_finished)
        PC_LEN };
 
 constexpr int OPF_RES = 1;        // op flags: fused residual wanted
@@ -79,7 +80,7 @@ struct __align__(16) PSlot {      // 176 bytes
     int pow_step; float pow_norm2, pow_alpha; int resume;           // block power iteration state; resume: which token phase comes next
     int noboost, mptr, mend, zcur;                                  // noboost: the scaled steps are over for this matrix; members [mptr, mend) still to be served
     int xsum, pow_buf, mu_idx, sym_count;                           // X ping-pong: next = xsum - xcur; buffer of the running power iteration; trial mu; symmetric GEMMs run
-    int elem_kind, abuf, op_seq, pad1;                              // SK_ELEM variant; buffer that keeps the mu-independent A0 (several trial mu); ops installed so far
+    int elem_kind, abuf, op_seq; float pow_g;                       // pow_g: growth est_k / est_{k-1} of the last power step. SK_ELEM variant; buffer that keeps the mu-independent A0 (several trial mu); ops installed so far
 };
 
 struct PEngine {
@@ -90,6 +91,7 @@ struct PEngine {
     long long bufsz, slotsz;
     float tol_inv, tol_sign, safety_s, safety_a;
     int max_inv, max_sign, p_s, p_a;
+    int p_cap;                    // the power iteration for rho(A) may run on up to this many steps while its estimate is not settled
     int gather_rowatoms, elem_chunks, dcols_chunks;   // row-atoms of N(i) per gather chunk; chunks of the other tasks
     int* next_atom; int a_end, total;                 // feed position, its end, units of this call
     const int* feed;              // feed position -> unit id (nullptr: the position is the unit id)
@@ -226,6 +228,7 @@ __device__ __forceinline__ void p_start_power(const PEngine& e, int slot, int ki
     __stcg(&s->pow_step, 0);
     __stcg(&s->pow_norm2, (float)NVC * (float)__ldcg(&s->n));
     __stcg(&s->pow_alpha, 1.f);
+    __stcg(&s->pow_g, 1.f);
     __stcg(&s->pow_buf, buf);
     p_install_gemm(e, slot, kind);
 }
@@ -376,7 +379,19 @@ __device__ __forceinline__ void p_tile_finished(const PEngine& e, int slot, int 
         if (!(est > 1e-20f) || !(est < 1e20f)) est = 1.f;
         const int step = __ldcg(&s->pow_step) + 1;
         const int P = kind == OP_POW_S ? e.p_s : e.p_a;
-        if (step < P) {
+        // rho(A): the estimate approaches rho from below, and the fixed safety factor covers a dense spectrum edge, where
+        // the growth est_k / est_{k-1} falls from step to step (1.03 -> 1.02 at steps 5 -> 6). An eigenvalue outside the
+        // bulk enters the start block with weight 1 / n only: the estimate sits at the bulk's edge and then starts to
+        // climb, the growth RISES. A scaled sign step on such an underestimate would flip that eigenvalue's sign and
+        // nothing would flag it, so the iteration goes on while the growth is still large or rising (up to p_cap steps).
+        bool unsettled = false;
+        if (kind == OP_POW_A && step >= P && step >= 3 && step < e.p_cap) {
+            const float g = est * alpha, gp = __ldcg(&s->pow_g);        // alpha = 1 / est_{k-1} from the second step on
+            unsettled = g > 1.05f || (g > gp + 0.003f && g > 1.004f);
+            if (unsettled) atomicAdd(&e.ctr[PC_POW_EXTRA], 1ull);
+        }
+        if (step >= 2) __stcg(&s->pow_g, est * alpha);
+        if (step < P || unsettled) {
             __stcg(&s->pow_step, step);
             __stcg(&s->pow_norm2, r_new);
             __stcg(&s->pow_alpha, 1.f / est);                         // keeps ||V_k||_F at its starting magnitude

@@ -797,3 +797,45 @@ def test_pageable_host_output_arrives_with_the_wait(cfg0):
     ref = Dd.cpu().numpy()
     for got, e in ((Dp, e1), (Dq.numpy(), e2), (Dr, e0)):
         assert np.isfinite(got).all() and np.abs(got - ref).max() <= 2e-3 and abs(e - e0) <= 1e-4 * abs(e0)
+
+
+def test_eigenvalue_outside_the_bulk_is_not_flipped_by_the_scaled_steps():
+    """rho(A) comes from a few block power steps on a +-1 start block. One eigenvalue well outside a dense bulk (here 1.0
+    against 1,507 eigenvalues of modulus 0.60-0.68) has weight 1 / n in that start: after the default six steps the estimate
+    is 0.67 rho, the 1.25 safety leaves alpha x = 1.79 > sqrt(3), and the first scaled Newton-Schulz step would carry that
+    eigenvalue to the other sign -- a wrong D with no status bit (one electron too many in the state built here, whose
+    eigenvector is a single basis function: D_00 = 1 instead of 0). The power iteration goes on while its estimate is
+    visibly not settled (growth rising from step to step), so D matches the oracle; the extra steps are counted."""
+    rng = np.random.default_rng(11)
+    n_at, nb = 116, 13
+    n = n_at * nb
+    lam = np.concatenate([[1.0], rng.uniform(0.60, 0.68, n - 1) * rng.choice([-1.0, 1.0], n - 1)])
+    Q, _ = np.linalg.qr(rng.standard_normal((n - 1, n - 1)))
+    H = np.zeros((n, n))
+    H[0, 0] = lam[0]
+    H[1:, 1:] = (Q * lam[1:]) @ Q.T
+    H = 0.5 * (H + H.T)
+    atom_nb = np.full(n_at, nb, dtype=np.int32)
+    row_ptr = np.arange(n_at + 1, dtype=np.int64) * n_at
+    col_idx = np.tile(np.arange(n_at, dtype=np.int32), n_at)
+    blocks = lambda M: np.ascontiguousarray(M.reshape(n_at, nb, n_at, nb).transpose(0, 2, 1, 3)).reshape(-1)
+    Hv, Sv = blocks(H), blocks(np.eye(n))
+    D = torch.zeros(Hv.shape[0], dtype=torch.float64, device="cuda")
+    with _nolsm() as ctx:
+        ctx.assemble(torch.from_numpy(atom_nb).cuda(), torch.from_numpy(row_ptr).cuda(), torch.from_numpy(col_idx).cuda(),
+                     torch.from_numpy(Hv).cuda(), torch.from_numpy(Sv).cuda())
+        ctx.density_matrix(0.0, D)
+        E = ctx.energy()
+        n_elec = ctx.electron_count()
+        st = ctx.atom_stats()
+        extra = ctx.engine_counters()["power_steps_extra"]
+    assert (st["status"] == 0).all()
+    # full pattern: every submatrix is the whole matrix (P3), so the oracle is Eq. 5 on the dense matrices
+    w, V = np.linalg.eigh(H)
+    D_ref = (V[:, w < 0] @ V[:, w < 0].T)
+    got = D.cpu().numpy().reshape(n_at, n_at, nb, nb).transpose(0, 2, 1, 3).reshape(n, n)     # slot (i, j) = (D_ji)^T: D^T = D
+    print("outlier: extra power steps", extra, "max|dD|", np.abs(got - D_ref).max(), "D_00", got[0, 0], "Tr(DS)", n_elec, int((w < 0).sum()))
+    assert abs(got[0, 0]) <= TOL_MIXED_D and np.abs(got - D_ref).max() <= TOL_MIXED_D
+    assert abs(n_elec - (w < 0).sum()) <= 0.05
+    assert abs(E - w[w < 0].sum()) <= TOL_MIXED_E * abs(w[w < 0].sum())
+    assert extra >= n_at                                               # every submatrix needed more than the default steps

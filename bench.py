@@ -278,8 +278,6 @@ def main():
     ap.add_argument("--iteration", type=int, default=0, choices=[0, 1], help="0 = Eq. 6 as printed, 1 = symmetric (Loewdin) form")
     ap.add_argument("--symmetric-tiles", type=int, default=0, choices=[0, -1])
     ap.add_argument("--transposed-tiles", type=int, default=0, choices=[0, -1])
-    ap.add_argument("--diag-drop-operand-loads", type=int, default=0, choices=[0, 1, 2, 3],
-                    help="DIAGNOSTIC (include/nolsm.h): results are meaningless, the line is marked invalid")
     ap.add_argument("--heavy-slots", type=int, default=0)
     ap.add_argument("--claim-lead", type=int, default=0)
     ap.add_argument("--no-extra-legs", "--no-combine-leg", action="store_true", dest="no_extra",
@@ -325,7 +323,7 @@ def main():
     stream = torch.cuda.current_stream().cuda_stream
     head_opts = dict(profile_every=args.profile_every, combine=args.combine, iteration=args.iteration,
                      symmetric_tiles=args.symmetric_tiles, heavy_slots=args.heavy_slots, claim_lead=args.claim_lead,
-                     transposed_tiles=args.transposed_tiles, diag_drop_operand_loads=args.diag_drop_operand_loads)
+                     transposed_tiles=args.transposed_tiles)
     ctx = Nolsm(local_rank, **head_opts)
     perf_table = load_perf_table()
     if perf_table and args.combine == 2:
@@ -591,12 +589,6 @@ def main():
             "other_configs": others, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
             "gpu_launches": int(prof_acc["kernel_launches"]),
             "paper_context": "1.1 EFLOP/s FP16/FP32 on 4400 A100 (~257 TFLOP/s per GPU, ~80% of 312), other hardware"}
-    if args.diag_drop_operand_loads:
-        # not a bench line: the producers left operand boxes out, D is meaningless; only rates, clocks and power are read
-        line = {"diagnostic": "diag_drop_operand_loads=%d: results invalid, not a benchmark value" % args.diag_drop_operand_loads,
-                "value": None, "metric": line["metric"], "ms_per_step": ms_step, "config": line["config"],
-                "kernel_tflops_executed": roofline["achieved"], "kernel_tflops_padded": roofline["achieved_padded"],
-                "gemms_per_submatrix": line["gemms_per_submatrix"], "clocks": clocks}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

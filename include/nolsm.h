@@ -102,8 +102,6 @@ typedef struct {
                                 the Loewdin form) multiply only the tiles on and above the diagonal of the tile grid and mirror
                                 them [0 = on; -1 = off: every tile is multiplied] */
     int heavy_slots;         /* persistent engine: submatrices inside the GEMM chains at once [0 = auto: L2 size / (3.5 n^2 FP16)] */
-    int claim_lead;          /* persistent engine: a CTA pair claims its next tile when its TMA producer is this many k-blocks
-                                from the end of the current one [14] */
     int mu_trials;           /* nolsm_find_mu, persistent engine: trial mu evaluated per pass on the resident S_sub^-1, A0 [1 = bisection:
                                 a trial after the first costs ~3/4 of a pass and K trials gain log2(K + 1) bits, so K = 1 needs the
                                 least work per bit (measured: bench.py other_configs.cfg1.mu_search); max 8] */
@@ -113,20 +111,16 @@ typedef struct {
                                 records) that lasts timeout_s (at least 20 s) counts as a stall and stops the kernel too. The abort
                                 of any kernel launched since the last wait is reported by that wait, also when later calls on
                                 the context (a series of nolsm_density_matrix_range) went through [300] */
-    int scan_order;          /* persistent engine, tile schedulers: 1 = every CTA pair scans the slots from slot 0 (the chains of the first
-                                slots advance first), 2 = every pair from its own slot (74 schedulers do not queue on one claim word)
-                                [0 = auto: 2 for mean dimensions up to 768, where a tile is as short as a claim] */
-    int l2_load_policy;      /* persistent engine: L2 eviction priority of the TMA operand loads: 1 evict_first, 2 evict_last, 3 normal [1] */
-    int l2_store_policy;     /* the same for the TMA stores of the GEMM results [2: a result stays in L2 until the next GEMM of its
-                                chain reads it instead of being pushed out by operand traffic; measured +5 % on configs[2]] */
     int transposed_tiles;    /* persistent engine: the tiles of a ragged last row block (r < 256 rows left) are computed transposed,
                                 C^T = B^T A^T, so the MMA's M = 256 runs over full columns and its N = r over the rows that exist,
                                 instead of M = 256 (or 128) over r rows [0 = on; -1 = off] */
-    int diag_drop_operand_loads; /* DIAGNOSTIC, persistent engine: bit 0: the TMA producers do not load the second 64-row box of the
-                                A operand of a tile, bit 1: not the second 64-column box of B; the tensor cores multiply what the
-                                stage held before. The results of such a call are MEANINGLESS (status words report what the
-                                iterations did with them); the call measures what the operand traffic costs: a quarter / a half
-                                fewer bytes per FLOP (profiles/r02_persist.md) [0] */
+    int tuning[8];           /* engine tuning words with measured defaults (profiles/r02_persist.md); they carry no meaning for a
+                                user of the method, are not part of the stable interface, and should stay zero. Persistent
+                                engine: [0] claim lead: a CTA pair claims its next tile when its TMA producer is this many
+                                k-blocks from the end of the current one [14]; [1] slot scan order of the tile schedulers,
+                                1 = every pair from slot 0, 2 = every pair from its own slot [auto: 2 for mean dimensions up
+                                to 768]; [2] / [3] L2 eviction priority of the TMA operand loads / of the TMA stores of the GEMM
+                                results, 1 evict_first, 2 evict_last, 3 normal [1 / 2]; [4..7] unused */
 } nolsm_options;
 
 typedef struct {
@@ -152,7 +146,7 @@ typedef struct {
  * whenever a field of nolsm_options / nolsm_stats or the meaning of an existing argument changes, and the two sizes are the
  * library's own sizeof. A binding compares all three with its own at load time and refuses a stale libnolsm.so instead
  * of silently misreading every option behind the first changed field. Needs no context and no GPU. */
-#define NOLSM_ABI_VERSION 5
+#define NOLSM_ABI_VERSION 6
 int nolsm_abi_version(void);
 size_t nolsm_sizeof_options(void);
 size_t nolsm_sizeof_stats(void);

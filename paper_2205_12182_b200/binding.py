@@ -14,7 +14,7 @@ ENGINE_AUTO, ENGINE_PERSISTENT, ENGINE_ROUNDS = 0, 1, 2
 ITER_EQ6, ITER_LOWDIN = 0, 1
 STATUS_NAMES = {0: "OK", 1: "EINVAL", 2: "ECUDA", 3: "ENOMEM", 4: "ESTATE", 5: "ENOTSPD", 6: "ENOCONV"}
 
-ABI_VERSION = 5                                     # NOLSM_ABI_VERSION of the include/nolsm.h this file restates
+ABI_VERSION = 6                                     # NOLSM_ABI_VERSION of the include/nolsm.h this file restates
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
@@ -27,9 +27,12 @@ class NolsmOptions(C.Structure):
                 ("engine", C.c_int), ("sign_scaled_iters", C.c_int), ("sign_scale", C.c_float),
                 ("combine", C.c_int), ("combine_max_dim", C.c_int),
                 ("combine_max_members", C.c_int), ("combine_max_candidates", C.c_int), ("iteration", C.c_int),
-                ("symmetric_tiles", C.c_int), ("heavy_slots", C.c_int), ("claim_lead", C.c_int), ("mu_trials", C.c_int),
-                ("timeout_s", C.c_double), ("scan_order", C.c_int), ("l2_load_policy", C.c_int), ("l2_store_policy", C.c_int),
-                ("transposed_tiles", C.c_int), ("diag_drop_operand_loads", C.c_int)]
+                ("symmetric_tiles", C.c_int), ("heavy_slots", C.c_int), ("mu_trials", C.c_int),
+                ("timeout_s", C.c_double), ("transposed_tiles", C.c_int), ("tuning", C.c_int * 8)]
+
+
+# names of the engine tuning words options.tuning[k] (include/nolsm.h): accepted as keyword options by Nolsm(...)
+TUNING_WORDS = {"claim_lead": 0, "scan_order": 1, "l2_load_policy": 2, "l2_store_policy": 3}
 
 
 class NolsmStats(C.Structure):
@@ -144,7 +147,10 @@ class Nolsm:
         self._h = C.c_void_p()
         o = NolsmOptions()
         for k, v in opts.items():
-            if not hasattr(o, k):
+            if k in TUNING_WORDS:
+                o.tuning[TUNING_WORDS[k]] = int(v)
+                continue
+            if not hasattr(o, k) or k == "tuning":
                 raise TypeError(f"unknown option {k}")
             setattr(o, k, v)
         rc = self._lib.nolsm_create(C.byref(self._h), device, C.byref(o))

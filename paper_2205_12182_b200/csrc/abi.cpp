@@ -221,7 +221,7 @@ int nolsm_create(nolsm_ctx** out, int cuda_device, const nolsm_options* opt) try
     bad = bad || !(o.sign_scale > 1.f && o.sign_scale < 1.7320508f);
     bad = bad || o.engine < 0 || o.engine > NOLSM_ENGINE_ROUNDS;
     bad = bad || o.iteration < 0 || o.iteration > NOLSM_ITER_LOWDIN;
-    bad = bad || o.heavy_slots < 0 || o.claim_lead < 0;
+    bad = bad || o.heavy_slots < 0 || o.tuning[0] < 0;
     if (bad) { delete c; return NOLSM_EINVAL; }
     cudaSetDevice(cuda_device);
     cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, cuda_device);

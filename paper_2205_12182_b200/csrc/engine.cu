@@ -452,13 +452,12 @@ int engine_plan(nolsm_ctx* c, cudaStream_t s) {
             }
         }
         pe.g_max = std::max(1, std::min(g_max, S));
-        pe.want_lead = c->opt.claim_lead > 0 ? c->opt.claim_lead : G2_WANT_LEAD;
+        pe.want_lead = c->opt.tuning[0] > 0 ? c->opt.tuning[0] : G2_WANT_LEAD;
         pe.lowdin = c->opt.iteration == NOLSM_ITER_LOWDIN ? 1 : 0;
-        pe.scan_rotate = c->opt.scan_order == 2 ? 1 : c->opt.scan_order == 1 ? 0 : (mean_n2 <= 768.0 * 768.0 ? 1 : 0);
-        pe.l2_load = c->opt.l2_load_policy > 0 ? c->opt.l2_load_policy : 1; pe.l2_store = c->opt.l2_store_policy > 0 ? c->opt.l2_store_policy : 2;
+        pe.scan_rotate = c->opt.tuning[1] == 2 ? 1 : c->opt.tuning[1] == 1 ? 0 : (mean_n2 <= 768.0 * 768.0 ? 1 : 0);
+        pe.l2_load = c->opt.tuning[2] > 0 ? c->opt.tuning[2] : 1; pe.l2_store = c->opt.tuning[3] > 0 ? c->opt.tuning[3] : 2;
         pe.sym_tiles = c->opt.symmetric_tiles >= 0 ? 1 : 0;
         pe.trans_tiles = c->opt.transposed_tiles >= 0 ? 1 : 0;
-        pe.diag_drop = c->opt.diag_drop_operand_loads & 3;
         pe.n_mu = 1; pe.count_only = 0;
         pe.nelec_mu = c->d_mu_acc; pe.e_mu = c->d_mu_acc + NOLSM_MAX_MU;
         pe.elem_chunks = 16;

@@ -358,7 +358,7 @@ __device__ __forceinline__ void g2_finisher(const G2Smem& sm, int lane, Done don
 // values of its operands; the k-block then took ~650 cycles whatever the tile's width, the producer was busy 85 % of the
 // time and the MMA warp waited for operands: profiles/r02_persist.md.)
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap* maps, uint32_t rank, int lane, int want_lead, volatile int* abort_flag, int l2_load, int diag_drop) {
+__device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap* maps, uint32_t rank, int lane, int want_lead, volatile int* abort_flag, int l2_load) {
     const uint64_t pol = ptx::l2_policy(l2_load);
     int stage = 0; uint32_t phase = 0;
     int q = 0; uint32_t tph = 0;
@@ -380,10 +380,6 @@ __device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap*
         const int row0 = ti.m0 + (hh ? 64 : 128) * (int)rank;
         const int col0 = ti.n0 + half * (int)rank;
         const int kb_want = rank == 0 ? max(0, nkb - want_lead) : -1;
-        // diagnostic (options.diag_drop_operand_loads): the second box of A / of B is not loaded (the MMA multiplies what
-        // the stage held before: the results are meaningless, the traffic per FLOP is a quarter / a half lower)
-        const bool ld_a2 = !hh && !(diag_drop & 1), ld_b2 = nbox > 1 && !(diag_drop & 2);
-        const uint32_t nbytes = diag_drop ? 2u * ((ld_a2 ? 2u : 1u) + (ld_b2 ? 2u : 1u)) * 8192u : bytes;
         // transposed tile: the A stage takes this CTA's 128 columns of B (two boxes), the B stage its bn / 2 rows of A
         const bool tr = (ti.valid & TI_TRANS) != 0;
         const int tcol0 = ti.n0 + 128 * (int)rank, trow0 = ti.m0 + half * (int)rank;
@@ -406,13 +402,13 @@ __device__ __forceinline__ void g2_producer(const G2Smem& sm, const CUtensorMap*
             if (ptx::elect_one()) {
                 if (kb == kb_want) ptx::st_shared_volatile_u32(sm.want(), started);   // the scheduler may claim the next tile now
                 const uint32_t fb = full0 + 8u * stage;
-                if (rank == 0) ptx::mbar_expect_tx(sm.full(stage), nbytes);
+                if (rank == 0) ptx::mbar_expect_tx(sm.full(stage), bytes);
                 const uint32_t sa = sm.stage_a(stage), sb = sm.stage_b(stage);
                 const int k0 = kb * BK;
                 ptx::tma_load_2d_pair(sa, map_a, k0, row0, fb, pol);
-                if (ld_a2) ptx::tma_load_2d_pair(sa + 8192, map_a, k0, row0 + 64, fb, pol);
+                if (!hh) ptx::tma_load_2d_pair(sa + 8192, map_a, k0, row0 + 64, fb, pol);
                 ptx::tma_load_2d_pair(sb, map_b, col0, k0, fb, pol);
-                if (ld_b2) ptx::tma_load_2d_pair(sb + B_BOX_BYTES, map_b, col0 + 64, k0, fb, pol);
+                if (nbox > 1) ptx::tma_load_2d_pair(sb + B_BOX_BYTES, map_b, col0 + 64, k0, fb, pol);
             }
             __syncwarp();
             if (++stage == G2_STAGES) { stage = 0; phase ^= 1; }

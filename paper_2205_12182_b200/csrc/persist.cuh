@@ -105,7 +105,6 @@ struct PEngine {
     int lowdin;                   // 0: Eq. 6 on A = S^-1 H0 - mu I; 1: symmetric (Loewdin) form
     int sym_tiles;                // 1: symmetric products multiply the upper triangle of tiles only
     int trans_tiles;              // 1: tiles of a ragged last row block are computed transposed (TI_TRANS)
-    int diag_drop;                // diagnostic: operand boxes the producers leave out (options.diag_drop_operand_loads)
     int n_mu; float mu[P_MAX_MU]; // trial chemical potentials of this call (1 for nolsm_density_matrix)
     int count_only;               // 1: D is not written, only e and q per trial mu (nolsm_electron_counts)
     double* nelec_mu;             // [P_MAX_MU] sum_i q_i per trial mu (count_only)
@@ -1085,7 +1084,7 @@ nolsm_persist_kernel(const __grid_constant__ PEngine e) {
     } else if (warp == G2_WARP_SCHED) {
         if (rank == 0) p_scheduler(sm, e, lane);
     } else if (warp == G2_WARP_TMA) {
-        g2_producer(sm, e.maps, rank, lane, e.want_lead, e.abort_flag, e.l2_load, e.diag_drop);
+        g2_producer(sm, e.maps, rank, lane, e.want_lead, e.abort_flag, e.l2_load);
     } else if (warp == G2_WARP_MMA) {
         if (rank == 0) g2_mma(sm, tmem_base, lane, e.abort_flag, &e.ctr[PC_MMA_NS]);
         else g2_finisher(sm, lane, done, e.abort_flag);

@@ -34,7 +34,7 @@ def test_option_and_stats_structs_match_header():
     text = open(os.path.join(ROOT, "include", "nolsm.h")).read()
     opt = re.search(r"typedef struct \{(.*?)\} nolsm_options;", text, flags=re.S).group(1)
     opt = re.sub(r"/\*.*?\*/", "", opt, flags=re.S)
-    fields = [m.group(1) for m in re.finditer(r"\b([a-z_0-9]+)\s*;", opt)]
+    fields = [m.group(1) for m in re.finditer(r"\b([a-z_0-9]+)(?:\[\d+\])?\s*;", opt)]
     assert fields == [f for f, _ in NolsmOptions._fields_]
     st = re.search(r"typedef struct \{((?:(?!typedef).)*?)\} nolsm_stats;", text, flags=re.S).group(1)
     st = re.sub(r"/\*.*?\*/", "", st, flags=re.S)

@@ -736,22 +736,6 @@ def test_random_shapes_against_oracle(seed, n_at, nbs, p_link, combine):
     assert abs(e_gpu - e_ref) <= TOL_MIXED_E * abs(e_ref)
 
 
-@pytest.mark.parametrize("drop", [1, 3])
-def test_diagnostic_drop_of_operand_loads_completes(drop):
-    """options.diag_drop_operand_loads leaves operand boxes out: the results are meaningless by definition, but the call must
-    run to its end (every wait of the pipeline counts the bytes that are really loaded) and report through the status words."""
-    s = make_system("cfg2", n_atoms=300)
-    nb, rp, ci, Hv, Sv = _arrays(s)
-    with _nolsm(diag_drop_operand_loads=drop, max_sign_iters=20) as ctx:
-        ctx.assemble(nb, rp, ci, Hv, Sv)
-        D = torch.zeros(Hv.shape[0], dtype=torch.float64, device="cuda")
-        ctx.density_matrix(s.mu, D)
-        ctx.energy(strict=False)
-        st = ctx.atom_stats()
-        stats = ctx.stats()
-    assert stats["gemms_executed"] == int(st["gemms"].sum()) and stats["gemms_executed"] > 0
-
-
 def test_time_limit_abort_is_reported_by_the_next_wait_and_the_context_recovers():
     """options.timeout_s counts from the launch. A kernel that overruns it is stopped by the call that waits, and the abort is
     not forgotten when a later call on the context went through in the meantime (a series of density_matrix_range calls

@@ -159,3 +159,98 @@ def test_large_dimension_submatrices():
     assert (st["status"][a0:a1] == 0).all()
     assert abs(e - st["e_atom"][a0:a1].sum()) <= 1e-9 * abs(e)
     _check_sample(s, D, st["e_atom"], [a0 + 5], "pn-14-8.5, one atom of ~3600 dimensions")
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# The variants bench.py quotes on the full headline config (32,768 atoms): symmetric (Loewdin) form, Eq. 9 groups, Eq. 10
+# groups with the measured p(n). The oracle sees the neighbourhoods of the sampled atoms / groups only (restrict), the
+# library the whole system; groups are compared over ALL atoms (the oracle's grouping is integer work).
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def cfg2_full():
+    s = make_system("cfg2")
+    return s, _device_inputs(s)
+
+
+def test_cfg2_full_lowdin_form(cfg2_full):
+    """configs[2] at full size in the symmetric form (C-21): twice the chains in flight, every
+    product on the upper triangle of tiles with mirrored stores. 32 seeded atoms and the two extremes against the oracle."""
+    from paper_2205_12182_b200 import ITER_LOWDIN, Nolsm
+    s, (nb, rp, ci, Hv, Sv) = cfg2_full
+    D = torch.empty_like(Hv)
+    with Nolsm(0, iteration=ITER_LOWDIN) as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        ctx.density_matrix(s.mu, D)
+        E = ctx.energy()
+        st = ctx.atom_stats()
+        stats = ctx.stats()
+    # every product of the form is symmetric except M = H0 Z (one per submatrix)
+    assert (st["status"] == 0).all() and stats["gemms_symmetric"] == stats["gemms_executed"] - s.n_atoms > 0
+    assert abs(E - st["e_atom"].sum()) <= 1e-9 * abs(E)
+    atoms = np.sort(np.random.default_rng(52).choice(s.n_atoms, 32, replace=False))
+    _check_sample(s, D, st["e_atom"], atoms, "cfg2 full, Loewdin form, 32 atoms")
+    _check_sample(s, D, st["e_atom"], [int(np.argmin(st["dims"])), int(np.argmax(st["dims"]))], "cfg2 full, Loewdin form, extremes")
+
+
+def _perf_table():
+    import json
+    import os
+    with open(os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "workloads", "pn_b200.json")) as f:
+        tab = json.load(f)["table"]
+    n, tf = [int(r["n"]) for r in tab], [float(r["tflops"]) for r in tab]
+    return (n, tf), (n, [int(round(x * 1000)) for x in tf])
+
+
+@pytest.mark.parametrize("mode", [1, "2+table"])
+def test_cfg2_full_combined_groups_and_parity(cfg2_full, mode):
+    """configs[2] at full size with submatrix combination (Eq. 9; Eq. 10 with the measured and
+    interpolated p(n), L89-91): the library's groups and union index sets equal the oracle's over all 32,768 atoms bit for
+    bit; D and e_i of every member of six groups (the largest by dimension and five seeded ones) match the oracle's
+    evaluation of Eq. 8 on the union set."""
+    from oracle import nolsm_oracle as orc
+    from paper_2205_12182_b200 import Nolsm
+    from tests.helpers import d_row_from_oracle
+    s, (nb, rp, ci, Hv, Sv) = cfg2_full
+    lib_table, orc_table = _perf_table()
+    sets = [orc.index_set(i, s.row_ptr, s.col_idx) for i in range(s.n_atoms)]
+    groups = orc.combine_groups(s.atom_nb, sets, mode=1 if mode == 1 else 2, perf_table=None if mode == 1 else orc_table)
+    D = torch.empty_like(Hv)
+    with Nolsm(0, combine=1 if mode == 1 else 2) as ctx:
+        if mode != 1:
+            ctx.set_perf_table(*lib_table)
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        gdims = []
+        for g in groups:
+            mem, st_, dim = ctx.group(g[0])
+            assert mem.tolist() == g
+            assert np.array_equal(st_, np.unique(np.concatenate([sets[i] for i in g])).astype(np.int32))
+            gdims.append(dim)
+        ctx.density_matrix(s.mu, D)
+        E = ctx.energy()
+        st = ctx.atom_stats()
+        stats = ctx.stats()
+    assert stats["n_units"] == len(groups) < s.n_atoms // 2 and (st["status"] == 0).all()
+    assert abs(E - st["e_atom"].sum()) <= 1e-9 * abs(E)
+    blk = s.blk_off()
+    rows = _DeviceRows(D)
+    picks = {int(np.argmax(gdims)), *np.random.default_rng(9).choice(len(groups), 5, replace=False).tolist()}
+    max_d, e_ref, e_gpu = 0.0, 0.0, 0.0
+    for k in sorted(picks):
+        g = groups[k]
+        need = np.unique(np.concatenate([sets[i] for i in g]))
+        sub = s.restrict(need)
+        parent = sub.meta["parent_atoms"]
+        sblk = orc.block_offsets(sub.atom_nb, sub.row_ptr, sub.col_idx)
+        local = [int(np.searchsorted(parent, i)) for i in g]
+        res = orc.group_result(local, sub.atom_nb, sub.row_ptr, sub.col_idx, sblk, sub.fill_np(MAT_H), sub.fill_np(MAT_S), s.mu)
+        assert res["n"] == gdims[k]
+        for i, li in zip(g, local):
+            r = dict(res[li])
+            r["N"] = parent[r["N"]].astype(np.int32)
+            ref = d_row_from_oracle(s, i, r, blk)
+            p0, p1 = int(s.row_ptr[i]), int(s.row_ptr[i + 1])
+            max_d = max(max_d, float(np.abs(rows[blk[p0]:blk[p1]] - ref).max()))
+            e_ref += r["e_i"]
+            e_gpu += float(st["e_atom"][i])
+    print("cfg2 full combined", mode, len(groups), "groups, largest", max(gdims), "max|dD|", max_d, "rel dE", abs(e_gpu - e_ref) / abs(e_ref))
+    assert max_d <= TOL_D and abs(e_gpu - e_ref) / abs(e_ref) <= TOL_E

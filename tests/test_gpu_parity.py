@@ -623,7 +623,10 @@ def test_find_mu_reaches_the_target_count(cfg0):
         mu, n_mu, evals = ctx.find_mu(target, -7.0, 8.0, D, tol_n=0.05, tol_mu=1e-4)
         E = ctx.energy()
         st = ctx.atom_stats()
-        assert abs(n_mu - target) <= 0.05 and 3 < evals <= 40 and -0.9 < mu < 0.9
+        # evaluations: the two end points, then bisection of a bracket of 15 down to tol_mu = 1e-4 (log2(15 / 1e-4) = 17.2 ->
+        # at most 18 trial mu) unless tol_n is met first, then the final density-matrix call: at most 21; the search also
+        # stops at max_evals = 40 (the default), which this case must not reach
+        assert abs(n_mu - target) <= 0.05 and 3 < evals <= 21 and -0.9 < mu < 0.9
         n_ref = orc.electron_count(s.atom_nb, s.row_ptr, s.col_idx, Hn, Sn, mu)
         assert abs(n_ref - n_mu) <= TOL_MIXED_E * target
         s_mu = make_system("cfg0")
@@ -635,6 +638,31 @@ def test_find_mu_reaches_the_target_count(cfg0):
         with pytest.raises(NolsmError) as ei:                       # target above the number of basis functions
             ctx.find_mu(2.0 * float(s.atom_nb.sum()), -8.0, 8.0, D)
         assert ei.value.code == 1
+
+
+def test_find_mu_with_three_trials_per_pass(cfg0):
+    """nolsm_find_mu with options.mu_trials = 3 (bench.py runs it): three equidistant trial mu per pass on the resident
+    S_sub^-1 and A0, the bracket shrinks by four per pass. The returned mu gives the requested Tr(D S) within tol_n, the
+    oracle's count at that mu agrees within the mixed-precision tolerance, and D_vals holds D(mu)."""
+    s = cfg0
+    nb, rp, ci, Hv, Sv = _arrays(s)
+    Hn, Sn = s.fill_np(MAT_H), s.fill_np(MAT_S)
+    target = 0.5 * float(s.atom_nb.sum())
+    with _nolsm(mu_trials=3) as ctx:
+        ctx.assemble(nb, rp, ci, Hv, Sv)
+        D = torch.zeros(Hv.shape[0], dtype=torch.float64, device="cuda")
+        mu, n_mu, evals = ctx.find_mu(target, -7.0, 8.0, D, tol_n=0.05, tol_mu=1e-4)
+        E = ctx.energy()
+        st = ctx.atom_stats()
+    # two end points, then passes of three trial mu (bracket / 4 each: log4(15 / 1e-4) = 8.6 -> at most 9 passes), the final call
+    assert abs(n_mu - target) <= 0.05 and 3 < evals <= 2 + 3 * 9 + 1 and -0.9 < mu < 0.9
+    n_ref = orc.electron_count(s.atom_nb, s.row_ptr, s.col_idx, Hn, Sn, mu)
+    assert abs(n_ref - n_mu) <= TOL_MIXED_E * target
+    s_mu = make_system("cfg0")
+    s_mu.mu = mu
+    cmp = compare_atoms(s_mu, D.cpu().numpy(), st["e_atom"], range(0, s.n_atoms, 4))
+    print("find_mu K=3", mu, n_mu, evals, n_ref, cmp["max_abs_dD"], cmp["rel_dE"])
+    assert cmp["max_abs_dD"] <= TOL_MIXED_D and cmp["rel_dE"] <= TOL_MIXED_E and abs(E - st["e_atom"].sum()) <= 1e-9 * abs(E)
 
 
 @pytest.mark.parametrize("kw", [dict(combine=1, iteration=1), dict(combine=2, eps_filter=0.02), dict(combine=1, sign_scaled_iters=-1)])

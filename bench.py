@@ -280,6 +280,7 @@ def main():
     ap.add_argument("--transposed-tiles", type=int, default=0, choices=[0, -1])
     ap.add_argument("--heavy-slots", type=int, default=0)
     ap.add_argument("--claim-lead", type=int, default=0)
+    ap.add_argument("--side-l2", type=int, default=0, choices=[0, 1, 2, 3, 4], help="options.tuning[4] (include/nolsm.h)")
     ap.add_argument("--no-extra-legs", "--no-combine-leg", action="store_true", dest="no_extra",
                     help="skip the variants / combination / other-config / side-task measurements")
     ap.add_argument("--pn-sweep", action="store_true", help="measure p(n) of Eq. 10 and print / write the table")
@@ -322,7 +323,7 @@ def main():
     D = torch.empty_like(Hv)
     stream = torch.cuda.current_stream().cuda_stream
     head_opts = dict(profile_every=args.profile_every, combine=args.combine, iteration=args.iteration,
-                     symmetric_tiles=args.symmetric_tiles, heavy_slots=args.heavy_slots, claim_lead=args.claim_lead,
+                     symmetric_tiles=args.symmetric_tiles, heavy_slots=args.heavy_slots, claim_lead=args.claim_lead, side_l2_policy=args.side_l2,
                      transposed_tiles=args.transposed_tiles)
     ctx = Nolsm(local_rank, **head_opts)
     perf_table = load_perf_table()

@@ -79,7 +79,8 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+                "power_w_max": max(pw) if pw else None, "power_w_median": float(np.median(pw)) if pw else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
 
 
 _ORC = {}          # state shared with forked workers (copy-on-write): restricted system and its values
@@ -280,7 +281,6 @@ def main():
     ap.add_argument("--transposed-tiles", type=int, default=0, choices=[0, -1])
     ap.add_argument("--heavy-slots", type=int, default=0)
     ap.add_argument("--claim-lead", type=int, default=0)
-    ap.add_argument("--side-l2", type=int, default=0, choices=[0, 1, 2, 3, 4], help="options.tuning[4] (include/nolsm.h)")
     ap.add_argument("--no-extra-legs", "--no-combine-leg", action="store_true", dest="no_extra",
                     help="skip the variants / combination / other-config / side-task measurements")
     ap.add_argument("--pn-sweep", action="store_true", help="measure p(n) of Eq. 10 and print / write the table")
@@ -323,7 +323,7 @@ def main():
     D = torch.empty_like(Hv)
     stream = torch.cuda.current_stream().cuda_stream
     head_opts = dict(profile_every=args.profile_every, combine=args.combine, iteration=args.iteration,
-                     symmetric_tiles=args.symmetric_tiles, heavy_slots=args.heavy_slots, claim_lead=args.claim_lead, side_l2_policy=args.side_l2,
+                     symmetric_tiles=args.symmetric_tiles, heavy_slots=args.heavy_slots, claim_lead=args.claim_lead,
                      transposed_tiles=args.transposed_tiles)
     ctx = Nolsm(local_rank, **head_opts)
     perf_table = load_perf_table()
@@ -358,7 +358,8 @@ def main():
         if ctr_acc is None:
             ctr_acc = ct
         else:
-            for k in ("kernel_ms", "tiles", "sched_idle_ms", "sched_busy_ms", "overshoots"):
+            for k in ("kernel_ms", "tiles", "sched_idle_ms", "sched_busy_ms", "overshoots", "mma_wait_record_ms",
+                      "mma_wait_accumulator_ms", "mma_kloop_ms", "sched_wait_ring_ms", "sched_wait_claim_point_ms", "power_steps_extra"):
                 ctr_acc[k] += ct[k]
             for kind, v in ct["side"].items():
                 acc = ctr_acc["side"].setdefault(kind, {"busy_ms": 0.0, "bytes": 0.0, "tasks": 0.0})
@@ -543,14 +544,25 @@ def main():
             hbm["gather_gbs"], hbm["scatter_gbs"] = side_alone["gather_gbs"], side_alone["scatter_gbs"]
         else:
             hbm["gather_gbs"], hbm["scatter_gbs"] = hbm["in_kernel_busy_time_gather_gbs"], hbm["in_kernel_busy_time_scatter_gbs"]
-        engine = {"tiles": ctr_acc["tiles"], "sched_idle_frac": ctr_acc["sched_idle_ms"] / max(ctr_acc["pairs"] * prof_acc["gemm_ms"], 1e-9),
-                  "slots": ctr_acc["slots"], "pairs": ctr_acc["pairs"]}
+        pair_ms = max(ctr_acc["pairs"] * prof_acc["gemm_ms"], 1e-9)       # kernel time summed over the CTA pairs
+        engine = {"tiles": ctr_acc["tiles"], "sched_idle_frac": ctr_acc["sched_idle_ms"] / pair_ms,
+                  "slots": ctr_acc["slots"], "pairs": ctr_acc["pairs"],
+                  # where the MMA-issuing warp of every pair spends the kernel (nolsm_get_engine_counters out[33..35])
+                  "mma_warp_frac": {"tile_record_wait": ctr_acc["mma_wait_record_ms"] / pair_ms,
+                                    "accumulator_wait": ctr_acc["mma_wait_accumulator_ms"] / pair_ms,
+                                    "k_loops": ctr_acc["mma_kloop_ms"] / pair_ms},
+                  "sched_frac": {"ring_wait": ctr_acc["sched_wait_ring_ms"] / pair_ms,
+                                 "claim_point_wait": ctr_acc["sched_wait_claim_point_ms"] / pair_ms},
+                  "power_steps_extra_per_submatrix": ctr_acc["power_steps_extra"] / max(stats["n_units"] * args.steps, 1)}
     else:
         roofline["share_of_sampled_kernel_time"] = prof_acc["gemm_ms"] / max(sampled_ms, 1e-9)
         hbm = {"gather_gbs": prof_acc["gather_bytes"] / max(prof_acc["gather_ms"], 1e-9) / 1e6,
                "scatter_gbs": prof_acc["dcols_bytes"] / max(prof_acc["dcols_ms"], 1e-9) / 1e6,
                "peak_gbs": peaks["hbm_gbs"], "peak_source": peaks["source"]}
         engine = None
+    if clocks.get("power_w_median") and roofline.get("achieved"):
+        # energy per FLOP of the headline run as a driver-visible number: median board power over the timed region / executed rate
+        clocks["watts_per_tflops_executed"] = clocks["power_w_median"] / roofline["achieved"]
     hbm["gather_frac"] = hbm["gather_gbs"] / peaks["hbm_gbs"]
     hbm["scatter_frac"] = hbm["scatter_gbs"] / peaks["hbm_gbs"]
 

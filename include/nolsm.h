@@ -120,9 +120,7 @@ typedef struct {
                                 k-blocks from the end of the current one [14]; [1] slot scan order of the tile schedulers,
                                 1 = every pair from slot 0, 2 = every pair from its own slot [auto: 2 for mean dimensions up
                                 to 768]; [2] / [3] L2 eviction priority of the TMA operand loads / of the TMA stores of the GEMM
-                                results, 1 evict_first, 2 evict_last, 3 normal [1 / 2]; [4] streaming (no L1 allocation, L2 evict_first) accesses
-                                of the side tasks: bit 0 source blocks read by the gather and the D / H0 / S rows of the scatter,
-                                bit 1 the gathered dense rows; 4 = none [3]; [5..7] unused */
+                                results, 1 evict_first, 2 evict_last, 3 normal [1 / 2]; [4..7] unused */
 } nolsm_options;
 
 typedef struct {

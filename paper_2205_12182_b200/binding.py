@@ -32,7 +32,7 @@ class NolsmOptions(C.Structure):
 
 
 # names of the engine tuning words options.tuning[k] (include/nolsm.h): accepted as keyword options by Nolsm(...)
-TUNING_WORDS = {"claim_lead": 0, "scan_order": 1, "l2_load_policy": 2, "l2_store_policy": 3, "side_l2_policy": 4}
+TUNING_WORDS = {"claim_lead": 0, "scan_order": 1, "l2_load_policy": 2, "l2_store_policy": 3}
 
 
 class NolsmStats(C.Structure):

@@ -15,7 +15,6 @@ using namespace nolsm_host;
 namespace {
 
 enum { K_GATHER = 0, K_GEMM = 1, K_DCOLS = 2, K_OTHER = 3 };
-constexpr int NOLSM_SIDE_L2_DEFAULT = 3;   // tuning[4]: measured in profiles/r03_side_l2.md
 
 size_t prof_begin(nolsm_ctx* c, int kind, cudaStream_t s) {
     c->launches += 1;
@@ -456,7 +455,6 @@ int engine_plan(nolsm_ctx* c, cudaStream_t s) {
         pe.want_lead = c->opt.tuning[0] > 0 ? c->opt.tuning[0] : G2_WANT_LEAD;
         pe.lowdin = c->opt.iteration == NOLSM_ITER_LOWDIN ? 1 : 0;
         pe.scan_rotate = c->opt.tuning[1] == 2 ? 1 : c->opt.tuning[1] == 1 ? 0 : (mean_n2 <= 768.0 * 768.0 ? 1 : 0);
-        pe.side_l2 = c->opt.tuning[4] == 4 ? 0 : c->opt.tuning[4] > 0 ? (c->opt.tuning[4] & 3) : NOLSM_SIDE_L2_DEFAULT;
         pe.l2_load = c->opt.tuning[2] > 0 ? c->opt.tuning[2] : 1; pe.l2_store = c->opt.tuning[3] > 0 ? c->opt.tuning[3] : 2;
         pe.sym_tiles = c->opt.symmetric_tiles >= 0 ? 1 : 0;
         pe.trans_tiles = c->opt.transposed_tiles >= 0 ? 1 : 0;

@@ -105,8 +105,6 @@ struct PEngine {
     int lowdin;                   // 0: Eq. 6 on A = S^-1 H0 - mu I; 1: symmetric (Loewdin) form
     int sym_tiles;                // 1: symmetric products multiply the upper triangle of tiles only
     int trans_tiles;              // 1: tiles of a ragged last row block are computed transposed (TI_TRANS)
-    int side_l2;                  // streaming L2 policy of the side tasks: bit 0 source blocks read / D rows written / H0, S rows read,
-                                  // bit 1 the gathered dense rows written
     int n_mu; float mu[P_MAX_MU]; // trial chemical potentials of this call (1 for nolsm_density_matrix)
     int count_only;               // 1: D is not written, only e and q per trial mu (nolsm_electron_counts)
     double* nelec_mu;             // [P_MAX_MU] sum_i q_i per trial mu (count_only)
@@ -144,30 +142,6 @@ __device__ __forceinline__ float* pcols_ptr(const PEngine& e, int slot) { return
 
 namespace pl {
 __device__ __forceinline__ unsigned long long gtime() { return ptx::globaltimer_ns(); }
-// Streaming accesses of the side tasks (source blocks read once per submatrix, rows of D written once, gathered dense rows that
-// wait for their chain): no L1 allocation and a 64-bit L2 cache-policy operand, so that this traffic is the first to leave L2
-// instead of competing with the evict_last iterates of the GEMM chains. (The `.L2::evict_first` qualifier itself exists only for
-// 256-bit accesses; the policy operand serves every width.) use == false: the plain access.
-__device__ __forceinline__ double ld_stream(const double* p, uint64_t pol, bool use) {
-    if (!use) return __ldg(p);
-    double v; asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol)); return v;
-}
-__device__ __forceinline__ float ld_stream(const float* p, uint64_t pol, bool use) {
-    if (!use) return __ldg(p);
-    float v; asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(p), "l"(pol)); return v;
-}
-__device__ __forceinline__ void st_stream(uint4* p, uint4 v, uint64_t pol, bool use) {
-    if (!use) { *p = v; return; }
-    asm volatile("st.global.L1::no_allocate.L2::cache_hint.v4.b32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void st_stream(double* p, double v, uint64_t pol, bool use) {
-    if (!use) { *p = v; return; }
-    asm volatile("st.global.L1::no_allocate.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(p), "d"(v), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void st_stream(float* p, float v, uint64_t pol, bool use) {
-    if (!use) { *p = v; return; }
-    asm volatile("st.global.L1::no_allocate.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(p), "f"(v), "l"(pol) : "memory");
-}
 __device__ __forceinline__ void side_sync() { asm volatile("bar.sync 2, %0;" ::"n"(P_SIDE_THREADS) : "memory"); }
 }  // namespace pl
 
@@ -720,9 +694,7 @@ constexpr int G_NB = 2;                           // blocks a warp has in flight
 template <typename TV>
 __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_vals, const TV* __restrict__ H_vals,
                                   __half* __restrict__ dstS, __half* __restrict__ dstH, int unit, int n, int n16, int ld,
-                                  int chunk, int nchunks, unsigned char* sm, int tid, unsigned long long* bytes, int side_l2 = 0) {
-    const uint64_t pol = ptx::l2_policy(1);
-    const bool s_src = side_l2 & 1, s_dst = side_l2 & 2;
+                                  int chunk, int nchunks, unsigned char* sm, int tid, unsigned long long* bytes) {
     const long long p0 = sv.uset_ptr[unit];
     const int cnt = (int)(sv.uset_ptr[unit + 1] - p0);
     const int warp = tid >> 5, lane = tid & 31;
@@ -801,7 +773,7 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
 #pragma unroll
                             for (int k = 0; k < 8; ++k) {
                                 const int e = lane + 32 * k;
-                                v[u][k] = e < bs ? pl::ld_stream(src + e, pol, s_src) : (TV)0;
+                                v[u][k] = e < bs ? __ldg(src + e) : (TV)0;
                             }
                             nread += (lane == 0) ? (unsigned long long)bs : 0ull;
                         }
@@ -829,7 +801,7 @@ __device__ void side_gather_chunk(const SysView& sv, const TV* __restrict__ S_va
                     const uint4* s4 = reinterpret_cast<const uint4*>(strip);
                     for (int q = tid; q < nr * vpr; q += P_SIDE_THREADS) {
                         const int rr = q / vpr, v = q - rr * vpr;
-                        pl::st_stream(reinterpret_cast<uint4*>(dst + (long long)(row0 + r0 + rr) * ld + v * 8), s4[q], pol, s_dst);
+                        *reinterpret_cast<uint4*>(dst + (long long)(row0 + r0 + rr) * ld + v * 8) = s4[q];
                     }
                 }
                 pl::side_sync();
@@ -916,9 +888,7 @@ __device__ void side_wcols(const float* __restrict__ P, const __half* __restrict
 template <typename TV, typename TD>
 __device__ void side_dcols_chunk(const SysView& sv, const float* __restrict__ P, const __half* __restrict__ Y, float ysc, float psc,
                                  const TV* __restrict__ H_vals, const TV* __restrict__ S_vals, TD* __restrict__ D_vals, double* e_acc,
-                                 double* q_acc, int atom, int n_own, int ld, int pos, int nbi, int chunk, int nchunks, unsigned char* sm, int tid, int side_l2 = 0) {
-    const uint64_t pol = ptx::l2_policy(1);
-    const bool s_src = side_l2 & 1;
+                                 double* q_acc, int atom, int n_own, int ld, int pos, int nbi, int chunk, int nchunks, unsigned char* sm, int tid) {
     const long long p0 = sv.nset_ptr[atom];
     const int cnt = (int)(sv.nset_ptr[atom + 1] - p0);
     int* s_pre = reinterpret_cast<int*>(sm);                               // [cnt + 1] first value row of each atom of N(i) in output order
@@ -941,9 +911,9 @@ __device__ void side_dcols_chunk(const SysView& sv, const float* __restrict__ P,
         const long long o = sv.blk_off[sv.nset_slot[p0 + a]] + rem;       // slot (i, j_a): [c][bb] = D_sub[r, pos + c]
         float d = psc * __ldcg(P + (size_t)r * PCW + (pos & 7) + c);
         if (ysc != 0.f) d = fmaf(ysc, __half2float(__ldcg(Y + (long long)r * ld + pos + c)), d);
-        if (D_vals) pl::st_stream(D_vals + o, (TD)d, pol, s_src);
-        e_part += (double)d * (double)pl::ld_stream(H_vals + o, pol, s_src);
-        q_part += (double)d * (double)pl::ld_stream(S_vals + o, pol, s_src);
+        if (D_vals) D_vals[o] = (TD)d;
+        e_part += (double)d * (double)H_vals[o];
+        q_part += (double)d * (double)S_vals[o];
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) { e_part += __shfl_xor_sync(0xffffffffu, e_part, o); q_part += __shfl_xor_sync(0xffffffffu, q_part, o); }
@@ -997,8 +967,8 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
             case SK_GATHER: {
                 __half* dS = e.base + buf_off(e, slot, 0);
                 __half* dH = e.base + buf_off(e, slot, 1);
-                if (e.val_f64) side_gather_chunk<double>(e.sv, (const double*)e.S_vals, (const double*)e.H_vals, dS, dH, g1.w, n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER], e.side_l2);
-                else side_gather_chunk<float>(e.sv, (const float*)e.S_vals, (const float*)e.H_vals, dS, dH, g1.w, n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER], e.side_l2);
+                if (e.val_f64) side_gather_chunk<double>(e.sv, (const double*)e.S_vals, (const double*)e.H_vals, dS, dH, g1.w, n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER]);
+                else side_gather_chunk<float>(e.sv, (const float*)e.S_vals, (const float*)e.H_vals, dS, dH, g1.w, n, n16, e.ld, chunk, nch, sm, tid, &e.ctr[PC_SIDE_BYTES + SK_GATHER]);
             } break;
             case SK_ELEM: {
                 const int ek = __ldcg(&s->elem_kind);
@@ -1023,11 +993,11 @@ __device__ void p_side_loop(const PEngine& e, unsigned char* sm, int tid) {
                 double* q_acc = e.count_only ? &e.nelec_mu[mu_idx] : &e.q_atom[atom];
                 void* Dv = e.count_only ? nullptr : e.D_vals;
                 if (e.val_f64) {
-                    if (e.d_f64) side_dcols_chunk<double, double>(e.sv, P, Y, ysc, psc, (const double*)e.H_vals, (const double*)e.S_vals, (double*)Dv, e_acc, q_acc, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid, e.side_l2);
-                    else side_dcols_chunk<double, float>(e.sv, P, Y, ysc, psc, (const double*)e.H_vals, (const double*)e.S_vals, (float*)Dv, e_acc, q_acc, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid, e.side_l2);
+                    if (e.d_f64) side_dcols_chunk<double, double>(e.sv, P, Y, ysc, psc, (const double*)e.H_vals, (const double*)e.S_vals, (double*)Dv, e_acc, q_acc, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
+                    else side_dcols_chunk<double, float>(e.sv, P, Y, ysc, psc, (const double*)e.H_vals, (const double*)e.S_vals, (float*)Dv, e_acc, q_acc, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
                 } else {
-                    if (e.d_f64) side_dcols_chunk<float, double>(e.sv, P, Y, ysc, psc, (const float*)e.H_vals, (const float*)e.S_vals, (double*)Dv, e_acc, q_acc, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid, e.side_l2);
-                    else side_dcols_chunk<float, float>(e.sv, P, Y, ysc, psc, (const float*)e.H_vals, (const float*)e.S_vals, (float*)Dv, e_acc, q_acc, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid, e.side_l2);
+                    if (e.d_f64) side_dcols_chunk<float, double>(e.sv, P, Y, ysc, psc, (const float*)e.H_vals, (const float*)e.S_vals, (double*)Dv, e_acc, q_acc, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
+                    else side_dcols_chunk<float, float>(e.sv, P, Y, ysc, psc, (const float*)e.H_vals, (const float*)e.S_vals, (float*)Dv, e_acc, q_acc, atom, e.adim[atom], e.ld, pos, nbi, chunk, nch, sm, tid);
                 }
             } break;
             default: break;                       // SK_REFILL: nothing to compute
